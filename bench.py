@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the FP64 ship-wave residual F(u) on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config cfg5_721x241]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input at the
+configuration the metric is quoted on (cfg5, 721x241): sws_residual(u) followed by
+sws_jv_batch(u, V[16]) = 18 residual evaluations (1 + (16 + 1)), 5.43e11 pair interactions.
+`value` = residual evaluations per second with u and V resident in HBM; `e2e` = the same
+through the host-buffer C-ABI calls (pinned host memory, H2D + D2H inside the timed region).
+
+The path does not shard ("replicas only"): with --gpus N (launched by torchrun,
+one rank per GPU) every rank runs the same step on its own GPU, no data-path collective;
+`value` = N * evaluations / max-over-ranks time, scaling "weak".
+
+--impl reference times the CPU oracle (oracle/, the paper's algorithm as plain C, as it
+stands) on the host cores, on a bounded row sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import workloads as W  # noqa: E402
+
+METRIC = "fp64_residual_evals_per_s_721x241"
+UNIT = "evals/s"
+# Algorithmic work of the all-pairs kernel per pair interaction, from its SASS inner loop
+# (DESIGN.md "Kernels"): 45 FP64-pipe instructions = 25 DFMA (2 flops) + 20 DMUL/DADD (1 flop).
+FP64_INSTR_PER_PAIR = 45
+FLOPS_PER_PAIR = 70
+FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks() -> dict:
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return json.loads(p.read_text())
+        except Exception:
+            return {}
+    return {}
+
+
+def oracle_sample(cfg, seconds: float, rows_fixed: int | None = None):
+    """Time the f64 oracle (as it stands) on a seeded sample of integral-equation rows of cfg;
+    returns (evals_per_s, rows, elapsed_s, threads).  rows/T of one evaluation's pairs are
+    computed; the O(NM) part is computed in full each call."""
+    import oracle
+    orc = oracle.Oracle("f64")
+    p, u = cfg.params(), W.state(cfg)
+    T = cfg.targets
+    threads = int(os.environ.get("OMP_NUM_THREADS", "0")) or (os.cpu_count() or 1)
+    rng = np.random.default_rng(99)
+    if rows_fixed is None:
+        probe = np.sort(rng.choice(T, size=min(T, 512), replace=False)).astype(np.int32)
+        t0 = time.perf_counter()
+        orc.residual(p, u, rows=probe)
+        dt = max(time.perf_counter() - t0, 1e-3)
+        rows_fixed = int(min(T, max(512, probe.size * seconds / dt)))
+    rows = np.sort(rng.choice(T, size=rows_fixed, replace=False)).astype(np.int32)
+    t0 = time.perf_counter()
+    orc.residual(p, u, rows=rows)
+    dt = time.perf_counter() - t0
+    return (rows.size / T) / dt, int(rows.size), dt, threads
+
+
+def run_reference(args) -> None:
+    """The oracle arm: rank 0 only; every step is one bounded row sample of cfg."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    cfg = W.BY_NAME[args.config]
+    rows = args.ref_rows
+    for _ in range(args.warmup):
+        oracle_sample(cfg, 0.0, rows_fixed=rows)
+    vals, threads, tot = [], 1, 0.0
+    for _ in range(args.steps):
+        v, nrows, dt, threads = oracle_sample(cfg, 0.0, rows_fixed=rows)
+        vals.append(v)
+        tot += dt
+    value = args.steps * (rows / cfg.targets) / tot
+    sample = (f"{rows} seeded integral-equation rows of {cfg.targets} per step (+ all O(NM) rows), "
+              f"{rows * cfg.sources:.3e} pair interactions per step, scaled by rows/T")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": cfg.name, "N": cfg.N, "M": cfg.M, "sample": sample},
+        "pairs_per_s": value * cfg.pairs,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args) -> None:
+    import torch
+
+    import paper_1403_5044_b200 as sws
+    from paper_1403_5044_b200 import replicas
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+    torch.cuda.set_device(local)
+    replicas.init("nccl", device=local)
+    cfg = W.BY_NAME[args.config]
+    b = cfg.b if cfg.b > 0 else 1
+    p = cfg.params()
+    u_h, V_h = W.state(cfg), W.directions(cfg, b)
+    evals_per_step = 1 + (b + 1)          # sws_residual + the (b + 1) states of sws_jv_batch
+    pairs_per_step = evals_per_step * cfg.pairs
+
+    ctx = sws.Context(p, max_batch=b, device=local)
+    u = torch.from_numpy(u_h).cuda(local)
+    V = torch.from_numpy(V_h).cuda(local)
+    F = torch.empty(cfg.n, dtype=torch.float64, device=u.device)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=u.device)  # > 126 MB L2
+    launches_per_step = 0
+
+    def step():
+        nonlocal launches_per_step
+        ctx.residual(u, out=F)
+        n1 = ctx.last_launch_count
+        JV = ctx.jv_batch(u, V)
+        launches_per_step = n1 + ctx.last_launch_count
+        return JV
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    torch.cuda.synchronize()
+
+    # ---- timed region: device-resident inputs -------------------------------------------
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    ctx.set_profiling(True)
+    ctx.profile_read(reset=True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    replicas.barrier()
+    torch.cuda.synchronize()
+    for e0, e1 in ev:
+        flush.zero_()                      # L2 flush between timed iterations (not timed)
+        e0.record()
+        step()
+        e1.record()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    ms_total = sum(e0.elapsed_time(e1) for e0, e1 in ev)
+    ap_ms, ap_launches = ctx.profile_read(reset=True)
+    ctx.set_profiling(False)
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = replicas.max_over_ranks(ms_total)
+    value = world * args.steps * evals_per_step / (ms_total * 1e-3)
+
+    # ---- end to end: host buffers through the C-ABI host calls ----------------------------
+    u_pin = torch.from_numpy(u_h).pin_memory()
+    V_pin = torch.from_numpy(V_h).pin_memory()
+    F_pin = torch.empty(cfg.n, dtype=torch.float64).pin_memory()
+    JV_pin = torch.empty((b, cfg.n), dtype=torch.float64).pin_memory()
+    Fp_pin = torch.empty((b, cfg.n), dtype=torch.float64).pin_memory()
+    F0_pin = torch.empty(cfg.n, dtype=torch.float64).pin_memory()
+
+    def step_host():
+        ctx.residual_host(u_pin.numpy(), out=F_pin.numpy())
+        ctx.jv_batch_host(u_pin.numpy(), V_pin.numpy(), out=JV_pin.numpy(), fpert=Fp_pin.numpy(),
+                          f0=F0_pin.numpy())
+        return float(JV_pin[0, 0])         # device -> host read of the step's result
+
+    step_host()
+    e2e_steps = args.steps
+    replicas.barrier()
+    torch.cuda.synchronize()
+    ms_e2e = 0.0
+    for _ in range(e2e_steps):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        step_host()                        # ends with a stream synchronise inside the library
+        ms_e2e += (time.perf_counter() - t0) * 1e3
+    replicas.barrier()
+    ms_e2e = replicas.max_over_ranks(ms_e2e)
+    e2e_value = world * e2e_steps * evals_per_step / (ms_e2e * 1e-3)
+    nb = cfg.n * 8
+    h2d = nb + (nb + b * nb)                # u; then u and V
+    d2h = nb + (b * nb + b * nb + nb)       # F; then JV, Fpert, F0
+
+    if rank != 0:
+        ctx.close()
+        replicas.finalize()
+        return
+
+    # ---- roofline of the dominant kernel (all-pairs), bound: FP64 ALU pipe ---------------
+    peaks = measured_peaks()
+    probe = sws.probe_fp64_peak(local)
+    sm_count = probe["sm_count"]
+    sm_max = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
+    peak_tf = sm_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    pairs_timed = args.steps * pairs_per_step
+    ap_s = ap_ms * 1e-3
+    achieved_tf = FLOPS_PER_PAIR * pairs_timed / ap_s / 1e12
+    sm_mhz = (clocks or {}).get("sm_mhz") or sm_max
+    pipe_frac = FP64_INSTR_PER_PAIR * pairs_timed / (sm_count * FP64_LANES_PER_SM * sm_mhz * 1e6 * ap_s)
+    roofline = {
+        "bound": "alu", "kernel": "k_allpairs", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+        "frac": achieved_tf / peak_tf, "traffic": None,
+        "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz "
+                       "(FP64 is not in MEASURED_PEAKS.json; DESIGN.md 'Peak')",
+        "flops_per_pair": FLOPS_PER_PAIR, "fp64_instr_per_pair": FP64_INSTR_PER_PAIR,
+        "launches_timed": ap_launches, "avg_launch_ms": ap_ms / max(ap_launches, 1),
+        "share_of_step": ap_ms / ms_total if world == 1 else None,
+        "dfma_probe_tflops": probe["tflops"], "dfma_probe_sm_mhz": probe["sm_mhz"],
+        "frac_of_dfma_probe": achieved_tf / probe["tflops"] if probe["tflops"] else None,
+        "fp64_pipe_issue_frac_at_sampled_clock": pipe_frac,
+    }
+
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, nrows, dt, threads = oracle_sample(cfg, args.cpu_seconds)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+                        "sample": f"{nrows} seeded integral-equation rows of {cfg.targets} (+ all O(NM) rows) of "
+                                  f"one F(u) at {cfg.name}, {nrows * cfg.sources:.3e} pair interactions in "
+                                  f"{dt:.1f} s, scaled by rows/T",
+                        "pairs_per_s": v * cfg.pairs}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "N": cfg.N, "M": cfg.M, "h": cfg.h, "eps": cfg.eps,
+                   "froude": cfg.froude, "jv_batch": b, "evals_per_step": evals_per_step,
+                   "pairs_per_eval": cfg.pairs, "step": "sws_residual(u) + sws_jv_batch(u, V[b])",
+                   "l2": "256 MB buffer written between timed iterations (L2 flush)",
+                   "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "plan": {"single": ctx.plan_info(1), "batch": ctx.plan_info(b + 1)}},
+        "pairs_per_s": value * cfg.pairs,
+        "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": ms_e2e / e2e_steps},
+        "gpu_launches": launches_per_step * args.steps,
+        "clocks": clocks,
+        "workspace_bytes": ctx.workspace_bytes,
+    }
+    print(json.dumps(line), flush=True)
+    ctx.close()
+    replicas.finalize()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", default="cfg5_721x241", choices=sorted(W.BY_NAME))
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline leg")
+    ap.add_argument("--ref-rows", type=int, default=2048, help="rows per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

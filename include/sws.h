@@ -1,0 +1,150 @@
+/*
+ * sws.h -- C-ABI of libsws: the nonlinear residual E(u) (called F(u) in
+ * BASELINE.json) of the boundary-integral discretisation of steady free-surface
+ * flow past a submerged source, and batched finite-difference Jacobian-vector
+ * products, on one NVIDIA B200 (sm_100a), in FP64.
+ *
+ * Paper: Pethiyagoda, McCue, Moroney & Back, "Jacobian-free Newton-Krylov
+ * methods with GPU acceleration for computing nonlinear ship wave patterns",
+ * arXiv 1403.5044.  Citations "L<n>" are lines of /root/reference/PAPER.md.
+ *
+ * What the path computes (section 3, App. A):
+ *   u in R^{2(N+1)M}, eq. (18): per y-line l = 1..M the block
+ *       [phi_{1,l}, (phi_x)_{1,l} .. (phi_x)_{N,l}], all lines; then the same for zeta.
+ *   E in R^{2(N+1)M}, App. A: per line l the block [E3_l, E4_l, E1_{1..N-1,l}],
+ *       all lines; then [E5_l, E6_l, E2_{1..N-1,l}].
+ *   a1  x-trapezoid reconstruction of zeta, phi                       eq. (19)
+ *   a2  zeta_y, phi_y by a cubic spline along y on each x-line (L160);
+ *       dy_scheme = 1 selects 2nd-order finite differences instead
+ *   a3  half-mesh values by two-point interpolation                    L162, L454
+ *   a4  all-pairs trapezoid quadrature of K1, K2 (L107, L109), each with its
+ *       y -> -y image, with the S2 singularity subtraction             eqs. (20)-(22) L164-177
+ *   a5  closed-form integral I of S2 over the truncated rectangle      eq. (23)
+ *   a6  integral-equation rows E2                                      eq. (12)
+ *   a7  Bernoulli rows E1                                              eq. (13)
+ *   a8  upstream radiation rows E3..E6, n = n_rad                      eq. (24)
+ *   a9  App. A ordering                                                L421
+ *   a10 J v ~ (E(u + sigma v) - E(u)) / sigma, b directions at once    eq. (25)
+ * Readings of the paper where it is silent or garbled are listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Every *_dev pointer is DEVICE memory owned by the caller (e.g. a PyTorch
+ *     tensor's data_ptr()), FP64, contiguous; it is never retained after the call.
+ *   - Every *_host pointer is HOST memory owned by the caller.
+ *   - The context owns all workspace.  sws_residual / sws_jv_batch only enqueue
+ *     work on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy
+ *     default stream) and return without synchronising and without allocating.
+ *   - One context must not be used from two streams at the same time.
+ *   - Results are deterministic: bitwise repeatable for fixed inputs and context.
+ *   - Return value: SWS_OK (0) or a negative error code; nothing throws across the
+ *     ABI.  There is no CPU fallback: without a CUDA device sws_setup fails with
+ *     SWS_ECUDA.
+ */
+#ifndef SWS_H_
+#define SWS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SWS_OK 0
+#define SWS_EINVAL (-1) /* bad argument (NULL pointer, N < 3, M < 4, spacing <= 0, ...) */
+#define SWS_ENOMEM (-2) /* device or host allocation failed                             */
+#define SWS_ECUDA (-3)  /* a CUDA runtime call failed; see sws_last_cuda_error()         */
+#define SWS_EBATCH (-4) /* b < 1 or b > max_batch                                        */
+
+typedef struct sws_ctx sws_ctx; /* opaque, owned by the library */
+
+typedef struct {
+  int32_t N, M;        /* mesh nodes in x and y (N >= 3, M >= 4)                       L145 */
+  double x1, y1;       /* first node; x1 = upstream truncation, configs use y1 = 0     L162 */
+  double dx, dy;       /* spacings Delta x, Delta y (> 0)                              L145 */
+  double froude, eps;  /* Froude number F, eq. (9); source strength eq. (6)         */
+  double n_rad;        /* radiation exponent n, paper value 0.05                       L189 */
+  int32_t dy_scheme;   /* 0 cubic spline (L160), 1 finite differences                       */
+  int32_t precision;   /* 0 = FP64 pair arithmetic; 1 = FP32 pair arithmetic (reported only) */
+  int32_t max_batch;   /* largest b accepted by sws_jv_batch (0 = residual only)            */
+  int32_t device;      /* CUDA ordinal                                                      */
+} sws_params;
+
+/* Validate, allocate the workspace on p->device, precompute mesh and spline tables.
+ * *out receives the context.  Synchronises the device once. */
+int sws_setup(const sws_params* p, sws_ctx** out);
+
+/* F_dev[0..n) = E(u_dev[0..n)), n = 2(N+1)M.  Steps a0-a9. */
+int sws_residual(sws_ctx* ctx, const double* u_dev, double* F_dev, void* cuda_stream);
+
+/* JV_dev[b][n] (row-major) = (E(u_b) - E(u)) / sigma_b with u_b = fma(sigma_b, v_b, u)
+ * entry by entry in FP64, for the b rows v_b of V_dev[b][n].  Step a10, eq. (25) L219.
+ *   sigma_host  [b] shifts in pageable host memory, read during the call; NULL selects
+ *               sigma_b = 1e-7 (1 + ||u||_2) / ||v_b||_2 computed on the device.
+ *   Fpert_dev   [b][n] or NULL; receives E(u_b).
+ *   F0_dev      [n] or NULL; receives E(u) (the base evaluation the batch performs anyway). */
+int sws_jv_batch(sws_ctx* ctx, const double* u_dev, const double* V_dev, int32_t b,
+                 const double* sigma_host, double* JV_dev, double* Fpert_dev, double* F0_dev,
+                 void* cuda_stream);
+
+/* The same two calls on HOST buffers: host->device copy, compute, device->host copy,
+ * then a stream synchronise.  `cuda_stream` as above. */
+int sws_residual_host(sws_ctx* ctx, const double* u_host, double* F_host, void* cuda_stream);
+int sws_jv_batch_host(sws_ctx* ctx, const double* u_host, const double* V_host, int32_t b,
+                      const double* sigma_host, double* JV_host, double* Fpert_host,
+                      double* F0_host, void* cuda_stream);
+
+/* The shifts the last sws_jv_batch used (device-computed or copied), after a
+ * synchronise of `cuda_stream`.  sigma_host_out has room for b values. */
+int sws_last_sigma(sws_ctx* ctx, int32_t b, double* sigma_host_out, void* cuda_stream);
+
+size_t sws_num_unknowns(const sws_ctx* ctx); /* 2(N+1)M */
+size_t sws_num_targets(const sws_ctx* ctx);  /* (N-1)M half-mesh points */
+size_t sws_num_sources(const sws_ctx* ctx);  /* NM nodes */
+size_t sws_workspace_bytes(const sws_ctx* ctx);
+
+/* Number of kernels the last sws_residual / sws_jv_batch call launched. */
+int sws_last_launch_count(const sws_ctx* ctx);
+
+/* Time (ms, CUDA events on `cuda_stream`) of the all-pairs kernel alone for `states`
+ * states (1 = single residual) using the fields left by the previous call; used by
+ * bench.py for the roofline of the dominant kernel.  Synchronises. */
+int sws_time_allpairs(sws_ctx* ctx, int32_t states, int32_t reps, float* ms_per_launch,
+                      void* cuda_stream);
+
+/* Live timing of the dominant kernel inside ordinary calls.  While profiling is on, every
+ * sws_residual / sws_jv_batch brackets its all-pairs launch with a CUDA event pair on the
+ * call's stream (no synchronisation, two event records per call).  sws_profile_read
+ * synchronises those events and returns the summed all-pairs time (ms) and the number of
+ * launches since the last reset; reset != 0 clears the list. */
+int sws_set_profiling(sws_ctx* ctx, int32_t on);
+int sws_profile_read(sws_ctx* ctx, double* allpairs_ms, int32_t* launches, int32_t reset);
+
+/* Tuning knob of the all-pairs launch: number of source-column groups a target tile's
+ * quadrature is split into (0 = library default, chosen from the SM count and occupancy;
+ * clamped to what the workspace was sized for). */
+int sws_set_tuning(sws_ctx* ctx, int32_t chunks);
+
+/* The all-pairs launch geometry for `states` states: out5 = {target tiles, column groups,
+ * columns per group, nodes staged per bulk copy, segments per column}. */
+int sws_plan_info(sws_ctx* ctx, int32_t states, int32_t* out5);
+
+int sws_destroy(sws_ctx* ctx);
+
+const char* sws_strerror(int code);
+const char* sws_last_cuda_error(void);
+
+/* Measurement helpers (no part of the path).
+ * sws_probe_fp64_peak: register-only DFMA loop on every SM; reports achieved FP64
+ * TFLOP/s (2 flops per DFMA), the SM count and the SM clock (MHz) read back from the
+ * device clock64/globaltimer ratio. */
+int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, double* sm_mhz);
+
+/* y[i] = the library's device reciprocal square root of x[i] (host buffers), for the
+ * unit test of that primitive. */
+int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, int32_t n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SWS_H_ */

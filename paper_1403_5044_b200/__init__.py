@@ -1,0 +1,274 @@
+"""Thin Python binding of libsws.so (include/sws.h): argument marshalling only.
+
+Every step of the path (section 3: reconstruction, all-pairs quadrature,
+Bernoulli/radiation rows, assembly; eq. (25): batched finite-difference Jv) runs in the
+CUDA kernels behind the C-ABI.  PyTorch is used for device memory and streams only.  There
+is no CPU fallback: importing works without a GPU (so that the symbols can be checked), but
+creating a `Context` needs a CUDA device and a built libsws.so.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libsws.so"
+
+SWS_OK, SWS_EINVAL, SWS_ENOMEM, SWS_ECUDA, SWS_EBATCH = 0, -1, -2, -3, -4
+
+# every symbol include/sws.h declares
+SYMBOLS = (
+    "sws_setup", "sws_residual", "sws_jv_batch", "sws_residual_host", "sws_jv_batch_host",
+    "sws_last_sigma", "sws_num_unknowns", "sws_num_targets", "sws_num_sources",
+    "sws_workspace_bytes", "sws_last_launch_count", "sws_time_allpairs", "sws_set_tuning",
+    "sws_plan_info", "sws_set_profiling", "sws_profile_read", "sws_destroy", "sws_strerror", "sws_last_cuda_error",
+    "sws_probe_fp64_peak", "sws_debug_rsqrt_host",
+)
+
+
+class SwsParams(C.Structure):
+    """sws_params of include/sws.h."""
+    _fields_ = [("N", C.c_int32), ("M", C.c_int32), ("x1", C.c_double), ("y1", C.c_double),
+                ("dx", C.c_double), ("dy", C.c_double), ("froude", C.c_double), ("eps", C.c_double),
+                ("n_rad", C.c_double), ("dy_scheme", C.c_int32), ("precision", C.c_int32),
+                ("max_batch", C.c_int32), ("device", C.c_int32)]
+
+
+class SwsError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libsws.so and declare the prototypes.  Fails loudly if it was not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise SwsError(f"{LIB_PATH} is missing: run `python -m paper_1403_5044_b200.build` "
+                       "(nvcc, sm_100a).  There is no CPU fallback.")
+    lib = C.CDLL(str(LIB_PATH))
+    vp, dp, ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)
+    proto = {
+        "sws_setup": (C.c_int, [C.POINTER(SwsParams), C.POINTER(vp)]),
+        "sws_residual": (C.c_int, [vp, dp, dp, vp]),
+        "sws_jv_batch": (C.c_int, [vp, dp, dp, C.c_int32, dp, dp, dp, dp, vp]),
+        "sws_residual_host": (C.c_int, [vp, dp, dp, vp]),
+        "sws_jv_batch_host": (C.c_int, [vp, dp, dp, C.c_int32, dp, dp, dp, dp, vp]),
+        "sws_last_sigma": (C.c_int, [vp, C.c_int32, dp, vp]),
+        "sws_num_unknowns": (C.c_size_t, [vp]),
+        "sws_num_targets": (C.c_size_t, [vp]),
+        "sws_num_sources": (C.c_size_t, [vp]),
+        "sws_workspace_bytes": (C.c_size_t, [vp]),
+        "sws_last_launch_count": (C.c_int, [vp]),
+        "sws_time_allpairs": (C.c_int, [vp, C.c_int32, C.c_int32, C.POINTER(C.c_float), vp]),
+        "sws_set_tuning": (C.c_int, [vp, C.c_int32]),
+        "sws_plan_info": (C.c_int, [vp, C.c_int32, ip]),
+        "sws_set_profiling": (C.c_int, [vp, C.c_int32]),
+        "sws_profile_read": (C.c_int, [vp, C.POINTER(C.c_double), ip, C.c_int32]),
+        "sws_destroy": (C.c_int, [vp]),
+        "sws_strerror": (C.c_char_p, [C.c_int]),
+        "sws_last_cuda_error": (C.c_char_p, []),
+        "sws_probe_fp64_peak": (C.c_int, [C.c_int32, C.POINTER(C.c_double), ip, C.POINTER(C.c_double)]),
+        "sws_debug_rsqrt_host": (C.c_int, [C.c_int32, dp, dp, C.c_int32]),
+    }
+    for name, (res, args) in proto.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != SWS_OK:
+        lib = load_library()
+        msg = lib.sws_strerror(rc).decode()
+        if rc == SWS_ECUDA:
+            msg += ": " + lib.sws_last_cuda_error().decode()
+        raise SwsError(f"{what} failed ({rc}): {msg}")
+
+
+def _np_ptr(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _torch():
+    import torch
+    return torch
+
+
+class Context:
+    """sws_setup / sws_destroy.  `params` is a dict with the keys of sws_params (N, M, x1, y1,
+    dx, dy, froude, eps, n_rad[, dy_scheme]) - e.g. workloads.Config.params()."""
+
+    def __init__(self, params: dict, max_batch: int = 0, device: int = 0, precision: int = 0):
+        self._h = None
+        self.lib = load_library()
+        p = SwsParams(int(params["N"]), int(params["M"]), float(params["x1"]), float(params["y1"]),
+                      float(params["dx"]), float(params["dy"]), float(params["froude"]),
+                      float(params["eps"]), float(params["n_rad"]), int(params.get("dy_scheme", 0)),
+                      int(precision), int(max_batch), int(device))
+        h = C.c_void_p()
+        _check(self.lib.sws_setup(C.byref(p), C.byref(h)), "sws_setup")
+        self._h = h
+        self.device = int(device)
+        self.max_batch = int(max_batch)
+        self.n = int(self.lib.sws_num_unknowns(h))
+        self.targets = int(self.lib.sws_num_targets(h))
+        self.sources = int(self.lib.sws_num_sources(h))
+
+    # -- lifetime ------------------------------------------------------------------
+    def close(self) -> None:
+        if self._h is not None:
+            self.lib.sws_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- helpers ---------------------------------------------------------------------
+    def _stream(self, stream=None) -> C.c_void_p:
+        torch = _torch()
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        return C.c_void_p(s.cuda_stream)
+
+    def _dev(self, t, shape, name):
+        torch = _torch()
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64
+                and t.is_contiguous() and t.device.index == self.device):
+            raise SwsError(f"{name}: need a contiguous float64 CUDA tensor on device {self.device}")
+        if tuple(t.shape) != tuple(shape):
+            raise SwsError(f"{name}: shape {tuple(t.shape)} != {tuple(shape)}")
+        return C.c_void_p(t.data_ptr())
+
+    def _new(self, *shape):
+        torch = _torch()
+        return torch.empty(shape, dtype=torch.float64, device=f"cuda:{self.device}")
+
+    # -- the path ----------------------------------------------------------------------
+    def residual(self, u, out=None, stream=None):
+        """F = E(u) on device tensors (sws_residual); asynchronous on the stream."""
+        F = out if out is not None else self._new(self.n)
+        _check(self.lib.sws_residual(self._h, self._dev(u, (self.n,), "u"),
+                                     self._dev(F, (self.n,), "F"), self._stream(stream)), "sws_residual")
+        return F
+
+    def jv_batch(self, u, V, sigma=None, want_fpert: bool = False, want_f0: bool = False, stream=None):
+        """JV[b] = (E(u + sigma_b v_b) - E(u)) / sigma_b (sws_jv_batch).  sigma: None (device
+        formula 1e-7 (1 + |u|) / |v_b|) or b host floats.  Returns JV or (JV, Fpert, F0)."""
+        b = int(V.shape[0])
+        JV = self._new(b, self.n)
+        Fp = self._new(b, self.n) if want_fpert else None
+        F0 = self._new(self.n) if want_f0 else None
+        sg = None
+        if sigma is not None:
+            sg = np.ascontiguousarray(sigma, dtype=np.float64)
+            if sg.shape != (b,):
+                raise SwsError("sigma: need b values")
+        rc = self.lib.sws_jv_batch(
+            self._h, self._dev(u, (self.n,), "u"), self._dev(V, (b, self.n), "V"), b,
+            _np_ptr(sg) if sg is not None else None, C.c_void_p(JV.data_ptr()),
+            C.c_void_p(Fp.data_ptr()) if Fp is not None else None,
+            C.c_void_p(F0.data_ptr()) if F0 is not None else None, self._stream(stream))
+        _check(rc, "sws_jv_batch")
+        if want_fpert or want_f0:
+            return JV, Fp, F0
+        return JV
+
+    def residual_host(self, u: np.ndarray, out: np.ndarray | None = None, stream=None) -> np.ndarray:
+        """E(u) on HOST buffers (sws_residual_host): H2D copy, compute, D2H copy, synchronise."""
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        if u.shape != (self.n,):
+            raise SwsError("u: wrong length")
+        F = out if out is not None else np.empty(self.n)
+        _check(self.lib.sws_residual_host(self._h, _np_ptr(u), _np_ptr(F), self._stream(stream)),
+               "sws_residual_host")
+        return F
+
+    def jv_batch_host(self, u: np.ndarray, V: np.ndarray, sigma=None, out=None, fpert=None, f0=None,
+                      stream=None):
+        """Batched Jv on HOST buffers (sws_jv_batch_host).  Returns (JV, Fpert, F0)."""
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        V = np.ascontiguousarray(V, dtype=np.float64)
+        b = int(V.shape[0])
+        if u.shape != (self.n,) or V.shape != (b, self.n):
+            raise SwsError("u/V: wrong shape")
+        JV = out if out is not None else np.empty((b, self.n))
+        Fp = fpert if fpert is not None else np.empty((b, self.n))
+        F0 = f0 if f0 is not None else np.empty(self.n)
+        sg = np.ascontiguousarray(sigma, dtype=np.float64) if sigma is not None else None
+        rc = self.lib.sws_jv_batch_host(self._h, _np_ptr(u), _np_ptr(V), b,
+                                        _np_ptr(sg) if sg is not None else None, _np_ptr(JV),
+                                        _np_ptr(Fp), _np_ptr(F0), self._stream(stream))
+        _check(rc, "sws_jv_batch_host")
+        return JV, Fp, F0
+
+    def last_sigma(self, b: int, stream=None) -> np.ndarray:
+        out = np.empty(int(b))
+        _check(self.lib.sws_last_sigma(self._h, int(b), _np_ptr(out), self._stream(stream)), "sws_last_sigma")
+        return out
+
+    # -- measurement / tuning ------------------------------------------------------------
+    def time_allpairs(self, states: int = 1, reps: int = 1, stream=None) -> float:
+        """ms per launch of the all-pairs kernel alone (CUDA events on the stream)."""
+        ms = C.c_float()
+        _check(self.lib.sws_time_allpairs(self._h, int(states), int(reps), C.byref(ms),
+                                          self._stream(stream)), "sws_time_allpairs")
+        return float(ms.value)
+
+    def set_profiling(self, on: bool = True) -> None:
+        _check(self.lib.sws_set_profiling(self._h, int(bool(on))), "sws_set_profiling")
+
+    def profile_read(self, reset: bool = True):
+        """(summed all-pairs kernel ms, launches) since the last reset; synchronises."""
+        ms, n = C.c_double(), C.c_int32()
+        _check(self.lib.sws_profile_read(self._h, C.byref(ms), C.byref(n), int(bool(reset))),
+               "sws_profile_read")
+        return float(ms.value), int(n.value)
+
+    def set_tuning(self, chunks: int = 0) -> None:
+        _check(self.lib.sws_set_tuning(self._h, int(chunks)), "sws_set_tuning")
+
+    def plan_info(self, states: int = 1) -> dict:
+        out = (C.c_int32 * 5)()
+        _check(self.lib.sws_plan_info(self._h, int(states), out), "sws_plan_info")
+        return dict(tiles=out[0], chunks=out[1], cols_per_chunk=out[2], seg_len=out[3], nseg=out[4])
+
+    @property
+    def last_launch_count(self) -> int:
+        return int(self.lib.sws_last_launch_count(self._h))
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(self.lib.sws_workspace_bytes(self._h))
+
+
+def probe_fp64_peak(device: int = 0) -> dict:
+    """Register-only DFMA microbenchmark: {'tflops', 'sm_count', 'sm_mhz'} (sws_probe_fp64_peak)."""
+    lib = load_library()
+    tf, sms, mhz = C.c_double(), C.c_int32(), C.c_double()
+    _check(lib.sws_probe_fp64_peak(int(device), C.byref(tf), C.byref(sms), C.byref(mhz)),
+           "sws_probe_fp64_peak")
+    return dict(tflops=tf.value, sm_count=int(sms.value), sm_mhz=mhz.value)
+
+
+def debug_rsqrt(x: np.ndarray, device: int = 0) -> np.ndarray:
+    """The library's device reciprocal square root applied to host values (unit test hook)."""
+    lib = load_library()
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    y = np.empty_like(x)
+    _check(lib.sws_debug_rsqrt_host(int(device), _np_ptr(x), _np_ptr(y), int(x.size)), "sws_debug_rsqrt_host")
+    return y

@@ -1,0 +1,312 @@
+// Step a4: the all-pairs trapezoid quadrature of eq. (12) with the
+// singularity subtraction of L181, for every half-mesh target and every state.
+//
+//   sum_{i,j} w(i,j) [ (phi_ij - phi* - x_i + x*) K1 + (zeta_x)_ij K2 - zeta_x* S2 ]
+//   K1 (L107, reading Q1/Q2), K2 (L109), S2 = S2_direct + S2_image (eqs. (21),(22) L169-172),
+//   w(i,j) = dx dy c_i c_j, c = 1/2 on the first/last index (L189, reading Q4).
+//
+// Mapping (B200): one thread = one target, 128 targets per CTA; a CTA walks a group of
+// source COLUMNS (fixed x_i, all y_j).  Each column (M records of 32 B, contiguous in the
+// transposed SrcRec layout) is brought into shared memory by ONE bulk async copy
+// (cp.async.bulk -> UBLKCP, completion on an mbarrier), double buffered.  Every lane of a
+// warp reads the same record (shared-memory broadcast), so the kernel is bound by the FP64
+// pipe: 45 FP64 instructions + 4 MUFU.RSQ64H per pair.  Everything that depends only on
+// (target, column) - dx, dx^2, A dx^2, B dx - is hoisted out of the j loop; the half
+// weights are applied by peeling the first/last node and scaling edge columns, so the
+// inner loop carries no weight multiply.  Partial sums per (state, chunk, target) are
+// written to global memory and added in a fixed order by the assemble kernel: no atomics,
+// bitwise repeatable.
+#include "sws_internal.cuh"
+
+namespace sws {
+
+// 1/sqrt(x) for normal positive x, full double precision.
+// Seed: MUFU.RSQ64H (PTX rsqrt.approx.ftz.f64: works on the upper 32 bits of x, so the seed
+// carries a relative error d with |d| < ~2^-20).  With e = 1 - x y0^2 (= -2d - d^2) the
+// exact result is y0 (1 - e)^(-1/2) = y0 (1 + e/2 + 3e^2/8 + 5e^3/16 + ...); the two-term
+// correction below leaves 5/16 |e|^3 < 2^-59, i.e. below the rounding of the final FMA.
+// 5 FP64 instructions (DMUL, DFMA, DFMA, DMUL, DFMA) + 1 MUFU.
+__device__ __forceinline__ double rsqrt_seed(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  return y;
+}
+
+__device__ __forceinline__ double rsqrt_fp64(double x) {
+  const double y0 = rsqrt_seed(x);
+  const double t = x * y0;
+  const double e = fma(-t, y0, 1.0);
+  const double p = fma(0.375, e, 0.5);
+  const double ye = y0 * e;
+  return fma(ye, p, y0);
+}
+
+// Per-thread constants of one target and of the current source column.
+struct TgtC {
+  double ys, zs, psis, C;
+};
+struct ColC {
+  double dx, dx2, Adx2, Bdx;  // x_i - x*, its square, A dx^2, B dx
+};
+
+// One source node against one target: adds (phi-phi*-x+x*) K1 + zeta_x K2 to a1 and
+// S2 to aS (unit weight).
+__device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, const double yj,
+                                          const TgtC& t, const ColC& c, double& a1, double& aS) {
+  const double z = zp.x, psi = zp.y, zx = sl.x, zy = sl.y;
+  const double dm = yj - t.ys;  // y - y*
+  const double dp = yj + t.ys;  // y + y*  (image, L107-109)
+  const double dz = z - t.zs;
+  const double q = fma(dz, dz, c.dx2);
+  const double Rm2 = fma(dm, dm, q);
+  const double Rp2 = fma(dp, dp, q);
+  const double rm = rsqrt_fp64(Rm2);
+  const double rp = rsqrt_fp64(Rp2);
+  // K1 numerators: zeta - zeta* - (x-x*) zeta_x - (y -+ y*) zeta_y, slopes at the source (Q2)
+  const double n0 = fma(-c.dx, zx, dz);
+  const double nm = fma(-dm, zy, n0);
+  const double np = fma(-dp, zy, n0);
+  const double rm3 = (rm * rm) * rm;
+  const double rp3 = (rp * rp) * rp;
+  const double k1 = fma(np, rp3, nm * rm3);
+  const double dpsi = psi - t.psis;
+  a1 = fma(dpsi, k1, a1);
+  a1 = fma(zx, rm + rp, a1);  // K2 = 1/R- + 1/R+
+  // S2: A dx^2 + B dx (y-y*) + C (y-y*)^2  and  A dx^2 - B dx (y+y*) + C (y+y*)^2
+  const double Qm = fma(fma(t.C, dm, c.Bdx), dm, c.Adx2);
+  const double Qp = fma(fma(t.C, dp, -c.Bdx), dp, c.Adx2);
+  aS += rsqrt_fp64(Qm) + rsqrt_fp64(Qp);
+}
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+               "r"(bytes)
+               : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
+// global -> shared bulk async copy (TMA engine, 1-D), bytes % 16 == 0, both 16 B aligned.
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+
+struct PairArgs {
+  const SrcRec* src;  // [state][N][M]
+  const double* x;    // [N]
+  const double* y;    // [M + pad]
+  const TgtRec* tgt;  // [state][T]
+  double* part;       // [state][chunks][T]
+  int N, M, T;
+  int chunks, cols_per_chunk, seg_len, nseg;
+  double dxdy;
+};
+
+template <int MINB>
+__global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs a) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int seg_pad = a.seg_len;  // even by construction
+  SrcRec* s_rec = reinterpret_cast<SrcRec*>(smem_raw);                            // [kStages][seg_pad]
+  double* s_y = reinterpret_cast<double*>(s_rec + (size_t)kStages * seg_pad);     // [kStages][seg_pad]
+  uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_y + (size_t)kStages * seg_pad);  // [kStages]
+
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x, chunk = blockIdx.y, state = blockIdx.z;
+  const int t = tile * kPairThreads + tid;
+  const int tc = t < a.T ? t : a.T - 1;  // ragged tail: recompute the last target, never stored
+
+  const TgtRec tr = a.tgt[(size_t)state * a.T + tc];
+  const TgtC tg = {tr.ys, tr.zs, tr.psis, tr.C};
+  const double xs = tr.xs, tA = tr.A, tB = tr.B;
+
+  const int c0 = chunk * a.cols_per_chunk;
+  const int c1 = min(a.N, c0 + a.cols_per_chunk);
+  const int nitems = (c1 - c0) * a.nseg;  // (column, segment) work items of this CTA
+  const SrcRec* src = a.src + (size_t)state * a.N * a.M;
+
+  if (tid == 0) {
+    for (int s = 0; s < kStages; ++s) mbar_init(&s_bar[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  auto issue = [&](int q) {
+    const int s = q % kStages;
+    const int i = c0 + q / a.nseg, j0 = (q % a.nseg) * a.seg_len;
+    const int len = min(a.seg_len, a.M - j0);
+    const uint32_t rec_bytes = (uint32_t)len * (uint32_t)sizeof(SrcRec);
+    const uint32_t y_bytes = (uint32_t)((len + 1) & ~1) * 8u;  // y is padded to an even count
+    mbar_expect_tx(&s_bar[s], rec_bytes + y_bytes);
+    bulk_g2s(s_rec + (size_t)s * seg_pad, src + (size_t)i * a.M + j0, rec_bytes, &s_bar[s]);
+    bulk_g2s(s_y + (size_t)s * seg_pad, a.y + j0, y_bytes, &s_bar[s]);
+  };
+
+  if (tid == 0 && nitems > 0) issue(0);
+
+  double tot1 = 0.0, totS = 0.0;
+  for (int q = 0; q < nitems; ++q) {
+    const int s = q % kStages;
+    // the buffer written here was last read in iteration q-1, which ended with __syncthreads()
+    if (tid == 0 && q + 1 < nitems) issue(q + 1);
+
+    const int i = c0 + q / a.nseg, j0 = (q % a.nseg) * a.seg_len;
+    const int len = min(a.seg_len, a.M - j0);
+    ColC cc;
+    cc.dx = __ldg(a.x + i) - xs;
+    cc.dx2 = cc.dx * cc.dx;
+    cc.Adx2 = tA * cc.dx2;
+    cc.Bdx = tB * cc.dx;
+    const double ci = (i == 0 || i == a.N - 1) ? 0.5 : 1.0;  // trapezoid weight in x (Q4)
+
+    mbar_wait(&s_bar[s], (uint32_t)((q / kStages) & 1));
+
+    const double2* rec = reinterpret_cast<const double2*>(s_rec + (size_t)s * seg_pad);
+    const double* yy = s_y + (size_t)s * seg_pad;
+    double col1 = 0.0, colS = 0.0;
+    int jlo = 0, jhi = len;
+    if (j0 == 0) {  // first node of the column: weight 1/2 in y
+      double h1 = 0.0, hS = 0.0;
+      pair_term(rec[0], rec[1], yy[0], tg, cc, h1, hS);
+      col1 = 0.5 * h1;
+      colS = 0.5 * hS;
+      jlo = 1;
+    }
+    const bool last = (j0 + len == a.M);
+    if (last) jhi = len - 1;
+#pragma unroll 2
+    for (int j = jlo; j < jhi; ++j) pair_term(rec[2 * j], rec[2 * j + 1], yy[j], tg, cc, col1, colS);
+    if (last && jhi >= jlo) {  // last node of the column: weight 1/2 in y
+      double h1 = 0.0, hS = 0.0;
+      pair_term(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], tg, cc, h1, hS);
+      col1 = fma(0.5, h1, col1);
+      colS = fma(0.5, hS, colS);
+    }
+    tot1 = fma(ci, col1, tot1);
+    totS = fma(ci, colS, totS);
+    __syncthreads();
+  }
+
+  if (t < a.T)
+    a.part[((size_t)state * a.chunks + chunk) * a.T + t] = a.dxdy * fma(-tr.zxs, totS, tot1);
+}
+
+// ---------------------------------------------------------------------------------------
+// host side
+
+static int g_occ = 0;  // resident CTAs per SM of the instantiation in use
+constexpr int kMinB = 6;
+
+size_t allpairs_smem_bytes(const PairPlan& p) {
+  return (size_t)kStages * p.seg_len * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
+}
+
+cudaError_t allpairs_configure() {
+  cudaError_t e = cudaFuncSetAttribute(k_allpairs<kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)(kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + 64));
+  if (e != cudaSuccess) return e;
+  int occ = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+      &occ, k_allpairs<kMinB>, kPairThreads,
+      kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t));
+  if (e != cudaSuccess) return e;
+  g_occ = occ > 0 ? occ : 1;
+  return cudaSuccess;
+}
+
+// Choose the number of column groups so that (a) the grid is many waves of the
+// sm_count * occupancy resident CTAs and (b) wave quantisation of both the grid and the
+// columns-per-CTA count is small.  cost(c) ~ ceil(CTAs / slots) * (ceil(N / c) + overhead).
+// The split depends on the MESH ONLY, never on the number of states in the launch: the
+// summation order of a state's quadrature is then the same in sws_residual and in every
+// slot of sws_jv_batch, so a batch is bitwise a loop of single evaluations.
+PairPlan make_plan(const sws_ctx* c) {
+  const Mesh& m = c->mesh;
+  PairPlan p;
+  p.tiles = (m.T + kPairThreads - 1) / kPairThreads;
+  p.nseg = (m.M + kSegMax - 1) / kSegMax;
+  int seg = (m.M + p.nseg - 1) / p.nseg;
+  p.seg_len = (seg + 1) & ~1;
+  p.nseg = (m.M + p.seg_len - 1) / p.seg_len;
+  const long slots = (long)c->sm_count * (g_occ > 0 ? g_occ : 4);
+  int best = 1;
+  // a CTA should see at least ~256 source nodes
+  int min_cols = (256 + m.M - 1) / m.M;
+  int cmax = m.N / (min_cols > 0 ? min_cols : 1);
+  if (cmax < 1) cmax = 1;
+  if (cmax > 256) cmax = 256;
+  if (c->chunks_user > 0) {
+    best = c->chunks_user < cmax ? c->chunks_user : cmax;
+  } else {
+    double best_cost = 1e300;
+    for (int ch = 1; ch <= cmax; ++ch) {
+      const int cols = (m.N + ch - 1) / ch;
+      const int used = (m.N + cols - 1) / cols;  // groups that are not empty
+      if (used != ch) continue;
+      const long ctas = (long)p.tiles * ch;
+      const long waves = (ctas + slots - 1) / slots;
+      const double cost = (double)waves * (cols + 0.25) + 1e-3 * ch;
+      if (cost < best_cost) { best_cost = cost; best = ch; }
+    }
+  }
+  p.cols_per_chunk = (m.N + best - 1) / best;
+  p.chunks = (m.N + p.cols_per_chunk - 1) / p.cols_per_chunk;
+  return p;
+}
+
+int max_chunks(const sws_ctx* c) {
+  int min_cols = (256 + c->mesh.M - 1) / c->mesh.M;
+  int cmax = c->mesh.N / (min_cols > 0 ? min_cols : 1);
+  if (cmax < 1) cmax = 1;
+  if (cmax > 256) cmax = 256;
+  return cmax;
+}
+
+cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st) {
+  const Mesh& m = c->mesh;
+  PairArgs a;
+  a.src = c->src; a.x = c->x; a.y = c->y; a.tgt = c->tgt; a.part = c->part;
+  a.N = m.N; a.M = m.M; a.T = m.T;
+  a.chunks = plan.chunks; a.cols_per_chunk = plan.cols_per_chunk;
+  a.seg_len = plan.seg_len; a.nseg = plan.nseg;
+  a.dxdy = m.dx * m.dy;
+  dim3 grid(plan.tiles, plan.chunks, states);
+  k_allpairs<kMinB><<<grid, kPairThreads, allpairs_smem_bytes(plan), st>>>(a);
+  return cudaGetLastError();
+}
+
+// --- unit-test hook for the reciprocal square root --------------------------------------
+__global__ void k_debug_rsqrt(const double* x, double* y, int n) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) y[i] = rsqrt_fp64(x[i]);
+}
+
+cudaError_t launch_debug_rsqrt(const double* x, double* y, int n, cudaStream_t st) {
+  k_debug_rsqrt<<<(n + 255) / 256, 256, 0, st>>>(x, y, n);
+  return cudaGetLastError();
+}
+
+}  // namespace sws

@@ -1,0 +1,418 @@
+// C-ABI of libsws (include/sws.h): context, workspace and the call sequences of
+// sws_residual (steps a0-a9) and sws_jv_batch (step a10).  Host code only; the kernels
+// live in sws_fields.cu and sws_allpairs.cu.  No CPU fallback anywhere: without a CUDA
+// device sws_setup fails with SWS_ECUDA.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "sws_internal.cuh"
+
+namespace sws {
+cudaError_t launch_debug_rsqrt(const double* x, double* y, int n, cudaStream_t st);
+cudaError_t launch_fp64_probe(int blocks, int iters, double* sink, unsigned long long* clk,
+                              cudaStream_t st);
+}  // namespace sws
+
+static thread_local char g_cuda_err[256] = "";
+
+static int cuda_fail(cudaError_t e, const char* where) {
+  snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s", where, cudaGetErrorString(e));
+  return SWS_ECUDA;
+}
+
+#define CK(call)                                              \
+  do {                                                        \
+    cudaError_t e_ = (call);                                  \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call);       \
+  } while (0)
+
+template <typename T>
+static cudaError_t dev_alloc(T** p, size_t count, size_t* total) {
+  size_t bytes = count * sizeof(T);
+  if (bytes == 0) bytes = sizeof(T);
+  *total += bytes;
+  return cudaMalloc((void**)p, bytes);
+}
+
+static void free_all(sws_ctx* c) {
+  void* ptrs[] = {c->x, c->y, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zx, c->px, c->zy, c->py,
+                  c->src, c->tgt, c->e2loc, c->part, c->F0, c->Fpert, c->sigma, c->norm_part,
+                  c->u_stage, c->V_stage, c->out_stage};
+  for (void* p : ptrs)
+    if (p) cudaFree(p);
+  if (c->ev0) cudaEventDestroy(c->ev0);
+  if (c->ev1) cudaEventDestroy(c->ev1);
+  if (c->prof_events) {
+    for (cudaEvent_t ev : *c->prof_events) cudaEventDestroy(ev);
+    delete c->prof_events;
+  }
+}
+
+extern "C" {
+
+const char* sws_strerror(int code) {
+  switch (code) {
+    case SWS_OK: return "ok";
+    case SWS_EINVAL: return "invalid argument";
+    case SWS_ENOMEM: return "out of memory";
+    case SWS_ECUDA: return "CUDA runtime error (see sws_last_cuda_error)";
+    case SWS_EBATCH: return "batch size out of range";
+    default: return "unknown error";
+  }
+}
+
+const char* sws_last_cuda_error(void) { return g_cuda_err; }
+
+int sws_setup(const sws_params* p, sws_ctx** out) {
+  if (!p || !out) return SWS_EINVAL;
+  *out = nullptr;
+  if (p->N < 3 || p->M < 4 || !(p->dx > 0) || !(p->dy > 0) || !(p->froude > 0)) return SWS_EINVAL;
+  if (p->dy_scheme != 0 && p->dy_scheme != 1) return SWS_EINVAL;
+  if (p->precision != 0) return SWS_EINVAL;  // FP32 pair arithmetic: not built yet
+  if (p->max_batch < 0 || p->max_batch > 1024) return SWS_EINVAL;
+  if ((long long)p->N * p->M > (1ll << 30)) return SWS_EINVAL;
+  if (sws::reconstruct_smem_bytes(p->N) > 200 * 1024) return SWS_EINVAL;  // N <= 6400
+
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (p->device < 0 || p->device >= ndev) return SWS_EINVAL;
+  CK(cudaSetDevice(p->device));
+
+  sws_ctx* c = new (std::nothrow) sws_ctx();
+  if (!c) return SWS_ENOMEM;
+  memset(c, 0, sizeof *c);
+  c->params = *p;
+  c->device = p->device;
+  sws::Mesh& m = c->mesh;
+  m.N = p->N; m.M = p->M;
+  m.T = (p->N - 1) * p->M; m.S = p->N * p->M; m.n = 2 * (p->N + 1) * p->M;
+  m.x1 = p->x1; m.y1 = p->y1; m.dx = p->dx; m.dy = p->dy;
+  m.froude = p->froude; m.eps = p->eps; m.n_rad = p->n_rad;
+  m.dy_scheme = p->dy_scheme;
+  m.sym_first = (p->y1 == 0.0) ? 1 : 0;
+  c->max_states = p->max_batch + 1;
+
+  cudaDeviceProp prop;
+  cudaError_t e = cudaGetDeviceProperties(&prop, p->device);
+  if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaGetDeviceProperties"); }
+  c->sm_count = prop.multiProcessorCount;
+
+  e = sws::allpairs_configure();
+  if (e == cudaSuccess) e = sws::fields_configure(c);
+  if (e != cudaSuccess) { delete c; return cuda_fail(e, "kernel configuration (is this an sm_100 device?)"); }
+
+  // workspace
+  const size_t S = m.S, T = m.T, n = m.n, st = c->max_states, mb = p->max_batch;
+  // partial sums: [state][chunk][t]; capacity for the automatic plan, or 32 groups if more
+  // (room for sws_set_tuning experiments), never more than the mesh allows
+  int part_chunks = sws::make_plan(c).chunks;
+  if (part_chunks < 32) part_chunks = 32;
+  if (part_chunks > sws::max_chunks(c)) part_chunks = sws::max_chunks(c);
+  if (part_chunks < sws::make_plan(c).chunks) part_chunks = sws::make_plan(c).chunks;
+  c->part_chunks = part_chunks;
+  const size_t part_elems = (size_t)part_chunks * c->max_states * T;
+  size_t tot = 0;
+  bool ok = true;
+#define ALLOC(ptr, count) ok = ok && (dev_alloc(&c->ptr, (count), &tot) == cudaSuccess)
+  ALLOC(x, (size_t)m.N + 2);
+  ALLOC(y, (size_t)m.M + 2);
+  ALLOC(sp_cp, (size_t)m.M);
+  ALLOC(sp_inv, (size_t)m.M);
+  ALLOC(zeta, st * S); ALLOC(phi, st * S); ALLOC(zx, st * S);
+  ALLOC(px, st * S); ALLOC(zy, st * S); ALLOC(py, st * S);
+  ALLOC(src, st * S);
+  ALLOC(tgt, st * T);
+  ALLOC(e2loc, st * T);
+  ALLOC(part, part_elems);
+  ALLOC(F0, n);
+  ALLOC(Fpert, mb * n);
+  ALLOC(sigma, mb);
+  ALLOC(norm_part, st * sws::kNormBlocks);
+  ALLOC(u_stage, n);
+  ALLOC(V_stage, mb * n);
+  ALLOC(out_stage, (2 * mb + 1) * n);
+#undef ALLOC
+  if (!ok) {
+    cudaGetLastError();
+    free_all(c);
+    delete c;
+    return SWS_ENOMEM;
+  }
+  c->ws_bytes = tot;
+
+  // mesh (L145): x_k = x_1 + (k-1) dx, y_l = y_1 + (l-1) dy, in FP64
+  std::vector<double> hx(m.N + 2, 0.0), hy(m.M + 2, 0.0), cp(m.M, 0.0), inv(m.M, 0.0);
+  for (int k = 0; k < m.N; ++k) hx[k] = p->x1 + (double)k * p->dx;
+  for (int l = 0; l < m.M; ++l) hy[l] = p->y1 + (double)l * p->dy;
+  // Thomas factors of the spline system (see k_dy): rows (a_l, b_l, c_l)
+  {
+    const int M = m.M;
+    const double c0 = m.sym_first ? 0.0 : 2.0;  // first row: m_1 = 0, or m_1 + 2 m_2 = ...
+    inv[0] = 1.0;
+    cp[0] = c0;
+    for (int l = 1; l < M; ++l) {
+      const double a = (l == M - 1) ? 2.0 : 1.0, b = (l == M - 1) ? 1.0 : 4.0,
+                   cc = (l == M - 1) ? 0.0 : 1.0;
+      const double den = b - a * cp[l - 1];
+      inv[l] = 1.0 / den;
+      cp[l] = cc / den;
+    }
+  }
+  e = cudaMemcpy(c->x, hx.data(), hx.size() * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(c->y, hy.data(), hy.size() * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(c->sp_cp, cp.data(), cp.size() * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(c->sp_inv, inv.data(), inv.size() * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
+  if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) {
+    free_all(c);
+    delete c;
+    return cuda_fail(e, "sws_setup upload");
+  }
+  *out = c;
+  return SWS_OK;
+}
+
+int sws_destroy(sws_ctx* c) {
+  if (!c) return SWS_EINVAL;
+  cudaSetDevice(c->device);
+  cudaDeviceSynchronize();
+  free_all(c);
+  delete c;
+  return SWS_OK;
+}
+
+size_t sws_num_unknowns(const sws_ctx* c) { return c ? (size_t)c->mesh.n : 0; }
+size_t sws_num_targets(const sws_ctx* c) { return c ? (size_t)c->mesh.T : 0; }
+size_t sws_num_sources(const sws_ctx* c) { return c ? (size_t)c->mesh.S : 0; }
+size_t sws_workspace_bytes(const sws_ctx* c) { return c ? c->ws_bytes : 0; }
+int sws_last_launch_count(const sws_ctx* c) { return c ? c->last_launches : 0; }
+
+int sws_set_tuning(sws_ctx* c, int32_t chunks) {
+  if (!c || chunks < 0) return SWS_EINVAL;
+  if (chunks > c->part_chunks) chunks = c->part_chunks;  // the partial-sum buffer is sized at setup
+  c->chunks_user = chunks;
+  return SWS_OK;
+}
+
+// a0-a9 for `states` states (state 0 = u, state s = u + sigma_{s-1} v_{s-1}).
+static int run_states(sws_ctx* c, const double* u, const double* V, int states, double* F0,
+                      double* Fpert, cudaStream_t st, int* launches) {
+  const sws::PairPlan plan = sws::make_plan(c);
+  CK(sws::launch_reconstruct(c, u, V, states, F0, Fpert, st));
+  CK(sws::launch_dy(c, states, st));
+  CK(sws::launch_targets(c, states, F0, Fpert, st));
+  cudaEvent_t pe0 = nullptr, pe1 = nullptr;
+  if (c->profiling) {
+    if (!c->prof_events) c->prof_events = new (std::nothrow) std::vector<cudaEvent_t>();
+    if (!c->prof_events) return SWS_ENOMEM;
+    while (c->prof_events->size() < c->prof_used + 2) {
+      cudaEvent_t ev;
+      CK(cudaEventCreate(&ev));
+      c->prof_events->push_back(ev);
+    }
+    pe0 = (*c->prof_events)[c->prof_used];
+    pe1 = (*c->prof_events)[c->prof_used + 1];
+    c->prof_used += 2;
+    CK(cudaEventRecord(pe0, st));
+  }
+  CK(sws::launch_allpairs(c, states, plan, st));
+  if (pe1) CK(cudaEventRecord(pe1, st));
+  CK(sws::launch_assemble(c, states, plan, F0, Fpert, st));
+  *launches += 5;
+  c->last_states = states;
+  return SWS_OK;
+}
+
+int sws_residual(sws_ctx* c, const double* u_dev, double* F_dev, void* cuda_stream) {
+  if (!c || !u_dev || !F_dev) return SWS_EINVAL;
+  CK(cudaSetDevice(c->device));
+  int launches = 0;
+  int rc = run_states(c, u_dev, nullptr, 1, F_dev, nullptr, (cudaStream_t)cuda_stream, &launches);
+  c->last_launches = launches;
+  return rc;
+}
+
+int sws_jv_batch(sws_ctx* c, const double* u_dev, const double* V_dev, int32_t b,
+                 const double* sigma_host, double* JV_dev, double* Fpert_dev, double* F0_dev,
+                 void* cuda_stream) {
+  if (!c || !u_dev || !V_dev || !JV_dev) return SWS_EINVAL;
+  if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int launches = 0;
+  if (sigma_host) {
+    CK(cudaMemcpyAsync(c->sigma, sigma_host, (size_t)b * sizeof(double), cudaMemcpyHostToDevice, st));
+  } else {
+    CK(sws::launch_sigma(c, u_dev, V_dev, b, st));
+    launches += 2;
+  }
+  double* F0 = F0_dev ? F0_dev : c->F0;
+  double* Fp = Fpert_dev ? Fpert_dev : c->Fpert;
+  int rc = run_states(c, u_dev, V_dev, b + 1, F0, Fp, st, &launches);
+  if (rc != SWS_OK) return rc;
+  CK(sws::launch_jv_quotient(c, F0, Fp, b, JV_dev, st));
+  launches += 1;
+  c->last_launches = launches;
+  return SWS_OK;
+}
+
+int sws_residual_host(sws_ctx* c, const double* u_host, double* F_host, void* cuda_stream) {
+  if (!c || !u_host || !F_host) return SWS_EINVAL;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nb = (size_t)c->mesh.n * sizeof(double);
+  CK(cudaMemcpyAsync(c->u_stage, u_host, nb, cudaMemcpyHostToDevice, st));
+  int rc = sws_residual(c, c->u_stage, c->out_stage, cuda_stream);
+  if (rc != SWS_OK) return rc;
+  CK(cudaMemcpyAsync(F_host, c->out_stage, nb, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  return SWS_OK;
+}
+
+int sws_jv_batch_host(sws_ctx* c, const double* u_host, const double* V_host, int32_t b,
+                      const double* sigma_host, double* JV_host, double* Fpert_host,
+                      double* F0_host, void* cuda_stream) {
+  if (!c || !u_host || !V_host || !JV_host) return SWS_EINVAL;
+  if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t n = c->mesh.n, nb = n * sizeof(double);
+  CK(cudaMemcpyAsync(c->u_stage, u_host, nb, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(c->V_stage, V_host, nb * b, cudaMemcpyHostToDevice, st));
+  double* JV = c->out_stage;                              // [b][n]
+  double* Fp = c->out_stage + (size_t)b * n;              // [b][n]
+  double* F0 = c->out_stage + (size_t)2 * b * n;          // [n]
+  int rc = sws_jv_batch(c, c->u_stage, c->V_stage, b, sigma_host, JV, Fp, F0, cuda_stream);
+  if (rc != SWS_OK) return rc;
+  CK(cudaMemcpyAsync(JV_host, JV, nb * b, cudaMemcpyDeviceToHost, st));
+  if (Fpert_host) CK(cudaMemcpyAsync(Fpert_host, Fp, nb * b, cudaMemcpyDeviceToHost, st));
+  if (F0_host) CK(cudaMemcpyAsync(F0_host, F0, nb, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  return SWS_OK;
+}
+
+int sws_last_sigma(sws_ctx* c, int32_t b, double* sigma_host_out, void* cuda_stream) {
+  if (!c || !sigma_host_out) return SWS_EINVAL;
+  if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CK(cudaMemcpyAsync(sigma_host_out, c->sigma, (size_t)b * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  return SWS_OK;
+}
+
+int sws_time_allpairs(sws_ctx* c, int32_t states, int32_t reps, float* ms_per_launch,
+                      void* cuda_stream) {
+  if (!c || !ms_per_launch || reps < 1) return SWS_EINVAL;
+  if (states < 1 || states > c->max_states || states > c->last_states) return SWS_EBATCH;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const sws::PairPlan plan = sws::make_plan(c);
+  CK(sws::launch_allpairs(c, states, plan, st));  // warm-up
+  CK(cudaEventRecord(c->ev0, st));
+  for (int r = 0; r < reps; ++r) CK(sws::launch_allpairs(c, states, plan, st));
+  CK(cudaEventRecord(c->ev1, st));
+  CK(cudaEventSynchronize(c->ev1));
+  float ms = 0.f;
+  CK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+  *ms_per_launch = ms / reps;
+  return SWS_OK;
+}
+
+int sws_set_profiling(sws_ctx* c, int32_t on) {
+  if (!c) return SWS_EINVAL;
+  c->profiling = on ? 1 : 0;
+  return SWS_OK;
+}
+
+int sws_profile_read(sws_ctx* c, double* allpairs_ms, int32_t* launches, int32_t reset) {
+  if (!c || !allpairs_ms || !launches) return SWS_EINVAL;
+  CK(cudaSetDevice(c->device));
+  double tot = 0.0;
+  for (size_t i = 0; i + 1 < c->prof_used; i += 2) {
+    float ms = 0.f;
+    CK(cudaEventSynchronize((*c->prof_events)[i + 1]));
+    CK(cudaEventElapsedTime(&ms, (*c->prof_events)[i], (*c->prof_events)[i + 1]));
+    tot += ms;
+  }
+  *allpairs_ms = tot;
+  *launches = (int32_t)(c->prof_used / 2);
+  if (reset) c->prof_used = 0;
+  return SWS_OK;
+}
+
+int sws_plan_info(sws_ctx* c, int32_t states, int32_t* out5) {
+  if (!c || !out5 || states < 1 || states > c->max_states) return SWS_EINVAL;
+  const sws::PairPlan p = sws::make_plan(c);
+  out5[0] = p.tiles; out5[1] = p.chunks; out5[2] = p.cols_per_chunk; out5[3] = p.seg_len; out5[4] = p.nseg;
+  return SWS_OK;
+}
+
+int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, double* sm_mhz) {
+  if (!tflops) return SWS_EINVAL;
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (device < 0 || device >= ndev) return SWS_EINVAL;
+  CK(cudaSetDevice(device));
+  cudaDeviceProp prop;
+  CK(cudaGetDeviceProperties(&prop, device));
+  const int sms = prop.multiProcessorCount;
+  const int blocks = sms * 8, threads = 256, iters = 1 << 15;
+  double* sink = nullptr;
+  unsigned long long* clk = nullptr;
+  CK(cudaMalloc((void**)&sink, (size_t)blocks * threads * sizeof(double)));
+  CK(cudaMalloc((void**)&clk, 4 * sizeof(unsigned long long)));
+  cudaEvent_t e0, e1;
+  CK(cudaEventCreate(&e0));
+  CK(cudaEventCreate(&e1));
+  CK(sws::launch_fp64_probe(blocks, iters / 8, sink, clk, 0));  // warm-up
+  double best = 0.0, mhz = 0.0;
+  for (int rep = 0; rep < 3; ++rep) {
+    CK(cudaEventRecord(e0, 0));
+    CK(sws::launch_fp64_probe(blocks, iters, sink, clk, 0));
+    CK(cudaEventRecord(e1, 0));
+    CK(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, e0, e1));
+    unsigned long long h[4];
+    CK(cudaMemcpy(h, clk, sizeof h, cudaMemcpyDeviceToHost));
+    // 16 DFMA per iteration per thread, 2 flops each
+    const double fl = (double)blocks * threads * (double)iters * 16.0 * 2.0;
+    const double tf = fl / (ms * 1e-3) / 1e12;
+    if (tf > best) {
+      best = tf;
+      mhz = (h[3] > h[2]) ? (double)(h[1] - h[0]) / (double)(h[3] - h[2]) * 1e3 : 0.0;
+    }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  cudaFree(clk);
+  *tflops = best;
+  if (sm_count) *sm_count = sms;
+  if (sm_mhz) *sm_mhz = mhz;
+  return SWS_OK;
+}
+
+int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, int32_t n) {
+  if (!x_host || !y_host || n < 1) return SWS_EINVAL;
+  CK(cudaSetDevice(device));
+  double *x = nullptr, *y = nullptr;
+  CK(cudaMalloc((void**)&x, (size_t)n * 8));
+  CK(cudaMalloc((void**)&y, (size_t)n * 8));
+  CK(cudaMemcpy(x, x_host, (size_t)n * 8, cudaMemcpyHostToDevice));
+  CK(sws::launch_debug_rsqrt(x, y, n, 0));
+  CK(cudaMemcpy(y_host, y, (size_t)n * 8, cudaMemcpyDeviceToHost));
+  cudaFree(x);
+  cudaFree(y);
+  return SWS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,353 @@
+// Steps a0-a3, a5-a9 of the residual (everything that is O(NM)): unpack + x-trapezoid
+// reconstruction + radiation rows, y-derivatives, midpoint values with A/B/C, the closed
+// form I, Bernoulli rows, assembly of the integral-equation rows, and the small kernels of
+// the batched finite-difference Jv (shift, quotient).  Citations: PAPER.md lines.
+//
+// These kernels use explicitly rounded __dadd_rn/__dmul_rn where the paper's formula is a
+// short expression, so that no FMA contraction changes the rounding of the nodal fields.
+#include <math_constants.h>
+
+#include "sws_internal.cuh"
+
+namespace sws {
+
+#define ADD(a, b) __dadd_rn((a), (b))
+#define SUB(a, b) __dadd_rn((a), -(b))
+#define MUL(a, b) __dmul_rn((a), (b))
+
+__device__ __forceinline__ double* state_out(double* F0, double* Fpert, int state, int n) {
+  return state == 0 ? F0 : Fpert + (size_t)(state - 1) * n;
+}
+
+// ---------------------------------------------------------------------------------------
+// a0 + a1 + a8.  One CTA per (y-line l, state).  eq. (18): the line block of u is
+// [phi_{1,l}, (phi_x)_{1..N,l}]; the zeta half follows at offset (N+1)M.  eq. (19):
+// zeta_{k+1,l} = zeta_{k,l} + (dx/2)((zeta_x)_{k,l} + (zeta_x)_{k+1,l}), same for phi (L160).
+// The increments are formed by all threads; the running sum itself is sequential (one
+// thread per field) so that its rounding is that of the recurrence as printed.
+// Radiation rows eq. (24) L191-197 / App. A L417 with forward differences (L201, B.1 L431).
+__global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ u,
+                                                     const double* __restrict__ V,
+                                                     const double* __restrict__ sigma, Mesh m,
+                                                     double* zeta, double* phi, double* zx,
+                                                     double* px, double* F0, double* Fpert) {
+  extern __shared__ double sm[];
+  const int N = m.N, l = blockIdx.x, state = blockIdx.y, tid = threadIdx.x;
+  double* s_zx = sm;
+  double* s_px = sm + N;
+  double* s_z = sm + 2 * (size_t)N;
+  double* s_p = sm + 3 * (size_t)N;
+  __shared__ double s_first[2];
+
+  const size_t half = (size_t)(N + 1) * m.M;
+  const size_t offp = (size_t)l * (N + 1), offz = half + offp;
+  const double* v = state > 0 ? V + (size_t)(state - 1) * m.n : nullptr;
+  const double sg = state > 0 ? sigma[state - 1] : 0.0;
+  auto get = [&](size_t idx) -> double {
+    const double a = u[idx];
+    return v ? fma(sg, v[idx], a) : a;  // u_b = fl(u + sigma v), one rounding per entry
+  };
+  for (int k = tid; k < N; k += blockDim.x) {
+    s_px[k] = get(offp + 1 + k);
+    s_zx[k] = get(offz + 1 + k);
+  }
+  if (tid == 0) s_first[0] = get(offp);
+  if (tid == 32) s_first[1] = get(offz);
+  __syncthreads();
+  const double hdx = m.dx / 2;
+  for (int k = tid; k + 1 < N; k += blockDim.x) {
+    s_z[k + 1] = MUL(hdx, ADD(s_zx[k], s_zx[k + 1]));
+    s_p[k + 1] = MUL(hdx, ADD(s_px[k], s_px[k + 1]));
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double acc = s_first[0];
+    s_p[0] = acc;
+    for (int k = 1; k < N; ++k) { acc = ADD(acc, s_p[k]); s_p[k] = acc; }
+  } else if (tid == 32) {
+    double acc = s_first[1];
+    s_z[0] = acc;
+    for (int k = 1; k < N; ++k) { acc = ADD(acc, s_z[k]); s_z[k] = acc; }
+  } else if (tid == 64) {
+    // a8: E3..E6 at x_1 (n = n_rad); positions App. A
+    double* F = state_out(F0, Fpert, state, m.n);
+    const double x1 = m.x1, nr = m.n_rad;
+    const double p1 = s_first[0], z1 = s_first[1];
+    F[offp + 0] = ADD(MUL(x1, SUB(s_px[0], 1.0)), MUL(nr, SUB(p1, x1)));
+    F[offp + 1] = ADD(MUL(x1, SUB(s_px[1], s_px[0]) / m.dx), MUL(nr, SUB(s_px[0], 1.0)));
+    F[offz + 0] = ADD(MUL(x1, s_zx[0]), MUL(nr, z1));
+    F[offz + 1] = ADD(MUL(x1, SUB(s_zx[1], s_zx[0]) / m.dx), MUL(nr, s_zx[0]));
+  }
+  __syncthreads();
+  const size_t base = ((size_t)state * m.M + l) * N;
+  for (int k = tid; k < N; k += blockDim.x) {
+    zeta[base + k] = s_z[k];
+    phi[base + k] = s_p[k];
+    zx[base + k] = s_zx[k];
+    px[base + k] = s_px[k];
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// a2.  y-derivatives along each x-line k (L160).  One thread per (k, field, state); the
+// planes are [l][k] so a warp's accesses are coalesced at every step of the march.
+// dy_scheme 0: cubic spline, unknowns = knot slopes m_l, d_l = (f_{l+1}-f_l)/h:
+//   interior  m_{l-1} + 4 m_l + m_{l+1} = 3 (d_{l-1} + d_l)
+//   first     m_1 = 0 (y_1 = 0, even extension, Q3)  or not-a-knot, reduced with the first
+//             interior row to  m_1 + 2 m_2 = (5 d_1 + d_2)/2
+//   last      not-a-knot, reduced with the last interior row to
+//             2 m_{M-1} + m_M = (d_{M-2} + 5 d_{M-1})/2
+// solved by the Thomas recurrences with the data-independent factors cp[], inv[] made in
+// sws_setup.  The output plane is used as the forward-sweep scratch.
+__global__ void __launch_bounds__(128) k_dy(Mesh m, const double* __restrict__ cp,
+                                            const double* __restrict__ inv, const double* zeta,
+                                            const double* phi, double* zy, double* py) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= m.N) return;
+  const int N = m.N, M = m.M, state = blockIdx.z;
+  const size_t base = (size_t)state * m.S + k;
+  const double* f = (blockIdx.y == 0 ? zeta : phi) + base;
+  double* out = (blockIdx.y == 0 ? zy : py) + base;
+  const double h = m.dy;
+#define F_(l) f[(size_t)(l) * N]
+#define O_(l) out[(size_t)(l) * N]
+  if (m.dy_scheme == 0) {
+    double f0 = F_(0), f1 = F_(1), f2 = F_(2);
+    double dprev = SUB(f1, f0) / h, dcur = SUB(f2, f1) / h;  // d_0, d_1
+    double r = m.sym_first ? 0.0 : ADD(MUL(5.0, dprev), dcur) / 2;
+    double g = MUL(r, inv[0]);
+    O_(0) = g;
+    for (int l = 1; l < M - 1; ++l) {
+      // here dprev = d_{l-1}, dcur = d_l
+      r = MUL(3.0, ADD(dprev, dcur));
+      g = MUL(SUB(r, g), inv[l]);  // a_l = 1
+      O_(l) = g;
+      if (l + 2 < M) {
+        const double fn = F_(l + 2);
+        dprev = dcur;
+        dcur = SUB(fn, f2) / h;
+        f2 = fn;
+      }
+    }
+    // after the loop dprev = d_{M-3}, dcur = d_{M-2}
+    r = ADD(dprev, MUL(5.0, dcur)) / 2;
+    g = MUL(SUB(r, MUL(2.0, g)), inv[M - 1]);  // a_{M-1} = 2
+    O_(M - 1) = g;
+    for (int l = M - 2; l >= 0; --l) {
+      g = SUB(O_(l), MUL(cp[l], g));
+      O_(l) = g;
+    }
+  } else {
+    // finite differences (BASELINE.json wording; reading Q3)
+    const double h2 = 2 * h;
+    O_(0) = m.sym_first ? 0.0 : ADD(ADD(MUL(-3.0, F_(0)), MUL(4.0, F_(1))), -F_(2)) / h2;
+    for (int l = 1; l < M - 1; ++l) O_(l) = SUB(F_(l + 1), F_(l - 1)) / h2;
+    O_(M - 1) = ADD(SUB(MUL(3.0, F_(M - 1)), MUL(4.0, F_(M - 2))), F_(M - 3)) / h2;
+  }
+#undef F_
+#undef O_
+}
+
+// ---------------------------------------------------------------------------------------
+// a5.  Antiderivative G with d2G/ds dt = 1/sqrt(A s^2 + B s t + C t^2) (reading Q5; the paper
+// says only "exactly in terms of logarithms", L187).  D = 4AC - B^2 > 0.  A term whose
+// prefactor is 0 is 0 (the limit of t asinh(c/|t|) as t -> 0).
+__device__ double G_anti(double A, double B, double C, double sqA, double sqC, double sqD, double s,
+                         double t) {
+  double g = 0.0;
+  if (t != 0.0) g += (t / sqA) * asinh((2 * A * s + B * t) / (fabs(t) * sqD));
+  if (s != 0.0) g += (s / sqC) * asinh((2 * C * t + B * s) / (fabs(s) * sqD));
+  return g;
+}
+
+__device__ double box_int(double A, double B, double C, double sqA, double sqC, double sqD,
+                          double s1, double s2, double t1, double t2) {
+  return G_anti(A, B, C, sqA, sqC, sqD, s2, t2) - G_anti(A, B, C, sqA, sqC, sqD, s1, t2) -
+         G_anti(A, B, C, sqA, sqC, sqD, s2, t1) + G_anti(A, B, C, sqA, sqC, sqD, s1, t1);
+}
+
+// a3 + a5 + a6 (local part) + a7 + packing of the transposed source records.
+// One thread per node (k, l) of one state; threads with k < N-1 also own target (k, l).
+__global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restrict__ x,
+                                                 const double* __restrict__ y,
+                                                 const double* __restrict__ zeta,
+                                                 const double* __restrict__ phi,
+                                                 const double* __restrict__ zx,
+                                                 const double* __restrict__ px,
+                                                 const double* __restrict__ zy,
+                                                 const double* __restrict__ py, SrcRec* src,
+                                                 TgtRec* tgt, double* e2loc, double* F0,
+                                                 double* Fpert) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= m.N) return;
+  const int N = m.N, M = m.M, l = blockIdx.y, state = blockIdx.z;
+  const size_t nd = (size_t)state * m.S + (size_t)l * N + k;
+  const double xk = x[k], yl = y[l];
+  const double z0 = zeta[nd], p0 = phi[nd], zx0 = zx[nd], px0 = px[nd], zy0 = zy[nd], py0 = py[nd];
+
+  SrcRec r;
+  r.z = z0; r.psi = SUB(p0, xk); r.zx = zx0; r.zy = zy0;
+  src[(size_t)state * m.S + (size_t)k * M + l] = r;  // transposed [i][j]
+  if (k >= N - 1) return;
+
+  // two-point interpolation to the half-mesh point, L162 / L454
+  const double xs = ADD(xk, x[k + 1]) / 2, ys = yl;
+  const double zs = ADD(z0, zeta[nd + 1]) / 2, ps = ADD(p0, phi[nd + 1]) / 2;
+  const double zxs = ADD(zx0, zx[nd + 1]) / 2, zys = ADD(zy0, zy[nd + 1]) / 2;
+  const double pxs = ADD(px0, px[nd + 1]) / 2, pys = ADD(py0, py[nd + 1]) / 2;
+  const double zx2 = MUL(zxs, zxs), zy2 = MUL(zys, zys);
+  const double A = ADD(1.0, zx2), B = MUL(MUL(2.0, zxs), zys), C = ADD(1.0, zy2);  // L177
+
+  const size_t t = (size_t)l * (N - 1) + k, ts = (size_t)state * m.T + t;
+  TgtRec tr;
+  tr.xs = xs; tr.ys = ys; tr.zs = zs; tr.psis = SUB(ps, xs); tr.zxs = zxs;
+  tr.A = A; tr.B = B; tr.C = C;
+  tgt[ts] = tr;
+
+  double* F = state_out(F0, Fpert, state, m.n);
+  // a7: Bernoulli, eq. (13) L113 at the starred values (Q6)
+  {
+    const double t1 = MUL(MUL(ADD(1.0, zx2), pys), pys);
+    const double t2 = MUL(MUL(ADD(1.0, zy2), pxs), pxs);
+    const double t3 = MUL(MUL(MUL(MUL(2.0, zxs), zys), pxs), pys);
+    const double num = SUB(ADD(t1, t2), t3);
+    const double den = ADD(ADD(1.0, zx2), zy2);
+    const double F2 = MUL(m.froude, m.froude);
+    F[(size_t)l * (N + 1) + 2 + k] = SUB(ADD(num / den / 2, zs / F2), 0.5);
+  }
+  // a5: I = int int S2 over [x_1,x_N] x [y_1,y_M], direct + image term, eq. (23) L185.
+  // Image: t' = -(y + y*) maps A s^2 - B s (y+y*) + C (y+y*)^2 onto the direct form.
+  const double sqA = sqrt(A), sqC = sqrt(C), sqD = sqrt(4 * A * C - B * B);
+  const double s1 = x[0] - xs, s2 = x[N - 1] - xs;
+  const double ya = y[0], yb = y[M - 1];
+  double I;
+  if (ya == 0.0) {
+    // the two boxes share the edge t = -y*: one box over t in [-(y_M + y*), y_M - y*]
+    I = box_int(A, B, C, sqA, sqC, sqD, s1, s2, -(yb + ys), yb - ys);
+  } else {
+    I = box_int(A, B, C, sqA, sqC, sqD, s1, s2, ya - ys, yb - ys) +
+        box_int(A, B, C, sqA, sqC, sqD, s1, s2, -(yb + ys), -(ya + ys));
+  }
+  // a6 local part: 2 pi (phi* - x*) + eps / sqrt(x*^2 + y*^2 + (zeta*+1)^2) - zeta_x* I
+  const double rho2 = xs * xs + ys * ys + (zs + 1.0) * (zs + 1.0);
+  e2loc[ts] = 2.0 * CUDART_PI * (ps - xs) + m.eps / sqrt(rho2) - zxs * I;
+}
+
+// a6 + a9: E2_{k,l} = local - sum over chunks (fixed order) of the all-pairs partials.
+__global__ void __launch_bounds__(256) k_assemble(Mesh m, int chunks, const double* __restrict__ e2loc,
+                                                  const double* __restrict__ part, double* F0,
+                                                  double* Fpert) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= m.T) return;
+  const int state = blockIdx.y;
+  const double* p = part + (size_t)state * chunks * m.T + t;
+  double s = 0.0;
+  for (int c = 0; c < chunks; ++c) s += p[(size_t)c * m.T];
+  const int l = t / (m.N - 1), k = t - l * (m.N - 1);
+  double* F = state_out(F0, Fpert, state, m.n);
+  F[(size_t)(m.N + 1) * m.M + (size_t)l * (m.N + 1) + 2 + k] = e2loc[(size_t)state * m.T + t] - s;
+}
+
+// ---------------------------------------------------------------------------------------
+// a10 helpers.  sigma_b = 1e-7 (1 + ||u||_2) / ||v_b||_2 (BASELINE.json; the paper says only
+// "a suitably-chosen shift", L221).  Two-stage fixed-order reduction: repeatable.
+__global__ void __launch_bounds__(256) k_sumsq(const double* __restrict__ u, const double* __restrict__ V,
+                                               int n, double* part) {
+  const int row = blockIdx.y;  // 0: u, r >= 1: v_{r-1}
+  const double* a = row == 0 ? u : V + (size_t)(row - 1) * n;
+  double s = 0.0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)n;
+       i += (size_t)gridDim.x * blockDim.x)
+    s = fma(a[i], a[i], s);
+  __shared__ double sh[256];
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) part[(size_t)row * gridDim.x + blockIdx.x] = sh[0];
+}
+
+__global__ void k_sigma(const double* __restrict__ part, int nblk, int b, double* sigma) {
+  const int r = threadIdx.x;
+  if (r >= b) return;
+  double su = 0.0, sv = 0.0;
+  for (int i = 0; i < nblk; ++i) su += part[i];
+  for (int i = 0; i < nblk; ++i) sv += part[(size_t)(r + 1) * nblk + i];
+  sigma[r] = 1e-7 * (1.0 + sqrt(su)) / sqrt(sv);
+}
+
+// eq. (25): JV_b = (E(u_b) - E(u)) / sigma_b
+__global__ void __launch_bounds__(256) k_quotient(const double* __restrict__ F0,
+                                                  const double* __restrict__ Fpert,
+                                                  const double* __restrict__ sigma, int n, double* JV) {
+  const int b = blockIdx.y;
+  const double sg = sigma[b];
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)n;
+       i += (size_t)gridDim.x * blockDim.x)
+    JV[(size_t)b * n + i] = (Fpert[(size_t)b * n + i] - F0[i]) / sg;
+}
+
+// ---------------------------------------------------------------------------------------
+// host launchers
+
+size_t reconstruct_smem_bytes(int N) { return (size_t)4 * N * sizeof(double); }
+
+cudaError_t fields_configure(const sws_ctx* c) {
+  return cudaFuncSetAttribute(k_reconstruct, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)reconstruct_smem_bytes(c->mesh.N));
+}
+
+cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states, double* F0,
+                               double* Fpert, cudaStream_t st) {
+  const Mesh& m = c->mesh;
+  dim3 grid(m.M, states);
+  k_reconstruct<<<grid, 256, reconstruct_smem_bytes(m.N), st>>>(u, V, c->sigma, m, c->zeta, c->phi,
+                                                                 c->zx, c->px, F0, Fpert);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st) {
+  const Mesh& m = c->mesh;
+  dim3 grid((m.N + 127) / 128, 2, states);
+  k_dy<<<grid, 128, 0, st>>>(m, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zy, c->py);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, cudaStream_t st) {
+  const Mesh& m = c->mesh;
+  dim3 grid((m.N + 127) / 128, m.M, states);
+  k_targets<<<grid, 128, 0, st>>>(m, c->x, c->y, c->zeta, c->phi, c->zx, c->px, c->zy, c->py, c->src,
+                                  c->tgt, c->e2loc, F0, Fpert);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_assemble(sws_ctx* c, int states, const PairPlan& plan, double* F0, double* Fpert,
+                            cudaStream_t st) {
+  const Mesh& m = c->mesh;
+  dim3 grid((m.T + 255) / 256, states);
+  k_assemble<<<grid, 256, 0, st>>>(m, plan.chunks, c->e2loc, c->part, F0, Fpert);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_sigma(sws_ctx* c, const double* u, const double* V, int b, cudaStream_t st) {
+  dim3 grid(kNormBlocks, b + 1);
+  k_sumsq<<<grid, 256, 0, st>>>(u, V, c->mesh.n, c->norm_part);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_sigma<<<1, ((b + 31) / 32) * 32, 0, st>>>(c->norm_part, kNormBlocks, b, c->sigma);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_jv_quotient(sws_ctx* c, const double* F0, const double* Fpert, int b, double* JV,
+                               cudaStream_t st) {
+  const int n = c->mesh.n;
+  int bx = (n + 255) / 256;
+  if (bx > 1024) bx = 1024;
+  dim3 grid(bx, b);
+  k_quotient<<<grid, 256, 0, st>>>(F0, Fpert, c->sigma, n, JV);
+  return cudaGetLastError();
+}
+
+}  // namespace sws

@@ -1,0 +1,121 @@
+// Internal declarations of libsws (CUDA path, sm_100a).  Shares nothing with oracle/.
+// Citations "L<n>" are lines of /root/reference/PAPER.md; "Qn" are DESIGN.md readings.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "sws.h"
+
+namespace sws {
+
+// One source node (x_i, y_j) of one state as the all-pairs kernel consumes it: 32 B.
+// Stored TRANSPOSED, [i][j] with j fastest, so that one x-column is one contiguous
+// M * 32 B run that a single bulk async copy (TMA, UBLKCP) moves into shared memory.
+//   z = zeta_ij, psi = phi_ij - x_i, zx = (zeta_x)_ij, zy = (zeta_y)_ij
+struct __align__(32) SrcRec {
+  double z, psi, zx, zy;
+};
+
+// One target midpoint (x_{k+1/2}, y_l) of one state (starred values, L162 / L177): 64 B.
+struct __align__(32) TgtRec {
+  double xs, ys;    // x*, y*
+  double zs, psis;  // zeta*, phi* - x*
+  double zxs;       // zeta_x*
+  double A, B, C;   // 1 + zeta_x*^2, 2 zeta_x* zeta_y*, 1 + zeta_y*^2   (L177)
+};
+
+struct Mesh {
+  int N, M;     // nodes
+  int T, S, n;  // (N-1)M targets, NM sources, 2(N+1)M unknowns
+  double x1, y1, dx, dy;
+  double froude, eps, n_rad;
+  int dy_scheme;  // 0 spline, 1 FD
+  int sym_first;  // y1 == 0: even extension across the centre line (Q3)
+};
+
+// All-pairs launch geometry (host-computed, see make_plan()).
+struct PairPlan {
+  int tiles;      // ceil(T / kPairThreads) target tiles
+  int chunks;     // groups of source columns; one CTA = (tile, chunk, state)
+  int seg_len;    // nodes of one column staged per bulk copy (<= kSegMax)
+  int nseg;       // segments per column = ceil(M / seg_len)
+  int cols_per_chunk;  // ceil(N / chunks)
+};
+
+constexpr int kPairThreads = 128;  // threads (= targets) per CTA of the all-pairs kernel
+constexpr int kSegMax = 256;       // max nodes staged per bulk copy (10 KB per stage)
+constexpr int kStages = 2;         // staging ring depth
+constexpr int kNormBlocks = 64;    // partial blocks of the 2-norm reductions
+
+}  // namespace sws
+
+struct sws_ctx {
+  sws::Mesh mesh;
+  sws_params params;
+  int device;
+  int sm_count;
+  int max_states;       // max_batch + 1
+  int chunks_user;      // 0 = auto
+  size_t ws_bytes;
+  int last_launches;
+  int last_states;      // states the workspace fields currently describe
+
+  // geometry (device)
+  double* x;  // [N]
+  double* y;  // [M]
+  // spline tables (device): Thomas forward-elimination factors, data independent
+  double* sp_cp;   // [M] c'_l
+  double* sp_inv;  // [M] 1 / (b_l - a_l c'_{l-1})
+
+  // per-state node planes, [state][l][k] (k fastest)
+  double* zeta;
+  double* phi;
+  double* zx;
+  double* px;
+  double* zy;
+  double* py;
+  sws::SrcRec* src;  // [state][i][j]  (transposed)
+  sws::TgtRec* tgt;  // [state][t], t = l (N-1) + k
+  double* e2loc;     // [state][t]   2 pi (phi*-x*) + eps/rho* - zeta_x* I
+  double* part;      // [state][chunk][t] partial all-pairs sums (already times dx dy)
+  int part_chunks;   // chunk capacity of `part` per state
+
+  double* F0;         // [n] base residual of a batch when the caller passes no F0_dev
+  double* Fpert;      // [max_batch][n] when the caller passes no Fpert_dev
+  double* sigma;      // [max_batch] device
+  double* norm_part;  // [max_batch + 1][kNormBlocks]
+  // host-call staging (device)
+  double* u_stage;    // [n]
+  double* V_stage;    // [max_batch][n]
+  double* out_stage;  // [2 max_batch + 1][n]
+  cudaEvent_t ev0, ev1;
+  int profiling;                       // sws_set_profiling
+  std::vector<cudaEvent_t>* prof_events;  // pairs (before, after) of all-pairs launches
+  size_t prof_used;                    // events in use (the vector only grows)
+};
+
+namespace sws {
+
+// Launches (all asynchronous on `st`); each returns the cudaError_t of its launch.
+// states = 1: base state only.  State s >= 1 is u + sigma[s-1] * V[s-1].
+cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states,
+                               double* F0, double* Fpert, cudaStream_t st);
+cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st);
+cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, cudaStream_t st);
+cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
+cudaError_t launch_assemble(sws_ctx* c, int states, const PairPlan& plan, double* F0,
+                            double* Fpert, cudaStream_t st);
+cudaError_t launch_sigma(sws_ctx* c, const double* u, const double* V, int b, cudaStream_t st);
+cudaError_t launch_jv_quotient(sws_ctx* c, const double* F0, const double* Fpert, int b,
+                               double* JV, cudaStream_t st);
+
+PairPlan make_plan(const sws_ctx* c);
+int max_chunks(const sws_ctx* c);
+size_t allpairs_smem_bytes(const PairPlan& p);
+cudaError_t allpairs_configure();
+cudaError_t fields_configure(const sws_ctx* c);
+size_t reconstruct_smem_bytes(int N);
+
+}  // namespace sws

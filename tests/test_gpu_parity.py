@@ -1,0 +1,234 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by
+element on the same seeded inputs.  Bar (BASELINE.json north_star): FP64 residual within
+1e-10 relative to |F|_inf; ordering/indexing exact.  All tests here need a B200."""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10  # BASELINE.json: "within 1e-10 relative to ||F||_inf"
+
+
+@pytest.fixture(scope="module")
+def sws():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test run without a CUDA device")
+    import paper_1403_5044_b200 as m
+    m.load_library()  # fails loudly if libsws.so is missing
+    return m
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def relerr(F, E, mask=None):
+    if mask is not None:
+        F, E = F[mask], E[mask]
+    return float(np.abs(F - E).max() / np.abs(E).max())
+
+
+def gpu_residual(sws, cfg, u, dy_scheme=0, chunks=0):
+    with sws.Context(cfg.params(dy_scheme)) as ctx:
+        if chunks:
+            ctx.set_tuning(chunks)
+        return ctx.residual(dev(u)).cpu().numpy()
+
+
+# ---------------------------------------------------------------------------------------
+def test_rsqrt_primitive(sws):
+    """The kernel's reciprocal square root (MUFU.RSQ64H seed + cubic correction) against
+    1/sqrt in long double: <= 1 ulp over the magnitudes R^2 and the S2 quadratic forms take."""
+    rng = np.random.default_rng(0)
+    x = np.concatenate([
+        10.0 ** rng.uniform(-8, 8, 200000),
+        rng.uniform(1.0, 4.0, 200000),                      # one full binade pair of the seed table
+        np.nextafter(2.0 ** np.arange(-20, 20, dtype=np.float64), 0),  # just below powers of two
+        2.0 ** np.arange(-20, 20, dtype=np.float64),
+    ])
+    y = sws.debug_rsqrt(x)
+    ref = 1.0 / np.sqrt(x.astype(np.longdouble))
+    rel = np.abs((y.astype(np.longdouble) - ref) / ref).astype(np.float64)
+    assert rel.max() <= 2.0 ** -52, rel.max()
+
+
+@pytest.mark.parametrize("i", [0, 1, 2])
+def test_residual_full_parity(sws, oracle80, i):
+    """cfg 1-3: every entry of F against the long-double oracle."""
+    cfg = W.CONFIGS[i]
+    u = W.state(cfg)
+    E = oracle80.residual(cfg.params(), u)
+    F = gpu_residual(sws, cfg, u)
+    assert F.shape == E.shape and np.isfinite(F).all()
+    assert relerr(F, E) <= TOL
+    # the O(NM) rows alone (Bernoulli, radiation): formed with the oracle's roundings
+    half = (cfg.N + 1) * cfg.M
+    assert np.abs(F[:half] - E[:half]).max() <= 1e-13 * max(1.0, np.abs(E[:half]).max())
+
+
+@pytest.mark.parametrize("i", [0, 1])
+def test_residual_vs_f64_oracle(sws, oracle64, i):
+    """Same against the plain double oracle (the timed baseline): both are FP64 programs that
+    differ only in summation order."""
+    cfg = W.CONFIGS[i]
+    u = W.state(cfg)
+    E = oracle64.residual(cfg.params(), u)
+    assert relerr(gpu_residual(sws, cfg, u), E) <= TOL
+
+
+RAGGED = [
+    dict(N=3, M=4, h=0.5, x1=-1.0),                 # minimum sizes
+    dict(N=37, M=9, h=0.45, x1=-5.0, seed=7),       # one ragged tile
+    dict(N=131, M=7, h=0.2, x1=-6.0, seed=8),       # 130*7 = 910 targets: 7 tiles + ragged tail
+    dict(N=5, M=601, h=0.05, x1=-0.3, seed=9),      # column longer than one staged segment (odd M)
+    dict(N=6, M=514, h=0.05, x1=-0.3, seed=10),     # two segments, second one short
+    dict(N=44, M=12, h=0.4, x1=-3.0, y1=0.8, seed=11),  # y1 != 0: not-a-knot at both ends, two boxes in I
+]
+
+
+@pytest.mark.parametrize("kw", RAGGED, ids=lambda k: f"{k['N']}x{k['M']}")
+@pytest.mark.parametrize("dy_scheme", [0, 1])
+def test_residual_ragged_shapes(sws, oracle80, kw, dy_scheme):
+    cfg = W.custom(eps=0.3, amp=0.05, **kw)
+    u = W.state(cfg) + 1e-3 * np.random.default_rng(3).standard_normal(cfg.n)
+    E = oracle80.residual(cfg.params(dy_scheme), u)
+    F = gpu_residual(sws, cfg, u, dy_scheme)
+    assert relerr(F, E) <= TOL
+
+
+def test_uniform_stream_is_a_zero(sws):
+    """eps = 0, u = u_0 (L227): F == 0 to round-off (pin P6, on the GPU path)."""
+    import dataclasses
+    cfg = dataclasses.replace(W.CONFIGS[1], eps=0.0)
+    F = gpu_residual(sws, cfg, W.flat_state(cfg))
+    assert np.abs(F).max() <= 1e-12
+
+
+def test_chunking_invariance_and_determinism(sws, oracle80):
+    """The split of the quadrature into column groups only reorders the sum; repeated calls are
+    bitwise identical (no atomics)."""
+    import torch
+    cfg = W.CONFIGS[2]
+    u = W.state(cfg)
+    with sws.Context(cfg.params()) as ctx:
+        ud = dev(u)
+        F_auto = ctx.residual(ud).cpu().numpy()
+        F_again = ctx.residual(ud).cpu().numpy()
+        assert np.array_equal(F_auto, F_again)
+        info = ctx.plan_info(1)
+        assert info["tiles"] == -(-cfg.targets // 128)
+        for ch in (1, 2, 5):
+            ctx.set_tuning(ch)
+            Fc = ctx.residual(ud).cpu().numpy()
+            assert relerr(Fc, F_auto) <= 1e-13
+        torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("i,rows", [(3, 192), (4, 96)])
+def test_large_configs_sampled_rows(sws, oracle80, i, rows):
+    """cfg 4 and cfg 5 at full size in the launch configuration bench.py times: the O(NM) rows
+    in full, and a seeded sample of integral-equation rows the oracle computes one by one."""
+    cfg = W.CONFIGS[i]
+    u = W.state(cfg)
+    rng = np.random.default_rng(1234 + i)
+    T = cfg.targets
+    pick = np.unique(np.concatenate([
+        rng.integers(0, T, rows),
+        [0, cfg.N - 2, T - 1, T - (cfg.N - 1), (cfg.M // 2) * (cfg.N - 1) + cfg.N // 2],  # corners, centre
+    ])).astype(np.int32)
+    E = oracle80.residual(cfg.params(), u, rows=pick)
+    F = gpu_residual(sws, cfg, u)
+    mask = ~np.isnan(E)
+    assert mask.sum() == (cfg.N + 1) * cfg.M + 2 * cfg.M + pick.size
+    assert np.isfinite(F).all()
+    scale = np.abs(F).max()
+    assert np.abs(F[mask] - E[mask]).max() / scale <= TOL
+
+
+# ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("i", [1, 2])
+def test_jv_batch_parity(sws, oracle80, i):
+    """eq. (25) L219 in batch: F(u + sigma_b v_b) of every direction against the oracle at the
+    SAME shift (reading Q9 (i)); the shift itself against its formula; F0 of the batch
+    against sws_residual; JV against the long-double oracle (reported, loose bound)."""
+    import torch
+    cfg = W.CONFIGS[i]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg)
+    b = V.shape[0]
+    E0 = oracle80.residual(p, u)
+    scale = np.abs(E0).max()
+    with sws.Context(p, max_batch=b) as ctx:
+        ud, Vd = dev(u), dev(V)
+        JV, Fp, F0 = ctx.jv_batch(ud, Vd, want_fpert=True, want_f0=True)
+        torch.cuda.synchronize()
+        sig = ctx.last_sigma(b)
+        F = ctx.residual(ud).cpu().numpy()
+        JV, Fp, F0 = JV.cpu().numpy(), Fp.cpu().numpy(), F0.cpu().numpy()
+        # explicit shifts give the same batch
+        JV2 = ctx.jv_batch(ud, Vd, sigma=sig).cpu().numpy()
+    assert np.array_equal(F0, F)
+    assert np.array_equal(JV2, JV)
+    worst_jv = 0.0
+    for k in range(b):
+        s_ref = oracle80.sigma(u, V[k])
+        assert abs(sig[k] - s_ref) <= 1e-13 * s_ref
+        JV_ref, Ep = oracle80.jv(p, u, V[k], float(sig[k]))
+        assert np.abs(Fp[k] - Ep).max() / scale <= TOL
+        # the quotient is formed from the two GPU residuals exactly as eq. (25) says
+        assert np.array_equal(JV[k], (Fp[k] - F0) / sig[k])
+        worst_jv = max(worst_jv, float(np.abs(JV[k] - JV_ref).max() / np.abs(JV_ref).max()))
+    # raw FD quotient: rounding floor eps_mach / sigma_rel (reading Q9 (ii)); reported bound
+    assert worst_jv <= 1e-5, worst_jv
+
+
+def test_host_api_matches_device_api(sws):
+    cfg = W.CONFIGS[1]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg, 3)
+    with sws.Context(p, max_batch=4) as ctx:
+        Fd = ctx.residual(dev(u)).cpu().numpy()
+        Fh = ctx.residual_host(u)
+        assert np.array_equal(Fd, Fh)
+        JVd, Fpd, F0d = ctx.jv_batch(dev(u), dev(V), want_fpert=True, want_f0=True)
+        JVh, Fph, F0h = ctx.jv_batch_host(u, V)
+        assert np.array_equal(JVd.cpu().numpy(), JVh)
+        assert np.array_equal(Fpd.cpu().numpy(), Fph)
+        assert np.array_equal(F0d.cpu().numpy(), F0h)
+        assert ctx.last_launch_count == 8   # 2 (shift) + 5 (a0-a9) + 1 (quotient)
+
+
+def test_layout_unit_perturbations(sws, oracle64):
+    """eq. (18) L149 / App. A L421 positions: perturbing one unknown moves exactly the rows the
+    oracle says it moves (radiation rows of its own line; Bernoulli rows of neighbouring lines
+    through the spline; every integral-equation row)."""
+    cfg = W.custom(13, 5, 0.4, -2.2, seed=21, eps=0.2)
+    p, u = cfg.params(), W.state(cfg)
+    half = (cfg.N + 1) * cfg.M
+    with sws.Context(p) as ctx:
+        F0 = ctx.residual(dev(u)).cpu().numpy()
+        E0 = oracle64.residual(p, u)
+        for idx in (0, 1, 2, cfg.N, cfg.N + 1, half, half + 1, half + 3 * (cfg.N + 1) + 5, cfg.n - 1):
+            up = u.copy()
+            up[idx] += 1e-3
+            dF = ctx.residual(dev(up)).cpu().numpy() - F0
+            dE = oracle64.residual(p, up) - E0
+            assert np.array_equal(np.abs(dF) > 1e-9, np.abs(dE) > 1e-9), idx
+            assert np.abs(dF - dE).max() <= 1e-11
+
+
+def test_error_codes(sws):
+    cfg = W.CONFIGS[0]
+    p = cfg.params()
+    with pytest.raises(sws.SwsError, match="invalid"):
+        sws.Context(dict(p, N=2))
+    with pytest.raises(sws.SwsError, match="invalid"):
+        sws.Context(dict(p, dx=0.0))
+    with sws.Context(p, max_batch=2) as ctx:
+        u, V = dev(W.state(cfg)), dev(W.directions(cfg, 3))
+        with pytest.raises(sws.SwsError, match="batch"):
+            ctx.jv_batch(u, V)
+        with pytest.raises(sws.SwsError):
+            ctx.residual(u[:-1])
