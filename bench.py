@@ -35,12 +35,12 @@ if str(ROOT) not in sys.path:
 
 import workloads as W  # noqa: E402
 
-METRIC = "fp64_residual_evals_per_s_721x241"
+METRIC = "fp64_residual_evals_per_s"
 UNIT = "evals/s"
 # Algorithmic work of the all-pairs kernel per pair interaction, from its SASS inner loop
-# (DESIGN.md "Kernels"): 45 FP64-pipe instructions = 25 DFMA (2 flops) + 20 DMUL/DADD (1 flop).
+# (DESIGN.md "Kernels"): 45 FP64-pipe instructions = 23 DFMA (2 flops) + 22 DMUL/DADD (1 flop).
 FP64_INSTR_PER_PAIR = 45
-FLOPS_PER_PAIR = 70
+FLOPS_PER_PAIR = 68
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
 
 
@@ -151,7 +151,7 @@ def run_reference(args) -> None:
     sample = (f"{rows} seeded integral-equation rows of {cfg.targets} per step (+ all O(NM) rows), "
               f"{rows * cfg.sources:.3e} pair interactions per step, scaled by rows/T")
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "metric": f"{METRIC}_{cfg.N}x{cfg.M}", "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": {"workload": cfg.name, "N": cfg.N, "M": cfg.M, "sample": sample},
@@ -296,7 +296,7 @@ def run_ours(args) -> None:
                         "pairs_per_s": v * cfg.pairs}
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": f"{METRIC}_{cfg.N}x{cfg.M}", "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "N": cfg.N, "M": cfg.M, "h": cfg.h, "eps": cfg.eps,

@@ -11,14 +11,24 @@
 // (cp.async.bulk -> UBLKCP, completion on an mbarrier), double buffered.  Every lane of a
 // warp reads the same record (shared-memory broadcast), so the kernel is bound by the FP64
 // pipe: 45 FP64 instructions + 4 MUFU.RSQ64H per pair.  Everything that depends only on
-// (target, column) - dx, dx^2, A dx^2, B dx - is hoisted out of the j loop; the half
+// (target, column) - dx, dx^2 and the completed-square constants of S2 - is hoisted out of the j loop; the half
 // weights are applied by peeling the first/last node and scaling edge columns, so the
 // inner loop carries no weight multiply.  Partial sums per (state, chunk, target) are
 // written to global memory and added in a fixed order by the assemble kernel: no atomics,
 // bitwise repeatable.
 #include "sws_internal.cuh"
 
+// build-time tuning of the all-pairs kernel (defaults measured on B200)
+#ifndef SWS_MINB
+#define SWS_MINB 4  // resident CTAs per SM asked of __launch_bounds__ (caps registers at 128)
+#endif
+#ifndef SWS_UNROLL
+#define SWS_UNROLL 8  // source nodes per inner-loop iteration
+#endif
+
 namespace sws {
+
+constexpr int kUnroll = SWS_UNROLL;
 
 // 1/sqrt(x) for normal positive x, full double precision.
 // Seed: MUFU.RSQ64H (PTX rsqrt.approx.ftz.f64: works on the upper 32 bits of x, so the seed
@@ -26,6 +36,12 @@ namespace sws {
 // exact result is y0 (1 - e)^(-1/2) = y0 (1 + e/2 + 3e^2/8 + 5e^3/16 + ...); the two-term
 // correction below leaves 5/16 |e|^3 < 2^-59, i.e. below the rounding of the final FMA.
 // 5 FP64 instructions (DMUL, DFMA, DFMA, DMUL, DFMA) + 1 MUFU.
+//
+// Operand shapes matter on B200: a DFMA with three DISTINCT register sources issues every
+// 3 cycles per SM sub-partition, one with <= 2 distinct registers (a repeated operand, an
+// immediate) every 2 (measured).  Every step
+// here is written with at most two distinct registers: the last one is
+// y0 + y0 * (e p) = fma(y0, e p, y0), not fma(y0 e, p, y0).
 __device__ __forceinline__ double rsqrt_seed(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
@@ -37,20 +53,26 @@ __device__ __forceinline__ double rsqrt_fp64(double x) {
   const double t = x * y0;
   const double e = fma(-t, y0, 1.0);
   const double p = fma(0.375, e, 0.5);
-  const double ye = y0 * e;
-  return fma(ye, p, y0);
+  const double w = e * p;
+  return fma(y0, w, y0);
 }
 
 // Per-thread constants of one target and of the current source column.
+// The S2 quadratic forms are used with the square completed (C > 0):
+//   A dx^2 + B dx (y-y*) + C (y-y*)^2 = C [ (y - c)^2 + g ],
+//   A dx^2 - B dx (y+y*) + C (y+y*)^2 = C [ (y + c)^2 + g ],
+//   c = y* - (B / 2C) dx,   g = (A/C - (B/2C)^2) dx^2 = (4AC - B^2) dx^2 / (4 C^2) > 0,
+// so that each form costs one add and one two-register FMA per pair, c and g are per
+// (target, column), and the common factor 1/sqrt(C) is applied once per target at the end.
 struct TgtC {
-  double ys, zs, psis, C;
+  double ys, zs, psis;
 };
 struct ColC {
-  double dx, dx2, Adx2, Bdx;  // x_i - x*, its square, A dx^2, B dx
+  double dx, dx2, c, g;  // x_i - x*, its square, and the S2 constants above
 };
 
 // One source node against one target: adds (phi-phi*-x+x*) K1 + zeta_x K2 to a1 and
-// S2 to aS (unit weight).
+// sqrt(C) S2 to aS (unit weight).
 __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, const double yj,
                                           const TgtC& t, const ColC& c, double& a1, double& aS) {
   const double z = zp.x, psi = zp.y, zx = sl.x, zy = sl.y;
@@ -72,9 +94,11 @@ __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, co
   const double dpsi = psi - t.psis;
   a1 = fma(dpsi, k1, a1);
   a1 = fma(zx, rm + rp, a1);  // K2 = 1/R- + 1/R+
-  // S2: A dx^2 + B dx (y-y*) + C (y-y*)^2  and  A dx^2 - B dx (y+y*) + C (y+y*)^2
-  const double Qm = fma(fma(t.C, dm, c.Bdx), dm, c.Adx2);
-  const double Qp = fma(fma(t.C, dp, -c.Bdx), dp, c.Adx2);
+  // S2 (eqs. (21), (22)) up to the factor 1/sqrt(C)
+  const double sm = yj - c.c;
+  const double sp = yj + c.c;
+  const double Qm = fma(sm, sm, c.g);
+  const double Qp = fma(sp, sp, c.g);
   aS += rsqrt_fp64(Qm) + rsqrt_fp64(Qp);
 }
 
@@ -140,8 +164,10 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
   const int tc = t < a.T ? t : a.T - 1;  // ragged tail: recompute the last target, never stored
 
   const TgtRec tr = a.tgt[(size_t)state * a.T + tc];
-  const TgtC tg = {tr.ys, tr.zs, tr.psis, tr.C};
-  const double xs = tr.xs, tA = tr.A, tB = tr.B;
+  const TgtC tg = {tr.ys, tr.zs, tr.psis};
+  const double xs = tr.xs;
+  const double kb = tr.B / (2.0 * tr.C);          // B / 2C
+  const double kg = tr.A / tr.C - kb * kb;        // (4AC - B^2) / (4 C^2)
 
   const int c0 = chunk * a.cols_per_chunk;
   const int c1 = min(a.N, c0 + a.cols_per_chunk);
@@ -178,8 +204,8 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
     ColC cc;
     cc.dx = __ldg(a.x + i) - xs;
     cc.dx2 = cc.dx * cc.dx;
-    cc.Adx2 = tA * cc.dx2;
-    cc.Bdx = tB * cc.dx;
+    cc.c = fma(-kb, cc.dx, tg.ys);
+    cc.g = kg * cc.dx2;
     const double ci = (i == 0 || i == a.N - 1) ? 0.5 : 1.0;  // trapezoid weight in x (Q4)
 
     mbar_wait(&s_bar[s], (uint32_t)((q / kStages) & 1));
@@ -197,7 +223,7 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
     }
     const bool last = (j0 + len == a.M);
     if (last) jhi = len - 1;
-#pragma unroll 2
+#pragma unroll kUnroll
     for (int j = jlo; j < jhi; ++j) pair_term(rec[2 * j], rec[2 * j + 1], yy[j], tg, cc, col1, colS);
     if (last && jhi >= jlo) {  // last node of the column: weight 1/2 in y
       double h1 = 0.0, hS = 0.0;
@@ -211,14 +237,15 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
   }
 
   if (t < a.T)
-    a.part[((size_t)state * a.chunks + chunk) * a.T + t] = a.dxdy * fma(-tr.zxs, totS, tot1);
+    a.part[((size_t)state * a.chunks + chunk) * a.T + t] =
+        a.dxdy * fma(-tr.zxs * rsqrt_fp64(tr.C), totS, tot1);
 }
 
 // ---------------------------------------------------------------------------------------
 // host side
 
 static int g_occ = 0;  // resident CTAs per SM of the instantiation in use
-constexpr int kMinB = 6;
+constexpr int kMinB = SWS_MINB;
 
 size_t allpairs_smem_bytes(const PairPlan& p) {
   return (size_t)kStages * p.seg_len * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
