@@ -42,6 +42,9 @@ UNIT = "evals/s"
 FP64_INSTR_PER_PAIR = 45
 FLOPS_PER_PAIR = 68
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
+# dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
+# ncu --set full capture summarised in profiles/r1_allpairs_ncu.md (algorithmic: 16.67 MB)
+NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 16.813e6}
 
 
 def dist_env():
@@ -275,7 +278,10 @@ def run_ours(args) -> None:
     pipe_frac = FP64_INSTR_PER_PAIR * pairs_timed / (sm_count * FP64_LANES_PER_SM * sm_mhz * 1e6 * ap_s)
     roofline = {
         "bound": "alu", "kernel": "k_allpairs", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-        "frac": achieved_tf / peak_tf, "traffic": None,
+        "frac": achieved_tf / peak_tf, "traffic": NCU_DRAM_BYTES_PER_STATE_LAUNCH.get(cfg.name),
+        "traffic_note": "DRAM bytes per state per all-pairs launch, ncu capture profiles/r1_allpairs_ncu.md; "
+                        "algorithmic = S*32 + T*64 bytes read once",
+        "algorithmic_bytes_per_state": cfg.sources * 32 + cfg.targets * 64,
         "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz "
                        "(FP64 is not in MEASURED_PEAKS.json; DESIGN.md 'Peak')",
         "flops_per_pair": FLOPS_PER_PAIR, "fp64_instr_per_pair": FP64_INSTR_PER_PAIR,
