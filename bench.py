@@ -166,6 +166,46 @@ def run_reference(args) -> None:
     print(json.dumps(line), flush=True)
 
 
+def fp32_variant_report(sws, device: int, names=("cfg4_361x121",), steps: int = 3) -> dict:
+    """BASELINE.json config 4: "an FP32-accumulate variant, reported separately with its measured
+    error".  sws_params.precision = 1 (FP32 pair arithmetic, Q12) timed on the same step
+    (sws_residual + sws_jv_batch) with CUDA events; the error is the max-norm distance of its F(u)
+    from the FP64 CUDA path on the same input (which the gpu tests hold to 1e-10 of the oracle;
+    tests/test_gpu_parity.py measures the variant against the oracle itself)."""
+    import torch
+    out = {}
+    for name in names:
+        cfg = W.BY_NAME[name]
+        b = cfg.b if cfg.b > 0 else 1
+        u = torch.from_numpy(W.state(cfg)).cuda(device)
+        V = torch.from_numpy(W.directions(cfg, b)).cuda(device)
+        with sws.Context(cfg.params(), device=device) as c64:
+            F64 = c64.residual(u).clone()
+        with sws.Context(cfg.params(), max_batch=b, device=device, precision=1) as c32:
+            F32 = c32.residual(u)
+            c32.jv_batch(u, V)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(steps):
+                c32.residual(u, out=F32)
+                c32.jv_batch(u, V)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            ap_ms = c32.time_allpairs(b + 1, 2)
+            err = float((F32 - F64).abs().max() / F64.abs().max())
+        evals = 1 + (b + 1)
+        out[name] = {"evals_per_s": evals / (ms * 1e-3), "pairs_per_s": evals * cfg.pairs / (ms * 1e-3),
+                     "ms_per_step": ms, "jv_batch": b, "evals_per_step": evals,
+                     "allpairs_pairs_per_s": (b + 1) * cfg.pairs / (ap_ms * 1e-3),
+                     "max_rel_err_vs_fp64_path": err}
+    out["note"] = ("precision=1: FP32 pair arithmetic (packed f32x2, MUFU.RSQ), FP32 accumulation per source "
+                   "column, FP64 across columns and everywhere outside the all-pairs kernel; bound by the XU "
+                   "pipe (4 MUFU.RSQ per pair); reported, not part of `value`")
+    return out
+
+
 def run_ours(args) -> None:
     import torch
 
@@ -301,6 +341,10 @@ def run_ours(args) -> None:
                                   f"{dt:.1f} s, scaled by rows/T",
                         "pairs_per_s": v * cfg.pairs}
 
+    fp32 = None
+    if world == 1 and not args.no_fp32:
+        fp32 = fp32_variant_report(sws, local, names=tuple(dict.fromkeys(["cfg4_361x121", cfg.name])))
+
     line = {
         "metric": f"{METRIC}_{cfg.N}x{cfg.M}", "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
@@ -318,6 +362,7 @@ def run_ours(args) -> None:
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
         "workspace_bytes": ctx.workspace_bytes,
+        "fp32_variant": fp32,
     }
     print(json.dumps(line), flush=True)
     ctx.close()
@@ -334,6 +379,7 @@ def main() -> None:
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline leg")
     ap.add_argument("--ref-rows", type=int, default=2048, help="rows per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fp32", action="store_true", help="skip the reported FP32-variant section")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)

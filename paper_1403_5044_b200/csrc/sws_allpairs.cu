@@ -17,6 +17,7 @@
 // written to global memory and added in a fixed order by the assemble kernel: no atomics,
 // bitwise repeatable.
 #include "sws_internal.cuh"
+#include "sws_stage.cuh"
 
 // build-time tuning of the all-pairs kernel (defaults measured on B200)
 #ifndef SWS_MINB
@@ -100,43 +101,6 @@ __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, co
   const double Qm = fma(sm, sm, c.g);
   const double Qp = fma(sp, sp, c.g);
   aS += rsqrt_fp64(Qm) + rsqrt_fp64(Qp);
-}
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
-               "r"(bytes)
-               : "memory");
-}
-
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"(smem_u32(bar)),
-      "r"(parity)
-      : "memory");
-}
-
-// global -> shared bulk async copy (TMA engine, 1-D), bytes % 16 == 0, both 16 B aligned.
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-          smem_u32(dst)),
-      "l"(src), "r"(bytes), "r"(smem_u32(bar))
-      : "memory");
 }
 
 struct PairArgs {
@@ -244,14 +208,13 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
 // ---------------------------------------------------------------------------------------
 // host side
 
-static int g_occ = 0;  // resident CTAs per SM of the instantiation in use
 constexpr int kMinB = SWS_MINB;
 
 size_t allpairs_smem_bytes(const PairPlan& p) {
   return (size_t)kStages * p.seg_len * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
 }
 
-cudaError_t allpairs_configure() {
+cudaError_t allpairs_configure(int* occ_out) {
   cudaError_t e = cudaFuncSetAttribute(k_allpairs<kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)(kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + 64));
   if (e != cudaSuccess) return e;
@@ -260,7 +223,7 @@ cudaError_t allpairs_configure() {
       &occ, k_allpairs<kMinB>, kPairThreads,
       kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t));
   if (e != cudaSuccess) return e;
-  g_occ = occ > 0 ? occ : 1;
+  *occ_out = occ > 0 ? occ : 1;
   return cudaSuccess;
 }
 
@@ -278,7 +241,7 @@ PairPlan make_plan(const sws_ctx* c) {
   int seg = (m.M + p.nseg - 1) / p.nseg;
   p.seg_len = (seg + 1) & ~1;
   p.nseg = (m.M + p.seg_len - 1) / p.seg_len;
-  const long slots = (long)c->sm_count * (g_occ > 0 ? g_occ : 4);
+  const long slots = (long)c->sm_count * (c->pair_occ > 0 ? c->pair_occ : 4);
   int best = 1;
   // a CTA should see at least ~256 source nodes
   int min_cols = (256 + m.M - 1) / m.M;
@@ -313,6 +276,7 @@ int max_chunks(const sws_ctx* c) {
 }
 
 cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st) {
+  if (c->params.precision == 1) return launch_allpairs_f32(c, states, plan, st);
   const Mesh& m = c->mesh;
   PairArgs a;
   a.src = c->src; a.x = c->x; a.y = c->y; a.tgt = c->tgt; a.part = c->part;

@@ -41,7 +41,7 @@ static cudaError_t dev_alloc(T** p, size_t count, size_t* total) {
 
 static void free_all(sws_ctx* c) {
   void* ptrs[] = {c->x, c->y, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zx, c->px, c->zy, c->py,
-                  c->src, c->tgt, c->e2loc, c->part, c->F0, c->Fpert, c->sigma, c->norm_part,
+                  c->src, c->srcf, c->tgt, c->e2loc, c->part, c->F0, c->Fpert, c->sigma, c->norm_part,
                   c->u_stage, c->V_stage, c->out_stage};
   for (void* p : ptrs)
     if (p) cudaFree(p);
@@ -73,7 +73,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   *out = nullptr;
   if (p->N < 3 || p->M < 4 || !(p->dx > 0) || !(p->dy > 0) || !(p->froude > 0)) return SWS_EINVAL;
   if (p->dy_scheme != 0 && p->dy_scheme != 1) return SWS_EINVAL;
-  if (p->precision != 0) return SWS_EINVAL;  // FP32 pair arithmetic: not built yet
+  if (p->precision != 0 && p->precision != 1) return SWS_EINVAL;
   if (p->max_batch < 0 || p->max_batch > 1024) return SWS_EINVAL;
   if ((long long)p->N * p->M > (1ll << 30)) return SWS_EINVAL;
   if (sws::reconstruct_smem_bytes(p->N) > 200 * 1024) return SWS_EINVAL;  // N <= 6400
@@ -102,7 +102,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaGetDeviceProperties"); }
   c->sm_count = prop.multiProcessorCount;
 
-  e = sws::allpairs_configure();
+  e = p->precision == 1 ? sws::allpairs_f32_configure(&c->pair_occ) : sws::allpairs_configure(&c->pair_occ);
   if (e == cudaSuccess) e = sws::fields_configure(c);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "kernel configuration (is this an sm_100 device?)"); }
 
@@ -126,6 +126,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   ALLOC(zeta, st * S); ALLOC(phi, st * S); ALLOC(zx, st * S);
   ALLOC(px, st * S); ALLOC(zy, st * S); ALLOC(py, st * S);
   ALLOC(src, st * S);
+  if (p->precision == 1) ALLOC(srcf, st * S);
   ALLOC(tgt, st * T);
   ALLOC(e2loc, st * T);
   ALLOC(part, part_elems);

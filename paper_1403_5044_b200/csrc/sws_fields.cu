@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restric
                                                  const double* __restrict__ px,
                                                  const double* __restrict__ zy,
                                                  const double* __restrict__ py, SrcRec* src,
-                                                 TgtRec* tgt, double* e2loc, double* F0,
+                                                 SrcRecF* srcf, TgtRec* tgt, double* e2loc, double* F0,
                                                  double* Fpert) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= m.N) return;
@@ -188,6 +188,14 @@ __global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restric
   SrcRec r;
   r.z = z0; r.psi = SUB(p0, xk); r.zx = zx0; r.zy = zy0;
   src[(size_t)state * m.S + (size_t)k * M + l] = r;  // transposed [i][j]
+  if (srcf) {  // FP32 variant (Q12): zeta as hi + lo, packed-instruction operands duplicated
+    SrcRecF f;
+    f.z_hi = (float)r.z; f.z_lo = (float)(r.z - (double)f.z_hi);
+    f.psi = f.psi_dup = (float)r.psi;
+    f.zx = f.zx_dup = (float)r.zx;
+    f.nzy = f.nzy_dup = -(float)r.zy;
+    srcf[(size_t)state * m.S + (size_t)k * M + l] = f;
+  }
   if (k >= N - 1) return;
 
   // two-point interpolation to the half-mesh point, L162 / L454
@@ -319,7 +327,7 @@ cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, cu
   const Mesh& m = c->mesh;
   dim3 grid((m.N + 127) / 128, m.M, states);
   k_targets<<<grid, 128, 0, st>>>(m, c->x, c->y, c->zeta, c->phi, c->zx, c->px, c->zy, c->py, c->src,
-                                  c->tgt, c->e2loc, F0, Fpert);
+                                  c->srcf, c->tgt, c->e2loc, F0, Fpert);
   return cudaGetLastError();
 }
 

@@ -18,6 +18,14 @@ struct __align__(32) SrcRec {
   double z, psi, zx, zy;
 };
 
+// The same node for the FP32 pair-arithmetic variant (sws_allpairs_f32.cu), 32 B, same
+// transposed layout.  zeta is a two-float number (z_hi + z_lo); fields the packed f32x2
+// instructions consume as (v, v) pairs are stored twice, zeta_y negated.
+struct __align__(16) SrcRecF {
+  float z_hi, z_lo, psi, psi_dup;
+  float zx, zx_dup, nzy, nzy_dup;
+};
+
 // One target midpoint (x_{k+1/2}, y_l) of one state (starred values, L162 / L177): 64 B.
 struct __align__(32) TgtRec {
   double xs, ys;    // x*, y*
@@ -77,6 +85,8 @@ struct sws_ctx {
   double* zy;
   double* py;
   sws::SrcRec* src;  // [state][i][j]  (transposed)
+  sws::SrcRecF* srcf;  // the same in FP32 (precision = 1 only, else NULL)
+  int pair_occ;        // resident CTAs per SM of the all-pairs kernel in use
   sws::TgtRec* tgt;  // [state][t], t = l (N-1) + k
   double* e2loc;     // [state][t]   2 pi (phi*-x*) + eps/rho* - zeta_x* I
   double* part;      // [state][chunk][t] partial all-pairs sums (already times dx dy)
@@ -104,7 +114,9 @@ cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int
                                double* F0, double* Fpert, cudaStream_t st);
 cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st);
 cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, cudaStream_t st);
+// dispatches on sws_params.precision (0: FP64 kernel, 1: FP32 pair arithmetic)
 cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
+cudaError_t launch_allpairs_f32(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
 cudaError_t launch_assemble(sws_ctx* c, int states, const PairPlan& plan, double* F0,
                             double* Fpert, cudaStream_t st);
 cudaError_t launch_sigma(sws_ctx* c, const double* u, const double* V, int b, cudaStream_t st);
@@ -114,7 +126,9 @@ cudaError_t launch_jv_quotient(sws_ctx* c, const double* F0, const double* Fpert
 PairPlan make_plan(const sws_ctx* c);
 int max_chunks(const sws_ctx* c);
 size_t allpairs_smem_bytes(const PairPlan& p);
-cudaError_t allpairs_configure();
+cudaError_t allpairs_configure(int* occ_out);
+cudaError_t allpairs_f32_configure(int* occ_out);
+size_t allpairs_f32_smem_bytes(int seg_len);
 cudaError_t fields_configure(const sws_ctx* c);
 size_t reconstruct_smem_bytes(int N);
 

@@ -232,3 +232,63 @@ def test_error_codes(sws):
             ctx.jv_batch(u, V)
         with pytest.raises(sws.SwsError):
             ctx.residual(u[:-1])
+
+
+# ---------------------------------------------------------------------------------------
+# FP32 pair-arithmetic variant (sws_params.precision = 1, BASELINE.json config 4, reading Q12):
+# reported, not gated by the 1e-10 bar.  The bounds below are sanity bounds (FP32 round-off of
+# O(10^2) sums that cancel to O(1)): a wrong term, sign or index is O(1), not 1e-4.
+F32_SANITY = 5e-4
+
+
+@pytest.mark.parametrize("i", [0, 1, 2])
+def test_fp32_variant_error_vs_oracle(sws, oracle80, i, record_property):
+    cfg = W.CONFIGS[i]
+    u = W.state(cfg)
+    E = oracle80.residual(cfg.params(), u)
+    with sws.Context(cfg.params(), precision=1) as c32, sws.Context(cfg.params()) as c64:
+        F32 = c32.residual(dev(u)).cpu().numpy()
+        F64 = c64.residual(dev(u)).cpu().numpy()
+    half = (cfg.N + 1) * cfg.M
+    # everything outside a4 is the FP64 path unchanged: Bernoulli and radiation rows bitwise
+    assert np.array_equal(F32[:half], F64[:half])
+    rad = np.arange(cfg.M) * (cfg.N + 1) + half
+    assert np.array_equal(F32[rad], F64[rad]) and np.array_equal(F32[rad + 1], F64[rad + 1])
+    err = relerr(F32, E)
+    record_property("fp32_rel_err_inf", err)
+    print(f"\nFP32 variant {cfg.name}: |F32 - E|_inf / |E|_inf = {err:.3e}")
+    assert 1e-9 < err <= F32_SANITY  # really FP32 (not the FP64 kernel), and not wrong
+
+
+@pytest.mark.parametrize("kw", [RAGGED[2], RAGGED[3], RAGGED[5]], ids=lambda k: f"{k['N']}x{k['M']}")
+def test_fp32_variant_ragged(sws, oracle80, kw):
+    """ragged tail, several staged segments per column, y1 != 0 (image offset 2 y1)."""
+    cfg = W.custom(eps=0.3, amp=0.05, **kw)
+    u = W.state(cfg) + 1e-3 * np.random.default_rng(3).standard_normal(cfg.n)
+    E = oracle80.residual(cfg.params(), u)
+    with sws.Context(cfg.params(), precision=1) as ctx:
+        F = ctx.residual(dev(u)).cpu().numpy()
+    assert relerr(F, E) <= F32_SANITY
+
+
+def test_fp32_variant_cfg4_sampled_and_batch(sws, oracle80):
+    """cfg 4 (361x121, the configuration BASELINE.json names for the variant): error on a seeded
+    sample of integral-equation rows against the FP64 oracle; the Jv batch runs and its base
+    evaluation is bitwise the single evaluation."""
+    import torch
+    cfg = W.CONFIGS[3]
+    u = W.state(cfg)
+    rng = np.random.default_rng(77)
+    pick = np.unique(rng.integers(0, cfg.targets, 256)).astype(np.int32)
+    E = oracle80.residual(cfg.params(), u, rows=pick)
+    mask = ~np.isnan(E)
+    V = W.directions(cfg, 2)
+    with sws.Context(cfg.params(), precision=1, max_batch=2) as ctx:
+        F = ctx.residual(dev(u)).cpu().numpy()
+        JV, Fp, F0 = ctx.jv_batch(dev(u), dev(V), want_fpert=True, want_f0=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(F0.cpu().numpy(), F)
+        assert np.isfinite(JV.cpu().numpy()).all()
+    err = float(np.abs(F[mask] - E[mask]).max() / np.abs(F).max())
+    print(f"\nFP32 variant cfg4 sampled rows: {err:.3e}")
+    assert 1e-9 < err <= F32_SANITY
