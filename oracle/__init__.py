@@ -6,7 +6,9 @@ nothing from the CUDA package and shares no code with it.
 
 `Oracle(precision="f64")` is the plain double program (the timed CPU baseline);
 `Oracle(precision="f80")` is the same source compiled with REAL = long double
-(x86 80-bit), the accuracy reference.
+(x86 80-bit), the accuracy reference.  `Oracle(precision="c80")` is the same source
+compiled with REAL = long double _Complex: `jv_exact` evaluates the residual at
+u + i h v and returns Im/h, the exact Jacobian action J(u) v (complex-step derivative).
 """
 from __future__ import annotations
 
@@ -19,8 +21,11 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "sws_oracle.c"
-_LIBS = {"f64": _HERE / "libsws_oracle_f64.so", "f80": _HERE / "libsws_oracle_f80.so"}
-_REAL = {"f64": "double", "f80": "long double"}
+_LIBS = {"f64": _HERE / "libsws_oracle_f64.so", "f80": _HERE / "libsws_oracle_f80.so",
+         "c80": _HERE / "libsws_oracle_c80.so"}
+# c80: the same source with REAL = long double _Complex (complex-step derivative, -DCSTEP);
+# -fcx-limited-range = textbook complex multiply/divide (no NaN-recovery library calls)
+_DEFS = {"f64": ["-DREAL=double"], "f80": ["-DREAL=long double"], "c80": ["-DCSTEP", "-fcx-limited-range"]}
 
 
 def build(force: bool = False) -> None:
@@ -29,7 +34,7 @@ def build(force: bool = False) -> None:
         if not force and lib.exists() and lib.stat().st_mtime >= _SRC.stat().st_mtime:
             continue
         cmd = ["gcc", "-std=c11", "-O2", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared",
-               f"-DREAL={_REAL[suf]}", f"-DSUF={suf}", str(_SRC), "-o", str(lib), "-lm"]
+               *_DEFS[suf], f"-DSUF={suf}", str(_SRC), "-o", str(lib), "-lm"]
         subprocess.run(cmd, check=True)
 
 
@@ -68,7 +73,8 @@ class Oracle:
             ("weight", C.c_double, [C.POINTER(_Params), C.c_int, C.c_int]),
             ("dy_line", C.c_int, [C.c_int, C.c_double, C.c_int, C.c_int, _dp, _dp]),
             ("sizeof_real", C.c_int, []),
-        ]:
+        ] + ([("jv_exact", C.c_int, [C.POINTER(_Params), _dp, _dp, _ip, C.c_int, _dp, _dp])]
+             if precision == "c80" else []):
             fn = getattr(self.lib, f"sws_oracle_{name}_{s}")
             fn.restype, fn.argtypes = res, args
             f[name] = fn
@@ -123,6 +129,20 @@ class Oracle:
         if rc:
             raise RuntimeError(f"sws_oracle_jv rc={rc}")
         return JV, Ep
+
+    def jv_exact(self, p: dict, u, v, rows=None, want_e0: bool = False):
+        """J(u) v by complex-step differentiation of the residual (c80 build only)."""
+        if self.suf != "c80":
+            raise ValueError("jv_exact needs Oracle('c80')")
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        assert u.size == self._n(p) and v.size == u.size
+        JV, E0 = np.empty_like(u), np.empty_like(u)
+        rp, nr, _keep = self._rows(rows)
+        rc = self._f["jv_exact"](C.byref(self._params(p)), _d(u), _d(v), rp, nr, _d(JV), _d(E0))
+        if rc:
+            raise RuntimeError(f"sws_oracle_jv_exact rc={rc}")
+        return (JV, E0) if want_e0 else JV
 
     # -- pieces for the pins -------------------------------------------------
     def fields(self, p: dict, u):

@@ -15,8 +15,16 @@
  * reordering.  The only parallelism is an OpenMP `for` over the independent
  * integral-equation rows E2_{k,l}.
  *
- * Compiled twice: -DREAL=double -DSUF=f64 (the timed baseline) and
- * -DREAL="long double" -DSUF=f80 (x86 80-bit accuracy reference).
+ * Compiled three times: -DREAL=double -DSUF=f64 (the timed baseline),
+ * -DREAL="long double" -DSUF=f80 (x86 80-bit accuracy reference), and
+ * -DCSTEP -DSUF=c80 (REAL = long double _Complex): the SAME residual code run
+ * on u + i h v, whose imaginary part / h is the exact directional derivative
+ * J(u) v = d/d sigma E(u + sigma v) at sigma = 0 (complex-step differentiation:
+ * no subtraction, truncation error O(h^2) with h = 1e-40).  That is the oracle
+ * of the analytic Jacobian action (the limit of eq. (25) L219 as sigma -> 0);
+ * it contains no hand-derived derivative formula.  Every function of u the
+ * residual uses is analytic (sqrt and asinh of arguments with positive real
+ * part, rational expressions); |.| is applied to mesh geometry only.
  *
  * Readings of the paper where it is silent/garbled are DESIGN.md "Readings"
  * Q1..Q12; each is flagged at the line that uses it.
@@ -24,7 +32,10 @@
  * Pins (tests/test_oracle_pins.py): P1 full-plane identity, P2 Gauss flux,
  * P3 spline == scipy CubicSpline, P4 sum of weights, P5 closed-form I vs
  * adaptive quadrature, P6 uniform stream, P7 tilted plane, P8 O(h^2)
- * convergence, P9 linear-Jacobian closed forms B.5/B.6 and B.2, layout tests.
+ * convergence, P9 linear-Jacobian closed forms B.5/B.6 and B.2, layout tests;
+ * for the complex-step Jacobian action: PJ1 the same closed forms B.5/B.6/B.2
+ * to round-off, PJ2 Richardson-extrapolated central differences of the f80
+ * residual at a nonlinear state, PJ3 the linear radiation rows applied to v.
  * Beyond those the residual's absolute values are "parity unpinned" (the
  * paper prints no numeric value of E for any worked example).
  */
@@ -33,8 +44,18 @@
 #include <string.h>
 #include <tgmath.h>
 
+#ifdef CSTEP
+#include <complex.h>
+#undef REAL
+#define REAL long double _Complex
+#define RREAL long double             /* quantities that never depend on u */
+#define RE(z) creall(z)
+#else
 #ifndef REAL
 #define REAL double
+#endif
+#define RREAL REAL
+#define RE(z) (z)
 #endif
 #ifndef SUF
 #define SUF f64
@@ -67,24 +88,24 @@ static const REAL PI_R = (REAL)3.14159265358979323846264338327950288L;
 /* ---------------------------------------------------------------------- */
 /* Dense LU with partial pivoting; the spline's linear system is solved by */
 /* the plainest possible method.                                           */
-static int lu_factor(int n, REAL *A, int *piv) {
+static int lu_factor(int n, RREAL *A, int *piv) {
   for (int c = 0; c < n; ++c) {
     int p = c;
-    REAL best = fabs(A[(size_t)c * n + c]);
+    RREAL best = fabs(A[(size_t)c * n + c]);
     for (int r = c + 1; r < n; ++r) {
-      REAL v = fabs(A[(size_t)r * n + c]);
+      RREAL v = fabs(A[(size_t)r * n + c]);
       if (v > best) { best = v; p = r; }
     }
     if (best == 0) return -1;
     piv[c] = p;
     if (p != c)
       for (int j = 0; j < n; ++j) {
-        REAL t = A[(size_t)c * n + j];
+        RREAL t = A[(size_t)c * n + j];
         A[(size_t)c * n + j] = A[(size_t)p * n + j];
         A[(size_t)p * n + j] = t;
       }
     for (int r = c + 1; r < n; ++r) {
-      REAL f = A[(size_t)r * n + c] / A[(size_t)c * n + c];
+      RREAL f = A[(size_t)r * n + c] / A[(size_t)c * n + c];
       A[(size_t)r * n + c] = f;
       for (int j = c + 1; j < n; ++j) A[(size_t)r * n + j] -= f * A[(size_t)c * n + j];
     }
@@ -92,7 +113,7 @@ static int lu_factor(int n, REAL *A, int *piv) {
   return 0;
 }
 
-static void lu_solve(int n, const REAL *A, const int *piv, REAL *b) {
+static void lu_solve(int n, const RREAL *A, const int *piv, REAL *b) {
   for (int c = 0; c < n; ++c) {
     int p = piv[c];
     if (p != c) { REAL t = b[c]; b[c] = b[p]; b[p] = t; }
@@ -116,14 +137,14 @@ static void lu_solve(int n, const REAL *A, const int *piv, REAL *b) {
 /*   not-a-knot (S''' continuous) at y_2:     m_1 - m_3 = 2(d_1 - d_2)       */
 /*   not-a-knot at y_{M-1}:          m_{M-2} - m_M = 2(d_{M-2} - d_{M-1})    */
 /* The matrix does not depend on f: it is factorised once per call.          */
-typedef struct { int M; int clamped_first; REAL *LU; int *piv; } spline_t;
+typedef struct { int M; int clamped_first; RREAL *LU; int *piv; } spline_t;
 
 static int spline_setup(spline_t *s, int M, int clamped_first) {
   s->M = M; s->clamped_first = clamped_first;
-  s->LU = (REAL *)calloc((size_t)M * M, sizeof(REAL));
+  s->LU = (RREAL *)calloc((size_t)M * M, sizeof(RREAL));
   s->piv = (int *)calloc((size_t)M, sizeof(int));
   if (!s->LU || !s->piv) return -1;
-  REAL *A = s->LU;
+  RREAL *A = s->LU;
   if (clamped_first) {
     A[0] = 1;                                   /* m_1 = 0 */
   } else {
@@ -169,8 +190,18 @@ static void fields_free(fields_t *f) {
   memset(f, 0, sizeof *f);
 }
 
-/* Steps 1-3 of the residual: unpack u, x-trapezoid, y-derivatives. */
-static int fields_build(const sws_oracle_params *p, const double *u, fields_t *f) {
+/* Entry idx of the state: u[idx], or u[idx] + i h v[idx] in the complex-step build. */
+#ifdef CSTEP
+#define UVAL(arr_u, arr_v, idx) ((REAL)(arr_u)[idx] + _Complex_I * (cs_h * (RREAL)(arr_v)[idx]))
+#else
+#define UVAL(arr_u, arr_v, idx) ((REAL)(arr_u)[idx])
+#endif
+
+/* Steps 1-3 of the residual: unpack u, x-trapezoid, y-derivatives.  (v, cs_h): the
+ * complex-step direction and step; used by the CSTEP build only. */
+static int fields_build(const sws_oracle_params *p, const double *u, const double *v, RREAL cs_h,
+                        fields_t *f) {
+  (void)v; (void)cs_h;
   int N = p->N, M = p->M;
   size_t S = (size_t)N * M;
   memset(f, 0, sizeof *f);
@@ -189,17 +220,17 @@ static int fields_build(const sws_oracle_params *p, const double *u, fields_t *f
   for (int l = 0; l < M; ++l) f->y[l] = (REAL)(p->y1 + (double)l * p->dy);
 
   /* eq. (18): u = [phi_{1,l}, (phi_x)_{1..N,l}]_{l=1..M}, then the same for zeta. */
-  const double *u_phi = u, *u_zeta = u + (size_t)(N + 1) * M;
+  const size_t off_zeta = (size_t)(N + 1) * M;
   for (int l = 0; l < M; ++l) {
-    const double *lp = u_phi + (size_t)l * (N + 1), *lz = u_zeta + (size_t)l * (N + 1);
+    const size_t lp = (size_t)l * (N + 1), lz = off_zeta + (size_t)l * (N + 1);
     for (int k = 0; k < N; ++k) {
-      f->phi_x[AT(k, l)] = (REAL)lp[1 + k];
-      f->zeta_x[AT(k, l)] = (REAL)lz[1 + k];
+      f->phi_x[AT(k, l)] = UVAL(u, v, lp + 1 + k);
+      f->zeta_x[AT(k, l)] = UVAL(u, v, lz + 1 + k);
     }
     /* eq. (19): zeta_{k+1,l} = zeta_{k,l} + (dx/2)((zeta_x)_{k,l} + (zeta_x)_{k+1,l}); */
     /* L160: "Values of phi ... similarly computed using phi_x".                             */
-    f->phi[AT(0, l)] = (REAL)lp[0];
-    f->zeta[AT(0, l)] = (REAL)lz[0];
+    f->phi[AT(0, l)] = UVAL(u, v, lp);
+    f->zeta[AT(0, l)] = UVAL(u, v, lz);
     for (int k = 0; k + 1 < N; ++k) {
       f->zeta[AT(k + 1, l)] = f->zeta[AT(k, l)] + (dx / 2) * (f->zeta_x[AT(k, l)] + f->zeta_x[AT(k + 1, l)]);
       f->phi[AT(k + 1, l)] = f->phi[AT(k, l)] + (dx / 2) * (f->phi_x[AT(k, l)] + f->phi_x[AT(k + 1, l)]);
@@ -349,11 +380,12 @@ static REAL E1_row(const sws_oracle_params *p, const fields_t *f, int k, int l) 
  *   first half, per l:  [E3_l, E4_l, E1_{1..N-1,l}];  second half: [E5_l, E6_l, E2_{1..N-1,l}].
  * rows (optional): flat target indices t = l*(N-1) + k whose E2 is wanted;
  * every other E2 entry is NaN.  rows == NULL: all.  Output widened REAL. */
-static int residual_real(const sws_oracle_params *p, const double *u, const int *rows, int nrows, REAL *E) {
+static int residual_cs(const sws_oracle_params *p, const double *u, const double *v, RREAL cs_h,
+                       const int *rows, int nrows, REAL *E) {
   int N = p->N, M = p->M;
   if (N < 3 || M < 4 || !(p->dx > 0) || !(p->dy > 0)) return -1;
   fields_t f;
-  int rc = fields_build(p, u, &f);
+  int rc = fields_build(p, u, v, cs_h, &f);
   if (rc) return rc;
   size_t half = (size_t)(N + 1) * M;
   REAL x1 = f.x[0], n = (REAL)p->n_rad, dx = (REAL)p->dx;
@@ -382,6 +414,10 @@ static int residual_real(const sws_oracle_params *p, const double *u, const int 
   return 0;
 }
 
+static int residual_real(const sws_oracle_params *p, const double *u, const int *rows, int nrows, REAL *E) {
+  return residual_cs(p, u, u, 0, rows, nrows, E);   /* zero step: the plain residual */
+}
+
 /* ============================ exported C-ABI ============================ */
 
 int FN(sws_oracle_residual)(const sws_oracle_params *p, const double *u, const int *rows, int nrows, double *E) {
@@ -389,7 +425,7 @@ int FN(sws_oracle_residual)(const sws_oracle_params *p, const double *u, const i
   REAL *Er = (REAL *)malloc(n * sizeof(REAL));
   if (!Er) return -2;
   int rc = residual_real(p, u, rows, nrows, Er);
-  if (!rc) for (size_t i = 0; i < n; ++i) E[i] = (double)Er[i];
+  if (!rc) for (size_t i = 0; i < n; ++i) E[i] = (double)RE(Er[i]);
   free(Er);
   return rc;
 }
@@ -410,8 +446,8 @@ int FN(sws_oracle_jv)(const sws_oracle_params *p, const double *u, const double 
     rc = residual_real(p, u, rows, nrows, E0);
     if (!rc) rc = residual_real(p, ub, rows, nrows, E1);
     if (!rc) for (size_t i = 0; i < n; ++i) {
-      JV[i] = (double)((E1[i] - E0[i]) / (REAL)sigma);
-      if (Epert) Epert[i] = (double)E1[i];
+      JV[i] = (double)RE((E1[i] - E0[i]) / (REAL)sigma);
+      if (Epert) Epert[i] = (double)RE(E1[i]);
     }
   }
   free(ub); free(E0); free(E1);
@@ -423,7 +459,7 @@ int FN(sws_oracle_jv)(const sws_oracle_params *p, const double *u, const double 
 double FN(sws_oracle_sigma)(int n, const double *u, const double *v) {
   REAL su = 0, sv = 0;
   for (int i = 0; i < n; ++i) { su += (REAL)u[i] * (REAL)u[i]; sv += (REAL)v[i] * (REAL)v[i]; }
-  return (double)((REAL)1e-7 * (1 + sqrt(su)) / sqrt(sv));
+  return (double)RE((REAL)1e-7 * (1 + sqrt(su)) / sqrt(sv));
 }
 
 /* --- pieces exposed so that the pins can reach every term separately --- */
@@ -432,12 +468,12 @@ double FN(sws_oracle_sigma)(int n, const double *u, const double *v) {
 int FN(sws_oracle_fields)(const sws_oracle_params *p, const double *u, double *zeta, double *phi,
                           double *zeta_y, double *phi_y) {
   fields_t f;
-  int rc = fields_build(p, u, &f);
+  int rc = fields_build(p, u, u, 0, &f);
   if (rc) return rc;
   size_t S = (size_t)p->N * p->M;
   for (size_t i = 0; i < S; ++i) {
-    zeta[i] = (double)f.zeta[i]; phi[i] = (double)f.phi[i];
-    zeta_y[i] = (double)f.zeta_y[i]; phi_y[i] = (double)f.phi_y[i];
+    zeta[i] = (double)RE(f.zeta[i]); phi[i] = (double)RE(f.phi[i]);
+    zeta_y[i] = (double)RE(f.zeta_y[i]); phi_y[i] = (double)RE(f.phi_y[i]);
   }
   fields_free(&f);
   return 0;
@@ -447,12 +483,12 @@ int FN(sws_oracle_fields)(const sws_oracle_params *p, const double *u, double *z
 int FN(sws_oracle_e2_terms)(const sws_oracle_params *p, const double *u, int k, int l, double *out) {
   if (k < 0 || k >= p->N - 1 || l < 0 || l >= p->M) return -1;
   fields_t f;
-  int rc = fields_build(p, u, &f);
+  int rc = fields_build(p, u, u, 0, &f);
   if (rc) return rc;
   REAL o[6], zxs;
   E2_terms(p, &f, k, l, o, &zxs);
-  for (int i = 0; i < 6; ++i) out[i] = (double)o[i];
-  out[6] = (double)zxs;
+  for (int i = 0; i < 6; ++i) out[i] = (double)RE(o[i]);
+  out[6] = (double)RE(zxs);
   fields_free(&f);
   return 0;
 }
@@ -462,19 +498,19 @@ void FN(sws_oracle_pair_kernels)(double x, double y, double zeta, double zeta_x,
                                  double *out3) {
   REAL K1, K2, S2;
   pair_kernels(x, y, zeta, zeta_x, zeta_y, xs, ys, zetas, A, B, C, &K1, &K2, &S2);
-  out3[0] = (double)K1; out3[1] = (double)K2; out3[2] = (double)S2;
+  out3[0] = (double)RE(K1); out3[1] = (double)RE(K2); out3[2] = (double)RE(S2);
 }
 
 double FN(sws_oracle_s2_integral)(double A, double B, double C, double xs, double ys,
                                   double xa, double xb, double ya, double yb) {
-  return (double)S2_integral(A, B, C, xs, ys, xa, xb, ya, yb);
+  return (double)RE(S2_integral(A, B, C, xs, ys, xa, xb, ya, yb));
 }
 
 double FN(sws_oracle_box_integral)(double A, double B, double C, double s1, double s2, double t1, double t2) {
-  return (double)box_integral(A, B, C, s1, s2, t1, t2);
+  return (double)RE(box_integral(A, B, C, s1, s2, t1, t2));
 }
 
-double FN(sws_oracle_weight)(const sws_oracle_params *p, int i, int j) { return (double)weight(p, i, j); }
+double FN(sws_oracle_weight)(const sws_oracle_params *p, int i, int j) { return (double)RE(weight(p, i, j)); }
 
 /* y-derivative of one line of M samples (spacing h), same routine the residual uses. */
 int FN(sws_oracle_dy_line)(int M, double h, int scheme, int first_is_symmetric, const double *f, double *m) {
@@ -490,9 +526,33 @@ int FN(sws_oracle_dy_line)(int M, double h, int scheme, int first_is_symmetric, 
   } else {
     fd_slopes(M, first_is_symmetric, (REAL)h, fr, 1, mr);
   }
-  for (int l = 0; l < M; ++l) m[l] = (double)mr[l];
+  for (int l = 0; l < M; ++l) m[l] = (double)RE(mr[l]);
   free(fr); free(mr); free(rhs);
   return rc;
 }
 
 int FN(sws_oracle_sizeof_real)(void) { return (int)sizeof(REAL); }
+
+
+#ifdef CSTEP
+/* Exact Jacobian action J(u) v = d/d sigma E(u + sigma v)|_{sigma=0} (the limit of eq. (25)
+ * L219), by complex-step differentiation of the residual above:
+ *   JV = Im E(u + i h v) / h,   h = 1e-40  (no cancellation; truncation O(h^2)).
+ * rows as in sws_oracle_residual (E2 rows not asked for are NaN).  E0 (optional) receives
+ * Re E(u + i h v) = E(u) + O(h^2). */
+int FN(sws_oracle_jv_exact)(const sws_oracle_params *p, const double *u, const double *v,
+                            const int *rows, int nrows, double *JV, double *E0) {
+  size_t n = (size_t)2 * (p->N + 1) * p->M;
+  const RREAL h = 1e-40L;
+  REAL *Ec = (REAL *)malloc(n * sizeof(REAL));
+  if (!Ec) return -2;
+  int rc = residual_cs(p, u, v, h, rows, nrows, Ec);
+  if (!rc) for (size_t i = 0; i < n; ++i) {
+    RREAL re = creall(Ec[i]);
+    JV[i] = (re != re) ? (double)NAN : (double)(cimagl(Ec[i]) / h);
+    if (E0) E0[i] = (double)re;
+  }
+  free(Ec);
+  return rc;
+}
+#endif

@@ -23,3 +23,10 @@ def oracle64():
 def oracle80():
     import oracle
     return oracle.Oracle("f80")
+
+
+@pytest.fixture(scope="session")
+def oracleC():
+    """REAL = long double _Complex build: exact Jacobian action by complex-step differentiation."""
+    import oracle
+    return oracle.Oracle("c80")

@@ -573,3 +573,118 @@ def test_row_subset_equals_full(oracle64):
         assert Es[i] == E[i]
     assert np.array_equal(Es[:half], E[:half])
     assert np.isnan(Es[half:]).sum() == c.targets - len(rows)
+
+
+# ----------------------------------------------------------------------------
+# The exact Jacobian action J(u) v (oracle c80: complex-step derivative of the SAME residual
+# code, Im E(u + i h v) / h).  PJ1: closed forms of App. B; PJ2: Richardson-extrapolated
+# central differences of the long-double residual at a nonlinear state; PJ3: linear rows.
+# ----------------------------------------------------------------------------
+def test_PJ1_exact_jacobian_reproduces_appendix_B(oracleC, oracle64):
+    """Columns of J at u_0, eps = 0, to round-off (the FD pin P9 above can only reach 1e-7)."""
+    c = dataclasses.replace(small(N=13, M=5, h=0.4, x1=-2.2), eps=0.0)
+    p = c.params()
+    u0 = W.flat_state(c)
+    co = _coeffs()
+    x, y = W.mesh(c)
+    TOLJ = 2e-13
+
+    def col(idx):
+        e = np.zeros(c.n); e[idx] = 1.0
+        return oracleC.jv_exact(p, u0, e)
+
+    m = 2
+    J = col(idx_phi1(c, m))
+    for l in range(c.M):
+        for k in range(c.N - 1):
+            assert J[row_E2(c, k, l)] == pytest.approx(2 * PI if l == m else 0.0, abs=TOLJ)
+            assert J[row_E1(c, k, l)] == pytest.approx(0.0, abs=TOLJ)
+    J = col(idx_zeta1(c, m))
+    for l in range(c.M):
+        for k in range(c.N - 1):
+            assert J[row_E1(c, k, l)] == pytest.approx(1 / c.froude ** 2 if l == m else 0.0, abs=TOLJ)
+            assert J[row_E2(c, k, l)] == pytest.approx(0.0, abs=TOLJ)
+    for n0 in (0, 1, 5, c.N - 1):
+        J = col(idx_phix(c, n0, m))
+        for l in range(c.M):
+            for k in range(c.N - 1):
+                case = _case(n0 + 1, k + 1) if l == m else None
+                ref2 = co[("E2_phix", case)] * PI * c.h if case else 0.0
+                ref1 = 0.5 if (l == m and n0 in (k, k + 1)) else 0.0
+                assert J[row_E2(c, k, l)] == pytest.approx(ref2, abs=TOLJ)
+                assert J[row_E1(c, k, l)] == pytest.approx(ref1, abs=TOLJ)
+
+    def K3(i, j, k, l):
+        xs = 0.5 * (x[k] + x[k + 1])
+        return 1 / np.hypot(x[i] - xs, y[j] - y[l]) + 1 / np.hypot(x[i] - xs, y[j] + y[l])
+    for n0 in (0, 4, c.N - 1):
+        J = col(idx_zetax(c, n0, m))
+        for l in range(c.M):
+            for k in range(c.N - 1):
+                ref = -oracle64.weight(p, n0, m) * K3(n0, m, k, l)
+                if l == m and n0 in (k, k + 1):
+                    xs = 0.5 * (x[k] + x[k + 1])
+                    sumwK3 = sum(oracle64.weight(p, i, j) * K3(i, j, k, l) for i in range(c.N) for j in range(c.M))
+                    I = oracle64.box_integral(1.0, 0.0, 1.0, x[0] - xs, x[-1] - xs, -(y[-1] + y[l]), y[-1] - y[l])
+                    ref += 0.5 * sumwK3 - 0.5 * I
+                assert J[row_E2(c, k, l)] == pytest.approx(ref, abs=1e-12), (n0, k, l)
+                case = _case(n0 + 1, k + 1) if l == m else None
+                ref1 = co[("E1_zetax", case)] * c.h / c.froude ** 2 if case else 0.0
+                assert J[row_E1(c, k, l)] == pytest.approx(ref1, abs=TOLJ)
+
+
+@pytest.mark.parametrize("scheme,y1", [(0, 0.0), (1, 0.0), (0, 0.6)])
+def test_PJ2_exact_jv_vs_richardson_central_differences(oracleC, oracle80, scheme, y1):
+    """Nonlinear state, random direction: D(s) = (E(u+sv) - E(u-sv)) / 2s in long double has error
+    c2 s^2 + c4 s^4 + rounding; (4 D(s/2) - D(s)) / 3 removes the s^2 term.  Both sides use every
+    term of the residual (K1, K2, S2, I, Bernoulli, spline), so a derivative that silently drops the
+    dependence of anything on u (e.g. of A, B, C inside S2 or I) fails here."""
+    c = W.custom(11, 6, 0.5, -2.0, y1=y1, seed=5, eps=0.4, amp=0.08)
+    p = c.params(scheme)
+    rng = np.random.default_rng(8)
+    u = W.state(c) + 1e-2 * rng.standard_normal(c.n)
+    v = rng.standard_normal(c.n)
+    JV, E0 = oracleC.jv_exact(p, u, v, want_e0=True)
+    assert np.abs(E0 - oracle80.residual(p, u)).max() <= 1e-15 * np.abs(E0).max()  # Re part is E(u)
+
+    def D(s):
+        return (oracle80.residual(p, u + s * v) - oracle80.residual(p, u - s * v)) / (2 * s)
+    s = 2.0 ** -12   # exactly representable: u +- s v is rounded once per entry (error ~1e-16 / s)
+    rich = (4 * D(s / 2) - D(s)) / 3
+    scale = np.abs(JV).max()
+    # remaining error: c4 s^4 (s^4 = 4e-15, large fourth derivatives near the singular pairs),
+    # rounding of u +- s v in FP64 ~ 1e-16 |J| / s
+    assert np.abs(JV - rich).max() / scale <= 1e-10
+    # and the plain central difference converges to it at second order
+    e1 = np.abs(JV - D(s)).max()
+    e2 = np.abs(JV - D(s / 2)).max()
+    assert 3.5 <= e1 / e2 <= 4.5
+
+
+def test_PJ3_exact_jv_linear_rows_and_linearity(oracleC):
+    """E3-E6 are linear in u (eq. (24)): their JV rows are the homogeneous formulas applied to
+    v (B.1 L431); J(u)(a v + b w) = a J(u) v + b J(u) w to round-off; sampled rows leave NaN."""
+    c = small(N=9, M=5, h=0.5, x1=-1.7)
+    p = c.params()
+    rng = np.random.default_rng(4)
+    u = W.state(c) + 1e-2 * rng.standard_normal(c.n)
+    v, w = rng.standard_normal(c.n), rng.standard_normal(c.n)
+    JV = oracleC.jv_exact(p, u, v)
+    half = (c.N + 1) * c.M
+    n_rad, x1, dx = c.n_rad, c.x1, c.h
+    for l in range(c.M):
+        p1, px1, px2 = v[idx_phi1(c, l)], v[idx_phix(c, 0, l)], v[idx_phix(c, 1, l)]
+        z1, zx1, zx2 = v[idx_zeta1(c, l)], v[idx_zetax(c, 0, l)], v[idx_zetax(c, 1, l)]
+        b = l * (c.N + 1)
+        assert JV[b] == pytest.approx(x1 * px1 + n_rad * p1, rel=1e-14)
+        assert JV[b + 1] == pytest.approx(x1 * (px2 - px1) / dx + n_rad * px1, rel=1e-14)
+        assert JV[half + b] == pytest.approx(x1 * zx1 + n_rad * z1, rel=1e-14)
+        assert JV[half + b + 1] == pytest.approx(x1 * (zx2 - zx1) / dx + n_rad * zx1, rel=1e-14)
+    JW = oracleC.jv_exact(p, u, w)
+    Jc = oracleC.jv_exact(p, u, 0.3 * v - 1.7 * w)
+    assert np.abs(Jc - (0.3 * JV - 1.7 * JW)).max() <= 1e-13 * np.abs(Jc).max()
+    rows = np.array([0, 7, 21], dtype=np.int32)
+    Js = oracleC.jv_exact(p, u, v, rows=rows)
+    mask = ~np.isnan(Js)
+    assert mask.sum() == half + 2 * c.M + rows.size
+    assert np.array_equal(Js[mask], JV[mask])
