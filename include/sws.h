@@ -87,12 +87,27 @@ int sws_jv_batch(sws_ctx* ctx, const double* u_dev, const double* V_dev, int32_t
                  const double* sigma_host, double* JV_dev, double* Fpert_dev, double* F0_dev,
                  void* cuda_stream);
 
+/* The analytic Jacobian action: JV_dev[b][n] = J(u) v_b with J = dE/du at
+ * u_dev, i.e. the sigma -> 0 limit of eq. (25), every step a0-a9 of E differentiated by
+ * hand: the reconstruction (19), the spline and the midpoint averages are linear; the Bernoulli
+ * row (13), the source term, the closed form I (through A, B, C, L177) and the kernels K1, K2,
+ * S2 (L107-109, L169-172) are linearised about u.  No shift, no difference of two residuals:
+ * the result is accurate to summation round-off (~1e-13 of |JV|_inf), where the quotient of
+ * sws_jv_batch carries eps_mach / sigma ~ 1e-9..1e-7.  The pair coefficients are computed once
+ * per pair for all b directions ((71 + 4 b) FP64 instructions per pair instead of 45 (b + 1)).
+ * V_dev [b][n] row-major, 1 <= b <= max_batch.  Deterministic.  E(u) itself is not formed. */
+int sws_jv_exact_batch(sws_ctx* ctx, const double* u_dev, const double* V_dev, int32_t b,
+                       double* JV_dev, void* cuda_stream);
+
 /* The same two calls on HOST buffers: host->device copy, compute, device->host copy,
  * then a stream synchronise.  `cuda_stream` as above. */
 int sws_residual_host(sws_ctx* ctx, const double* u_host, double* F_host, void* cuda_stream);
 int sws_jv_batch_host(sws_ctx* ctx, const double* u_host, const double* V_host, int32_t b,
                       const double* sigma_host, double* JV_host, double* Fpert_host,
                       double* F0_host, void* cuda_stream);
+
+int sws_jv_exact_batch_host(sws_ctx* ctx, const double* u_host, const double* V_host, int32_t b,
+                            double* JV_host, void* cuda_stream);
 
 /* The shifts the last sws_jv_batch used (device-computed or copied), after a
  * synchronise of `cuda_stream`.  sigma_host_out has room for b values. */
@@ -112,8 +127,16 @@ int sws_last_launch_count(const sws_ctx* ctx);
 int sws_time_allpairs(sws_ctx* ctx, int32_t states, int32_t reps, float* ms_per_launch,
                       void* cuda_stream);
 
+/* The same for the all-pairs kernel of sws_jv_exact_batch, with the fields and the batch size
+ * of the previous sws_jv_exact_batch call (SWS_EBATCH if there was none). */
+int sws_time_allpairs_lin(sws_ctx* ctx, int32_t reps, float* ms_per_launch, void* cuda_stream);
+
+/* Launch geometry of that kernel for b directions: out6 = {target tiles, column groups, columns
+ * per group, nodes staged per bulk copy, segments per column, directions per tile}. */
+int sws_lin_plan_info(sws_ctx* ctx, int32_t b, int32_t* out6);
+
 /* Live timing of the dominant kernel inside ordinary calls.  While profiling is on, every
- * sws_residual / sws_jv_batch brackets its all-pairs launch with a CUDA event pair on the
+ * sws_residual / sws_jv_batch / sws_jv_exact_batch brackets its all-pairs launch with a CUDA event pair on the
  * call's stream (no synchronisation, two event records per call).  sws_profile_read
  * synchronises those events and returns the summed all-pairs time (ms) and the number of
  * launches since the last reset; reset != 0 clears the list. */

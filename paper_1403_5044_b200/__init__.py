@@ -25,6 +25,7 @@ SYMBOLS = (
     "sws_workspace_bytes", "sws_last_launch_count", "sws_time_allpairs", "sws_set_tuning",
     "sws_plan_info", "sws_set_profiling", "sws_profile_read", "sws_destroy", "sws_strerror", "sws_last_cuda_error",
     "sws_probe_fp64_peak", "sws_debug_rsqrt_host",
+    "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
 )
 
 
@@ -57,6 +58,10 @@ def load_library() -> C.CDLL:
         "sws_setup": (C.c_int, [C.POINTER(SwsParams), C.POINTER(vp)]),
         "sws_residual": (C.c_int, [vp, dp, dp, vp]),
         "sws_jv_batch": (C.c_int, [vp, dp, dp, C.c_int32, dp, dp, dp, dp, vp]),
+        "sws_jv_exact_batch": (C.c_int, [vp, dp, dp, C.c_int32, dp, vp]),
+        "sws_jv_exact_batch_host": (C.c_int, [vp, dp, dp, C.c_int32, dp, vp]),
+        "sws_time_allpairs_lin": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_float), vp]),
+        "sws_lin_plan_info": (C.c_int, [vp, C.c_int32, ip]),
         "sws_residual_host": (C.c_int, [vp, dp, dp, vp]),
         "sws_jv_batch_host": (C.c_int, [vp, dp, dp, C.c_int32, dp, dp, dp, dp, vp]),
         "sws_last_sigma": (C.c_int, [vp, C.c_int32, dp, vp]),
@@ -188,6 +193,28 @@ class Context:
             return JV, Fp, F0
         return JV
 
+    def jv_exact_batch(self, u, V, out=None, stream=None):
+        """JV[b] = J(u) v_b, the analytic Jacobian action (sws_jv_exact_batch); asynchronous."""
+        b = int(V.shape[0])
+        JV = out if out is not None else self._new(b, self.n)
+        _check(self.lib.sws_jv_exact_batch(self._h, self._dev(u, (self.n,), "u"),
+                                           self._dev(V, (b, self.n), "V"), b,
+                                           self._dev(JV, (b, self.n), "JV"), self._stream(stream)),
+               "sws_jv_exact_batch")
+        return JV
+
+    def jv_exact_batch_host(self, u: np.ndarray, V: np.ndarray, out=None, stream=None) -> np.ndarray:
+        """The same on HOST buffers (sws_jv_exact_batch_host): H2D, compute, D2H, synchronise."""
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        V = np.ascontiguousarray(V, dtype=np.float64)
+        b = int(V.shape[0])
+        if u.shape != (self.n,) or V.shape != (b, self.n):
+            raise SwsError("u/V: wrong shape")
+        JV = out if out is not None else np.empty((b, self.n))
+        _check(self.lib.sws_jv_exact_batch_host(self._h, _np_ptr(u), _np_ptr(V), b, _np_ptr(JV),
+                                                self._stream(stream)), "sws_jv_exact_batch_host")
+        return JV
+
     def residual_host(self, u: np.ndarray, out: np.ndarray | None = None, stream=None) -> np.ndarray:
         """E(u) on HOST buffers (sws_residual_host): H2D copy, compute, D2H copy, synchronise."""
         u = np.ascontiguousarray(u, dtype=np.float64)
@@ -228,6 +255,19 @@ class Context:
         _check(self.lib.sws_time_allpairs(self._h, int(states), int(reps), C.byref(ms),
                                           self._stream(stream)), "sws_time_allpairs")
         return float(ms.value)
+
+    def time_allpairs_lin(self, reps: int = 1, stream=None) -> float:
+        """ms per launch of the analytic-Jv all-pairs kernel alone (after a jv_exact_batch call)."""
+        ms = C.c_float()
+        _check(self.lib.sws_time_allpairs_lin(self._h, int(reps), C.byref(ms), self._stream(stream)),
+               "sws_time_allpairs_lin")
+        return float(ms.value)
+
+    def lin_plan_info(self, b: int) -> dict:
+        out = (C.c_int32 * 6)()
+        _check(self.lib.sws_lin_plan_info(self._h, int(b), out), "sws_lin_plan_info")
+        return dict(tiles=out[0], chunks=out[1], cols_per_chunk=out[2], seg_len=out[3], nseg=out[4],
+                    dirs_per_tile=out[5])
 
     def set_profiling(self, on: bool = True) -> None:
         _check(self.lib.sws_set_profiling(self._h, int(bool(on))), "sws_set_profiling")

@@ -13,7 +13,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libsws.so"
-SOURCES = ["sws_api.cu", "sws_fields.cu", "sws_allpairs.cu", "sws_allpairs_f32.cu", "sws_probe.cu"]
+SOURCES = ["sws_api.cu", "sws_fields.cu", "sws_allpairs.cu", "sws_allpairs_f32.cu", "sws_jv_exact.cu", "sws_probe.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
 

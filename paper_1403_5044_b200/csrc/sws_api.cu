@@ -42,6 +42,7 @@ static cudaError_t dev_alloc(T** p, size_t count, size_t* total) {
 static void free_all(sws_ctx* c) {
   void* ptrs[] = {c->x, c->y, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zx, c->px, c->zy, c->py,
                   c->src, c->srcf, c->tgt, c->e2loc, c->part, c->F0, c->Fpert, c->sigma, c->norm_part,
+                  c->dsrc, c->dtgt, c->e2lin, c->tgtI,
                   c->u_stage, c->V_stage, c->out_stage};
   for (void* p : ptrs)
     if (p) cudaFree(p);
@@ -104,6 +105,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
 
   e = p->precision == 1 ? sws::allpairs_f32_configure(&c->pair_occ) : sws::allpairs_configure(&c->pair_occ);
   if (e == cudaSuccess) e = sws::fields_configure(c);
+  if (e == cudaSuccess && p->max_batch > 0) e = sws::lin_configure(c);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "kernel configuration (is this an sm_100 device?)"); }
 
   // workspace
@@ -115,7 +117,17 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   if (part_chunks > sws::max_chunks(c)) part_chunks = sws::max_chunks(c);
   if (part_chunks < sws::make_plan(c).chunks) part_chunks = sws::make_plan(c).chunks;
   c->part_chunks = part_chunks;
-  const size_t part_elems = (size_t)part_chunks * c->max_states * T;
+  c->part_rows = (size_t)part_chunks * c->max_states;
+  int lin_bt = 0, lin_groups = 0;
+  if (p->max_batch > 0) {
+    // the analytic Jacobian action keeps [group][chunk][6 + BT] rows per target in `part`
+    lin_bt = sws::lin_tile(p->max_batch);
+    lin_groups = (p->max_batch + lin_bt - 1) / lin_bt;
+    int lin_chunks = sws::max_chunks(c) < 32 ? sws::max_chunks(c) : 32;
+    const size_t need = (size_t)lin_chunks * (6 + lin_bt) * lin_groups;
+    if (need > c->part_rows) c->part_rows = need;
+  }
+  const size_t part_elems = c->part_rows * T;
   size_t tot = 0;
   bool ok = true;
 #define ALLOC(ptr, count) ok = ok && (dev_alloc(&c->ptr, (count), &tot) == cudaSuccess)
@@ -137,6 +149,12 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   ALLOC(u_stage, n);
   ALLOC(V_stage, mb * n);
   ALLOC(out_stage, (2 * mb + 1) * n);
+  if (mb > 0) {
+    ALLOC(dsrc, (size_t)lin_groups * lin_bt * S);
+    ALLOC(dtgt, mb * T);
+    ALLOC(e2lin, mb * T);
+    ALLOC(tgtI, T);
+  }
 #undef ALLOC
   if (!ok) {
     cudaGetLastError();
@@ -168,6 +186,8 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   if (e == cudaSuccess) e = cudaMemcpy(c->y, hy.data(), hy.size() * 8, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(c->sp_cp, cp.data(), cp.size() * 8, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(c->sp_inv, inv.data(), inv.size() * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess && c->dsrc)  // unused direction slots of the last tile stay zero
+    e = cudaMemset(c->dsrc, 0, (size_t)lin_groups * lin_bt * S * sizeof(double4));
   if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
   if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -202,32 +222,40 @@ int sws_set_tuning(sws_ctx* c, int32_t chunks) {
   return SWS_OK;
 }
 
+// While profiling is on: take the next (before, after) event pair and record `before`.
+static int prof_begin(sws_ctx* c, cudaStream_t st, cudaEvent_t* pe0, cudaEvent_t* pe1) {
+  *pe0 = *pe1 = nullptr;
+  if (!c->profiling) return SWS_OK;
+  if (!c->prof_events) c->prof_events = new (std::nothrow) std::vector<cudaEvent_t>();
+  if (!c->prof_events) return SWS_ENOMEM;
+  while (c->prof_events->size() < c->prof_used + 2) {
+    cudaEvent_t ev;
+    CK(cudaEventCreate(&ev));
+    c->prof_events->push_back(ev);
+  }
+  *pe0 = (*c->prof_events)[c->prof_used];
+  *pe1 = (*c->prof_events)[c->prof_used + 1];
+  c->prof_used += 2;
+  CK(cudaEventRecord(*pe0, st));
+  return SWS_OK;
+}
+
 // a0-a9 for `states` states (state 0 = u, state s = u + sigma_{s-1} v_{s-1}).
 static int run_states(sws_ctx* c, const double* u, const double* V, int states, double* F0,
                       double* Fpert, cudaStream_t st, int* launches) {
   const sws::PairPlan plan = sws::make_plan(c);
-  CK(sws::launch_reconstruct(c, u, V, states, F0, Fpert, st));
+  CK(sws::launch_reconstruct(c, u, V, states, 0, F0, Fpert, st));
   CK(sws::launch_dy(c, states, st));
-  CK(sws::launch_targets(c, states, F0, Fpert, st));
+  CK(sws::launch_targets(c, states, F0, Fpert, nullptr, st));
   cudaEvent_t pe0 = nullptr, pe1 = nullptr;
-  if (c->profiling) {
-    if (!c->prof_events) c->prof_events = new (std::nothrow) std::vector<cudaEvent_t>();
-    if (!c->prof_events) return SWS_ENOMEM;
-    while (c->prof_events->size() < c->prof_used + 2) {
-      cudaEvent_t ev;
-      CK(cudaEventCreate(&ev));
-      c->prof_events->push_back(ev);
-    }
-    pe0 = (*c->prof_events)[c->prof_used];
-    pe1 = (*c->prof_events)[c->prof_used + 1];
-    c->prof_used += 2;
-    CK(cudaEventRecord(pe0, st));
-  }
+  int rc = prof_begin(c, st, &pe0, &pe1);
+  if (rc != SWS_OK) return rc;
   CK(sws::launch_allpairs(c, states, plan, st));
   if (pe1) CK(cudaEventRecord(pe1, st));
   CK(sws::launch_assemble(c, states, plan, F0, Fpert, st));
   *launches += 5;
   c->last_states = states;
+  c->last_lin_b = 0;
   return SWS_OK;
 }
 
@@ -261,6 +289,76 @@ int sws_jv_batch(sws_ctx* c, const double* u_dev, const double* V_dev, int32_t b
   CK(sws::launch_jv_quotient(c, F0, Fp, b, JV_dev, st));
   launches += 1;
   c->last_launches = launches;
+  return SWS_OK;
+}
+
+int sws_jv_exact_batch(sws_ctx* c, const double* u_dev, const double* V_dev, int32_t b, double* JV_dev,
+                       void* cuda_stream) {
+  if (!c || !u_dev || !V_dev || !JV_dev) return SWS_EINVAL;
+  if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
+  const sws::PairPlan plan = sws::make_lin_plan(c, BT, groups);
+  // derivative fields of every direction (states 1..b) beside the base fields (state 0);
+  // the derivative radiation rows go straight to JV, the base rows to scratch
+  CK(sws::launch_reconstruct(c, u_dev, V_dev, b + 1, 1, c->F0, JV_dev, st));
+  CK(sws::launch_dy(c, b + 1, st));
+  CK(sws::launch_targets(c, 1, c->F0, nullptr, c->tgtI, st));
+  CK(sws::launch_targets_lin(c, b, BT, JV_dev, st));
+  cudaEvent_t pe0 = nullptr, pe1 = nullptr;
+  int rc = prof_begin(c, st, &pe0, &pe1);
+  if (rc != SWS_OK) return rc;
+  CK(sws::launch_allpairs_lin(c, BT, groups, plan, st));
+  if (pe1) CK(cudaEventRecord(pe1, st));
+  CK(sws::launch_assemble_lin(c, b, BT, plan, JV_dev, st));
+  c->last_launches = 6;
+  c->last_states = 1;
+  c->last_lin_b = b;
+  return SWS_OK;
+}
+
+int sws_jv_exact_batch_host(sws_ctx* c, const double* u_host, const double* V_host, int32_t b,
+                            double* JV_host, void* cuda_stream) {
+  if (!c || !u_host || !V_host || !JV_host) return SWS_EINVAL;
+  if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nb = (size_t)c->mesh.n * sizeof(double);
+  CK(cudaMemcpyAsync(c->u_stage, u_host, nb, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(c->V_stage, V_host, nb * b, cudaMemcpyHostToDevice, st));
+  int rc = sws_jv_exact_batch(c, c->u_stage, c->V_stage, b, c->out_stage, cuda_stream);
+  if (rc != SWS_OK) return rc;
+  CK(cudaMemcpyAsync(JV_host, c->out_stage, nb * b, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  return SWS_OK;
+}
+
+int sws_time_allpairs_lin(sws_ctx* c, int32_t reps, float* ms_per_launch, void* cuda_stream) {
+  if (!c || !ms_per_launch || reps < 1) return SWS_EINVAL;
+  if (c->last_lin_b < 1) return SWS_EBATCH;  // needs the fields of a previous sws_jv_exact_batch
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int b = c->last_lin_b, BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
+  const sws::PairPlan plan = sws::make_lin_plan(c, BT, groups);
+  CK(sws::launch_allpairs_lin(c, BT, groups, plan, st));
+  CK(cudaEventRecord(c->ev0, st));
+  for (int r = 0; r < reps; ++r) CK(sws::launch_allpairs_lin(c, BT, groups, plan, st));
+  CK(cudaEventRecord(c->ev1, st));
+  CK(cudaEventSynchronize(c->ev1));
+  float ms = 0.f;
+  CK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+  *ms_per_launch = ms / reps;
+  return SWS_OK;
+}
+
+int sws_lin_plan_info(sws_ctx* c, int32_t b, int32_t* out6) {
+  if (!c || !out6) return SWS_EINVAL;
+  if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
+  const int BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
+  const sws::PairPlan p = sws::make_lin_plan(c, BT, groups);
+  out6[0] = p.tiles; out6[1] = p.chunks; out6[2] = p.cols_per_chunk; out6[3] = p.seg_len; out6[4] = p.nseg;
+  out6[5] = BT;
   return SWS_OK;
 }
 

@@ -29,7 +29,7 @@ __device__ __forceinline__ double* state_out(double* F0, double* Fpert, int stat
 __global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ u,
                                                      const double* __restrict__ V,
                                                      const double* __restrict__ sigma, Mesh m,
-                                                     double* zeta, double* phi, double* zx,
+                                                     int lin, double* zeta, double* phi, double* zx,
                                                      double* px, double* F0, double* Fpert) {
   extern __shared__ double sm[];
   const int N = m.N, l = blockIdx.x, state = blockIdx.y, tid = threadIdx.x;
@@ -43,7 +43,12 @@ __global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ 
   const size_t offp = (size_t)l * (N + 1), offz = half + offp;
   const double* v = state > 0 ? V + (size_t)(state - 1) * m.n : nullptr;
   const double sg = state > 0 ? sigma[state - 1] : 0.0;
+  // lin != 0 (analytic Jacobian action, sws_jv_exact_batch): state s >= 1 is the DIRECTION v_{s-1}
+  // itself - the reconstruction (19) is linear and homogeneous in u, so the same recurrence
+  // applied to v gives the directional derivatives of the nodal fields.
+  const bool dir = lin && state > 0;
   auto get = [&](size_t idx) -> double {
+    if (dir) return v[idx];
     const double a = u[idx];
     return v ? fma(sg, v[idx], a) : a;  // u_b = fl(u + sigma v), one rounding per entry
   };
@@ -73,8 +78,10 @@ __global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ 
     double* F = state_out(F0, Fpert, state, m.n);
     const double x1 = m.x1, nr = m.n_rad;
     const double p1 = s_first[0], z1 = s_first[1];
-    F[offp + 0] = ADD(MUL(x1, SUB(s_px[0], 1.0)), MUL(nr, SUB(p1, x1)));
-    F[offp + 1] = ADD(MUL(x1, SUB(s_px[1], s_px[0]) / m.dx), MUL(nr, SUB(s_px[0], 1.0)));
+    // derivative rows: the constants (-1, -x_1) of E3, E4 drop out (B.1 L431)
+    const double one = dir ? 0.0 : 1.0, xoff = dir ? 0.0 : x1;
+    F[offp + 0] = ADD(MUL(x1, SUB(s_px[0], one)), MUL(nr, SUB(p1, xoff)));
+    F[offp + 1] = ADD(MUL(x1, SUB(s_px[1], s_px[0]) / m.dx), MUL(nr, SUB(s_px[0], one)));
     F[offz + 0] = ADD(MUL(x1, s_zx[0]), MUL(nr, z1));
     F[offz + 1] = ADD(MUL(x1, SUB(s_zx[1], s_zx[0]) / m.dx), MUL(nr, s_zx[0]));
   }
@@ -166,6 +173,43 @@ __device__ double box_int(double A, double B, double C, double sqA, double sqC, 
          G_anti(A, B, C, sqA, sqC, sqD, s2, t1) + G_anti(A, B, C, sqA, sqC, sqD, s1, t1);
 }
 
+// The same antiderivative together with its partial derivatives with respect to A, B, C
+// (analytic Jacobian action: dI = I_A dA + I_B dB + I_C dC).  With Q = A s^2 + B s t + C t^2,
+// w1, w2 the two asinh arguments above, and 1 + w1^2 = 4 A Q / (t^2 D):
+//   dG/dB = 2 sqrt(Q) / D
+//   dG/dA = -B sqrt(Q) / (A D) - t asinh(w1) / (2 A^(3/2))
+//   dG/dC = -B sqrt(Q) / (C D) - s asinh(w2) / (2 C^(3/2))
+// (checked: d^2/ds dt of dG/dB is -s t / (2 Q^(3/2)) = d/dB of the integrand).
+struct G4 {
+  double g, gA, gB, gC;
+};
+
+__device__ G4 G_anti4(double A, double B, double C, double sqA, double sqC, double sqD, double s,
+                      double t) {
+  const double D = sqD * sqD;
+  const double sqQ = sqrt(A * s * s + B * s * t + C * t * t);
+  const double a1 = t != 0.0 ? t * asinh((2 * A * s + B * t) / (fabs(t) * sqD)) : 0.0;
+  const double a2 = s != 0.0 ? s * asinh((2 * C * t + B * s) / (fabs(s) * sqD)) : 0.0;
+  G4 r;
+  r.g = a1 / sqA + a2 / sqC;
+  r.gB = 2.0 * sqQ / D;
+  r.gA = -B * sqQ / (A * D) - a1 / (2.0 * A * sqA);
+  r.gC = -B * sqQ / (C * D) - a2 / (2.0 * C * sqC);
+  return r;
+}
+
+__device__ G4 box_int4(double A, double B, double C, double sqA, double sqC, double sqD, double s1,
+                       double s2, double t1, double t2) {
+  const G4 a = G_anti4(A, B, C, sqA, sqC, sqD, s2, t2), b = G_anti4(A, B, C, sqA, sqC, sqD, s1, t2),
+           c = G_anti4(A, B, C, sqA, sqC, sqD, s2, t1), d = G_anti4(A, B, C, sqA, sqC, sqD, s1, t1);
+  G4 r;
+  r.g = a.g - b.g - c.g + d.g;
+  r.gA = a.gA - b.gA - c.gA + d.gA;
+  r.gB = a.gB - b.gB - c.gB + d.gB;
+  r.gC = a.gC - b.gC - c.gC + d.gC;
+  return r;
+}
+
 // a3 + a5 + a6 (local part) + a7 + packing of the transposed source records.
 // One thread per node (k, l) of one state; threads with k < N-1 also own target (k, l).
 __global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restrict__ x,
@@ -176,8 +220,8 @@ __global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restric
                                                  const double* __restrict__ px,
                                                  const double* __restrict__ zy,
                                                  const double* __restrict__ py, SrcRec* src,
-                                                 SrcRecF* srcf, TgtRec* tgt, double* e2loc, double* F0,
-                                                 double* Fpert) {
+                                                 SrcRecF* srcf, TgtRec* tgt, double* e2loc, double4* tgtI,
+                                                 double* F0, double* Fpert) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= m.N) return;
   const int N = m.N, M = m.M, l = blockIdx.y, state = blockIdx.z;
@@ -228,6 +272,20 @@ __global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restric
   const double sqA = sqrt(A), sqC = sqrt(C), sqD = sqrt(4 * A * C - B * B);
   const double s1 = x[0] - xs, s2 = x[N - 1] - xs;
   const double ya = y[0], yb = y[M - 1];
+  if (tgtI) {
+    // analytic Jacobian action: {I, dI/dA, dI/dB, dI/dC} of the base state; the residual rows
+    // of this state are not needed (and not formed) in that mode
+    G4 r;
+    if (ya == 0.0) {
+      r = box_int4(A, B, C, sqA, sqC, sqD, s1, s2, -(yb + ys), yb - ys);
+    } else {
+      const G4 r1 = box_int4(A, B, C, sqA, sqC, sqD, s1, s2, ya - ys, yb - ys);
+      const G4 r2 = box_int4(A, B, C, sqA, sqC, sqD, s1, s2, -(yb + ys), -(ya + ys));
+      r.g = r1.g + r2.g; r.gA = r1.gA + r2.gA; r.gB = r1.gB + r2.gB; r.gC = r1.gC + r2.gC;
+    }
+    tgtI[t] = make_double4(r.g, r.gA, r.gB, r.gC);
+    return;
+  }
   double I;
   if (ya == 0.0) {
     // the two boxes share the edge t = -y*: one box over t in [-(y_M + y*), y_M - y*]
@@ -307,11 +365,11 @@ cudaError_t fields_configure(const sws_ctx* c) {
                               (int)reconstruct_smem_bytes(c->mesh.N));
 }
 
-cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states, double* F0,
-                               double* Fpert, cudaStream_t st) {
+cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states, int lin,
+                               double* F0, double* Fpert, cudaStream_t st) {
   const Mesh& m = c->mesh;
   dim3 grid(m.M, states);
-  k_reconstruct<<<grid, 256, reconstruct_smem_bytes(m.N), st>>>(u, V, c->sigma, m, c->zeta, c->phi,
+  k_reconstruct<<<grid, 256, reconstruct_smem_bytes(m.N), st>>>(u, V, c->sigma, m, lin, c->zeta, c->phi,
                                                                  c->zx, c->px, F0, Fpert);
   return cudaGetLastError();
 }
@@ -323,11 +381,12 @@ cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, cudaStream_t st) {
+cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, double4* tgtI,
+                           cudaStream_t st) {
   const Mesh& m = c->mesh;
   dim3 grid((m.N + 127) / 128, m.M, states);
   k_targets<<<grid, 128, 0, st>>>(m, c->x, c->y, c->zeta, c->phi, c->zx, c->px, c->zy, c->py, c->src,
-                                  c->srcf, c->tgt, c->e2loc, F0, Fpert);
+                                  c->srcf, c->tgt, c->e2loc, tgtI, F0, Fpert);
   return cudaGetLastError();
 }
 

@@ -34,6 +34,13 @@ struct __align__(32) TgtRec {
   double A, B, C;   // 1 + zeta_x*^2, 2 zeta_x* zeta_y*, 1 + zeta_y*^2   (L177)
 };
 
+// Directional derivatives of one target's starred values for one direction (analytic Jacobian
+// action, sws_jv_exact.cu): 48 B.
+struct DTgtRec {
+  double dzs, dpsis, dzxs;  // d zeta*, d phi*, d zeta_x*
+  double dA, dB, dC;
+};
+
 struct Mesh {
   int N, M;     // nodes
   int T, S, n;  // (N-1)M targets, NM sources, 2(N+1)M unknowns
@@ -69,6 +76,7 @@ struct sws_ctx {
   size_t ws_bytes;
   int last_launches;
   int last_states;      // states the workspace fields currently describe
+  int last_lin_b;       // directions the derivative fields describe (0: none)
 
   // geometry (device)
   double* x;  // [N]
@@ -91,6 +99,14 @@ struct sws_ctx {
   double* e2loc;     // [state][t]   2 pi (phi*-x*) + eps/rho* - zeta_x* I
   double* part;      // [state][chunk][t] partial all-pairs sums (already times dx dy)
   int part_chunks;   // chunk capacity of `part` per state
+  size_t part_rows;  // capacity of `part` in rows of T doubles
+
+  // analytic Jacobian action (max_batch > 0 only)
+  double4* dsrc;          // [group][i][j][BT] {d zeta, d phi, d zeta_x, -d zeta_y}
+  sws::DTgtRec* dtgt;     // [direction][t]
+  double* e2lin;          // [direction][t] local part of the derivative of E2
+  double4* tgtI;          // [t] {I, dI/dA, dI/dB, dI/dC} of the base state
+  int lin_occ[4];         // resident CTAs per SM of k_allpairs_lin<1,4,8,16>
 
   double* F0;         // [n] base residual of a batch when the caller passes no F0_dev
   double* Fpert;      // [max_batch][n] when the caller passes no Fpert_dev
@@ -110,10 +126,13 @@ namespace sws {
 
 // Launches (all asynchronous on `st`); each returns the cudaError_t of its launch.
 // states = 1: base state only.  State s >= 1 is u + sigma[s-1] * V[s-1].
-cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states,
+// lin != 0: states >= 1 are the directions v themselves (derivative fields, homogeneous rows)
+cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states, int lin,
                                double* F0, double* Fpert, cudaStream_t st);
 cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st);
-cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, cudaStream_t st);
+// tgtI != NULL: base state of the analytic Jacobian action ({I, I_A, I_B, I_C} instead of e2loc)
+cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, double4* tgtI,
+                           cudaStream_t st);
 // dispatches on sws_params.precision (0: FP64 kernel, 1: FP32 pair arithmetic)
 cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
 cudaError_t launch_allpairs_f32(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
@@ -122,6 +141,15 @@ cudaError_t launch_assemble(sws_ctx* c, int states, const PairPlan& plan, double
 cudaError_t launch_sigma(sws_ctx* c, const double* u, const double* V, int b, cudaStream_t st);
 cudaError_t launch_jv_quotient(sws_ctx* c, const double* F0, const double* Fpert, int b,
                                double* JV, cudaStream_t st);
+
+// analytic Jacobian action (sws_jv_exact.cu); BT = directions per tile (1, 4, 8 or 16)
+int lin_tile(int b);
+cudaError_t lin_configure(sws_ctx* c);
+PairPlan make_lin_plan(const sws_ctx* c, int BT, int groups);
+cudaError_t launch_targets_lin(sws_ctx* c, int b, int BT, double* JV, cudaStream_t st);
+cudaError_t launch_allpairs_lin(sws_ctx* c, int BT, int groups, const PairPlan& plan, cudaStream_t st);
+cudaError_t launch_assemble_lin(sws_ctx* c, int b, int BT, const PairPlan& plan, double* JV,
+                                cudaStream_t st);
 
 PairPlan make_plan(const sws_ctx* c);
 int max_chunks(const sws_ctx* c);

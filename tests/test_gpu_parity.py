@@ -292,3 +292,110 @@ def test_fp32_variant_cfg4_sampled_and_batch(sws, oracle80):
     err = float(np.abs(F[mask] - E[mask]).max() / np.abs(F).max())
     print(f"\nFP32 variant cfg4 sampled rows: {err:.3e}")
     assert 1e-9 < err <= F32_SANITY
+
+
+# ---------------------------------------------------------------------------------------
+# The analytic Jacobian action sws_jv_exact_batch against the complex-step
+# oracle (oracle c80: Im E(u + i h v) / h of the SAME residual code the other tests use, no
+# hand-derived formula on that side).  Bar: 1e-10 relative to |JV|_inf per direction.
+def jv_exact_gpu(sws, p, u, V, max_batch=None):
+    import torch
+    b = V.shape[0]
+    with sws.Context(p, max_batch=max_batch or b) as ctx:
+        JV = ctx.jv_exact_batch(dev(u), dev(V))
+        torch.cuda.synchronize()
+        n_launch = ctx.last_launch_count
+        JV2 = ctx.jv_exact_batch(dev(u), dev(V)).cpu().numpy()
+        JV = JV.cpu().numpy()
+    assert n_launch == 6
+    assert np.array_equal(JV, JV2)  # deterministic
+    return JV
+
+
+@pytest.mark.parametrize("i,b", [(0, 1), (0, 3), (1, 8), (1, 5), (1, 17)])
+def test_jv_exact_full_parity(sws, oracleC, i, b):
+    """cfg 1, 2: every entry of every direction; b = 1, 3, 5, 8, 17 exercise each direction-tile
+    width (1, 4, 8, 16), a partly filled tile and two tiles."""
+    cfg = W.CONFIGS[i]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg, b)
+    JV = jv_exact_gpu(sws, p, u, V)
+    for k in range(b):
+        ref = oracleC.jv_exact(p, u, V[k])
+        assert relerr(JV[k], ref) <= TOL, (k, relerr(JV[k], ref))
+
+
+@pytest.mark.parametrize("kw", RAGGED, ids=lambda k: f"{k['N']}x{k['M']}")
+@pytest.mark.parametrize("dy_scheme", [0, 1])
+def test_jv_exact_ragged_shapes(sws, oracleC, kw, dy_scheme):
+    cfg = W.custom(eps=0.3, amp=0.05, **kw)
+    rng = np.random.default_rng(13)
+    u = W.state(cfg) + 1e-3 * rng.standard_normal(cfg.n)
+    V = rng.standard_normal((2, cfg.n))
+    p = cfg.params(dy_scheme)
+    JV = jv_exact_gpu(sws, p, u, V, max_batch=4)
+    for k in range(2):
+        ref = oracleC.jv_exact(p, u, V[k])
+        assert relerr(JV[k], ref) <= TOL, (k, relerr(JV[k], ref))
+
+
+def test_jv_exact_cfg3_batch16(sws, oracleC):
+    """cfg 3 (181x61), b = 16 in one launch: three directions in full against the oracle, the
+    rest on sampled rows; plus consistency with the finite-difference batch (eq. (25)) at its
+    own accuracy (reading Q9 (ii): ~1e-7 relative)."""
+    import torch
+    cfg = W.CONFIGS[2]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg)
+    b = V.shape[0]
+    assert b == 16
+    with sws.Context(p, max_batch=b) as ctx:
+        JV = ctx.jv_exact_batch(dev(u), dev(V)).cpu().numpy()
+        JV_fd = ctx.jv_batch(dev(u), dev(V)).cpu().numpy()
+        torch.cuda.synchronize()
+    rows = np.unique(np.random.default_rng(5).integers(0, cfg.targets, 48)).astype(np.int32)
+    for k in range(b):
+        full = k in (0, 7, 15)
+        ref = oracleC.jv_exact(p, u, V[k], rows=None if full else rows)
+        mask = ~np.isnan(ref)
+        err = np.abs(JV[k][mask] - ref[mask]).max() / np.abs(JV[k]).max()
+        assert err <= TOL, (k, err)
+        assert relerr(JV_fd[k], JV[k]) <= 1e-5
+
+
+@pytest.mark.parametrize("i,rows,dirs", [(3, 64, (0, 31)), (4, 32, (0, 15))])
+def test_jv_exact_large_configs_sampled_rows(sws, oracleC, i, rows, dirs):
+    """cfg 4 (b = 32, two direction tiles) and cfg 5 (b = 16) at full size, in the launch
+    configuration bench.py times: all O(NM) rows and a seeded sample of integral-equation rows of
+    two directions against the oracle."""
+    cfg = W.CONFIGS[i]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg)
+    JV = jv_exact_gpu(sws, p, u, V)
+    assert np.isfinite(JV).all()
+    rng = np.random.default_rng(4321 + i)
+    T = cfg.targets
+    pick = np.unique(np.concatenate([
+        rng.integers(0, T, rows), [0, cfg.N - 2, T - 1, T - (cfg.N - 1), (cfg.M // 2) * (cfg.N - 1) + cfg.N // 2],
+    ])).astype(np.int32)
+    for k in dirs:
+        ref = oracleC.jv_exact(p, u, V[k], rows=pick)
+        mask = ~np.isnan(ref)
+        err = np.abs(JV[k][mask] - ref[mask]).max() / np.abs(JV[k]).max()
+        assert err <= TOL, (k, err)
+
+
+def test_jv_exact_host_api_and_errors(sws):
+    cfg = W.CONFIGS[1]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg, 3)
+    with sws.Context(p, max_batch=4) as ctx:
+        JVd = ctx.jv_exact_batch(dev(u), dev(V)).cpu().numpy()
+        JVh = ctx.jv_exact_batch_host(u, V)
+        assert np.array_equal(JVd, JVh)
+        info = ctx.lin_plan_info(3)
+        assert info["dirs_per_tile"] == 4 and info["tiles"] == -(-cfg.targets // 128)
+        with pytest.raises(sws.SwsError, match="batch"):
+            ctx.jv_exact_batch(dev(u), dev(W.directions(cfg, 5)))
+        # the FD path still works on the same context afterwards (shared workspace)
+        F = ctx.residual(dev(u)).cpu().numpy()
+    with sws.Context(p) as c0:
+        assert np.array_equal(c0.residual(dev(u)).cpu().numpy(), F)
+        with pytest.raises(sws.SwsError, match="batch"):
+            c0.jv_exact_batch(dev(u), dev(V))
