@@ -206,6 +206,48 @@ def fp32_variant_report(sws, device: int, names=("cfg4_361x121",), steps: int = 
     return out
 
 
+# FP64 instructions per pair of k_allpairs_lin<BT> (SASS inner loop): 71 shared by the
+# BT directions (31 DFMA + 40 DMUL/DADD) + 4 DFMA per direction
+LIN_INSTR_SHARED, LIN_FLOPS_SHARED = 71, 102
+
+
+def jv_exact_report(ctx, cfg, u, V, steps: int, flush, peak_tf: float) -> dict:
+    """sws_jv_exact_batch on the bench workload: b analytic Jacobian-vector
+    products per call, timed like the main step (CUDA events, L2 flush between iterations)."""
+    import torch
+    b = int(V.shape[0])
+    JV = torch.empty((b, cfg.n), dtype=torch.float64, device=u.device)
+    for _ in range(2):
+        ctx.jv_exact_batch(u, V, out=JV)
+    torch.cuda.synchronize()
+    ctx.set_profiling(True)
+    ctx.profile_read(reset=True)
+    ms = 0.0
+    for _ in range(steps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.jv_exact_batch(u, V, out=JV)
+        e1.record()
+        torch.cuda.synchronize()
+        ms += e0.elapsed_time(e1)
+    ap_ms, ap_n = ctx.profile_read(reset=True)
+    ctx.set_profiling(False)
+    ms /= steps
+    info = ctx.lin_plan_info(b)
+    bt = info["dirs_per_tile"]
+    groups = -(-b // bt)
+    flops_pair = LIN_FLOPS_SHARED + 8 * bt
+    ach = flops_pair * cfg.pairs * groups / (ap_ms / max(ap_n, 1) * 1e-3) / 1e12
+    return {"jv_per_s": b / (ms * 1e-3), "ms_per_batch": ms, "b": b, "launches_per_batch": ctx.last_launch_count,
+            "allpairs_lin_ms": ap_ms / max(ap_n, 1), "share_of_batch": ap_ms / max(ap_n, 1) / ms,
+            "pair_direction_products_per_s": b * cfg.pairs / (ms * 1e-3),
+            "fp64_instr_per_pair": LIN_INSTR_SHARED + 4 * bt, "flops_per_pair": flops_pair,
+            "achieved_tflops": ach, "frac_of_fp64_peak": ach / peak_tf, "plan": info,
+            "note": "analytic J(u)v (no finite difference); parity 1e-10 of |JV|_inf against the complex-step "
+                    "oracle in tests/test_gpu_parity.py"}
+
+
 def run_ours(args) -> None:
     import torch
 
@@ -341,6 +383,13 @@ def run_ours(args) -> None:
                                   f"{dt:.1f} s, scaled by rows/T",
                         "pairs_per_s": v * cfg.pairs}
 
+    jvx = None
+    if world == 1 and not args.no_jv_exact:
+        jvx = jv_exact_report(ctx, cfg, u, V, max(2, args.steps), flush, peak_tf)
+        # the finite-difference batch of the main step computes the same b products from b + 1 evaluations
+        jvx["speedup_vs_fd_batch"] = (jvx["jv_per_s"] /
+                                      (b / ((ms_total / args.steps) * 1e-3 * (b + 1) / evals_per_step)))
+
     fp32 = None
     if world == 1 and not args.no_fp32:
         fp32 = fp32_variant_report(sws, local, names=tuple(dict.fromkeys(["cfg4_361x121", cfg.name])))
@@ -362,6 +411,7 @@ def run_ours(args) -> None:
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
         "workspace_bytes": ctx.workspace_bytes,
+        "jv_exact": jvx,
         "fp32_variant": fp32,
     }
     print(json.dumps(line), flush=True)
@@ -380,6 +430,7 @@ def main() -> None:
     ap.add_argument("--ref-rows", type=int, default=2048, help="rows per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fp32", action="store_true", help="skip the reported FP32-variant section")
+    ap.add_argument("--no-jv-exact", action="store_true", help="skip the analytic-Jv section")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)

@@ -33,6 +33,16 @@
 
 namespace sws {
 
+#ifndef SWS_LIN_ORDER
+#define SWS_LIN_ORDER 1  // 1: coefficient-major accumulation, 0: direction-major
+#endif
+#ifndef SWS_LIN_UNROLL
+#define SWS_LIN_UNROLL 1
+#endif
+#ifndef SWS_LIN_MINB16
+#define SWS_LIN_MINB16 3
+#endif
+
 // ---------------------------------------------------------------------------------------
 // Per node / per target linearisation for direction d (grid.z).  Base fields = state 0 of the
 // planes, direction fields = state d + 1 (written by k_reconstruct in lin mode and k_dy).
@@ -175,16 +185,41 @@ __device__ __forceinline__ void pair_lin(const double2 zp, const double2 sl, con
   s.u3y += vm - vp;
   s.u3yy = fma(dm, vm, s.u3yy);
   s.u3yy = fma(dp, vp, s.u3yy);
+  // Coefficient-major order: runs of BT DFMAs that share one coefficient register in the same
+  // operand slot (the operand-reuse cache then leaves two fresh 64-bit register reads per DFMA,
+  // which is what the FP64 pipe can be fed at full rate).
+  const double2* dv2 = reinterpret_cast<const double2*>(dv);
+#if SWS_LIN_ORDER == 1
+  {
+    double2 lo[BT];
+#pragma unroll
+    for (int d = 0; d < BT; ++d) lo[d] = dv2[2 * d];  // {d zeta, d phi}
+#pragma unroll
+    for (int d = 0; d < BT; ++d) acc[d] = fma(K1, lo[d].y, acc[d]);
+#pragma unroll
+    for (int d = 0; d < BT; ++d) acc[d] = fma(cz, lo[d].x, acc[d]);
+  }
+  {
+    double2 hi[BT];
+#pragma unroll
+    for (int d = 0; d < BT; ++d) hi[d] = dv2[2 * d + 1];  // {d zeta_x, -d zeta_y}
+#pragma unroll
+    for (int d = 0; d < BT; ++d) acc[d] = fma(czx, hi[d].x, acc[d]);
+#pragma unroll
+    for (int d = 0; d < BT; ++d) acc[d] = fma(czy, hi[d].y, acc[d]);
+  }
+#else
 #pragma unroll
   for (int d = 0; d < BT; ++d) {
-    const double4 v = dv[d];  // {d zeta, d phi, d zeta_x, -d zeta_y} of direction d at this node
+    const double2 lo = dv2[2 * d], hi = dv2[2 * d + 1];
     double a = acc[d];
-    a = fma(K1, v.y, a);
-    a = fma(cz, v.x, a);
-    a = fma(czx, v.z, a);
-    a = fma(czy, v.w, a);
+    a = fma(K1, lo.y, a);
+    a = fma(cz, lo.x, a);
+    a = fma(czx, hi.x, a);
+    a = fma(czy, hi.y, a);
     acc[d] = a;
   }
+#endif
 }
 
 struct LinArgs {
@@ -198,10 +233,11 @@ struct LinArgs {
   int chunks, cols_per_chunk, seg_len, nseg;
 };
 
+constexpr int kLinUnroll = SWS_LIN_UNROLL;
 constexpr int kLinShared = 6;  // direction-independent sums per (chunk, target)
 
 template <int BT>
-__global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? 2 : BT >= 8 ? 3 : 4)) k_allpairs_lin(const LinArgs a) {
+__global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT >= 8 ? 3 : 4)) k_allpairs_lin(const LinArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int seg_pad = a.seg_len;  // even
   SrcRec* s_rec = reinterpret_cast<SrcRec*>(smem_raw);                          // [kStages][seg]
@@ -282,7 +318,7 @@ __global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? 2 : BT >= 8 ? 3 : 4)
       for (int j = jlo; j < jhi; ++j)
         pair_lin<BT, true>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * BT, ci, tg, cc, col, acc);
     } else {
-#pragma unroll 2
+#pragma unroll kLinUnroll
       for (int j = jlo; j < jhi; ++j)
         pair_lin<BT, false>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * BT, 1.0, tg, cc, col, acc);
     }
