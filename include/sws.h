@@ -113,6 +113,9 @@ int sws_jv_exact_batch_host(sws_ctx* ctx, const double* u_host, const double* V_
  * synchronise of `cuda_stream`.  sigma_host_out has room for b values. */
 int sws_last_sigma(sws_ctx* ctx, int32_t b, double* sigma_host_out, void* cuda_stream);
 
+/* Copy of the parameters the context was set up with (max_batch and device included). */
+int sws_get_params(const sws_ctx* ctx, sws_params* out);
+
 size_t sws_num_unknowns(const sws_ctx* ctx); /* 2(N+1)M */
 size_t sws_num_targets(const sws_ctx* ctx);  /* (N-1)M half-mesh points */
 size_t sws_num_sources(const sws_ctx* ctx);  /* NM nodes */

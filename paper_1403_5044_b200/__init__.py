@@ -26,6 +26,7 @@ SYMBOLS = (
     "sws_plan_info", "sws_set_profiling", "sws_profile_read", "sws_destroy", "sws_strerror", "sws_last_cuda_error",
     "sws_probe_fp64_peak", "sws_debug_rsqrt_host",
     "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
+    "sws_get_params",
 )
 
 
@@ -52,10 +53,11 @@ def load_library() -> C.CDLL:
     if not LIB_PATH.exists():
         raise SwsError(f"{LIB_PATH} is missing: run `python -m paper_1403_5044_b200.build` "
                        "(nvcc, sm_100a).  There is no CPU fallback.")
-    lib = C.CDLL(str(LIB_PATH))
+    lib = C.CDLL(str(LIB_PATH), mode=C.RTLD_GLOBAL)  # libsws_jfnk.so resolves sws_* against it
     vp, dp, ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)
     proto = {
         "sws_setup": (C.c_int, [C.POINTER(SwsParams), C.POINTER(vp)]),
+        "sws_get_params": (C.c_int, [vp, C.POINTER(SwsParams)]),
         "sws_residual": (C.c_int, [vp, dp, dp, vp]),
         "sws_jv_batch": (C.c_int, [vp, dp, dp, C.c_int32, dp, dp, dp, dp, vp]),
         "sws_jv_exact_batch": (C.c_int, [vp, dp, dp, C.c_int32, dp, vp]),

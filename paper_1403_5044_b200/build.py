@@ -13,6 +13,9 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libsws.so"
+LIB_JFNK = PKG / "libsws_jfnk.so"  # the Newton-Krylov driver: calls libsws through its C-ABI, + cuBLAS/cuSOLVER
+SOURCES_JFNK = ["jfnk_precond.cu", "jfnk_solver.cu"]
+CUDA_LIB64 = "/usr/local/cuda/lib64"
 SOURCES = ["sws_api.cu", "sws_fields.cu", "sws_allpairs.cu", "sws_allpairs_f32.cu", "sws_jv_exact.cu", "sws_probe.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
@@ -26,10 +29,12 @@ def _nvcc() -> str:
 
 
 def needs_build() -> bool:
-    if not LIB.exists():
+    if not LIB.exists() or not LIB_JFNK.exists():
         return True
-    t = LIB.stat().st_mtime
-    deps = [CSRC / s for s in SOURCES] + [CSRC / "sws_internal.cuh", CSRC / "sws_stage.cuh", ROOT / "include" / "sws.h"]
+    t = min(LIB.stat().st_mtime, LIB_JFNK.stat().st_mtime)
+    deps = [CSRC / s for s in SOURCES + SOURCES_JFNK] + [CSRC / "sws_internal.cuh", CSRC / "sws_stage.cuh",
+                                                         CSRC / "jfnk_internal.cuh", ROOT / "include" / "sws.h",
+                                                         ROOT / "include" / "sws_jfnk.h"]
     return any(d.stat().st_mtime > t for d in deps)
 
 
@@ -39,7 +44,14 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     cmd = [_nvcc(), *NVCC_FLAGS, f"-I{ROOT / 'include'}"]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += [str(CSRC / s) for s in SOURCES] + ["-o", str(LIB)]
+    cmd += [str(CSRC / s) for s in SOURCES] + ["-Xlinker", "-soname=libsws.so", "-o", str(LIB)]
+    subprocess.run(cmd, check=True)
+    cmd = [_nvcc(), *NVCC_FLAGS, f"-I{ROOT / 'include'}"]
+    if verbose:
+        cmd += ["-Xptxas", "-v"]
+    cmd += [str(CSRC / s) for s in SOURCES_JFNK] + [f"-L{PKG}", "-l:libsws.so", "-lcublas", "-lcusolver",
+                                                    "-Xlinker", "-rpath=$ORIGIN", "-Xlinker", f"-rpath={CUDA_LIB64}",
+                                                    "-Xlinker", "-soname=libsws_jfnk.so", "-o", str(LIB_JFNK)]
     subprocess.run(cmd, check=True)
     return LIB
 

@@ -1,0 +1,424 @@
+// Device-resident drivers of the Jacobian-free Newton-Krylov method (section 4.1
+// L205-229): right-preconditioned GMRES(m) on J(u) P^-1 (L209-215, Saad & Schultz [47]) and the
+// damped Newton iteration (2), (3) L41-45 with a backtracking line search (L209).
+//
+// Every vector (Krylov basis, residuals, corrections) lives on the device; per iteration the
+// host reads back only the new Hessenberg column and a norm (one synchronisation, next to a
+// Jacobian-vector product that costs milliseconds).  E(u) and J(u) v are libsws's, called
+// through its public C-ABI; P^-1 is jfnk_precond.cu.  Orthogonalisation is classical
+// Gram-Schmidt applied twice (two fused multi-dot + multi-axpy passes instead of j dependent
+// dot products), which spans the same Krylov space as the textbook modified Gram-Schmidt.
+// All reductions have a fixed order (per-CTA partials, then a serial sum): deterministic.
+#include <chrono>
+#include <cmath>
+#include <cstdio>
+#include <new>
+#include <vector>
+
+#include "jfnk_internal.cuh"
+
+namespace jfnk {
+
+__device__ __forceinline__ double block_sum(double v, double* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  const int w = threadIdx.x >> 5;
+  __syncthreads();  // red may still be read from the previous call
+  if ((threadIdx.x & 31) == 0) red[w] = v;
+  __syncthreads();
+  double s = 0.0;
+  if (threadIdx.x == 0)
+    for (int i = 0; i < kDotThreads / 32; ++i) s += red[i];
+  return s;
+}
+__device__ __forceinline__ double block_max(double v, double* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+  const int w = threadIdx.x >> 5;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) red[w] = v;
+  __syncthreads();
+  double s = 0.0;
+  if (threadIdx.x == 0)
+    for (int i = 0; i < kDotThreads / 32; ++i) s = fmax(s, red[i]);
+  return s;
+}
+
+// partial[blk][i] = sum over the CTA's slice of V_i . w, i < nv  (V_i = V + i ld)
+__global__ void __launch_bounds__(kDotThreads) k_dots(const double* __restrict__ V, size_t ld, int nv,
+                                                      const double* __restrict__ w, int n,
+                                                      double* __restrict__ partial) {
+  __shared__ double red[kDotThreads / 32];
+  for (int i = 0; i < nv; ++i) {
+    const double* v = V + (size_t)i * ld;
+    double a = 0.0;
+    for (int idx = blockIdx.x * kDotThreads + threadIdx.x; idx < n; idx += gridDim.x * kDotThreads)
+      a = fma(v[idx], w[idx], a);
+    const double s = block_sum(a, red);
+    if (threadIdx.x == 0) partial[(size_t)blockIdx.x * nv + i] = s;
+  }
+}
+
+// out[i] (+)= sum_blk partial[blk][i]
+__global__ void k_dots_finish(const double* __restrict__ partial, int nblk, int nv, double* out, int accumulate) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nv) return;
+  double s = 0.0;
+  for (int b = 0; b < nblk; ++b) s += partial[(size_t)b * nv + i];
+  out[i] = accumulate ? out[i] + s : s;
+}
+
+// w -= sum_i coef[i] V_i
+__global__ void __launch_bounds__(256) k_project(double* __restrict__ w, const double* __restrict__ V, size_t ld,
+                                                 int nv, const double* __restrict__ coef, int n) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n) return;
+  double a = w[idx];
+  for (int i = 0; i < nv; ++i) a = fma(-coef[i], V[(size_t)i * ld + idx], a);
+  w[idx] = a;
+}
+
+// out = sum_i coef[i] V_i
+__global__ void __launch_bounds__(256) k_lincomb(double* __restrict__ out, const double* __restrict__ V, size_t ld,
+                                                 int nv, const double* __restrict__ coef, int n) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n) return;
+  double a = 0.0;
+  for (int i = 0; i < nv; ++i) a = fma(coef[i], V[(size_t)i * ld + idx], a);
+  out[idx] = a;
+}
+
+// out = w / sqrt(*normsq)   (out unchanged when *normsq == 0: breakdown, handled by the host)
+__global__ void __launch_bounds__(256) k_normalise(double* __restrict__ out, const double* __restrict__ w,
+                                                   const double* __restrict__ normsq, int n) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n) return;
+  const double q = *normsq;
+  if (q > 0.0) out[idx] = w[idx] / sqrt(q);
+}
+
+// out = a x + b y
+__global__ void __launch_bounds__(256) k_axpby(double* __restrict__ out, double a, const double* __restrict__ x,
+                                               double b, const double* __restrict__ y, int n) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < n) out[idx] = a * x[idx] + b * y[idx];
+}
+
+// partial[blk] = {sum e^2, max |e|}
+__global__ void __launch_bounds__(kDotThreads) k_norms(const double* __restrict__ e, int n, double* __restrict__ partial) {
+  __shared__ double red[kDotThreads / 32];
+  double a = 0.0, mx = 0.0;
+  for (int idx = blockIdx.x * kDotThreads + threadIdx.x; idx < n; idx += gridDim.x * kDotThreads) {
+    const double v = e[idx];
+    a = fma(v, v, a);
+    mx = fmax(mx, fabs(v));
+  }
+  const double s = block_sum(a, red);
+  const double m = block_max(mx, red);
+  if (threadIdx.x == 0) {
+    partial[2 * blockIdx.x] = s;
+    partial[2 * blockIdx.x + 1] = m;
+  }
+}
+__global__ void k_norms_finish(const double* __restrict__ partial, int nblk, double* out) {
+  double s = 0.0, m = 0.0;
+  for (int b = 0; b < nblk; ++b) {
+    s += partial[2 * b];
+    m = fmax(m, partial[2 * b + 1]);
+  }
+  out[0] = s;
+  out[1] = m;
+}
+
+}  // namespace jfnk
+
+using namespace jfnk;
+
+struct sws_solver {
+  sws_ctx* ctx;
+  sws_precond* pc;
+  int device, n, m_max;
+  double* V;        // [m_max + 1][n] Krylov basis
+  double *w, *z, *t, *r;
+  double *E, *Et, *du, *ut, *rhs;
+  double* partial;  // [kDotBlocks][m_max + 2]
+  double* hdev;     // [2 (m_max + 1) + 2]: h1 | h2 | normsq, scratch
+  double* ydev;     // [m_max]
+  double* hpin;     // pinned host mirror of hdev
+  cudaEvent_t ev[4];
+  // accounting of the current driver call
+  int n_jv, n_pc, n_res;
+  double ms_jv, ms_pc, ms_res;
+};
+
+namespace {
+
+thread_local char g_err[256] = "";
+int fail_cuda(cudaError_t e, const char* where) {
+  snprintf(g_err, sizeof g_err, "%s: %s", where, cudaGetErrorString(e));
+  return SWS_ECUDA;
+}
+#define RC(call)                       \
+  do {                                 \
+    int rc_ = (call);                  \
+    if (rc_ != SWS_OK) return rc_;     \
+  } while (0)
+#define CU(call)                                        \
+  do {                                                  \
+    cudaError_t e_ = (call);                            \
+    if (e_ != cudaSuccess) return fail_cuda(e_, #call); \
+  } while (0)
+
+inline int nblk(int n) { return (n + 255) / 256; }
+
+// out = sum of squares and max of e, read back (synchronises)
+int norms(sws_solver* s, const double* e, double* l2, double* linf, cudaStream_t st) {
+  k_norms<<<kDotBlocks, kDotThreads, 0, st>>>(e, s->n, s->partial);
+  k_norms_finish<<<1, 1, 0, st>>>(s->partial, kDotBlocks, s->hdev);
+  CU(cudaMemcpyAsync(s->hpin, s->hdev, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  *l2 = std::sqrt(s->hpin[0]);
+  if (linf) *linf = s->hpin[1];
+  return SWS_OK;
+}
+
+int apply_pinv(sws_solver* s, const double* v, double* out, cudaStream_t st) {
+  if (!s->pc) {
+    CU(cudaMemcpyAsync(out, v, sizeof(double) * s->n, cudaMemcpyDeviceToDevice, st));
+    return SWS_OK;
+  }
+  ++s->n_pc;
+  return sws_precond_apply(s->pc, v, out, st);
+}
+
+int apply_jv(sws_solver* s, const double* u, const double* v, double* out, int mode, cudaStream_t st) {
+  ++s->n_jv;
+  if (mode == 1) return sws_jv_batch(s->ctx, u, v, 1, nullptr, out, nullptr, nullptr, st);
+  return sws_jv_exact_batch(s->ctx, u, v, 1, out, st);
+}
+
+int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opts* o, double* d,
+          sws_gmres_stats* stats, double* hist, cudaStream_t st) {
+  const int n = s->n, m = o->restart;
+  if (m < 1 || m > s->m_max || o->maxit < 1) return SWS_EINVAL;
+  const size_t ld = (size_t)n;
+  double bnorm = 0.0;
+  RC(norms(s, rhs, &bnorm, nullptr, st));
+  CU(cudaMemsetAsync(d, 0, sizeof(double) * n, st));
+  stats->its = 0; stats->converged = 0; stats->rel_res = 0.0; stats->rhs_norm = bnorm;
+  if (bnorm == 0.0) { stats->converged = 1; return SWS_OK; }
+  std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m), sn(m), g(m + 1), y(m);
+  auto Hm = [&](int i, int j) -> double& { return H[(size_t)i * m + j]; };
+  CU(cudaMemcpyAsync(s->r, rhs, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+  int its = 0;
+  double rel = 1.0;
+  double beta = bnorm;
+  bool first = true;
+  while (its < o->maxit) {
+    if (!first) RC(norms(s, s->r, &beta, nullptr, st));
+    first = false;
+    k_axpby<<<nblk(n), 256, 0, st>>>(s->V, 1.0 / beta, s->r, 0.0, s->r, n);
+    std::fill(g.begin(), g.end(), 0.0);
+    g[0] = beta;
+    int jd = 0;
+    for (int j = 0; j < m; ++j) {
+      const int nv = j + 1;
+      double* h1 = s->hdev;
+      double* h2 = s->hdev + (m + 1);
+      double* nq = s->hdev + 2 * (m + 1);
+      CU(cudaEventRecord(s->ev[0], st));
+      RC(apply_pinv(s, s->V + (size_t)j * ld, s->z, st));
+      CU(cudaEventRecord(s->ev[1], st));
+      RC(apply_jv(s, u, s->z, s->w, o->jv_mode, st));
+      CU(cudaEventRecord(s->ev[2], st));
+      ++its;
+      // classical Gram-Schmidt, twice
+      k_dots<<<kDotBlocks, kDotThreads, 0, st>>>(s->V, ld, nv, s->w, n, s->partial);
+      k_dots_finish<<<(nv + 127) / 128, 128, 0, st>>>(s->partial, kDotBlocks, nv, h1, 0);
+      k_project<<<nblk(n), 256, 0, st>>>(s->w, s->V, ld, nv, h1, n);
+      k_dots<<<kDotBlocks, kDotThreads, 0, st>>>(s->V, ld, nv, s->w, n, s->partial);
+      k_dots_finish<<<(nv + 127) / 128, 128, 0, st>>>(s->partial, kDotBlocks, nv, h2, 0);
+      k_project<<<nblk(n), 256, 0, st>>>(s->w, s->V, ld, nv, h2, n);
+      k_dots<<<kDotBlocks, kDotThreads, 0, st>>>(s->w, ld, 1, s->w, n, s->partial);
+      k_dots_finish<<<1, 128, 0, st>>>(s->partial, kDotBlocks, 1, nq, 0);
+      k_normalise<<<nblk(n), 256, 0, st>>>(s->V + (size_t)(j + 1) * ld, s->w, nq, n);
+      CU(cudaMemcpyAsync(s->hpin, s->hdev, sizeof(double) * (2 * (m + 1) + 1), cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+      {
+        float a = 0.f, b = 0.f;
+        cudaEventElapsedTime(&a, s->ev[0], s->ev[1]);
+        cudaEventElapsedTime(&b, s->ev[1], s->ev[2]);
+        s->ms_pc += a; s->ms_jv += b;
+      }
+      for (int i = 0; i <= j; ++i) Hm(i, j) = s->hpin[i] + s->hpin[(m + 1) + i];
+      Hm(j + 1, j) = std::sqrt(s->hpin[2 * (m + 1)]);
+      for (int i = 0; i < j; ++i) {
+        const double tmp = cs[i] * Hm(i, j) + sn[i] * Hm(i + 1, j);
+        Hm(i + 1, j) = -sn[i] * Hm(i, j) + cs[i] * Hm(i + 1, j);
+        Hm(i, j) = tmp;
+      }
+      const double rho = std::hypot(Hm(j, j), Hm(j + 1, j));
+      cs[j] = Hm(j, j) / rho; sn[j] = Hm(j + 1, j) / rho;
+      Hm(j, j) = rho; Hm(j + 1, j) = 0.0;
+      g[j + 1] = -sn[j] * g[j];
+      g[j] = cs[j] * g[j];
+      jd = j + 1;
+      rel = std::fabs(g[j + 1]) / bnorm;
+      if (hist) hist[its - 1] = rel;
+      if (std::fabs(g[j + 1]) <= o->tol * bnorm || its >= o->maxit) break;
+    }
+    // y = R^-1 g (back substitution), d += P^-1 (V y)
+    for (int i = jd - 1; i >= 0; --i) {
+      double acc = g[i];
+      for (int k = i + 1; k < jd; ++k) acc -= Hm(i, k) * y[k];
+      y[i] = acc / Hm(i, i);
+    }
+    CU(cudaMemcpyAsync(s->ydev, y.data(), sizeof(double) * jd, cudaMemcpyHostToDevice, st));
+    k_lincomb<<<nblk(n), 256, 0, st>>>(s->t, s->V, ld, jd, s->ydev, n);
+    RC(apply_pinv(s, s->t, s->z, st));
+    k_axpby<<<nblk(n), 256, 0, st>>>(d, 1.0, d, 1.0, s->z, n);
+    CU(cudaStreamSynchronize(st));  // y is host memory reused by the next cycle
+    if (rel <= o->tol || its >= o->maxit) break;
+    // restart: r = rhs - J d
+    RC(apply_jv(s, u, d, s->w, o->jv_mode, st));
+    k_axpby<<<nblk(n), 256, 0, st>>>(s->r, 1.0, rhs, -1.0, s->w, n);
+  }
+  stats->its = its;
+  stats->rel_res = rel;
+  stats->converged = rel <= o->tol ? 1 : 0;
+  CU(cudaGetLastError());
+  return SWS_OK;
+}
+
+int residual(sws_solver* s, const double* u, double* E, cudaStream_t st) {
+  ++s->n_res;
+  CU(cudaEventRecord(s->ev[0], st));
+  RC(sws_residual(s->ctx, u, E, st));
+  CU(cudaEventRecord(s->ev[1], st));
+  return SWS_OK;
+}
+void account_residual(sws_solver* s) {  // after a synchronise
+  float a = 0.f;
+  cudaEventElapsedTime(&a, s->ev[0], s->ev[1]);
+  s->ms_res += a;
+}
+void reset_accounting(sws_solver* s) {
+  s->n_jv = s->n_pc = s->n_res = 0;
+  s->ms_jv = s->ms_pc = s->ms_res = 0.0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* sws_solver_last_error(void) { return g_err; }
+
+int sws_solver_create(sws_ctx* ctx, sws_precond* pc, int32_t max_restart, sws_solver** out) {
+  if (!ctx || !out || max_restart < 1 || max_restart > 512) return SWS_EINVAL;
+  *out = nullptr;
+  sws_params p;
+  RC(sws_get_params(ctx, &p));
+  if (p.max_batch < 1) return SWS_EBATCH;
+  if (pc && (pc->lm.N != p.N || pc->lm.M != p.M || pc->device != p.device)) return SWS_EINVAL;
+  sws_solver* s = new (std::nothrow) sws_solver();
+  if (!s) return SWS_ENOMEM;
+  s->ctx = ctx; s->pc = pc; s->device = p.device;
+  s->n = (int)sws_num_unknowns(ctx);
+  s->m_max = max_restart;
+  reset_accounting(s);
+  const size_t n = (size_t)s->n;
+  double* base = nullptr;
+  const size_t vec = (size_t)(max_restart + 1) + 9;
+  cudaError_t e = cudaSetDevice(p.device);
+  if (e == cudaSuccess) e = cudaMalloc(&base, vec * n * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&s->partial, sizeof(double) * kDotBlocks * (max_restart + 2));
+  if (e == cudaSuccess) e = cudaMalloc(&s->hdev, sizeof(double) * (2 * (max_restart + 1) + 2));
+  if (e == cudaSuccess) e = cudaMalloc(&s->ydev, sizeof(double) * max_restart);
+  if (e == cudaSuccess) e = cudaMallocHost(&s->hpin, sizeof(double) * (2 * (max_restart + 1) + 2));
+  for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&s->ev[i]);
+  if (e != cudaSuccess) {
+    s->V = base;
+    sws_solver_destroy(s);
+    return e == cudaErrorMemoryAllocation ? SWS_ENOMEM : fail_cuda(e, "sws_solver_create");
+  }
+  s->V = base;
+  double* q = base + (size_t)(max_restart + 1) * n;
+  s->w = q; s->z = q + n; s->t = q + 2 * n; s->r = q + 3 * n;
+  s->E = q + 4 * n; s->Et = q + 5 * n; s->du = q + 6 * n; s->ut = q + 7 * n; s->rhs = q + 8 * n;
+  *out = s;
+  return SWS_OK;
+}
+
+int sws_solver_gmres(sws_solver* s, const double* u_dev, const double* rhs_dev, const sws_gmres_opts* opts,
+                     double* d_dev, sws_gmres_stats* stats, double* hist_host, void* cuda_stream) {
+  if (!s || !u_dev || !rhs_dev || !opts || !d_dev || !stats) return SWS_EINVAL;
+  CU(cudaSetDevice(s->device));
+  reset_accounting(s);
+  return gmres(s, u_dev, rhs_dev, opts, d_dev, stats, hist_host, (cudaStream_t)cuda_stream);
+}
+
+int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sws_newton_log* log, int32_t* nlog,
+                      sws_newton_stats* stats, void* cuda_stream) {
+  if (!s || !u_dev || !o || !log || !nlog || !stats) return SWS_EINVAL;
+  if (o->max_newton < 0 || o->max_halvings < 0) return SWS_EINVAL;
+  CU(cudaSetDevice(s->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const auto t0 = std::chrono::steady_clock::now();
+  reset_accounting(s);
+  const int n = s->n;
+  sws_gmres_opts go = o->gmres;
+  go.tol = o->eta;
+  int nl = 0, converged = 0, steps = 0;
+  double fn = 0.0, finf = 0.0;
+  RC(residual(s, u_dev, s->E, st));
+  RC(norms(s, s->E, &fn, &finf, st));
+  account_residual(s);
+  for (int it = 0; it < o->max_newton; ++it) {
+    if (finf <= o->ftol) { converged = 1; break; }
+    k_axpby<<<nblk(n), 256, 0, st>>>(s->rhs, -1.0, s->E, 0.0, s->E, n);
+    sws_gmres_stats gs;
+    RC(gmres(s, u_dev, s->rhs, &go, s->du, &gs, nullptr, st));
+    double lam = 1.0, fnt = 0.0, finft = 0.0;
+    bool ok = false;
+    for (int hv = 0; hv <= o->max_halvings; ++hv) {
+      k_axpby<<<nblk(n), 256, 0, st>>>(s->ut, 1.0, u_dev, lam, s->du, n);
+      RC(residual(s, s->ut, s->Et, st));
+      RC(norms(s, s->Et, &fnt, &finft, st));
+      account_residual(s);
+      if (fnt < (1.0 - o->alpha * lam) * fn) { ok = true; break; }
+      lam *= 0.5;
+    }
+    log[nl++] = sws_newton_log{it, gs.its, fn, finf, gs.rel_res, ok ? lam : 0.0};
+    if (!ok) break;
+    CU(cudaMemcpyAsync(u_dev, s->ut, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    CU(cudaMemcpyAsync(s->E, s->Et, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    fn = fnt; finf = finft;
+    ++steps;
+  }
+  if (finf <= o->ftol) converged = 1;
+  log[nl] = sws_newton_log{nl, 0, fn, finf, 0.0, 0.0};
+  ++nl;
+  CU(cudaStreamSynchronize(st));
+  *nlog = nl;
+  stats->steps = steps; stats->converged = converged;
+  stats->residual_evals = s->n_res; stats->jv_products = s->n_jv; stats->precond_applies = s->n_pc;
+  stats->ms_jv = s->ms_jv; stats->ms_precond = s->ms_pc; stats->ms_residual = s->ms_res;
+  stats->ms_total = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  return SWS_OK;
+}
+
+int sws_solver_destroy(sws_solver* s) {
+  if (!s) return SWS_OK;
+  cudaSetDevice(s->device);
+  if (s->V) cudaFree(s->V);
+  if (s->partial) cudaFree(s->partial);
+  if (s->hdev) cudaFree(s->hdev);
+  if (s->ydev) cudaFree(s->ydev);
+  if (s->hpin) cudaFreeHost(s->hpin);
+  for (int i = 0; i < 4; ++i)
+    if (s->ev[i]) cudaEventDestroy(s->ev[i]);
+  delete s;
+  return SWS_OK;
+}
+
+}  // extern "C"

@@ -213,6 +213,12 @@ size_t sws_num_unknowns(const sws_ctx* c) { return c ? (size_t)c->mesh.n : 0; }
 size_t sws_num_targets(const sws_ctx* c) { return c ? (size_t)c->mesh.T : 0; }
 size_t sws_num_sources(const sws_ctx* c) { return c ? (size_t)c->mesh.S : 0; }
 size_t sws_workspace_bytes(const sws_ctx* c) { return c ? c->ws_bytes : 0; }
+int sws_get_params(const sws_ctx* c, sws_params* out) {
+  if (!c || !out) return SWS_EINVAL;
+  *out = c->params;
+  return SWS_OK;
+}
+
 int sws_last_launch_count(const sws_ctx* c) { return c ? c->last_launches : 0; }
 
 int sws_set_tuning(sws_ctx* c, int32_t chunks) {

@@ -1,0 +1,224 @@
+"""GPU parity of libsws_jfnk (preconditioner, GMRES, Newton) against
+oracle/jfnk.py, through the C-ABI binding.  All tests here need a B200.
+
+Tolerances.  Assembled blocks: entry by entry, 1e-13 of the largest entry (same formulas, FP64,
+different rounding order).  P^-1 v: the Schur complement has condition number ~1e6 (its diagonal
+blocks carry the double-integration operator C A^-1 B), and the library applies explicit inverses
+of the diagonal blocks, so two correct solvers differ by ~cond * eps ~ 1e-10 relative; bar 1e-8.
+GMRES / Newton: iteration histories agree while they are far above that floor (1e-6 relative),
+converged roots agree to 1e-8 (the Newton stopping tolerance is 1e-10 on ||E||_inf).
+"""
+import numpy as np
+import pytest
+
+import oracle.jfnk as OJ
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mods():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test run without a CUDA device")
+    import paper_1403_5044_b200 as sws
+    import paper_1403_5044_b200.jfnk as jf
+    sws.load_library()
+    jf.load_jfnk()   # fails loudly if libsws_jfnk.so is missing
+    return sws, jf
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+SHAPES = [dict(N=9, M=5, h=0.5, x1=-2.0), dict(N=6, M=7, h=0.3, x1=-1.1), dict(N=14, M=4, h=0.25, x1=-3.0, y1=0.5)]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("bw", [1, 3, 0])
+def test_assembled_blocks(mods, oracle64, shape, bw):
+    """D blocks ((B.6) L498-501, rows E5/E6 L466-468) and Schur blocks D - C A^-1 B, every block in the band."""
+    sws, jf = mods
+    c = W.custom(**shape)
+    p = c.params()
+    n1, H, M = c.N + 1, (c.N + 1) * c.M, c.M
+    P = OJ.linear_jacobian(p, oracle64.box_integral)
+    A, B, C_, D = P[:H, :H], P[:H, H:], P[H:, :H], P[H:, H:]
+    S = D - C_ @ np.linalg.solve(A, B)
+    with jf.Preconditioner(p, bandwidth=bw, factorise=False) as pc:
+        hb = (pc.bandwidth - 1) // 2
+        assert pc.bandwidth == (bw if bw else 2 * M - 1)
+        for l in range(M):
+            for m in range(max(0, l - hb), min(M, l + hb + 1)):
+                ref = D[l * n1:(l + 1) * n1, m * n1:(m + 1) * n1]
+                got = pc.block(0, l, m)
+                assert np.abs(got - ref).max() <= 1e-13 * np.abs(D).max(), (l, m)
+                refS = S[l * n1:(l + 1) * n1, m * n1:(m + 1) * n1]
+                gotS = pc.block(1, l, m)
+                assert np.abs(gotS - refS).max() <= 1e-12 * np.abs(S).max(), (l, m)
+
+
+def _pinv_case(mods, oracle64, c, bw, seed=0, nvec=3, tol=1e-8):
+    sws, jf = mods
+    p = c.params()
+    P = OJ.band_truncate(OJ.linear_jacobian(p, oracle64.box_integral), p, bw if bw else 2 * c.M - 1)
+    rng = np.random.default_rng(seed)
+    with jf.Preconditioner(p, bandwidth=bw) as pc:
+        for _ in range(nvec):
+            v = rng.standard_normal(c.n)
+            ref = np.linalg.solve(P, v)
+            got = pc.apply(dev(v)).cpu().numpy()
+            assert np.abs(got - ref).max() <= tol * np.abs(ref).max()
+            # and it is a solve of the banded P itself
+            assert np.abs(P @ got - v).max() <= 1e-7 * np.abs(v).max()
+        # in place, deterministic
+        vd = dev(v)
+        r1 = pc.apply(vd).cpu().numpy()
+        pc.apply(vd, out=vd)
+        assert np.array_equal(vd.cpu().numpy(), r1)
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("bw", [1, 3, 5, 0])
+def test_precond_apply_small(mods, oracle64, shape, bw):
+    _pinv_case(mods, oracle64, W.custom(**shape), bw)
+
+
+@pytest.mark.parametrize("bw", [1, 7, 0])
+def test_precond_apply_cfg2(mods, oracle64, bw):
+    _pinv_case(mods, oracle64, W.CONFIGS[1], bw, nvec=2)
+
+
+def test_precond_matches_app_c_steps(mods, oracle64):
+    """The oracle's literal App. C block steps and the library agree (cfg1, b = 5)."""
+    sws, jf = mods
+    c = W.CONFIGS[0]
+    p = c.params()
+    P = OJ.band_truncate(OJ.linear_jacobian(p, oracle64.box_integral), p, 5)
+    v = np.random.default_rng(3).standard_normal(c.n)
+    ref = OJ.precond_solve_blocks(P, v)
+    with jf.Preconditioner(p, bandwidth=5) as pc:
+        got = pc.apply(dev(v)).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-8 * np.abs(ref).max()
+
+
+def test_error_codes(mods):
+    sws, jf = mods
+    c = W.CONFIGS[0]
+    with pytest.raises(sws.SwsError):
+        jf.Preconditioner(c.params(), bandwidth=4)
+    with sws.Context(c.params(), max_batch=0) as ctx:
+        with pytest.raises(sws.SwsError):
+            jf.Solver(ctx, None)
+    with jf.Preconditioner(c.params(), bandwidth=3, factorise=False) as pc:
+        import torch
+        with pytest.raises(sws.SwsError):
+            pc.apply(torch.zeros(c.n, dtype=torch.float64, device="cuda"))
+        with pytest.raises(sws.SwsError):
+            pc.block(0, 0, 5)     # outside the band
+
+
+# ---------------------------------------------------------------------------------------
+def _oracle_ops(oracle64, oracleC, p, P):
+    import scipy.linalg as sl
+    lu = sl.lu_factor(P)
+    return (lambda u: oracle64.residual(p, u), lambda u, v: oracleC.jv_exact(p, u, v), lambda v: sl.lu_solve(lu, v))
+
+
+@pytest.mark.parametrize("bw,restart", [(0, 30), (3, 30), (3, 4)])
+def test_gmres_parity_cfg1(mods, oracle64, oracleC, bw, restart):
+    """J(u) d = -E(u) at the seeded nonlinear state of cfg1: residual history and solution."""
+    sws, jf = mods
+    c = W.CONFIGS[0]
+    p = c.params()
+    u = W.state(c)
+    P = OJ.band_truncate(OJ.linear_jacobian(p, oracle64.box_integral), p, bw if bw else 2 * c.M - 1)
+    res, jv, pinv = _oracle_ops(oracle64, oracleC, p, P)
+    rhs = -res(u)
+    d_ref, h_ref = OJ.gmres_right(lambda v: jv(u, v), pinv, rhs, 1e-9, restart, 60)
+    with sws.Context(p, max_batch=1) as ctx, jf.Preconditioner(p, bandwidth=bw) as pc, jf.Solver(ctx, pc, 30) as s:
+        d, st, hist = s.gmres(dev(u), dev(rhs), tol=1e-9, restart=restart, maxit=60)
+        d = d.cpu().numpy()
+    assert st["converged"] and st["its"] == len(h_ref)
+    h_ref = np.array(h_ref)
+    big = h_ref > 1e-7
+    assert np.allclose(hist[big], h_ref[big], rtol=1e-5)
+    assert np.abs(d - d_ref).max() <= 1e-7 * np.abs(d_ref).max()
+    # it solves the system: the oracle's J applied to the library's d
+    assert np.linalg.norm(jv(u, d) - rhs) <= 5e-9 * np.linalg.norm(rhs)
+
+
+def test_gmres_unpreconditioned_and_fd(mods, oracle64, oracleC):
+    """No preconditioner (pc = NULL) and the finite-difference J v of eq. (25) (jv_mode 1)."""
+    sws, jf = mods
+    c = W.CONFIGS[0]
+    p = c.params()
+    u = W.state(c)
+    rhs = -oracle64.residual(p, u)
+    jv = lambda v: oracleC.jv_exact(p, u, v)
+    d_ref, h_ref = OJ.gmres_right(jv, lambda v: v, rhs, 1e-30, 20, 20)
+    with sws.Context(p, max_batch=1) as ctx, jf.Solver(ctx, None, 20) as s:
+        d, st, hist = s.gmres(dev(u), dev(rhs), tol=1e-30, restart=20, maxit=20)
+        assert st["its"] == 20 and not st["converged"]
+        assert np.allclose(hist, np.array(h_ref), rtol=1e-5)
+        d2, st2, hist2 = s.gmres(dev(u), dev(rhs), tol=1e-30, restart=20, maxit=20, jv_mode=1)
+        assert np.allclose(hist2, np.array(h_ref), rtol=1e-3)     # first-order difference quotient
+        # zero right-hand side
+        import torch
+        d0, st0, _ = s.gmres(dev(u), torch.zeros_like(dev(u)), tol=1e-8, maxit=5)
+        assert st0["converged"] and st0["its"] == 0 and not d0.cpu().numpy().any()
+    assert np.abs(d.cpu().numpy() - d_ref).max() <= 1e-6 * np.abs(d_ref).max()
+
+
+@pytest.mark.parametrize("bw", [0, 3])
+def test_newton_parity_cfg1_mesh(mods, oracle64, oracleC, bw):
+    """The whole JFNK solve on the 31x11 mesh from the flat guess (L227), eps = 1, F = 0.7: same
+    Newton history and the same root as the oracle's driver."""
+    sws, jf = mods
+    c = W.custom(31, 11, 0.8, -8.0, eps=1.0)
+    p = c.params()
+    P = OJ.band_truncate(OJ.linear_jacobian(p, oracle64.box_integral), p, bw if bw else 2 * c.M - 1)
+    res, jv, pinv = _oracle_ops(oracle64, oracleC, p, P)
+    u0 = W.flat_state(c)
+    kw = dict(ftol=1e-10, eta=1e-3, restart=30, gmres_maxit=60)
+    u_ref, log_ref = OJ.newton(res, jv, pinv, u0, **kw)
+    with sws.Context(p, max_batch=1) as ctx, jf.Preconditioner(p, bandwidth=bw) as pc, jf.Solver(ctx, pc, 30) as s:
+        u, log, st = s.newton(dev(u0), **kw)
+        u = u.cpu().numpy()
+    assert st["converged"] and log_ref[-1]["finf"] <= 1e-10
+    assert len(log) == len(log_ref)
+    for a, b in zip(log, log_ref):
+        assert a["gmres_its"] == b["gmres_its"] and a["lambda"] == b["lambda"]
+        if b["fnorm"] > 1e-6:
+            assert a["fnorm"] == pytest.approx(b["fnorm"], rel=1e-6)
+    assert np.abs(u - u_ref).max() <= 1e-8
+    assert np.abs(oracle64.residual(p, u)).max() <= 2e-10     # a root for the oracle too
+    assert st["jv_products"] == sum(e["gmres_its"] for e in log)
+    assert st["residual_evals"] == 1 + st["steps"]
+
+
+def test_newton_paper_mesh_91x31(mods, oracle64):
+    """The paper's 'contemporary' mesh (91 x 31, dx = dy = 0.3, x0 = -9, eps = 1, F = 0.7; L259):
+    converges from the flat guess with the block-banded preconditioner; the root satisfies the
+    ORACLE's residual; the finite-difference Jacobian action of eq. (25) reaches the same root."""
+    sws, jf = mods
+    c = W.custom(91, 31, 0.3, -9.0, eps=1.0)
+    p = c.params()
+    u0 = dev(W.flat_state(c))
+    with sws.Context(p, max_batch=1) as ctx, jf.Preconditioner(p, bandwidth=7) as pc, jf.Solver(ctx, pc, 40) as s:
+        u, log, st = s.newton(u0, ftol=1e-10, eta=1e-3, restart=40, gmres_maxit=80)
+        assert st["converged"] and st["steps"] <= 8
+        assert max(e["gmres_its"] for e in log) <= 30
+        un = u.cpu().numpy()
+        assert np.abs(oracle64.residual(p, un)).max() <= 1e-9
+        u2, log2, st2 = s.newton(u0, ftol=1e-8, eta=1e-3, restart=40, gmres_maxit=80, jv_mode=1)
+        assert st2["converged"]
+        assert np.abs(u2.cpu().numpy() - un).max() <= 1e-6
+        # deterministic
+        u3, _, _ = s.newton(u0, ftol=1e-10, eta=1e-3, restart=40, gmres_maxit=80)
+        assert np.array_equal(u3.cpu().numpy(), un)
+    zeta_x = un[c.n // 2:].reshape(c.M, c.N + 1)[:, 1:]
+    assert np.abs(zeta_x).max() > 0.05      # a real wave pattern, not the flat state
