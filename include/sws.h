@@ -55,6 +55,7 @@ extern "C" {
 #define SWS_ENOMEM (-2) /* device or host allocation failed                             */
 #define SWS_ECUDA (-3)  /* a CUDA runtime call failed; see sws_last_cuda_error()         */
 #define SWS_EBATCH (-4) /* b < 1 or b > max_batch                                        */
+#define SWS_ESTATE (-5) /* sws_jv_apply without a valid sws_linearize                    */
 
 typedef struct sws_ctx sws_ctx; /* opaque, owned by the library */
 
@@ -98,6 +99,19 @@ int sws_jv_batch(sws_ctx* ctx, const double* u_dev, const double* V_dev, int32_t
  * V_dev [b][n] row-major, 1 <= b <= max_batch.  Deterministic.  E(u) itself is not formed. */
 int sws_jv_exact_batch(sws_ctx* ctx, const double* u_dev, const double* V_dev, int32_t b,
                        double* JV_dev, void* cuda_stream);
+
+/* The same action split for Newton-Krylov use, where many products share one u:
+ *   sws_linearize(u)      forms everything that depends on u alone (base fields, starred values,
+ *                         the closed form I and its A, B, C derivatives, and the six
+ *                         direction-independent all-pairs sums) and keeps it in the context;
+ *   sws_jv_apply(V[b])    JV_dev[b][n] = J(u) v_b for that u: (41 + 4 b) FP64 instructions per pair
+ *                         (b = 1: the cost of one residual evaluation, with no shift and no
+ *                         cancellation).
+ * The linearisation stays valid until the next sws_residual / sws_jv_batch / sws_jv_exact_batch /
+ * sws_linearize on the same context; sws_jv_apply returns SWS_ESTATE otherwise.  Results agree with
+ * sws_jv_exact_batch to summation round-off (the column split of the quadrature differs). */
+int sws_linearize(sws_ctx* ctx, const double* u_dev, void* cuda_stream);
+int sws_jv_apply(sws_ctx* ctx, const double* V_dev, int32_t b, double* JV_dev, void* cuda_stream);
 
 /* The same two calls on HOST buffers: host->device copy, compute, device->host copy,
  * then a stream synchronise.  `cuda_stream` as above. */

@@ -16,7 +16,7 @@ import numpy as np
 _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libsws.so"
 
-SWS_OK, SWS_EINVAL, SWS_ENOMEM, SWS_ECUDA, SWS_EBATCH = 0, -1, -2, -3, -4
+SWS_OK, SWS_EINVAL, SWS_ENOMEM, SWS_ECUDA, SWS_EBATCH, SWS_ESTATE = 0, -1, -2, -3, -4, -5
 
 # every symbol include/sws.h declares
 SYMBOLS = (
@@ -26,7 +26,7 @@ SYMBOLS = (
     "sws_plan_info", "sws_set_profiling", "sws_profile_read", "sws_destroy", "sws_strerror", "sws_last_cuda_error",
     "sws_probe_fp64_peak", "sws_debug_rsqrt_host",
     "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
-    "sws_get_params",
+    "sws_get_params", "sws_linearize", "sws_jv_apply",
 )
 
 
@@ -58,6 +58,8 @@ def load_library() -> C.CDLL:
     proto = {
         "sws_setup": (C.c_int, [C.POINTER(SwsParams), C.POINTER(vp)]),
         "sws_get_params": (C.c_int, [vp, C.POINTER(SwsParams)]),
+        "sws_linearize": (C.c_int, [vp, dp, vp]),
+        "sws_jv_apply": (C.c_int, [vp, dp, C.c_int32, dp, vp]),
         "sws_residual": (C.c_int, [vp, dp, dp, vp]),
         "sws_jv_batch": (C.c_int, [vp, dp, dp, C.c_int32, dp, dp, dp, dp, vp]),
         "sws_jv_exact_batch": (C.c_int, [vp, dp, dp, C.c_int32, dp, vp]),
@@ -204,6 +206,20 @@ class Context:
                                            self._dev(JV, (b, self.n), "JV"), self._stream(stream)),
                "sws_jv_exact_batch")
         return JV
+
+    def linearize(self, u, stream=None) -> None:
+        """sws_linearize: form and keep everything of J(u) that depends on u alone."""
+        _check(self.lib.sws_linearize(self._h, self._dev(u, (self.n,), "u"), self._stream(stream)), "sws_linearize")
+
+    def jv_apply(self, V, out=None, stream=None):
+        """sws_jv_apply: J(u) v_b for the u of the last linearize(); V [b, n] or [n]."""
+        single = V.dim() == 1
+        V2 = V.reshape(1, -1) if single else V
+        b = int(V2.shape[0])
+        JV = self._new(b, self.n) if out is None else out.reshape(b, -1)
+        _check(self.lib.sws_jv_apply(self._h, self._dev(V2, (b, self.n), "V"), b,
+                                     self._dev(JV, (b, self.n), "out"), self._stream(stream)), "sws_jv_apply")
+        return JV[0] if single else JV
 
     def jv_exact_batch_host(self, u: np.ndarray, V: np.ndarray, out=None, stream=None) -> np.ndarray:
         """The same on HOST buffers (sws_jv_exact_batch_host): H2D, compute, D2H, synchronise."""

@@ -194,7 +194,7 @@ int apply_pinv(sws_solver* s, const double* v, double* out, cudaStream_t st) {
 int apply_jv(sws_solver* s, const double* u, const double* v, double* out, int mode, cudaStream_t st) {
   ++s->n_jv;
   if (mode == 1) return sws_jv_batch(s->ctx, u, v, 1, nullptr, out, nullptr, nullptr, st);
-  return sws_jv_exact_batch(s->ctx, u, v, 1, out, st);
+  return sws_jv_apply(s->ctx, v, 1, out, st);  // the linearisation at u was formed by gmres()
 }
 
 int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opts* o, double* d,
@@ -207,6 +207,15 @@ int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opt
   CU(cudaMemsetAsync(d, 0, sizeof(double) * n, st));
   stats->its = 0; stats->converged = 0; stats->rel_res = 0.0; stats->rhs_norm = bnorm;
   if (bnorm == 0.0) { stats->converged = 1; return SWS_OK; }
+  if (o->jv_mode == 0) {  // linearise once per solve: everything of J(u) that depends on u alone
+    CU(cudaEventRecord(s->ev[0], st));
+    RC(sws_linearize(s->ctx, u, st));
+    CU(cudaEventRecord(s->ev[1], st));
+    CU(cudaStreamSynchronize(st));
+    float a = 0.f;
+    cudaEventElapsedTime(&a, s->ev[0], s->ev[1]);
+    s->ms_jv += a;
+  }
   std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m), sn(m), g(m + 1), y(m);
   auto Hm = [&](int i, int j) -> double& { return H[(size_t)i * m + j]; };
   CU(cudaMemcpyAsync(s->r, rhs, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));

@@ -42,7 +42,7 @@ static cudaError_t dev_alloc(T** p, size_t count, size_t* total) {
 static void free_all(sws_ctx* c) {
   void* ptrs[] = {c->x, c->y, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zx, c->px, c->zy, c->py,
                   c->src, c->srcf, c->tgt, c->e2loc, c->part, c->F0, c->Fpert, c->sigma, c->norm_part,
-                  c->dsrc, c->dtgt, c->e2lin, c->tgtI,
+                  c->dsrc, c->dtgt, c->e2lin, c->tgtI, c->lin_sums,
                   c->u_stage, c->V_stage, c->out_stage};
   for (void* p : ptrs)
     if (p) cudaFree(p);
@@ -63,6 +63,7 @@ const char* sws_strerror(int code) {
     case SWS_ENOMEM: return "out of memory";
     case SWS_ECUDA: return "CUDA runtime error (see sws_last_cuda_error)";
     case SWS_EBATCH: return "batch size out of range";
+    case SWS_ESTATE: return "no valid linearisation (call sws_linearize first)";
     default: return "unknown error";
   }
 }
@@ -154,6 +155,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
     ALLOC(dtgt, mb * T);
     ALLOC(e2lin, mb * T);
     ALLOC(tgtI, T);
+    ALLOC(lin_sums, 6 * T);
   }
 #undef ALLOC
   if (!ok) {
@@ -262,6 +264,7 @@ static int run_states(sws_ctx* c, const double* u, const double* V, int states, 
   *launches += 5;
   c->last_states = states;
   c->last_lin_b = 0;
+  c->lin_valid = 0;
   return SWS_OK;
 }
 
@@ -305,7 +308,7 @@ int sws_jv_exact_batch(sws_ctx* c, const double* u_dev, const double* V_dev, int
   CK(cudaSetDevice(c->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
-  const sws::PairPlan plan = sws::make_lin_plan(c, BT, groups);
+  const sws::PairPlan plan = sws::make_lin_plan(c, BT, groups, 0);
   // derivative fields of every direction (states 1..b) beside the base fields (state 0);
   // the derivative radiation rows go straight to JV, the base rows to scratch
   CK(sws::launch_reconstruct(c, u_dev, V_dev, b + 1, 1, c->F0, JV_dev, st));
@@ -315,12 +318,62 @@ int sws_jv_exact_batch(sws_ctx* c, const double* u_dev, const double* V_dev, int
   cudaEvent_t pe0 = nullptr, pe1 = nullptr;
   int rc = prof_begin(c, st, &pe0, &pe1);
   if (rc != SWS_OK) return rc;
-  CK(sws::launch_allpairs_lin(c, BT, groups, plan, st));
+  CK(sws::launch_allpairs_lin(c, BT, groups, 0, plan, st));
   if (pe1) CK(cudaEventRecord(pe1, st));
-  CK(sws::launch_assemble_lin(c, b, BT, plan, JV_dev, st));
+  CK(sws::launch_assemble_lin(c, b, BT, 0, plan, JV_dev, st));
   c->last_launches = 6;
   c->last_states = 1;
   c->last_lin_b = b;
+  c->lin_valid = 0;  // the base planes now describe this u, but lin_sums does not
+  return SWS_OK;
+}
+
+// Linearise once, apply many times (the shape of a Newton-Krylov step): everything that depends
+// on u alone - base fields, starred values, {I, dI/dA, dI/dB, dI/dC}, and the six
+// direction-independent all-pairs sums - is formed here and kept until the next call that
+// overwrites the base state.
+int sws_linearize(sws_ctx* c, const double* u_dev, void* cuda_stream) {
+  if (!c || !u_dev) return SWS_EINVAL;
+  if (c->params.max_batch < 1) return SWS_EBATCH;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const sws::PairPlan plan = sws::make_lin_plan(c, 1, 1, 1);
+  CK(sws::launch_reconstruct(c, u_dev, nullptr, 1, 1, c->F0, nullptr, st));
+  CK(sws::launch_dy(c, 1, st));
+  CK(sws::launch_targets(c, 1, c->F0, nullptr, c->tgtI, st));
+  cudaEvent_t pe0 = nullptr, pe1 = nullptr;
+  int rc = prof_begin(c, st, &pe0, &pe1);
+  if (rc != SWS_OK) return rc;
+  CK(sws::launch_allpairs_lin(c, 1, 1, 1, plan, st));
+  if (pe1) CK(cudaEventRecord(pe1, st));
+  CK(sws::launch_reduce_base(c, plan, st));
+  c->last_launches = 5;
+  c->last_states = 1;
+  c->last_lin_b = 0;
+  c->lin_valid = 1;
+  return SWS_OK;
+}
+
+int sws_jv_apply(sws_ctx* c, const double* V_dev, int32_t b, double* JV_dev, void* cuda_stream) {
+  if (!c || !V_dev || !JV_dev) return SWS_EINVAL;
+  if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
+  if (!c->lin_valid) return SWS_ESTATE;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
+  const sws::PairPlan plan = sws::make_lin_plan(c, BT, groups, 2);
+  // directions only: states 1..b of the planes; the base state (state 0) stays as linearised
+  CK(sws::launch_reconstruct(c, nullptr, V_dev, b + 1, 1, c->F0, JV_dev, st, 1));
+  CK(sws::launch_dy(c, b + 1, st, 1));
+  CK(sws::launch_targets_lin(c, b, BT, JV_dev, st));
+  cudaEvent_t pe0 = nullptr, pe1 = nullptr;
+  int rc = prof_begin(c, st, &pe0, &pe1);
+  if (rc != SWS_OK) return rc;
+  CK(sws::launch_allpairs_lin(c, BT, groups, 2, plan, st));
+  if (pe1) CK(cudaEventRecord(pe1, st));
+  CK(sws::launch_assemble_lin(c, b, BT, 2, plan, JV_dev, st));
+  c->last_launches = 5;
+  c->last_lin_b = -b;  // direction fields of an apply (sws_time_allpairs_lin replays mode 2)
   return SWS_OK;
 }
 
@@ -342,14 +395,15 @@ int sws_jv_exact_batch_host(sws_ctx* c, const double* u_host, const double* V_ho
 
 int sws_time_allpairs_lin(sws_ctx* c, int32_t reps, float* ms_per_launch, void* cuda_stream) {
   if (!c || !ms_per_launch || reps < 1) return SWS_EINVAL;
-  if (c->last_lin_b < 1) return SWS_EBATCH;  // needs the fields of a previous sws_jv_exact_batch
+  if (c->last_lin_b == 0) return SWS_EBATCH;  // needs the fields of a previous sws_jv_exact_batch / sws_jv_apply
   CK(cudaSetDevice(c->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const int b = c->last_lin_b, BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
-  const sws::PairPlan plan = sws::make_lin_plan(c, BT, groups);
-  CK(sws::launch_allpairs_lin(c, BT, groups, plan, st));
+  const int mode = c->last_lin_b < 0 ? 2 : 0;
+  const int b = c->last_lin_b < 0 ? -c->last_lin_b : c->last_lin_b, BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
+  const sws::PairPlan plan = sws::make_lin_plan(c, BT, groups, mode);
+  CK(sws::launch_allpairs_lin(c, BT, groups, mode, plan, st));
   CK(cudaEventRecord(c->ev0, st));
-  for (int r = 0; r < reps; ++r) CK(sws::launch_allpairs_lin(c, BT, groups, plan, st));
+  for (int r = 0; r < reps; ++r) CK(sws::launch_allpairs_lin(c, BT, groups, mode, plan, st));
   CK(cudaEventRecord(c->ev1, st));
   CK(cudaEventSynchronize(c->ev1));
   float ms = 0.f;
@@ -362,7 +416,7 @@ int sws_lin_plan_info(sws_ctx* c, int32_t b, int32_t* out6) {
   if (!c || !out6) return SWS_EINVAL;
   if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
   const int BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
-  const sws::PairPlan p = sws::make_lin_plan(c, BT, groups);
+  const sws::PairPlan p = sws::make_lin_plan(c, BT, groups, 0);
   out6[0] = p.tiles; out6[1] = p.chunks; out6[2] = p.cols_per_chunk; out6[3] = p.seg_len; out6[4] = p.nseg;
   out6[5] = BT;
   return SWS_OK;

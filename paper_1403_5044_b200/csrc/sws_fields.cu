@@ -29,10 +29,10 @@ __device__ __forceinline__ double* state_out(double* F0, double* Fpert, int stat
 __global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ u,
                                                      const double* __restrict__ V,
                                                      const double* __restrict__ sigma, Mesh m,
-                                                     int lin, double* zeta, double* phi, double* zx,
+                                                     int lin, int first, double* zeta, double* phi, double* zx,
                                                      double* px, double* F0, double* Fpert) {
   extern __shared__ double sm[];
-  const int N = m.N, l = blockIdx.x, state = blockIdx.y, tid = threadIdx.x;
+  const int N = m.N, l = blockIdx.x, state = blockIdx.y + first, tid = threadIdx.x;
   double* s_zx = sm;
   double* s_px = sm + N;
   double* s_z = sm + 2 * (size_t)N;
@@ -106,12 +106,12 @@ __global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ 
 //             2 m_{M-1} + m_M = (d_{M-2} + 5 d_{M-1})/2
 // solved by the Thomas recurrences with the data-independent factors cp[], inv[] made in
 // sws_setup.  The output plane is used as the forward-sweep scratch.
-__global__ void __launch_bounds__(128) k_dy(Mesh m, const double* __restrict__ cp,
+__global__ void __launch_bounds__(128) k_dy(Mesh m, int first, const double* __restrict__ cp,
                                             const double* __restrict__ inv, const double* zeta,
                                             const double* phi, double* zy, double* py) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= m.N) return;
-  const int N = m.N, M = m.M, state = blockIdx.z;
+  const int N = m.N, M = m.M, state = blockIdx.z + first;
   const size_t base = (size_t)state * m.S + k;
   const double* f = (blockIdx.y == 0 ? zeta : phi) + base;
   double* out = (blockIdx.y == 0 ? zy : py) + base;
@@ -366,18 +366,18 @@ cudaError_t fields_configure(const sws_ctx* c) {
 }
 
 cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states, int lin,
-                               double* F0, double* Fpert, cudaStream_t st) {
+                               double* F0, double* Fpert, cudaStream_t st, int first) {
   const Mesh& m = c->mesh;
-  dim3 grid(m.M, states);
-  k_reconstruct<<<grid, 256, reconstruct_smem_bytes(m.N), st>>>(u, V, c->sigma, m, lin, c->zeta, c->phi,
+  dim3 grid(m.M, states - first);
+  k_reconstruct<<<grid, 256, reconstruct_smem_bytes(m.N), st>>>(u, V, c->sigma, m, lin, first, c->zeta, c->phi,
                                                                  c->zx, c->px, F0, Fpert);
   return cudaGetLastError();
 }
 
-cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st) {
+cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st, int first) {
   const Mesh& m = c->mesh;
-  dim3 grid((m.N + 127) / 128, 2, states);
-  k_dy<<<grid, 128, 0, st>>>(m, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zy, c->py);
+  dim3 grid((m.N + 127) / 128, 2, states - first);
+  k_dy<<<grid, 128, 0, st>>>(m, first, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zy, c->py);
   return cudaGetLastError();
 }
 

@@ -106,7 +106,11 @@ struct sws_ctx {
   sws::DTgtRec* dtgt;     // [direction][t]
   double* e2lin;          // [direction][t] local part of the derivative of E2
   double4* tgtI;          // [t] {I, dI/dA, dI/dB, dI/dC} of the base state
-  int lin_occ[4];         // resident CTAs per SM of k_allpairs_lin<1,4,8,16>
+  int lin_occ[4];         // resident CTAs per SM of k_allpairs_lin<1,4,8,16> (fused)
+  int lin_occ2[4];        // the same for the directions-only kernels (sws_jv_apply)
+  int lin_occ1;           // the base-sums kernel (sws_linearize)
+  double* lin_sums;       // [6][t] direction-independent sums of the linearisation at lin_u
+  int lin_valid;          // the base fields, tgtI and lin_sums describe the u of the last sws_linearize
 
   double* F0;         // [n] base residual of a batch when the caller passes no F0_dev
   double* Fpert;      // [max_batch][n] when the caller passes no Fpert_dev
@@ -127,9 +131,10 @@ namespace sws {
 // Launches (all asynchronous on `st`); each returns the cudaError_t of its launch.
 // states = 1: base state only.  State s >= 1 is u + sigma[s-1] * V[s-1].
 // lin != 0: states >= 1 are the directions v themselves (derivative fields, homogeneous rows)
+// first: the first state processed (states first..states-1); sws_jv_apply skips the base state
 cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states, int lin,
-                               double* F0, double* Fpert, cudaStream_t st);
-cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st);
+                               double* F0, double* Fpert, cudaStream_t st, int first = 0);
+cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st, int first = 0);
 // tgtI != NULL: base state of the analytic Jacobian action ({I, I_A, I_B, I_C} instead of e2loc)
 cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, double4* tgtI,
                            cudaStream_t st);
@@ -145,10 +150,13 @@ cudaError_t launch_jv_quotient(sws_ctx* c, const double* F0, const double* Fpert
 // analytic Jacobian action (sws_jv_exact.cu); BT = directions per tile (1, 4, 8 or 16)
 int lin_tile(int b);
 cudaError_t lin_configure(sws_ctx* c);
-PairPlan make_lin_plan(const sws_ctx* c, int BT, int groups);
+// mode 0: fused kernel (sws_jv_exact_batch); 1: direction-independent sums (sws_linearize);
+// 2: direction sums only (sws_jv_apply)
+PairPlan make_lin_plan(const sws_ctx* c, int BT, int groups, int mode);
 cudaError_t launch_targets_lin(sws_ctx* c, int b, int BT, double* JV, cudaStream_t st);
-cudaError_t launch_allpairs_lin(sws_ctx* c, int BT, int groups, const PairPlan& plan, cudaStream_t st);
-cudaError_t launch_assemble_lin(sws_ctx* c, int b, int BT, const PairPlan& plan, double* JV,
+cudaError_t launch_allpairs_lin(sws_ctx* c, int BT, int groups, int mode, const PairPlan& plan, cudaStream_t st);
+cudaError_t launch_reduce_base(sws_ctx* c, const PairPlan& plan, cudaStream_t st);
+cudaError_t launch_assemble_lin(sws_ctx* c, int b, int BT, int mode, const PairPlan& plan, double* JV,
                                 cudaStream_t st);
 
 PairPlan make_plan(const sws_ctx* c);

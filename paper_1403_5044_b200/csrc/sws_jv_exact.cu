@@ -145,7 +145,10 @@ struct LinS {  // direction-independent sums of one thread
   double u3, u3y, u3yy;  // per column: sum_j w (u-^3 + u+^3), (d- u-^3 - d+ u+^3), (d-^2 u-^3 + d+^2 u+^3)
 };
 
-template <int BT, bool SCALE>
+// MODE 0: everything (sws_jv_exact_batch).  MODE 1: the direction-independent sums only
+// (sws_linearize: they depend on u alone, so a Newton step forms them once).  MODE 2: the
+// direction sums only (sws_jv_apply): no S2, 41 + 4 BT FP64 instructions per pair.
+template <int BT, bool SCALE, int MODE>
 __device__ __forceinline__ void pair_lin(const double2 zp, const double2 sl, const double yj,
                                          const double4* __restrict__ dv, const double wgt,
                                          const LinT& t, const LinC& c, LinS& s, double (&acc)[BT]) {
@@ -169,22 +172,25 @@ __device__ __forceinline__ void pair_lin(const double2 zp, const double2 sl, con
   double cz = fma(-3.0, t3, R3 * t1);
   double czx = fma(-c.dx, dpsi * R3, K2);
   double czy = dpsi * D3;  // applied to the stored -d zeta_y
-  // S2 and its A, B, C sensitivities
-  const double sm = yj - c.c, sp = yj + c.c;
-  double um = rsqrt_l(fma(sm, sm, c.g)), up = rsqrt_l(fma(sp, sp, c.g));
-  double um3 = (um * um) * um, up3 = (up * up) * up;
   if (SCALE) {  // trapezoid half weights on the first/last row and column (Q4)
     K1 *= wgt; cz *= wgt; czx *= wgt; czy *= wgt;
-    um *= wgt; up *= wgt; um3 *= wgt; up3 *= wgt;
   }
-  s.cpsi += K1;
-  s.cz += cz;
-  s.s0 += um + up;
-  s.u3 += um3 + up3;
-  const double vm = dm * um3, vp = dp * up3;
-  s.u3y += vm - vp;
-  s.u3yy = fma(dm, vm, s.u3yy);
-  s.u3yy = fma(dp, vp, s.u3yy);
+  if (MODE != 2) {
+    // S2 and its A, B, C sensitivities
+    const double sm = yj - c.c, sp = yj + c.c;
+    double um = rsqrt_l(fma(sm, sm, c.g)), up = rsqrt_l(fma(sp, sp, c.g));
+    double um3 = (um * um) * um, up3 = (up * up) * up;
+    if (SCALE) { um *= wgt; up *= wgt; um3 *= wgt; up3 *= wgt; }
+    s.cpsi += K1;
+    s.cz += cz;
+    s.s0 += um + up;
+    s.u3 += um3 + up3;
+    const double vm = dm * um3, vp = dp * up3;
+    s.u3y += vm - vp;
+    s.u3yy = fma(dm, vm, s.u3yy);
+    s.u3yy = fma(dp, vp, s.u3yy);
+  }
+  if (MODE == 1) return;
   // Coefficient-major order: runs of BT DFMAs that share one coefficient register in the same
   // operand slot (the operand-reuse cache then leaves two fresh 64-bit register reads per DFMA,
   // which is what the FP64 pipe can be fed at full rate).
@@ -236,13 +242,15 @@ struct LinArgs {
 constexpr int kLinUnroll = SWS_LIN_UNROLL;
 constexpr int kLinShared = 6;  // direction-independent sums per (chunk, target)
 
-template <int BT>
+template <int BT, int MODE>
 __global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT >= 8 ? 3 : 4)) k_allpairs_lin(const LinArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int DV = MODE == 1 ? 0 : BT;          // direction records staged per node
+  constexpr int NSH = MODE == 2 ? 0 : kLinShared; // direction-independent sums written
   const int seg_pad = a.seg_len;  // even
   SrcRec* s_rec = reinterpret_cast<SrcRec*>(smem_raw);                          // [kStages][seg]
-  double4* s_dv = reinterpret_cast<double4*>(s_rec + (size_t)kStages * seg_pad);  // [kStages][seg][BT]
-  double* s_y = reinterpret_cast<double*>(s_dv + (size_t)kStages * seg_pad * BT);  // [kStages][seg]
+  double4* s_dv = reinterpret_cast<double4*>(s_rec + (size_t)kStages * seg_pad);  // [kStages][seg][DV]
+  double* s_y = reinterpret_cast<double*>(s_dv + (size_t)kStages * seg_pad * DV);  // [kStages][seg]
   uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_y + (size_t)kStages * seg_pad);
 
   const int tid = threadIdx.x;
@@ -260,6 +268,7 @@ __global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT 
   const int c1 = min(a.N, c0 + a.cols_per_chunk);
   const int nitems = (c1 - c0) * a.nseg;
   const double4* dsrc = a.dsrc + (size_t)group * a.N * a.M * BT;
+  (void)dsrc;
 
   if (tid == 0) {
     for (int s = 0; s < kStages; ++s) mbar_init(&s_bar[s], 1);
@@ -272,11 +281,12 @@ __global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT 
     const int i = c0 + q / a.nseg, j0 = (q % a.nseg) * a.seg_len;
     const int len = min(a.seg_len, a.M - j0);
     const uint32_t rec_bytes = (uint32_t)len * (uint32_t)sizeof(SrcRec);
-    const uint32_t dv_bytes = (uint32_t)len * (uint32_t)(BT * sizeof(double4));
+    const uint32_t dv_bytes = (uint32_t)len * (uint32_t)(DV * sizeof(double4));
     const uint32_t y_bytes = (uint32_t)((len + 1) & ~1) * 8u;
     mbar_expect_tx(&s_bar[s], rec_bytes + dv_bytes + y_bytes);
     bulk_g2s(s_rec + (size_t)s * seg_pad, a.src + (size_t)i * a.M + j0, rec_bytes, &s_bar[s]);
-    bulk_g2s(s_dv + (size_t)s * seg_pad * BT, dsrc + ((size_t)i * a.M + j0) * BT, dv_bytes, &s_bar[s]);
+    if (DV > 0)
+      bulk_g2s(s_dv + (size_t)s * seg_pad * DV, dsrc + ((size_t)i * a.M + j0) * DV, dv_bytes, &s_bar[s]);
     bulk_g2s(s_y + (size_t)s * seg_pad, a.y + j0, y_bytes, &s_bar[s]);
   };
 
@@ -304,27 +314,27 @@ __global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT 
     mbar_wait(&s_bar[s], (uint32_t)((q / kStages) & 1));
 
     const double2* rec = reinterpret_cast<const double2*>(s_rec + (size_t)s * seg_pad);
-    const double4* dv = s_dv + (size_t)s * seg_pad * BT;
+    const double4* dv = s_dv + (size_t)s * seg_pad * DV;
     const double* yy = s_y + (size_t)s * seg_pad;
     LinS col = {tot.cpsi, tot.cz, tot.s0, 0.0, 0.0, 0.0};
     int jlo = 0, jhi = len;
     if (j0 == 0) {
-      pair_lin<BT, true>(rec[0], rec[1], yy[0], dv, 0.5 * ci, tg, cc, col, acc);
+      pair_lin<BT, true, MODE>(rec[0], rec[1], yy[0], dv, 0.5 * ci, tg, cc, col, acc);
       jlo = 1;
     }
     const bool last = (j0 + len == a.M);
     if (last) jhi = len - 1;
     if (edge_col) {
       for (int j = jlo; j < jhi; ++j)
-        pair_lin<BT, true>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * BT, ci, tg, cc, col, acc);
+        pair_lin<BT, true, MODE>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * DV, ci, tg, cc, col, acc);
     } else {
-#pragma unroll kLinUnroll
+#pragma unroll (MODE == 0 ? kLinUnroll : 2)
       for (int j = jlo; j < jhi; ++j)
-        pair_lin<BT, false>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * BT, 1.0, tg, cc, col, acc);
+        pair_lin<BT, false, MODE>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * DV, 1.0, tg, cc, col, acc);
     }
     if (last && jhi >= jlo)
-      pair_lin<BT, true>(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], dv + (size_t)jhi * BT, 0.5 * ci, tg, cc,
-                         col, acc);
+      pair_lin<BT, true, MODE>(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], dv + (size_t)jhi * DV, 0.5 * ci, tg, cc,
+                               col, acc);
     tot.cpsi = col.cpsi; tot.cz = col.cz; tot.s0 = col.s0;
     tot.u3 = fma(cc.dx2, col.u3, tot.u3);
     tot.u3y = fma(cc.dx, col.u3y, tot.u3y);
@@ -333,37 +343,50 @@ __global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT 
   }
 
   if (t < a.T) {
-    double* o = a.out + ((size_t)(group * a.chunks + chunk) * (kLinShared + BT)) * a.T + t;
-    o[0] = tot.cpsi;
-    o[(size_t)1 * a.T] = tot.cz;
-    o[(size_t)2 * a.T] = tot.s0;
-    o[(size_t)3 * a.T] = tot.u3;
-    o[(size_t)4 * a.T] = tot.u3y;
-    o[(size_t)5 * a.T] = tot.u3yy;
+    double* o = a.out + ((size_t)(group * a.chunks + chunk) * (NSH + DV)) * a.T + t;
+    if (MODE != 2) {
+      o[0] = tot.cpsi;
+      o[(size_t)1 * a.T] = tot.cz;
+      o[(size_t)2 * a.T] = tot.s0;
+      o[(size_t)3 * a.T] = tot.u3;
+      o[(size_t)4 * a.T] = tot.u3y;
+      o[(size_t)5 * a.T] = tot.u3yy;
+    }
+    if (MODE != 1) {
 #pragma unroll
-    for (int d = 0; d < BT; ++d) o[(size_t)(kLinShared + d) * a.T] = acc[d];
+      for (int d = 0; d < BT; ++d) o[(size_t)(NSH + d) * a.T] = acc[d];
+    }
   }
 }
 
 // JV_d[E2 row of t] = e2lin_d - dx dy { sum_chunks acc_d - d psi*_d sum K1 - d zeta*_d sum cz
 //                     - d zeta_x*_d / sqrt(C) sum (u-+u+)
 //                     + zeta_x* / (2 C^(3/2)) (dA_d U3 + dB_d U3y + dC_d U3yy) }
-__global__ void __launch_bounds__(256) k_assemble_lin(Mesh m, int BT, int chunks, int b,
+__global__ void __launch_bounds__(256) k_assemble_lin(Mesh m, int BT, int chunks, int nsh,
+                                                      const double* __restrict__ sums,
                                                       const TgtRec* __restrict__ tgt,
                                                       const DTgtRec* __restrict__ dtgt,
                                                       const double* __restrict__ e2lin,
                                                       const double* __restrict__ part, double* JV) {
+  // nsh = 6: `part` rows are [group][chunk][6 + BT] (fused kernel); nsh = 0: [group][chunk][BT]
+  // and the six direction-independent sums come pre-reduced from `sums` [6][T] (sws_linearize)
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= m.T) return;
   const int d = blockIdx.y, g = d / BT, dd = d - g * BT;
-  const size_t T = m.T, stride = (size_t)(kLinShared + BT) * T;
+  const size_t T = m.T, stride = (size_t)(nsh + BT) * T;
   const double* p = part + (size_t)g * chunks * stride + t;
   double sh[kLinShared] = {0, 0, 0, 0, 0, 0}, sa = 0.0;
   for (int c = 0; c < chunks; ++c) {
     const double* pc = p + (size_t)c * stride;
+    if (nsh) {
 #pragma unroll
-    for (int q = 0; q < kLinShared; ++q) sh[q] += pc[(size_t)q * T];
-    sa += pc[(size_t)(kLinShared + dd) * T];
+      for (int q = 0; q < kLinShared; ++q) sh[q] += pc[(size_t)q * T];
+    }
+    sa += pc[(size_t)(nsh + dd) * T];
+  }
+  if (!nsh) {
+#pragma unroll
+    for (int q = 0; q < kLinShared; ++q) sh[q] = sums[(size_t)q * T + t];
   }
   const TgtRec tr = tgt[t];
   const DTgtRec dr = dtgt[(size_t)d * T + t];
@@ -373,7 +396,17 @@ __global__ void __launch_bounds__(256) k_assemble_lin(Mesh m, int BT, int chunks
   const int l = t / (m.N - 1), k = t - l * (m.N - 1);
   JV[(size_t)d * m.n + (size_t)(m.N + 1) * m.M + (size_t)l * (m.N + 1) + 2 + k] =
       e2lin[(size_t)d * T + t] - (m.dx * m.dy) * dsum;
-  (void)b;
+}
+
+// sums[q][t] = sum over column groups (fixed order) of the MODE 1 partials [chunk][6][T]
+__global__ void __launch_bounds__(256) k_reduce_base(int T, int chunks, const double* __restrict__ part,
+                                                     double* __restrict__ sums) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= T) return;
+  const int q = blockIdx.y;
+  double a = 0.0;
+  for (int c = 0; c < chunks; ++c) a += part[((size_t)c * kLinShared + q) * T + t];
+  sums[(size_t)q * T + t] = a;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -381,60 +414,69 @@ __global__ void __launch_bounds__(256) k_assemble_lin(Mesh m, int BT, int chunks
 
 int lin_tile(int b) { return b <= 1 ? 1 : b <= 4 ? 4 : b <= 8 ? 8 : 16; }
 
-static int lin_seg_cap(int BT) {
-  // nodes per staged segment: stage = seg (32 + 8 + 32 BT) bytes, two stages <= ~36 KB per CTA
-  int seg = (18 * 1024) / (40 + 32 * BT);
+static int lin_seg_cap(int DV) {
+  // nodes per staged segment: stage = seg (32 + 8 + 32 DV) bytes, two stages <= ~36 KB per CTA
+  int seg = (18 * 1024) / (40 + 32 * DV);
   seg &= ~1;
   if (seg > kSegMax) seg = kSegMax;
   if (seg < 8) seg = 8;
   return seg;
 }
 
-static size_t lin_smem_bytes(int BT, int seg) {
-  return (size_t)kStages * seg * (sizeof(SrcRec) + sizeof(double) + BT * sizeof(double4)) +
+static size_t lin_smem_bytes(int DV, int seg) {
+  return (size_t)kStages * seg * (sizeof(SrcRec) + sizeof(double) + DV * sizeof(double4)) +
          kStages * sizeof(uint64_t);
 }
 
-template <int BT>
+template <int BT, int MODE>
 static cudaError_t lin_configure_one(int* occ) {
-  const size_t smem = lin_smem_bytes(BT, lin_seg_cap(BT));
-  cudaError_t e = cudaFuncSetAttribute(k_allpairs_lin<BT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  const int DV = MODE == 1 ? 0 : BT;
+  const size_t smem = lin_smem_bytes(DV, lin_seg_cap(DV));
+  cudaError_t e = cudaFuncSetAttribute(k_allpairs_lin<BT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)smem + 64);
   if (e != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, k_allpairs_lin<BT>, kPairThreads, smem);
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, k_allpairs_lin<BT, MODE>, kPairThreads, smem);
 }
 
 cudaError_t lin_configure(sws_ctx* c) {
-  cudaError_t e = lin_configure_one<1>(&c->lin_occ[0]);
-  if (e == cudaSuccess) e = lin_configure_one<4>(&c->lin_occ[1]);
-  if (e == cudaSuccess) e = lin_configure_one<8>(&c->lin_occ[2]);
-  if (e == cudaSuccess) e = lin_configure_one<16>(&c->lin_occ[3]);
+  cudaError_t e = lin_configure_one<1, 0>(&c->lin_occ[0]);
+  if (e == cudaSuccess) e = lin_configure_one<4, 0>(&c->lin_occ[1]);
+  if (e == cudaSuccess) e = lin_configure_one<8, 0>(&c->lin_occ[2]);
+  if (e == cudaSuccess) e = lin_configure_one<16, 0>(&c->lin_occ[3]);
+  if (e == cudaSuccess) e = lin_configure_one<1, 2>(&c->lin_occ2[0]);
+  if (e == cudaSuccess) e = lin_configure_one<4, 2>(&c->lin_occ2[1]);
+  if (e == cudaSuccess) e = lin_configure_one<8, 2>(&c->lin_occ2[2]);
+  if (e == cudaSuccess) e = lin_configure_one<16, 2>(&c->lin_occ2[3]);
+  if (e == cudaSuccess) e = lin_configure_one<1, 1>(&c->lin_occ1);
   return e;
 }
 
-static int lin_occ_of(const sws_ctx* c, int BT) {
-  const int o = c->lin_occ[BT == 1 ? 0 : BT == 4 ? 1 : BT == 8 ? 2 : 3];
+static int lin_occ_of(const sws_ctx* c, int BT, int mode) {
+  const int i = BT == 1 ? 0 : BT == 4 ? 1 : BT == 8 ? 2 : 3;
+  const int o = mode == 1 ? c->lin_occ1 : mode == 2 ? c->lin_occ2[i] : c->lin_occ[i];
   return o > 0 ? o : 1;
 }
 
-// Launch geometry of the analytic all-pairs kernel: same tiles, a column split chosen from the
-// mesh, the SM count and this kernel's occupancy (wave quantisation), and short staged
+// Launch geometry of the analytic all-pairs kernels: same tiles, a column split chosen from the
+// mesh, the SM count and the kernel's occupancy (wave quantisation), and short staged
 // segments (the direction records make a node 40 + 32 BT bytes).
-PairPlan make_lin_plan(const sws_ctx* c, int BT, int groups) {
+// mode 0: fused (6 + BT rows per (group, chunk, target)); 1: base sums (6 rows); 2: directions (BT rows)
+PairPlan make_lin_plan(const sws_ctx* c, int BT, int groups, int mode) {
   const Mesh& m = c->mesh;
+  const int DV = mode == 1 ? 0 : BT, rows = (mode == 2 ? 0 : kLinShared) + DV;
   PairPlan p;
   p.tiles = (m.T + kPairThreads - 1) / kPairThreads;
-  const int cap = lin_seg_cap(BT);
+  const int cap = lin_seg_cap(DV);
   p.nseg = (m.M + cap - 1) / cap;
   int seg = (m.M + p.nseg - 1) / p.nseg;
   p.seg_len = (seg + 1) & ~1;
   p.nseg = (m.M + p.seg_len - 1) / p.seg_len;
-  const long slots = (long)c->sm_count * lin_occ_of(c, BT);
+  const long slots = (long)c->sm_count * lin_occ_of(c, BT, mode);
   int min_cols = (256 + m.M - 1) / m.M;
   int cmax = m.N / (min_cols > 0 ? min_cols : 1);
   if (cmax < 1) cmax = 1;
-  // the partial-sum buffer holds [group][chunk][6 + BT][T]
-  const long cap_chunks = (long)(c->part_rows / ((size_t)groups * (kLinShared + BT)));
+  // the partial-sum buffer holds [group][chunk][rows][T]
+  const long cap_chunks = (long)(c->part_rows / ((size_t)groups * rows));
   if (cmax > cap_chunks) cmax = (int)cap_chunks;
   if (cmax > 256) cmax = 256;
   if (cmax < 1) cmax = 1;
@@ -461,7 +503,7 @@ cudaError_t launch_targets_lin(sws_ctx* c, int b, int BT, double* JV, cudaStream
   return cudaGetLastError();
 }
 
-template <int BT>
+template <int BT, int MODE>
 static cudaError_t launch_lin_t(sws_ctx* c, int groups, const PairPlan& plan, cudaStream_t st) {
   const Mesh& m = c->mesh;
   LinArgs a;
@@ -470,24 +512,41 @@ static cudaError_t launch_lin_t(sws_ctx* c, int groups, const PairPlan& plan, cu
   a.chunks = plan.chunks; a.cols_per_chunk = plan.cols_per_chunk;
   a.seg_len = plan.seg_len; a.nseg = plan.nseg;
   dim3 grid(plan.tiles, plan.chunks, groups);
-  k_allpairs_lin<BT><<<grid, kPairThreads, lin_smem_bytes(BT, plan.seg_len), st>>>(a);
+  k_allpairs_lin<BT, MODE><<<grid, kPairThreads, lin_smem_bytes(MODE == 1 ? 0 : BT, plan.seg_len), st>>>(a);
   return cudaGetLastError();
 }
 
-cudaError_t launch_allpairs_lin(sws_ctx* c, int BT, int groups, const PairPlan& plan, cudaStream_t st) {
+cudaError_t launch_allpairs_lin(sws_ctx* c, int BT, int groups, int mode, const PairPlan& plan, cudaStream_t st) {
+  if (mode == 1) return launch_lin_t<1, 1>(c, 1, plan, st);
+  if (mode == 2) {
+    switch (BT) {
+      case 1: return launch_lin_t<1, 2>(c, groups, plan, st);
+      case 4: return launch_lin_t<4, 2>(c, groups, plan, st);
+      case 8: return launch_lin_t<8, 2>(c, groups, plan, st);
+      default: return launch_lin_t<16, 2>(c, groups, plan, st);
+    }
+  }
   switch (BT) {
-    case 1: return launch_lin_t<1>(c, groups, plan, st);
-    case 4: return launch_lin_t<4>(c, groups, plan, st);
-    case 8: return launch_lin_t<8>(c, groups, plan, st);
-    default: return launch_lin_t<16>(c, groups, plan, st);
+    case 1: return launch_lin_t<1, 0>(c, groups, plan, st);
+    case 4: return launch_lin_t<4, 0>(c, groups, plan, st);
+    case 8: return launch_lin_t<8, 0>(c, groups, plan, st);
+    default: return launch_lin_t<16, 0>(c, groups, plan, st);
   }
 }
 
-cudaError_t launch_assemble_lin(sws_ctx* c, int b, int BT, const PairPlan& plan, double* JV,
+cudaError_t launch_reduce_base(sws_ctx* c, const PairPlan& plan, cudaStream_t st) {
+  dim3 grid((c->mesh.T + 255) / 256, kLinShared);
+  k_reduce_base<<<grid, 256, 0, st>>>(c->mesh.T, plan.chunks, c->part, c->lin_sums);
+  return cudaGetLastError();
+}
+
+// mode 0: partials of the fused kernel; mode 2: direction partials + c->lin_sums
+cudaError_t launch_assemble_lin(sws_ctx* c, int b, int BT, int mode, const PairPlan& plan, double* JV,
                                 cudaStream_t st) {
   const Mesh& m = c->mesh;
   dim3 grid((m.T + 255) / 256, b);
-  k_assemble_lin<<<grid, 256, 0, st>>>(m, BT, plan.chunks, b, c->tgt, c->dtgt, c->e2lin, c->part, JV);
+  k_assemble_lin<<<grid, 256, 0, st>>>(m, BT, plan.chunks, mode == 2 ? 0 : kLinShared, c->lin_sums, c->tgt,
+                                       c->dtgt, c->e2lin, c->part, JV);
   return cudaGetLastError();
 }
 

@@ -399,3 +399,60 @@ def test_jv_exact_host_api_and_errors(sws):
         assert np.array_equal(c0.residual(dev(u)).cpu().numpy(), F)
         with pytest.raises(sws.SwsError, match="batch"):
             c0.jv_exact_batch(dev(u), dev(V))
+
+
+# ---------------------------------------------------------------------------------------
+# sws_linearize + sws_jv_apply: the same analytic action with the u-only part hoisted
+@pytest.mark.parametrize("i,b", [(0, 1), (0, 5), (1, 1), (1, 8), (1, 16)])
+def test_jv_apply_full_parity(sws, oracleC, i, b):
+    cfg = W.CONFIGS[i]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg, b)
+    with sws.Context(p, max_batch=b) as ctx:
+        ctx.linearize(dev(u))
+        JV = ctx.jv_apply(dev(V)).cpu().numpy()
+        JV1 = ctx.jv_apply(dev(V[0])).cpu().numpy()       # a second apply on the same linearisation
+        fused = ctx.jv_exact_batch(dev(u), dev(V)).cpu().numpy()
+    for k in range(b):
+        ref = oracleC.jv_exact(p, u, V[k])
+        assert relerr(JV[k], ref) <= TOL, (k, relerr(JV[k], ref))
+        assert relerr(JV[k], fused[k]) <= 1e-11
+    assert relerr(JV1, JV[0]) <= 1e-12
+
+
+@pytest.mark.parametrize("kw", RAGGED, ids=lambda k: f"{k['N']}x{k['M']}")
+def test_jv_apply_ragged_shapes(sws, oracleC, kw):
+    cfg = W.custom(eps=0.3, amp=0.05, **kw)
+    rng = np.random.default_rng(17)
+    u = W.state(cfg) + 1e-3 * rng.standard_normal(cfg.n)
+    V = rng.standard_normal((3, cfg.n))
+    p = cfg.params()
+    with sws.Context(p, max_batch=4) as ctx:
+        ctx.linearize(dev(u))
+        JV = ctx.jv_apply(dev(V)).cpu().numpy()
+    for k in range(3):
+        ref = oracleC.jv_exact(p, u, V[k])
+        assert relerr(JV[k], ref) <= TOL, (k, relerr(JV[k], ref))
+
+
+def test_jv_apply_cfg5_sampled_rows_and_state(sws, oracleC):
+    """cfg 5 at full size, b = 1 (the GMRES shape) and b = 16, sampled rows against the oracle;
+    the linearisation is invalidated by any call that overwrites the base state."""
+    cfg = W.CONFIGS[4]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg)
+    rng = np.random.default_rng(99)
+    T = cfg.targets
+    pick = np.unique(np.concatenate([rng.integers(0, T, 24), [0, cfg.N - 2, T - 1]])).astype(np.int32)
+    with sws.Context(p, max_batch=16) as ctx:
+        with pytest.raises(sws.SwsError, match="linearis"):
+            ctx.jv_apply(dev(V[0]))
+        ctx.linearize(dev(u))
+        JV1 = ctx.jv_apply(dev(V[3])).cpu().numpy()
+        JV = ctx.jv_apply(dev(V)).cpu().numpy()
+        ctx.residual(dev(u))
+        with pytest.raises(sws.SwsError, match="linearis"):
+            ctx.jv_apply(dev(V[0]))
+    for k, got in ((3, JV1), (3, JV[3]), (15, JV[15])):
+        ref = oracleC.jv_exact(p, u, V[k], rows=pick)
+        mask = ~np.isnan(ref)
+        err = np.abs(got[mask] - ref[mask]).max() / np.abs(got).max()
+        assert err <= TOL, (k, err)
