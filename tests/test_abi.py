@@ -22,8 +22,8 @@ def sws():
     return m
 
 
-def declared_functions():
-    text = re.sub(r"/\*.*?\*/", "", HEADER.read_text(), flags=re.S)
+def declared_functions(header=HEADER):
+    text = re.sub(r"/\*.*?\*/", "", header.read_text(), flags=re.S)
     return sorted(set(re.findall(r"\b(sws_[a-z0-9_]+)\s*\(", text)))
 
 
@@ -34,6 +34,34 @@ def test_header_symbols_exported(sws):
     for n in names:
         assert hasattr(lib, n), f"{n} declared in sws.h but not exported by libsws.so"
     assert sorted(sws.SYMBOLS) == names, "binding's SYMBOLS list and sws.h disagree"
+
+
+def test_jfnk_header_symbols_exported(sws):
+    """libsws_jfnk.so (Newton-Krylov driver) loads without a GPU and exports what sws_jfnk.h declares."""
+    import paper_1403_5044_b200.jfnk as jf
+    lib = jf.load_jfnk()
+    names = declared_functions(ROOT / "include" / "sws_jfnk.h")
+    assert len(names) >= 11
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in sws_jfnk.h but not exported by libsws_jfnk.so"
+    assert set(names) <= set(jf.SYMBOLS)
+    assert lib.sws_precond_create(None, 1, 0, None) == sws.SWS_EINVAL
+    assert lib.sws_solver_create(None, None, 10, None) == sws.SWS_EINVAL
+    assert lib.sws_precond_destroy(None) == 0 and lib.sws_solver_destroy(None) == 0
+
+
+def test_jfnk_struct_layouts(sws, tmp_path):
+    import paper_1403_5044_b200.jfnk as jf
+    structs = {"sws_gmres_opts": jf.GmresOpts, "sws_gmres_stats": jf.GmresStats, "sws_newton_opts": jf.NewtonOpts,
+               "sws_newton_log": jf.NewtonLog, "sws_newton_stats": jf.NewtonStats}
+    src = tmp_path / "layout2.c"
+    body = "".join(f'printf("%zu\\n", sizeof({c}));\n' for c in structs)
+    src.write_text('#include <stdio.h>\n#include "sws_jfnk.h"\nint main(void){\n' + body + "return 0;}\n")
+    exe = tmp_path / "layout2"
+    subprocess.run(["gcc", f"-I{ROOT / 'include'}", str(src), "-o", str(exe)], check=True)
+    out = [int(x) for x in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
+    for (cname, ct), size in zip(structs.items(), out):
+        assert ctypes.sizeof(ct) == size, cname
 
 
 def test_params_struct_layout(sws, tmp_path):
@@ -56,7 +84,7 @@ def test_params_struct_layout(sws, tmp_path):
 def test_error_strings(sws):
     lib = sws.load_library()
     assert lib.sws_strerror(0) == b"ok"
-    for code in (-1, -2, -3, -4):
+    for code in (-1, -2, -3, -4, -5):
         assert lib.sws_strerror(code) not in (b"ok", b"unknown error")
     assert lib.sws_strerror(-99) == b"unknown error"
 
