@@ -248,6 +248,69 @@ def jv_exact_report(ctx, cfg, u, V, steps: int, flush, peak_tf: float) -> dict:
                     "oracle in tests/test_gpu_parity.py"}
 
 
+def jv_apply_report(ctx, cfg, u, V, steps: int, flush) -> dict:
+    """sws_linearize once + sws_jv_apply (the Newton-Krylov shape): b = 1 (one GMRES product) and the
+    full batch, CUDA events, L2 flush between iterations."""
+    import torch
+    out = {}
+    ctx.linearize(u)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    flush.zero_()
+    e0.record(); ctx.linearize(u); e1.record()
+    torch.cuda.synchronize()
+    out["linearize_ms"] = e0.elapsed_time(e1)
+    for b in (1, int(V.shape[0])):
+        Vb = V[:b].contiguous()
+        JV = torch.empty((b, cfg.n), dtype=torch.float64, device=u.device)
+        ctx.jv_apply(Vb, out=JV)
+        torch.cuda.synchronize()
+        ms = 0.0
+        for _ in range(steps):
+            flush.zero_()
+            e0.record(); ctx.jv_apply(Vb, out=JV); e1.record()
+            torch.cuda.synchronize()
+            ms += e0.elapsed_time(e1)
+        ms /= steps
+        out[f"b{b}"] = {"ms_per_call": ms, "jv_per_s": b / (ms * 1e-3), "fp64_instr_per_pair": 41 + 4 * b,
+                        "pair_direction_products_per_s": b * cfg.pairs / (ms * 1e-3)}
+    return out
+
+
+def solve_report(sws, device: int, names=("paper_361x121", "paper_721x241"), bandwidth: int = 31) -> dict:
+    """The whole preconditioned JFNK solve on the paper's own meshes, from the flat
+    initial guess, eps = 1, F = 0.7: wall time of the Newton driver with u resident on the
+    device, plus the one-off preconditioner assembly + factorisation.  Context (other hardware): the paper
+    reports 3.5 min (361x121) and 1.5 h (721x241) on a Tesla M2090 workstation, 75 min (361x121) on a desktop."""
+    import torch
+
+    import paper_1403_5044_b200.jfnk as jf
+    out = {}
+    for name in names:
+        cfg = W.PAPER_BY_NAME[name]
+        p = cfg.params()
+        with sws.Context(p, max_batch=1, device=device) as ctx, \
+                jf.Preconditioner(p, bandwidth=bandwidth, device=device) as pc, jf.Solver(ctx, pc, 60) as s:
+            u0 = torch.from_numpy(W.flat_state(cfg)).cuda(device)
+            kw = dict(ftol=1e-9, eta=1e-3, restart=60, gmres_maxit=120)
+            s.newton(u0, max_newton=1, **kw)                # warm-up (one Newton step)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            u, log, st = s.newton(u0, **kw)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            out[name] = {"solve_s": dt, "precond_setup_s": pc.setup_ms * 1e-3, "precond_GB": pc.bytes / 1e9,
+                         "block_bandwidth": pc.bandwidth, "newton_steps": st["steps"], "converged": st["converged"],
+                         "jv_products": st["jv_products"], "residual_evals": st["residual_evals"],
+                         "precond_applies": st["precond_applies"], "final_residual_inf": log[-1]["finf"],
+                         "ms_jv": st["ms_jv"], "ms_precond": st["ms_precond"], "ms_residual": st["ms_residual"],
+                         "gmres_its_per_step": [e["gmres_its"] for e in log[:-1]]}
+    out["note"] = ("flat initial guess, eps=1, F=0.7, ||E||_inf <= 1e-9, inexact Newton eta=1e-3, analytic Jv "
+                   "(sws_linearize + sws_jv_apply), block-banded linear-Jacobian preconditioner; paper (other "
+                   "hardware, KINSOL + FD Jv): 361x121 in ~3.5 min and 721x241 in 1.5 h on a Tesla M2090 workstation")
+    return out
+
+
 def run_ours(args) -> None:
     import torch
 
@@ -390,6 +453,13 @@ def run_ours(args) -> None:
         jvx["speedup_vs_fd_batch"] = (jvx["jv_per_s"] /
                                       (b / ((ms_total / args.steps) * 1e-3 * (b + 1) / evals_per_step)))
 
+    if jvx is not None:
+        jvx["linearize_apply"] = jv_apply_report(ctx, cfg, u, V, max(2, args.steps), flush)
+
+    solve = None
+    if world == 1 and not args.no_solve:
+        solve = solve_report(sws, local)
+
     fp32 = None
     if world == 1 and not args.no_fp32:
         fp32 = fp32_variant_report(sws, local, names=tuple(dict.fromkeys(["cfg4_361x121", cfg.name])))
@@ -413,6 +483,7 @@ def run_ours(args) -> None:
         "workspace_bytes": ctx.workspace_bytes,
         "jv_exact": jvx,
         "fp32_variant": fp32,
+        "solve": solve,
     }
     print(json.dumps(line), flush=True)
     ctx.close()
@@ -431,6 +502,7 @@ def main() -> None:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fp32", action="store_true", help="skip the reported FP32-variant section")
     ap.add_argument("--no-jv-exact", action="store_true", help="skip the analytic-Jv section")
+    ap.add_argument("--no-solve", action="store_true", help="skip the full JFNK solve section")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)

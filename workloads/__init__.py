@@ -77,6 +77,19 @@ CONFIGS = (
 )
 BY_NAME = {c.name: c for c in CONFIGS}
 
+# The meshes the paper itself solves on, eps = 1: 91x31 "contemporary" and
+# 361x121, 721x241 (L275), all F = 0.7; Fig. 2/3's 45x13 (L247); Fig. 7's
+# F = 1.4 mesh (L336: 721x241, dx = dy = 0.3, x0 = -56).  The solver tests and bench.py's `solve`
+# section start these from the flat state (L227); the seeded Gaussian state is also defined.
+PAPER_MESHES = (
+    Config("paper_45x13",    45,  13, 0.4,    -9.0, 0.0, 0.7, 1.0, 0.05, 0.05, 11, 0, 111),
+    Config("paper_91x31",    91,  31, 0.3,    -9.0, 0.0, 0.7, 1.0, 0.05, 0.05, 12, 0, 112),
+    Config("paper_361x121", 361, 121, 0.15,  -14.0, 0.0, 0.7, 1.0, 0.05, 0.05, 13, 0, 113),
+    Config("paper_721x241", 721, 241, 0.075, -14.0, 0.0, 0.7, 1.0, 0.05, 0.05, 14, 0, 114),
+    Config("paper_fig7_721x241", 721, 241, 0.3, -56.0, 0.0, 1.4, 1.0, 0.05, 0.05, 15, 0, 115),
+)
+PAPER_BY_NAME = {c.name: c for c in PAPER_MESHES}
+
 
 def custom(N, M, h, x1, *, y1=0.0, froude=0.7, eps=0.1, n_rad=0.05, amp=0.02,
            seed=0, b=0, seed_V=None, name=None) -> Config:
