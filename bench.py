@@ -37,10 +37,12 @@ import workloads as W  # noqa: E402
 
 METRIC = "fp64_residual_evals_per_s"
 UNIT = "evals/s"
-# Algorithmic work of the all-pairs kernel per pair interaction, from its SASS inner loop
-# (DESIGN.md "Kernels"): 45 FP64-pipe instructions = 23 DFMA (2 flops) + 22 DMUL/DADD (1 flop).
-FP64_INSTR_PER_PAIR = 45
-FLOPS_PER_PAIR = 68
+# Work of the all-pairs kernel per pair interaction, from its SASS inner loops:
+#   near columns (S2 summed pair by pair): 45 FP64-pipe instructions = 23 DFMA (2 flops) + 22 DMUL/DADD;
+#   far columns (S2 column sum from its Euler-Maclaurin form): 29 = 15 DFMA + 14 DMUL/DADD.
+# The ~200 FP64 instructions of the expansion per (target, far column) are NOT counted as achieved work.
+FP64_INSTR_NEAR, FLOPS_NEAR = 45, 68
+FP64_INSTR_FAR, FLOPS_FAR = 29, 44
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
 # dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
 # ncu --set full capture summarised in profiles/r1_allpairs_ncu.md (algorithmic: 16.67 MB)
@@ -369,6 +371,7 @@ def run_ours(args) -> None:
     ms_total = sum(e0.elapsed_time(e1) for e0, e1 in ev)
     ap_ms, ap_launches = ctx.profile_read(reset=True)
     ctx.set_profiling(False)
+    near = ctx.farfield_stats(b + 1)       # of the b + 1 states of the last sws_jv_batch
     clocks = sampler.stop() if rank == 0 else None
     ms_total = replicas.max_over_ranks(ms_total)
     value = world * args.steps * evals_per_step / (ms_total * 1e-3)
@@ -418,9 +421,11 @@ def run_ours(args) -> None:
     peak_tf = sm_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     pairs_timed = args.steps * pairs_per_step
     ap_s = ap_ms * 1e-3
-    achieved_tf = FLOPS_PER_PAIR * pairs_timed / ap_s / 1e12
+    flops_pair = near * FLOPS_NEAR + (1.0 - near) * FLOPS_FAR
+    instr_pair = near * FP64_INSTR_NEAR + (1.0 - near) * FP64_INSTR_FAR
+    achieved_tf = flops_pair * pairs_timed / ap_s / 1e12
     sm_mhz = (clocks or {}).get("sm_mhz") or sm_max
-    pipe_frac = FP64_INSTR_PER_PAIR * pairs_timed / (sm_count * FP64_LANES_PER_SM * sm_mhz * 1e6 * ap_s)
+    pipe_frac = instr_pair * pairs_timed / (sm_count * FP64_LANES_PER_SM * sm_mhz * 1e6 * ap_s)
     roofline = {
         "bound": "alu", "kernel": "k_allpairs", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
         "frac": achieved_tf / peak_tf, "traffic": NCU_DRAM_BYTES_PER_STATE_LAUNCH.get(cfg.name),
@@ -429,7 +434,12 @@ def run_ours(args) -> None:
         "algorithmic_bytes_per_state": cfg.sources * 32 + cfg.targets * 64,
         "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz "
                        "(FP64 is not in MEASURED_PEAKS.json; DESIGN.md 'Peak')",
-        "flops_per_pair": FLOPS_PER_PAIR, "fp64_instr_per_pair": FP64_INSTR_PER_PAIR,
+        "flops_per_pair": flops_pair, "fp64_instr_per_pair": instr_pair,
+        "near_column_fraction": near,
+        "work_note": f"executed pair-loop work: {FLOPS_NEAR} flops/pair on the near columns (direct S2), "
+                     f"{FLOPS_FAR} on the far ones (S2 column sum in closed form + Euler-Maclaurin, sws_set_farfield); "
+                     "with the plain 68 flops/pair definition the same time reads "
+                     f"{FLOPS_NEAR * pairs_timed / ap_s / 1e12:.1f} TFLOP/s-equivalent",
         "launches_timed": ap_launches, "avg_launch_ms": ap_ms / max(ap_launches, 1),
         "share_of_step": ap_ms / ms_total if world == 1 else None,
         "dfma_probe_tflops": probe["tflops"], "dfma_probe_sm_mhz": probe["sm_mhz"],

@@ -165,6 +165,19 @@ int sws_profile_read(sws_ctx* ctx, double* allpairs_ms, int32_t* launches, int32
  * clamped to what the workspace was sized for). */
 int sws_set_tuning(sws_ctx* ctx, int32_t chunks);
 
+/* Far-field evaluation of the S2 terms (sws_allpairs.cu).  For a source
+ * column whose completed-square constant g of L169-177 satisfies sqrt(g) >= radius_in_dy * dy for
+ * all 32 targets of a warp, the column's S2 trapezoid sum (which does not depend on the source
+ * data) is replaced by its integral (asinh) plus 7 Euler-Maclaurin end corrections, exact to
+ * < 1e-16 / sqrt(g) for radius >= 8; the K1 and K2 terms are always summed pair by pair.
+ * radius_in_dy <= 0 switches the expansion off (every S2 term summed directly, the plain
+ * definition); 0 < radius < 6 is refused (SWS_EINVAL).  Default 8. */
+int sws_set_farfield(sws_ctx* ctx, double radius_in_dy);
+
+/* Fraction of (warp, source column) combinations of the first `states` states of the last call
+ * that take the direct S2 loop (bench.py: executed FP64 work of a launch).  Synchronises. */
+int sws_farfield_stats(sws_ctx* ctx, int32_t states, double* near_fraction, void* cuda_stream);
+
 /* The all-pairs launch geometry for `states` states: out5 = {target tiles, column groups,
  * columns per group, nodes staged per bulk copy, segments per column}. */
 int sws_plan_info(sws_ctx* ctx, int32_t states, int32_t* out5);
@@ -183,6 +196,12 @@ int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, doubl
 /* y[i] = the library's device reciprocal square root of x[i] (host buffers), for the
  * unit test of that primitive. */
 int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, int32_t n);
+
+/* Unit test of the far-field expansion: for n pairs (c, g) and the column y1, y1+dy, ..., M nodes,
+ * em_host[i] = the library's expansion of sum_j c_j [((y_j-c)^2+g)^-1/2 + ((y_j+c)^2+g)^-1/2]
+ * (c_j = 1/2 at both ends) and direct_host[i] = the same sum term by term on the device. */
+int sws_debug_s2col_host(int32_t device, double y1, double dy, int32_t M, const double* c_host,
+                         const double* g_host, int32_t n, double* direct_host, double* em_host);
 
 #ifdef __cplusplus
 }

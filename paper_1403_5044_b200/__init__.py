@@ -27,6 +27,7 @@ SYMBOLS = (
     "sws_probe_fp64_peak", "sws_debug_rsqrt_host",
     "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
     "sws_get_params", "sws_linearize", "sws_jv_apply",
+    "sws_set_farfield", "sws_farfield_stats", "sws_debug_s2col_host",
 )
 
 
@@ -84,6 +85,9 @@ def load_library() -> C.CDLL:
         "sws_last_cuda_error": (C.c_char_p, []),
         "sws_probe_fp64_peak": (C.c_int, [C.c_int32, C.POINTER(C.c_double), ip, C.POINTER(C.c_double)]),
         "sws_debug_rsqrt_host": (C.c_int, [C.c_int32, dp, dp, C.c_int32]),
+        "sws_set_farfield": (C.c_int, [vp, C.c_double]),
+        "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
+        "sws_debug_s2col_host": (C.c_int, [C.c_int32, C.c_double, C.c_double, C.c_int32, dp, dp, C.c_int32, dp, dp]),
     }
     for name, (res, args) in proto.items():
         fn = getattr(lib, name)
@@ -300,6 +304,16 @@ class Context:
     def set_tuning(self, chunks: int = 0) -> None:
         _check(self.lib.sws_set_tuning(self._h, int(chunks)), "sws_set_tuning")
 
+    def set_farfield(self, radius_in_dy: float = 8.0) -> None:
+        """sws_set_farfield: <= 0 sums every S2 term directly (the plain definition)."""
+        _check(self.lib.sws_set_farfield(self._h, float(radius_in_dy)), "sws_set_farfield")
+
+    def farfield_stats(self, states: int = 1) -> float:
+        """Fraction of (warp, column) combinations that take the direct S2 loop."""
+        f = C.c_double()
+        _check(self.lib.sws_farfield_stats(self._h, int(states), C.byref(f), self._stream()), "sws_farfield_stats")
+        return float(f.value)
+
     def plan_info(self, states: int = 1) -> dict:
         out = (C.c_int32 * 5)()
         _check(self.lib.sws_plan_info(self._h, int(states), out), "sws_plan_info")
@@ -330,3 +344,15 @@ def debug_rsqrt(x: np.ndarray, device: int = 0) -> np.ndarray:
     y = np.empty_like(x)
     _check(lib.sws_debug_rsqrt_host(int(device), _np_ptr(x), _np_ptr(y), int(x.size)), "sws_debug_rsqrt_host")
     return y
+
+
+def debug_s2col(y1: float, dy: float, M: int, c: np.ndarray, g: np.ndarray, device: int = 0):
+    """(direct, em): the S2 column sum term by term on the device and by the library's far-field
+    expansion (unit test hook, sws_debug_s2col_host)."""
+    lib = load_library()
+    c = np.ascontiguousarray(c, dtype=np.float64)
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    d, e = np.empty_like(c), np.empty_like(c)
+    _check(lib.sws_debug_s2col_host(int(device), float(y1), float(dy), int(M), _np_ptr(c), _np_ptr(g),
+                                    int(c.size), _np_ptr(d), _np_ptr(e)), "sws_debug_s2col_host")
+    return d, e

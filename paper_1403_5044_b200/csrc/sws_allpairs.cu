@@ -72,8 +72,10 @@ struct ColC {
   double dx, dx2, c, g;  // x_i - x*, its square, and the S2 constants above
 };
 
-// One source node against one target: adds (phi-phi*-x+x*) K1 + zeta_x K2 to a1 and
-// sqrt(C) S2 to aS (unit weight).
+// One source node against one target: adds (phi-phi*-x+x*) K1 + zeta_x K2 to a1 and, if S2T,
+// sqrt(C) S2 to aS (unit weight).  S2T = false is the far-field form: the S2 terms of the
+// whole column come from s2_column_em() below, 29 FP64 instructions + 2 MUFU.RSQ64H remain.
+template <bool S2T>
 __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, const double yj,
                                           const TgtC& t, const ColC& c, double& a1, double& aS) {
   const double z = zp.x, psi = zp.y, zx = sl.x, zy = sl.y;
@@ -95,12 +97,120 @@ __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, co
   const double dpsi = psi - t.psis;
   a1 = fma(dpsi, k1, a1);
   a1 = fma(zx, rm + rp, a1);  // K2 = 1/R- + 1/R+
-  // S2 (eqs. (21), (22)) up to the factor 1/sqrt(C)
-  const double sm = yj - c.c;
-  const double sp = yj + c.c;
-  const double Qm = fma(sm, sm, c.g);
-  const double Qp = fma(sp, sp, c.g);
-  aS += rsqrt_fp64(Qm) + rsqrt_fp64(Qp);
+  if (S2T) {
+    // S2 (eqs. (21), (22)) up to the factor 1/sqrt(C)
+    const double sm = yj - c.c;
+    const double sp = yj + c.c;
+    const double Qm = fma(sm, sm, c.g);
+    const double Qp = fma(sp, sp, c.g);
+    aS += rsqrt_fp64(Qm) + rsqrt_fp64(Qp);
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// Far-field form of the S2 column sums.
+//
+// For one target and one source column the S2 terms of the quadrature are, up to 1/sqrt(C),
+//     sum_j c_j [ f(y_j; c) + f(y_j; -c) ],   f(y; c) = ((y - c)^2 + g)^(-1/2),
+// a composite trapezoid sum (step dy, c_j = 1/2 at both ends, reading Q4) of a function that
+// does NOT depend on the source data: c and g depend on the target's A, B, C and on x_i - x*
+// only.  f is analytic with its nearest singularities at y = c +- i sqrt(g), sqrt(g) ~ |x_i - x*|,
+// so once sqrt(g) >= r dy the sum equals its Euler-Maclaurin expansion to round-off:
+//     dy sum_j c_j f(y_j) = int_a^b f dy + sum_{k=1..K} B_2k dy^2k / (2k)! (f^(2k-1)(b) - f^(2k-1)(a)) + R_K,
+//     int f dy = asinh((y - c) / sqrt(g)),
+//     f^(n)(y) = (-1)^n n! P_n(mu) / rho^(n+1),  rho = sqrt((y-c)^2 + g), mu = (y - c) / rho
+// (P_n = Legendre polynomial: 1/rho is the generating function of P_n), i.e. the k-th term is
+//     -(B_2k / 2k) (dy / rho)^2k P_{2k-1}(mu)  at b minus the same at a.
+// With K = 7 and r = 8 the remainder is < 1e-16 / sqrt(g) (measured against 50-digit sums over
+// the whole range of c), below the rounding of the direct sum itself.
+// The same quantity, evaluated another way: the result still matches the oracle's plain sum.
+// Cost: ~120 FP64 instructions per (target, column) instead of 16 per pair.
+// (default r = kEmRadius of sws_internal.cuh; sws_set_farfield changes it, r <= 0 sums directly)
+
+// sum_{k=1..7} (B_2k / 2k) s^k P_{2k-1}(mu) at the end point u = y_e - c;  *rho = sqrt(u^2 + g)
+__device__ __forceinline__ double em_tail(const double u, const double g, const double h2, double* rho) {
+  const double r2 = fma(u, u, g);
+  const double ri = rsqrt_fp64(r2);
+  *rho = r2 * ri;
+  const double mu = u * ri;
+  const double s = h2 * (ri * ri);
+  double P[14];
+  P[0] = 1.0;
+  P[1] = mu;
+#pragma unroll
+  for (int n = 1; n <= 12; ++n)  // (n+1) P_{n+1} = (2n+1) mu P_n - n P_{n-1}
+    P[n + 1] = ((2.0 * n + 1.0) / (n + 1.0)) * (mu * P[n]) - (n / (n + 1.0)) * P[n - 1];
+  double t = (1.0 / 12.0) * P[13];              // B_14 / 14
+  t = fma(s, t, (-691.0 / 32760.0) * P[11]);    // B_12 / 12
+  t = fma(s, t, (1.0 / 132.0) * P[9]);          // B_10 / 10
+  t = fma(s, t, (-1.0 / 240.0) * P[7]);         // B_8 / 8
+  t = fma(s, t, (1.0 / 252.0) * P[5]);          // B_6 / 6
+  t = fma(s, t, (-1.0 / 120.0) * P[3]);         // B_4 / 4
+  t = fma(s, t, (1.0 / 12.0) * P[1]);           // B_2 / 2
+  return s * t;
+}
+
+// dy * (trapezoid sum of f(.; c) over the nodes a, a + dy, ..., b), by the expansion above
+__device__ __forceinline__ double em_interval(const double a, const double b, const double c, const double g,
+                                              const double h2) {
+  const double ua = a - c, ub = b - c;
+  double rhoa, rhob;
+  const double ta = em_tail(ua, g, h2, &rhoa);
+  const double tb = em_tail(ub, g, h2, &rhob);
+  // asinh(ub / sqrt g) - asinh(ua / sqrt g) = log(q),  q = L(ub) / L(ua),  L(u) = u + rho = g / (rho - u),
+  // each L taken in the form without cancellation.  q - 1 = (L(ub) - L(ua)) / L(ua) with
+  // L(ub) - L(ua) = (b - a) (L(ua) + L(ub)) / (rho_a + rho_b), so log(q) = log1p((b - a)(1 + q) / (rho_a + rho_b))
+  // keeps full relative accuracy when the interval is short against sqrt(g) (q -> 1).
+  const double nb = ub >= 0.0 ? ub + rhob : g, db = ub >= 0.0 ? 1.0 : rhob - ub;
+  const double na = ua >= 0.0 ? ua + rhoa : g, da = ua >= 0.0 ? 1.0 : rhoa - ua;
+  const double q = (nb * da) / (db * na);
+  return log1p((b - a) * (1.0 + q) / (rhoa + rhob)) - (tb - ta);
+}
+
+struct EmGeom {
+  double y1, yM;   // first and last node of a column
+  double h2, inv_h;  // dy^2, 1 / dy
+  double gmin;     // (r dy)^2; a column is "far" for a target when g >= gmin  (inf: never)
+  int sym;         // y1 == 0: direct + image = one trapezoid sum over [-yM, yM]
+};
+
+// sum_j c_j [ f(y_j; c) + f(y_j; -c) ]  (unit node weights, as the direct loop accumulates it)
+__device__ __forceinline__ double s2_column_em(const EmGeom& e, const double c, const double g) {
+  const double v = e.sym ? em_interval(-e.yM, e.yM, c, g, e.h2)
+                         : em_interval(e.y1, e.yM, c, g, e.h2) + em_interval(e.y1, e.yM, -c, g, e.h2);
+  return v * e.inv_h;
+}
+
+// The far/near decision is taken per WARP (all 32 targets of the warp must be far), so the j loop
+// has no divergence.  Used by k_allpairs and by the counting kernel of sws_farfield_stats.
+__device__ __forceinline__ bool column_is_far(const double g, const double gmin) {
+  return __all_sync(0xffffffffu, g >= gmin) != 0;
+}
+
+// One staged segment [j0, j0 + len) of a column: trapezoid half weights on the column's first and
+// last node by peeling (Q4), unit weights inside.
+template <bool S2T>
+__device__ __forceinline__ void walk_segment(const double2* rec, const double* yy, const int j0, const int len,
+                                             const int M, const TgtC& tg, const ColC& cc, double& col1,
+                                             double& colS) {
+  int jlo = 0, jhi = len;
+  if (j0 == 0) {  // first node of the column: weight 1/2 in y
+    double h1 = 0.0, hS = 0.0;
+    pair_term<S2T>(rec[0], rec[1], yy[0], tg, cc, h1, hS);
+    col1 = 0.5 * h1;
+    colS = 0.5 * hS;
+    jlo = 1;
+  }
+  const bool last = (j0 + len == M);
+  if (last) jhi = len - 1;
+#pragma unroll kUnroll
+  for (int j = jlo; j < jhi; ++j) pair_term<S2T>(rec[2 * j], rec[2 * j + 1], yy[j], tg, cc, col1, colS);
+  if (last && jhi >= jlo) {  // last node of the column: weight 1/2 in y
+    double h1 = 0.0, hS = 0.0;
+    pair_term<S2T>(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], tg, cc, h1, hS);
+    col1 = fma(0.5, h1, col1);
+    colS = fma(0.5, hS, colS);
+  }
 }
 
 struct PairArgs {
@@ -112,6 +222,7 @@ struct PairArgs {
   int N, M, T;
   int chunks, cols_per_chunk, seg_len, nseg;
   double dxdy;
+  EmGeom em;
 };
 
 template <int MINB>
@@ -177,23 +288,11 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
     const double2* rec = reinterpret_cast<const double2*>(s_rec + (size_t)s * seg_pad);
     const double* yy = s_y + (size_t)s * seg_pad;
     double col1 = 0.0, colS = 0.0;
-    int jlo = 0, jhi = len;
-    if (j0 == 0) {  // first node of the column: weight 1/2 in y
-      double h1 = 0.0, hS = 0.0;
-      pair_term(rec[0], rec[1], yy[0], tg, cc, h1, hS);
-      col1 = 0.5 * h1;
-      colS = 0.5 * hS;
-      jlo = 1;
-    }
-    const bool last = (j0 + len == a.M);
-    if (last) jhi = len - 1;
-#pragma unroll kUnroll
-    for (int j = jlo; j < jhi; ++j) pair_term(rec[2 * j], rec[2 * j + 1], yy[j], tg, cc, col1, colS);
-    if (last && jhi >= jlo) {  // last node of the column: weight 1/2 in y
-      double h1 = 0.0, hS = 0.0;
-      pair_term(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], tg, cc, h1, hS);
-      col1 = fma(0.5, h1, col1);
-      colS = fma(0.5, hS, colS);
+    if (column_is_far(cc.g, a.em.gmin)) {  // warp-uniform
+      walk_segment<false>(rec, yy, j0, len, a.M, tg, cc, col1, colS);
+      if (j0 == 0) colS = s2_column_em(a.em, cc.c, cc.g);  // the column's S2 terms, once
+    } else {
+      walk_segment<true>(rec, yy, j0, len, a.M, tg, cc, col1, colS);
     }
     tot1 = fma(ci, col1, tot1);
     totS = fma(ci, colS, totS);
@@ -207,6 +306,19 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
 
 // ---------------------------------------------------------------------------------------
 // host side
+
+static EmGeom em_geometry(const sws_ctx* c) {
+  const Mesh& m = c->mesh;
+  EmGeom e;
+  e.y1 = m.y1;
+  e.yM = m.y1 + (m.M - 1) * m.dy;
+  e.h2 = m.dy * m.dy;
+  e.inv_h = 1.0 / m.dy;
+  const double r = c->em_radius;
+  e.gmin = r > 0.0 ? (r * m.dy) * (r * m.dy) : __builtin_inf();
+  e.sym = m.sym_first;
+  return e;
+}
 
 constexpr int kMinB = SWS_MINB;
 
@@ -284,8 +396,62 @@ cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaSt
   a.chunks = plan.chunks; a.cols_per_chunk = plan.cols_per_chunk;
   a.seg_len = plan.seg_len; a.nseg = plan.nseg;
   a.dxdy = m.dx * m.dy;
+  a.em = em_geometry(c);
   dim3 grid(plan.tiles, plan.chunks, states);
   k_allpairs<kMinB><<<grid, kPairThreads, allpairs_smem_bytes(plan), st>>>(a);
+  return cudaGetLastError();
+}
+
+// --- far-field statistics (bench.py: executed work of a launch) ----------------------------
+// One warp = the same 32 targets as a warp of k_allpairs; counts the columns that warp treats
+// as near (direct S2 loop).  out[state * warps + w].
+__global__ void k_count_near(const TgtRec* tgt, const double* x, int N, int T, double gmin, int* out) {
+  const int warps = (T + 31) / 32;
+  const int w = blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32, state = blockIdx.y;
+  if (w >= warps) return;
+  const int t = w * 32 + (threadIdx.x & 31);
+  const TgtRec tr = tgt[(size_t)state * T + (t < T ? t : T - 1)];
+  const double kb = tr.B / (2.0 * tr.C);
+  const double kg = tr.A / tr.C - kb * kb;
+  int near = 0;
+  for (int i = 0; i < N; ++i) {
+    const double dx = __ldg(x + i) - tr.xs;
+    const double dx2 = dx * dx;
+    if (!column_is_far(kg * dx2, gmin)) ++near;
+  }
+  if ((threadIdx.x & 31) == 0) out[(size_t)state * warps + w] = near;
+}
+
+cudaError_t launch_count_near(sws_ctx* c, int states, int* out, cudaStream_t st) {
+  const Mesh& m = c->mesh;
+  const int warps = (m.T + 31) / 32;
+  dim3 grid((warps + 3) / 4, states);
+  k_count_near<<<grid, 128, 0, st>>>(c->tgt, c->x, m.N, m.T, em_geometry(c).gmin, out);
+  return cudaGetLastError();
+}
+
+// --- unit-test hook of the far-field expansion ---------------------------------------------
+// out_em[i] = s2_column_em(c[i], g[i]); out_direct[i] = the plain trapezoid sum it stands for
+__global__ void k_debug_s2col(EmGeom e, int M, const double* c, const double* g, int n, double* out_direct,
+                              double* out_em) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  out_em[i] = s2_column_em(e, c[i], g[i]);
+  double acc = 0.0;
+  for (int j = 0; j < M; ++j) {
+    const double yj = e.y1 + j * sqrt(e.h2);
+    const double sm = yj - c[i], sp = yj + c[i];
+    const double v = rsqrt_fp64(fma(sm, sm, g[i])) + rsqrt_fp64(fma(sp, sp, g[i]));
+    acc += (j == 0 || j == M - 1) ? 0.5 * v : v;
+  }
+  out_direct[i] = acc;
+}
+
+cudaError_t launch_debug_s2col(double y1, double dy, int M, const double* c, const double* g, int n,
+                               double* out_direct, double* out_em, cudaStream_t st) {
+  EmGeom e;
+  e.y1 = y1; e.yM = y1 + (M - 1) * dy; e.h2 = dy * dy; e.inv_h = 1.0 / dy; e.gmin = 0.0; e.sym = (y1 == 0.0);
+  k_debug_s2col<<<(n + 127) / 128, 128, 0, st>>>(e, M, c, g, n, out_direct, out_em);
   return cudaGetLastError();
 }
 

@@ -88,6 +88,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   sws_ctx* c = new (std::nothrow) sws_ctx();
   if (!c) return SWS_ENOMEM;
   memset(c, 0, sizeof *c);
+  c->em_radius = sws::kEmRadius;  // far-field radius of the S2 column sums (sws_allpairs.cu, sws_set_farfield)
   c->params = *p;
   c->device = p->device;
   sws::Mesh& m = c->mesh;
@@ -227,6 +228,34 @@ int sws_set_tuning(sws_ctx* c, int32_t chunks) {
   if (!c || chunks < 0) return SWS_EINVAL;
   if (chunks > c->part_chunks) chunks = c->part_chunks;  // the partial-sum buffer is sized at setup
   c->chunks_user = chunks;
+  return SWS_OK;
+}
+
+int sws_set_farfield(sws_ctx* c, double radius_in_dy) {
+  if (!c || radius_in_dy != radius_in_dy) return SWS_EINVAL;
+  if (radius_in_dy > 0.0 && radius_in_dy < 6.0) return SWS_EINVAL;  // the expansion is not accurate there
+  c->em_radius = radius_in_dy;
+  return SWS_OK;
+}
+
+int sws_farfield_stats(sws_ctx* c, int32_t states, double* near_fraction, void* cuda_stream) {
+  if (!c || !near_fraction) return SWS_EINVAL;
+  if (states < 1 || states > c->max_states || states > c->last_states) return SWS_EBATCH;
+  CK(cudaSetDevice(c->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int warps = (c->mesh.T + 31) / 32;
+  const size_t cnt = (size_t)states * warps;
+  int* d = nullptr;
+  CK(cudaMalloc((void**)&d, cnt * sizeof(int)));
+  std::vector<int> h(cnt);
+  cudaError_t e = sws::launch_count_near(c, states, d, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h.data(), d, cnt * sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d);
+  CK(e);
+  double near = 0.0;
+  for (size_t i = 0; i < cnt; ++i) near += h[i];
+  *near_fraction = near / ((double)cnt * c->mesh.N);
   return SWS_OK;
 }
 
@@ -571,6 +600,23 @@ int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, i
   CK(cudaMemcpy(y_host, y, (size_t)n * 8, cudaMemcpyDeviceToHost));
   cudaFree(x);
   cudaFree(y);
+  return SWS_OK;
+}
+
+int sws_debug_s2col_host(int32_t device, double y1, double dy, int32_t M, const double* c_host,
+                         const double* g_host, int32_t n, double* direct_host, double* em_host) {
+  if (!c_host || !g_host || !direct_host || !em_host || n < 1 || M < 2 || !(dy > 0.0)) return SWS_EINVAL;
+  CK(cudaSetDevice(device));
+  double* d = nullptr;
+  const size_t nb = (size_t)n * 8;
+  CK(cudaMalloc((void**)&d, 4 * nb));
+  CK(cudaMemcpy(d, c_host, nb, cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(d + n, g_host, nb, cudaMemcpyHostToDevice));
+  cudaError_t e = sws::launch_debug_s2col(y1, dy, M, d, d + n, n, d + 2 * (size_t)n, d + 3 * (size_t)n, 0);
+  if (e == cudaSuccess) e = cudaMemcpy(direct_host, d + 2 * (size_t)n, nb, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(em_host, d + 3 * (size_t)n, nb, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  CK(e);
   return SWS_OK;
 }
 

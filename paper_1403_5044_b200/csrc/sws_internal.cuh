@@ -62,6 +62,7 @@ struct PairPlan {
 constexpr int kPairThreads = 128;  // threads (= targets) per CTA of the all-pairs kernel
 constexpr int kSegMax = 256;       // max nodes staged per bulk copy (10 KB per stage)
 constexpr int kStages = 2;         // staging ring depth
+constexpr double kEmRadius = 8.0;  // default far-field radius of the S2 column sums, in units of dy
 constexpr int kNormBlocks = 64;    // partial blocks of the 2-norm reductions
 
 }  // namespace sws
@@ -73,6 +74,7 @@ struct sws_ctx {
   int sm_count;
   int max_states;       // max_batch + 1
   int chunks_user;      // 0 = auto
+  double em_radius;     // far-field radius r of the S2 column sums in units of dy (<= 0: all direct)
   size_t ws_bytes;
   int last_launches;
   int last_states;      // states the workspace fields currently describe
@@ -140,6 +142,9 @@ cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, do
                            cudaStream_t st);
 // dispatches on sws_params.precision (0: FP64 kernel, 1: FP32 pair arithmetic)
 cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
+cudaError_t launch_count_near(sws_ctx* c, int states, int* out, cudaStream_t st);
+cudaError_t launch_debug_s2col(double y1, double dy, int M, const double* cc, const double* g, int n,
+                               double* out_direct, double* out_em, cudaStream_t st);
 cudaError_t launch_allpairs_f32(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
 cudaError_t launch_assemble(sws_ctx* c, int states, const PairPlan& plan, double* F0,
                             double* Fpert, cudaStream_t st);

@@ -128,6 +128,68 @@ def test_chunking_invariance_and_determinism(sws, oracle80):
         torch.cuda.synchronize()
 
 
+def _column_sum_longdouble(y1, dy, M, c, g):
+    """sum_j c_j [((y_j-c)^2+g)^-1/2 + ((y_j+c)^2+g)^-1/2], c_j = 1/2 at both ends, term by term."""
+    y = (np.longdouble(y1) + np.arange(M, dtype=np.longdouble) * np.longdouble(dy))[None, :]
+    c = c.astype(np.longdouble)[:, None]
+    g = g.astype(np.longdouble)[:, None]
+    v = 1.0 / np.sqrt((y - c) ** 2 + g) + 1.0 / np.sqrt((y + c) ** 2 + g)
+    v[:, 0] *= 0.5
+    v[:, -1] *= 0.5
+    return v.sum(axis=1)
+
+
+@pytest.mark.parametrize("y1,dy,M", [(0.0, 0.075, 241), (0.0, 0.8, 11), (0.8, 0.4, 12), (0.0, 0.05, 601),
+                                     (0.0, 0.5, 4), (1.3, 0.3, 2)])
+def test_farfield_expansion_primitive(sws, y1, dy, M):
+    """The Euler-Maclaurin form of an S2 column sum (sws_allpairs.cu) against the plain
+    trapezoid sum in long double, for sqrt(g) from the switch-over radius 8 dy upwards and c
+    (the completed-square centre) inside, at the ends of and outside the column."""
+    rng = np.random.default_rng(5)
+    n = 4000
+    yM = y1 + (M - 1) * dy
+    c = np.concatenate([rng.uniform(-yM - 5, yM + 5, n - 6), [y1, yM, -yM, 0.0, 0.5 * (y1 + yM), yM + 40.0]])
+    r = np.concatenate([np.full(n // 4, 8.0), rng.uniform(8.0, 12.0, n // 4), 10 ** rng.uniform(0.9, 2.9, n - 2 * (n // 4))])
+    g = (r * dy) ** 2
+    direct, em = sws.debug_s2col(y1, dy, M, c, g)
+    ref = _column_sum_longdouble(y1, dy, M, c, g)
+    scale = np.maximum(np.abs(ref), 1.0 / (r * dy) / dy).astype(np.float64)
+    err_em = np.abs((em.astype(np.longdouble) - ref).astype(np.float64)) / scale
+    err_direct = np.abs((direct.astype(np.longdouble) - ref).astype(np.float64)) / scale
+    assert err_direct.max() <= 1e-13          # the device's own term-by-term sum
+    assert err_em.max() <= 4e-15, (err_em.max(), c[err_em.argmax()], r[err_em.argmax()])
+
+
+@pytest.mark.parametrize("name", ["cfg3", "ragged_y1", "steep"])
+def test_farfield_on_off_equivalence(sws, oracle80, name):
+    """sws_set_farfield(0) sums every S2 term pair by pair (the plain definition); the default
+    (radius 8 dy) must give the same residual to summation round-off, and both match the oracle."""
+    if name == "cfg3":
+        cfg = W.CONFIGS[2]
+        u = W.state(cfg)
+    elif name == "ragged_y1":
+        cfg = W.custom(eps=0.3, amp=0.05, N=90, M=40, h=0.2, x1=-4.0, y1=0.6, seed=21)
+        u = W.state(cfg) + 1e-3 * np.random.default_rng(3).standard_normal(cfg.n)
+    else:  # steep surface: zeta_x*, zeta_y* of order one move A, B, C (and the radius in columns) a lot
+        cfg = W.custom(eps=0.5, amp=1.5, N=120, M=50, h=0.15, x1=-2.0, seed=22)
+        u = W.state(cfg)
+    E = oracle80.residual(cfg.params(), u)
+    with sws.Context(cfg.params()) as ctx:
+        F_on = ctx.residual(dev(u)).cpu().numpy()
+        near = ctx.farfield_stats(1)
+        ctx.set_farfield(0.0)
+        F_off = ctx.residual(dev(u)).cpu().numpy()
+        assert ctx.farfield_stats(1) == 1.0
+        ctx.set_farfield(12.0)
+        F_12 = ctx.residual(dev(u)).cpu().numpy()
+        with pytest.raises(sws.SwsError):
+            ctx.set_farfield(3.0)
+    assert 0.0 < near < 1.0
+    assert relerr(F_on, F_off) <= 2e-13
+    assert relerr(F_12, F_off) <= 2e-13
+    assert relerr(F_on, E) <= TOL and relerr(F_off, E) <= TOL
+
+
 @pytest.mark.parametrize("i,rows", [(3, 192), (4, 96)])
 def test_large_configs_sampled_rows(sws, oracle80, i, rows):
     """cfg 4 and cfg 5 at full size in the launch configuration bench.py times: the O(NM) rows
