@@ -45,8 +45,8 @@ FP64_INSTR_NEAR, FLOPS_NEAR = 45, 68
 FP64_INSTR_FAR, FLOPS_FAR = 29, 44
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
 # dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
-# ncu --set full capture summarised in profiles/r1_allpairs_ncu.md (algorithmic: 16.67 MB)
-NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 16.813e6}
+# ncu --set full capture summarised in profiles/r1b_allpairs_ncu.md (algorithmic: 16.67 MB)
+NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 16.903e6}
 
 
 def dist_env():
@@ -203,8 +203,8 @@ def fp32_variant_report(sws, device: int, names=("cfg4_361x121",), steps: int = 
                      "allpairs_pairs_per_s": (b + 1) * cfg.pairs / (ap_ms * 1e-3),
                      "max_rel_err_vs_fp64_path": err}
     out["note"] = ("precision=1: FP32 pair arithmetic (packed f32x2, MUFU.RSQ), FP32 accumulation per source "
-                   "column, FP64 across columns and everywhere outside the all-pairs kernel; bound by the XU "
-                   "pipe (4 MUFU.RSQ per pair); reported, not part of `value`")
+                   "column, FP64 across columns, for the far-field S2 column sums and everywhere outside the "
+                   "all-pairs kernel; reported, not part of `value`")
     return out
 
 
@@ -429,7 +429,7 @@ def run_ours(args) -> None:
     roofline = {
         "bound": "alu", "kernel": "k_allpairs", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
         "frac": achieved_tf / peak_tf, "traffic": NCU_DRAM_BYTES_PER_STATE_LAUNCH.get(cfg.name),
-        "traffic_note": "DRAM bytes per state per all-pairs launch, ncu capture profiles/r1_allpairs_ncu.md; "
+        "traffic_note": "DRAM bytes per state per all-pairs launch, ncu capture profiles/r1b_allpairs_ncu.md; "
                         "algorithmic = S*32 + T*64 bytes read once",
         "algorithmic_bytes_per_state": cfg.sources * 32 + cfg.targets * 64,
         "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz "

@@ -32,7 +32,7 @@ def needs_build() -> bool:
     if not LIB.exists() or not LIB_JFNK.exists():
         return True
     t = min(LIB.stat().st_mtime, LIB_JFNK.stat().st_mtime)
-    deps = [CSRC / s for s in SOURCES + SOURCES_JFNK] + [CSRC / "sws_internal.cuh", CSRC / "sws_stage.cuh",
+    deps = [CSRC / s for s in SOURCES + SOURCES_JFNK] + [CSRC / "sws_internal.cuh", CSRC / "sws_stage.cuh", CSRC / "sws_farfield.cuh",
                                                          CSRC / "jfnk_internal.cuh", ROOT / "include" / "sws.h",
                                                          ROOT / "include" / "sws_jfnk.h"]
     return any(d.stat().st_mtime > t for d in deps)

@@ -16,6 +16,7 @@
 // inner loop carries no weight multiply.  Partial sums per (state, chunk, target) are
 // written to global memory and added in a fixed order by the assemble kernel: no atomics,
 // bitwise repeatable.
+#include "sws_farfield.cuh"
 #include "sws_internal.cuh"
 #include "sws_stage.cuh"
 
@@ -30,33 +31,6 @@
 namespace sws {
 
 constexpr int kUnroll = SWS_UNROLL;
-
-// 1/sqrt(x) for normal positive x, full double precision.
-// Seed: MUFU.RSQ64H (PTX rsqrt.approx.ftz.f64: works on the upper 32 bits of x, so the seed
-// carries a relative error d with |d| < ~2^-20).  With e = 1 - x y0^2 (= -2d - d^2) the
-// exact result is y0 (1 - e)^(-1/2) = y0 (1 + e/2 + 3e^2/8 + 5e^3/16 + ...); the two-term
-// correction below leaves 5/16 |e|^3 < 2^-59, i.e. below the rounding of the final FMA.
-// 5 FP64 instructions (DMUL, DFMA, DFMA, DMUL, DFMA) + 1 MUFU.
-//
-// Operand shapes matter on B200: a DFMA with three DISTINCT register sources issues every
-// 3 cycles per SM sub-partition, one with <= 2 distinct registers (a repeated operand, an
-// immediate) every 2 (measured).  Every step
-// here is written with at most two distinct registers: the last one is
-// y0 + y0 * (e p) = fma(y0, e p, y0), not fma(y0 e, p, y0).
-__device__ __forceinline__ double rsqrt_seed(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  return y;
-}
-
-__device__ __forceinline__ double rsqrt_fp64(double x) {
-  const double y0 = rsqrt_seed(x);
-  const double t = x * y0;
-  const double e = fma(-t, y0, 1.0);
-  const double p = fma(0.375, e, 0.5);
-  const double w = e * p;
-  return fma(y0, w, y0);
-}
 
 // Per-thread constants of one target and of the current source column.
 // The S2 quadratic forms are used with the square completed (C > 0):
@@ -105,86 +79,6 @@ __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, co
     const double Qp = fma(sp, sp, c.g);
     aS += rsqrt_fp64(Qm) + rsqrt_fp64(Qp);
   }
-}
-
-// ---------------------------------------------------------------------------------------
-// Far-field form of the S2 column sums.
-//
-// For one target and one source column the S2 terms of the quadrature are, up to 1/sqrt(C),
-//     sum_j c_j [ f(y_j; c) + f(y_j; -c) ],   f(y; c) = ((y - c)^2 + g)^(-1/2),
-// a composite trapezoid sum (step dy, c_j = 1/2 at both ends, reading Q4) of a function that
-// does NOT depend on the source data: c and g depend on the target's A, B, C and on x_i - x*
-// only.  f is analytic with its nearest singularities at y = c +- i sqrt(g), sqrt(g) ~ |x_i - x*|,
-// so once sqrt(g) >= r dy the sum equals its Euler-Maclaurin expansion to round-off:
-//     dy sum_j c_j f(y_j) = int_a^b f dy + sum_{k=1..K} B_2k dy^2k / (2k)! (f^(2k-1)(b) - f^(2k-1)(a)) + R_K,
-//     int f dy = asinh((y - c) / sqrt(g)),
-//     f^(n)(y) = (-1)^n n! P_n(mu) / rho^(n+1),  rho = sqrt((y-c)^2 + g), mu = (y - c) / rho
-// (P_n = Legendre polynomial: 1/rho is the generating function of P_n), i.e. the k-th term is
-//     -(B_2k / 2k) (dy / rho)^2k P_{2k-1}(mu)  at b minus the same at a.
-// With K = 7 and r = 8 the remainder is < 1e-16 / sqrt(g) (measured against 50-digit sums over
-// the whole range of c), below the rounding of the direct sum itself.
-// The same quantity, evaluated another way: the result still matches the oracle's plain sum.
-// Cost: ~120 FP64 instructions per (target, column) instead of 16 per pair.
-// (default r = kEmRadius of sws_internal.cuh; sws_set_farfield changes it, r <= 0 sums directly)
-
-// sum_{k=1..7} (B_2k / 2k) s^k P_{2k-1}(mu) at the end point u = y_e - c;  *rho = sqrt(u^2 + g)
-__device__ __forceinline__ double em_tail(const double u, const double g, const double h2, double* rho) {
-  const double r2 = fma(u, u, g);
-  const double ri = rsqrt_fp64(r2);
-  *rho = r2 * ri;
-  const double mu = u * ri;
-  const double s = h2 * (ri * ri);
-  double P[14];
-  P[0] = 1.0;
-  P[1] = mu;
-#pragma unroll
-  for (int n = 1; n <= 12; ++n)  // (n+1) P_{n+1} = (2n+1) mu P_n - n P_{n-1}
-    P[n + 1] = ((2.0 * n + 1.0) / (n + 1.0)) * (mu * P[n]) - (n / (n + 1.0)) * P[n - 1];
-  double t = (1.0 / 12.0) * P[13];              // B_14 / 14
-  t = fma(s, t, (-691.0 / 32760.0) * P[11]);    // B_12 / 12
-  t = fma(s, t, (1.0 / 132.0) * P[9]);          // B_10 / 10
-  t = fma(s, t, (-1.0 / 240.0) * P[7]);         // B_8 / 8
-  t = fma(s, t, (1.0 / 252.0) * P[5]);          // B_6 / 6
-  t = fma(s, t, (-1.0 / 120.0) * P[3]);         // B_4 / 4
-  t = fma(s, t, (1.0 / 12.0) * P[1]);           // B_2 / 2
-  return s * t;
-}
-
-// dy * (trapezoid sum of f(.; c) over the nodes a, a + dy, ..., b), by the expansion above
-__device__ __forceinline__ double em_interval(const double a, const double b, const double c, const double g,
-                                              const double h2) {
-  const double ua = a - c, ub = b - c;
-  double rhoa, rhob;
-  const double ta = em_tail(ua, g, h2, &rhoa);
-  const double tb = em_tail(ub, g, h2, &rhob);
-  // asinh(ub / sqrt g) - asinh(ua / sqrt g) = log(q),  q = L(ub) / L(ua),  L(u) = u + rho = g / (rho - u),
-  // each L taken in the form without cancellation.  q - 1 = (L(ub) - L(ua)) / L(ua) with
-  // L(ub) - L(ua) = (b - a) (L(ua) + L(ub)) / (rho_a + rho_b), so log(q) = log1p((b - a)(1 + q) / (rho_a + rho_b))
-  // keeps full relative accuracy when the interval is short against sqrt(g) (q -> 1).
-  const double nb = ub >= 0.0 ? ub + rhob : g, db = ub >= 0.0 ? 1.0 : rhob - ub;
-  const double na = ua >= 0.0 ? ua + rhoa : g, da = ua >= 0.0 ? 1.0 : rhoa - ua;
-  const double q = (nb * da) / (db * na);
-  return log1p((b - a) * (1.0 + q) / (rhoa + rhob)) - (tb - ta);
-}
-
-struct EmGeom {
-  double y1, yM;   // first and last node of a column
-  double h2, inv_h;  // dy^2, 1 / dy
-  double gmin;     // (r dy)^2; a column is "far" for a target when g >= gmin  (inf: never)
-  int sym;         // y1 == 0: direct + image = one trapezoid sum over [-yM, yM]
-};
-
-// sum_j c_j [ f(y_j; c) + f(y_j; -c) ]  (unit node weights, as the direct loop accumulates it)
-__device__ __forceinline__ double s2_column_em(const EmGeom& e, const double c, const double g) {
-  const double v = e.sym ? em_interval(-e.yM, e.yM, c, g, e.h2)
-                         : em_interval(e.y1, e.yM, c, g, e.h2) + em_interval(e.y1, e.yM, -c, g, e.h2);
-  return v * e.inv_h;
-}
-
-// The far/near decision is taken per WARP (all 32 targets of the warp must be far), so the j loop
-// has no divergence.  Used by k_allpairs and by the counting kernel of sws_farfield_stats.
-__device__ __forceinline__ bool column_is_far(const double g, const double gmin) {
-  return __all_sync(0xffffffffu, g >= gmin) != 0;
 }
 
 // One staged segment [j0, j0 + len) of a column: trapezoid half weights on the column's first and
@@ -306,19 +200,6 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
 
 // ---------------------------------------------------------------------------------------
 // host side
-
-static EmGeom em_geometry(const sws_ctx* c) {
-  const Mesh& m = c->mesh;
-  EmGeom e;
-  e.y1 = m.y1;
-  e.yM = m.y1 + (m.M - 1) * m.dy;
-  e.h2 = m.dy * m.dy;
-  e.inv_h = 1.0 / m.dy;
-  const double r = c->em_radius;
-  e.gmin = r > 0.0 ? (r * m.dy) * (r * m.dy) : __builtin_inf();
-  e.sym = m.sym_first;
-  return e;
-}
 
 constexpr int kMinB = SWS_MINB;
 

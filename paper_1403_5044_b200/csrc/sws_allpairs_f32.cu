@@ -15,9 +15,14 @@
 //     per-(state, column group, target) partial goes to the same `part` buffer, so
 //     everything outside a4 is the FP64 path unchanged.
 //
-// Bound: the XU pipe (4 MUFU.RSQ per pair, 16 results per clock per SM), not the FP64 pipe.
+//   * far columns (sws_farfield.cuh: sqrt(g) >= r dy for the whole warp) take their S2 column sum
+//     from the FP64 Euler-Maclaurin form, exactly as the FP64 kernel does: the FP64 pipe is
+//     idle here, and the pair loop drops to 2 MUFU.RSQ per pair.
+//
+// Bound: the XU pipe (4 MUFU.RSQ per near pair, 2 per far pair; 16 results per clock per SM), not the FP64 pipe.
 // The variant is reported, never gated: tests/test_gpu_parity.py measures its error against
 // the FP64 oracle.
+#include "sws_farfield.cuh"
 #include "sws_internal.cuh"
 #include "sws_stage.cuh"
 
@@ -78,6 +83,7 @@ struct ColF {
 // One source node against one target.  ra = {z_hi, z_lo, psi, psi}, rb = {zx, zx, -zy, -zy};
 // t2 = (j - l, j + l) as floats.  Adds the K1/K2 terms to a1 (lanes summed later) and
 // sqrt(C) S2 to aS.
+template <bool S2T>
 __device__ __forceinline__ void pair_f32(const float4 ra, const float4 rb, const u64 t2,
                                          const TgtF& t, const ColF& c, u64& a1, u64& aS) {
   const u64 dmp = fma2(t2, t.dy2, t.off2);  // (y - y*, y + y*)
@@ -94,8 +100,40 @@ __device__ __forceinline__ void pair_f32(const float4 ra, const float4 rb, const
   const u64 r3 = mul2(mul2(r, r), r);
   a1 = fma2(dpsi2, mul2(nmp, r3), a1);  // (phi - phi* - x + x*) K1
   a1 = fma2(pk(rb.x, rb.y), r, a1);     // zeta_x K2
-  const u64 smp = add2(dmp, c.kb2);
-  aS = add2(aS, rsq2(fma2(smp, smp, c.g2)));  // S2 up to 1/sqrt(C)
+  if (S2T) {
+    const u64 smp = add2(dmp, c.kb2);
+    aS = add2(aS, rsq2(fma2(smp, smp, c.g2)));  // S2 up to 1/sqrt(C)
+  }
+}
+
+// One staged segment of a column: half weights on the column's first and last node (Q4).
+template <bool S2T>
+__device__ __forceinline__ void walk_f32(const float4* rec, const int j0, const int len, const int M, const int l,
+                                         const TgtF& tg, const ColF& cc, u64& col1, u64& colS) {
+  const u64 one2 = pk(1.f, 1.f), half2 = pk(.5f, .5f), zero2 = pk(0.f, 0.f);
+  u64 t2 = pk((float)(j0 - l), (float)(j0 + l));
+  int jlo = 0, jhi = len;
+  if (j0 == 0) {  // first node of the column: weight 1/2 in y
+    u64 h1 = zero2, hS = zero2;
+    pair_f32<S2T>(rec[0], rec[1], t2, tg, cc, h1, hS);
+    col1 = mul2(half2, h1);
+    colS = mul2(half2, hS);
+    t2 = add2(t2, one2);
+    jlo = 1;
+  }
+  const bool last = (j0 + len == M);
+  if (last) jhi = len - 1;
+#pragma unroll 4
+  for (int j = jlo; j < jhi; ++j) {
+    pair_f32<S2T>(rec[2 * j], rec[2 * j + 1], t2, tg, cc, col1, colS);
+    t2 = add2(t2, one2);
+  }
+  if (last && jhi >= jlo) {  // last node of the column: weight 1/2 in y
+    u64 h1 = zero2, hS = zero2;
+    pair_f32<S2T>(rec[2 * jhi], rec[2 * jhi + 1], t2, tg, cc, h1, hS);
+    col1 = fma2(half2, h1, col1);
+    colS = fma2(half2, hS, colS);
+  }
 }
 
 __device__ __forceinline__ double lanes_sum(u64 v) {
@@ -114,6 +152,7 @@ struct PairArgsF {
   int N, M, T;
   int chunks, cols_per_chunk, seg_len, nseg;
   double dxdy, dy, y1;
+  EmGeom em;
 };
 
 __global__ void __launch_bounds__(kPairThreads, 8) k_allpairs_f32(const PairArgsF a) {
@@ -141,7 +180,7 @@ __global__ void __launch_bounds__(kPairThreads, 8) k_allpairs_f32(const PairArgs
     tg.dy2 = pk(dyf, dyf);
     tg.off2 = pk(0.f, (float)(2.0 * a.y1));
   }
-  const u64 one2 = pk(1.f, 1.f), half2 = pk(.5f, .5f), zero2 = pk(0.f, 0.f);
+  const u64 zero2 = pk(0.f, 0.f);
 
   const int c0 = chunk * a.cols_per_chunk;
   const int c1 = min(a.N, c0 + a.cols_per_chunk);
@@ -173,9 +212,10 @@ __global__ void __launch_bounds__(kPairThreads, 8) k_allpairs_f32(const PairArgs
     const int i = c0 + q / a.nseg, j0 = (q % a.nseg) * a.seg_len;
     const int len = min(a.seg_len, a.M - j0);
     ColF cc;
+    const double dxd = __ldg(a.x + i) - xs, dxd2 = dxd * dxd;
+    const double gd = kg * dxd2;  // the S2 constants of sws_allpairs.cu, in FP64 for the far-field form
     {
-      const double dxd = __ldg(a.x + i) - xs, dxd2 = dxd * dxd;
-      const float kbdx = (float)(kb * dxd), g = (float)(kg * dxd2);
+      const float kbdx = (float)(kb * dxd), g = (float)gd;
       cc.ndx = -(float)dxd;
       cc.dx2 = (float)dxd2;
       cc.kb2 = pk(kbdx, -kbdx);
@@ -187,31 +227,16 @@ __global__ void __launch_bounds__(kPairThreads, 8) k_allpairs_f32(const PairArgs
 
     const float4* rec = reinterpret_cast<const float4*>(s_rec + (size_t)s * seg_pad);
     u64 col1 = zero2, colS = zero2;
-    u64 t2 = pk((float)(j0 - l), (float)(j0 + l));
-    int jlo = 0, jhi = len;
-    if (j0 == 0) {  // first node of the column: weight 1/2 in y
-      u64 h1 = zero2, hS = zero2;
-      pair_f32(rec[0], rec[1], t2, tg, cc, h1, hS);
-      col1 = mul2(half2, h1);
-      colS = mul2(half2, hS);
-      t2 = add2(t2, one2);
-      jlo = 1;
-    }
-    const bool last = (j0 + len == a.M);
-    if (last) jhi = len - 1;
-#pragma unroll 4
-    for (int j = jlo; j < jhi; ++j) {
-      pair_f32(rec[2 * j], rec[2 * j + 1], t2, tg, cc, col1, colS);
-      t2 = add2(t2, one2);
-    }
-    if (last && jhi >= jlo) {  // last node of the column: weight 1/2 in y
-      u64 h1 = zero2, hS = zero2;
-      pair_f32(rec[2 * jhi], rec[2 * jhi + 1], t2, tg, cc, h1, hS);
-      col1 = fma2(half2, h1, col1);
-      colS = fma2(half2, hS, colS);
+    double colS_far = 0.0;
+    if (column_is_far(gd, a.em.gmin)) {  // warp-uniform
+      walk_f32<false>(rec, j0, len, a.M, l, tg, cc, col1, colS);
+      colS = zero2;
+      if (j0 == 0) colS_far = s2_column_em(a.em, fma(-kb, dxd, tr.ys), gd);
+    } else {
+      walk_f32<true>(rec, j0, len, a.M, l, tg, cc, col1, colS);
     }
     tot1 = fma(ci, lanes_sum(col1), tot1);  // columns are added in FP64
-    totS = fma(ci, lanes_sum(colS), totS);
+    totS = fma(ci, lanes_sum(colS) + colS_far, totS);
     __syncthreads();
   }
 
@@ -247,6 +272,7 @@ cudaError_t launch_allpairs_f32(sws_ctx* c, int states, const PairPlan& plan, cu
   a.chunks = plan.chunks; a.cols_per_chunk = plan.cols_per_chunk;
   a.seg_len = plan.seg_len; a.nseg = plan.nseg;
   a.dxdy = m.dx * m.dy; a.dy = m.dy; a.y1 = m.y1;
+  a.em = em_geometry(c);
   dim3 grid(plan.tiles, plan.chunks, states);
   k_allpairs_f32<<<grid, kPairThreads, allpairs_f32_smem_bytes(plan.seg_len), st>>>(a);
   return cudaGetLastError();

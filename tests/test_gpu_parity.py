@@ -247,6 +247,37 @@ def test_jv_batch_parity(sws, oracle80, i):
     assert worst_jv <= 1e-5, worst_jv
 
 
+def test_jv_batch_cfg5_bench_configuration(sws, oracle80):
+    """The step bench.py times (cfg5, 721x241, b = 16, 17 states in one all-pairs launch): perturbed
+    residuals of the first and last direction on seeded rows the oracle computes one by one, at the
+    library's own shifts; the batch's F0 is bitwise sws_residual(u)."""
+    import torch
+    cfg = W.CONFIGS[4]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg)
+    b = V.shape[0]
+    assert b == 16
+    rng = np.random.default_rng(77)
+    T = cfg.targets
+    pick = np.unique(np.concatenate([rng.integers(0, T, 40), [0, T - 1, cfg.N - 2]])).astype(np.int32)
+    with sws.Context(p, max_batch=b) as ctx:
+        ud, Vd = dev(u), dev(V)
+        JV, Fp, F0 = ctx.jv_batch(ud, Vd, want_fpert=True, want_f0=True)
+        torch.cuda.synchronize()
+        sig = ctx.last_sigma(b)
+        F = ctx.residual(ud).cpu().numpy()
+        Fp, F0, JV = Fp.cpu().numpy(), F0.cpu().numpy(), JV.cpu().numpy()
+    assert np.array_equal(F0, F)
+    scale = np.abs(F).max()
+    for k in (0, b - 1):
+        s_ref = oracle80.sigma(u, V[k])
+        assert abs(sig[k] - s_ref) <= 1e-13 * s_ref
+        _, Ep = oracle80.jv(p, u, V[k], float(sig[k]), rows=pick)
+        mask = ~np.isnan(Ep)
+        assert mask.sum() >= (cfg.N + 1) * cfg.M + pick.size
+        assert np.abs(Fp[k][mask] - Ep[mask]).max() / scale <= TOL
+        assert np.array_equal(JV[k], (Fp[k] - F0) / sig[k])
+
+
 def test_host_api_matches_device_api(sws):
     cfg = W.CONFIGS[1]
     p, u, V = cfg.params(), W.state(cfg), W.directions(cfg, 3)
