@@ -65,7 +65,10 @@ typedef struct {
   double tol;       /* stop when ||rhs - J d||_2 <= tol ||rhs||_2 (Arnoldi estimate)          */
   int32_t restart;  /* Krylov dimension m before a restart (<= the solver's max_restart)      */
   int32_t maxit;    /* cap on Jacobian-vector products in total                              */
-  int32_t jv_mode;  /* 0 analytic J v (sws_jv_exact_batch); 1 eq. (25) with libsws's sigma   */
+  int32_t jv_mode;  /* 0 analytic J v (sws_linearize + sws_jv_apply); 1 eq. (25) through
+                       sws_jv_batch (base and shifted state evaluated per product); 2 eq. (25)
+                       with the base residual E(u) the driver already holds: ONE sws_residual
+                       per product, the paper's own scheme (L219), same shift sigma        */
 } sws_gmres_opts;
 
 typedef struct {

@@ -141,6 +141,7 @@ struct sws_solver {
   double* V;        // [m_max + 1][n] Krylov basis
   double *w, *z, *t, *r;
   double *E, *Et, *du, *ut, *rhs;
+  double *ub, *Eb;  // jv_mode 2: shifted state u + sigma v and E of it
   double* partial;  // [kDotBlocks][m_max + 2]
   double* hdev;     // [2 (m_max + 1) + 2]: h1 | h2 | normsq, scratch
   double* ydev;     // [m_max]
@@ -191,16 +192,56 @@ int apply_pinv(sws_solver* s, const double* v, double* out, cudaStream_t st) {
   return sws_precond_apply(s->pc, v, out, st);
 }
 
-int apply_jv(sws_solver* s, const double* u, const double* v, double* out, int mode, cudaStream_t st) {
+// ub = fma(sigma, v, u) entry by entry, as sws_jv_batch forms its shifted states
+__global__ void __launch_bounds__(256) k_shift(double* __restrict__ ub, double sigma, const double* __restrict__ v,
+                                               const double* __restrict__ u, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) ub[i] = fma(sigma, v[i], u[i]);
+}
+// out = (Eb - E0) / sigma, eq. (25)
+__global__ void __launch_bounds__(256) k_fd_quotient(double* __restrict__ out, const double* __restrict__ Eb,
+                                                     const double* __restrict__ E0, double sigma, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = (Eb[i] - E0[i]) / sigma;
+}
+
+// mode 2: eq. (25) with the base residual E0 = E(u) the caller already holds (the Newton driver's E_k):
+// one residual evaluation per product.  unorm = ||u||_2; the shift is libsws's 1e-7 (1 + ||u||) / ||v||.
+int apply_jv(sws_solver* s, const double* u, const double* v, double* out, int mode, cudaStream_t st,
+             const double* E0 = nullptr, double unorm = 0.0) {
   ++s->n_jv;
   if (mode == 1) return sws_jv_batch(s->ctx, u, v, 1, nullptr, out, nullptr, nullptr, st);
+  if (mode == 2) {
+    double vn = 0.0;
+    RC(norms(s, v, &vn, nullptr, st));
+    if (vn == 0.0) {
+      CU(cudaMemsetAsync(out, 0, sizeof(double) * s->n, st));
+      return SWS_OK;
+    }
+    const double sigma = 1e-7 * (1.0 + unorm) / vn;
+    k_shift<<<nblk(s->n), 256, 0, st>>>(s->ub, sigma, v, u, s->n);
+    ++s->n_res;
+    RC(sws_residual(s->ctx, s->ub, s->Eb, st));
+    k_fd_quotient<<<nblk(s->n), 256, 0, st>>>(out, s->Eb, E0, sigma, s->n);
+    return SWS_OK;
+  }
   return sws_jv_apply(s->ctx, v, 1, out, st);  // the linearisation at u was formed by gmres()
 }
 
+// E0: E(u) if the caller has it (jv_mode 2 only; computed here otherwise)
 int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opts* o, double* d,
-          sws_gmres_stats* stats, double* hist, cudaStream_t st) {
+          sws_gmres_stats* stats, double* hist, cudaStream_t st, const double* E0 = nullptr) {
   const int n = s->n, m = o->restart;
-  if (m < 1 || m > s->m_max || o->maxit < 1) return SWS_EINVAL;
+  if (m < 1 || m > s->m_max || o->maxit < 1 || o->jv_mode < 0 || o->jv_mode > 2) return SWS_EINVAL;
+  double unorm = 0.0;
+  if (o->jv_mode == 2) {
+    RC(norms(s, u, &unorm, nullptr, st));
+    if (!E0) {  // standalone solve: the base residual, once
+      ++s->n_res;
+      RC(sws_residual(s->ctx, u, s->Et, st));
+      E0 = s->Et;
+    }
+  }
   const size_t ld = (size_t)n;
   double bnorm = 0.0;
   RC(norms(s, rhs, &bnorm, nullptr, st));
@@ -238,7 +279,7 @@ int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opt
       CU(cudaEventRecord(s->ev[0], st));
       RC(apply_pinv(s, s->V + (size_t)j * ld, s->z, st));
       CU(cudaEventRecord(s->ev[1], st));
-      RC(apply_jv(s, u, s->z, s->w, o->jv_mode, st));
+      RC(apply_jv(s, u, s->z, s->w, o->jv_mode, st, E0, unorm));
       CU(cudaEventRecord(s->ev[2], st));
       ++its;
       // classical Gram-Schmidt, twice
@@ -289,7 +330,7 @@ int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opt
     CU(cudaStreamSynchronize(st));  // y is host memory reused by the next cycle
     if (rel <= o->tol || its >= o->maxit) break;
     // restart: r = rhs - J d
-    RC(apply_jv(s, u, d, s->w, o->jv_mode, st));
+    RC(apply_jv(s, u, d, s->w, o->jv_mode, st, E0, unorm));
     k_axpby<<<nblk(n), 256, 0, st>>>(s->r, 1.0, rhs, -1.0, s->w, n);
   }
   stats->its = its;
@@ -337,7 +378,7 @@ int sws_solver_create(sws_ctx* ctx, sws_precond* pc, int32_t max_restart, sws_so
   reset_accounting(s);
   const size_t n = (size_t)s->n;
   double* base = nullptr;
-  const size_t vec = (size_t)(max_restart + 1) + 9;
+  const size_t vec = (size_t)(max_restart + 1) + 11;
   cudaError_t e = cudaSetDevice(p.device);
   if (e == cudaSuccess) e = cudaMalloc(&base, vec * n * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&s->partial, sizeof(double) * kDotBlocks * (max_restart + 2));
@@ -354,6 +395,7 @@ int sws_solver_create(sws_ctx* ctx, sws_precond* pc, int32_t max_restart, sws_so
   double* q = base + (size_t)(max_restart + 1) * n;
   s->w = q; s->z = q + n; s->t = q + 2 * n; s->r = q + 3 * n;
   s->E = q + 4 * n; s->Et = q + 5 * n; s->du = q + 6 * n; s->ut = q + 7 * n; s->rhs = q + 8 * n;
+  s->ub = q + 9 * n; s->Eb = q + 10 * n;
   *out = s;
   return SWS_OK;
 }
@@ -386,7 +428,7 @@ int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sw
     if (finf <= o->ftol) { converged = 1; break; }
     k_axpby<<<nblk(n), 256, 0, st>>>(s->rhs, -1.0, s->E, 0.0, s->E, n);
     sws_gmres_stats gs;
-    RC(gmres(s, u_dev, s->rhs, &go, s->du, &gs, nullptr, st));
+    RC(gmres(s, u_dev, s->rhs, &go, s->du, &gs, nullptr, st, s->E));
     double lam = 1.0, fnt = 0.0, finft = 0.0;
     bool ok = false;
     for (int hv = 0; hv <= o->max_halvings; ++hv) {

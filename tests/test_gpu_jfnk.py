@@ -166,6 +166,11 @@ def test_gmres_unpreconditioned_and_fd(mods, oracle64, oracleC):
         assert np.allclose(hist, np.array(h_ref), rtol=1e-5)
         d2, st2, hist2 = s.gmres(dev(u), dev(rhs), tol=1e-30, restart=20, maxit=20, jv_mode=1)
         assert np.allclose(hist2, np.array(h_ref), rtol=1e-3)     # first-order difference quotient
+        # jv_mode 2: the same quotient from ONE residual evaluation per product (base E(u) held by the driver)
+        d3, st3, hist3 = s.gmres(dev(u), dev(rhs), tol=1e-30, restart=20, maxit=20, jv_mode=2)
+        assert st3["its"] == 20
+        assert np.allclose(hist3, hist2, rtol=1e-5)
+        assert np.abs((d3 - d2).cpu().numpy()).max() <= 1e-5 * np.abs(d_ref).max()
         # zero right-hand side
         import torch
         d0, st0, _ = s.gmres(dev(u), torch.zeros_like(dev(u)), tol=1e-8, maxit=5)
@@ -217,6 +222,11 @@ def test_newton_paper_mesh_91x31(mods, oracle64):
         u2, log2, st2 = s.newton(u0, ftol=1e-8, eta=1e-3, restart=40, gmres_maxit=80, jv_mode=1)
         assert st2["converged"]
         assert np.abs(u2.cpu().numpy() - un).max() <= 1e-6
+        u4, log4, st4 = s.newton(u0, ftol=1e-8, eta=1e-3, restart=40, gmres_maxit=80, jv_mode=2)
+        assert st4["converged"]
+        assert np.abs(u4.cpu().numpy() - un).max() <= 1e-6
+        # one residual per product + one per Newton step (+ the initial one)
+        assert st4["residual_evals"] == 1 + st4["steps"] + st4["jv_products"]
         # deterministic
         u3, _, _ = s.newton(u0, ftol=1e-10, eta=1e-3, restart=40, gmres_maxit=80)
         assert np.array_equal(u3.cpu().numpy(), un)
