@@ -85,6 +85,11 @@ typedef struct {
   int32_t max_newton;   /* cap on Newton steps                                               */
   int32_t max_halvings; /* cap on lam = 1, 1/2, 1/4, ...                                     */
   sws_gmres_opts gmres; /* tol is overridden by eta                                          */
+  int32_t forcing;      /* 0: every inner solve to eta.  1: forcing term "choice 2" of Eisenstat &
+                           Walker as in the survey the paper cites for its inexact Newton method
+                           ([21], L223): eta_0 = eta_max, eta_k = 0.9 (||E_k||/||E_{k-1}||)^2,
+                           raised to 0.9 eta_{k-1}^2 when that exceeds 0.1, clipped to [eta, eta_max] */
+  double eta_max;       /* forcing = 1 only (0 < eta <= eta_max < 1)                         */
 } sws_newton_opts;
 
 typedef struct {

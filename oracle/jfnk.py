@@ -209,22 +209,28 @@ def gmres_right(apply_J, apply_Pinv, rhs, tol: float, restart: int, maxit: int):
 
 
 def newton(residual, jv, apply_Pinv, u0, *, ftol: float, eta: float, restart: int, gmres_maxit: int,
-           max_newton: int = 30, alpha: float = 1e-4, max_halvings: int = 20):
+           max_newton: int = 30, alpha: float = 1e-4, max_halvings: int = 20, forcing: int = 0,
+           eta_max: float = 0.5):
     """Damped Newton iteration (2), (3) L41-45 with the simple line search of L209: lambda = 1,
     1/2, 1/4, ... until ||E(u + lambda du)||_2 < (1 - alpha lambda) ||E(u)||_2 (reading Q14: the
     paper only asks for a sufficient decrease; it used KINSOL's line search, L255).  The Newton
     correction solves J(u_k) du = -E(u_k) approximately (inexact Newton, L223) by `gmres_right`
     to the relative tolerance eta.  Stops when ||E||_inf <= ftol.
+    forcing = 1: the tolerance of step k follows the nonlinear progress (the forcing term "choice 2" of
+    Eisenstat & Walker as stated in the survey the paper cites for its inexact Newton method, [21] L223,
+    L372): eta_0 = eta_max, eta_k = 0.9 (||E_k|| / ||E_{k-1}||)^2, raised to 0.9 eta_{k-1}^2 when that
+    exceeds 0.1 (safeguard), then clipped to [eta, eta_max].
       residual(u) -> E(u);   jv(u, v) -> J(u) v.
     Returns (u, log) with one log entry per Newton step."""
     u = np.array(u0, dtype=np.float64)
     E = residual(u)
     log = []
+    eta_k = eta_max if forcing == 1 else eta
     for it in range(max_newton):
         fn = float(np.linalg.norm(E))
         if float(np.abs(E).max()) <= ftol:
             break
-        du, hist = gmres_right(lambda v: jv(u, v), apply_Pinv, -E, eta, restart, gmres_maxit)
+        du, hist = gmres_right(lambda v: jv(u, v), apply_Pinv, -E, eta_k, restart, gmres_maxit)
         lam, ok = 1.0, False
         for _ in range(max_halvings + 1):
             Et = residual(u + lam * du)
@@ -238,6 +244,13 @@ def newton(residual, jv, apply_Pinv, u0, *, ftol: float, eta: float, restart: in
             break
         u = u + lam * du
         E = Et
+        if forcing == 1:
+            fnt = float(np.linalg.norm(E))
+            e = 0.9 * (fnt / fn) ** 2
+            sg = 0.9 * eta_k * eta_k
+            if sg > 0.1:
+                e = max(e, sg)
+            eta_k = min(eta_max, max(e, eta))
     log.append({"newton": len(log), "fnorm": float(np.linalg.norm(E)), "finf": float(np.abs(E).max()),
                 "gmres_its": 0, "gmres_rel": 0.0, "lambda": 0.0})
     return u, log

@@ -9,6 +9,7 @@
 // Gram-Schmidt applied twice (two fused multi-dot + multi-axpy passes instead of j dependent
 // dot products), which spans the same Krylov space as the textbook modified Gram-Schmidt.
 // All reductions have a fixed order (per-CTA partials, then a serial sum): deterministic.
+#include <algorithm>
 #include <chrono>
 #include <cmath>
 #include <cstdio>
@@ -412,13 +413,15 @@ int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sw
                       sws_newton_stats* stats, void* cuda_stream) {
   if (!s || !u_dev || !o || !log || !nlog || !stats) return SWS_EINVAL;
   if (o->max_newton < 0 || o->max_halvings < 0) return SWS_EINVAL;
+  if (o->forcing != 0 && o->forcing != 1) return SWS_EINVAL;
+  if (o->forcing == 1 && !(o->eta > 0.0 && o->eta <= o->eta_max && o->eta_max < 1.0)) return SWS_EINVAL;
   CU(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const auto t0 = std::chrono::steady_clock::now();
   reset_accounting(s);
   const int n = s->n;
   sws_gmres_opts go = o->gmres;
-  go.tol = o->eta;
+  double eta_k = o->forcing == 1 ? o->eta_max : o->eta;
   int nl = 0, converged = 0, steps = 0;
   double fn = 0.0, finf = 0.0;
   RC(residual(s, u_dev, s->E, st));
@@ -428,6 +431,7 @@ int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sw
     if (finf <= o->ftol) { converged = 1; break; }
     k_axpby<<<nblk(n), 256, 0, st>>>(s->rhs, -1.0, s->E, 0.0, s->E, n);
     sws_gmres_stats gs;
+    go.tol = eta_k;
     RC(gmres(s, u_dev, s->rhs, &go, s->du, &gs, nullptr, st, s->E));
     double lam = 1.0, fnt = 0.0, finft = 0.0;
     bool ok = false;
@@ -443,6 +447,12 @@ int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sw
     if (!ok) break;
     CU(cudaMemcpyAsync(u_dev, s->ut, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
     CU(cudaMemcpyAsync(s->E, s->Et, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    if (o->forcing == 1) {  // eta_{k+1} from the decrease just obtained (sws_jfnk.h)
+      double e = 0.9 * (fnt / fn) * (fnt / fn);
+      const double sg = 0.9 * eta_k * eta_k;
+      if (sg > 0.1) e = std::max(e, sg);
+      eta_k = std::min(o->eta_max, std::max(e, o->eta));
+    }
     fn = fnt; finf = finft;
     ++steps;
   }

@@ -31,7 +31,7 @@ class GmresStats(C.Structure):
 
 class NewtonOpts(C.Structure):
     _fields_ = [("ftol", C.c_double), ("eta", C.c_double), ("alpha", C.c_double), ("max_newton", C.c_int32),
-                ("max_halvings", C.c_int32), ("gmres", GmresOpts)]
+                ("max_halvings", C.c_int32), ("gmres", GmresOpts), ("forcing", C.c_int32), ("eta_max", C.c_double)]
 
 
 class NewtonLog(C.Structure):
@@ -203,11 +203,11 @@ class Solver:
 
     def newton(self, u0, ftol: float = 1e-9, eta: float = 1e-3, restart: int | None = None,
                gmres_maxit: int = 200, max_newton: int = 30, alpha: float = 1e-4, max_halvings: int = 20,
-               jv_mode: int = 0, stream=None):
+               jv_mode: int = 0, forcing: int = 0, eta_max: float = 0.5, stream=None):
         """Damped Newton from u0 (device tensor, not modified); returns (u, log list, stats dict)."""
         restart = self.max_restart if restart is None else int(restart)
         o = NewtonOpts(float(ftol), float(eta), float(alpha), int(max_newton), int(max_halvings),
-                       GmresOpts(float(eta), restart, int(gmres_maxit), int(jv_mode)))
+                       GmresOpts(float(eta), restart, int(gmres_maxit), int(jv_mode)), int(forcing), float(eta_max))
         log = (NewtonLog * (int(max_newton) + 1))()
         nlog = C.c_int32(0)
         st = NewtonStats()

@@ -205,6 +205,28 @@ def test_newton_parity_cfg1_mesh(mods, oracle64, oracleC, bw):
     assert st["residual_evals"] == 1 + st["steps"]
 
 
+def test_newton_forcing_parity(mods, oracle64, oracleC):
+    """forcing = 1 (Eisenstat-Walker choice 2): same Newton history as the oracle's driver."""
+    sws, jf = mods
+    c = W.custom(31, 11, 0.8, -8.0, eps=1.0)
+    p = c.params()
+    P = OJ.band_truncate(OJ.linear_jacobian(p, oracle64.box_integral), p, 3)
+    res, jv, pinv = _oracle_ops(oracle64, oracleC, p, P)
+    u0 = W.flat_state(c)
+    kw = dict(ftol=1e-10, eta=1e-4, restart=30, gmres_maxit=60, forcing=1, eta_max=0.5)
+    u_ref, log_ref = OJ.newton(res, jv, pinv, u0, **kw)
+    with sws.Context(p, max_batch=1) as ctx, jf.Preconditioner(p, bandwidth=3) as pc, jf.Solver(ctx, pc, 30) as s:
+        u, log, st = s.newton(dev(u0), **kw)
+        u_c, log_c, _ = s.newton(dev(u0), ftol=1e-10, eta=1e-4, restart=30, gmres_maxit=60)
+        with pytest.raises(Exception):
+            s.newton(dev(u0), ftol=1e-10, eta=0.6, forcing=1, eta_max=0.5)
+    assert st["converged"] and len(log) == len(log_ref)
+    for a, b in zip(log, log_ref):
+        assert a["gmres_its"] == b["gmres_its"] and a["lambda"] == b["lambda"]
+    assert np.abs(u.cpu().numpy() - u_ref).max() <= 1e-8
+    assert sum(e["gmres_its"] for e in log) < sum(e["gmres_its"] for e in log_c)
+
+
 def test_newton_paper_mesh_91x31(mods, oracle64):
     """The paper's 'contemporary' mesh (91 x 31, dx = dy = 0.3, x0 = -9, eps = 1, F = 0.7; L259):
     converges from the flat guess with the block-banded preconditioner; the root satisfies the

@@ -195,6 +195,34 @@ def test_newton_known_root_quadratic_convergence():
     assert f[-2] < 1e-3 * f[-3]                    # superlinear tail (quadratic: f_{k+1} ~ f_k^2)
 
 
+def test_newton_forcing_terms_follow_the_decrease():
+    """forcing = 1: the inner tolerance starts at eta_max, then is 0.9 (||E_k||/||E_{k-1}||)^2 with the
+    0.9 eta^2 safeguard, clipped to [eta, eta_max]; the root is the same, with fewer Krylov iterations
+    than solving every step to eta."""
+    rng = np.random.default_rng(4)
+    n = 40
+    A = rng.standard_normal((n, n)) / np.sqrt(n) + 3 * np.eye(n)
+    ustar = rng.standard_normal(n)
+    rhs = A @ ustar + 0.1 * ustar ** 3
+    res = lambda u: A @ u + 0.1 * u ** 3 - rhs
+    jv = lambda u, v: A @ v + 0.3 * u ** 2 * v
+    kw = dict(ftol=1e-12, eta=1e-8, restart=40, gmres_maxit=40)
+    u0, log0 = J.newton(res, jv, lambda v: v, np.zeros(n), **kw)
+    u1, log1 = J.newton(res, jv, lambda v: v, np.zeros(n), forcing=1, eta_max=0.5, **kw)
+    assert np.abs(u0 - ustar).max() <= 1e-11 and np.abs(u1 - ustar).max() <= 1e-11
+    assert sum(e["gmres_its"] for e in log1) < sum(e["gmres_its"] for e in log0)
+    # the tolerances actually used, recomputed from the logged norms
+    eta_k, f = 0.5, [e["fnorm"] for e in log1]
+    for k, e in enumerate(log1[:-1]):
+        assert e["gmres_rel"] <= eta_k                   # the inner solve met the tolerance of its step
+        if k + 1 < len(log1):
+            t = 0.9 * (f[k + 1] / f[k]) ** 2
+            if 0.9 * eta_k ** 2 > 0.1:
+                t = max(t, 0.9 * eta_k ** 2)
+            eta_k = min(0.5, max(t, 1e-8))
+    assert log1[0]["gmres_rel"] > 1e-3                   # first step solved loosely
+
+
 def test_newton_line_search_damps():
     """arctan: the full Newton step from u0 = 3 overshoots and diverges; the damped iteration (2) converges."""
     res = lambda u: np.arctan(u)
