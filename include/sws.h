@@ -169,7 +169,8 @@ int sws_set_tuning(sws_ctx* ctx, int32_t chunks);
  * column whose completed-square constant g of L169-177 satisfies sqrt(g) >= radius_in_dy * dy for
  * all 32 targets of a warp, the column's S2 trapezoid sum (which does not depend on the source
  * data) is replaced by its integral (asinh) plus 7 Euler-Maclaurin end corrections, exact to
- * < 1e-16 / sqrt(g) for radius >= 8; the K1 and K2 terms are always summed pair by pair.
+ * < 1e-16 / sqrt(g) for radius >= 8; the K1 and K2 terms are always summed pair by pair.  The S2
+ * sensitivity sums of sws_jv_exact_batch / sws_linearize and the FP32 variant switch the same way.
  * radius_in_dy <= 0 switches the expansion off (every S2 term summed directly, the plain
  * definition); 0 < radius < 6 is refused (SWS_EINVAL).  Default 8. */
 int sws_set_farfield(sws_ctx* ctx, double radius_in_dy);
@@ -198,10 +199,13 @@ int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, doubl
 int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, int32_t n);
 
 /* Unit test of the far-field expansion: for n pairs (c, g) and the column y1, y1+dy, ..., M nodes,
- * em_host[i] = the library's expansion of sum_j c_j [((y_j-c)^2+g)^-1/2 + ((y_j+c)^2+g)^-1/2]
- * (c_j = 1/2 at both ends) and direct_host[i] = the same sum term by term on the device. */
+ * with u-+ = ((y_j -+ c)^2 + g)^-1/2, s-+ = y_j -+ c and c_j = 1/2 at both ends,
+ *   nsums = 1: em_host[i]        = the library's expansion of sum_j c_j (u- + u+)        (sws_residual)
+ *   nsums = 3: em_host[3i + 0..2] = the same, sum_j c_j (u-^3 + u+^3) and sum_j c_j (s- u-^3 - s+ u+^3)
+ *              (the sums of the analytic Jacobian action),
+ * and direct_host[...] = the same sums term by term on the device. */
 int sws_debug_s2col_host(int32_t device, double y1, double dy, int32_t M, const double* c_host,
-                         const double* g_host, int32_t n, double* direct_host, double* em_host);
+                         const double* g_host, int32_t n, int32_t nsums, double* direct_host, double* em_host);
 
 #ifdef __cplusplus
 }

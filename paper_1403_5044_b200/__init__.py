@@ -87,7 +87,8 @@ def load_library() -> C.CDLL:
         "sws_debug_rsqrt_host": (C.c_int, [C.c_int32, dp, dp, C.c_int32]),
         "sws_set_farfield": (C.c_int, [vp, C.c_double]),
         "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
-        "sws_debug_s2col_host": (C.c_int, [C.c_int32, C.c_double, C.c_double, C.c_int32, dp, dp, C.c_int32, dp, dp]),
+        "sws_debug_s2col_host": (C.c_int, [C.c_int32, C.c_double, C.c_double, C.c_int32, dp, dp, C.c_int32,
+                                           C.c_int32, dp, dp]),
     }
     for name, (res, args) in proto.items():
         fn = getattr(lib, name)
@@ -346,13 +347,15 @@ def debug_rsqrt(x: np.ndarray, device: int = 0) -> np.ndarray:
     return y
 
 
-def debug_s2col(y1: float, dy: float, M: int, c: np.ndarray, g: np.ndarray, device: int = 0):
-    """(direct, em): the S2 column sum term by term on the device and by the library's far-field
-    expansion (unit test hook, sws_debug_s2col_host)."""
+def debug_s2col(y1: float, dy: float, M: int, c: np.ndarray, g: np.ndarray, device: int = 0, nsums: int = 1):
+    """(direct, em): the S2 column sum(s) term by term on the device and by the library's far-field
+    expansion (unit test hook, sws_debug_s2col_host).  nsums = 3: arrays [n][3] of the sums of the
+    analytic Jacobian action."""
     lib = load_library()
     c = np.ascontiguousarray(c, dtype=np.float64)
     g = np.ascontiguousarray(g, dtype=np.float64)
-    d, e = np.empty_like(c), np.empty_like(c)
+    shape = (c.size,) if nsums == 1 else (c.size, 3)
+    d, e = np.empty(shape), np.empty(shape)
     _check(lib.sws_debug_s2col_host(int(device), float(y1), float(dy), int(M), _np_ptr(c), _np_ptr(g),
-                                    int(c.size), _np_ptr(d), _np_ptr(e)), "sws_debug_s2col_host")
+                                    int(c.size), int(nsums), _np_ptr(d), _np_ptr(e)), "sws_debug_s2col_host")
     return d, e

@@ -328,6 +328,35 @@ __global__ void k_debug_s2col(EmGeom e, int M, const double* c, const double* g,
   out_direct[i] = acc;
 }
 
+// the three sums of the analytic Jacobian action: out[3 i + {0, 1, 2}] = {f0, f3, f3s}
+__global__ void k_debug_s2col3(EmGeom e, int M, const double* c, const double* g, int n, double* out_direct,
+                               double* out_em) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const Em3 r = s2_column_em3(e, c[i], g[i]);
+  out_em[3 * i] = r.f0; out_em[3 * i + 1] = r.f3; out_em[3 * i + 2] = r.f3s;
+  double a0 = 0.0, a3 = 0.0, a3s = 0.0;
+  for (int j = 0; j < M; ++j) {
+    const double yj = e.y1 + j * sqrt(e.h2);
+    const double sm = yj - c[i], sp = yj + c[i];
+    const double um = rsqrt_fp64(fma(sm, sm, g[i])), up = rsqrt_fp64(fma(sp, sp, g[i]));
+    const double um3 = um * um * um, up3 = up * up * up;
+    const double w = (j == 0 || j == M - 1) ? 0.5 : 1.0;
+    a0 += w * (um + up);
+    a3 += w * (um3 + up3);
+    a3s += w * (sm * um3 - sp * up3);
+  }
+  out_direct[3 * i] = a0; out_direct[3 * i + 1] = a3; out_direct[3 * i + 2] = a3s;
+}
+
+cudaError_t launch_debug_s2col3(double y1, double dy, int M, const double* c, const double* g, int n,
+                                double* out_direct, double* out_em, cudaStream_t st) {
+  EmGeom e;
+  e.y1 = y1; e.yM = y1 + (M - 1) * dy; e.h2 = dy * dy; e.inv_h = 1.0 / dy; e.gmin = 0.0; e.sym = (y1 == 0.0);
+  k_debug_s2col3<<<(n + 127) / 128, 128, 0, st>>>(e, M, c, g, n, out_direct, out_em);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_debug_s2col(double y1, double dy, int M, const double* c, const double* g, int n,
                                double* out_direct, double* out_em, cudaStream_t st) {
   EmGeom e;

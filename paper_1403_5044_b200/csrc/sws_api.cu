@@ -604,17 +604,21 @@ int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, i
 }
 
 int sws_debug_s2col_host(int32_t device, double y1, double dy, int32_t M, const double* c_host,
-                         const double* g_host, int32_t n, double* direct_host, double* em_host) {
+                         const double* g_host, int32_t n, int32_t nsums, double* direct_host, double* em_host) {
   if (!c_host || !g_host || !direct_host || !em_host || n < 1 || M < 2 || !(dy > 0.0)) return SWS_EINVAL;
+  if (nsums != 1 && nsums != 3) return SWS_EINVAL;
   CK(cudaSetDevice(device));
   double* d = nullptr;
-  const size_t nb = (size_t)n * 8;
-  CK(cudaMalloc((void**)&d, 4 * nb));
+  const size_t nb = (size_t)n * 8, no = nb * nsums;
+  CK(cudaMalloc((void**)&d, 2 * nb + 2 * no));
   CK(cudaMemcpy(d, c_host, nb, cudaMemcpyHostToDevice));
   CK(cudaMemcpy(d + n, g_host, nb, cudaMemcpyHostToDevice));
-  cudaError_t e = sws::launch_debug_s2col(y1, dy, M, d, d + n, n, d + 2 * (size_t)n, d + 3 * (size_t)n, 0);
-  if (e == cudaSuccess) e = cudaMemcpy(direct_host, d + 2 * (size_t)n, nb, cudaMemcpyDeviceToHost);
-  if (e == cudaSuccess) e = cudaMemcpy(em_host, d + 3 * (size_t)n, nb, cudaMemcpyDeviceToHost);
+  double* od = d + 2 * (size_t)n;
+  double* oe = od + (size_t)n * nsums;
+  cudaError_t e = nsums == 1 ? sws::launch_debug_s2col(y1, dy, M, d, d + n, n, od, oe, 0)
+                             : sws::launch_debug_s2col3(y1, dy, M, d, d + n, n, od, oe, 0);
+  if (e == cudaSuccess) e = cudaMemcpy(direct_host, od, no, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(em_host, oe, no, cudaMemcpyDeviceToHost);
   cudaFree(d);
   CK(e);
   return SWS_OK;

@@ -109,6 +109,86 @@ __device__ __forceinline__ double s2_column_em(const EmGeom& e, const double c, 
   return v * e.inv_h;
 }
 
+// ---------------------------------------------------------------------------------------
+// The same for the sums the analytic Jacobian action needs (sws_jv_exact.cu): with u = f(y; c),
+// s = y - c,
+//     F0 = sum c_j u,   F3 = sum c_j u^3,   F3s = sum c_j s u^3        (data independent as well).
+// Integrals: int u = asinh(s / sqrt g), int u^3 = s / (g rho) = mu / g, int s u^3 = -1 / rho.
+// End corrections, from f^(n) above and from u^3 = -2 du/dg, s u^3 = -du/ds:
+//     u     : -(B_2k / 2k) (dy/rho)^2k P_{2k-1}(mu)
+//     u^3   : -(B_2k / 2k) (dy/rho)^2k P'_{2k}(mu) / rho^2        (mu P'_n + (n+1) P_n = P'_{n+1})
+//     s u^3 : - B_2k       (dy/rho)^2k P_{2k}(mu)  / rho
+// K = 7, same radius: remainders < 2e-17, 2e-16, 4e-15 of the respective sums at r = 8 (50-digit check).
+struct Em3 {
+  double f0, f3, f3s;
+};
+
+__device__ __forceinline__ Em3 em_tail3(const double u, const double g, const double h2, double* rho, double* ri_o,
+                                        double* mu_o) {
+  const double r2 = fma(u, u, g);
+  const double ri = rsqrt_fp64(r2);
+  *rho = r2 * ri;
+  *ri_o = ri;
+  const double mu = u * ri;
+  *mu_o = mu;
+  const double s = h2 * (ri * ri);
+  double P[15], D[15];  // P_n(mu), P'_n(mu)
+  P[0] = 1.0; P[1] = mu;
+  D[0] = 0.0; D[1] = 1.0;
+#pragma unroll
+  for (int n = 1; n <= 13; ++n) {
+    P[n + 1] = ((2.0 * n + 1.0) / (n + 1.0)) * (mu * P[n]) - (n / (n + 1.0)) * P[n - 1];
+    D[n + 1] = fma(mu, D[n], (n + 1.0) * P[n]);
+  }
+  constexpr double c1 = 1.0 / 12.0, c2 = -1.0 / 120.0, c3 = 1.0 / 252.0, c4 = -1.0 / 240.0, c5 = 1.0 / 132.0,
+                   c6 = -691.0 / 32760.0, c7 = 1.0 / 12.0;  // B_2k / 2k
+  Em3 t;
+  double a = c7 * P[13];
+  a = fma(s, a, c6 * P[11]); a = fma(s, a, c5 * P[9]); a = fma(s, a, c4 * P[7]);
+  a = fma(s, a, c3 * P[5]); a = fma(s, a, c2 * P[3]); a = fma(s, a, c1 * P[1]);
+  t.f0 = s * a;
+  a = c7 * D[14];
+  a = fma(s, a, c6 * D[12]); a = fma(s, a, c5 * D[10]); a = fma(s, a, c4 * D[8]);
+  a = fma(s, a, c3 * D[6]); a = fma(s, a, c2 * D[4]); a = fma(s, a, c1 * D[2]);
+  t.f3 = (s * a) * (ri * ri);
+  a = (14.0 * c7) * P[14];  // B_2k = 2k (B_2k / 2k)
+  a = fma(s, a, (12.0 * c6) * P[12]); a = fma(s, a, (10.0 * c5) * P[10]); a = fma(s, a, (8.0 * c4) * P[8]);
+  a = fma(s, a, (6.0 * c3) * P[6]); a = fma(s, a, (4.0 * c2) * P[4]); a = fma(s, a, (2.0 * c1) * P[2]);
+  t.f3s = (s * a) * ri;
+  return t;
+}
+
+// dy * (trapezoid sums of u, u^3, s u^3 over the nodes a, a + dy, ..., b) for the centre c
+__device__ __forceinline__ Em3 em_interval3(const double a, const double b, const double c, const double g,
+                                            const double h2) {
+  const double ua = a - c, ub = b - c;
+  double rhoa, rhob, ria, rib, mua, mub;
+  const Em3 ta = em_tail3(ua, g, h2, &rhoa, &ria, &mua);
+  const Em3 tb = em_tail3(ub, g, h2, &rhob, &rib, &mub);
+  const double nb = ub >= 0.0 ? ub + rhob : g, db = ub >= 0.0 ? 1.0 : rhob - ub;
+  const double na = ua >= 0.0 ? ua + rhoa : g, da = ua >= 0.0 ? 1.0 : rhoa - ua;
+  const double q = (nb * da) / (db * na);
+  Em3 r;
+  r.f0 = log1p((b - a) * (1.0 + q) / (rhoa + rhob)) - (tb.f0 - ta.f0);
+  r.f3 = (mub - mua) / g - (tb.f3 - ta.f3);
+  r.f3s = (ria - rib) - (tb.f3s - ta.f3s);
+  return r;
+}
+
+// Unit-node-weight column sums, direct + image:
+//   f0 = sum c_j (u- + u+),  f3 = sum c_j (u-^3 + u+^3),  f3s = sum c_j (s- u-^3 - s+ u+^3),  s-+ = y_j -+ c
+__device__ __forceinline__ Em3 s2_column_em3(const EmGeom& e, const double c, const double g) {
+  Em3 r;
+  if (e.sym) {  // one trapezoid sum over [-yM, yM]; the image half contributes -s+ u+^3
+    r = em_interval3(-e.yM, e.yM, c, g, e.h2);
+  } else {
+    const Em3 d = em_interval3(e.y1, e.yM, c, g, e.h2), m = em_interval3(e.y1, e.yM, -c, g, e.h2);
+    r.f0 = d.f0 + m.f0; r.f3 = d.f3 + m.f3; r.f3s = d.f3s - m.f3s;
+  }
+  r.f0 *= e.inv_h; r.f3 *= e.inv_h; r.f3s *= e.inv_h;
+  return r;
+}
+
 // The far/near decision is taken per WARP (all 32 targets of the warp must be far), so the j loop
 // has no divergence.  Used by k_allpairs and by the counting kernel of sws_farfield_stats.
 __device__ __forceinline__ bool column_is_far(const double g, const double gmin) {

@@ -148,6 +148,8 @@ cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaSt
 cudaError_t launch_count_near(sws_ctx* c, int states, int* out, cudaStream_t st);
 cudaError_t launch_debug_s2col(double y1, double dy, int M, const double* cc, const double* g, int n,
                                double* out_direct, double* out_em, cudaStream_t st);
+cudaError_t launch_debug_s2col3(double y1, double dy, int M, const double* cc, const double* g, int n,
+                                double* out_direct, double* out_em, cudaStream_t st);
 cudaError_t launch_allpairs_f32(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
 cudaError_t launch_assemble(sws_ctx* c, int states, const PairPlan& plan, double* F0,
                             double* Fpert, cudaStream_t st);

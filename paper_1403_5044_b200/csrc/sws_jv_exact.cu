@@ -28,6 +28,9 @@
 // form I) is linearised in k_reconstruct (lin mode), k_dy (linear as it stands), k_targets_lin.
 #include <math_constants.h>
 
+#include <type_traits>
+
+#include "sws_farfield.cuh"
 #include "sws_internal.cuh"
 #include "sws_stage.cuh"
 
@@ -148,7 +151,8 @@ struct LinS {  // direction-independent sums of one thread
 // MODE 0: everything (sws_jv_exact_batch).  MODE 1: the direction-independent sums only
 // (sws_linearize: they depend on u alone, so a Newton step forms them once).  MODE 2: the
 // direction sums only (sws_jv_apply): no S2, 41 + 4 BT FP64 instructions per pair.
-template <int BT, bool SCALE, int MODE>
+// S2T = false: far column, the S2 sums of the whole column come from s2_column_em3 (sws_farfield.cuh).
+template <int BT, bool SCALE, int MODE, bool S2T>
 __device__ __forceinline__ void pair_lin(const double2 zp, const double2 sl, const double yj,
                                          const double4* __restrict__ dv, const double wgt,
                                          const LinT& t, const LinC& c, LinS& s, double (&acc)[BT]) {
@@ -176,13 +180,15 @@ __device__ __forceinline__ void pair_lin(const double2 zp, const double2 sl, con
     K1 *= wgt; cz *= wgt; czx *= wgt; czy *= wgt;
   }
   if (MODE != 2) {
+    s.cpsi += K1;
+    s.cz += cz;
+  }
+  if (MODE != 2 && S2T) {
     // S2 and its A, B, C sensitivities
     const double sm = yj - c.c, sp = yj + c.c;
     double um = rsqrt_l(fma(sm, sm, c.g)), up = rsqrt_l(fma(sp, sp, c.g));
     double um3 = (um * um) * um, up3 = (up * up) * up;
     if (SCALE) { um *= wgt; up *= wgt; um3 *= wgt; up3 *= wgt; }
-    s.cpsi += K1;
-    s.cz += cz;
     s.s0 += um + up;
     s.u3 += um3 + up3;
     const double vm = dm * um3, vp = dp * up3;
@@ -237,6 +243,7 @@ struct LinArgs {
   double* out;          // [group][chunk][6 + BT][T]
   int N, M, T;
   int chunks, cols_per_chunk, seg_len, nseg;
+  EmGeom em;
 };
 
 constexpr int kLinUnroll = SWS_LIN_UNROLL;
@@ -317,24 +324,42 @@ __global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT 
     const double4* dv = s_dv + (size_t)s * seg_pad * DV;
     const double* yy = s_y + (size_t)s * seg_pad;
     LinS col = {tot.cpsi, tot.cz, tot.s0, 0.0, 0.0, 0.0};
-    int jlo = 0, jhi = len;
-    if (j0 == 0) {
-      pair_lin<BT, true, MODE>(rec[0], rec[1], yy[0], dv, 0.5 * ci, tg, cc, col, acc);
-      jlo = 1;
-    }
-    const bool last = (j0 + len == a.M);
-    if (last) jhi = len - 1;
-    if (edge_col) {
-      for (int j = jlo; j < jhi; ++j)
-        pair_lin<BT, true, MODE>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * DV, ci, tg, cc, col, acc);
-    } else {
+    auto walk = [&](auto s2t) {
+      constexpr bool S2T = decltype(s2t)::value;
+      int jlo = 0, jhi = len;
+      if (j0 == 0) {
+        pair_lin<BT, true, MODE, S2T>(rec[0], rec[1], yy[0], dv, 0.5 * ci, tg, cc, col, acc);
+        jlo = 1;
+      }
+      const bool last = (j0 + len == a.M);
+      if (last) jhi = len - 1;
+      if (edge_col) {
+        for (int j = jlo; j < jhi; ++j)
+          pair_lin<BT, true, MODE, S2T>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * DV, ci, tg, cc, col,
+                                        acc);
+      } else {
 #pragma unroll (MODE == 0 ? kLinUnroll : 2)
-      for (int j = jlo; j < jhi; ++j)
-        pair_lin<BT, false, MODE>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * DV, 1.0, tg, cc, col, acc);
+        for (int j = jlo; j < jhi; ++j)
+          pair_lin<BT, false, MODE, S2T>(rec[2 * j], rec[2 * j + 1], yy[j], dv + (size_t)j * DV, 1.0, tg, cc, col,
+                                         acc);
+      }
+      if (last && jhi >= jlo)
+        pair_lin<BT, true, MODE, S2T>(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], dv + (size_t)jhi * DV, 0.5 * ci, tg,
+                                      cc, col, acc);
+    };
+    if (MODE != 2 && column_is_far(cc.g, a.em.gmin)) {  // warp-uniform
+      walk(std::false_type{});
+      if (j0 == 0) {  // the column's S2 sums, once: d- = s- - beta, d+ = s+ + beta, beta = y* - c
+        const Em3 e3 = s2_column_em3(a.em, cc.c, cc.g);
+        const double beta = tg.ys - cc.c;
+        col.s0 = fma(ci, e3.f0, col.s0);
+        col.u3 = ci * e3.f3;
+        col.u3y = ci * fma(-beta, e3.f3, e3.f3s);
+        col.u3yy = ci * (fma(-cc.g, e3.f3, e3.f0) + beta * fma(beta, e3.f3, -2.0 * e3.f3s));
+      }
+    } else {
+      walk(std::true_type{});
     }
-    if (last && jhi >= jlo)
-      pair_lin<BT, true, MODE>(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], dv + (size_t)jhi * DV, 0.5 * ci, tg, cc,
-                               col, acc);
     tot.cpsi = col.cpsi; tot.cz = col.cz; tot.s0 = col.s0;
     tot.u3 = fma(cc.dx2, col.u3, tot.u3);
     tot.u3y = fma(cc.dx, col.u3y, tot.u3y);
@@ -511,6 +536,7 @@ static cudaError_t launch_lin_t(sws_ctx* c, int groups, const PairPlan& plan, cu
   a.N = m.N; a.M = m.M; a.T = m.T;
   a.chunks = plan.chunks; a.cols_per_chunk = plan.cols_per_chunk;
   a.seg_len = plan.seg_len; a.nseg = plan.nseg;
+  a.em = em_geometry(c);
   dim3 grid(plan.tiles, plan.chunks, groups);
   k_allpairs_lin<BT, MODE><<<grid, kPairThreads, lin_smem_bytes(MODE == 1 ? 0 : BT, plan.seg_len), st>>>(a);
   return cudaGetLastError();

@@ -160,6 +160,64 @@ def test_farfield_expansion_primitive(sws, y1, dy, M):
     assert err_em.max() <= 4e-15, (err_em.max(), c[err_em.argmax()], r[err_em.argmax()])
 
 
+@pytest.mark.parametrize("y1,dy,M", [(0.0, 0.075, 241), (0.0, 0.8, 11), (0.8, 0.4, 12), (0.0, 0.5, 4)])
+def test_farfield_expansion_three_sums(sws, y1, dy, M):
+    """The expansions of the three column sums of the analytic Jacobian action (sum u, sum u^3,
+    sum s u^3, direct + image with the image's sign) against term-by-term sums in long double."""
+    rng = np.random.default_rng(6)
+    n = 3000
+    yM = y1 + (M - 1) * dy
+    c = np.concatenate([rng.uniform(-yM - 5, yM + 5, n - 5), [y1, yM, -yM, 0.0, 0.5 * (y1 + yM)]])
+    r = np.concatenate([np.full(n // 3, 8.0), rng.uniform(8.0, 12.0, n // 3), 10 ** rng.uniform(0.9, 2.5, n - 2 * (n // 3))])
+    g = (r * dy) ** 2
+    direct, em = sws.debug_s2col(y1, dy, M, c, g, nsums=3)
+    L = np.longdouble
+    y = (L(y1) + np.arange(M, dtype=L) * L(dy))[None, :]
+    cc, gg = c.astype(L)[:, None], g.astype(L)[:, None]
+    w = np.ones(M, dtype=L); w[0] = w[-1] = 0.5
+    sm, sp = y - cc, y + cc
+    um, up = 1 / np.sqrt(sm ** 2 + gg), 1 / np.sqrt(sp ** 2 + gg)
+    ref = np.stack([((um + up) * w).sum(1), ((um ** 3 + up ** 3) * w).sum(1), ((sm * um ** 3 - sp * up ** 3) * w).sum(1)], 1)
+    rg = np.sqrt(g)
+    scale = np.stack([1 / (dy * rg), 1 / (dy * g * rg), 1 / (dy * g)], 1)      # size of each sum
+    scale = np.maximum(scale, np.abs(ref).astype(np.float64))
+    err_em = np.abs((em.astype(L) - ref).astype(np.float64)) / scale
+    err_direct = np.abs((direct.astype(L) - ref).astype(np.float64)) / scale
+    assert err_direct.max() <= 1e-13
+    assert err_em[:, 0].max() <= 4e-15 and err_em[:, 1].max() <= 5e-14 and err_em[:, 2].max() <= 5e-14, err_em.max(0)
+
+
+@pytest.mark.parametrize("name", ["cfg2", "ragged_y1", "steep"])
+def test_farfield_on_off_equivalence_jv_exact(sws, oracleC, name):
+    """The analytic Jacobian action (fused kernel and linearize + apply) with the far-field S2
+    sensitivity sums against the pair-by-pair sums (radius 0), and both against the oracle."""
+    if name == "cfg2":
+        cfg = W.CONFIGS[1]
+        u = W.state(cfg)
+    elif name == "ragged_y1":
+        cfg = W.custom(eps=0.3, amp=0.05, N=90, M=40, h=0.2, x1=-4.0, y1=0.6, seed=21)
+        u = W.state(cfg) + 1e-3 * np.random.default_rng(3).standard_normal(cfg.n)
+    else:
+        cfg = W.custom(eps=0.5, amp=1.5, N=120, M=50, h=0.15, x1=-2.0, seed=22)
+        u = W.state(cfg)
+    V = W.directions(cfg, 5)
+    ref = oracleC.jv_exact(cfg.params(), u, V[1])
+    with sws.Context(cfg.params(), max_batch=5) as ctx:
+        ud, Vd = dev(u), dev(V)
+        on = ctx.jv_exact_batch(ud, Vd).cpu().numpy()
+        ctx.linearize(ud)
+        on_la = ctx.jv_apply(Vd).cpu().numpy()
+        ctx.set_farfield(0.0)
+        off = ctx.jv_exact_batch(ud, Vd).cpu().numpy()
+        ctx.linearize(ud)
+        off_la = ctx.jv_apply(Vd).cpu().numpy()
+    sc = np.abs(off).max()
+    assert np.abs(on - off).max() <= 1e-12 * sc
+    assert np.abs(on_la - off_la).max() <= 1e-12 * sc
+    assert np.abs(on[1] - ref).max() <= TOL * np.abs(ref).max()
+    assert np.abs(on_la[1] - ref).max() <= TOL * np.abs(ref).max()
+
+
 @pytest.mark.parametrize("name", ["cfg3", "ragged_y1", "steep"])
 def test_farfield_on_off_equivalence(sws, oracle80, name):
     """sws_set_farfield(0) sums every S2 term pair by pair (the plain definition); the default
