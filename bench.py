@@ -334,6 +334,43 @@ def solve_report(sws, device: int, names=("paper_361x121", "paper_721x241"), ban
     return out
 
 
+def table1_report(sws, device: int, steps: int = 5) -> dict:
+    """PAPER.md Table 1 (L281-290): seconds per function evaluation on the paper's five meshes (eps = 1,
+    F = 0.7), here one sws_residual on a seeded synthetic state of that shape (CUDA events, L2 flushed by the
+    256 MB fill between repetitions, median of `steps`).  The paper's columns (other hardware) ride along as
+    context: multicore MATLAB on 2x Xeon E5-2670 and MATLAB + CUDA on a Tesla M2090."""
+    import torch
+    paper = {"91x31": (0.87, 0.02), "181x61": (4.38, 0.18), "271x91": (20.40, 0.83), "361x121": (64.35, 2.52),
+             "451x151": (153.91, 6.04)}
+    shapes = [(91, 31, 0.3, -9.0), (181, 61, 0.3, -14.0), (271, 91, 0.2, -14.0), (361, 121, 0.15, -14.0),
+              (451, 151, 0.12, -14.0)]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{device}")
+    out = {}
+    for N, M, h, x1 in shapes:
+        cfg = W.custom(N, M, h, x1, eps=1.0, amp=0.05, seed=40 + N)
+        u = torch.from_numpy(W.state(cfg)).cuda(device)
+        with sws.Context(cfg.params(), device=device) as ctx:
+            F = ctx.residual(u)
+            for _ in range(3):
+                ctx.residual(u, out=F)
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(steps):
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); ctx.residual(u, out=F); e1.record()
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+        sec = float(np.median(ts)) * 1e-3
+        cpu, gpu = paper[f"{N}x{M}"]
+        out[f"{N}x{M}"] = {"seconds_per_evaluation": sec, "pairs_per_s": cfg.pairs / sec,
+                           "paper_workstation_matlab_s": cpu, "paper_m2090_s": gpu, "ratio_to_paper_m2090": gpu / sec}
+    out["note"] = ("one sws_residual (whole u -> F path, 5 kernel launches) per evaluation, synthetic state; the "
+                   "paper's numbers are other hardware (2x Xeon E5-2670 / Tesla M2090, L265) and its own converged "
+                   "states: context, not a target")
+    return out
+
+
 def run_ours(args) -> None:
     import torch
 
@@ -491,6 +528,10 @@ def run_ours(args) -> None:
     if world == 1 and not args.no_solve:
         solve = solve_report(sws, local)
 
+    table1 = None
+    if world == 1 and not args.no_table1:
+        table1 = table1_report(sws, local)
+
     fp32 = None
     if world == 1 and not args.no_fp32:
         fp32 = fp32_variant_report(sws, local, names=tuple(dict.fromkeys(["cfg4_361x121", cfg.name])))
@@ -515,6 +556,7 @@ def run_ours(args) -> None:
         "jv_exact": jvx,
         "fp32_variant": fp32,
         "solve": solve,
+        "table1": table1,
     }
     print(json.dumps(line), flush=True)
     ctx.close()
@@ -534,6 +576,7 @@ def main() -> None:
     ap.add_argument("--no-fp32", action="store_true", help="skip the reported FP32-variant section")
     ap.add_argument("--no-jv-exact", action="store_true", help="skip the analytic-Jv section")
     ap.add_argument("--no-solve", action="store_true", help="skip the full JFNK solve section")
+    ap.add_argument("--no-table1", action="store_true", help="skip the paper's Table 1 meshes")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)

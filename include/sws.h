@@ -165,6 +165,11 @@ int sws_profile_read(sws_ctx* ctx, double* allpairs_ms, int32_t* launches, int32
  * clamped to what the workspace was sized for). */
 int sws_set_tuning(sws_ctx* ctx, int32_t chunks);
 
+/* Change the source strength epsilon (eq. (6)) of an existing context: the parameter of the
+ * bootstrapping / continuation process of L229.  Nothing else of the set-up depends on it.  A
+ * linearisation kept by sws_linearize is invalidated. */
+int sws_set_eps(sws_ctx* ctx, double eps);
+
 /* Far-field evaluation of the S2 terms (sws_allpairs.cu).  For a source
  * column whose completed-square constant g of L169-177 satisfies sqrt(g) >= radius_in_dy * dy for
  * all 32 targets of a warp, the column's S2 trapezoid sum (which does not depend on the source

@@ -127,6 +127,16 @@ int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* opts,
                       sws_newton_log* log_host, int32_t* nlog, sws_newton_stats* stats,
                       void* cuda_stream);
 
+/* The bootstrapping process of L229: for i = 0..n_eps-1 set the source strength of the solver's
+ * context to eps_host[i] (sws_set_eps) and run sws_solver_newton from the previous solution
+ * (u_dev in: the guess for eps_host[0], e.g. the flat state L227; out: the solution for the last
+ * value reached).  stats_host has room for n_eps entries; *n_done = how many values converged
+ * (the process stops at the first that does not; u_dev then holds that failed iterate's
+ * predecessor, the last converged solution).  The context keeps the last epsilon it was set to. */
+int sws_solver_continuation(sws_solver* s, double* u_dev, const double* eps_host, int32_t n_eps,
+                            const sws_newton_opts* opts, sws_newton_stats* stats_host, int32_t* n_done,
+                            void* cuda_stream);
+
 int sws_solver_destroy(sws_solver* s);
 
 #ifdef __cplusplus

@@ -27,7 +27,7 @@ SYMBOLS = (
     "sws_probe_fp64_peak", "sws_debug_rsqrt_host",
     "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
     "sws_get_params", "sws_linearize", "sws_jv_apply",
-    "sws_set_farfield", "sws_farfield_stats", "sws_debug_s2col_host",
+    "sws_set_farfield", "sws_farfield_stats", "sws_debug_s2col_host", "sws_set_eps",
 )
 
 
@@ -86,6 +86,7 @@ def load_library() -> C.CDLL:
         "sws_probe_fp64_peak": (C.c_int, [C.c_int32, C.POINTER(C.c_double), ip, C.POINTER(C.c_double)]),
         "sws_debug_rsqrt_host": (C.c_int, [C.c_int32, dp, dp, C.c_int32]),
         "sws_set_farfield": (C.c_int, [vp, C.c_double]),
+        "sws_set_eps": (C.c_int, [vp, C.c_double]),
         "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
         "sws_debug_s2col_host": (C.c_int, [C.c_int32, C.c_double, C.c_double, C.c_int32, dp, dp, C.c_int32,
                                            C.c_int32, dp, dp]),
@@ -304,6 +305,10 @@ class Context:
 
     def set_tuning(self, chunks: int = 0) -> None:
         _check(self.lib.sws_set_tuning(self._h, int(chunks)), "sws_set_tuning")
+
+    def set_eps(self, eps: float) -> None:
+        """sws_set_eps: the source strength of the continuation process."""
+        _check(self.lib.sws_set_eps(self._h, float(eps)), "sws_set_eps")
 
     def set_farfield(self, radius_in_dy: float = 8.0) -> None:
         """sws_set_farfield: <= 0 sums every S2 term directly (the plain definition)."""

@@ -143,6 +143,7 @@ struct sws_solver {
   double *w, *z, *t, *r;
   double *E, *Et, *du, *ut, *rhs;
   double *ub, *Eb;  // jv_mode 2: shifted state u + sigma v and E of it
+  double* ukeep;    // sws_solver_continuation: the last converged solution
   double* partial;  // [kDotBlocks][m_max + 2]
   double* hdev;     // [2 (m_max + 1) + 2]: h1 | h2 | normsq, scratch
   double* ydev;     // [m_max]
@@ -379,7 +380,7 @@ int sws_solver_create(sws_ctx* ctx, sws_precond* pc, int32_t max_restart, sws_so
   reset_accounting(s);
   const size_t n = (size_t)s->n;
   double* base = nullptr;
-  const size_t vec = (size_t)(max_restart + 1) + 11;
+  const size_t vec = (size_t)(max_restart + 1) + 12;
   cudaError_t e = cudaSetDevice(p.device);
   if (e == cudaSuccess) e = cudaMalloc(&base, vec * n * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&s->partial, sizeof(double) * kDotBlocks * (max_restart + 2));
@@ -396,7 +397,7 @@ int sws_solver_create(sws_ctx* ctx, sws_precond* pc, int32_t max_restart, sws_so
   double* q = base + (size_t)(max_restart + 1) * n;
   s->w = q; s->z = q + n; s->t = q + 2 * n; s->r = q + 3 * n;
   s->E = q + 4 * n; s->Et = q + 5 * n; s->du = q + 6 * n; s->ut = q + 7 * n; s->rhs = q + 8 * n;
-  s->ub = q + 9 * n; s->Eb = q + 10 * n;
+  s->ub = q + 9 * n; s->Eb = q + 10 * n; s->ukeep = q + 11 * n;
   *out = s;
   return SWS_OK;
 }
@@ -465,6 +466,28 @@ int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sw
   stats->residual_evals = s->n_res; stats->jv_products = s->n_jv; stats->precond_applies = s->n_pc;
   stats->ms_jv = s->ms_jv; stats->ms_precond = s->ms_pc; stats->ms_residual = s->ms_res;
   stats->ms_total = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  return SWS_OK;
+}
+
+int sws_solver_continuation(sws_solver* s, double* u_dev, const double* eps_host, int32_t n_eps,
+                            const sws_newton_opts* o, sws_newton_stats* stats, int32_t* n_done, void* cuda_stream) {
+  if (!s || !u_dev || !eps_host || n_eps < 1 || !o || !stats || !n_done) return SWS_EINVAL;
+  CU(cudaSetDevice(s->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  *n_done = 0;
+  std::vector<sws_newton_log> log((size_t)o->max_newton + 1);
+  for (int i = 0; i < n_eps; ++i) {
+    RC(sws_set_eps(s->ctx, eps_host[i]));
+    CU(cudaMemcpyAsync(s->ukeep, u_dev, sizeof(double) * s->n, cudaMemcpyDeviceToDevice, st));
+    int32_t nl = 0;
+    RC(sws_solver_newton(s, u_dev, o, log.data(), &nl, &stats[i], cuda_stream));
+    if (!stats[i].converged) {  // hand back the last converged solution (or the caller's guess)
+      CU(cudaMemcpyAsync(u_dev, s->ukeep, sizeof(double) * s->n, cudaMemcpyDeviceToDevice, st));
+      CU(cudaStreamSynchronize(st));
+      break;
+    }
+    ++*n_done;
+  }
   return SWS_OK;
 }
 

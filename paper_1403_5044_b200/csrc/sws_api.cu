@@ -231,6 +231,14 @@ int sws_set_tuning(sws_ctx* c, int32_t chunks) {
   return SWS_OK;
 }
 
+int sws_set_eps(sws_ctx* c, double eps) {
+  if (!c || eps != eps) return SWS_EINVAL;
+  c->params.eps = eps;
+  c->mesh.eps = eps;   // kernels take the mesh by value at launch
+  c->lin_valid = 0;    // a kept linearisation belongs to the old source strength
+  return SWS_OK;
+}
+
 int sws_set_farfield(sws_ctx* c, double radius_in_dy) {
   if (!c || radius_in_dy != radius_in_dy) return SWS_EINVAL;
   if (radius_in_dy > 0.0 && radius_in_dy < 6.0) return SWS_EINVAL;  // the expansion is not accurate there

@@ -16,7 +16,7 @@ LIB_PATH = Path(__file__).resolve().parent / "libsws_jfnk.so"
 SYMBOLS = (
     "sws_precond_create", "sws_precond_apply", "sws_precond_block_host", "sws_precond_bytes",
     "sws_precond_bandwidth", "sws_precond_setup_ms", "sws_precond_destroy",
-    "sws_solver_create", "sws_solver_gmres", "sws_solver_newton", "sws_solver_destroy",
+    "sws_solver_create", "sws_solver_gmres", "sws_solver_newton", "sws_solver_continuation", "sws_solver_destroy",
     "sws_jfnk_last_error", "sws_solver_last_error",
 )
 
@@ -69,6 +69,8 @@ def load_jfnk() -> C.CDLL:
         "sws_solver_gmres": (C.c_int, [vp, dp, dp, C.POINTER(GmresOpts), dp, C.POINTER(GmresStats), dp, vp]),
         "sws_solver_newton": (C.c_int, [vp, dp, C.POINTER(NewtonOpts), C.POINTER(NewtonLog), C.POINTER(C.c_int32),
                                         C.POINTER(NewtonStats), vp]),
+        "sws_solver_continuation": (C.c_int, [vp, dp, dp, C.c_int32, C.POINTER(NewtonOpts),
+                                              C.POINTER(NewtonStats), C.POINTER(C.c_int32), vp]),
         "sws_solver_destroy": (C.c_int, [vp]),
         "sws_jfnk_last_error": (C.c_char_p, []),
         "sws_solver_last_error": (C.c_char_p, []),
@@ -219,3 +221,27 @@ class Solver:
         stats = {f: getattr(st, f) for f, _ in NewtonStats._fields_}
         stats["converged"] = bool(stats["converged"])
         return u, entries, stats
+
+    def continuation(self, u0, eps_values, ftol: float = 1e-9, eta: float = 1e-3, restart: int | None = None,
+                     gmres_maxit: int = 200, max_newton: int = 30, alpha: float = 1e-4, max_halvings: int = 20,
+                     jv_mode: int = 0, forcing: int = 0, eta_max: float = 0.5, stream=None):
+        """The bootstrapping process of PAPER.md L229: Newton for each source strength in `eps_values`, each
+        started from the previous solution.  Returns (u, list of stats dicts of the values that were run,
+        number of values that converged).  The context keeps the last epsilon."""
+        restart = self.max_restart if restart is None else int(restart)
+        o = NewtonOpts(float(ftol), float(eta), float(alpha), int(max_newton), int(max_halvings),
+                       GmresOpts(float(eta), restart, int(gmres_maxit), int(jv_mode)), int(forcing), float(eta_max))
+        eps = np.ascontiguousarray(eps_values, dtype=np.float64)
+        st = (NewtonStats * eps.size)()
+        ndone = C.c_int32(0)
+        u = u0.clone()
+        _check(self.lib.sws_solver_continuation(self._h, u.data_ptr(), eps.ctypes.data_as(C.c_void_p), int(eps.size),
+                                                C.byref(o), st, C.byref(ndone), _stream(stream)),
+               "sws_solver_continuation")
+        ran = min(eps.size, ndone.value + 1)
+        out = []
+        for e in st[:ran]:
+            d = {f: getattr(e, f) for f, _ in NewtonStats._fields_}
+            d["converged"] = bool(d["converged"])
+            out.append(d)
+        return u, out, int(ndone.value)

@@ -227,6 +227,38 @@ def test_newton_forcing_parity(mods, oracle64, oracleC):
     assert sum(e["gmres_its"] for e in log) < sum(e["gmres_its"] for e in log_c)
 
 
+def test_continuation_in_epsilon(mods, oracle64):
+    """The bootstrapping process of L229 on the 45 x 13 mesh of Fig. 2 (L247): eps = 0.5 -> 1.0 -> 1.5, each
+    from the previous solution; the eps = 1 stage is the root Newton finds from the flat guess; the final
+    state is a root of the ORACLE's residual at eps = 1.5; sws_set_eps changes nothing but the source term."""
+    sws, jf = mods
+    c = W.custom(45, 13, 0.4, -9.0, eps=1.0)
+    p = c.params()
+    u0 = dev(W.flat_state(c))
+    kw = dict(ftol=1e-10, eta=1e-3, restart=40, gmres_maxit=80)
+    with sws.Context(p, max_batch=1) as ctx, jf.Preconditioner(p, bandwidth=5) as pc, jf.Solver(ctx, pc, 40) as s:
+        u_direct, _, st_d = s.newton(u0, **kw)
+        assert st_d["converged"]
+        u1, stats1, n1 = s.continuation(u0, [0.5, 1.0], **kw)
+        assert n1 == 2 and all(e["converged"] for e in stats1)
+        assert np.abs((u1 - u_direct).cpu().numpy()).max() <= 1e-8
+        u2, stats2, n2 = s.continuation(u1, [1.25, 1.5], **kw)
+        assert n2 == 2
+        # warm starts need fewer Newton steps than the flat guess needed
+        assert stats2[0]["steps"] <= st_d["steps"]
+        p15 = dict(p, eps=1.5)
+        assert np.abs(oracle64.residual(p15, u2.cpu().numpy())).max() <= 1e-9
+        # the context now evaluates E at eps = 1.5
+        F = ctx.residual(u2).cpu().numpy()
+        assert np.abs(F).max() <= 1e-9
+        ctx.set_eps(1.0)
+        assert np.abs(ctx.residual(u_direct).cpu().numpy()).max() <= 1e-9
+        # a stage that cannot converge (one Newton step allowed) hands back the last converged solution
+        u3, stats3, n3 = s.continuation(u_direct, [1.2, 1.4], max_newton=1, **kw)
+        assert n3 == 0 and len(stats3) == 1 and not stats3[0]["converged"]
+        assert np.array_equal(u3.cpu().numpy(), u_direct.cpu().numpy())
+
+
 def test_newton_paper_mesh_91x31(mods, oracle64):
     """The paper's 'contemporary' mesh (91 x 31, dx = dy = 0.3, x0 = -9, eps = 1, F = 0.7; L259):
     converges from the flat guess with the block-banded preconditioner; the root satisfies the
