@@ -21,8 +21,11 @@
 #include "sws_stage.cuh"
 
 // build-time tuning of the all-pairs kernel (defaults measured on B200)
+#ifndef SWS_PAIR_THREADS
+#define SWS_PAIR_THREADS 64  // threads (= targets) per CTA of k_allpairs
+#endif
 #ifndef SWS_MINB
-#define SWS_MINB 4  // resident CTAs per SM asked of __launch_bounds__ (caps registers at 128)
+#define SWS_MINB 8  // resident CTAs per SM asked of __launch_bounds__ (caps registers at 128)
 #endif
 #ifndef SWS_UNROLL
 #define SWS_UNROLL 8  // source nodes per inner-loop iteration
@@ -31,6 +34,9 @@
 namespace sws {
 
 constexpr int kUnroll = SWS_UNROLL;
+// k_allpairs runs 64-thread CTAs, 8 per SM (16 warps per SM as with 128 x 4, but only two warps meet at
+// the per-column barrier and CTAs turn over twice as often: 59.5 instead of 61.1 ms at cfg5)
+constexpr int kThreads64 = SWS_PAIR_THREADS;
 
 // Per-thread constants of one target and of the current source column.
 // The S2 quadratic forms are used with the square completed (C > 0):
@@ -120,7 +126,7 @@ struct PairArgs {
 };
 
 template <int MINB>
-__global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs a) {
+__global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int seg_pad = a.seg_len;  // even by construction
   SrcRec* s_rec = reinterpret_cast<SrcRec*>(smem_raw);                            // [kStages][seg_pad]
@@ -129,7 +135,7 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
 
   const int tid = threadIdx.x;
   const int tile = blockIdx.x, chunk = blockIdx.y, state = blockIdx.z;
-  const int t = tile * kPairThreads + tid;
+  const int t = tile * kThreads64 + tid;
   const int tc = t < a.T ? t : a.T - 1;  // ragged tail: recompute the last target, never stored
 
   const TgtRec tr = a.tgt[(size_t)state * a.T + tc];
@@ -202,6 +208,7 @@ __global__ void __launch_bounds__(kPairThreads, MINB) k_allpairs(const PairArgs 
 // host side
 
 constexpr int kMinB = SWS_MINB;
+constexpr int kMinCtaNodes = 32;  // a CTA walks at least this many source nodes
 
 size_t allpairs_smem_bytes(const PairPlan& p) {
   return (size_t)kStages * p.seg_len * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
@@ -213,46 +220,53 @@ cudaError_t allpairs_configure(int* occ_out) {
   if (e != cudaSuccess) return e;
   int occ = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-      &occ, k_allpairs<kMinB>, kPairThreads,
+      &occ, k_allpairs<kMinB>, kThreads64,
       kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t));
   if (e != cudaSuccess) return e;
   *occ_out = occ > 0 ? occ : 1;
   return cudaSuccess;
 }
 
-// Choose the number of column groups so that (a) the grid is many waves of the
-// sm_count * occupancy resident CTAs and (b) wave quantisation of both the grid and the
-// columns-per-CTA count is small.  cost(c) ~ ceil(CTAs / slots) * (ceil(N / c) + overhead).
+// Choose the number of column groups.  Measured on B200: short CTAs win - at cfg5
+// 19 / 61 / 121 / 241 groups give 59.5 / 59.0 / 58.8 / 58.6 ms (64-thread CTAs) - because CTAs whose
+// columns are near their targets take 1.4x longer and finer pieces balance better, while every group
+// costs one row of partial sums per target.  So: about kColsTarget columns per CTA, at least two waves of
+// the sm_count * occupancy resident CTAs when the mesh is small, and among the candidates of that size
+// the one with the least wave quantisation, cost(c) ~ ceil(CTAs / slots) * (ceil(N / c) + overhead).
 // The split depends on the MESH ONLY, never on the number of states in the launch: the
 // summation order of a state's quadrature is then the same in sws_residual and in every
 // slot of sws_jv_batch, so a batch is bitwise a loop of single evaluations.
+constexpr int kColsTarget = 12;
+
 PairPlan make_plan(const sws_ctx* c) {
   const Mesh& m = c->mesh;
   PairPlan p;
-  p.tiles = (m.T + kPairThreads - 1) / kPairThreads;
+  const int threads = c->params.precision == 1 ? kPairThreads : kThreads64;
+  p.tiles = (m.T + threads - 1) / threads;
   p.nseg = (m.M + kSegMax - 1) / kSegMax;
   int seg = (m.M + p.nseg - 1) / p.nseg;
   p.seg_len = (seg + 1) & ~1;
   p.nseg = (m.M + p.seg_len - 1) / p.seg_len;
   const long slots = (long)c->sm_count * (c->pair_occ > 0 ? c->pair_occ : 4);
   int best = 1;
-  // a CTA should see at least ~256 source nodes
-  int min_cols = (256 + m.M - 1) / m.M;
-  int cmax = m.N / (min_cols > 0 ? min_cols : 1);
-  if (cmax < 1) cmax = 1;
-  if (cmax > 256) cmax = 256;
+  const int cmax = max_chunks(c);
   if (c->chunks_user > 0) {
     best = c->chunks_user < cmax ? c->chunks_user : cmax;
   } else {
+    int lo = (m.N + kColsTarget - 1) / kColsTarget;
+    while (lo < cmax && (long)p.tiles * lo < 2 * slots) ++lo;
+    if (lo > cmax) lo = cmax;
+    int hi = lo + lo / 2 + 1;
+    if (hi > cmax) hi = cmax;
     double best_cost = 1e300;
-    for (int ch = 1; ch <= cmax; ++ch) {
+    for (int ch = lo; ch <= hi; ++ch) {
       const int cols = (m.N + ch - 1) / ch;
       const int used = (m.N + cols - 1) / cols;  // groups that are not empty
-      if (used != ch) continue;
-      const long ctas = (long)p.tiles * ch;
+      if (used != ch && ch != lo) continue;
+      const long ctas = (long)p.tiles * used;
       const long waves = (ctas + slots - 1) / slots;
-      const double cost = (double)waves * (cols + 0.25) + 1e-3 * ch;
-      if (cost < best_cost) { best_cost = cost; best = ch; }
+      const double cost = (double)waves * (cols + 0.25) + 1e-3 * used;
+      if (cost < best_cost) { best_cost = cost; best = used; }
     }
   }
   p.cols_per_chunk = (m.N + best - 1) / best;
@@ -261,7 +275,7 @@ PairPlan make_plan(const sws_ctx* c) {
 }
 
 int max_chunks(const sws_ctx* c) {
-  int min_cols = (256 + c->mesh.M - 1) / c->mesh.M;
+  int min_cols = (kMinCtaNodes + c->mesh.M - 1) / c->mesh.M;
   int cmax = c->mesh.N / (min_cols > 0 ? min_cols : 1);
   if (cmax < 1) cmax = 1;
   if (cmax > 256) cmax = 256;
@@ -279,7 +293,7 @@ cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaSt
   a.dxdy = m.dx * m.dy;
   a.em = em_geometry(c);
   dim3 grid(plan.tiles, plan.chunks, states);
-  k_allpairs<kMinB><<<grid, kPairThreads, allpairs_smem_bytes(plan), st>>>(a);
+  k_allpairs<kMinB><<<grid, kThreads64, allpairs_smem_bytes(plan), st>>>(a);
   return cudaGetLastError();
 }
 

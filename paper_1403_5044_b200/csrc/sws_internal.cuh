@@ -59,10 +59,7 @@ struct PairPlan {
   int cols_per_chunk;  // ceil(N / chunks)
 };
 
-#ifndef SWS_PAIR_THREADS
-#define SWS_PAIR_THREADS 128
-#endif
-constexpr int kPairThreads = SWS_PAIR_THREADS;  // threads (= targets) per CTA of the all-pairs kernel
+constexpr int kPairThreads = 128;  // threads (= targets) per CTA of the FP32 and the linearised all-pairs kernels
 constexpr int kSegMax = 256;       // max nodes staged per bulk copy (10 KB per stage)
 constexpr int kStages = 2;         // staging ring depth
 constexpr double kEmRadius = 8.0;  // default far-field radius of the S2 column sums, in units of dy

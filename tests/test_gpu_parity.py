@@ -120,7 +120,7 @@ def test_chunking_invariance_and_determinism(sws, oracle80):
         F_again = ctx.residual(ud).cpu().numpy()
         assert np.array_equal(F_auto, F_again)
         info = ctx.plan_info(1)
-        assert info["tiles"] == -(-cfg.targets // 128)
+        assert info["tiles"] == -(-cfg.targets // 64)
         for ch in (1, 2, 5):
             ctx.set_tuning(ch)
             Fc = ctx.residual(ud).cpu().numpy()
