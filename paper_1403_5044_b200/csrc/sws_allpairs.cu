@@ -5,17 +5,19 @@
 //   K1 (L107, reading Q1/Q2), K2 (L109), S2 = S2_direct + S2_image (eqs. (21),(22) L169-172),
 //   w(i,j) = dx dy c_i c_j, c = 1/2 on the first/last index (L189, reading Q4).
 //
-// Mapping (B200): one thread = one target, 128 targets per CTA; a CTA walks a group of
-// source COLUMNS (fixed x_i, all y_j).  Each column (M records of 32 B, contiguous in the
+// Mapping (B200): one thread = one target, 64 targets per CTA, 8 CTAs per SM; a CTA walks a group
+// of ~12 source COLUMNS (fixed x_i, all y_j).  Each column (M records of 32 B, contiguous in the
 // transposed SrcRec layout) is brought into shared memory by ONE bulk async copy
 // (cp.async.bulk -> UBLKCP, completion on an mbarrier), double buffered.  Every lane of a
 // warp reads the same record (shared-memory broadcast), so the kernel is bound by the FP64
-// pipe: 45 FP64 instructions + 4 MUFU.RSQ64H per pair.  Everything that depends only on
-// (target, column) - dx, dx^2 and the completed-square constants of S2 - is hoisted out of the j loop; the half
-// weights are applied by peeling the first/last node and scaling edge columns, so the
-// inner loop carries no weight multiply.  Partial sums per (state, chunk, target) are
-// written to global memory and added in a fixed order by the assemble kernel: no atomics,
-// bitwise repeatable.
+// pipe.  Columns at least 8 dy away from all 32 targets of a warp ("far", 93.5 % at 721x241)
+// take their S2 terms - which do not depend on the source data - from the Euler-Maclaurin form of
+// the column sum (sws_farfield.cuh): 29 FP64 instructions + 2 MUFU.RSQ64H per pair; the others
+// sum S2 pair by pair: 45 + 4.  Everything that depends only on (target, column) - dx, dx^2 and
+// the completed-square constants of S2 - is hoisted out of the j loop; the half weights are
+// applied by peeling the first/last node and scaling edge columns, so the inner loop carries no
+// weight multiply.  Partial sums per (state, chunk, target) are written to global memory and
+// added in a fixed order by the assemble kernel: no atomics, bitwise repeatable.
 #include "sws_farfield.cuh"
 #include "sws_internal.cuh"
 #include "sws_stage.cuh"
