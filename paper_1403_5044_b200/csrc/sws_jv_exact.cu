@@ -45,6 +45,9 @@ namespace sws {
 #ifndef SWS_LIN_MINB16
 #define SWS_LIN_MINB16 3
 #endif
+#ifndef SWS_LIN_THREADS
+#define SWS_LIN_THREADS 128  // threads (= targets) per CTA of k_allpairs_lin
+#endif
 
 // ---------------------------------------------------------------------------------------
 // Per node / per target linearisation for direction d (grid.z).  Base fields = state 0 of the
@@ -247,10 +250,12 @@ struct LinArgs {
 };
 
 constexpr int kLinUnroll = SWS_LIN_UNROLL;
+constexpr int kLinThreads = SWS_LIN_THREADS;
 constexpr int kLinShared = 6;  // direction-independent sums per (chunk, target)
 
 template <int BT, int MODE>
-__global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT >= 8 ? 3 : 4)) k_allpairs_lin(const LinArgs a) {
+__global__ void __launch_bounds__(kLinThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT >= 8 ? 3 : 4) * (128 / kLinThreads))
+    k_allpairs_lin(const LinArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int DV = MODE == 1 ? 0 : BT;          // direction records staged per node
   constexpr int NSH = MODE == 2 ? 0 : kLinShared; // direction-independent sums written
@@ -262,7 +267,7 @@ __global__ void __launch_bounds__(kPairThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT 
 
   const int tid = threadIdx.x;
   const int tile = blockIdx.x, chunk = blockIdx.y, group = blockIdx.z;
-  const int t = tile * kPairThreads + tid;
+  const int t = tile * kLinThreads + tid;
   const int tc = t < a.T ? t : a.T - 1;
 
   const TgtRec tr = a.tgt[tc];
@@ -460,7 +465,7 @@ static cudaError_t lin_configure_one(int* occ) {
   cudaError_t e = cudaFuncSetAttribute(k_allpairs_lin<BT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)smem + 64);
   if (e != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, k_allpairs_lin<BT, MODE>, kPairThreads, smem);
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, k_allpairs_lin<BT, MODE>, kLinThreads, smem);
 }
 
 cudaError_t lin_configure(sws_ctx* c) {
@@ -490,7 +495,7 @@ PairPlan make_lin_plan(const sws_ctx* c, int BT, int groups, int mode) {
   const Mesh& m = c->mesh;
   const int DV = mode == 1 ? 0 : BT, rows = (mode == 2 ? 0 : kLinShared) + DV;
   PairPlan p;
-  p.tiles = (m.T + kPairThreads - 1) / kPairThreads;
+  p.tiles = (m.T + kLinThreads - 1) / kLinThreads;
   const int cap = lin_seg_cap(DV);
   p.nseg = (m.M + cap - 1) / cap;
   int seg = (m.M + p.nseg - 1) / p.nseg;
@@ -538,7 +543,7 @@ static cudaError_t launch_lin_t(sws_ctx* c, int groups, const PairPlan& plan, cu
   a.seg_len = plan.seg_len; a.nseg = plan.nseg;
   a.em = em_geometry(c);
   dim3 grid(plan.tiles, plan.chunks, groups);
-  k_allpairs_lin<BT, MODE><<<grid, kPairThreads, lin_smem_bytes(MODE == 1 ? 0 : BT, plan.seg_len), st>>>(a);
+  k_allpairs_lin<BT, MODE><<<grid, kLinThreads, lin_smem_bytes(MODE == 1 ? 0 : BT, plan.seg_len), st>>>(a);
   return cudaGetLastError();
 }
 

@@ -100,6 +100,28 @@ def test_residual_ragged_shapes(sws, oracle80, kw, dy_scheme):
     assert relerr(F, E) <= TOL
 
 
+@pytest.mark.parametrize("ratio", [0.55, 1.8])
+def test_residual_and_jv_anisotropic_mesh(sws, oracle80, oracleC, ratio):
+    """dx != dy (the configs all have dx = dy): the far-field switch works in units of dy while the
+    distance to a column is a multiple of dx; residual, analytic Jv and the on/off equivalence."""
+    cfg = W.custom(eps=0.4, amp=0.08, N=96, M=37, h=0.25, x1=-5.0, seed=31)
+    p = cfg.params()
+    p["dy"] = ratio * p["dx"]
+    u = W.state(cfg) + 1e-3 * np.random.default_rng(8).standard_normal(cfg.n)
+    V = W.directions(cfg, 2)
+    E = oracle80.residual(p, u)
+    ref = oracleC.jv_exact(p, u, V[0])
+    with sws.Context(p, max_batch=2) as ctx:
+        F = ctx.residual(dev(u)).cpu().numpy()
+        near = ctx.farfield_stats(1)
+        JV = ctx.jv_exact_batch(dev(u), dev(V)).cpu().numpy()
+        ctx.set_farfield(0.0)
+        F0 = ctx.residual(dev(u)).cpu().numpy()
+    assert 0.0 < near < 1.0
+    assert relerr(F, E) <= TOL and relerr(F0, E) <= TOL and relerr(F, F0) <= 2e-13
+    assert np.abs(JV[0] - ref).max() <= TOL * np.abs(ref).max()
+
+
 def test_uniform_stream_is_a_zero(sws):
     """eps = 0, u = u_0 (L227): F == 0 to round-off (pin P6, on the GPU path)."""
     import dataclasses
