@@ -432,8 +432,12 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
       CKB(cublasDgeam(hb_blas, CUBLAS_OP_T, CUBLAS_OP_N, n1, n1, &one, Sinv, n1, &zero, Fk + (size_t)lk * n1, Kf,
                       Fk + (size_t)lk * n1, Kf));
       if (uk > 0) {
-        double* Uk = Pk + blk * (hb + 1);  // S~k,k+1..k+uk -> S~kk^-1 S~k,*
-        CKB(cusolverDnDgetrs(hb_sol, CUBLAS_OP_N, n1, uk * n1, Dkk, n1, ipiv, Uk, n1, info + 2 * k + 1));
+        // S~kk^-1 S~k,k+1..k+uk by ONE product with the explicit inverse formed above (a getrs on this
+        // wide right-hand side spends most of its time in row interchanges and triangular solves: 60 % of
+        // the whole set-up when it was used here)
+        const double* Uk0 = Pk + blk * (hb + 1);
+        double* Uk = W;  // n1 x uk n1, column-major (W's use for the forward panel above is stream-ordered)
+        CKB(cublasDgemm(hb_blas, CUBLAS_OP_N, CUBLAS_OP_N, n1, uk * n1, n1, &one, Sinv, n1, Uk0, n1, &zero, Uk, n1));
         double* Bk = pc->bwd + pc->bwd_off[k];
         CKB(cublasDgeam(hb_blas, CUBLAS_OP_T, CUBLAS_OP_N, uk * n1, n1, &one, Uk, n1, &zero, Bk, uk * n1, Bk, uk * n1));
         for (int i = k + 1; i <= k + uk; ++i) {
