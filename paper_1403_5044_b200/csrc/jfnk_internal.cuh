@@ -23,7 +23,7 @@ struct LinMesh {
   double a11, a12;  // n - x1/dx, x1/dx
 };
 
-constexpr int kGemvThreads = 128;
+constexpr int kGemvThreads = 256;
 constexpr int kDotBlocks = 296;   // 2 CTAs per SM on 148 SMs
 constexpr int kDotThreads = 256;
 

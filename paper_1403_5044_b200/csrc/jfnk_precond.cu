@@ -194,7 +194,45 @@ __device__ __forceinline__ double cta_sum(double v, double* red) {
   return s;
 }
 
+// dot product of one panel row with a vector, both of length K: 16-byte loads, four independent
+// accumulators per thread (these kernels only stream the factor panels: ~62 MB per launch at 721x241,
+// so what matters is the number of bytes in flight per SM); K even and 16-byte aligned operands when VEC
+template <bool VEC>
+__device__ __forceinline__ double row_dot(const double* __restrict__ row, const double* __restrict__ x, int K) {
+  double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+  if (VEC) {
+    const double2* r2 = reinterpret_cast<const double2*>(row);
+    const double2* x2 = reinterpret_cast<const double2*>(x);
+    const int K2 = K >> 1;
+    int c = threadIdx.x;
+    for (; c + 3 * kGemvThreads < K2; c += 4 * kGemvThreads) {
+      const double2 a0 = __ldcs(r2 + c), a1 = __ldcs(r2 + c + kGemvThreads), a2 = __ldcs(r2 + c + 2 * kGemvThreads),
+                    a3 = __ldcs(r2 + c + 3 * kGemvThreads);
+      const double2 b0 = x2[c], b1 = x2[c + kGemvThreads], b2 = x2[c + 2 * kGemvThreads], b3 = x2[c + 3 * kGemvThreads];
+      acc0 = fma(a0.x, b0.x, acc0); acc0 = fma(a0.y, b0.y, acc0);
+      acc1 = fma(a1.x, b1.x, acc1); acc1 = fma(a1.y, b1.y, acc1);
+      acc2 = fma(a2.x, b2.x, acc2); acc2 = fma(a2.y, b2.y, acc2);
+      acc3 = fma(a3.x, b3.x, acc3); acc3 = fma(a3.y, b3.y, acc3);
+    }
+    for (; c < K2; c += kGemvThreads) {
+      const double2 a0 = __ldcs(r2 + c), b0 = x2[c];
+      acc0 = fma(a0.x, b0.x, acc0); acc0 = fma(a0.y, b0.y, acc0);
+    }
+  } else {
+    int c = threadIdx.x;
+    for (; c + 3 * kGemvThreads < K; c += 4 * kGemvThreads) {
+      acc0 = fma(row[c], x[c], acc0);
+      acc1 = fma(row[c + kGemvThreads], x[c + kGemvThreads], acc1);
+      acc2 = fma(row[c + 2 * kGemvThreads], x[c + 2 * kGemvThreads], acc2);
+      acc3 = fma(row[c + 3 * kGemvThreads], x[c + 3 * kGemvThreads], acc3);
+    }
+    for (; c < K; c += kGemvThreads) acc0 = fma(row[c], x[c], acc0);
+  }
+  return (acc0 + acc1) + (acc2 + acc3);
+}
+
 // y_k = [ -W_k | Sinv_k ] [ y_{k-lk..k-1} ; t_k ]      (forward: L~ y = t with unit... see header)
+template <bool VEC>
 __global__ void __launch_bounds__(kGemvThreads) k_fwd_row(const double* __restrict__ panel, int n1, int lk,
                                                           const double* __restrict__ yprev,
                                                           const double* __restrict__ tk,
@@ -203,38 +241,19 @@ __global__ void __launch_bounds__(kGemvThreads) k_fwd_row(const double* __restri
   const int r = blockIdx.x;
   const int K0 = lk * n1;
   const double* row = panel + (size_t)r * (K0 + n1);
-  double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
-  int c = threadIdx.x;
-  for (; c + 3 * kGemvThreads < K0; c += 4 * kGemvThreads) {
-    acc0 = fma(row[c], yprev[c], acc0);
-    acc1 = fma(row[c + kGemvThreads], yprev[c + kGemvThreads], acc1);
-    acc2 = fma(row[c + 2 * kGemvThreads], yprev[c + 2 * kGemvThreads], acc2);
-    acc3 = fma(row[c + 3 * kGemvThreads], yprev[c + 3 * kGemvThreads], acc3);
-  }
-  for (; c < K0; c += kGemvThreads) acc0 = fma(row[c], yprev[c], acc0);
-  for (c = threadIdx.x; c < n1; c += kGemvThreads) acc1 = fma(row[K0 + c], tk[c], acc1);
-  const double s = cta_sum((acc0 + acc1) + (acc2 + acc3), red);
+  const double s = cta_sum(row_dot<VEC>(row, yprev, K0) + row_dot<VEC>(row + K0, tk, n1), red);
   if (threadIdx.x == 0) yk[r] = s;
 }
 
 // x_k = y_k - U_k x_{k+1..k+uk}   (in place on y)
+template <bool VEC>
 __global__ void __launch_bounds__(kGemvThreads) k_bwd_row(const double* __restrict__ panel, int n1, int uk,
                                                           const double* __restrict__ xnext,
                                                           double* __restrict__ yk) {
   __shared__ double red[kGemvThreads / 32];
   const int r = blockIdx.x;
   const int K = uk * n1;
-  const double* row = panel + (size_t)r * K;
-  double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
-  int c = threadIdx.x;
-  for (; c + 3 * kGemvThreads < K; c += 4 * kGemvThreads) {
-    acc0 = fma(row[c], xnext[c], acc0);
-    acc1 = fma(row[c + kGemvThreads], xnext[c + kGemvThreads], acc1);
-    acc2 = fma(row[c + 2 * kGemvThreads], xnext[c + 2 * kGemvThreads], acc2);
-    acc3 = fma(row[c + 3 * kGemvThreads], xnext[c + 3 * kGemvThreads], acc3);
-  }
-  for (; c < K; c += kGemvThreads) acc0 = fma(row[c], xnext[c], acc0);
-  const double s = cta_sum((acc0 + acc1) + (acc2 + acc3), red);
+  const double s = cta_sum(row_dot<VEC>(panel + (size_t)r * K, xnext, K), red);
   if (threadIdx.x == 0) yk[r] -= s;
 }
 
@@ -487,17 +506,25 @@ int sws_precond_apply(sws_precond* pc, const double* v_dev, double* r_dev, void*
   const LinMesh& m = pc->lm;
   const int n1 = m.n1, M = m.M, hb = pc->hb;
   const size_t sh = 2 * (size_t)n1 * sizeof(double);
+  const bool vec = (n1 % 2) == 0;  // rows, y and t blocks then start on 16-byte boundaries
   k_stage1<<<M, 256, sh, st>>>(m, v_dev, pc->s1, pc->t2);
   for (int k = 0; k < M; ++k) {
     const int lk = k < hb ? k : hb;
-    k_fwd_row<<<n1, kGemvThreads, 0, st>>>(pc->fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
-                                           pc->t2 + (size_t)k * n1, pc->y + (size_t)k * n1);
+    if (vec)
+      k_fwd_row<true><<<n1, kGemvThreads, 0, st>>>(pc->fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
+                                                   pc->t2 + (size_t)k * n1, pc->y + (size_t)k * n1);
+    else
+      k_fwd_row<false><<<n1, kGemvThreads, 0, st>>>(pc->fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
+                                                    pc->t2 + (size_t)k * n1, pc->y + (size_t)k * n1);
   }
   for (int k = M - 2; k >= 0; --k) {
     const int uk = (M - 1 - k) < hb ? (M - 1 - k) : hb;
-    if (uk > 0)
-      k_bwd_row<<<n1, kGemvThreads, 0, st>>>(pc->bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
-                                             pc->y + (size_t)k * n1);
+    if (uk > 0 && vec)
+      k_bwd_row<true><<<n1, kGemvThreads, 0, st>>>(pc->bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
+                                                   pc->y + (size_t)k * n1);
+    else if (uk > 0)
+      k_bwd_row<false><<<n1, kGemvThreads, 0, st>>>(pc->bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
+                                                    pc->y + (size_t)k * n1);
   }
   k_stage3<<<M, 256, sh, st>>>(m, pc->s1, pc->y, r_dev);
   cudaError_t e = cudaGetLastError();
