@@ -270,7 +270,7 @@ def test_farfield_on_off_equivalence(sws, oracle80, name):
     assert relerr(F_on, E) <= TOL and relerr(F_off, E) <= TOL
 
 
-@pytest.mark.parametrize("i,rows", [(3, 192), (4, 96)])
+@pytest.mark.parametrize("i,rows", [(3, 2048), (4, 2048)])
 def test_large_configs_sampled_rows(sws, oracle80, i, rows):
     """cfg 4 and cfg 5 at full size in the launch configuration bench.py times: the O(NM) rows
     in full, and a seeded sample of integral-equation rows the oracle computes one by one."""
@@ -338,7 +338,7 @@ def test_jv_batch_cfg5_bench_configuration(sws, oracle80):
     assert b == 16
     rng = np.random.default_rng(77)
     T = cfg.targets
-    pick = np.unique(np.concatenate([rng.integers(0, T, 40), [0, T - 1, cfg.N - 2]])).astype(np.int32)
+    pick = np.unique(np.concatenate([rng.integers(0, T, 512), [0, T - 1, cfg.N - 2]])).astype(np.int32)
     with sws.Context(p, max_batch=b) as ctx:
         ud, Vd = dev(u), dev(V)
         JV, Fp, F0 = ctx.jv_batch(ud, Vd, want_fpert=True, want_f0=True)
@@ -534,7 +534,7 @@ def test_jv_exact_cfg3_batch16(sws, oracleC):
         assert relerr(JV_fd[k], JV[k]) <= 1e-5
 
 
-@pytest.mark.parametrize("i,rows,dirs", [(3, 64, (0, 31)), (4, 32, (0, 15))])
+@pytest.mark.parametrize("i,rows,dirs", [(3, 512, (0, 31)), (4, 256, (0, 15))])
 def test_jv_exact_large_configs_sampled_rows(sws, oracleC, i, rows, dirs):
     """cfg 4 (b = 32, two direction tiles) and cfg 5 (b = 16) at full size, in the launch
     configuration bench.py times: all O(NM) rows and a seeded sample of integral-equation rows of
@@ -614,7 +614,7 @@ def test_jv_apply_cfg5_sampled_rows_and_state(sws, oracleC):
     p, u, V = cfg.params(), W.state(cfg), W.directions(cfg)
     rng = np.random.default_rng(99)
     T = cfg.targets
-    pick = np.unique(np.concatenate([rng.integers(0, T, 24), [0, cfg.N - 2, T - 1]])).astype(np.int32)
+    pick = np.unique(np.concatenate([rng.integers(0, T, 256), [0, cfg.N - 2, T - 1]])).astype(np.int32)
     with sws.Context(p, max_batch=16) as ctx:
         with pytest.raises(sws.SwsError, match="linearis"):
             ctx.jv_apply(dev(V[0]))
