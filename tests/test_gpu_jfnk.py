@@ -286,3 +286,46 @@ def test_newton_paper_mesh_91x31(mods, oracle64):
         assert np.array_equal(u3.cpu().numpy(), un)
     zeta_x = un[c.n // 2:].reshape(c.M, c.N + 1)[:, 1:]
     assert np.abs(zeta_x).max() > 0.05      # a real wave pattern, not the flat state
+
+
+def _centreline(u, c):
+    """zeta on the line y = y_1 from the unknowns (eq. (18) layout, trapezoid rule (19))."""
+    half = (c.N + 1) * c.M
+    zb = u[half:].reshape(c.M, c.N + 1)
+    z1, zx = zb[0, 0], zb[0, 1:]
+    return np.concatenate([[z1], z1 + np.cumsum(0.5 * c.h * (zx[1:] + zx[:-1]))])
+
+
+def _wavelength(x, z, lo, hi):
+    sel = (x > lo) & (x < hi)
+    xs, zs = x[sel], z[sel]
+    i = np.where(np.sign(zs[:-1]) != np.sign(zs[1:]))[0]
+    xz = xs[i] - zs[i] * (xs[i + 1] - xs[i]) / (zs[i + 1] - zs[i])
+    assert len(xz) >= 8
+    return 2.0 * float(np.mean(np.diff(xz)))
+
+
+def test_wave_pattern_physics(mods):
+    """A pin of the whole method on something neither program defines: the converged free surface carries
+    the steady transverse waves of linear theory.  Their wavenumber on the centre line is 1/F^2 in the
+    paper's scaling (lengths by the source depth, L85), i.e. wavelength 2 pi F^2, approached at O(h^2);
+    they trail the source (radiation condition (24): nothing upstream); and the wavelength scales as F^2."""
+    sws, jf = mods
+    lam, quiet = {}, {}
+    for key, (N, M, h, x1, F, bw) in {"h0.3": (181, 61, 0.3, -14.0, 0.7, 15), "h0.2": (241, 41, 0.2, -10.0, 0.7, 21),
+                                      "F0.9": (181, 61, 0.3, -14.0, 0.9, 15)}.items():
+        c = W.custom(N, M, h, x1, eps=0.3, froude=F)
+        p = c.params()
+        with sws.Context(p, max_batch=1) as ctx, jf.Preconditioner(p, bandwidth=bw) as pc, jf.Solver(ctx, pc, 60) as s:
+            u, log, st = s.newton(dev(W.flat_state(c)), ftol=1e-10, eta=1e-3, restart=60, gmres_maxit=120, jv_mode=2)
+        assert st["converged"]
+        x = x1 + h * np.arange(N)
+        z = _centreline(u.cpu().numpy(), c)
+        lam[key] = _wavelength(x, z, 4.0, x[-1] - 4.0)
+        quiet[key] = np.abs(z[x < -4.0]).max() / np.abs(z[x > 2.0]).max()
+    th = 2 * np.pi * 0.7 ** 2
+    e3, e2 = lam["h0.3"] - th, lam["h0.2"] - th
+    assert abs(e3) <= 0.10 * th and abs(e2) <= 0.05 * th
+    assert 1.6 <= e3 / e2 <= 3.2                              # (0.3 / 0.2)^2 = 2.25
+    assert lam["F0.9"] / lam["h0.3"] == pytest.approx((0.9 / 0.7) ** 2, rel=0.08)
+    assert max(quiet.values()) <= 0.1
