@@ -36,8 +36,11 @@
  * for the complex-step Jacobian action: PJ1 the same closed forms B.5/B.6/B.2
  * to round-off, PJ2 Richardson-extrapolated central differences of the f80
  * residual at a nonlinear state, PJ3 the linear radiation rows applied to v.
- * Beyond those the residual's absolute values are "parity unpinned" (the
- * paper prints no numeric value of E for any worked example).
+ * PW (tests/test_oracle_jfnk.py): the ROOT of this residual, found by the oracle's
+ * own Newton driver, is the steady wave pattern of linear theory (centre-line
+ * wavelength 2 pi F^2 under refinement, F^2 scaling, nothing upstream).
+ * Beyond those the residual's absolute values at an arbitrary u are "parity
+ * unpinned" (the paper prints no numeric value of E for any worked example).
  */
 #include <math.h>
 #include <stdlib.h>

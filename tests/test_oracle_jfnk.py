@@ -259,3 +259,42 @@ def test_jfnk_reaches_the_root_of_dense_newton(oracle64, oracleC):
     assert np.abs(res(ud)).max() <= 1e-12
     assert np.abs(u - ud).max() <= 1e-9
     assert np.abs(u - W.flat_state(c)).max() > 1e-2      # the root is not the flat state
+
+
+# ----------------------------------------------------------------------------
+# PW: the ORACLE's residual has the steady wave pattern of linear theory as its root.  Nothing in the
+# paper prints a value of E, but the physics fixes what a root of E = 0 looks like: transverse waves of
+# wavenumber 1/F^2 on the centre line (lengths scaled by the source depth, L85), i.e. wavelength
+# 2 pi F^2, downstream of the source only (radiation condition (24)).  A wrong sign or factor in the
+# Bernoulli row (13), in the 2 pi phi term or in the kernels of (12), or radiation rows on the wrong end,
+# moves the wavelength or puts the waves upstream.
+# ----------------------------------------------------------------------------
+def _centreline_waves(oracle64, oracleC, N, M, h, x1, F, eps=0.3):
+    import scipy.linalg as sl
+    c = W.custom(N, M, h, x1, eps=eps, froude=F)
+    p = c.params()
+    lu = sl.lu_factor(J.linear_jacobian(p, oracle64.box_integral))
+    u, log = J.newton(lambda u: oracle64.residual(p, u), lambda u, v: oracleC.jv_exact(p, u, v),
+                      lambda v: sl.lu_solve(lu, v), W.flat_state(c), ftol=1e-10, eta=1e-3, restart=40, gmres_maxit=80)
+    assert log[-1]["finf"] <= 1e-10
+    zb = u[(N + 1) * M:].reshape(M, N + 1)
+    z1, zx = zb[0, 0], zb[0, 1:]
+    z = np.concatenate([[z1], z1 + np.cumsum(0.5 * h * (zx[1:] + zx[:-1]))])   # eq. (19) on y = 0
+    x = x1 + h * np.arange(N)
+    sel = (x > 3.0) & (x < x[-1] - 3.0)
+    xs, zs = x[sel], z[sel]
+    i = np.where(np.sign(zs[:-1]) != np.sign(zs[1:]))[0]
+    xz = xs[i] - zs[i] * (xs[i + 1] - xs[i]) / (zs[i + 1] - zs[i])
+    assert len(xz) >= 5
+    return 2.0 * float(np.mean(np.diff(xz))), float(np.abs(z[x < -3.0]).max() / np.abs(z[x > 2.0]).max())
+
+
+def test_oracle_root_is_the_kelvin_wave_pattern(oracle64, oracleC):
+    th = 2 * PI * 0.7 ** 2
+    lam3, quiet3 = _centreline_waves(oracle64, oracleC, 91, 11, 0.3, -9.0, 0.7)
+    lam2, quiet2 = _centreline_waves(oracle64, oracleC, 121, 9, 0.2, -6.0, 0.7)
+    assert abs(lam3 - th) <= 0.12 * th and abs(lam2 - th) <= 0.05 * th
+    assert abs(lam2 - th) < abs(lam3 - th)                 # converging under refinement
+    assert quiet3 <= 0.12 and quiet2 <= 0.12               # waves trail the source
+    lam9, _ = _centreline_waves(oracle64, oracleC, 91, 11, 0.3, -9.0, 0.9)
+    assert lam9 / lam3 == pytest.approx((0.9 / 0.7) ** 2, rel=0.10)
