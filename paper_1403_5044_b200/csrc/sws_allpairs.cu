@@ -238,7 +238,10 @@ cudaError_t allpairs_configure(int* occ_out) {
 // The split depends on the MESH ONLY, never on the number of states in the launch: the
 // summation order of a state's quadrature is then the same in sws_residual and in every
 // slot of sws_jv_batch, so a batch is bitwise a loop of single evaluations.
-constexpr int kColsTarget = 12;
+#ifndef SWS_COLS_TARGET
+#define SWS_COLS_TARGET 12
+#endif
+constexpr int kColsTarget = SWS_COLS_TARGET;
 
 PairPlan make_plan(const sws_ctx* c) {
   const Mesh& m = c->mesh;
