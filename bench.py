@@ -564,6 +564,19 @@ def run_ours(args) -> None:
     replicas.finalize()
 
 
+def run_microbench(args) -> None:
+    """--microbench: the FP64 instruction-mix probes behind the cycle model of DESIGN.md section 6, one JSON
+    line (not a bench value: no workload is run)."""
+    import torch
+
+    import paper_1403_5044_b200 as sws
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --microbench: no CUDA device")
+    rows = [sws.probe_fp64_mix(k, w) for k in range(len(sws.FP64_MIX_KINDS)) for w in (16, 32, 64)]
+    print(json.dumps({"microbench": "fp64_instruction_mix", "unit": "FP64 thread-instructions / SM / clk (64 = issue limit)",
+                      "rows": rows, "dfma_probe": sws.probe_fp64_peak(0)}), flush=True)
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -578,7 +591,11 @@ def main() -> None:
     ap.add_argument("--no-jv-exact", action="store_true", help="skip the analytic-Jv section")
     ap.add_argument("--no-solve", action="store_true", help="skip the full JFNK solve section")
     ap.add_argument("--no-table1", action="store_true", help="skip the paper's Table 1 meshes")
+    ap.add_argument("--microbench", action="store_true", help="only run the FP64 instruction-mix probes")
     args = ap.parse_args()
+    if args.microbench:
+        run_microbench(args)
+        return
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)
     if args.impl == "reference":

@@ -199,6 +199,15 @@ const char* sws_last_cuda_error(void);
  * device clock64/globaltimer ratio. */
 int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, double* sm_mhz);
 
+/* Instruction-mix probes behind the cycle model of DESIGN.md section 6 (register-only loops, one wave
+ * of 256-thread CTAs, warps_per_sm in {8, 16, ..., 64}).  kind: 0 DFMA with two distinct register
+ * sources; 1 DFMA with three distinct register sources; 2 DADD; 3 DMUL; 4 eleven two-register DFMA +
+ * DADD + DMUL + one MUFU.RSQ64H (+ the move that zeroes the seed's low word); 5 eleven two-register
+ * DFMA + three integer instructions.  Reports FP64 thread-instructions per SM per clock (64 = the
+ * pipe's issue limit) and the SM clock during the loop. */
+int sws_probe_fp64_mix(int32_t device, int32_t kind, int32_t warps_per_sm, double* fp64_instr_per_sm_clk,
+                       double* sm_mhz);
+
 /* y[i] = the library's device reciprocal square root of x[i] (host buffers), for the
  * unit test of that primitive. */
 int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, int32_t n);

@@ -27,7 +27,7 @@ SYMBOLS = (
     "sws_probe_fp64_peak", "sws_debug_rsqrt_host",
     "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
     "sws_get_params", "sws_linearize", "sws_jv_apply",
-    "sws_set_farfield", "sws_farfield_stats", "sws_debug_s2col_host", "sws_set_eps",
+    "sws_set_farfield", "sws_farfield_stats", "sws_debug_s2col_host", "sws_set_eps", "sws_probe_fp64_mix",
 )
 
 
@@ -87,6 +87,7 @@ def load_library() -> C.CDLL:
         "sws_debug_rsqrt_host": (C.c_int, [C.c_int32, dp, dp, C.c_int32]),
         "sws_set_farfield": (C.c_int, [vp, C.c_double]),
         "sws_set_eps": (C.c_int, [vp, C.c_double]),
+        "sws_probe_fp64_mix": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
         "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
         "sws_debug_s2col_host": (C.c_int, [C.c_int32, C.c_double, C.c_double, C.c_int32, dp, dp, C.c_int32,
                                            C.c_int32, dp, dp]),
@@ -341,6 +342,19 @@ def probe_fp64_peak(device: int = 0) -> dict:
     _check(lib.sws_probe_fp64_peak(int(device), C.byref(tf), C.byref(sms), C.byref(mhz)),
            "sws_probe_fp64_peak")
     return dict(tflops=tf.value, sm_count=int(sms.value), sm_mhz=mhz.value)
+
+
+FP64_MIX_KINDS = ("dfma_2reg", "dfma_3reg", "dadd", "dmul", "dfma11_dadd_dmul_mufu_rsq64h", "dfma11_int3")
+
+
+def probe_fp64_mix(kind: int, warps_per_sm: int = 16, device: int = 0) -> dict:
+    """sws_probe_fp64_mix: FP64 thread-instructions per SM per clock of one instruction mix."""
+    lib = load_library()
+    r, mhz = C.c_double(), C.c_double()
+    _check(lib.sws_probe_fp64_mix(int(device), int(kind), int(warps_per_sm), C.byref(r), C.byref(mhz)),
+           "sws_probe_fp64_mix")
+    return {"kind": FP64_MIX_KINDS[kind], "warps_per_sm": int(warps_per_sm), "fp64_instr_per_sm_clk": r.value,
+            "sm_mhz": mhz.value}
 
 
 def debug_rsqrt(x: np.ndarray, device: int = 0) -> np.ndarray:

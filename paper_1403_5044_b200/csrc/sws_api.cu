@@ -16,6 +16,7 @@ namespace sws {
 cudaError_t launch_debug_rsqrt(const double* x, double* y, int n, cudaStream_t st);
 cudaError_t launch_fp64_probe(int blocks, int iters, double* sink, unsigned long long* clk,
                               cudaStream_t st);
+cudaError_t launch_fp64_mix(int kind, int blocks, int iters, double* sink, unsigned long long* clk, cudaStream_t st);
 }  // namespace sws
 
 static thread_local char g_cuda_err[256] = "";
@@ -593,6 +594,54 @@ int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, doubl
   cudaFree(clk);
   *tflops = best;
   if (sm_count) *sm_count = sms;
+  if (sm_mhz) *sm_mhz = mhz;
+  return SWS_OK;
+}
+
+int sws_probe_fp64_mix(int32_t device, int32_t kind, int32_t warps_per_sm, double* fp64_instr_per_sm_clk,
+                       double* sm_mhz) {
+  if (!fp64_instr_per_sm_clk || kind < 0 || kind > 5) return SWS_EINVAL;
+  if (warps_per_sm < 8 || warps_per_sm > 64 || warps_per_sm % 8) return SWS_EINVAL;
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (device < 0 || device >= ndev) return SWS_EINVAL;
+  CK(cudaSetDevice(device));
+  cudaDeviceProp prop;
+  CK(cudaGetDeviceProperties(&prop, device));
+  const int sms = prop.multiProcessorCount;
+  const int blocks = sms * (warps_per_sm / 8), threads = 256, iters = 1 << 15;
+  static const int fp64_per_iter[6] = {12, 12, 12, 12, 13, 11};
+  double* sink = nullptr;
+  unsigned long long* clk = nullptr;
+  CK(cudaMalloc((void**)&sink, (size_t)blocks * threads * sizeof(double)));
+  CK(cudaMalloc((void**)&clk, 4 * sizeof(unsigned long long)));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  cudaError_t e = cudaEventCreate(&e0);
+  if (e == cudaSuccess) e = cudaEventCreate(&e1);
+  if (e == cudaSuccess) e = sws::launch_fp64_mix(kind, blocks, iters / 8, sink, clk, 0);  // warm-up
+  double best = 0.0, mhz = 0.0;
+  for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {
+    e = cudaEventRecord(e0, 0);
+    if (e == cudaSuccess) e = sws::launch_fp64_mix(kind, blocks, iters, sink, clk, 0);
+    if (e == cudaSuccess) e = cudaEventRecord(e1, 0);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    unsigned long long h[4] = {0, 0, 0, 0};
+    if (e == cudaSuccess) e = cudaMemcpy(h, clk, sizeof h, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess || h[1] <= h[0] || h[3] <= h[2] || ms <= 0.f) break;
+    // whole-launch time by CUDA events; SM clock during the loop from block 0's clock64 / globaltimer
+    const double clk_mhz = (double)(h[1] - h[0]) / (double)(h[3] - h[2]) * 1e3;
+    const double total = (double)fp64_per_iter[kind] * iters * threads * blocks;
+    const double rate = total / (ms * 1e-3 * clk_mhz * 1e6) / sms;
+    if (rate > best) { best = rate; mhz = clk_mhz; }
+  }
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  cudaFree(sink);
+  cudaFree(clk);
+  CK(e);
+  *fp64_instr_per_sm_clk = best;
   if (sm_mhz) *sm_mhz = mhz;
   return SWS_OK;
 }

@@ -30,6 +30,83 @@ __global__ void __launch_bounds__(256) k_fp64_probe(int iters, double* sink, uns
       ((r0 + r1) + (r2 + r3)) + ((r4 + r5) + (r6 + r7)) + ((q0 + q1) + (q2 + q3)) + ((q4 + q5) + (q6 + q7));
 }
 
+// ---------------------------------------------------------------------------------------
+// Instruction-mix probes behind the cycle model of DESIGN.md section 6.  Each runs 12 independent
+// chains per thread, `iters` times, register only.  KIND:
+//   0  DFMA with two distinct register sources      r = fma(r, r, b)
+//   1  DFMA with three distinct register sources    r_i = fma(r_i, q_i, s_i)   (no operand shared between
+//      neighbouring instructions, so the operand-reuse cache cannot help)
+//   2  DADD, two distinct registers                 r = r + b
+//   3  DMUL, two distinct registers                 r = r * a
+//   4  11 two-register DFMA + 1 MUFU.RSQ64H
+//   5  11 two-register DFMA + 3 integer instructions
+template <int KIND>
+__global__ void __launch_bounds__(256) k_fp64_mix(int iters, double* sink, unsigned long long* clk) {
+  const double a = 1.0 - 1e-9 * (threadIdx.x + 1), b = 1e-3 + 1e-12 * (blockIdx.x + 1);
+  double r[12], q[12], s[12];
+#pragma unroll
+  for (int i = 0; i < 12; ++i) {
+    r[i] = 0.1 + 0.01 * i + 1e-6 * threadIdx.x;
+    q[i] = 0.999 - 1e-4 * i - 1e-9 * threadIdx.x;
+    s[i] = 1e-4 * (i + 1) + 1e-10 * threadIdx.x;
+  }
+  unsigned int n0 = threadIdx.x, n1 = blockIdx.x, n2 = 12345u;
+  unsigned long long c0 = 0, g0 = 0;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    c0 = clock64();
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
+  }
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+    if (KIND == 0) {
+#pragma unroll
+      for (int i = 0; i < 12; ++i) r[i] = fma(r[i], r[i], b);
+    } else if (KIND == 1) {
+#pragma unroll
+      for (int i = 0; i < 12; ++i) r[i] = fma(r[i], q[i], s[i]);
+    } else if (KIND == 2) {
+#pragma unroll
+      for (int i = 0; i < 12; ++i) r[i] = r[i] + b;
+    } else if (KIND == 3) {
+#pragma unroll
+      for (int i = 0; i < 12; ++i) r[i] = r[i] * a;
+    } else if (KIND == 4) {
+      double t;
+      asm volatile("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(t) : "d"(r[0] + 1.0));
+#pragma unroll
+      for (int i = 0; i < 10; ++i) r[i] = fma(r[i], r[i], b);
+      r[10] = fma(r[10], r[10], t * 1e-3);  // DMUL + DFMA: 12 FP64 instructions + 1 DADD above, see host
+    } else {
+#pragma unroll
+      for (int i = 0; i < 11; ++i) r[i] = fma(r[i], r[i], b);
+      n0 = n0 * 3u + n1;
+      n1 = n1 + n2;
+      n2 = n2 ^ n0;
+    }
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    unsigned long long c1 = clock64(), g1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+    clk[0] = c0; clk[1] = c1; clk[2] = g0; clk[3] = g1;
+  }
+  double acc = (double)(n0 ^ n1 ^ n2) * 1e-300;
+#pragma unroll
+  for (int i = 0; i < 12; ++i) acc += r[i] + q[i] * s[i];
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
+cudaError_t launch_fp64_mix(int kind, int blocks, int iters, double* sink, unsigned long long* clk, cudaStream_t st) {
+  switch (kind) {
+    case 0: k_fp64_mix<0><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    case 1: k_fp64_mix<1><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    case 2: k_fp64_mix<2><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    case 3: k_fp64_mix<3><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    case 4: k_fp64_mix<4><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    default: k_fp64_mix<5><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+  }
+  return cudaGetLastError();
+}
+
 cudaError_t launch_fp64_probe(int blocks, int iters, double* sink, unsigned long long* clk,
                               cudaStream_t st) {
   k_fp64_probe<<<blocks, 256, 0, st>>>(iters, sink, clk);
