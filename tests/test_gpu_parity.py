@@ -122,6 +122,33 @@ def test_residual_and_jv_anisotropic_mesh(sws, oracle80, oracleC, ratio):
     assert np.abs(JV[0] - ref).max() <= TOL * np.abs(ref).max()
 
 
+@pytest.mark.parametrize("seed", range(12))
+def test_residual_and_jv_random_shapes(sws, oracle80, oracleC, seed):
+    """Seeded random meshes: N in [3, 160], M in [4, 320] (odd and even, columns of one and of several staged
+    segments, ragged tiles), dx != dy, y1 = 0 or not, either y-derivative scheme, smooth state + noise.
+    Residual against the long-double oracle and one analytic Jacobian action against the complex-step oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    N = int(rng.integers(3, 161))
+    M = int(rng.integers(4, 321)) if seed % 3 else int(rng.integers(4, 40))
+    while N * M > 12000:
+        M = max(4, M // 2)
+    h = float(rng.uniform(0.05, 0.6))
+    cfg = W.custom(N, M, h, float(rng.uniform(-6.0, -0.5)), y1=(0.0 if seed % 2 == 0 else float(rng.uniform(0.1, 1.0))),
+                   eps=float(rng.uniform(0.0, 1.0)), froude=float(rng.uniform(0.5, 1.2)), amp=0.05, seed=200 + seed)
+    dy_scheme = int(seed % 4 == 3)
+    p = cfg.params(dy_scheme)
+    p["dy"] = h * float(rng.uniform(0.5, 2.0))
+    u = W.state(cfg) + 1e-3 * rng.standard_normal(cfg.n)
+    v = rng.standard_normal(cfg.n)
+    E = oracle80.residual(p, u)
+    ref = oracleC.jv_exact(p, u, v)
+    with sws.Context(p, max_batch=1) as ctx:
+        F = ctx.residual(dev(u)).cpu().numpy()
+        JV = ctx.jv_exact_batch(dev(u), dev(v[None, :])).cpu().numpy()[0]
+    assert np.isfinite(F).all() and relerr(F, E) <= TOL, (N, M, p)
+    assert np.abs(JV - ref).max() <= TOL * np.abs(ref).max(), (N, M, p)
+
+
 def test_uniform_stream_is_a_zero(sws):
     """eps = 0, u = u_0 (L227): F == 0 to round-off (pin P6, on the GPU path)."""
     import dataclasses
