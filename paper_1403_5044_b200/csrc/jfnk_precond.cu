@@ -499,15 +499,10 @@ done:
   return SWS_OK;
 }
 
-int sws_precond_apply(sws_precond* pc, const double* v_dev, double* r_dev, void* cuda_stream) {
-  if (!pc || !v_dev || !r_dev) return SWS_EINVAL;
-  if (!pc->factored) return SWS_EINVAL;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  const LinMesh& m = pc->lm;
-  const int n1 = m.n1, M = m.M, hb = pc->hb;
-  const size_t sh = 2 * (size_t)n1 * sizeof(double);
+// the forward and backward block sweeps of App. C on the internal vectors t2 -> y (2 M - 1 dependent launches)
+static void launch_sweeps(sws_precond* pc, cudaStream_t st) {
+  const int n1 = pc->lm.n1, M = pc->lm.M, hb = pc->hb;
   const bool vec = (n1 % 2) == 0;  // rows, y and t blocks then start on 16-byte boundaries
-  k_stage1<<<M, 256, sh, st>>>(m, v_dev, pc->s1, pc->t2);
   for (int k = 0; k < M; ++k) {
     const int lk = k < hb ? k : hb;
     if (vec)
@@ -525,6 +520,40 @@ int sws_precond_apply(sws_precond* pc, const double* v_dev, double* r_dev, void*
     else if (uk > 0)
       k_bwd_row<false><<<n1, kGemvThreads, 0, st>>>(pc->bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
                                                     pc->y + (size_t)k * n1);
+  }
+}
+
+// Capture the sweeps once (on a private stream: the caller's may be the legacy default stream, which
+// cannot be captured); afterwards one graph launch replaces 2 M - 1 kernel launches.
+static void build_sweep_graph(sws_precond* pc) {
+  pc->sweep_graph_state = -1;
+  cudaStream_t cs = nullptr;
+  cudaGraph_t g = nullptr;
+  if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return; }
+  if (cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+    launch_sweeps(pc, cs);
+    if (cudaStreamEndCapture(cs, &g) == cudaSuccess && g &&
+        cudaGraphInstantiate(&pc->sweep_graph, g, 0) == cudaSuccess)
+      pc->sweep_graph_state = 1;
+  }
+  if (g) cudaGraphDestroy(g);
+  cudaStreamDestroy(cs);
+  cudaGetLastError();
+}
+
+int sws_precond_apply(sws_precond* pc, const double* v_dev, double* r_dev, void* cuda_stream) {
+  if (!pc || !v_dev || !r_dev) return SWS_EINVAL;
+  if (!pc->factored) return SWS_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const LinMesh& m = pc->lm;
+  const int n1 = m.n1, M = m.M;
+  const size_t sh = 2 * (size_t)n1 * sizeof(double);
+  if (pc->sweep_graph_state == 0) build_sweep_graph(pc);
+  k_stage1<<<M, 256, sh, st>>>(m, v_dev, pc->s1, pc->t2);
+  if (pc->sweep_graph_state == 1) {
+    if (cudaGraphLaunch(pc->sweep_graph, st) != cudaSuccess) return fail_cuda(cudaGetLastError(), "sws_precond_apply (graph)");
+  } else {
+    launch_sweeps(pc, st);
   }
   k_stage3<<<M, 256, sh, st>>>(m, pc->s1, pc->y, r_dev);
   cudaError_t e = cudaGetLastError();
@@ -555,6 +584,7 @@ double sws_precond_setup_ms(const sws_precond* pc) { return pc ? pc->setup_ms : 
 int sws_precond_destroy(sws_precond* pc) {
   if (!pc) return SWS_OK;
   cudaSetDevice(pc->device);
+  if (pc->sweep_graph) cudaGraphExecDestroy(pc->sweep_graph);
   double* bufs[] = {pc->G, pc->corr, pc->fwd, pc->bwd, pc->s1, pc->t2, pc->y, pc->panel};
   for (double* b : bufs)
     if (b) cudaFree(b);
