@@ -329,3 +329,22 @@ def test_wave_pattern_physics(mods):
     assert 1.6 <= e3 / e2 <= 3.2                              # (0.3 / 0.2)^2 = 2.25
     assert lam["F0.9"] / lam["h0.3"] == pytest.approx((0.9 / 0.7) ** 2, rel=0.08)
     assert max(quiet.values()) <= 0.1
+
+
+def test_solve_command_line(mods, oracle64, tmp_path):
+    """python -m paper_1403_5044_b200.solve on the 45 x 13 mesh of Fig. 2 (L247), eps passed through 0.5 -> 1: the
+    file it writes holds a root of the ORACLE's residual and the surface rebuilt by eq. (19)."""
+    import paper_1403_5044_b200.solve as cli
+    out = tmp_path / "surface.npz"
+    rc = cli.main(["--N", "45", "--M", "13", "--h", "0.4", "--x1", "-9", "--eps", "1.0", "--continuation", "0.5",
+                   "--bandwidth", "5", "--forcing", "--ftol", "1e-10", "--out", str(out)])
+    assert rc == 0
+    z = np.load(out)
+    c = W.custom(45, 13, 0.4, -9.0, eps=1.0)
+    assert z["u"].shape == (c.n,) and z["zeta"].shape == (13, 45) and z["phi"].shape == (13, 45)
+    assert np.abs(oracle64.residual(c.params(), z["u"])).max() <= 1e-9
+    half = (c.N + 1) * c.M
+    zb = z["u"][half:].reshape(c.M, c.N + 1)
+    assert np.array_equal(z["zeta"][:, 0], zb[:, 0])                    # zeta_1 is the first unknown of each line
+    assert np.allclose(np.diff(z["zeta"], axis=1), 0.5 * 0.4 * (zb[:, 2:] + zb[:, 1:-1]), atol=1e-15)
+    assert np.abs(z["zeta"]).max() > 0.02
