@@ -327,6 +327,24 @@ def solve_report(sws, device: int, names=("paper_361x121", "paper_721x241"), ban
                          "precond_applies": st["precond_applies"], "final_residual_inf": log[-1]["finf"],
                          "ms_jv": st["ms_jv"], "ms_precond": st["ms_precond"], "ms_residual": st["ms_residual"],
                          "gmres_its_per_step": [e["gmres_its"] for e in log[:-1]]}
+    # Fig. 7 of the paper (L336): F = 1.4, 721 x 241, dx = dy = 0.3, x_0 = -56; the fastest configuration only
+    cfg = W.PAPER_BY_NAME["paper_fig7_721x241"]
+    p = cfg.params()
+    with sws.Context(p, max_batch=1, device=device) as ctx, \
+            jf.Preconditioner(p, bandwidth=bandwidth, device=device) as pc, jf.Solver(ctx, pc, 60) as s:
+        u0 = torch.from_numpy(W.flat_state(cfg)).cuda(device)
+        kw = dict(ftol=1e-9, eta=1e-3, restart=60, gmres_maxit=120, jv_mode=2, forcing=1, eta_max=0.5)
+        s.newton(u0, max_newton=1, **kw)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        u, log, st = s.newton(u0, **kw)
+        torch.cuda.synchronize()
+        out["paper_fig7_721x241_F1.4"] = {
+            "fd_jv_forcing": {"solve_s": time.perf_counter() - t0, "newton_steps": st["steps"], "converged": st["converged"],
+                              "jv_products": st["jv_products"], "residual_evals": st["residual_evals"],
+                              "final_residual_inf": log[-1]["finf"],
+                              "gmres_its_per_step": [e["gmres_its"] for e in log[:-1]]},
+            "precond_setup_s": pc.setup_ms * 1e-3, "block_bandwidth": pc.bandwidth}
     out["note"] = ("flat initial guess, eps=1, F=0.7, ||E||_inf <= 1e-9, inexact Newton eta=1e-3, analytic Jv "
                    "(sws_linearize + sws_jv_apply; `fd_jv`: eq. (25) quotients, jv_mode 2, one sws_residual per "
                    "product; `fd_jv_forcing`: the same with Eisenstat-Walker forcing terms, eta_max 0.5), block-banded linear-Jacobian preconditioner; paper (other "
