@@ -163,8 +163,9 @@ __global__ void __launch_bounds__(kPairThreads, 8) k_allpairs_f32(const PairArgs
 
   const int tid = threadIdx.x;
   const int tile = blockIdx.x, chunk = blockIdx.y, state = blockIdx.z;
-  const int t = tile * kPairThreads + tid;
-  const int tc = t < a.T ? t : a.T - 1;
+  const int slot = tile * kPairThreads + tid;  // transposed target order (sws_farfield.cuh)
+  const int tc = target_of_slot(slot < a.T ? slot : a.T - 1, a.N, a.M);
+  const int t = slot < a.T ? tc : a.T;
   const int l = tc / (a.N - 1);
 
   const TgtRec tr = a.tgt[(size_t)state * a.T + tc];

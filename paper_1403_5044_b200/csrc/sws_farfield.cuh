@@ -195,6 +195,15 @@ __device__ __forceinline__ bool column_is_far(const double g, const double gmin)
   return __all_sync(0xffffffffu, g >= gmin) != 0;
 }
 
+// The all-pairs kernels hand the targets to their threads in TRANSPOSED order, slot = k M + l (k = x index
+// of the midpoint, l = y-line), so that the 32 targets of a warp share one x* (two at most): the columns that
+// are near for the warp are then the 2 r columns around one target instead of 32 + 2 r.  t = l (N-1) + k is
+// the index everything is stored by.
+__device__ __forceinline__ int target_of_slot(const int slot, const int N, const int M) {
+  const int k = slot / M, l = slot - k * M;
+  return l * (N - 1) + k;
+}
+
 // Host: the far-field geometry of a context's mesh and its current radius.
 inline EmGeom em_geometry(const sws_ctx* c) {
   const Mesh& m = c->mesh;

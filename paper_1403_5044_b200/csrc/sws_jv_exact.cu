@@ -267,8 +267,9 @@ __global__ void __launch_bounds__(kLinThreads, (BT >= 16 ? SWS_LIN_MINB16 : BT >
 
   const int tid = threadIdx.x;
   const int tile = blockIdx.x, chunk = blockIdx.y, group = blockIdx.z;
-  const int t = tile * kLinThreads + tid;
-  const int tc = t < a.T ? t : a.T - 1;
+  const int slot = tile * kLinThreads + tid;  // transposed target order (sws_farfield.cuh)
+  const int tc = target_of_slot(slot < a.T ? slot : a.T - 1, a.N, a.M);
+  const int t = slot < a.T ? tc : a.T;
 
   const TgtRec tr = a.tgt[tc];
   const LinT tg = {tr.ys, tr.zs, tr.psis};
