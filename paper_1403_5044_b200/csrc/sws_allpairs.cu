@@ -10,7 +10,7 @@
 // transposed SrcRec layout) is brought into shared memory by ONE bulk async copy
 // (cp.async.bulk -> UBLKCP, completion on an mbarrier), double buffered.  Every lane of a
 // warp reads the same record (shared-memory broadcast), so the kernel is bound by the FP64
-// pipe.  Columns at least 8 dy away from all 32 targets of a warp ("far", 93.5 % at 721x241)
+// pipe.  Columns at least 8 dy away from all 32 targets of a warp ("far", 97.8 % at 721x241)
 // take their S2 terms - which do not depend on the source data - from the Euler-Maclaurin form of
 // the column sum (sws_farfield.cuh): 29 FP64 instructions + 2 MUFU.RSQ64H per pair; the others
 // sum S2 pair by pair: 45 + 4.  Everything that depends only on (target, column) - dx, dx^2 and
