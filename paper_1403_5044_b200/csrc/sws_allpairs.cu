@@ -39,6 +39,16 @@ constexpr int kUnroll = SWS_UNROLL;
 // k_allpairs runs 64-thread CTAs, 8 per SM (16 warps per SM as with 128 x 4, but only two warps meet at
 // the per-column barrier and CTAs turn over twice as often: 59.5 instead of 61.1 ms at cfg5)
 constexpr int kThreads64 = SWS_PAIR_THREADS;
+// Targets per thread of k_allpairs: 1, or 2 on meshes with at least kNT2MinTargets targets.  With two targets
+// (kThreads64 slots apart, so usually the same x*) a thread loads every staged record once for both: 1.5
+// instead of 3 shared-memory loads and half the loop overhead per pair, i.e. fewer of the non-FP64
+// instructions that take issue time from the FP64 pipe: 55.4 instead of 56.8 ms at
+// 721x241 with 6 CTAs of 148 registers per SM.  Small meshes keep one target per thread (more CTAs).
+#ifndef SWS_NT2_MIN_TARGETS
+#define SWS_NT2_MIN_TARGETS 40000
+#endif
+constexpr int kNT2MinTargets = SWS_NT2_MIN_TARGETS;
+constexpr int kMinB2 = 6;  // resident CTAs per SM of the two-target kernel
 
 // Per-thread constants of one target and of the current source column.
 // The S2 quadratic forms are used with the square completed (C > 0):
@@ -89,29 +99,41 @@ __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, co
   }
 }
 
-// One staged segment [j0, j0 + len) of a column: trapezoid half weights on the column's first and
-// last node by peeling (Q4), unit weights inside.
-template <bool S2T>
+// One staged segment [j0, j0 + len) of a column for the NT targets of a thread: trapezoid half weights on the
+// column's first and last node by peeling (Q4), unit weights inside.  The staged record of a node is loaded
+// once for the NT targets.
+template <bool S2T, int NT>
 __device__ __forceinline__ void walk_segment(const double2* rec, const double* yy, const int j0, const int len,
-                                             const int M, const TgtC& tg, const ColC& cc, double& col1,
-                                             double& colS) {
+                                             const int M, const TgtC (&tg)[NT], const ColC (&cc)[NT],
+                                             double (&col1)[NT], double (&colS)[NT]) {
   int jlo = 0, jhi = len;
   if (j0 == 0) {  // first node of the column: weight 1/2 in y
-    double h1 = 0.0, hS = 0.0;
-    pair_term<S2T>(rec[0], rec[1], yy[0], tg, cc, h1, hS);
-    col1 = 0.5 * h1;
-    colS = 0.5 * hS;
+#pragma unroll
+    for (int n = 0; n < NT; ++n) {
+      double h1 = 0.0, hS = 0.0;
+      pair_term<S2T>(rec[0], rec[1], yy[0], tg[n], cc[n], h1, hS);
+      col1[n] = 0.5 * h1;
+      colS[n] = 0.5 * hS;
+    }
     jlo = 1;
   }
   const bool last = (j0 + len == M);
   if (last) jhi = len - 1;
 #pragma unroll kUnroll
-  for (int j = jlo; j < jhi; ++j) pair_term<S2T>(rec[2 * j], rec[2 * j + 1], yy[j], tg, cc, col1, colS);
+  for (int j = jlo; j < jhi; ++j) {
+    const double2 r0 = rec[2 * j], r1 = rec[2 * j + 1];
+    const double yj = yy[j];
+#pragma unroll
+    for (int n = 0; n < NT; ++n) pair_term<S2T>(r0, r1, yj, tg[n], cc[n], col1[n], colS[n]);
+  }
   if (last && jhi >= jlo) {  // last node of the column: weight 1/2 in y
-    double h1 = 0.0, hS = 0.0;
-    pair_term<S2T>(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], tg, cc, h1, hS);
-    col1 = fma(0.5, h1, col1);
-    colS = fma(0.5, hS, colS);
+#pragma unroll
+    for (int n = 0; n < NT; ++n) {
+      double h1 = 0.0, hS = 0.0;
+      pair_term<S2T>(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], tg[n], cc[n], h1, hS);
+      col1[n] = fma(0.5, h1, col1[n]);
+      colS[n] = fma(0.5, hS, colS[n]);
+    }
   }
 }
 
@@ -127,7 +149,7 @@ struct PairArgs {
   EmGeom em;
 };
 
-template <int MINB>
+template <int MINB, int NT>
 __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int seg_pad = a.seg_len;  // even by construction
@@ -140,16 +162,23 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
   // Threads take the targets in TRANSPOSED order, slot = k M + l: the 32 targets of a warp then share one
   // x* (two at most), so the columns that are near for a warp are the 2 r of one target, not 32 + 2 r
   // (near fraction 2.3 % instead of 6.5 % at 721x241).  t = l (N-1) + k is the index everything is stored by.
-  const int slot = tile * kThreads64 + tid;
-  const int sc = slot < a.T ? slot : a.T - 1;  // ragged tail: recompute the last target, never stored
-  const int tc = target_of_slot(sc, a.N, a.M);
-  const int t = slot < a.T ? tc : a.T;
-
-  const TgtRec tr = a.tgt[(size_t)state * a.T + tc];
-  const TgtC tg = {tr.ys, tr.zs, tr.psis};
-  const double xs = tr.xs;
-  const double kb = tr.B / (2.0 * tr.C);          // B / 2C
-  const double kg = tr.A / tr.C - kb * kb;        // (4AC - B^2) / (4 C^2)
+  // A thread owns NT targets, kThreads64 slots apart, and walks the staged records once for all of them.
+  int t[NT];
+  TgtC tg[NT];
+  double xs[NT], kb[NT], kg[NT], sfac[NT];
+#pragma unroll
+  for (int n = 0; n < NT; ++n) {
+    const int slot = (tile * NT + n) * kThreads64 + tid;
+    const int sc = slot < a.T ? slot : a.T - 1;  // ragged tail: recompute the last target, never stored
+    const int tc = target_of_slot(sc, a.N, a.M);
+    t[n] = slot < a.T ? tc : a.T;
+    const TgtRec tr = a.tgt[(size_t)state * a.T + tc];
+    tg[n] = {tr.ys, tr.zs, tr.psis};
+    xs[n] = tr.xs;
+    kb[n] = tr.B / (2.0 * tr.C);                 // B / 2C
+    kg[n] = tr.A / tr.C - kb[n] * kb[n];         // (4AC - B^2) / (4 C^2)
+    sfac[n] = -tr.zxs * rsqrt_fp64(tr.C);
+  }
 
   const int c0 = chunk * a.cols_per_chunk;
   const int c1 = min(a.N, c0 + a.cols_per_chunk);
@@ -175,7 +204,9 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
 
   if (tid == 0 && nitems > 0) issue(0);
 
-  double tot1 = 0.0, totS = 0.0;
+  double tot1[NT], totS[NT];
+#pragma unroll
+  for (int n = 0; n < NT; ++n) tot1[n] = totS[n] = 0.0;
   for (int q = 0; q < nitems; ++q) {
     const int s = q % kStages;
     // the buffer written here was last read in iteration q-1, which ended with __syncthreads()
@@ -183,32 +214,47 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
 
     const int i = c0 + q / a.nseg, j0 = (q % a.nseg) * a.seg_len;
     const int len = min(a.seg_len, a.M - j0);
-    ColC cc;
-    cc.dx = __ldg(a.x + i) - xs;
-    cc.dx2 = cc.dx * cc.dx;
-    cc.c = fma(-kb, cc.dx, tg.ys);
-    cc.g = kg * cc.dx2;
+    ColC cc[NT];
+    const double xi = __ldg(a.x + i);
+    bool far_t = true;
+#pragma unroll
+    for (int n = 0; n < NT; ++n) {
+      cc[n].dx = xi - xs[n];
+      cc[n].dx2 = cc[n].dx * cc[n].dx;
+      cc[n].c = fma(-kb[n], cc[n].dx, tg[n].ys);
+      cc[n].g = kg[n] * cc[n].dx2;
+      far_t = far_t && (cc[n].g >= a.em.gmin);
+    }
     const double ci = (i == 0 || i == a.N - 1) ? 0.5 : 1.0;  // trapezoid weight in x (Q4)
 
     mbar_wait(&s_bar[s], (uint32_t)((q / kStages) & 1));
 
     const double2* rec = reinterpret_cast<const double2*>(s_rec + (size_t)s * seg_pad);
     const double* yy = s_y + (size_t)s * seg_pad;
-    double col1 = 0.0, colS = 0.0;
-    if (column_is_far(cc.g, a.em.gmin)) {  // warp-uniform
-      walk_segment<false>(rec, yy, j0, len, a.M, tg, cc, col1, colS);
-      if (j0 == 0) colS = s2_column_em(a.em, cc.c, cc.g);  // the column's S2 terms, once
+    double col1[NT], colS[NT];
+#pragma unroll
+    for (int n = 0; n < NT; ++n) col1[n] = colS[n] = 0.0;
+    if (__all_sync(0xffffffffu, far_t)) {  // warp-uniform: far for every target of the warp
+      walk_segment<false, NT>(rec, yy, j0, len, a.M, tg, cc, col1, colS);
+      if (j0 == 0) {
+#pragma unroll
+        for (int n = 0; n < NT; ++n) colS[n] = s2_column_em(a.em, cc[n].c, cc[n].g);  // the column's S2 terms, once
+      }
     } else {
-      walk_segment<true>(rec, yy, j0, len, a.M, tg, cc, col1, colS);
+      walk_segment<true, NT>(rec, yy, j0, len, a.M, tg, cc, col1, colS);
     }
-    tot1 = fma(ci, col1, tot1);
-    totS = fma(ci, colS, totS);
+#pragma unroll
+    for (int n = 0; n < NT; ++n) {
+      tot1[n] = fma(ci, col1[n], tot1[n]);
+      totS[n] = fma(ci, colS[n], totS[n]);
+    }
     __syncthreads();
   }
 
-  if (t < a.T)
-    a.part[((size_t)state * a.chunks + chunk) * a.T + t] =
-        a.dxdy * fma(-tr.zxs * rsqrt_fp64(tr.C), totS, tot1);
+#pragma unroll
+  for (int n = 0; n < NT; ++n)
+    if (t[n] < a.T)
+      a.part[((size_t)state * a.chunks + chunk) * a.T + t[n]] = a.dxdy * fma(sfac[n], totS[n], tot1[n]);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -221,14 +267,21 @@ size_t allpairs_smem_bytes(const PairPlan& p) {
   return (size_t)kStages * p.seg_len * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
 }
 
-cudaError_t allpairs_configure(int* occ_out) {
-  cudaError_t e = cudaFuncSetAttribute(k_allpairs<kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)(kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + 64));
+// targets per thread of the FP64 kernel for this mesh (depends on the mesh only)
+int pair_nt(const sws_ctx* c) { return c->params.precision == 0 && c->mesh.T >= kNT2MinTargets ? 2 : 1; }
+
+cudaError_t allpairs_configure(const sws_ctx* c, int* occ_out) {
+  const int smem_max = (int)(kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + 64);
+  const size_t smem_occ = kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
+  cudaError_t e = cudaFuncSetAttribute(k_allpairs<kMinB, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(k_allpairs<kMinB2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
   if (e != cudaSuccess) return e;
   int occ = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-      &occ, k_allpairs<kMinB>, kThreads64,
-      kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t));
+  if (pair_nt(c) == 2)
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_allpairs<kMinB2, 2>, kThreads64, smem_occ);
+  else
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_allpairs<kMinB, 1>, kThreads64, smem_occ);
   if (e != cudaSuccess) return e;
   *occ_out = occ > 0 ? occ : 1;
   return cudaSuccess;
@@ -251,7 +304,7 @@ constexpr int kColsTarget = SWS_COLS_TARGET;
 PairPlan make_plan(const sws_ctx* c) {
   const Mesh& m = c->mesh;
   PairPlan p;
-  const int threads = c->params.precision == 1 ? kPairThreads : kThreads64;
+  const int threads = c->params.precision == 1 ? kPairThreads : kThreads64 * pair_nt(c);
   p.tiles = (m.T + threads - 1) / threads;
   p.nseg = (m.M + kSegMax - 1) / kSegMax;
   int seg = (m.M + p.nseg - 1) / p.nseg;
@@ -303,35 +356,53 @@ cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaSt
   a.dxdy = m.dx * m.dy;
   a.em = em_geometry(c);
   dim3 grid(plan.tiles, plan.chunks, states);
-  k_allpairs<kMinB><<<grid, kThreads64, allpairs_smem_bytes(plan), st>>>(a);
+  if (pair_nt(c) == 2)
+    k_allpairs<kMinB2, 2><<<grid, kThreads64, allpairs_smem_bytes(plan), st>>>(a);
+  else
+    k_allpairs<kMinB, 1><<<grid, kThreads64, allpairs_smem_bytes(plan), st>>>(a);
   return cudaGetLastError();
 }
 
 // --- far-field statistics (bench.py: executed work of a launch) ----------------------------
-// One warp = the same 32 targets as a warp of k_allpairs; counts the columns that warp treats
-// as near (direct S2 loop).  out[state * warps + w].
-__global__ void k_count_near(const TgtRec* tgt, const double* x, int N, int M, int T, double gmin, int* out) {
-  const int warps = (T + 31) / 32;
+// One warp = the same targets as a warp of k_allpairs (nt sets of 32 slots, kThreads64 slots apart); counts the
+// columns that warp treats as near (direct S2 loop).  out[state * warps + w], warps = tiles * tpc / 32.
+__global__ void k_count_near(const TgtRec* tgt, const double* x, int N, int M, int T, int nt, int tpc, int warps,
+                             double gmin, int* out) {
   const int w = blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32, state = blockIdx.y;
   if (w >= warps) return;
-  const int slot = w * 32 + (threadIdx.x & 31);
-  const TgtRec tr = tgt[(size_t)state * T + target_of_slot(slot < T ? slot : T - 1, N, M)];
-  const double kb = tr.B / (2.0 * tr.C);
-  const double kg = tr.A / tr.C - kb * kb;
+  const int wpc = tpc / 32;  // warps per CTA of the all-pairs kernel in use (tpc threads)
+  const int tile = w / wpc, tid = (w % wpc) * 32 + (threadIdx.x & 31);
+  double xs[2], kg[2];
+  for (int n = 0; n < nt; ++n) {
+    const int slot = (tile * nt + n) * tpc + tid;
+    const TgtRec tr = tgt[(size_t)state * T + target_of_slot(slot < T ? slot : T - 1, N, M)];
+    const double kb = tr.B / (2.0 * tr.C);
+    xs[n] = tr.xs;
+    kg[n] = tr.A / tr.C - kb * kb;
+  }
   int near = 0;
   for (int i = 0; i < N; ++i) {
-    const double dx = __ldg(x + i) - tr.xs;
-    const double dx2 = dx * dx;
-    if (!column_is_far(kg * dx2, gmin)) ++near;
+    const double xi = __ldg(x + i);
+    bool far_t = true;
+    for (int n = 0; n < nt; ++n) {
+      const double dx = xi - xs[n];
+      const double dx2 = dx * dx;
+      far_t = far_t && (kg[n] * dx2 >= gmin);
+    }
+    if (!__all_sync(0xffffffffu, far_t)) ++near;
   }
   if ((threadIdx.x & 31) == 0) out[(size_t)state * warps + w] = near;
 }
 
+static int pair_cta_threads(const sws_ctx* c) { return c->params.precision == 1 ? kPairThreads : kThreads64; }
+int count_near_warps(const sws_ctx* c) { return make_plan(c).tiles * (pair_cta_threads(c) / 32); }
+
 cudaError_t launch_count_near(sws_ctx* c, int states, int* out, cudaStream_t st) {
   const Mesh& m = c->mesh;
-  const int warps = (m.T + 31) / 32;
+  const int warps = count_near_warps(c);
   dim3 grid((warps + 3) / 4, states);
-  k_count_near<<<grid, 128, 0, st>>>(c->tgt, c->x, m.N, m.M, m.T, em_geometry(c).gmin, out);
+  k_count_near<<<grid, 128, 0, st>>>(c->tgt, c->x, m.N, m.M, m.T, pair_nt(c), pair_cta_threads(c), warps,
+                                     em_geometry(c).gmin, out);
   return cudaGetLastError();
 }
 

@@ -106,7 +106,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaGetDeviceProperties"); }
   c->sm_count = prop.multiProcessorCount;
 
-  e = p->precision == 1 ? sws::allpairs_f32_configure(&c->pair_occ) : sws::allpairs_configure(&c->pair_occ);
+  e = p->precision == 1 ? sws::allpairs_f32_configure(&c->pair_occ) : sws::allpairs_configure(c, &c->pair_occ);
   if (e == cudaSuccess) e = sws::fields_configure(c);
   if (e == cudaSuccess && p->max_batch > 0) e = sws::lin_configure(c);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "kernel configuration (is this an sm_100 device?)"); }
@@ -252,7 +252,7 @@ int sws_farfield_stats(sws_ctx* c, int32_t states, double* near_fraction, void* 
   if (states < 1 || states > c->max_states || states > c->last_states) return SWS_EBATCH;
   CK(cudaSetDevice(c->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const int warps = (c->mesh.T + 31) / 32;
+  const int warps = sws::count_near_warps(c);
   const size_t cnt = (size_t)states * warps;
   int* d = nullptr;
   CK(cudaMalloc((void**)&d, cnt * sizeof(int)));

@@ -169,7 +169,9 @@ cudaError_t launch_assemble_lin(sws_ctx* c, int b, int BT, int mode, const PairP
 PairPlan make_plan(const sws_ctx* c);
 int max_chunks(const sws_ctx* c);
 size_t allpairs_smem_bytes(const PairPlan& p);
-cudaError_t allpairs_configure(int* occ_out);
+cudaError_t allpairs_configure(const sws_ctx* c, int* occ_out);
+int pair_nt(const sws_ctx* c);
+int count_near_warps(const sws_ctx* c);
 cudaError_t allpairs_f32_configure(int* occ_out);
 size_t allpairs_f32_smem_bytes(int seg_len);
 cudaError_t fields_configure(const sws_ctx* c);
