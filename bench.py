@@ -45,8 +45,8 @@ FP64_INSTR_NEAR, FLOPS_NEAR = 45, 68
 FP64_INSTR_FAR, FLOPS_FAR = 29, 44
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
 # dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
-# ncu --set full capture summarised in profiles/r1d_allpairs_ncu.md
-NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 56.89e6}
+# ncu --set full capture summarised in profiles/r1e_allpairs_ncu.md
+NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 56.62e6}
 
 
 def dist_env():
@@ -505,7 +505,7 @@ def run_ours(args) -> None:
     roofline = {
         "bound": "alu", "kernel": "k_allpairs", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
         "frac": achieved_tf / peak_tf, "traffic": NCU_DRAM_BYTES_PER_STATE_LAUNCH.get(cfg.name),
-        "traffic_note": "DRAM bytes per state per all-pairs launch, ncu capture profiles/r1d_allpairs_ncu.md; "
+        "traffic_note": "DRAM bytes per state per all-pairs launch, ncu capture profiles/r1e_allpairs_ncu.md; "
                         "algorithmic = S*32 + T*64 bytes read once + one 8 B partial sum per target per column group "
                         "written (part of which stays in L2 until k_assemble reads it)",
         "algorithmic_bytes_per_state": cfg.sources * 32 + cfg.targets * 64 + ctx.plan_info(1)["chunks"] * cfg.targets * 8,
