@@ -5,7 +5,8 @@
 //   K1 (L107, reading Q1/Q2), K2 (L109), S2 = S2_direct + S2_image (eqs. (21),(22) L169-172),
 //   w(i,j) = dx dy c_i c_j, c = 1/2 on the first/last index (L189, reading Q4).
 //
-// Mapping (B200): one thread = one target, 64 targets per CTA, 8 CTAs per SM; a CTA walks a group
+// Mapping (B200): one thread = one target (two on large meshes, see kNT2MinTargets), 64 threads per CTA,
+// 8 (6) CTAs per SM, targets handed out in transposed order (sws_farfield.cuh); a CTA walks a group
 // of ~12 source COLUMNS (fixed x_i, all y_j).  Each column (M records of 32 B, contiguous in the
 // transposed SrcRec layout) is brought into shared memory by ONE bulk async copy
 // (cp.async.bulk -> UBLKCP, completion on an mbarrier), double buffered.  Every lane of a
