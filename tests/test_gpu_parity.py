@@ -149,6 +149,30 @@ def test_residual_and_jv_random_shapes(sws, oracle80, oracleC, seed):
     assert np.abs(JV - ref).max() <= TOL * np.abs(ref).max(), (N, M, p)
 
 
+@pytest.mark.parametrize("dy_scheme", [0, 1])
+def test_two_targets_per_thread_multisegment_ragged(sws, oracle80, dy_scheme):
+    """80 x 520: 41080 targets (>= 40000: two targets per thread), columns of three staged segments, a ragged
+    last tile (41080 = 320 * 128 + 120) and y1 != 0; seeded rows against the oracle, far field on and off."""
+    cfg = W.custom(80, 520, 0.05, -1.5, y1=0.35, eps=0.4, amp=0.05, seed=33)
+    p = cfg.params(dy_scheme)
+    u = W.state(cfg) + 1e-3 * np.random.default_rng(12).standard_normal(cfg.n)
+    T = cfg.targets
+    assert T >= 40000 and T % 128 != 0
+    rng = np.random.default_rng(5)
+    pick = np.unique(np.concatenate([rng.integers(0, T, 600), [0, T - 1, T - 121, T - 120, 78, 79 * 519]])).astype(np.int32)
+    E = oracle80.residual(p, u, rows=pick)
+    mask = ~np.isnan(E)
+    with sws.Context(p) as ctx:
+        assert ctx.plan_info(1)["tiles"] == -(-T // 128) and ctx.plan_info(1)["nseg"] == 3
+        F = ctx.residual(dev(u)).cpu().numpy()
+        ctx.set_farfield(0.0)
+        F0 = ctx.residual(dev(u)).cpu().numpy()
+    scale = np.abs(F).max()
+    assert np.isfinite(F).all()
+    assert np.abs(F[mask] - E[mask]).max() / scale <= TOL
+    assert np.abs(F - F0).max() / scale <= 2e-13
+
+
 def test_uniform_stream_is_a_zero(sws):
     """eps = 0, u = u_0 (L227): F == 0 to round-off (pin P6, on the GPU path)."""
     import dataclasses
