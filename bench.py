@@ -602,7 +602,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", default="cfg5_721x241", choices=sorted(W.BY_NAME))
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline leg")
+    ap.add_argument("--cpu-seconds", type=float, default=30.0, help="CPU work of the cpu_baseline leg")
     ap.add_argument("--ref-rows", type=int, default=2048, help="rows per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fp32", action="store_true", help="skip the reported FP32-variant section")
