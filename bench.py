@@ -38,11 +38,11 @@ import workloads as W  # noqa: E402
 METRIC = "fp64_residual_evals_per_s"
 UNIT = "evals/s"
 # Work of the all-pairs kernel per pair interaction, from its SASS inner loops:
-#   near columns (S2 summed pair by pair): 45 FP64-pipe instructions = 23 DFMA (2 flops) + 22 DMUL/DADD;
-#   far columns (S2 column sum from its Euler-Maclaurin form): 29 = 15 DFMA + 14 DMUL/DADD.
+#   near columns (S2 summed pair by pair): 44 FP64-pipe instructions = 23 DFMA (2 flops) + 21 DMUL/DADD;
+#   far columns (S2 column sum from its Euler-Maclaurin form): 28 = 15 DFMA + 13 DMUL/DADD.
 # The ~200 FP64 instructions of the expansion per (target, far column) are NOT counted as achieved work.
-FP64_INSTR_NEAR, FLOPS_NEAR = 45, 68
-FP64_INSTR_FAR, FLOPS_FAR = 29, 44
+FP64_INSTR_NEAR, FLOPS_NEAR = 44, 67
+FP64_INSTR_FAR, FLOPS_FAR = 28, 43
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
 # dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
 # ncu --set full capture summarised in profiles/r1e_allpairs_ncu.md
@@ -515,7 +515,7 @@ def run_ours(args) -> None:
         "near_column_fraction": near,
         "work_note": f"executed pair-loop work: {FLOPS_NEAR} flops/pair on the near columns (direct S2), "
                      f"{FLOPS_FAR} on the far ones (S2 column sum in closed form + Euler-Maclaurin, sws_set_farfield); "
-                     "with the plain 68 flops/pair definition the same time reads "
+                     "with the plain 67 flops/pair definition the same time reads "
                      f"{FLOPS_NEAR * pairs_timed / ap_s / 1e12:.1f} TFLOP/s-equivalent",
         "launches_timed": ap_launches, "avg_launch_ms": ap_ms / max(ap_launches, 1),
         "share_of_step": ap_ms / ms_total if world == 1 else None,

@@ -61,7 +61,8 @@ typedef struct sws_ctx sws_ctx; /* opaque, owned by the library */
 
 typedef struct {
   int32_t N, M;        /* mesh nodes in x and y (N >= 3, M >= 4)                       L145 */
-  double x1, y1;       /* first node; x1 = upstream truncation, configs use y1 = 0     L162 */
+  double x1, y1;       /* first node; x1 = upstream truncation; y1 >= 0 (half plane of eq. (12),
+                          L101), configs use y1 = 0                                    L162 */
   double dx, dy;       /* spacings Delta x, Delta y (> 0)                              L145 */
   double froude, eps;  /* Froude number F, eq. (9); source strength eq. (6)         */
   double n_rad;        /* radiation exponent n, paper value 0.05                       L189 */

@@ -13,8 +13,8 @@
 // warp reads the same record (shared-memory broadcast), so the kernel is bound by the FP64
 // pipe.  Columns at least 8 dy away from all 32 targets of a warp ("far", 97.8 % at 721x241)
 // take their S2 terms - which do not depend on the source data - from the Euler-Maclaurin form of
-// the column sum (sws_farfield.cuh): 29 FP64 instructions + 2 MUFU.RSQ64H per pair; the others
-// sum S2 pair by pair: 45 + 4.  Everything that depends only on (target, column) - dx, dx^2 and
+// the column sum (sws_farfield.cuh): 28 FP64 instructions + 2 MUFU.RSQ64H per pair; the others
+// sum S2 pair by pair: 44 + 4.  Everything that depends only on (target, column) - dx, dx^2 and
 // the completed-square constants of S2 - is hoisted out of the j loop; the half weights are
 // applied by peeling the first/last node and scaling edge columns, so the inner loop carries no
 // weight multiply.  Partial sums per (state, chunk, target) are written to global memory and
@@ -60,6 +60,7 @@ constexpr int kMinB2 = 6;  // resident CTAs per SM of the two-target kernel
 // (target, column), and the common factor 1/sqrt(C) is applied once per target at the end.
 struct TgtC {
   double ys, zs, psis;
+  double ys2, ys4;  // 2 y*, 4 y*: the image terms follow from the direct ones (below)
 };
 struct ColC {
   double dx, dx2, c, g;  // x_i - x*, its square, and the S2 constants above
@@ -67,23 +68,25 @@ struct ColC {
 
 // One source node against one target: adds (phi-phi*-x+x*) K1 + zeta_x K2 to a1 and, if S2T,
 // sqrt(C) S2 to aS (unit weight).  S2T = false is the far-field form: the S2 terms of the
-// whole column come from s2_column_em() below, 29 FP64 instructions + 2 MUFU.RSQ64H remain.
+// whole column come from s2_column_em() below, 28 FP64 instructions + 2 MUFU.RSQ64H remain.
 template <bool S2T>
 __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, const double yj,
                                           const TgtC& t, const ColC& c, double& a1, double& aS) {
   const double z = zp.x, psi = zp.y, zx = sl.x, zy = sl.y;
+  // Image terms from the direct ones (all y >= 0, sws_setup): (y + y*)^2 = (y - y*)^2 + 4 y y* and
+  // y + y* = (y - y*) + 2 y*, so y + y* itself is never formed: one DADD less per pair.  R+^2 >= R-^2, so
+  // the rounding of R-^2 it inherits is below its own.
   const double dm = yj - t.ys;  // y - y*
-  const double dp = yj + t.ys;  // y + y*  (image, L107-109)
   const double dz = z - t.zs;
   const double q = fma(dz, dz, c.dx2);
   const double Rm2 = fma(dm, dm, q);
-  const double Rp2 = fma(dp, dp, q);
+  const double Rp2 = fma(t.ys4, yj, Rm2);
   const double rm = rsqrt_fp64(Rm2);
   const double rp = rsqrt_fp64(Rp2);
   // K1 numerators: zeta - zeta* - (x-x*) zeta_x - (y -+ y*) zeta_y, slopes at the source (Q2)
   const double n0 = fma(-c.dx, zx, dz);
   const double nm = fma(-dm, zy, n0);
-  const double np = fma(-dp, zy, n0);
+  const double np = fma(-t.ys2, zy, nm);
   const double rm3 = (rm * rm) * rm;
   const double rp3 = (rp * rp) * rp;
   const double k1 = fma(np, rp3, nm * rm3);
@@ -174,7 +177,7 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
     const int tc = target_of_slot(sc, a.N, a.M);
     t[n] = slot < a.T ? tc : a.T;
     const TgtRec tr = a.tgt[(size_t)state * a.T + tc];
-    tg[n] = {tr.ys, tr.zs, tr.psis};
+    tg[n] = {tr.ys, tr.zs, tr.psis, 2.0 * tr.ys, 4.0 * tr.ys};
     xs[n] = tr.xs;
     kb[n] = tr.B / (2.0 * tr.C);                 // B / 2C
     kg[n] = tr.A / tr.C - kb[n] * kb[n];         // (4AC - B^2) / (4 C^2)

@@ -75,6 +75,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   if (!p || !out) return SWS_EINVAL;
   *out = nullptr;
   if (p->N < 3 || p->M < 4 || !(p->dx > 0) || !(p->dy > 0) || !(p->froude > 0)) return SWS_EINVAL;
+  if (!(p->y1 >= 0.0)) return SWS_EINVAL;  // eq. (12) integrates over the half plane y >= 0 and adds the images
   if (p->dy_scheme != 0 && p->dy_scheme != 1) return SWS_EINVAL;
   if (p->precision != 0 && p->precision != 1) return SWS_EINVAL;
   if (p->max_batch < 0 || p->max_batch > 1024) return SWS_EINVAL;
