@@ -46,7 +46,7 @@ FP64_INSTR_FAR, FLOPS_FAR = 28, 43
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
 # dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
 # ncu --set full capture summarised in profiles/r1e_allpairs_ncu.md
-NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 56.62e6}
+NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 56.46e6}
 
 
 def dist_env():
