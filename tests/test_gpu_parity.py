@@ -450,6 +450,8 @@ def test_error_codes(sws):
         sws.Context(dict(p, N=2))
     with pytest.raises(sws.SwsError, match="invalid"):
         sws.Context(dict(p, dx=0.0))
+    with pytest.raises(sws.SwsError, match="invalid"):
+        sws.Context(dict(p, y1=-0.1))      # eq. (12) is posed on the half plane y >= 0
     with sws.Context(p, max_batch=2) as ctx:
         u, V = dev(W.state(cfg)), dev(W.directions(cfg, 3))
         with pytest.raises(sws.SwsError, match="batch"):
