@@ -106,18 +106,13 @@ __global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ 
 //             2 m_{M-1} + m_M = (d_{M-2} + 5 d_{M-1})/2
 // solved by the Thomas recurrences with the data-independent factors cp[], inv[] made in
 // sws_setup.  The output plane is used as the forward-sweep scratch.
-__global__ void __launch_bounds__(128) k_dy(Mesh m, int first, const double* __restrict__ cp,
-                                            const double* __restrict__ inv, const double* zeta,
-                                            const double* phi, double* zy, double* py) {
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= m.N) return;
-  const int N = m.N, M = m.M, state = blockIdx.z + first;
-  const size_t base = (size_t)state * m.S + k;
-  const double* f = (blockIdx.y == 0 ? zeta : phi) + base;
-  double* out = (blockIdx.y == 0 ? zy : py) + base;
+// The march along one x-line: F_(l) reads the field at line l, O_(l) names the output at line l (also the
+// forward-sweep scratch).  Same operations in the same order whichever memory the accessors name.
+template <class FA, class OA>
+__device__ __forceinline__ void dy_line(const Mesh& m, const double* __restrict__ cp,
+                                        const double* __restrict__ inv, FA F_, OA O_) {
+  const int M = m.M;
   const double h = m.dy;
-#define F_(l) f[(size_t)(l) * N]
-#define O_(l) out[(size_t)(l) * N]
   if (m.dy_scheme == 0) {
     double f0 = F_(0), f1 = F_(1), f2 = F_(2);
     double dprev = SUB(f1, f0) / h, dcur = SUB(f2, f1) / h;  // d_0, d_1
@@ -151,8 +146,41 @@ __global__ void __launch_bounds__(128) k_dy(Mesh m, int first, const double* __r
     for (int l = 1; l < M - 1; ++l) O_(l) = SUB(F_(l + 1), F_(l - 1)) / h2;
     O_(M - 1) = ADD(SUB(MUL(3.0, F_(M - 1)), MUL(4.0, F_(M - 2))), F_(M - 3)) / h2;
   }
-#undef F_
-#undef O_
+}
+
+__global__ void __launch_bounds__(128) k_dy(Mesh m, int first, const double* __restrict__ cp,
+                                            const double* __restrict__ inv, const double* zeta,
+                                            const double* phi, double* zy, double* py) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= m.N) return;
+  const int N = m.N, state = blockIdx.z + first;
+  const size_t base = (size_t)state * m.S + k;
+  const double* f = (blockIdx.y == 0 ? zeta : phi) + base;
+  double* out = (blockIdx.y == 0 ? zy : py) + base;
+  dy_line(m, cp, inv, [&](int l) { return f[(size_t)l * N]; }, [&](int l) -> double& { return out[(size_t)l * N]; });
+}
+
+// The same with the 32 x-lines of a warp staged in shared memory ([l][lane], coalesced both ways): every step
+// of the two dependent sweeps then costs a shared-memory access instead of a global one (the march is pure
+// latency: 2 M dependent steps; 220 -> ~25 us at M = 241, which is 1/3 of a residual on the 91x31 mesh).
+__global__ void __launch_bounds__(32) k_dy_staged(Mesh m, int first, const double* __restrict__ cp,
+                                                  const double* __restrict__ inv, const double* zeta,
+                                                  const double* phi, double* zy, double* py) {
+  extern __shared__ double s_dy[];
+  const int N = m.N, M = m.M, state = blockIdx.z + first, lane = threadIdx.x;
+  const int k = blockIdx.x * 32 + lane;
+  const bool live = k < N;
+  const size_t base = (size_t)state * m.S + (live ? k : N - 1);
+  const double* f = (blockIdx.y == 0 ? zeta : phi) + base;
+  double* out = (blockIdx.y == 0 ? zy : py) + base;
+  double* sf = s_dy;
+  double* so = s_dy + (size_t)M * 32;
+  for (int l = 0; l < M; ++l) sf[l * 32 + lane] = f[(size_t)l * N];
+  __syncwarp();
+  dy_line(m, cp, inv, [&](int l) { return sf[l * 32 + lane]; }, [&](int l) -> double& { return so[l * 32 + lane]; });
+  __syncwarp();
+  if (live)
+    for (int l = 0; l < M; ++l) out[(size_t)l * N] = so[l * 32 + lane];
 }
 
 // ---------------------------------------------------------------------------------------
@@ -360,9 +388,17 @@ __global__ void __launch_bounds__(256) k_quotient(const double* __restrict__ F0,
 
 size_t reconstruct_smem_bytes(int N) { return (size_t)4 * N * sizeof(double); }
 
+constexpr size_t kDyStagedMaxSmem = 200 * 1024;
+static size_t dy_staged_smem_bytes(int M) { return (size_t)2 * M * 32 * sizeof(double); }
+
 cudaError_t fields_configure(const sws_ctx* c) {
-  return cudaFuncSetAttribute(k_reconstruct, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)reconstruct_smem_bytes(c->mesh.N));
+  cudaError_t e = cudaFuncSetAttribute(k_reconstruct, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)reconstruct_smem_bytes(c->mesh.N));
+  if (e != cudaSuccess) return e;
+  const size_t smem = dy_staged_smem_bytes(c->mesh.M);
+  if (smem <= kDyStagedMaxSmem)
+    e = cudaFuncSetAttribute(k_dy_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  return e;
 }
 
 cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states, int lin,
@@ -376,8 +412,14 @@ cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int
 
 cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st, int first) {
   const Mesh& m = c->mesh;
-  dim3 grid((m.N + 127) / 128, 2, states - first);
-  k_dy<<<grid, 128, 0, st>>>(m, first, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zy, c->py);
+  const size_t smem = dy_staged_smem_bytes(m.M);
+  if (smem <= kDyStagedMaxSmem) {
+    dim3 grid((m.N + 31) / 32, 2, states - first);
+    k_dy_staged<<<grid, 32, smem, st>>>(m, first, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zy, c->py);
+  } else {  // very long columns: march in global memory
+    dim3 grid((m.N + 127) / 128, 2, states - first);
+    k_dy<<<grid, 128, 0, st>>>(m, first, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zy, c->py);
+  }
   return cudaGetLastError();
 }
 
