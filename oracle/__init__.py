@@ -20,17 +20,23 @@ from pathlib import Path
 import numpy as np
 
 _HERE = Path(__file__).resolve().parent
-_SRC = _HERE / "sws_oracle.c"
-_LIBS = {"f64": _HERE / "libsws_oracle_f64.so", "f80": _HERE / "libsws_oracle_f80.so",
-         "c80": _HERE / "libsws_oracle_c80.so"}
+# SWS_ORACLE_SRC / SWS_ORACLE_LIBDIR: tests/test_oracle_mutations.py points these at a deliberately
+# broken copy of the source (and a scratch directory for its builds) to prove the pins catch it.
+_SRC = Path(os.environ.get("SWS_ORACLE_SRC", _HERE / "sws_oracle.c"))
+_LIBDIR = Path(os.environ.get("SWS_ORACLE_LIBDIR", _HERE))
+_LIBS = {"f64": _LIBDIR / "libsws_oracle_f64.so", "f80": _LIBDIR / "libsws_oracle_f80.so",
+         "c80": _LIBDIR / "libsws_oracle_c80.so"}
 # c80: the same source with REAL = long double _Complex (complex-step derivative, -DCSTEP);
 # -fcx-limited-range = textbook complex multiply/divide (no NaN-recovery library calls)
 _DEFS = {"f64": ["-DREAL=double"], "f80": ["-DREAL=long double"], "c80": ["-DCSTEP", "-fcx-limited-range"]}
 
 
-def build(force: bool = False) -> None:
-    """Compile the oracle with gcc: -O2 -fopenmp, no fast-math, no FMA contraction."""
+def build(force: bool = False, only: str | None = None) -> None:
+    """Compile the oracle with gcc: -O2 -fopenmp, no fast-math, no FMA contraction.
+    only: build just that precision's library (what Oracle(precision) needs)."""
     for suf, lib in _LIBS.items():
+        if only is not None and suf != only:
+            continue
         if not force and lib.exists() and lib.stat().st_mtime >= _SRC.stat().st_mtime:
             continue
         cmd = ["gcc", "-std=c11", "-O2", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared",
@@ -56,7 +62,7 @@ class Oracle:
     def __init__(self, precision: str = "f64"):
         if precision not in _LIBS:
             raise ValueError(precision)
-        build()
+        build(only=precision)
         self.suf = precision
         self.lib = C.CDLL(str(_LIBS[precision]))
         s = precision

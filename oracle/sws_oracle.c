@@ -39,8 +39,17 @@
  * PW (tests/test_oracle_jfnk.py): the ROOT of this residual, found by the oracle's
  * own Newton driver, is the steady wave pattern of linear theory (centre-line
  * wavelength 2 pi F^2 under refinement, F^2 scaling, nothing upstream).
- * Beyond those the residual's absolute values at an arbitrary u are "parity
- * unpinned" (the paper prints no numeric value of E for any worked example).
+ * PG (tests/test_oracle_green.py): for a manufactured harmonic psi on a curved
+ * surface, the K1 sum (PG1) and the whole row E2 the residual returns (PG2)
+ * converge at O(h^2) to the two sides of Green's third identity, evaluated by
+ * adaptive quadrature of continuous integrands that contain none of K1, K2, S2,
+ * I.  P1b: the returned row against eq. (12) assembled from full-plane direct
+ * sums with the printed signs.  tests/test_oracle_mutations.py compiles ~30
+ * single-line mutations of THIS file and requires the named pin to fail on each.
+ * The paper prints no numeric value of E for any worked example, so what pins
+ * the residual at an arbitrary u is PG2 (to the O(h^2) discretisation error)
+ * and P1b/P7 (to round-off); the nonlinear cross terms of the Bernoulli row E1
+ * and A, B, C of L177 are pinned by restating the printed formula only.
  */
 #include <math.h>
 #include <stdlib.h>

@@ -254,7 +254,7 @@ def test_mirror_symmetry_of_kernels(oracle64):
 # the evenly extended mesh y in [-y_M, y_M]  (pins the garbled K1 of L107, Q1,
 # the sign of the image S2 term L172, the source-point slopes Q2, weights Q4)
 # ----------------------------------------------------------------------------
-def _full_plane_sums(c, u, k, l, oracle):
+def _full_plane_sums(c, u, k, l, oracle, want_star=False):
     p = c.params()
     zeta, phi, zeta_y, _ = oracle.fields(p, u)
     zeta_x = u[(c.N + 1) * c.M:].reshape(c.M, c.N + 1)[:, 1:]
@@ -276,15 +276,14 @@ def _full_plane_sums(c, u, k, l, oracle):
     s1 = (Wt * (P - ps - X + xs) * K1).sum()
     s2 = (Wt * ZX / R).sum()
     s3 = (Wt / np.sqrt(A * dx ** 2 + B * dx * dy + C * dy ** 2)).sum()
+    if want_star:
+        return s1, s2, s3, dict(xs=xs, ys=ys, zs=zs, ps=ps, zxs=zxs, A=A, B=B, C=C)
     return s1, s2, s3
 
 
 @pytest.mark.parametrize("kl", [(0, 0), (5, 2), (11, 4), (7, 0), (3, 6)])
 def test_P1_full_plane_identity(oracle64, kl):
-    c = small(N=13, M=7, h=0.5, x1=-2.0, amp=0.3, seed=21)
-    c = dataclasses.replace(c, eps=0.3)
-    u = W.state(c)
-    u[: (c.N + 1) * c.M] += 0.2 * np.random.default_rng(1).standard_normal((c.N + 1) * c.M)  # phi - x = O(1)
+    c, u = _p1_fixture()
     k, l = kl
     t = oracle64.e2_terms(c.params(), u, k, l)
     s1, s2, s3 = _full_plane_sums(c, u, k, l, oracle64)
@@ -293,6 +292,51 @@ def test_P1_full_plane_identity(oracle64, kl):
     assert t[4] == pytest.approx(s3, rel=1e-12)
     # the pin discriminates: the terms are far from zero at this state
     assert abs(s1) > 1e-5 and abs(s2) > 1e-3
+
+
+def _p1_fixture():
+    c = small(N=13, M=7, h=0.5, x1=-2.0, amp=0.3, seed=21)
+    c = dataclasses.replace(c, eps=0.3)
+    u = W.state(c)
+    u[: (c.N + 1) * c.M] += 0.2 * np.random.default_rng(1).standard_normal((c.N + 1) * c.M)  # phi - x = O(1)
+    return c, u
+
+
+@pytest.mark.parametrize("prec", ["f64", "f80"])
+def test_P1b_residual_row_is_eq12_with_its_printed_signs(oracle64, oracle80, prec):
+    """The row the residual RETURNS (E2_row, not the parallel e2_terms), at a curved state with phi - x = O(1),
+    against eq. (12) L101 assembled here from full-plane DIRECT-kernel sums (no images), the quadrature-pinned
+    box integral (P5) and the printed signs:
+        2 pi (phi* - x*) = -eps/rho* + int (phi - phi* - x + x*) K1 + int zeta_x K2,
+    int zeta_x K2 -> sum w (zeta_x K2 - zeta_x* S2) + zeta_x* I (L181).  Every row of the mesh."""
+    orc = oracle64 if prec == "f64" else oracle80
+    c, u = _p1_fixture()
+    x, y = W.mesh(c)
+    E = orc.residual(c.params(), u)
+    worst, k1_size = 0.0, 0.0
+    for l in range(c.M):
+        for k in range(c.N - 1):
+            s1, s2, s3, st = _full_plane_sums(c, u, k, l, orc, want_star=True)
+            I = orc.box_integral(st["A"], st["B"], st["C"], x[0] - st["xs"], x[-1] - st["xs"],
+                                 -(y[-1] + st["ys"]), y[-1] - st["ys"])            # y_1 = 0: merged box
+            rho = np.sqrt(st["xs"] ** 2 + st["ys"] ** 2 + (st["zs"] + 1) ** 2)
+            ref = 2 * PI * (st["ps"] - st["xs"]) + c.eps / rho - s1 - (s2 - st["zxs"] * s3) - st["zxs"] * I
+            worst = max(worst, abs(E[row_E2(c, k, l)] - ref))
+            k1_size = max(k1_size, abs(s1))
+    assert worst <= 1e-11 * np.abs(E).max(), worst
+    assert k1_size > 1e-2            # the K1 sum is two orders above the tolerance: its sign and density are seen
+
+
+def test_e2_terms_tie_to_residual_row(oracle64, oracle80):
+    """e2_terms (the pieces the pins P1, PG1 look at) and the residual's own row are the same quantity:
+    E2 = out0 + out1 - out2 - (out3 - zeta_x* out4) - zeta_x* out5."""
+    c, u = _p1_fixture()
+    for orc, tol in ((oracle64, 2e-12), (oracle80, 2e-14)):
+        E = orc.residual(c.params(), u)
+        for (k, l) in [(0, 0), (5, 2), (11, 4), (7, 0), (3, 6), (11, 6)]:
+            t = orc.e2_terms(c.params(), u, k, l)
+            ref = t[0] + t[1] - t[2] - (t[3] - t[6] * t[4]) - t[6] * t[5]
+            assert abs(E[row_E2(c, k, l)] - ref) <= tol * max(1.0, abs(t[3])), (k, l)
 
 
 # ----------------------------------------------------------------------------
