@@ -40,13 +40,15 @@ UNIT = "evals/s"
 # Work of the all-pairs kernel per pair interaction, from its SASS inner loops:
 #   near columns (S2 summed pair by pair): 44 FP64-pipe instructions = 23 DFMA (2 flops) + 21 DMUL/DADD;
 #   far columns (S2 column sum from its Euler-Maclaurin form): 28 = 15 DFMA + 13 DMUL/DADD.
-# The ~200 FP64 instructions of the expansion per (target, far column) are NOT counted as achieved work.
+# The 216 FP64 instructions (SASS count, sws_farfield.cuh) of the expansion per (target, far column) - 0.9 per
+# pair at M = 241 - are NOT counted as achieved work.
 FP64_INSTR_NEAR, FLOPS_NEAR = 44, 67
 FP64_INSTR_FAR, FLOPS_FAR = 28, 43
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
 # dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
-# ncu --set full capture summarised in profiles/r1e_allpairs_ncu.md
+# ncu --set full capture summarised in NCU_PROFILE (a static figure: this run does not measure it)
 NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 56.46e6}
+NCU_PROFILE = "profiles/r1e_allpairs_ncu.md"
 
 
 def dist_env():
@@ -389,6 +391,67 @@ def table1_report(sws, device: int, steps: int = 5) -> dict:
     return out
 
 
+def configs_report(sws, device: int, peak_tf: float, names, steps: int = 20) -> dict:
+    """BASELINE.json configs 1-4 in FP64 on their own step (single F(u) + the config's b-batch; cfg1: the single
+    evaluation only): evaluations/s, pair interactions/s, share and executed-flop fraction of the all-pairs kernel.
+    CUDA events per step on the launching stream, the 256 MB L2 flush between steps (not timed); `warm` = the same
+    steps back to back without the flush (the working set of these meshes is far below the 126 MB L2)."""
+    import torch
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{device}")
+    out = {}
+    for name in names:
+        cfg = W.BY_NAME[name]
+        b = cfg.b
+        u = torch.from_numpy(W.state(cfg)).cuda(device)
+        V = torch.from_numpy(W.directions(cfg, b)).cuda(device) if b else None
+        evals = 1 + ((b + 1) if b else 0)
+        with sws.Context(cfg.params(), max_batch=b, device=device) as ctx:
+            F = ctx.residual(u)
+
+            def step():
+                ctx.residual(u, out=F)
+                n1 = ctx.last_launch_count
+                if b:
+                    ctx.jv_batch(u, V)
+                    return n1 + ctx.last_launch_count
+                return n1
+            for _ in range(3):
+                launches = step()
+            torch.cuda.synchronize()
+            ctx.set_profiling(True)
+            ctx.profile_read(reset=True)
+            ms = 0.0
+            for _ in range(steps):
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); step(); e1.record()
+                torch.cuda.synchronize()
+                ms += e0.elapsed_time(e1)
+            ap_ms, ap_n = ctx.profile_read(reset=True)
+            ctx.set_profiling(False)
+            ms /= steps
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(steps):
+                step()
+            e1.record()
+            torch.cuda.synchronize()
+            ms_warm = e0.elapsed_time(e1) / steps
+            near = ctx.farfield_stats((b + 1) if b else 1)
+            flops_pair = near * FLOPS_NEAR + (1.0 - near) * FLOPS_FAR
+            ach = flops_pair * evals * cfg.pairs * steps / (ap_ms * 1e-3) / 1e12
+            out[name] = {"N": cfg.N, "M": cfg.M, "jv_batch": b, "evals_per_step": evals, "ms_per_step": ms,
+                         "evals_per_s": evals / (ms * 1e-3), "pairs_per_s": evals * cfg.pairs / (ms * 1e-3),
+                         "ms_per_step_warm": ms_warm, "evals_per_s_warm": evals / (ms_warm * 1e-3),
+                         "launches_per_step": launches, "allpairs_share_of_step": ap_ms / steps / ms,
+                         "near_column_fraction": near, "flops_per_pair": flops_pair,
+                         "allpairs_achieved_tflops": ach, "allpairs_frac_of_fp64_peak": ach / peak_tf,
+                         "plan": ctx.plan_info(1)}
+    out["note"] = ("FP64, step = sws_residual(u) + sws_jv_batch(u, V[b]) as BASELINE.json states each config (cfg1: one "
+                   "F(u)); parity of every one of these steps: tests/test_gpu_parity.py")
+    return out
+
+
 def run_ours(args) -> None:
     import torch
 
@@ -414,10 +477,12 @@ def run_ours(args) -> None:
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=u.device)  # > 126 MB L2
     launches_per_step = 0
 
-    def step():
+    def step(mid=None):
         nonlocal launches_per_step
         ctx.residual(u, out=F)
         n1 = ctx.last_launch_count
+        if mid is not None:
+            mid.record()
         JV = ctx.jv_batch(u, V)
         launches_per_step = n1 + ctx.last_launch_count
         return JV
@@ -433,18 +498,19 @@ def run_ours(args) -> None:
         time.sleep(0.25)
     ctx.set_profiling(True)
     ctx.profile_read(reset=True)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-          for _ in range(args.steps)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True),
+           torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     replicas.barrier()
     torch.cuda.synchronize()
-    for e0, e1 in ev:
+    for e0, em, e1 in ev:
         flush.zero_()                      # L2 flush between timed iterations (not timed)
         e0.record()
-        step()
+        step(em)
         e1.record()
     torch.cuda.synchronize()
     replicas.barrier()
-    ms_total = sum(e0.elapsed_time(e1) for e0, e1 in ev)
+    ms_total = sum(e0.elapsed_time(e1) for e0, _, e1 in ev)
+    ms_batch = sum(em.elapsed_time(e1) for _, em, e1 in ev)   # the sws_jv_batch part of the steps
     ap_ms, ap_launches = ctx.profile_read(reset=True)
     ctx.set_profiling(False)
     near = ctx.farfield_stats(b + 1)       # of the b + 1 states of the last sws_jv_batch
@@ -491,10 +557,13 @@ def run_ours(args) -> None:
 
     # ---- roofline of the dominant kernel (all-pairs), bound: FP64 ALU pipe ---------------
     peaks = measured_peaks()
-    probe = sws.probe_fp64_peak(local)
+    from paper_1403_5044_b200 import debug as sws_debug
+    probe = sws_debug.probe_fp64_peak(local)
     sm_count = probe["sm_count"]
     sm_max = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
     peak_tf = sm_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    mix = sws_debug.probe_fp64_mix(0, 32, local)      # measured issue rate of two-register DFMAs
+    peak_measured_tf = mix["fp64_instr_per_sm_clk"] * 2 * sm_count * sm_max * 1e6 / 1e12
     pairs_timed = args.steps * pairs_per_step
     ap_s = ap_ms * 1e-3
     flops_pair = near * FLOPS_NEAR + (1.0 - near) * FLOPS_FAR
@@ -505,7 +574,13 @@ def run_ours(args) -> None:
     roofline = {
         "bound": "alu", "kernel": "k_allpairs", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
         "frac": achieved_tf / peak_tf, "traffic": NCU_DRAM_BYTES_PER_STATE_LAUNCH.get(cfg.name),
-        "traffic_note": "DRAM bytes per state per all-pairs launch, ncu capture profiles/r1e_allpairs_ncu.md; "
+        "traffic_source": f"{NCU_PROFILE} (static: one ncu --set full capture of this kernel, not measured by this run)",
+        "peak_measured": peak_measured_tf,
+        "peak_measured_source": f"sws_probe_fp64_mix kind 0 (register-only two-register DFMA loop, libsws_debug): "
+                                f"{mix['fp64_instr_per_sm_clk']:.2f} of {FP64_LANES_PER_SM} FP64 thread-instructions/SM/clk "
+                                f"x 2 flops x {sm_count} SMs x {sm_max:.0f} MHz",
+        "frac_of_peak_measured": achieved_tf / peak_measured_tf if peak_measured_tf else None,
+        "traffic_note": "DRAM bytes per state per all-pairs launch; "
                         "algorithmic = S*32 + T*64 bytes read once + one 8 B partial sum per target per column group "
                         "written (part of which stays in L2 until k_assemble reads it)",
         "algorithmic_bytes_per_state": cfg.sources * 32 + cfg.targets * 64 + ctx.plan_info(1)["chunks"] * cfg.targets * 8,
@@ -551,6 +626,10 @@ def run_ours(args) -> None:
     if world == 1 and not args.no_table1:
         table1 = table1_report(sws, local)
 
+    configs = None
+    if world == 1 and not args.no_configs:
+        configs = configs_report(sws, local, peak_tf, [c.name for c in W.CONFIGS[:4]])
+
     fp32 = None
     if world == 1 and not args.no_fp32:
         fp32 = fp32_variant_report(sws, local, names=tuple(dict.fromkeys(["cfg4_361x121", cfg.name])))
@@ -566,12 +645,18 @@ def run_ours(args) -> None:
                    "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "plan": {"single": ctx.plan_info(1), "batch": ctx.plan_info(b + 1)}},
         "pairs_per_s": value * cfg.pairs,
+        # the step evaluates E(u) twice (sws_residual and state 0 of the batch, as BASELINE.json words the config):
+        # a JFNK consumer that takes F0 from the batch needs the b + 1 DISTINCT states of sws_jv_batch alone
+        "jv_batch_alone": {"ms": ms_batch / args.steps, "distinct_states": b + 1,
+                           "distinct_state_evals_per_s": world * args.steps * (b + 1) / (ms_batch * 1e-3)}
+        if world == 1 else None,
         "roofline": roofline, "cpu_baseline": cpu_baseline,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": ms_e2e / e2e_steps},
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
         "workspace_bytes": ctx.workspace_bytes,
+        "configs": configs,
         "jv_exact": jvx,
         "fp32_variant": fp32,
         "solve": solve,
@@ -590,9 +675,10 @@ def run_microbench(args) -> None:
     import paper_1403_5044_b200 as sws
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --microbench: no CUDA device")
-    rows = [sws.probe_fp64_mix(k, w) for k in range(len(sws.FP64_MIX_KINDS)) for w in (16, 32, 64)]
+    from paper_1403_5044_b200 import debug as sws_debug
+    rows = [sws_debug.probe_fp64_mix(k, w) for k in range(len(sws_debug.FP64_MIX_KINDS)) for w in (16, 32, 64)]
     print(json.dumps({"microbench": "fp64_instruction_mix", "unit": "FP64 thread-instructions / SM / clk (64 = issue limit)",
-                      "rows": rows, "dfma_probe": sws.probe_fp64_peak(0)}), flush=True)
+                      "rows": rows, "dfma_probe": sws_debug.probe_fp64_peak(0)}), flush=True)
 
 
 def main() -> None:
@@ -609,6 +695,7 @@ def main() -> None:
     ap.add_argument("--no-jv-exact", action="store_true", help="skip the analytic-Jv section")
     ap.add_argument("--no-solve", action="store_true", help="skip the full JFNK solve section")
     ap.add_argument("--no-table1", action="store_true", help="skip the paper's Table 1 meshes")
+    ap.add_argument("--no-configs", action="store_true", help="skip the FP64 section on BASELINE configs 1-4")
     ap.add_argument("--microbench", action="store_true", help="only run the FP64 instruction-mix probes")
     args = ap.parse_args()
     if args.microbench:

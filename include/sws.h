@@ -82,9 +82,18 @@ int sws_residual(sws_ctx* ctx, const double* u_dev, double* F_dev, void* cuda_st
 /* JV_dev[b][n] (row-major) = (E(u_b) - E(u)) / sigma_b with u_b = fma(sigma_b, v_b, u)
  * entry by entry in FP64, for the b rows v_b of V_dev[b][n].  Step a10, eq. (25) L219.
  *   sigma_host  [b] shifts in pageable host memory, read during the call; NULL selects
- *               sigma_b = 1e-7 (1 + ||u||_2) / ||v_b||_2 computed on the device.
+ *               sigma_b = 1e-7 (1 + ||u||_2) / ||v_b||_2 computed on the device.  A zero direction
+ *               (||v_b|| = 0) gets sigma_b = 0, E(u_b) = E(u) and the exact row JV_b = 0; a caller's
+ *               sigma_b = 0 means the same; NaN / inf shifts are refused (SWS_EINVAL).
  *   Fpert_dev   [b][n] or NULL; receives E(u_b).
- *   F0_dev      [n] or NULL; receives E(u) (the base evaluation the batch performs anyway). */
+ *   F0_dev      [n] or NULL; receives E(u) (the base evaluation the batch performs anyway).
+ * Slot b is bitwise sws_residual(u_b) and F0 is bitwise sws_residual(u): what is guaranteed to
+ * 1e-10 of |E|_inf against the oracle is each E(u_b) (reading Q9 (i)).  The QUOTIENT
+ * inherits the cancellation of eq. (25): two independently rounded FP64 residuals differ by
+ * ~1e-13 |E| before the division by sigma ~ 1e-7, so JV_b carries a relative rounding floor of
+ * 1e-9 .. 1e-7 (measured <= 1e-5 of |JV|_inf against the long-double quotient at every config;
+ * the oracle's own FP64 quotient has the same floor).  Callers who need products to <= 1e-10 use
+ * sws_jv_exact_batch / sws_linearize + sws_jv_apply below, which form J(u) v without a difference. */
 int sws_jv_batch(sws_ctx* ctx, const double* u_dev, const double* V_dev, int32_t b,
                  const double* sigma_host, double* JV_dev, double* Fpert_dev, double* F0_dev,
                  void* cuda_stream);
@@ -128,6 +137,13 @@ int sws_jv_exact_batch_host(sws_ctx* ctx, const double* u_host, const double* V_
  * synchronise of `cuda_stream`.  sigma_host_out has room for b values. */
 int sws_last_sigma(sws_ctx* ctx, int32_t b, double* sigma_host_out, void* cuda_stream);
 
+/* The nodal fields of the state the last sws_residual / sws_jv_batch / sws_linearize call left in the
+ * workspace as state 0 (= its u): zeta, phi (eq. (19)) and zeta_y, phi_y (L160), each [M][N] row-major
+ * (index l N + k) into HOST buffers; any pointer may be NULL.  Synchronises `cuda_stream`.  SWS_ESTATE if
+ * no call has filled the workspace yet. */
+int sws_get_fields_host(sws_ctx* ctx, double* zeta_host, double* phi_host, double* zeta_y_host,
+                        double* phi_y_host, void* cuda_stream);
+
 /* Copy of the parameters the context was set up with (max_batch and device included). */
 int sws_get_params(const sws_ctx* ctx, sws_params* out);
 
@@ -166,6 +182,13 @@ int sws_profile_read(sws_ctx* ctx, double* allpairs_ms, int32_t* launches, int32
  * clamped to what the workspace was sized for). */
 int sws_set_tuning(sws_ctx* ctx, int32_t chunks);
 
+/* Batched all-pairs launches (sws_jv_batch) let one CTA carry `ns` states: the y_j run is staged once and
+ * y_j - y* is formed once per (target, node) for the ns states (north_star: "a batched mode that shares each
+ * staged source tile across b perturbed states" - what the states share is the mesh geometry; the source
+ * records differ).  ns = 1: one state per CTA, states on the grid's z axis; 2: two states per CTA; 0 = library
+ * default (1: measured 4-5 % faster than 2 on B200).  Results do not depend on ns, bit for bit. */
+int sws_set_states_per_cta(sws_ctx* ctx, int32_t ns);
+
 /* Change the source strength epsilon (eq. (6)) of an existing context: the parameter of the
  * bootstrapping / continuation process of L229.  Nothing else of the set-up depends on it.  A
  * linearisation kept by sws_linearize is invalidated. */
@@ -193,34 +216,6 @@ int sws_destroy(sws_ctx* ctx);
 
 const char* sws_strerror(int code);
 const char* sws_last_cuda_error(void);
-
-/* Measurement helpers (no part of the path).
- * sws_probe_fp64_peak: register-only DFMA loop on every SM; reports achieved FP64
- * TFLOP/s (2 flops per DFMA), the SM count and the SM clock (MHz) read back from the
- * device clock64/globaltimer ratio. */
-int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, double* sm_mhz);
-
-/* Instruction-mix probes behind the cycle model of DESIGN.md section 6 (register-only loops, one wave
- * of 256-thread CTAs, warps_per_sm in {8, 16, ..., 64}).  kind: 0 DFMA with two distinct register
- * sources; 1 DFMA with three distinct register sources; 2 DADD; 3 DMUL; 4 eleven two-register DFMA +
- * DADD + DMUL + one MUFU.RSQ64H (+ the move that zeroes the seed's low word); 5 eleven two-register
- * DFMA + three integer instructions.  Reports FP64 thread-instructions per SM per clock (64 = the
- * pipe's issue limit) and the SM clock during the loop. */
-int sws_probe_fp64_mix(int32_t device, int32_t kind, int32_t warps_per_sm, double* fp64_instr_per_sm_clk,
-                       double* sm_mhz);
-
-/* y[i] = the library's device reciprocal square root of x[i] (host buffers), for the
- * unit test of that primitive. */
-int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, int32_t n);
-
-/* Unit test of the far-field expansion: for n pairs (c, g) and the column y1, y1+dy, ..., M nodes,
- * with u-+ = ((y_j -+ c)^2 + g)^-1/2, s-+ = y_j -+ c and c_j = 1/2 at both ends,
- *   nsums = 1: em_host[i]        = the library's expansion of sum_j c_j (u- + u+)        (sws_residual)
- *   nsums = 3: em_host[3i + 0..2] = the same, sum_j c_j (u-^3 + u+^3) and sum_j c_j (s- u-^3 - s+ u+^3)
- *              (the sums of the analytic Jacobian action),
- * and direct_host[...] = the same sums term by term on the device. */
-int sws_debug_s2col_host(int32_t device, double y1, double dy, int32_t M, const double* c_host,
-                         const double* g_host, int32_t n, int32_t nsums, double* direct_host, double* em_host);
 
 #ifdef __cplusplus
 }

@@ -24,10 +24,9 @@ SYMBOLS = (
     "sws_last_sigma", "sws_num_unknowns", "sws_num_targets", "sws_num_sources",
     "sws_workspace_bytes", "sws_last_launch_count", "sws_time_allpairs", "sws_set_tuning",
     "sws_plan_info", "sws_set_profiling", "sws_profile_read", "sws_destroy", "sws_strerror", "sws_last_cuda_error",
-    "sws_probe_fp64_peak", "sws_debug_rsqrt_host",
     "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
     "sws_get_params", "sws_linearize", "sws_jv_apply",
-    "sws_set_farfield", "sws_farfield_stats", "sws_debug_s2col_host", "sws_set_eps", "sws_probe_fp64_mix",
+    "sws_set_farfield", "sws_farfield_stats", "sws_set_eps", "sws_get_fields_host", "sws_set_states_per_cta",
 )
 
 
@@ -83,14 +82,11 @@ def load_library() -> C.CDLL:
         "sws_destroy": (C.c_int, [vp]),
         "sws_strerror": (C.c_char_p, [C.c_int]),
         "sws_last_cuda_error": (C.c_char_p, []),
-        "sws_probe_fp64_peak": (C.c_int, [C.c_int32, C.POINTER(C.c_double), ip, C.POINTER(C.c_double)]),
-        "sws_debug_rsqrt_host": (C.c_int, [C.c_int32, dp, dp, C.c_int32]),
+        "sws_get_fields_host": (C.c_int, [vp, dp, dp, dp, dp, vp]),
         "sws_set_farfield": (C.c_int, [vp, C.c_double]),
         "sws_set_eps": (C.c_int, [vp, C.c_double]),
-        "sws_probe_fp64_mix": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+        "sws_set_states_per_cta": (C.c_int, [vp, C.c_int32]),
         "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
-        "sws_debug_s2col_host": (C.c_int, [C.c_int32, C.c_double, C.c_double, C.c_int32, dp, dp, C.c_int32,
-                                           C.c_int32, dp, dp]),
     }
     for name, (res, args) in proto.items():
         fn = getattr(lib, name)
@@ -136,6 +132,7 @@ class Context:
         self.n = int(self.lib.sws_num_unknowns(h))
         self.targets = int(self.lib.sws_num_targets(h))
         self.sources = int(self.lib.sws_num_sources(h))
+        self._N = int(params["N"])
 
     # -- lifetime ------------------------------------------------------------------
     def close(self) -> None:
@@ -268,6 +265,14 @@ class Context:
         _check(rc, "sws_jv_batch_host")
         return JV, Fp, F0
 
+    def fields_host(self, stream=None):
+        """sws_get_fields_host: (zeta, phi, zeta_y, phi_y), each [M, N], of the state the last call evaluated."""
+        M, N = self.sources // self._N, self._N
+        out = [np.empty((M, N)) for _ in range(4)]
+        _check(self.lib.sws_get_fields_host(self._h, *[_np_ptr(o) for o in out], self._stream(stream)),
+               "sws_get_fields_host")
+        return tuple(out)
+
     def last_sigma(self, b: int, stream=None) -> np.ndarray:
         out = np.empty(int(b))
         _check(self.lib.sws_last_sigma(self._h, int(b), _np_ptr(out), self._stream(stream)), "sws_last_sigma")
@@ -307,6 +312,10 @@ class Context:
     def set_tuning(self, chunks: int = 0) -> None:
         _check(self.lib.sws_set_tuning(self._h, int(chunks)), "sws_set_tuning")
 
+    def set_states_per_cta(self, ns: int = 0) -> None:
+        """sws_set_states_per_cta: states one CTA of a batched all-pairs launch carries (0 default, 1, 2)."""
+        _check(self.lib.sws_set_states_per_cta(self._h, int(ns)), "sws_set_states_per_cta")
+
     def set_eps(self, eps: float) -> None:
         """sws_set_eps: the source strength of the continuation process."""
         _check(self.lib.sws_set_eps(self._h, float(eps)), "sws_set_eps")
@@ -333,48 +342,3 @@ class Context:
     @property
     def workspace_bytes(self) -> int:
         return int(self.lib.sws_workspace_bytes(self._h))
-
-
-def probe_fp64_peak(device: int = 0) -> dict:
-    """Register-only DFMA microbenchmark: {'tflops', 'sm_count', 'sm_mhz'} (sws_probe_fp64_peak)."""
-    lib = load_library()
-    tf, sms, mhz = C.c_double(), C.c_int32(), C.c_double()
-    _check(lib.sws_probe_fp64_peak(int(device), C.byref(tf), C.byref(sms), C.byref(mhz)),
-           "sws_probe_fp64_peak")
-    return dict(tflops=tf.value, sm_count=int(sms.value), sm_mhz=mhz.value)
-
-
-FP64_MIX_KINDS = ("dfma_2reg", "dfma_3reg", "dadd", "dmul", "dfma11_dadd_dmul_mufu_rsq64h", "dfma11_int3")
-
-
-def probe_fp64_mix(kind: int, warps_per_sm: int = 16, device: int = 0) -> dict:
-    """sws_probe_fp64_mix: FP64 thread-instructions per SM per clock of one instruction mix."""
-    lib = load_library()
-    r, mhz = C.c_double(), C.c_double()
-    _check(lib.sws_probe_fp64_mix(int(device), int(kind), int(warps_per_sm), C.byref(r), C.byref(mhz)),
-           "sws_probe_fp64_mix")
-    return {"kind": FP64_MIX_KINDS[kind], "warps_per_sm": int(warps_per_sm), "fp64_instr_per_sm_clk": r.value,
-            "sm_mhz": mhz.value}
-
-
-def debug_rsqrt(x: np.ndarray, device: int = 0) -> np.ndarray:
-    """The library's device reciprocal square root applied to host values (unit test hook)."""
-    lib = load_library()
-    x = np.ascontiguousarray(x, dtype=np.float64)
-    y = np.empty_like(x)
-    _check(lib.sws_debug_rsqrt_host(int(device), _np_ptr(x), _np_ptr(y), int(x.size)), "sws_debug_rsqrt_host")
-    return y
-
-
-def debug_s2col(y1: float, dy: float, M: int, c: np.ndarray, g: np.ndarray, device: int = 0, nsums: int = 1):
-    """(direct, em): the S2 column sum(s) term by term on the device and by the library's far-field
-    expansion (unit test hook, sws_debug_s2col_host).  nsums = 3: arrays [n][3] of the sums of the
-    analytic Jacobian action."""
-    lib = load_library()
-    c = np.ascontiguousarray(c, dtype=np.float64)
-    g = np.ascontiguousarray(g, dtype=np.float64)
-    shape = (c.size,) if nsums == 1 else (c.size, 3)
-    d, e = np.empty(shape), np.empty(shape)
-    _check(lib.sws_debug_s2col_host(int(device), float(y1), float(dy), int(M), _np_ptr(c), _np_ptr(g),
-                                    int(c.size), int(nsums), _np_ptr(d), _np_ptr(e)), "sws_debug_s2col_host")
-    return d, e

@@ -1,4 +1,4 @@
-"""Build libsws.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+"""Build libsws.so, libsws_jfnk.so and libsws_debug.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_1403_5044_b200.build [--force] [--verbose]
 """
@@ -16,7 +16,10 @@ LIB = PKG / "libsws.so"
 LIB_JFNK = PKG / "libsws_jfnk.so"  # the Newton-Krylov driver: calls libsws through its C-ABI, + cuBLAS/cuSOLVER
 SOURCES_JFNK = ["jfnk_precond.cu", "jfnk_solver.cu"]
 CUDA_LIB64 = "/usr/local/cuda/lib64"
-SOURCES = ["sws_api.cu", "sws_fields.cu", "sws_allpairs.cu", "sws_allpairs_f32.cu", "sws_jv_exact.cu", "sws_probe.cu"]
+SOURCES = ["sws_api.cu", "sws_fields.cu", "sws_allpairs.cu", "sws_allpairs_f32.cu", "sws_jv_exact.cu"]
+# test hooks and FP64 issue-rate probes (include/sws_debug.h): a library of its own, not part of the product
+LIB_DEBUG = PKG / "libsws_debug.so"
+SOURCES_DEBUG = ["sws_debug.cu", "sws_probe.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -29,10 +32,10 @@ def _nvcc() -> str:
 
 
 def needs_build() -> bool:
-    if not LIB.exists() or not LIB_JFNK.exists():
+    if not LIB.exists() or not LIB_JFNK.exists() or not LIB_DEBUG.exists():
         return True
-    t = min(LIB.stat().st_mtime, LIB_JFNK.stat().st_mtime)
-    deps = [CSRC / s for s in SOURCES + SOURCES_JFNK] + [CSRC / "sws_internal.cuh", CSRC / "sws_stage.cuh", CSRC / "sws_farfield.cuh",
+    t = min(LIB.stat().st_mtime, LIB_JFNK.stat().st_mtime, LIB_DEBUG.stat().st_mtime)
+    deps = [CSRC / s for s in SOURCES + SOURCES_JFNK + SOURCES_DEBUG] + [ROOT / "include" / "sws_debug.h"] + [CSRC / "sws_internal.cuh", CSRC / "sws_stage.cuh", CSRC / "sws_farfield.cuh",
                                                          CSRC / "jfnk_internal.cuh", ROOT / "include" / "sws.h",
                                                          ROOT / "include" / "sws_jfnk.h"]
     return any(d.stat().st_mtime > t for d in deps)
@@ -52,6 +55,9 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     cmd += [str(CSRC / s) for s in SOURCES_JFNK] + [f"-L{PKG}", "-l:libsws.so", "-lcublas", "-lcusolver",
                                                     "-Xlinker", "-rpath=$ORIGIN", "-Xlinker", f"-rpath={CUDA_LIB64}",
                                                     "-Xlinker", "-soname=libsws_jfnk.so", "-o", str(LIB_JFNK)]
+    subprocess.run(cmd, check=True)
+    cmd = [_nvcc(), *NVCC_FLAGS, "-DSWS_BUILD_DEBUG_HOOKS", f"-I{ROOT / 'include'}"]
+    cmd += [str(CSRC / s) for s in SOURCES_DEBUG] + ["-Xlinker", "-soname=libsws_debug.so", "-o", str(LIB_DEBUG)]
     subprocess.run(cmd, check=True)
     return LIB
 

@@ -23,6 +23,20 @@ struct LinMesh {
   double a11, a12;  // n - x1/dx, x1/dx
 };
 
+// Entry points run on their object's device and put the caller's current device back on return.
+struct DevGuard {
+  int prev = -1;
+  cudaError_t err;
+  explicit DevGuard(int dev) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev);
+    else prev = -1;
+  }
+  ~DevGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
 constexpr int kGemvThreads = 256;
 constexpr int kDotBlocks = 296;   // 2 CTAs per SM on 148 SMs
 constexpr int kDotThreads = 256;

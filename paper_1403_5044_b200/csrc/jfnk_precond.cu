@@ -381,8 +381,9 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
   std::vector<double> Gh;
   std::vector<int> info_h;
   cudaStream_t st = nullptr;
+  DevGuard dg(p->device);
 
-  CK(cudaSetDevice(p->device));
+  CK(dg.err);
   CK(cudaMalloc(&pc->G, blk * sizeof(double)));
   CK(cudaMalloc(&pc->corr, (size_t)T * sizeof(double)));
   CK(cudaMalloc(&pc->s1, (size_t)m.H * sizeof(double)));
@@ -544,6 +545,8 @@ static void build_sweep_graph(sws_precond* pc) {
 int sws_precond_apply(sws_precond* pc, const double* v_dev, double* r_dev, void* cuda_stream) {
   if (!pc || !v_dev || !r_dev) return SWS_EINVAL;
   if (!pc->factored) return SWS_EINVAL;
+  DevGuard dg(pc->device);
+  if (dg.err != cudaSuccess) return fail_cuda(dg.err, "sws_precond_apply (device)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const LinMesh& m = pc->lm;
   const int n1 = m.n1, M = m.M;
@@ -566,7 +569,8 @@ int sws_precond_block_host(sws_precond* pc, int32_t which, int32_t l, int32_t mm
   const int s = mm - l + pc->hb;
   if (s < 0 || s > 2 * pc->hb) return SWS_EINVAL;
   const int n1 = pc->lm.n1;
-  cudaError_t e = cudaSetDevice(pc->device);
+  DevGuard dg(pc->device);
+  cudaError_t e = dg.err;
   if (e == cudaSuccess) e = launch_assemble_row(pc, l, which, pc->panel, nullptr);
   std::vector<double> cm((size_t)n1 * n1);
   if (e == cudaSuccess)
@@ -583,7 +587,7 @@ double sws_precond_setup_ms(const sws_precond* pc) { return pc ? pc->setup_ms : 
 
 int sws_precond_destroy(sws_precond* pc) {
   if (!pc) return SWS_OK;
-  cudaSetDevice(pc->device);
+  DevGuard dg(pc->device);
   if (pc->sweep_graph) cudaGraphExecDestroy(pc->sweep_graph);
   double* bufs[] = {pc->G, pc->corr, pc->fwd, pc->bwd, pc->s1, pc->t2, pc->y, pc->panel};
   for (double* b : bufs)

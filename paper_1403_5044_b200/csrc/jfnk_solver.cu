@@ -269,6 +269,7 @@ int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opt
   while (its < o->maxit) {
     if (!first) RC(norms(s, s->r, &beta, nullptr, st));
     first = false;
+    if (!(beta > 0.0)) { rel = 0.0; break; }  // the restart residual vanished: d is exact, nothing to normalise
     k_axpby<<<nblk(n), 256, 0, st>>>(s->V, 1.0 / beta, s->r, 0.0, s->r, n);
     std::fill(g.begin(), g.end(), 0.0);
     g[0] = beta;
@@ -309,7 +310,17 @@ int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opt
         Hm(i + 1, j) = -sn[i] * Hm(i, j) + cs[i] * Hm(i + 1, j);
         Hm(i, j) = tmp;
       }
+      // happy breakdown: w lies in the span of the basis (h_{j+1,j} = 0 up to rounding); k_normalise left
+      // V_{j+1} alone, the least-squares problem is solved exactly with the j + 1 columns at hand
+      double hcol = 0.0;
+      for (int i = 0; i <= j; ++i) hcol = std::max(hcol, std::fabs(Hm(i, j)));
+      const bool breakdown = !(Hm(j + 1, j) > 1e-300) || Hm(j + 1, j) <= 1e-15 * hcol;
+      if (breakdown) Hm(j + 1, j) = 0.0;
       const double rho = std::hypot(Hm(j, j), Hm(j + 1, j));
+      if (rho == 0.0) {  // J P^-1 v_j = 0: the column adds nothing; stop with what was reached
+        jd = j;
+        break;
+      }
       cs[j] = Hm(j, j) / rho; sn[j] = Hm(j + 1, j) / rho;
       Hm(j, j) = rho; Hm(j + 1, j) = 0.0;
       g[j + 1] = -sn[j] * g[j];
@@ -317,7 +328,7 @@ int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opt
       jd = j + 1;
       rel = std::fabs(g[j + 1]) / bnorm;
       if (hist) hist[its - 1] = rel;
-      if (std::fabs(g[j + 1]) <= o->tol * bnorm || its >= o->maxit) break;
+      if (breakdown || std::fabs(g[j + 1]) <= o->tol * bnorm || its >= o->maxit) break;
     }
     // y = R^-1 g (back substitution), d += P^-1 (V y)
     for (int i = jd - 1; i >= 0; --i) {
@@ -330,7 +341,7 @@ int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opt
     RC(apply_pinv(s, s->t, s->z, st));
     k_axpby<<<nblk(n), 256, 0, st>>>(d, 1.0, d, 1.0, s->z, n);
     CU(cudaStreamSynchronize(st));  // y is host memory reused by the next cycle
-    if (rel <= o->tol || its >= o->maxit) break;
+    if (rel <= o->tol || its >= o->maxit || jd == 0) break;
     // restart: r = rhs - J d
     RC(apply_jv(s, u, d, s->w, o->jv_mode, st, E0, unorm));
     k_axpby<<<nblk(n), 256, 0, st>>>(s->r, 1.0, rhs, -1.0, s->w, n);
@@ -381,7 +392,8 @@ int sws_solver_create(sws_ctx* ctx, sws_precond* pc, int32_t max_restart, sws_so
   const size_t n = (size_t)s->n;
   double* base = nullptr;
   const size_t vec = (size_t)(max_restart + 1) + 12;
-  cudaError_t e = cudaSetDevice(p.device);
+  DevGuard dg(p.device);
+  cudaError_t e = dg.err;
   if (e == cudaSuccess) e = cudaMalloc(&base, vec * n * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&s->partial, sizeof(double) * kDotBlocks * (max_restart + 2));
   if (e == cudaSuccess) e = cudaMalloc(&s->hdev, sizeof(double) * (2 * (max_restart + 1) + 2));
@@ -405,7 +417,8 @@ int sws_solver_create(sws_ctx* ctx, sws_precond* pc, int32_t max_restart, sws_so
 int sws_solver_gmres(sws_solver* s, const double* u_dev, const double* rhs_dev, const sws_gmres_opts* opts,
                      double* d_dev, sws_gmres_stats* stats, double* hist_host, void* cuda_stream) {
   if (!s || !u_dev || !rhs_dev || !opts || !d_dev || !stats) return SWS_EINVAL;
-  CU(cudaSetDevice(s->device));
+  DevGuard dg(s->device);
+  CU(dg.err);
   reset_accounting(s);
   return gmres(s, u_dev, rhs_dev, opts, d_dev, stats, hist_host, (cudaStream_t)cuda_stream);
 }
@@ -416,7 +429,8 @@ int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sw
   if (o->max_newton < 0 || o->max_halvings < 0) return SWS_EINVAL;
   if (o->forcing != 0 && o->forcing != 1) return SWS_EINVAL;
   if (o->forcing == 1 && !(o->eta > 0.0 && o->eta <= o->eta_max && o->eta_max < 1.0)) return SWS_EINVAL;
-  CU(cudaSetDevice(s->device));
+  DevGuard dg(s->device);
+  CU(dg.err);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const auto t0 = std::chrono::steady_clock::now();
   reset_accounting(s);
@@ -472,7 +486,8 @@ int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sw
 int sws_solver_continuation(sws_solver* s, double* u_dev, const double* eps_host, int32_t n_eps,
                             const sws_newton_opts* o, sws_newton_stats* stats, int32_t* n_done, void* cuda_stream) {
   if (!s || !u_dev || !eps_host || n_eps < 1 || !o || !stats || !n_done) return SWS_EINVAL;
-  CU(cudaSetDevice(s->device));
+  DevGuard dg(s->device);
+  CU(dg.err);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   *n_done = 0;
   std::vector<sws_newton_log> log((size_t)o->max_newton + 1);
@@ -493,7 +508,7 @@ int sws_solver_continuation(sws_solver* s, double* u_dev, const double* eps_host
 
 int sws_solver_destroy(sws_solver* s) {
   if (!s) return SWS_OK;
-  cudaSetDevice(s->device);
+  DevGuard dg(s->device);
   if (s->V) cudaFree(s->V);
   if (s->partial) cudaFree(s->partial);
   if (s->hdev) cudaFree(s->hdev);

@@ -50,94 +50,131 @@ constexpr int kThreads64 = SWS_PAIR_THREADS;
 #endif
 constexpr int kNT2MinTargets = SWS_NT2_MIN_TARGETS;
 constexpr int kMinB2 = 6;  // resident CTAs per SM of the two-target kernel
+#ifndef SWS_MINB12
+#define SWS_MINB12 6
+#endif
+#ifndef SWS_MINB22
+#define SWS_MINB22 4
+#endif
+constexpr int kMinB12 = SWS_MINB12;  // ... of the one-target, two-state kernel (batches on small meshes)
+constexpr int kMinB22 = SWS_MINB22;  // ... of the two-target, two-state kernel (batches on large meshes)
 
-// Per-thread constants of one target and of the current source column.
+// Per-thread constants of one target and of the current source column, split into what is GEOMETRY (the same
+// for every state of a batch: the mesh does not move) and what depends on the state.
 // The S2 quadratic forms are used with the square completed (C > 0):
 //   A dx^2 + B dx (y-y*) + C (y-y*)^2 = C [ (y - c)^2 + g ],
 //   A dx^2 - B dx (y+y*) + C (y+y*)^2 = C [ (y + c)^2 + g ],
 //   c = y* - (B / 2C) dx,   g = (A/C - (B/2C)^2) dx^2 = (4AC - B^2) dx^2 / (4 C^2) > 0,
 // so that each form costs one add and one two-register FMA per pair, c and g are per
 // (target, column), and the common factor 1/sqrt(C) is applied once per target at the end.
-struct TgtC {
-  double ys, zs, psis;
-  double ys2, ys4;  // 2 y*, 4 y*: the image terms follow from the direct ones (below)
+struct TgtG {
+  double ys, ys2, ys4;  // y*, 2 y*, 4 y*: the image terms follow from the direct ones (below)
 };
-struct ColC {
-  double dx, dx2, c, g;  // x_i - x*, its square, and the S2 constants above
+struct TgtS {
+  double zs, psis;  // zeta*, phi* - x*
+};
+struct ColG {
+  double dx, dx2;  // x_i - x*, its square
+};
+struct ColS {
+  double c, g;  // the S2 constants above (A, B, C belong to the state)
 };
 
 // One source node against one target: adds (phi-phi*-x+x*) K1 + zeta_x K2 to a1 and, if S2T,
 // sqrt(C) S2 to aS (unit weight).  S2T = false is the far-field form: the S2 terms of the
 // whole column come from s2_column_em() below, 28 FP64 instructions + 2 MUFU.RSQ64H remain.
+// dm = y_j - y* is passed in: it is geometry, formed once per (target, node) for all states of the CTA.
 template <bool S2T>
-__device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, const double yj,
-                                          const TgtC& t, const ColC& c, double& a1, double& aS) {
+__device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, const double yj, const double dm,
+                                          const TgtG& tg, const TgtS& ts, const ColG& cg, const ColS& cs,
+                                          double& a1, double& aS) {
   const double z = zp.x, psi = zp.y, zx = sl.x, zy = sl.y;
   // Image terms from the direct ones (all y >= 0, sws_setup): (y + y*)^2 = (y - y*)^2 + 4 y y* and
   // y + y* = (y - y*) + 2 y*, so y + y* itself is never formed: one DADD less per pair.  R+^2 >= R-^2, so
   // the rounding of R-^2 it inherits is below its own.
-  const double dm = yj - t.ys;  // y - y*
-  const double dz = z - t.zs;
-  const double q = fma(dz, dz, c.dx2);
+  const double dz = z - ts.zs;
+  const double q = fma(dz, dz, cg.dx2);
   const double Rm2 = fma(dm, dm, q);
-  const double Rp2 = fma(t.ys4, yj, Rm2);
+  const double Rp2 = fma(tg.ys4, yj, Rm2);
   const double rm = rsqrt_fp64(Rm2);
   const double rp = rsqrt_fp64(Rp2);
   // K1 numerators: zeta - zeta* - (x-x*) zeta_x - (y -+ y*) zeta_y, slopes at the source (Q2)
-  const double n0 = fma(-c.dx, zx, dz);
+  const double n0 = fma(-cg.dx, zx, dz);
   const double nm = fma(-dm, zy, n0);
-  const double np = fma(-t.ys2, zy, nm);
+  const double np = fma(-tg.ys2, zy, nm);
   const double rm3 = (rm * rm) * rm;
   const double rp3 = (rp * rp) * rp;
   const double k1 = fma(np, rp3, nm * rm3);
-  const double dpsi = psi - t.psis;
+  const double dpsi = psi - ts.psis;
   a1 = fma(dpsi, k1, a1);
   a1 = fma(zx, rm + rp, a1);  // K2 = 1/R- + 1/R+
   if (S2T) {
     // S2 (eqs. (21), (22)) up to the factor 1/sqrt(C)
-    const double sm = yj - c.c;
-    const double sp = yj + c.c;
-    const double Qm = fma(sm, sm, c.g);
-    const double Qp = fma(sp, sp, c.g);
+    const double sm = yj - cs.c;
+    const double sp = yj + cs.c;
+    const double Qm = fma(sm, sm, cs.g);
+    const double Qp = fma(sp, sp, cs.g);
     aS += rsqrt_fp64(Qm) + rsqrt_fp64(Qp);
   }
 }
 
-// One staged segment [j0, j0 + len) of a column for the NT targets of a thread: trapezoid half weights on the
-// column's first and last node by peeling (Q4), unit weights inside.  The staged record of a node is loaded
-// once for the NT targets.
-template <bool S2T, int NT>
-__device__ __forceinline__ void walk_segment(const double2* rec, const double* yy, const int j0, const int len,
-                                             const int M, const TgtC (&tg)[NT], const ColC (&cc)[NT],
-                                             double (&col1)[NT], double (&colS)[NT]) {
+// One staged segment [j0, j0 + len) of a column for the NT targets x NS states of a thread: trapezoid half
+// weights on the column's first and last node by peeling (Q4), unit weights inside.  A node's y_j and
+// y_j - y* are formed once for the NS states (batched Jv: the states share the mesh), its staged record of
+// each state is loaded once for the NT targets.  rec[m]: state m's records of this segment.
+template <bool S2T, int NT, int NS>
+__device__ __forceinline__ void walk_segment(const double2* const (&rec)[NS], const double* yy, const int j0,
+                                             const int len, const int M, const TgtG (&tg)[NT],
+                                             const TgtS (&ts)[NS][NT], const ColG (&cg)[NT],
+                                             const ColS (&cs)[NS][NT], double (&col1)[NS][NT],
+                                             double (&colS)[NS][NT]) {
   int jlo = 0, jhi = len;
-  if (j0 == 0) {  // first node of the column: weight 1/2 in y
+  auto node = [&](const int j, double (&o1)[NS][NT], double (&oS)[NS][NT]) {
+    const double yj = yy[j];
+    double dm[NT];
 #pragma unroll
-    for (int n = 0; n < NT; ++n) {
-      double h1 = 0.0, hS = 0.0;
-      pair_term<S2T>(rec[0], rec[1], yy[0], tg[n], cc[n], h1, hS);
-      col1[n] = 0.5 * h1;
-      colS[n] = 0.5 * hS;
+    for (int n = 0; n < NT; ++n) dm[n] = yj - tg[n].ys;  // y - y*
+#pragma unroll
+    for (int m = 0; m < NS; ++m) {
+      const double2 r0 = rec[m][2 * j], r1 = rec[m][2 * j + 1];
+#pragma unroll
+      for (int n = 0; n < NT; ++n) pair_term<S2T>(r0, r1, yj, dm[n], tg[n], ts[m][n], cg[n], cs[m][n], o1[m][n], oS[m][n]);
     }
+  };
+  if (j0 == 0) {  // first node of the column: weight 1/2 in y
+    double h1[NS][NT], hS[NS][NT];
+#pragma unroll
+    for (int m = 0; m < NS; ++m)
+#pragma unroll
+      for (int n = 0; n < NT; ++n) h1[m][n] = hS[m][n] = 0.0;
+    node(0, h1, hS);
+#pragma unroll
+    for (int m = 0; m < NS; ++m)
+#pragma unroll
+      for (int n = 0; n < NT; ++n) {
+        col1[m][n] = 0.5 * h1[m][n];
+        colS[m][n] = 0.5 * hS[m][n];
+      }
     jlo = 1;
   }
   const bool last = (j0 + len == M);
   if (last) jhi = len - 1;
 #pragma unroll kUnroll
-  for (int j = jlo; j < jhi; ++j) {
-    const double2 r0 = rec[2 * j], r1 = rec[2 * j + 1];
-    const double yj = yy[j];
-#pragma unroll
-    for (int n = 0; n < NT; ++n) pair_term<S2T>(r0, r1, yj, tg[n], cc[n], col1[n], colS[n]);
-  }
+  for (int j = jlo; j < jhi; ++j) node(j, col1, colS);
   if (last && jhi >= jlo) {  // last node of the column: weight 1/2 in y
+    double h1[NS][NT], hS[NS][NT];
 #pragma unroll
-    for (int n = 0; n < NT; ++n) {
-      double h1 = 0.0, hS = 0.0;
-      pair_term<S2T>(rec[2 * jhi], rec[2 * jhi + 1], yy[jhi], tg[n], cc[n], h1, hS);
-      col1[n] = fma(0.5, h1, col1[n]);
-      colS[n] = fma(0.5, hS, colS[n]);
-    }
+    for (int m = 0; m < NS; ++m)
+#pragma unroll
+      for (int n = 0; n < NT; ++n) h1[m][n] = hS[m][n] = 0.0;
+    node(jhi, h1, hS);
+#pragma unroll
+    for (int m = 0; m < NS; ++m)
+#pragma unroll
+      for (int n = 0; n < NT; ++n) {
+        col1[m][n] = fma(0.5, h1[m][n], col1[m][n]);
+        colS[m][n] = fma(0.5, hS[m][n], colS[m][n]);
+      }
   }
 }
 
@@ -148,46 +185,62 @@ struct PairArgs {
   const TgtRec* tgt;  // [state][T]
   double* part;       // [state][chunks][T]
   int N, M, T;
+  int states;         // states of this launch (NS of them per CTA)
   int chunks, cols_per_chunk, seg_len, nseg;
   double dxdy;
   EmGeom em;
 };
 
-template <int MINB, int NT>
+// NS = states per CTA.  NS = 1 is the single evaluation; NS = 2 is the batched mode of sws_jv_batch: the CTA
+// stages the y_j run once and one record run per state, and a thread forms y_j - y* once for its NS states.
+// Every (state, target) sum goes through the same operations in the same order whatever NS is, and a column
+// whose far/near decision differs between the states of a CTA is walked state by state, so that slot b of a
+// batch stays bitwise sws_residual(u_b).
+template <int MINB, int NT, int NS>
 __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int seg_pad = a.seg_len;  // even by construction
-  SrcRec* s_rec = reinterpret_cast<SrcRec*>(smem_raw);                            // [kStages][seg_pad]
-  double* s_y = reinterpret_cast<double*>(s_rec + (size_t)kStages * seg_pad);     // [kStages][seg_pad]
-  uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_y + (size_t)kStages * seg_pad);  // [kStages]
+  SrcRec* s_rec = reinterpret_cast<SrcRec*>(smem_raw);                                  // [kStages][NS][seg_pad]
+  double* s_y = reinterpret_cast<double*>(s_rec + (size_t)kStages * NS * seg_pad);      // [kStages][seg_pad]
+  uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_y + (size_t)kStages * seg_pad);       // [kStages]
 
   const int tid = threadIdx.x;
-  const int tile = blockIdx.x, chunk = blockIdx.y, state = blockIdx.z;
+  const int tile = blockIdx.x, chunk = blockIdx.y, state0 = blockIdx.z * NS;
+  int st[NS];  // the states of this CTA; a ragged last group recomputes the last state and stores nothing
+#pragma unroll
+  for (int m = 0; m < NS; ++m) st[m] = state0 + m < a.states ? state0 + m : a.states - 1;
   // Threads take the targets in TRANSPOSED order, slot = k M + l: the 32 targets of a warp then share one
   // x* (two at most), so the columns that are near for a warp are the 2 r of one target, not 32 + 2 r
   // (near fraction 2.3 % instead of 6.5 % at 721x241).  t = l (N-1) + k is the index everything is stored by.
   // A thread owns NT targets, kThreads64 slots apart, and walks the staged records once for all of them.
   int t[NT];
-  TgtC tg[NT];
-  double xs[NT], kb[NT], kg[NT], sfac[NT];
+  TgtG tg[NT];
+  TgtS ts[NS][NT];
+  double xs[NT], kb[NS][NT], kg[NS][NT], sfac[NS][NT];
 #pragma unroll
   for (int n = 0; n < NT; ++n) {
     const int slot = (tile * NT + n) * kThreads64 + tid;
     const int sc = slot < a.T ? slot : a.T - 1;  // ragged tail: recompute the last target, never stored
     const int tc = target_of_slot(sc, a.N, a.M);
     t[n] = slot < a.T ? tc : a.T;
-    const TgtRec tr = a.tgt[(size_t)state * a.T + tc];
-    tg[n] = {tr.ys, tr.zs, tr.psis, 2.0 * tr.ys, 4.0 * tr.ys};
-    xs[n] = tr.xs;
-    kb[n] = tr.B / (2.0 * tr.C);                 // B / 2C
-    kg[n] = tr.A / tr.C - kb[n] * kb[n];         // (4AC - B^2) / (4 C^2)
-    sfac[n] = -tr.zxs * rsqrt_fp64(tr.C);
+#pragma unroll
+    for (int m = 0; m < NS; ++m) {
+      const TgtRec tr = a.tgt[(size_t)st[m] * a.T + tc];
+      if (m == 0) {  // x*, y* are the mesh's: the same in every state
+        tg[n] = {tr.ys, 2.0 * tr.ys, 4.0 * tr.ys};
+        xs[n] = tr.xs;
+      }
+      ts[m][n] = {tr.zs, tr.psis};
+      kb[m][n] = tr.B / (2.0 * tr.C);                    // B / 2C
+      kg[m][n] = tr.A / tr.C - kb[m][n] * kb[m][n];      // (4AC - B^2) / (4 C^2)
+      sfac[m][n] = -tr.zxs * rsqrt_fp64(tr.C);
+    }
   }
 
   const int c0 = chunk * a.cols_per_chunk;
   const int c1 = min(a.N, c0 + a.cols_per_chunk);
   const int nitems = (c1 - c0) * a.nseg;  // (column, segment) work items of this CTA
-  const SrcRec* src = a.src + (size_t)state * a.N * a.M;
+  const size_t plane = (size_t)a.N * a.M;
 
   if (tid == 0) {
     for (int s = 0; s < kStages; ++s) mbar_init(&s_bar[s], 1);
@@ -201,16 +254,21 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
     const int len = min(a.seg_len, a.M - j0);
     const uint32_t rec_bytes = (uint32_t)len * (uint32_t)sizeof(SrcRec);
     const uint32_t y_bytes = (uint32_t)((len + 1) & ~1) * 8u;  // y is padded to an even count
-    mbar_expect_tx(&s_bar[s], rec_bytes + y_bytes);
-    bulk_g2s(s_rec + (size_t)s * seg_pad, src + (size_t)i * a.M + j0, rec_bytes, &s_bar[s]);
+    mbar_expect_tx(&s_bar[s], NS * rec_bytes + y_bytes);
+#pragma unroll
+    for (int m = 0; m < NS; ++m)
+      bulk_g2s(s_rec + ((size_t)s * NS + m) * seg_pad, a.src + st[m] * plane + (size_t)i * a.M + j0, rec_bytes,
+               &s_bar[s]);
     bulk_g2s(s_y + (size_t)s * seg_pad, a.y + j0, y_bytes, &s_bar[s]);
   };
 
   if (tid == 0 && nitems > 0) issue(0);
 
-  double tot1[NT], totS[NT];
+  double tot1[NS][NT], totS[NS][NT];
 #pragma unroll
-  for (int n = 0; n < NT; ++n) tot1[n] = totS[n] = 0.0;
+  for (int m = 0; m < NS; ++m)
+#pragma unroll
+    for (int n = 0; n < NT; ++n) tot1[m][n] = totS[m][n] = 0.0;
   for (int q = 0; q < nitems; ++q) {
     const int s = q % kStages;
     // the buffer written here was last read in iteration q-1, which ended with __syncthreads()
@@ -218,47 +276,90 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
 
     const int i = c0 + q / a.nseg, j0 = (q % a.nseg) * a.seg_len;
     const int len = min(a.seg_len, a.M - j0);
-    ColC cc[NT];
+    ColG cg[NT];
+    ColS cs[NS][NT];
     const double xi = __ldg(a.x + i);
-    bool far_t = true;
+    bool far_m[NS];
+#pragma unroll
+    for (int m = 0; m < NS; ++m) far_m[m] = true;
 #pragma unroll
     for (int n = 0; n < NT; ++n) {
-      cc[n].dx = xi - xs[n];
-      cc[n].dx2 = cc[n].dx * cc[n].dx;
-      cc[n].c = fma(-kb[n], cc[n].dx, tg[n].ys);
-      cc[n].g = kg[n] * cc[n].dx2;
-      far_t = far_t && (cc[n].g >= a.em.gmin);
+      cg[n].dx = xi - xs[n];
+      cg[n].dx2 = cg[n].dx * cg[n].dx;
+#pragma unroll
+      for (int m = 0; m < NS; ++m) {
+        cs[m][n].c = fma(-kb[m][n], cg[n].dx, tg[n].ys);
+        cs[m][n].g = kg[m][n] * cg[n].dx2;
+        far_m[m] = far_m[m] && (cs[m][n].g >= a.em.gmin);
+      }
     }
     const double ci = (i == 0 || i == a.N - 1) ? 0.5 : 1.0;  // trapezoid weight in x (Q4)
 
+    // warp-uniform far/near decision PER STATE (far for every target of the warp), as a single evaluation takes it
+    int nfar = 0;
+#pragma unroll
+    for (int m = 0; m < NS; ++m) {
+      far_m[m] = __all_sync(0xffffffffu, far_m[m]);
+      nfar += far_m[m] ? 1 : 0;
+    }
+
     mbar_wait(&s_bar[s], (uint32_t)((q / kStages) & 1));
 
-    const double2* rec = reinterpret_cast<const double2*>(s_rec + (size_t)s * seg_pad);
+    const double2* rec[NS];
+#pragma unroll
+    for (int m = 0; m < NS; ++m) rec[m] = reinterpret_cast<const double2*>(s_rec + ((size_t)s * NS + m) * seg_pad);
     const double* yy = s_y + (size_t)s * seg_pad;
-    double col1[NT], colS[NT];
+    double col1[NS][NT], colS[NS][NT];
 #pragma unroll
-    for (int n = 0; n < NT; ++n) col1[n] = colS[n] = 0.0;
-    if (__all_sync(0xffffffffu, far_t)) {  // warp-uniform: far for every target of the warp
-      walk_segment<false, NT>(rec, yy, j0, len, a.M, tg, cc, col1, colS);
-      if (j0 == 0) {
+    for (int m = 0; m < NS; ++m)
 #pragma unroll
-        for (int n = 0; n < NT; ++n) colS[n] = s2_column_em(a.em, cc[n].c, cc[n].g);  // the column's S2 terms, once
+      for (int n = 0; n < NT; ++n) col1[m][n] = colS[m][n] = 0.0;
+    if (nfar == NS) {
+      walk_segment<false, NT, NS>(rec, yy, j0, len, a.M, tg, ts, cg, cs, col1, colS);
+    } else if (nfar == 0) {
+      walk_segment<true, NT, NS>(rec, yy, j0, len, a.M, tg, ts, cg, cs, col1, colS);
+    } else if (NS > 1) {  // the states disagree (a column at the edge of the radius): one state at a time
+#pragma unroll
+      for (int m = 0; m < NS; ++m) {
+        const double2* const rec1[1] = {rec[m]};
+        TgtS ts1[1][NT];
+        ColS cs1[1][NT];
+        double c11[1][NT], c1S[1][NT];
+#pragma unroll
+        for (int n = 0; n < NT; ++n) { ts1[0][n] = ts[m][n]; cs1[0][n] = cs[m][n]; c11[0][n] = c1S[0][n] = 0.0; }
+        if (far_m[m]) walk_segment<false, NT, 1>(rec1, yy, j0, len, a.M, tg, ts1, cg, cs1, c11, c1S);
+        else walk_segment<true, NT, 1>(rec1, yy, j0, len, a.M, tg, ts1, cg, cs1, c11, c1S);
+#pragma unroll
+        for (int n = 0; n < NT; ++n) { col1[m][n] = c11[0][n]; colS[m][n] = c1S[0][n]; }
       }
-    } else {
-      walk_segment<true, NT>(rec, yy, j0, len, a.M, tg, cc, col1, colS);
+    }
+    if (j0 == 0) {
+#pragma unroll
+      for (int m = 0; m < NS; ++m)
+        if (far_m[m]) {
+#pragma unroll
+          for (int n = 0; n < NT; ++n) colS[m][n] = s2_column_em(a.em, cs[m][n].c, cs[m][n].g);  // the column's S2 terms, once
+        }
     }
 #pragma unroll
-    for (int n = 0; n < NT; ++n) {
-      tot1[n] = fma(ci, col1[n], tot1[n]);
-      totS[n] = fma(ci, colS[n], totS[n]);
-    }
+    for (int m = 0; m < NS; ++m)
+#pragma unroll
+      for (int n = 0; n < NT; ++n) {
+        tot1[m][n] = fma(ci, col1[m][n], tot1[m][n]);
+        totS[m][n] = fma(ci, colS[m][n], totS[m][n]);
+      }
     __syncthreads();
   }
 
 #pragma unroll
-  for (int n = 0; n < NT; ++n)
-    if (t[n] < a.T)
-      a.part[((size_t)state * a.chunks + chunk) * a.T + t[n]] = a.dxdy * fma(sfac[n], totS[n], tot1[n]);
+  for (int m = 0; m < NS; ++m)
+    if (state0 + m < a.states) {
+#pragma unroll
+      for (int n = 0; n < NT; ++n)
+        if (t[n] < a.T)
+          a.part[((size_t)(state0 + m) * a.chunks + chunk) * a.T + t[n]] =
+              a.dxdy * fma(sfac[m][n], totS[m][n], tot1[m][n]);
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -267,26 +368,46 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
 constexpr int kMinB = SWS_MINB;
 constexpr int kMinCtaNodes = 32;  // a CTA walks at least this many source nodes
 
-size_t allpairs_smem_bytes(const PairPlan& p) {
-  return (size_t)kStages * p.seg_len * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
+size_t allpairs_smem_bytes(const PairPlan& p, int ns) {
+  return (size_t)kStages * p.seg_len * (ns * sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
 }
 
 // targets per thread of the FP64 kernel for this mesh (depends on the mesh only)
 int pair_nt(const sws_ctx* c) { return c->params.precision == 0 && c->mesh.T >= kNT2MinTargets ? 2 : 1; }
 
+// states per CTA of a launch with `states` states: 1 for a single evaluation; kBatchNS for a batch unless
+// sws_set_states_per_cta says otherwise.  Results do not depend on it (bitwise).  Measured on B200 (DESIGN.md
+// section 6, round 2): two states per CTA are 4.4-4.8 % SLOWER than one (721x241 b=16: 971 against 926 ms;
+// 361x121 b=32: 127.4 against 119.0; 181x61 b=16: 4.63 against 4.42) - sharing y_j and y_j - y* saves one DADD
+// and one LDS.64 of 28 + 3 per pair, the doubled register footprint (212 against 150, 148 against 114) costs
+// more - so the default stays 1.
+#ifndef SWS_BATCH_NS
+#define SWS_BATCH_NS 1
+#endif
+constexpr int kBatchNS = SWS_BATCH_NS;
+int pair_ns(const sws_ctx* c, int states) {
+  if (states < 2 || c->params.precision != 0) return 1;
+  const int want = c->ns_user > 0 ? c->ns_user : kBatchNS;
+  return want >= 2 ? 2 : 1;
+}
+
+template <int MINB, int NT, int NS>
+static cudaError_t configure_one(int* occ) {
+  const int smem_max = (int)(kStages * kSegMax * (NS * sizeof(SrcRec) + sizeof(double)) + 64);
+  const size_t smem_occ = kStages * kSegMax * (NS * sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
+  cudaError_t e = cudaFuncSetAttribute(k_allpairs<MINB, NT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, k_allpairs<MINB, NT, NS>, kThreads64, smem_occ);
+}
+
 cudaError_t allpairs_configure(const sws_ctx* c, int* occ_out) {
-  const int smem_max = (int)(kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + 64);
-  const size_t smem_occ = kStages * kSegMax * (sizeof(SrcRec) + sizeof(double)) + kStages * sizeof(uint64_t);
-  cudaError_t e = cudaFuncSetAttribute(k_allpairs<kMinB, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
-  if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(k_allpairs<kMinB2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+  int occ11 = 0, occ21 = 0, occ12 = 0, occ22 = 0;
+  cudaError_t e = configure_one<kMinB, 1, 1>(&occ11);
+  if (e == cudaSuccess) e = configure_one<kMinB2, 2, 1>(&occ21);
+  if (e == cudaSuccess) e = configure_one<kMinB12, 1, 2>(&occ12);
+  if (e == cudaSuccess) e = configure_one<kMinB22, 2, 2>(&occ22);
   if (e != cudaSuccess) return e;
-  int occ = 0;
-  if (pair_nt(c) == 2)
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_allpairs<kMinB2, 2>, kThreads64, smem_occ);
-  else
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_allpairs<kMinB, 1>, kThreads64, smem_occ);
-  if (e != cudaSuccess) return e;
+  const int occ = pair_nt(c) == 2 ? occ21 : occ11;  // the plan is made for the single-evaluation kernel (mesh only)
   *occ_out = occ > 0 ? occ : 1;
   return cudaSuccess;
 }
@@ -355,15 +476,18 @@ cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaSt
   PairArgs a;
   a.src = c->src; a.x = c->x; a.y = c->y; a.tgt = c->tgt; a.part = c->part;
   a.N = m.N; a.M = m.M; a.T = m.T;
+  a.states = states;
   a.chunks = plan.chunks; a.cols_per_chunk = plan.cols_per_chunk;
   a.seg_len = plan.seg_len; a.nseg = plan.nseg;
   a.dxdy = m.dx * m.dy;
   a.em = em_geometry(c);
-  dim3 grid(plan.tiles, plan.chunks, states);
-  if (pair_nt(c) == 2)
-    k_allpairs<kMinB2, 2><<<grid, kThreads64, allpairs_smem_bytes(plan), st>>>(a);
-  else
-    k_allpairs<kMinB, 1><<<grid, kThreads64, allpairs_smem_bytes(plan), st>>>(a);
+  const int ns = pair_ns(c, states), nt = pair_nt(c);
+  dim3 grid(plan.tiles, plan.chunks, (states + ns - 1) / ns);
+  const size_t smem = allpairs_smem_bytes(plan, ns);
+  if (nt == 2 && ns == 2) k_allpairs<kMinB22, 2, 2><<<grid, kThreads64, smem, st>>>(a);
+  else if (nt == 2) k_allpairs<kMinB2, 2, 1><<<grid, kThreads64, smem, st>>>(a);
+  else if (ns == 2) k_allpairs<kMinB12, 1, 2><<<grid, kThreads64, smem, st>>>(a);
+  else k_allpairs<kMinB, 1, 1><<<grid, kThreads64, smem, st>>>(a);
   return cudaGetLastError();
 }
 
@@ -407,71 +531,6 @@ cudaError_t launch_count_near(sws_ctx* c, int states, int* out, cudaStream_t st)
   dim3 grid((warps + 3) / 4, states);
   k_count_near<<<grid, 128, 0, st>>>(c->tgt, c->x, m.N, m.M, m.T, pair_nt(c), pair_cta_threads(c), warps,
                                      em_geometry(c).gmin, out);
-  return cudaGetLastError();
-}
-
-// --- unit-test hook of the far-field expansion ---------------------------------------------
-// out_em[i] = s2_column_em(c[i], g[i]); out_direct[i] = the plain trapezoid sum it stands for
-__global__ void k_debug_s2col(EmGeom e, int M, const double* c, const double* g, int n, double* out_direct,
-                              double* out_em) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  out_em[i] = s2_column_em(e, c[i], g[i]);
-  double acc = 0.0;
-  for (int j = 0; j < M; ++j) {
-    const double yj = e.y1 + j * sqrt(e.h2);
-    const double sm = yj - c[i], sp = yj + c[i];
-    const double v = rsqrt_fp64(fma(sm, sm, g[i])) + rsqrt_fp64(fma(sp, sp, g[i]));
-    acc += (j == 0 || j == M - 1) ? 0.5 * v : v;
-  }
-  out_direct[i] = acc;
-}
-
-// the three sums of the analytic Jacobian action: out[3 i + {0, 1, 2}] = {f0, f3, f3s}
-__global__ void k_debug_s2col3(EmGeom e, int M, const double* c, const double* g, int n, double* out_direct,
-                               double* out_em) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const Em3 r = s2_column_em3(e, c[i], g[i]);
-  out_em[3 * i] = r.f0; out_em[3 * i + 1] = r.f3; out_em[3 * i + 2] = r.f3s;
-  double a0 = 0.0, a3 = 0.0, a3s = 0.0;
-  for (int j = 0; j < M; ++j) {
-    const double yj = e.y1 + j * sqrt(e.h2);
-    const double sm = yj - c[i], sp = yj + c[i];
-    const double um = rsqrt_fp64(fma(sm, sm, g[i])), up = rsqrt_fp64(fma(sp, sp, g[i]));
-    const double um3 = um * um * um, up3 = up * up * up;
-    const double w = (j == 0 || j == M - 1) ? 0.5 : 1.0;
-    a0 += w * (um + up);
-    a3 += w * (um3 + up3);
-    a3s += w * (sm * um3 - sp * up3);
-  }
-  out_direct[3 * i] = a0; out_direct[3 * i + 1] = a3; out_direct[3 * i + 2] = a3s;
-}
-
-cudaError_t launch_debug_s2col3(double y1, double dy, int M, const double* c, const double* g, int n,
-                                double* out_direct, double* out_em, cudaStream_t st) {
-  EmGeom e;
-  e.y1 = y1; e.yM = y1 + (M - 1) * dy; e.h2 = dy * dy; e.inv_h = 1.0 / dy; e.gmin = 0.0; e.sym = (y1 == 0.0);
-  k_debug_s2col3<<<(n + 127) / 128, 128, 0, st>>>(e, M, c, g, n, out_direct, out_em);
-  return cudaGetLastError();
-}
-
-cudaError_t launch_debug_s2col(double y1, double dy, int M, const double* c, const double* g, int n,
-                               double* out_direct, double* out_em, cudaStream_t st) {
-  EmGeom e;
-  e.y1 = y1; e.yM = y1 + (M - 1) * dy; e.h2 = dy * dy; e.inv_h = 1.0 / dy; e.gmin = 0.0; e.sym = (y1 == 0.0);
-  k_debug_s2col<<<(n + 127) / 128, 128, 0, st>>>(e, M, c, g, n, out_direct, out_em);
-  return cudaGetLastError();
-}
-
-// --- unit-test hook for the reciprocal square root --------------------------------------
-__global__ void k_debug_rsqrt(const double* x, double* y, int n) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) y[i] = rsqrt_fp64(x[i]);
-}
-
-cudaError_t launch_debug_rsqrt(const double* x, double* y, int n, cudaStream_t st) {
-  k_debug_rsqrt<<<(n + 255) / 256, 256, 0, st>>>(x, y, n);
   return cudaGetLastError();
 }
 

@@ -12,13 +12,6 @@
 
 #include "sws_internal.cuh"
 
-namespace sws {
-cudaError_t launch_debug_rsqrt(const double* x, double* y, int n, cudaStream_t st);
-cudaError_t launch_fp64_probe(int blocks, int iters, double* sink, unsigned long long* clk,
-                              cudaStream_t st);
-cudaError_t launch_fp64_mix(int kind, int blocks, int iters, double* sink, unsigned long long* clk, cudaStream_t st);
-}  // namespace sws
-
 static thread_local char g_cuda_err[256] = "";
 
 static int cuda_fail(cudaError_t e, const char* where) {
@@ -31,6 +24,24 @@ static int cuda_fail(cudaError_t e, const char* where) {
     cudaError_t e_ = (call);                                  \
     if (e_ != cudaSuccess) return cuda_fail(e_, #call);       \
   } while (0)
+
+// Every entry point runs on the context's device and puts the caller's current device back on return
+// (a multi-GPU PyTorch process keeps its own notion of the current device).
+struct DevGuard {
+  int prev = -1;
+  cudaError_t err;
+  explicit DevGuard(int dev) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev);
+    else prev = -1;
+  }
+  ~DevGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+#define ON_DEVICE(dev)  \
+  DevGuard dev_guard_(dev); \
+  CK(dev_guard_.err)
 
 template <typename T>
 static cudaError_t dev_alloc(T** p, size_t count, size_t* total) {
@@ -64,7 +75,7 @@ const char* sws_strerror(int code) {
     case SWS_ENOMEM: return "out of memory";
     case SWS_ECUDA: return "CUDA runtime error (see sws_last_cuda_error)";
     case SWS_EBATCH: return "batch size out of range";
-    case SWS_ESTATE: return "no valid linearisation (call sws_linearize first)";
+    case SWS_ESTATE: return "no valid linearisation / evaluated state in the context (call sws_linearize, resp. sws_residual, first)";
     default: return "unknown error";
   }
 }
@@ -80,12 +91,13 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   if (p->precision != 0 && p->precision != 1) return SWS_EINVAL;
   if (p->max_batch < 0 || p->max_batch > 1024) return SWS_EINVAL;
   if ((long long)p->N * p->M > (1ll << 30)) return SWS_EINVAL;
+  if (p->M > 65535) return SWS_EINVAL;  // the O(NM) kernels put the y-line index on gridDim.y
   if (sws::reconstruct_smem_bytes(p->N) > 200 * 1024) return SWS_EINVAL;  // N <= 6400
 
   int ndev = 0;
   CK(cudaGetDeviceCount(&ndev));
   if (p->device < 0 || p->device >= ndev) return SWS_EINVAL;
-  CK(cudaSetDevice(p->device));
+  ON_DEVICE(p->device);
 
   sws_ctx* c = new (std::nothrow) sws_ctx();
   if (!c) return SWS_ENOMEM;
@@ -207,7 +219,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
 
 int sws_destroy(sws_ctx* c) {
   if (!c) return SWS_EINVAL;
-  cudaSetDevice(c->device);
+  ON_DEVICE(c->device);
   cudaDeviceSynchronize();
   free_all(c);
   delete c;
@@ -224,12 +236,33 @@ int sws_get_params(const sws_ctx* c, sws_params* out) {
   return SWS_OK;
 }
 
+int sws_get_fields_host(sws_ctx* c, double* zeta_host, double* phi_host, double* zeta_y_host, double* phi_y_host,
+                        void* cuda_stream) {
+  if (!c) return SWS_EINVAL;
+  if (c->last_states < 1) return SWS_ESTATE;
+  ON_DEVICE(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nb = (size_t)c->mesh.S * sizeof(double);  // state 0 of each plane, [l][k]
+  if (zeta_host) CK(cudaMemcpyAsync(zeta_host, c->zeta, nb, cudaMemcpyDeviceToHost, st));
+  if (phi_host) CK(cudaMemcpyAsync(phi_host, c->phi, nb, cudaMemcpyDeviceToHost, st));
+  if (zeta_y_host) CK(cudaMemcpyAsync(zeta_y_host, c->zy, nb, cudaMemcpyDeviceToHost, st));
+  if (phi_y_host) CK(cudaMemcpyAsync(phi_y_host, c->py, nb, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  return SWS_OK;
+}
+
 int sws_last_launch_count(const sws_ctx* c) { return c ? c->last_launches : 0; }
 
 int sws_set_tuning(sws_ctx* c, int32_t chunks) {
   if (!c || chunks < 0) return SWS_EINVAL;
   if (chunks > c->part_chunks) chunks = c->part_chunks;  // the partial-sum buffer is sized at setup
   c->chunks_user = chunks;
+  return SWS_OK;
+}
+
+int sws_set_states_per_cta(sws_ctx* c, int32_t ns) {
+  if (!c || ns < 0 || ns > 2) return SWS_EINVAL;
+  c->ns_user = ns;
   return SWS_OK;
 }
 
@@ -251,7 +284,7 @@ int sws_set_farfield(sws_ctx* c, double radius_in_dy) {
 int sws_farfield_stats(sws_ctx* c, int32_t states, double* near_fraction, void* cuda_stream) {
   if (!c || !near_fraction) return SWS_EINVAL;
   if (states < 1 || states > c->max_states || states > c->last_states) return SWS_EBATCH;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int warps = sws::count_near_warps(c);
   const size_t cnt = (size_t)states * warps;
@@ -309,7 +342,7 @@ static int run_states(sws_ctx* c, const double* u, const double* V, int states, 
 
 int sws_residual(sws_ctx* c, const double* u_dev, double* F_dev, void* cuda_stream) {
   if (!c || !u_dev || !F_dev) return SWS_EINVAL;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   int launches = 0;
   int rc = run_states(c, u_dev, nullptr, 1, F_dev, nullptr, (cudaStream_t)cuda_stream, &launches);
   c->last_launches = launches;
@@ -321,10 +354,12 @@ int sws_jv_batch(sws_ctx* c, const double* u_dev, const double* V_dev, int32_t b
                  void* cuda_stream) {
   if (!c || !u_dev || !V_dev || !JV_dev) return SWS_EINVAL;
   if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int launches = 0;
   if (sigma_host) {
+    for (int i = 0; i < b; ++i)  // 0 is allowed (a zero direction: JV row = 0); NaN / inf are not
+      if (!isfinite(sigma_host[i])) return SWS_EINVAL;
     CK(cudaMemcpyAsync(c->sigma, sigma_host, (size_t)b * sizeof(double), cudaMemcpyHostToDevice, st));
   } else {
     CK(sws::launch_sigma(c, u_dev, V_dev, b, st));
@@ -344,7 +379,7 @@ int sws_jv_exact_batch(sws_ctx* c, const double* u_dev, const double* V_dev, int
                        void* cuda_stream) {
   if (!c || !u_dev || !V_dev || !JV_dev) return SWS_EINVAL;
   if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
   const sws::PairPlan plan = sws::make_lin_plan(c, BT, groups, 0);
@@ -374,7 +409,7 @@ int sws_jv_exact_batch(sws_ctx* c, const double* u_dev, const double* V_dev, int
 int sws_linearize(sws_ctx* c, const double* u_dev, void* cuda_stream) {
   if (!c || !u_dev) return SWS_EINVAL;
   if (c->params.max_batch < 1) return SWS_EBATCH;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const sws::PairPlan plan = sws::make_lin_plan(c, 1, 1, 1);
   CK(sws::launch_reconstruct(c, u_dev, nullptr, 1, 1, c->F0, nullptr, st));
@@ -397,7 +432,7 @@ int sws_jv_apply(sws_ctx* c, const double* V_dev, int32_t b, double* JV_dev, voi
   if (!c || !V_dev || !JV_dev) return SWS_EINVAL;
   if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
   if (!c->lin_valid) return SWS_ESTATE;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
   const sws::PairPlan plan = sws::make_lin_plan(c, BT, groups, 2);
@@ -420,7 +455,7 @@ int sws_jv_exact_batch_host(sws_ctx* c, const double* u_host, const double* V_ho
                             double* JV_host, void* cuda_stream) {
   if (!c || !u_host || !V_host || !JV_host) return SWS_EINVAL;
   if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t nb = (size_t)c->mesh.n * sizeof(double);
   CK(cudaMemcpyAsync(c->u_stage, u_host, nb, cudaMemcpyHostToDevice, st));
@@ -435,7 +470,7 @@ int sws_jv_exact_batch_host(sws_ctx* c, const double* u_host, const double* V_ho
 int sws_time_allpairs_lin(sws_ctx* c, int32_t reps, float* ms_per_launch, void* cuda_stream) {
   if (!c || !ms_per_launch || reps < 1) return SWS_EINVAL;
   if (c->last_lin_b == 0) return SWS_EBATCH;  // needs the fields of a previous sws_jv_exact_batch / sws_jv_apply
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int mode = c->last_lin_b < 0 ? 2 : 0;
   const int b = c->last_lin_b < 0 ? -c->last_lin_b : c->last_lin_b, BT = sws::lin_tile(b), groups = (b + BT - 1) / BT;
@@ -463,7 +498,7 @@ int sws_lin_plan_info(sws_ctx* c, int32_t b, int32_t* out6) {
 
 int sws_residual_host(sws_ctx* c, const double* u_host, double* F_host, void* cuda_stream) {
   if (!c || !u_host || !F_host) return SWS_EINVAL;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t nb = (size_t)c->mesh.n * sizeof(double);
   CK(cudaMemcpyAsync(c->u_stage, u_host, nb, cudaMemcpyHostToDevice, st));
@@ -479,7 +514,7 @@ int sws_jv_batch_host(sws_ctx* c, const double* u_host, const double* V_host, in
                       double* F0_host, void* cuda_stream) {
   if (!c || !u_host || !V_host || !JV_host) return SWS_EINVAL;
   if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t n = c->mesh.n, nb = n * sizeof(double);
   CK(cudaMemcpyAsync(c->u_stage, u_host, nb, cudaMemcpyHostToDevice, st));
@@ -499,7 +534,7 @@ int sws_jv_batch_host(sws_ctx* c, const double* u_host, const double* V_host, in
 int sws_last_sigma(sws_ctx* c, int32_t b, double* sigma_host_out, void* cuda_stream) {
   if (!c || !sigma_host_out) return SWS_EINVAL;
   if (b < 1 || b > c->params.max_batch) return SWS_EBATCH;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CK(cudaMemcpyAsync(sigma_host_out, c->sigma, (size_t)b * sizeof(double), cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
@@ -510,7 +545,7 @@ int sws_time_allpairs(sws_ctx* c, int32_t states, int32_t reps, float* ms_per_la
                       void* cuda_stream) {
   if (!c || !ms_per_launch || reps < 1) return SWS_EINVAL;
   if (states < 1 || states > c->max_states || states > c->last_states) return SWS_EBATCH;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const sws::PairPlan plan = sws::make_plan(c);
   CK(sws::launch_allpairs(c, states, plan, st));  // warm-up
@@ -532,7 +567,7 @@ int sws_set_profiling(sws_ctx* c, int32_t on) {
 
 int sws_profile_read(sws_ctx* c, double* allpairs_ms, int32_t* launches, int32_t reset) {
   if (!c || !allpairs_ms || !launches) return SWS_EINVAL;
-  CK(cudaSetDevice(c->device));
+  ON_DEVICE(c->device);
   double tot = 0.0;
   for (size_t i = 0; i + 1 < c->prof_used; i += 2) {
     float ms = 0.f;
@@ -550,135 +585,6 @@ int sws_plan_info(sws_ctx* c, int32_t states, int32_t* out5) {
   if (!c || !out5 || states < 1 || states > c->max_states) return SWS_EINVAL;
   const sws::PairPlan p = sws::make_plan(c);
   out5[0] = p.tiles; out5[1] = p.chunks; out5[2] = p.cols_per_chunk; out5[3] = p.seg_len; out5[4] = p.nseg;
-  return SWS_OK;
-}
-
-int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, double* sm_mhz) {
-  if (!tflops) return SWS_EINVAL;
-  int ndev = 0;
-  CK(cudaGetDeviceCount(&ndev));
-  if (device < 0 || device >= ndev) return SWS_EINVAL;
-  CK(cudaSetDevice(device));
-  cudaDeviceProp prop;
-  CK(cudaGetDeviceProperties(&prop, device));
-  const int sms = prop.multiProcessorCount;
-  const int blocks = sms * 8, threads = 256, iters = 1 << 15;
-  double* sink = nullptr;
-  unsigned long long* clk = nullptr;
-  CK(cudaMalloc((void**)&sink, (size_t)blocks * threads * sizeof(double)));
-  CK(cudaMalloc((void**)&clk, 4 * sizeof(unsigned long long)));
-  cudaEvent_t e0, e1;
-  CK(cudaEventCreate(&e0));
-  CK(cudaEventCreate(&e1));
-  CK(sws::launch_fp64_probe(blocks, iters / 8, sink, clk, 0));  // warm-up
-  double best = 0.0, mhz = 0.0;
-  for (int rep = 0; rep < 3; ++rep) {
-    CK(cudaEventRecord(e0, 0));
-    CK(sws::launch_fp64_probe(blocks, iters, sink, clk, 0));
-    CK(cudaEventRecord(e1, 0));
-    CK(cudaEventSynchronize(e1));
-    float ms = 0.f;
-    CK(cudaEventElapsedTime(&ms, e0, e1));
-    unsigned long long h[4];
-    CK(cudaMemcpy(h, clk, sizeof h, cudaMemcpyDeviceToHost));
-    // 16 DFMA per iteration per thread, 2 flops each
-    const double fl = (double)blocks * threads * (double)iters * 16.0 * 2.0;
-    const double tf = fl / (ms * 1e-3) / 1e12;
-    if (tf > best) {
-      best = tf;
-      mhz = (h[3] > h[2]) ? (double)(h[1] - h[0]) / (double)(h[3] - h[2]) * 1e3 : 0.0;
-    }
-  }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(sink);
-  cudaFree(clk);
-  *tflops = best;
-  if (sm_count) *sm_count = sms;
-  if (sm_mhz) *sm_mhz = mhz;
-  return SWS_OK;
-}
-
-int sws_probe_fp64_mix(int32_t device, int32_t kind, int32_t warps_per_sm, double* fp64_instr_per_sm_clk,
-                       double* sm_mhz) {
-  if (!fp64_instr_per_sm_clk || kind < 0 || kind > 5) return SWS_EINVAL;
-  if (warps_per_sm < 8 || warps_per_sm > 64 || warps_per_sm % 8) return SWS_EINVAL;
-  int ndev = 0;
-  CK(cudaGetDeviceCount(&ndev));
-  if (device < 0 || device >= ndev) return SWS_EINVAL;
-  CK(cudaSetDevice(device));
-  cudaDeviceProp prop;
-  CK(cudaGetDeviceProperties(&prop, device));
-  const int sms = prop.multiProcessorCount;
-  const int blocks = sms * (warps_per_sm / 8), threads = 256, iters = 1 << 15;
-  static const int fp64_per_iter[6] = {12, 12, 12, 12, 13, 11};
-  double* sink = nullptr;
-  unsigned long long* clk = nullptr;
-  CK(cudaMalloc((void**)&sink, (size_t)blocks * threads * sizeof(double)));
-  CK(cudaMalloc((void**)&clk, 4 * sizeof(unsigned long long)));
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
-  cudaError_t e = cudaEventCreate(&e0);
-  if (e == cudaSuccess) e = cudaEventCreate(&e1);
-  if (e == cudaSuccess) e = sws::launch_fp64_mix(kind, blocks, iters / 8, sink, clk, 0);  // warm-up
-  double best = 0.0, mhz = 0.0;
-  for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {
-    e = cudaEventRecord(e0, 0);
-    if (e == cudaSuccess) e = sws::launch_fp64_mix(kind, blocks, iters, sink, clk, 0);
-    if (e == cudaSuccess) e = cudaEventRecord(e1, 0);
-    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
-    float ms = 0.f;
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
-    unsigned long long h[4] = {0, 0, 0, 0};
-    if (e == cudaSuccess) e = cudaMemcpy(h, clk, sizeof h, cudaMemcpyDeviceToHost);
-    if (e != cudaSuccess || h[1] <= h[0] || h[3] <= h[2] || ms <= 0.f) break;
-    // whole-launch time by CUDA events; SM clock during the loop from block 0's clock64 / globaltimer
-    const double clk_mhz = (double)(h[1] - h[0]) / (double)(h[3] - h[2]) * 1e3;
-    const double total = (double)fp64_per_iter[kind] * iters * threads * blocks;
-    const double rate = total / (ms * 1e-3 * clk_mhz * 1e6) / sms;
-    if (rate > best) { best = rate; mhz = clk_mhz; }
-  }
-  if (e0) cudaEventDestroy(e0);
-  if (e1) cudaEventDestroy(e1);
-  cudaFree(sink);
-  cudaFree(clk);
-  CK(e);
-  *fp64_instr_per_sm_clk = best;
-  if (sm_mhz) *sm_mhz = mhz;
-  return SWS_OK;
-}
-
-int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, int32_t n) {
-  if (!x_host || !y_host || n < 1) return SWS_EINVAL;
-  CK(cudaSetDevice(device));
-  double *x = nullptr, *y = nullptr;
-  CK(cudaMalloc((void**)&x, (size_t)n * 8));
-  CK(cudaMalloc((void**)&y, (size_t)n * 8));
-  CK(cudaMemcpy(x, x_host, (size_t)n * 8, cudaMemcpyHostToDevice));
-  CK(sws::launch_debug_rsqrt(x, y, n, 0));
-  CK(cudaMemcpy(y_host, y, (size_t)n * 8, cudaMemcpyDeviceToHost));
-  cudaFree(x);
-  cudaFree(y);
-  return SWS_OK;
-}
-
-int sws_debug_s2col_host(int32_t device, double y1, double dy, int32_t M, const double* c_host,
-                         const double* g_host, int32_t n, int32_t nsums, double* direct_host, double* em_host) {
-  if (!c_host || !g_host || !direct_host || !em_host || n < 1 || M < 2 || !(dy > 0.0)) return SWS_EINVAL;
-  if (nsums != 1 && nsums != 3) return SWS_EINVAL;
-  CK(cudaSetDevice(device));
-  double* d = nullptr;
-  const size_t nb = (size_t)n * 8, no = nb * nsums;
-  CK(cudaMalloc((void**)&d, 2 * nb + 2 * no));
-  CK(cudaMemcpy(d, c_host, nb, cudaMemcpyHostToDevice));
-  CK(cudaMemcpy(d + n, g_host, nb, cudaMemcpyHostToDevice));
-  double* od = d + 2 * (size_t)n;
-  double* oe = od + (size_t)n * nsums;
-  cudaError_t e = nsums == 1 ? sws::launch_debug_s2col(y1, dy, M, d, d + n, n, od, oe, 0)
-                             : sws::launch_debug_s2col3(y1, dy, M, d, d + n, n, od, oe, 0);
-  if (e == cudaSuccess) e = cudaMemcpy(direct_host, od, no, cudaMemcpyDeviceToHost);
-  if (e == cudaSuccess) e = cudaMemcpy(em_host, oe, no, cudaMemcpyDeviceToHost);
-  cudaFree(d);
-  CK(e);
   return SWS_OK;
 }
 

@@ -21,9 +21,21 @@ namespace sws {
 // here is written with at most two distinct registers: the last one is
 // y0 + y0 * (e p) = fma(y0, e p, y0), not fma(y0 e, p, y0).
 __device__ __forceinline__ double rsqrt_seed(double x) {
+#ifdef SWS_RSQRT_F32SEED
+  // Experiment of round 2: FP32 seed, cvt + MUFU.RSQ + cvt instead of MUFU.RSQ64H + the
+  // move that zeroes its low word.  Measured slower at 721x241: 59.9 against 54.5 ms per launch (the two F2F
+  // conversions cost more issue than the move they save); kept behind this build flag for the record, off.
+  float xf, yf;
+  asm("cvt.rn.f32.f64 %0, %1;" : "=f"(xf) : "d"(x));
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(yf) : "f"(xf));
+  double y;
+  asm("cvt.f64.f32 %0, %1;" : "=d"(y) : "f"(yf));
+  return y;
+#else
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   return y;
+#endif
 }
 
 __device__ __forceinline__ double rsqrt_fp64(double x) {
@@ -52,7 +64,9 @@ __device__ __forceinline__ double rsqrt_fp64(double x) {
 // With K = 7 and r = 8 the remainder is < 1e-16 / sqrt(g) (measured against 50-digit sums over
 // the whole range of c), below the rounding of the direct sum itself.
 // The same quantity, evaluated another way: the result still matches the oracle's plain sum.
-// Cost: ~120 FP64 instructions per (target, column) instead of 16 per pair.
+// Cost: 216 FP64 instructions per (target, column) in SASS (y1 = 0 form: 100 DFMA + 93 DMUL + 23 DADD = 2 x 59 for
+// the end-point tails, the rest one log1p and two divisions; counted with cuobjdump) instead of 16 per pair
+// x M pairs: 0.9 per pair at M = 241.
 // (default r = kEmRadius of sws_internal.cuh; sws_set_farfield changes it, r <= 0 sums directly)
 
 // sum_{k=1..7} (B_2k / 2k) s^k P_{2k-1}(mu) at the end point u = y_e - c;  *rho = sqrt(u^2 + g)

@@ -369,7 +369,8 @@ __global__ void k_sigma(const double* __restrict__ part, int nblk, int b, double
   double su = 0.0, sv = 0.0;
   for (int i = 0; i < nblk; ++i) su += part[i];
   for (int i = 0; i < nblk; ++i) sv += part[(size_t)(r + 1) * nblk + i];
-  sigma[r] = 1e-7 * (1.0 + sqrt(su)) / sqrt(sv);
+  // v_b = 0: sigma_b = 0 marks the direction; u_b = u and k_quotient writes the exact row J 0 = 0
+  sigma[r] = sv > 0.0 ? 1e-7 * (1.0 + sqrt(su)) / sqrt(sv) : 0.0;
 }
 
 // eq. (25): JV_b = (E(u_b) - E(u)) / sigma_b
@@ -380,7 +381,7 @@ __global__ void __launch_bounds__(256) k_quotient(const double* __restrict__ F0,
   const double sg = sigma[b];
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)n;
        i += (size_t)gridDim.x * blockDim.x)
-    JV[(size_t)b * n + i] = (Fpert[(size_t)b * n + i] - F0[i]) / sg;
+    JV[(size_t)b * n + i] = sg != 0.0 ? (Fpert[(size_t)b * n + i] - F0[i]) / sg : 0.0;
 }
 
 // ---------------------------------------------------------------------------------------

@@ -74,6 +74,7 @@ struct sws_ctx {
   int sm_count;
   int max_states;       // max_batch + 1
   int chunks_user;      // 0 = auto
+  int ns_user;          // states per CTA of batched all-pairs launches: 0 = library default, 1, 2
   double em_radius;     // far-field radius r of the S2 column sums in units of dy (<= 0: all direct)
   size_t ws_bytes;
   int last_launches;
@@ -143,10 +144,6 @@ cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, do
 // dispatches on sws_params.precision (0: FP64 kernel, 1: FP32 pair arithmetic)
 cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
 cudaError_t launch_count_near(sws_ctx* c, int states, int* out, cudaStream_t st);
-cudaError_t launch_debug_s2col(double y1, double dy, int M, const double* cc, const double* g, int n,
-                               double* out_direct, double* out_em, cudaStream_t st);
-cudaError_t launch_debug_s2col3(double y1, double dy, int M, const double* cc, const double* g, int n,
-                                double* out_direct, double* out_em, cudaStream_t st);
 cudaError_t launch_allpairs_f32(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
 cudaError_t launch_assemble(sws_ctx* c, int states, const PairPlan& plan, double* F0,
                             double* Fpert, cudaStream_t st);
@@ -168,7 +165,8 @@ cudaError_t launch_assemble_lin(sws_ctx* c, int b, int BT, int mode, const PairP
 
 PairPlan make_plan(const sws_ctx* c);
 int max_chunks(const sws_ctx* c);
-size_t allpairs_smem_bytes(const PairPlan& p);
+size_t allpairs_smem_bytes(const PairPlan& p, int ns);
+int pair_ns(const sws_ctx* c, int states);
 cudaError_t allpairs_configure(const sws_ctx* c, int* occ_out);
 int pair_nt(const sws_ctx* c);
 int count_near_warps(const sws_ctx* c);

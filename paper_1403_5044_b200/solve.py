@@ -7,8 +7,8 @@ Builds the block-banded linear-Jacobian preconditioner (section 4.2, App. B/C), 
 Newton-GMRES iteration (section 4.1) from the flat surface (L227) - through the given source strengths in turn
 when --continuation is used (L229) - and writes the free surface zeta(x, y), the potential phi(x, y) and the
 unknown vector u (eq. (18)) to an .npz file.  Everything numerical runs in libsws / libsws_jfnk on the GPU; this
-file only parses arguments, rebuilds zeta and phi from u by the trapezoid rule (19) for the output, and prints
-the Newton log.  There is no CPU fallback.
+file only parses arguments, reads the nodal planes zeta, phi back from the library (sws_get_fields_host) and
+prints the Newton log.  There is no CPU fallback.
 """
 from __future__ import annotations
 
@@ -17,17 +17,6 @@ import json
 import time
 
 import numpy as np
-
-
-def fields_from_u(u: np.ndarray, N: int, M: int, dx: float):
-    """zeta, phi on the N x M nodes ([l][k]) from the unknowns, eq. (18) L149 and eq. (19) L156."""
-    half = (N + 1) * M
-    out = []
-    for blk in (u[half:], u[:half]):
-        b = blk.reshape(M, N + 1)
-        f1, fx = b[:, :1], b[:, 1:]
-        out.append(np.concatenate([f1, f1 + np.cumsum(0.5 * dx * (fx[:, 1:] + fx[:, :-1]), axis=1)], axis=1))
-    return out[0], out[1]
 
 
 def main(argv=None) -> int:
@@ -77,8 +66,8 @@ def main(argv=None) -> int:
         t2 = time.perf_counter()
         F = ctx.residual(u)
         res = float(F.abs().max())
+        zeta, phi, _, _ = ctx.fields_host()      # the nodal planes of the state sws_residual just evaluated
     u = u.cpu().numpy()
-    zeta, phi = fields_from_u(u, a.N, a.M, a.h)
     report = {"mesh": f"{a.N}x{a.M}", "h": a.h, "froude": a.froude, "eps_reached": stages[done - 1] if done else None,
               "converged": done == len(stages), "stages": [dict(eps=e, steps=st["steps"], jv_products=st["jv_products"],
                                                                 residual_evals=st["residual_evals"],

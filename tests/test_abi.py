@@ -36,6 +36,18 @@ def test_header_symbols_exported(sws):
     assert sorted(sws.SYMBOLS) == names, "binding's SYMBOLS list and sws.h disagree"
 
 
+def test_debug_header_symbols_exported(sws):
+    """libsws_debug.so (test hooks + probes) exports what sws_debug.h declares; the product library has none of them."""
+    from paper_1403_5044_b200 import debug
+    lib = debug.load_debug_library()
+    names = declared_functions(ROOT / "include" / "sws_debug.h")
+    assert sorted(names) == sorted(debug.SYMBOLS)
+    prod = sws.load_library()
+    for n in names:
+        assert hasattr(lib, n)
+        assert not hasattr(prod, n), f"{n} leaked into the product library"
+
+
 def test_jfnk_header_symbols_exported(sws):
     """libsws_jfnk.so (Newton-Krylov driver) loads without a GPU and exports what sws_jfnk.h declares."""
     import paper_1403_5044_b200.jfnk as jf

@@ -50,7 +50,8 @@ def test_rsqrt_primitive(sws):
         np.nextafter(2.0 ** np.arange(-20, 20, dtype=np.float64), 0),  # just below powers of two
         2.0 ** np.arange(-20, 20, dtype=np.float64),
     ])
-    y = sws.debug_rsqrt(x)
+    from paper_1403_5044_b200 import debug
+    y = debug.debug_rsqrt(x)
     ref = 1.0 / np.sqrt(x.astype(np.longdouble))
     rel = np.abs((y.astype(np.longdouble) - ref) / ref).astype(np.float64)
     assert rel.max() <= 2.0 ** -52, rel.max()
@@ -201,6 +202,34 @@ def test_chunking_invariance_and_determinism(sws, oracle80):
         torch.cuda.synchronize()
 
 
+@pytest.mark.parametrize("name,b", [("cfg3", 5), ("cfg4", 3), ("steep", 4)])
+def test_states_per_cta_is_bitwise_invisible(sws, name, b):
+    """sws_set_states_per_cta: two states per CTA (the y_j run staged once, y_j - y* formed once for both) give
+    bit for bit the batch of one state per CTA - odd state counts (ragged last group), the two-target kernel
+    (cfg4) and a steep state with LARGE shifts, where a column can be far for one state of a CTA and near for
+    the other (the kernel then walks it state by state)."""
+    if name == "steep":
+        cfg = W.custom(eps=0.5, amp=1.5, N=120, M=50, h=0.15, x1=-2.0, seed=22)
+        sigma = [3e-2, 1e-7, 5e-2, 2e-2]
+    else:
+        cfg = W.CONFIGS[2 if name == "cfg3" else 3]
+        sigma = None
+    u, V = dev(W.state(cfg)), dev(W.directions(cfg, b))
+    with sws.Context(cfg.params(), max_batch=b) as ctx:
+        out = {}
+        for ns in (1, 2, 0):
+            ctx.set_states_per_cta(ns)
+            JV, Fp, F0 = ctx.jv_batch(u, V, sigma=sigma, want_fpert=True, want_f0=True)
+            out[ns] = (JV.cpu().numpy(), Fp.cpu().numpy(), F0.cpu().numpy())
+        with pytest.raises(sws.SwsError):
+            ctx.set_states_per_cta(3)
+    for ns in (2, 0):
+        for a, r in zip(out[ns], out[1]):
+            assert np.isfinite(a).all() and np.array_equal(a, r)
+    if name == "steep":
+        assert np.abs(out[1][1][0] - out[1][2]).max() > 1e-4    # the shifts really moved the states
+
+
 def _column_sum_longdouble(y1, dy, M, c, g):
     """sum_j c_j [((y_j-c)^2+g)^-1/2 + ((y_j+c)^2+g)^-1/2], c_j = 1/2 at both ends, term by term."""
     y = (np.longdouble(y1) + np.arange(M, dtype=np.longdouble) * np.longdouble(dy))[None, :]
@@ -224,7 +253,8 @@ def test_farfield_expansion_primitive(sws, y1, dy, M):
     c = np.concatenate([rng.uniform(-yM - 5, yM + 5, n - 6), [y1, yM, -yM, 0.0, 0.5 * (y1 + yM), yM + 40.0]])
     r = np.concatenate([np.full(n // 4, 8.0), rng.uniform(8.0, 12.0, n // 4), 10 ** rng.uniform(0.9, 2.9, n - 2 * (n // 4))])
     g = (r * dy) ** 2
-    direct, em = sws.debug_s2col(y1, dy, M, c, g)
+    from paper_1403_5044_b200 import debug
+    direct, em = debug.debug_s2col(y1, dy, M, c, g)
     ref = _column_sum_longdouble(y1, dy, M, c, g)
     scale = np.maximum(np.abs(ref), 1.0 / (r * dy) / dy).astype(np.float64)
     err_em = np.abs((em.astype(np.longdouble) - ref).astype(np.float64)) / scale
@@ -243,7 +273,8 @@ def test_farfield_expansion_three_sums(sws, y1, dy, M):
     c = np.concatenate([rng.uniform(-yM - 5, yM + 5, n - 5), [y1, yM, -yM, 0.0, 0.5 * (y1 + yM)]])
     r = np.concatenate([np.full(n // 3, 8.0), rng.uniform(8.0, 12.0, n // 3), 10 ** rng.uniform(0.9, 2.5, n - 2 * (n // 3))])
     g = (r * dy) ** 2
-    direct, em = sws.debug_s2col(y1, dy, M, c, g, nsums=3)
+    from paper_1403_5044_b200 import debug
+    direct, em = debug.debug_s2col(y1, dy, M, c, g, nsums=3)
     L = np.longdouble
     y = (L(y1) + np.arange(M, dtype=L) * L(dy))[None, :]
     cc, gg = c.astype(L)[:, None], g.astype(L)[:, None]
@@ -338,7 +369,7 @@ def test_large_configs_sampled_rows(sws, oracle80, i, rows):
     mask = ~np.isnan(E)
     assert mask.sum() == (cfg.N + 1) * cfg.M + 2 * cfg.M + pick.size
     assert np.isfinite(F).all()
-    scale = np.abs(F).max()
+    scale = np.abs(E[mask]).max()          # the ORACLE's |F|_inf over what it computed (<= the full norm: stricter)
     assert np.abs(F[mask] - E[mask]).max() / scale <= TOL
 
 
@@ -398,7 +429,10 @@ def test_jv_batch_cfg5_bench_configuration(sws, oracle80):
         F = ctx.residual(ud).cpu().numpy()
         Fp, F0, JV = Fp.cpu().numpy(), F0.cpu().numpy(), JV.cpu().numpy()
     assert np.array_equal(F0, F)
-    scale = np.abs(F).max()
+    E0 = oracle80.residual(p, u, rows=pick)
+    m0 = ~np.isnan(E0)
+    scale = np.abs(E0[m0]).max()           # the oracle's |F(u)|_inf over the rows it computed
+    assert np.abs(F[m0] - E0[m0]).max() / scale <= TOL
     for k in (0, b - 1):
         s_ref = oracle80.sigma(u, V[k])
         assert abs(sig[k] - s_ref) <= 1e-13 * s_ref
@@ -407,6 +441,51 @@ def test_jv_batch_cfg5_bench_configuration(sws, oracle80):
         assert mask.sum() >= (cfg.N + 1) * cfg.M + pick.size
         assert np.abs(Fp[k][mask] - Ep[mask]).max() / scale <= TOL
         assert np.array_equal(JV[k], (Fp[k] - F0) / sig[k])
+
+
+def test_jv_batch_cfg4_b32(sws, oracle80):
+    """BASELINE.json config 4 in FP64: 361x121, single F(u) and the b = 32 finite-difference batch (33 states in
+    one all-pairs launch of the two-targets-per-thread kernel).  F(u) and the perturbed residuals of the first
+    and last direction on seeded rows the oracle computes one by one, at the library's own shifts, to 1e-10 of
+    the oracle's |F|_inf; one slot bitwise against sws_residual(fma(sigma, v, u)); a zero direction gives a
+    zero row (J 0 = 0), not NaN."""
+    import torch
+    cfg = W.CONFIGS[3]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg)
+    b = V.shape[0]
+    assert (cfg.N, cfg.M, b) == (361, 121, 32)
+    rng = np.random.default_rng(78)
+    T = cfg.targets
+    pick = np.unique(np.concatenate([rng.integers(0, T, 768), [0, T - 1, cfg.N - 2]])).astype(np.int32)
+    V = V.copy()
+    V[7] = 0.0                                  # ADVICE r1: sigma = 1e-7 (1 + |u|) / |v| must not poison the batch
+    with sws.Context(p, max_batch=b) as ctx:
+        ud, Vd = dev(u), dev(V)
+        JV, Fp, F0 = ctx.jv_batch(ud, Vd, want_fpert=True, want_f0=True)
+        torch.cuda.synchronize()
+        sig = ctx.last_sigma(b)
+        F = ctx.residual(ud).cpu().numpy()
+        Fp, F0, JV = Fp.cpu().numpy(), F0.cpu().numpy(), JV.cpu().numpy()
+        k_bit = 19
+        from fractions import Fraction      # exact product and sum, ONE rounding: what fma(sigma, v, u) returns
+        sg = Fraction(float(sig[k_bit]))
+        ub = np.array([float(sg * Fraction(float(vv)) + Fraction(float(uu))) for uu, vv in zip(u, V[k_bit])])
+        F_bit = ctx.residual(dev(ub)).cpu().numpy()
+    assert np.array_equal(F0, F)
+    assert np.array_equal(Fp[k_bit], F_bit)
+    E0 = oracle80.residual(p, u, rows=pick)
+    m0 = ~np.isnan(E0)
+    scale = np.abs(E0[m0]).max()
+    assert np.abs(F[m0] - E0[m0]).max() / scale <= TOL
+    for k in (0, b - 1):
+        s_ref = oracle80.sigma(u, V[k])
+        assert abs(sig[k] - s_ref) <= 1e-13 * s_ref
+        _, Ep = oracle80.jv(p, u, V[k], float(sig[k]), rows=pick)
+        mask = ~np.isnan(Ep)
+        assert np.abs(Fp[k][mask] - Ep[mask]).max() / scale <= TOL
+        assert np.array_equal(JV[k], (Fp[k] - F0) / sig[k])
+    assert np.isfinite(JV).all() and np.isfinite(Fp).all()
+    assert not JV[7].any() and np.array_equal(Fp[7], F0)
 
 
 def test_host_api_matches_device_api(sws):
@@ -458,6 +537,51 @@ def test_error_codes(sws):
             ctx.jv_batch(u, V)
         with pytest.raises(sws.SwsError):
             ctx.residual(u[:-1])
+        with pytest.raises(sws.SwsError, match="invalid"):     # NaN / inf shifts are refused, 0 is a zero direction
+            ctx.jv_batch(u, V[:2].contiguous(), sigma=[1e-7, float("nan")])
+        with pytest.raises(sws.SwsError, match="invalid"):
+            ctx.jv_batch(u, V[:2].contiguous(), sigma=[float("inf"), 1e-7])
+    with pytest.raises(sws.SwsError, match="invalid"):
+        sws.Context(dict(p, N=3, M=70000))  # M rides gridDim.y of the O(NM) kernels: refused at set-up, not at launch
+    with sws.Context(p) as ctx:
+        with pytest.raises(sws.SwsError):
+            ctx.fields_host()                # nothing evaluated yet
+
+
+def test_zero_direction_and_zero_shift(sws):
+    """A zero row of V (sigma = 1e-7 (1 + |u|) / 0) and a caller's sigma = 0 both give the exact row J 0 = 0 and
+    E(u_b) = E(u) bitwise, never NaN; the other rows are untouched."""
+    cfg = W.CONFIGS[1]
+    p, u, V = cfg.params(), W.state(cfg), W.directions(cfg, 4).copy()
+    with sws.Context(p, max_batch=4) as ctx:
+        JV_ref, Fp_ref, F0_ref = [t.cpu().numpy() for t in ctx.jv_batch(dev(u), dev(V), want_fpert=True, want_f0=True)]
+        sig_ref = ctx.last_sigma(4)
+        V[2] = 0.0
+        JV, Fp, F0 = [t.cpu().numpy() for t in ctx.jv_batch(dev(u), dev(V), want_fpert=True, want_f0=True)]
+        sig = ctx.last_sigma(4)
+        assert sig[2] == 0.0 and np.array_equal(np.delete(sig, 2), np.delete(sig_ref, 2))
+        assert np.isfinite(JV).all() and not JV[2].any() and np.array_equal(Fp[2], F0)
+        for k in (0, 1, 3):
+            assert np.array_equal(JV[k], JV_ref[k]) and np.array_equal(Fp[k], Fp_ref[k])
+        assert np.array_equal(F0, F0_ref)
+        s2 = sig_ref.copy()
+        s2[1] = 0.0
+        JV2 = ctx.jv_batch(dev(u), dev(W.directions(cfg, 4)), sigma=s2).cpu().numpy()
+        assert not JV2[1].any() and np.array_equal(JV2[0], JV_ref[0])
+
+
+def test_fields_host_matches_oracle(sws, oracle80):
+    """sws_get_fields_host: the nodal planes of steps a1, a2 as the library holds them, against the oracle's."""
+    cfg = W.custom(37, 9, 0.4, -3.0, y1=0.6, seed=5, amp=0.1)
+    u = W.state(cfg) + 1e-3 * np.random.default_rng(2).standard_normal(cfg.n)
+    for scheme in (0, 1):
+        ref = oracle80.fields(cfg.params(scheme), u)
+        with sws.Context(cfg.params(scheme)) as ctx:
+            ctx.residual(dev(u))
+            got = ctx.fields_host()
+        for g, r in zip(got, ref):
+            assert g.shape == r.shape == (cfg.M, cfg.N)
+            assert np.abs(g - r).max() <= 1e-13 * max(1.0, np.abs(r).max())
 
 
 # ---------------------------------------------------------------------------------------
