@@ -161,6 +161,17 @@ int sws_last_launch_count(const sws_ctx* ctx);
 int sws_time_allpairs(sws_ctx* ctx, int32_t states, int32_t reps, float* ms_per_launch,
                       void* cuda_stream);
 
+/* Time (ms per call, CUDA events on `cuda_stream`) of `reps` back-to-back sws_residual calls issued from
+ * inside the library (no binding overhead between the calls): what a compiled driver such as
+ * libsws_jfnk sees on small meshes, where an evaluation takes tens of microseconds.  Synchronises. */
+int sws_time_residual(sws_ctx* ctx, const double* u_dev, double* F_dev, int32_t reps, float* ms_per_call,
+                      void* cuda_stream);
+
+/* Steps a0-a3, a5-a8 run as ONE cooperative launch on meshes of up to 2^17 nodes (three phases separated by
+ * grid-wide barriers) and as three launches above that.  on = 0 forces the three launches; on != 0 restores
+ * the default choice.  Results do not depend on it (the phases call the same device functions). */
+int sws_set_fused_fields(sws_ctx* ctx, int32_t on);
+
 /* The same for the all-pairs kernel of sws_jv_exact_batch, with the fields and the batch size
  * of the previous sws_jv_exact_batch call (SWS_EBATCH if there was none). */
 int sws_time_allpairs_lin(sws_ctx* ctx, int32_t reps, float* ms_per_launch, void* cuda_stream);

@@ -26,7 +26,7 @@ SYMBOLS = (
     "sws_plan_info", "sws_set_profiling", "sws_profile_read", "sws_destroy", "sws_strerror", "sws_last_cuda_error",
     "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
     "sws_get_params", "sws_linearize", "sws_jv_apply",
-    "sws_set_farfield", "sws_farfield_stats", "sws_set_eps", "sws_get_fields_host", "sws_set_states_per_cta",
+    "sws_set_farfield", "sws_farfield_stats", "sws_set_eps", "sws_get_fields_host", "sws_set_states_per_cta", "sws_time_residual", "sws_set_fused_fields",
 )
 
 
@@ -86,6 +86,8 @@ def load_library() -> C.CDLL:
         "sws_set_farfield": (C.c_int, [vp, C.c_double]),
         "sws_set_eps": (C.c_int, [vp, C.c_double]),
         "sws_set_states_per_cta": (C.c_int, [vp, C.c_int32]),
+        "sws_time_residual": (C.c_int, [vp, dp, dp, C.c_int32, C.POINTER(C.c_float), vp]),
+        "sws_set_fused_fields": (C.c_int, [vp, C.c_int32]),
         "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
     }
     for name, (res, args) in proto.items():
@@ -285,6 +287,17 @@ class Context:
         _check(self.lib.sws_time_allpairs(self._h, int(states), int(reps), C.byref(ms),
                                           self._stream(stream)), "sws_time_allpairs")
         return float(ms.value)
+
+    def time_residual(self, u, F, reps: int = 20, stream=None) -> float:
+        """ms per sws_residual call, `reps` calls issued back to back inside the library (sws_time_residual)."""
+        ms = C.c_float()
+        _check(self.lib.sws_time_residual(self._h, self._dev(u, (self.n,), "u"), self._dev(F, (self.n,), "F"),
+                                          int(reps), C.byref(ms), self._stream(stream)), "sws_time_residual")
+        return float(ms.value)
+
+    def set_fused_fields(self, on: bool = True) -> None:
+        """sws_set_fused_fields: one cooperative launch (default on small meshes) or three for the O(NM) stages."""
+        _check(self.lib.sws_set_fused_fields(self._h, int(bool(on))), "sws_set_fused_fields")
 
     def time_allpairs_lin(self, reps: int = 1, stream=None) -> float:
         """ms per launch of the analytic-Jv all-pairs kernel alone (after a jv_exact_batch call)."""

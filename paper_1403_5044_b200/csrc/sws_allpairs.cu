@@ -19,6 +19,7 @@
 // applied by peeling the first/last node and scaling edge columns, so the inner loop carries no
 // weight multiply.  Partial sums per (state, chunk, target) are written to global memory and
 // added in a fixed order by the assemble kernel: no atomics, bitwise repeatable.
+#include "sws_closed_form.cuh"
 #include "sws_farfield.cuh"
 #include "sws_internal.cuh"
 #include "sws_stage.cuh"
@@ -189,7 +190,59 @@ struct PairArgs {
   int chunks, cols_per_chunk, seg_len, nseg;
   double dxdy;
   EmGeom em;
+  // fused assembly (a6 + a9), tile_count != NULL: the CTA that completes a (state, target tile) - the last of
+  // its `chunks` column groups to arrive - adds the partial sums in the fixed order c = 0 .. chunks-1 and writes
+  // E2 = e2loc - sum into the residual; no separate assemble launch, still no floating-point atomics
+  unsigned int* tile_count;  // [state][tiles], zero between launches
+  double* e2loc;             // [state][T], written by CTA row 0 of this launch (a5 + a6 local part)
+  double eps;
+  double* F0;                // [n] residual of state 0
+  double* Fpert;             // [states - 1][n]
+  int n;
 };
+
+// Fused assembly, a6 + a9.  Every CTA of a (state, target tile) - its `chunks` column groups and the local row -
+// counts itself in after its stores are visible; the last one adds the partial sums in the fixed order
+// c = 0 .. chunks-1 (the sum and order of k_assemble) and writes E2 = e2loc - sum.
+template <int NT, int NS>
+__device__ __forceinline__ void arrive_and_assemble(const PairArgs& a, const int (&t)[NT], const int tile,
+                                                    const int state0) {
+  const int tid = threadIdx.x;
+  __shared__ int s_last[NS];
+  __threadfence();  // this thread's stores are visible device-wide ...
+  __syncthreads();  // ... for every thread of the CTA, before the CTA counts itself in
+  if (tid == 0) {
+#pragma unroll
+    for (int m = 0; m < NS; ++m) {
+      s_last[m] = 0;
+      if (state0 + m < a.states) {
+        unsigned int* cnt = a.tile_count + (size_t)(state0 + m) * gridDim.x + tile;
+        const unsigned int seen = atomicAdd(cnt, 1u);
+        if (seen == (unsigned int)gridDim.y - 1u) {
+          s_last[m] = 1;
+          *cnt = 0u;  // ready for the next launch
+        }
+      }
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int m = 0; m < NS; ++m) {
+    if (!s_last[m]) continue;
+    __threadfence();
+    const int state = state0 + m;
+    double* F = state == 0 ? a.F0 : a.Fpert + (size_t)(state - 1) * a.n;
+#pragma unroll
+    for (int n = 0; n < NT; ++n) {
+      if (t[n] >= a.T) continue;
+      const double* p = a.part + (size_t)state * a.chunks * a.T + t[n];
+      double sum = 0.0;
+      for (int c = 0; c < a.chunks; ++c) sum += __ldcg(p + (size_t)c * a.T);
+      const int l = t[n] / (a.N - 1), k = t[n] - l * (a.N - 1);
+      F[(size_t)(a.N + 1) * a.M + (size_t)l * (a.N + 1) + 2 + k] = __ldcg(a.e2loc + (size_t)state * a.T + t[n]) - sum;
+    }
+  }
+}
 
 // NS = states per CTA.  NS = 1 is the single evaluation; NS = 2 is the batched mode of sws_jv_batch: the CTA
 // stages the y_j run once and one record run per state, and a thread forms y_j - y* once for its NS states.
@@ -205,7 +258,9 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
   uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_y + (size_t)kStages * seg_pad);       // [kStages]
 
   const int tid = threadIdx.x;
-  const int tile = blockIdx.x, chunk = blockIdx.y, state0 = blockIdx.z * NS;
+  // With fused assembly (tile_count != NULL) CTA row y = 0 is the LOCAL row: it evaluates a5 + a6's local part
+  // (the closed form I: 8 asinh per target) for the tile while the other rows walk their column groups.
+  const int tile = blockIdx.x, chunk = (int)blockIdx.y - (a.tile_count ? 1 : 0), state0 = blockIdx.z * NS;
   int st[NS];  // the states of this CTA; a ragged last group recomputes the last state and stores nothing
 #pragma unroll
   for (int m = 0; m < NS; ++m) st[m] = state0 + m < a.states ? state0 + m : a.states - 1;
@@ -235,6 +290,22 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
       kg[m][n] = tr.A / tr.C - kb[m][n] * kb[m][n];      // (4AC - B^2) / (4 C^2)
       sfac[m][n] = -tr.zxs * rsqrt_fp64(tr.C);
     }
+  }
+
+  if (chunk < 0) {  // the local row
+    const double xa = __ldg(a.x), xb = __ldg(a.x + a.N - 1), ya = __ldg(a.y), yb = __ldg(a.y + a.M - 1);
+#pragma unroll
+    for (int m = 0; m < NS; ++m) {
+      if (state0 + m >= a.states) continue;
+#pragma unroll
+      for (int n = 0; n < NT; ++n)
+        if (t[n] < a.T) {
+          const size_t ts_ = (size_t)(state0 + m) * a.T + t[n];
+          a.e2loc[ts_] = e2_local(a.tgt[ts_], a.eps, xa, xb, ya, yb);
+        }
+    }
+    arrive_and_assemble<NT, NS>(a, t, tile, state0);
+    return;
   }
 
   const int c0 = chunk * a.cols_per_chunk;
@@ -360,6 +431,8 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
           a.part[((size_t)(state0 + m) * a.chunks + chunk) * a.T + t[n]] =
               a.dxdy * fma(sfac[m][n], totS[m][n], tot1[m][n]);
     }
+
+  if (a.tile_count != nullptr) arrive_and_assemble<NT, NS>(a, t, tile, state0);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -470,7 +543,7 @@ int max_chunks(const sws_ctx* c) {
   return cmax;
 }
 
-cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st) {
+cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st, double* F0, double* Fpert) {
   if (c->params.precision == 1) return launch_allpairs_f32(c, states, plan, st);
   const Mesh& m = c->mesh;
   PairArgs a;
@@ -481,8 +554,10 @@ cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaSt
   a.seg_len = plan.seg_len; a.nseg = plan.nseg;
   a.dxdy = m.dx * m.dy;
   a.em = em_geometry(c);
+  a.tile_count = F0 ? c->tile_count : nullptr;  // F0 given: the kernel also assembles E2 (no k_assemble launch)
+  a.e2loc = c->e2loc; a.eps = m.eps; a.F0 = F0; a.Fpert = Fpert; a.n = m.n;
   const int ns = pair_ns(c, states), nt = pair_nt(c);
-  dim3 grid(plan.tiles, plan.chunks, (states + ns - 1) / ns);
+  dim3 grid(plan.tiles, plan.chunks + (a.tile_count ? 1 : 0), (states + ns - 1) / ns);
   const size_t smem = allpairs_smem_bytes(plan, ns);
   if (nt == 2 && ns == 2) k_allpairs<kMinB22, 2, 2><<<grid, kThreads64, smem, st>>>(a);
   else if (nt == 2) k_allpairs<kMinB2, 2, 1><<<grid, kThreads64, smem, st>>>(a);

@@ -53,7 +53,7 @@ static cudaError_t dev_alloc(T** p, size_t count, size_t* total) {
 
 static void free_all(sws_ctx* c) {
   void* ptrs[] = {c->x, c->y, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zx, c->px, c->zy, c->py,
-                  c->src, c->srcf, c->tgt, c->e2loc, c->part, c->F0, c->Fpert, c->sigma, c->norm_part,
+                  c->src, c->srcf, c->tgt, c->e2loc, c->tile_count, c->part, c->F0, c->Fpert, c->sigma, c->norm_part,
                   c->dsrc, c->dtgt, c->e2lin, c->tgtI, c->lin_sums,
                   c->u_stage, c->V_stage, c->out_stage};
   for (void* p : ptrs)
@@ -121,6 +121,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
 
   e = p->precision == 1 ? sws::allpairs_f32_configure(&c->pair_occ) : sws::allpairs_configure(c, &c->pair_occ);
   if (e == cudaSuccess) e = sws::fields_configure(c);
+  if (e == cudaSuccess) e = sws::fused_configure(c);
   if (e == cudaSuccess && p->max_batch > 0) e = sws::lin_configure(c);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "kernel configuration (is this an sm_100 device?)"); }
 
@@ -157,6 +158,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   if (p->precision == 1) ALLOC(srcf, st * S);
   ALLOC(tgt, st * T);
   ALLOC(e2loc, st * T);
+  ALLOC(tile_count, st * ((T + 63) / 64));
   ALLOC(part, part_elems);
   ALLOC(F0, n);
   ALLOC(Fpert, mb * n);
@@ -203,6 +205,7 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   if (e == cudaSuccess) e = cudaMemcpy(c->y, hy.data(), hy.size() * 8, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(c->sp_cp, cp.data(), cp.size() * 8, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(c->sp_inv, inv.data(), inv.size() * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemset(c->tile_count, 0, st * ((T + 63) / 64) * sizeof(unsigned int));
   if (e == cudaSuccess && c->dsrc)  // unused direction slots of the last tile stay zero
     e = cudaMemset(c->dsrc, 0, (size_t)lin_groups * lin_bt * S * sizeof(double4));
   if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
@@ -324,16 +327,28 @@ static int prof_begin(sws_ctx* c, cudaStream_t st, cudaEvent_t* pe0, cudaEvent_t
 static int run_states(sws_ctx* c, const double* u, const double* V, int states, double* F0,
                       double* Fpert, cudaStream_t st, int* launches) {
   const sws::PairPlan plan = sws::make_plan(c);
-  CK(sws::launch_reconstruct(c, u, V, states, 0, F0, Fpert, st));
-  CK(sws::launch_dy(c, states, st));
-  CK(sws::launch_targets(c, states, F0, Fpert, nullptr, st));
+  if (c->fused_grid > 0) {  // the three O(NM) stages as phases of one cooperative launch
+    CK(sws::launch_fields_fused(c, u, V, states, F0, Fpert, st));
+    *launches += 1;
+  } else {
+    CK(sws::launch_reconstruct(c, u, V, states, 0, F0, Fpert, st));
+    CK(sws::launch_dy(c, states, st));
+    CK(sws::launch_targets(c, states, F0, Fpert, nullptr, st));
+    *launches += 3;
+  }
   cudaEvent_t pe0 = nullptr, pe1 = nullptr;
   int rc = prof_begin(c, st, &pe0, &pe1);
   if (rc != SWS_OK) return rc;
-  CK(sws::launch_allpairs(c, states, plan, st));
-  if (pe1) CK(cudaEventRecord(pe1, st));
-  CK(sws::launch_assemble(c, states, plan, F0, Fpert, st));
-  *launches += 5;
+  if (c->params.precision == 0) {  // the FP64 kernel assembles E2 itself (last CTA of each target tile)
+    CK(sws::launch_allpairs(c, states, plan, st, F0, Fpert));
+    if (pe1) CK(cudaEventRecord(pe1, st));
+    *launches += 1;
+  } else {
+    CK(sws::launch_allpairs(c, states, plan, st));
+    if (pe1) CK(cudaEventRecord(pe1, st));
+    CK(sws::launch_assemble(c, states, plan, F0, Fpert, st));
+    *launches += 2;
+  }
   c->last_states = states;
   c->last_lin_b = 0;
   c->lin_valid = 0;
@@ -556,6 +571,37 @@ int sws_time_allpairs(sws_ctx* c, int32_t states, int32_t reps, float* ms_per_la
   float ms = 0.f;
   CK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
   *ms_per_launch = ms / reps;
+  return SWS_OK;
+}
+
+int sws_time_residual(sws_ctx* c, const double* u_dev, double* F_dev, int32_t reps, float* ms_per_call,
+                      void* cuda_stream) {
+  if (!c || !u_dev || !F_dev || !ms_per_call || reps < 1) return SWS_EINVAL;
+  ON_DEVICE(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = sws_residual(c, u_dev, F_dev, cuda_stream);  // warm-up
+  if (rc != SWS_OK) return rc;
+  CK(cudaEventRecord(c->ev0, st));
+  for (int r = 0; r < reps; ++r) {
+    rc = sws_residual(c, u_dev, F_dev, cuda_stream);
+    if (rc != SWS_OK) return rc;
+  }
+  CK(cudaEventRecord(c->ev1, st));
+  CK(cudaEventSynchronize(c->ev1));
+  float ms = 0.f;
+  CK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+  *ms_per_call = ms / reps;
+  return SWS_OK;
+}
+
+int sws_set_fused_fields(sws_ctx* c, int32_t on) {
+  if (!c) return SWS_EINVAL;
+  if (!on) {
+    c->fused_grid = 0;
+    return SWS_OK;
+  }
+  ON_DEVICE(c->device);
+  CK(sws::fused_configure(c));
   return SWS_OK;
 }
 

@@ -5,8 +5,10 @@
 //
 // These kernels use explicitly rounded __dadd_rn/__dmul_rn where the paper's formula is a
 // short expression, so that no FMA contraction changes the rounding of the nodal fields.
+#include <cooperative_groups.h>
 #include <math_constants.h>
 
+#include "sws_closed_form.cuh"
 #include "sws_internal.cuh"
 
 namespace sws {
@@ -26,18 +28,18 @@ __device__ __forceinline__ double* state_out(double* F0, double* Fpert, int stat
 // The increments are formed by all threads; the running sum itself is sequential (one
 // thread per field) so that its rounding is that of the recurrence as printed.
 // Radiation rows eq. (24) L191-197 / App. A L417 with forward differences (L201, B.1 L431).
-__global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ u,
-                                                     const double* __restrict__ V,
-                                                     const double* __restrict__ sigma, Mesh m,
-                                                     int lin, int first, double* zeta, double* phi, double* zx,
-                                                     double* px, double* F0, double* Fpert) {
-  extern __shared__ double sm[];
-  const int N = m.N, l = blockIdx.x, state = blockIdx.y + first, tid = threadIdx.x;
+// One (y-line l, state) by the whole CTA; sm: 4 N doubles of shared memory.  Ends with the line written to the
+// planes; the caller synchronises the CTA before the shared memory is used again.
+__device__ __forceinline__ void reconstruct_line(const double* __restrict__ u, const double* __restrict__ V,
+                                                 const double* __restrict__ sigma, const Mesh& m, const int lin,
+                                                 const int l, const int state, double* sm, double* s_first,
+                                                 double* zeta, double* phi, double* zx, double* px, double* F0,
+                                                 double* Fpert) {
+  const int N = m.N, tid = threadIdx.x;
   double* s_zx = sm;
   double* s_px = sm + N;
   double* s_z = sm + 2 * (size_t)N;
   double* s_p = sm + 3 * (size_t)N;
-  __shared__ double s_first[2];
 
   const size_t half = (size_t)(N + 1) * m.M;
   const size_t offp = (size_t)l * (N + 1), offz = half + offp;
@@ -93,6 +95,16 @@ __global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ 
     zx[base + k] = s_zx[k];
     px[base + k] = s_px[k];
   }
+}
+
+__global__ void __launch_bounds__(256) k_reconstruct(const double* __restrict__ u,
+                                                     const double* __restrict__ V,
+                                                     const double* __restrict__ sigma, Mesh m,
+                                                     int lin, int first, double* zeta, double* phi, double* zx,
+                                                     double* px, double* F0, double* Fpert) {
+  extern __shared__ double sm[];
+  __shared__ double s_first[2];
+  reconstruct_line(u, V, sigma, m, lin, blockIdx.x, blockIdx.y + first, sm, s_first, zeta, phi, zx, px, F0, Fpert);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -163,43 +175,86 @@ __global__ void __launch_bounds__(128) k_dy(Mesh m, int first, const double* __r
 // The same with the 32 x-lines of a warp staged in shared memory ([l][lane], coalesced both ways): every step
 // of the two dependent sweeps then costs a shared-memory access instead of a global one (the march is pure
 // latency: 2 M dependent steps; 220 -> ~25 us at M = 241, which is 1/3 of a residual on the 91x31 mesh).
-__global__ void __launch_bounds__(32) k_dy_staged(Mesh m, int first, const double* __restrict__ cp,
-                                                  const double* __restrict__ inv, const double* zeta,
-                                                  const double* phi, double* zy, double* py) {
+// One CTA: the 32 x-lines kblock*32 .. +31 of one field of one state; s_dy: (2 M 32 + 2 M) doubles of shared
+// memory.  Every thread of the CTA takes part in the loads, the stores and the passes whose elements are
+// independent; the two dependent sweeps are marched by warp 0, one x-line per lane.  Called by all threads.
+__device__ __forceinline__ void dy_block_staged(const Mesh& m, const double* __restrict__ cp,
+                                                const double* __restrict__ inv, const int kblock, const int field,
+                                                const int state, double* s_dy, const double* zeta,
+                                                const double* phi, double* zy, double* py) {
+  const int N = m.N, M = m.M, tid = threadIdx.x, nt = blockDim.x, lane = tid & 31;
+  const int k0 = kblock * 32;
+  const double* f = (field == 0 ? zeta : phi) + (size_t)state * m.S;
+  double* out = (field == 0 ? zy : py) + (size_t)state * m.S;
+  double* sa = s_dy;                       // [M][32]
+  double* sb = s_dy + (size_t)M * 32;      // [M][32]
+  double* s_inv = sb + (size_t)M * 32;     // [M]
+  double* s_cp = s_inv + M;                // [M]
+  const int tot = M * 32;
+#pragma unroll 8
+  for (int e = tid; e < tot; e += nt) {    // rows of 32 consecutive doubles: coalesced
+    const int k = k0 + (e & 31);
+    sa[e] = f[(size_t)(e >> 5) * N + (k < N ? k : N - 1)];
+  }
+  for (int l = tid; l < M; l += nt) { s_inv[l] = inv[l]; s_cp[l] = cp[l]; }
+  __syncthreads();
+  if (m.dy_scheme == 0) {
+    // The spline march of dy_line() with its operations regrouped, not changed: first every d_l and every
+    // right-hand side (independent of one another: the FP64 divisions overlap and spread over the CTA), then the
+    // two dependent sweeps, whose chain per step is one subtraction and one multiplication.  Same values.
+    const double h = m.dy;
+    for (int e = tid; e < tot - 32; e += nt) sb[e] = SUB(sa[e + 32], sa[e]) / h;  // d_l, l = 0 .. M-2
+    __syncthreads();
+    for (int e = tid; e < tot; e += nt) {  // right-hand sides r_l into sa (f is no longer needed)
+      const int l = e >> 5;
+      double r;
+      if (l == 0) r = m.sym_first ? 0.0 : ADD(MUL(5.0, sb[e]), sb[e + 32]) / 2;
+      else if (l == M - 1) r = ADD(sb[e - 64], MUL(5.0, sb[e - 32])) / 2;
+      else r = MUL(3.0, ADD(sb[e - 32], sb[e]));
+      sa[e] = r;
+    }
+    __syncthreads();
+    if (tid < 32) {
+#define SA(l) sa[(l) * 32 + lane]
+      double g = MUL(SA(0), s_inv[0]);
+      SA(0) = g;
+#pragma unroll 4
+      for (int l = 1; l < M - 1; ++l) {
+        g = MUL(SUB(SA(l), g), s_inv[l]);  // a_l = 1
+        SA(l) = g;
+      }
+      g = MUL(SUB(SA(M - 1), MUL(2.0, g)), s_inv[M - 1]);  // a_{M-1} = 2
+      SA(M - 1) = g;
+#pragma unroll 4
+      for (int l = M - 2; l >= 0; --l) {
+        g = SUB(SA(l), MUL(s_cp[l], g));
+        SA(l) = g;
+      }
+#undef SA
+    }
+  } else if (tid < 32) {
+    dy_line(m, cp, inv, [&](int l) { return sa[l * 32 + lane]; }, [&](int l) -> double& { return sb[l * 32 + lane]; });
+  }
+  __syncthreads();
+  const double* res = m.dy_scheme == 0 ? sa : sb;
+#pragma unroll 8
+  for (int e = tid; e < tot; e += nt) {
+    const int k = k0 + (e & 31);
+    if (k < N) out[(size_t)(e >> 5) * N + k] = res[e];
+  }
+  __syncthreads();  // the shared memory may be reused by the caller's next item
+}
+
+constexpr int kDyStagedThreads = 256;
+__global__ void __launch_bounds__(kDyStagedThreads) k_dy_staged(Mesh m, int first, const double* __restrict__ cp,
+                                                               const double* __restrict__ inv, const double* zeta,
+                                                               const double* phi, double* zy, double* py) {
   extern __shared__ double s_dy[];
-  const int N = m.N, M = m.M, state = blockIdx.z + first, lane = threadIdx.x;
-  const int k = blockIdx.x * 32 + lane;
-  const bool live = k < N;
-  const size_t base = (size_t)state * m.S + (live ? k : N - 1);
-  const double* f = (blockIdx.y == 0 ? zeta : phi) + base;
-  double* out = (blockIdx.y == 0 ? zy : py) + base;
-  double* sf = s_dy;
-  double* so = s_dy + (size_t)M * 32;
-  for (int l = 0; l < M; ++l) sf[l * 32 + lane] = f[(size_t)l * N];
-  __syncwarp();
-  dy_line(m, cp, inv, [&](int l) { return sf[l * 32 + lane]; }, [&](int l) -> double& { return so[l * 32 + lane]; });
-  __syncwarp();
-  if (live)
-    for (int l = 0; l < M; ++l) out[(size_t)l * N] = so[l * 32 + lane];
+  dy_block_staged(m, cp, inv, blockIdx.x, blockIdx.y, blockIdx.z + first, s_dy, zeta, phi, zy, py);
 }
 
-// ---------------------------------------------------------------------------------------
-// a5.  Antiderivative G with d2G/ds dt = 1/sqrt(A s^2 + B s t + C t^2) (reading Q5; the paper
-// says only "exactly in terms of logarithms", L187).  D = 4AC - B^2 > 0.  A term whose
-// prefactor is 0 is 0 (the limit of t asinh(c/|t|) as t -> 0).
-__device__ double G_anti(double A, double B, double C, double sqA, double sqC, double sqD, double s,
-                         double t) {
-  double g = 0.0;
-  if (t != 0.0) g += (t / sqA) * asinh((2 * A * s + B * t) / (fabs(t) * sqD));
-  if (s != 0.0) g += (s / sqC) * asinh((2 * C * t + B * s) / (fabs(s) * sqD));
-  return g;
-}
-
-__device__ double box_int(double A, double B, double C, double sqA, double sqC, double sqD,
-                          double s1, double s2, double t1, double t2) {
-  return G_anti(A, B, C, sqA, sqC, sqD, s2, t2) - G_anti(A, B, C, sqA, sqC, sqD, s1, t2) -
-         G_anti(A, B, C, sqA, sqC, sqD, s2, t1) + G_anti(A, B, C, sqA, sqC, sqD, s1, t1);
-}
+// a5: the closed form of I lives in sws_closed_form.cuh (shared with the all-pairs kernel, whose extra CTA row
+// evaluates it concurrently with the pair loops).
 
 // The same antiderivative together with its partial derivatives with respect to A, B, C
 // (analytic Jacobian action: dI = I_A dA + I_B dB + I_C dC).  With Q = A s^2 + B s t + C t^2,
@@ -240,19 +295,14 @@ __device__ G4 box_int4(double A, double B, double C, double sqA, double sqC, dou
 
 // a3 + a5 + a6 (local part) + a7 + packing of the transposed source records.
 // One thread per node (k, l) of one state; threads with k < N-1 also own target (k, l).
-__global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restrict__ x,
-                                                 const double* __restrict__ y,
-                                                 const double* __restrict__ zeta,
-                                                 const double* __restrict__ phi,
-                                                 const double* __restrict__ zx,
-                                                 const double* __restrict__ px,
-                                                 const double* __restrict__ zy,
-                                                 const double* __restrict__ py, SrcRec* src,
-                                                 SrcRecF* srcf, TgtRec* tgt, double* e2loc, double4* tgtI,
-                                                 double* F0, double* Fpert) {
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= m.N) return;
-  const int N = m.N, M = m.M, l = blockIdx.y, state = blockIdx.z;
+// One node (k, l) of one state.
+__device__ __forceinline__ void target_node(const Mesh& m, const int k, const int l, const int state,
+                                            const double* __restrict__ x, const double* __restrict__ y,
+                                            const double* zeta, const double* phi, const double* zx,
+                                            const double* px, const double* zy, const double* py, SrcRec* src,
+                                            SrcRecF* srcf, TgtRec* tgt, double* e2loc, double4* tgtI, double* F0,
+                                            double* Fpert) {
+  const int N = m.N, M = m.M;
   const size_t nd = (size_t)state * m.S + (size_t)l * N + k;
   const double xk = x[k], yl = y[l];
   const double z0 = zeta[nd], p0 = phi[nd], zx0 = zx[nd], px0 = px[nd], zy0 = zy[nd], py0 = py[nd];
@@ -314,17 +364,79 @@ __global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restric
     tgtI[t] = make_double4(r.g, r.gA, r.gB, r.gC);
     return;
   }
-  double I;
-  if (ya == 0.0) {
-    // the two boxes share the edge t = -y*: one box over t in [-(y_M + y*), y_M - y*]
-    I = box_int(A, B, C, sqA, sqC, sqD, s1, s2, -(yb + ys), yb - ys);
-  } else {
-    I = box_int(A, B, C, sqA, sqC, sqD, s1, s2, ya - ys, yb - ys) +
-        box_int(A, B, C, sqA, sqC, sqD, s1, s2, -(yb + ys), -(ya + ys));
+  // a5 + a6 local part; e2loc == NULL: the FP64 all-pairs launch forms it itself (its CTA row 0), off this path
+  if (e2loc) e2loc[ts] = e2_local(tr, m.eps, x[0], x[N - 1], ya, yb);
+}
+
+__global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restrict__ x,
+                                                 const double* __restrict__ y,
+                                                 const double* __restrict__ zeta,
+                                                 const double* __restrict__ phi,
+                                                 const double* __restrict__ zx,
+                                                 const double* __restrict__ px,
+                                                 const double* __restrict__ zy,
+                                                 const double* __restrict__ py, SrcRec* src,
+                                                 SrcRecF* srcf, TgtRec* tgt, double* e2loc, double4* tgtI,
+                                                 double* F0, double* Fpert) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= m.N) return;
+  target_node(m, k, blockIdx.y, blockIdx.z, x, y, zeta, phi, zx, px, zy, py, src, srcf, tgt, e2loc, tgtI, F0, Fpert);
+}
+
+// ---------------------------------------------------------------------------------------
+// a0-a3, a5, a6 (local), a7, a8 in ONE cooperative launch: the three O(NM) stages above run as phases of one
+// grid, separated by grid-wide barriers, instead of three dependent launches.  On the paper's small meshes
+// (Table 1: 91x31 ... 361x121) the residual is launch-latency bound outside the all-pairs kernel, and
+// this takes two launches and their drain/fill gaps out of every evaluation.  The phases call the very device
+// functions of k_reconstruct, k_dy_staged and k_targets: same operations, same order, same roundings.
+struct FusedArgs {
+  const double* u;
+  const double* V;
+  const double* sigma;
+  Mesh m;
+  int states;
+  const double* cp;
+  const double* inv;
+  const double* x;
+  const double* y;
+  double *zeta, *phi, *zx, *px, *zy, *py;
+  SrcRec* src;
+  SrcRecF* srcf;
+  TgtRec* tgt;
+  double* e2loc;
+  double *F0, *Fpert;
+};
+
+__global__ void __launch_bounds__(256) k_fields_fused(const FusedArgs a) {
+  extern __shared__ double sm[];  // max(4 N, 2 M 32 + 2 M) doubles
+  __shared__ double s_first[2];
+  namespace cg = cooperative_groups;
+  cg::grid_group grid = cg::this_grid();
+  const Mesh& m = a.m;
+  // phase 1: unpack + x-trapezoid + radiation rows, one (line, state) per CTA pass
+  for (int item = blockIdx.x; item < m.M * a.states; item += gridDim.x) {
+    reconstruct_line(a.u, a.V, a.sigma, m, 0, item % m.M, item / m.M, sm, s_first, a.zeta, a.phi, a.zx, a.px, a.F0,
+                     a.Fpert);
+    __syncthreads();
   }
-  // a6 local part: 2 pi (phi* - x*) + eps / sqrt(x*^2 + y*^2 + (zeta*+1)^2) - zeta_x* I
-  const double rho2 = xs * xs + ys * ys + (zs + 1.0) * (zs + 1.0);
-  e2loc[ts] = 2.0 * CUDART_PI * (ps - xs) + m.eps / sqrt(rho2) - zxs * I;
+  grid.sync();
+  // phase 2: y-derivatives, one (block of 32 x-lines, field, state) per CTA pass
+  {
+    const int kblocks = (m.N + 31) / 32;
+    for (int item = blockIdx.x; item < kblocks * 2 * a.states; item += gridDim.x)
+      dy_block_staged(m, a.cp, a.inv, item % kblocks, (item / kblocks) & 1, item / (2 * kblocks), sm, a.zeta, a.phi,
+                      a.zy, a.py);
+  }
+  grid.sync();
+  // phase 3: midpoints, A/B/C, Bernoulli rows, closed-form I, source/target records: one node per thread pass
+  const size_t total = (size_t)m.S * a.states;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+    const int state = (int)(idx / m.S);
+    const int rem = (int)(idx - (size_t)state * m.S);
+    const int l = rem / m.N, k = rem - l * m.N;
+    target_node(m, k, l, state, a.x, a.y, a.zeta, a.phi, a.zx, a.px, a.zy, a.py, a.src, a.srcf, a.tgt, a.e2loc,
+                nullptr, a.F0, a.Fpert);
+  }
 }
 
 // a6 + a9: E2_{k,l} = local - sum over chunks (fixed order) of the all-pairs partials.
@@ -390,7 +502,8 @@ __global__ void __launch_bounds__(256) k_quotient(const double* __restrict__ F0,
 size_t reconstruct_smem_bytes(int N) { return (size_t)4 * N * sizeof(double); }
 
 constexpr size_t kDyStagedMaxSmem = 200 * 1024;
-static size_t dy_staged_smem_bytes(int M) { return (size_t)2 * M * 32 * sizeof(double); }
+constexpr int kFusedMaxNodes = 1 << 17;  // the fused fields launch is used up to this many mesh nodes
+static size_t dy_staged_smem_bytes(int M) { return ((size_t)2 * M * 32 + 2 * M) * sizeof(double); }
 
 cudaError_t fields_configure(const sws_ctx* c) {
   cudaError_t e = cudaFuncSetAttribute(k_reconstruct, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -400,6 +513,55 @@ cudaError_t fields_configure(const sws_ctx* c) {
   if (smem <= kDyStagedMaxSmem)
     e = cudaFuncSetAttribute(k_dy_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   return e;
+}
+
+// The fused launch is used when both the line buffers of phase 1 and the staged block of phase 2 fit the CTA's
+// shared memory and the device can co-schedule the grid (cooperative launch); decided once per context.
+static size_t fused_smem_bytes(const Mesh& m) {
+  const size_t a = reconstruct_smem_bytes(m.N), b = dy_staged_smem_bytes(m.M);
+  return a > b ? a : b;
+}
+
+cudaError_t fused_configure(sws_ctx* c) {
+  c->fused_grid = 0;
+  const size_t smem = fused_smem_bytes(c->mesh);
+  if (smem > kDyStagedMaxSmem) return cudaSuccess;
+  // Larger meshes gain nothing (the all-pairs kernel is > 99 % of the evaluation there) and phase 3 would run
+  // at the low occupancy the staged block of phase 2 dictates.
+  if (c->mesh.S > kFusedMaxNodes) return cudaSuccess;
+  int coop = 0;
+  cudaError_t e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device);
+  if (e != cudaSuccess || !coop) return e;
+  e = cudaFuncSetAttribute(k_fields_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int occ = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_fields_fused, 256, smem);
+  if (e != cudaSuccess) return e;
+  if (occ < 1) return cudaSuccess;
+  if (occ > 2) occ = 2;  // a small grid keeps the two grid barriers cheap; the phases are latency bound
+  c->fused_grid = occ * c->sm_count;
+  return cudaSuccess;
+}
+
+cudaError_t launch_fields_fused(sws_ctx* c, const double* u, const double* V, int states, double* F0, double* Fpert,
+                                cudaStream_t st) {
+  const Mesh& m = c->mesh;
+  FusedArgs a;
+  a.u = u; a.V = V; a.sigma = c->sigma; a.m = m; a.states = states;
+  a.cp = c->sp_cp; a.inv = c->sp_inv; a.x = c->x; a.y = c->y;
+  a.zeta = c->zeta; a.phi = c->phi; a.zx = c->zx; a.px = c->px; a.zy = c->zy; a.py = c->py;
+  // FP64 path: the all-pairs launch forms e2loc itself (its local CTA row); the FP32 variant keeps it here
+  a.src = c->src; a.srcf = c->srcf; a.tgt = c->tgt; a.e2loc = c->params.precision == 0 ? nullptr : c->e2loc;
+  a.F0 = F0; a.Fpert = Fpert;
+  // no more CTAs than the largest phase has work for
+  size_t work = ((size_t)m.S * states + 255) / 256;
+  const size_t w1 = (size_t)m.M * states, w2 = (size_t)((m.N + 31) / 32) * 2 * states;
+  if (w1 > work) work = w1;
+  if (w2 > work) work = w2;
+  int grid = c->fused_grid;
+  if ((size_t)grid > work) grid = (int)work;
+  void* args[] = {(void*)&a};
+  return cudaLaunchCooperativeKernel((const void*)k_fields_fused, dim3(grid), dim3(256), args, fused_smem_bytes(m), st);
 }
 
 cudaError_t launch_reconstruct(sws_ctx* c, const double* u, const double* V, int states, int lin,
@@ -416,7 +578,7 @@ cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st, int first) {
   const size_t smem = dy_staged_smem_bytes(m.M);
   if (smem <= kDyStagedMaxSmem) {
     dim3 grid((m.N + 31) / 32, 2, states - first);
-    k_dy_staged<<<grid, 32, smem, st>>>(m, first, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zy, c->py);
+    k_dy_staged<<<grid, kDyStagedThreads, smem, st>>>(m, first, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zy, c->py);
   } else {  // very long columns: march in global memory
     dim3 grid((m.N + 127) / 128, 2, states - first);
     k_dy<<<grid, 128, 0, st>>>(m, first, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zy, c->py);
@@ -428,8 +590,10 @@ cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, do
                            cudaStream_t st) {
   const Mesh& m = c->mesh;
   dim3 grid((m.N + 127) / 128, m.M, states);
+  // residual path in FP64 (no tgtI): e2loc is formed by the all-pairs launch's local CTA row instead
+  double* e2loc = (c->params.precision == 0 && !tgtI) ? nullptr : c->e2loc;
   k_targets<<<grid, 128, 0, st>>>(m, c->x, c->y, c->zeta, c->phi, c->zx, c->px, c->zy, c->py, c->src,
-                                  c->srcf, c->tgt, c->e2loc, tgtI, F0, Fpert);
+                                  c->srcf, c->tgt, e2loc, tgtI, F0, Fpert);
   return cudaGetLastError();
 }
 

@@ -98,6 +98,8 @@ struct sws_ctx {
   sws::SrcRec* src;  // [state][i][j]  (transposed)
   sws::SrcRecF* srcf;  // the same in FP32 (precision = 1 only, else NULL)
   int pair_occ;        // resident CTAs per SM of the all-pairs kernel in use
+  int fused_grid;      // CTAs of the fused (cooperative) fields launch; 0: three separate launches
+  unsigned int* tile_count;  // [max_states][tiles] arrival counters of the all-pairs CTAs of a target tile
   sws::TgtRec* tgt;  // [state][t], t = l (N-1) + k
   double* e2loc;     // [state][t]   2 pi (phi*-x*) + eps/rho* - zeta_x* I
   double* part;      // [state][chunk][t] partial all-pairs sums (already times dx dy)
@@ -141,8 +143,10 @@ cudaError_t launch_dy(sws_ctx* c, int states, cudaStream_t st, int first = 0);
 // tgtI != NULL: base state of the analytic Jacobian action ({I, I_A, I_B, I_C} instead of e2loc)
 cudaError_t launch_targets(sws_ctx* c, int states, double* F0, double* Fpert, double4* tgtI,
                            cudaStream_t st);
-// dispatches on sws_params.precision (0: FP64 kernel, 1: FP32 pair arithmetic)
-cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
+// dispatches on sws_params.precision (0: FP64 kernel, 1: FP32 pair arithmetic).  FP64 kernel with F0 != NULL:
+// the kernel also assembles the rows E2 into F0 / Fpert (fused a6 + a9); otherwise launch_assemble follows.
+cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st, double* F0 = nullptr,
+                            double* Fpert = nullptr);
 cudaError_t launch_count_near(sws_ctx* c, int states, int* out, cudaStream_t st);
 cudaError_t launch_allpairs_f32(sws_ctx* c, int states, const PairPlan& plan, cudaStream_t st);
 cudaError_t launch_assemble(sws_ctx* c, int states, const PairPlan& plan, double* F0,
@@ -173,6 +177,9 @@ int count_near_warps(const sws_ctx* c);
 cudaError_t allpairs_f32_configure(int* occ_out);
 size_t allpairs_f32_smem_bytes(int seg_len);
 cudaError_t fields_configure(const sws_ctx* c);
+cudaError_t fused_configure(sws_ctx* c);
+cudaError_t launch_fields_fused(sws_ctx* c, const double* u, const double* V, int states, double* F0, double* Fpert,
+                                cudaStream_t st);
 size_t reconstruct_smem_bytes(int N);
 
 }  // namespace sws

@@ -230,6 +230,30 @@ def test_states_per_cta_is_bitwise_invisible(sws, name, b):
         assert np.abs(out[1][1][0] - out[1][2]).max() > 1e-4    # the shifts really moved the states
 
 
+def test_fused_and_separate_field_launches(sws, oracle80):
+    """Small meshes run a0-a3, a5-a8 as ONE cooperative launch (2 launches per residual), meshes above 2^17
+    nodes as three (4 per residual); both against the oracle in full / on sampled rows, and repeatable bit for
+    bit (the tile counters of the fused assembly return to zero)."""
+    cfg = W.CONFIGS[2]
+    u = W.state(cfg)
+    E = oracle80.residual(cfg.params(), u)
+    with sws.Context(cfg.params()) as ctx:
+        F1 = ctx.residual(dev(u)).cpu().numpy()
+        assert ctx.last_launch_count == 2
+        F2 = ctx.residual(dev(u)).cpu().numpy()
+    assert relerr(F1, E) <= TOL and np.array_equal(F1, F2)
+    big = W.CONFIGS[4]                                  # 173,761 nodes: separate launches
+    ub = W.state(big)
+    pick = np.arange(0, big.targets, 997, dtype=np.int32)
+    Eb = oracle80.residual(big.params(), ub, rows=pick)
+    mask = ~np.isnan(Eb)
+    with sws.Context(big.params()) as ctx:
+        Fb = ctx.residual(dev(ub)).cpu().numpy()
+        assert ctx.last_launch_count == 4
+        Fb2 = ctx.residual(dev(ub)).cpu().numpy()
+    assert np.abs(Fb[mask] - Eb[mask]).max() / np.abs(Eb[mask]).max() <= TOL and np.array_equal(Fb, Fb2)
+
+
 def _column_sum_longdouble(y1, dy, M, c, g):
     """sum_j c_j [((y_j-c)^2+g)^-1/2 + ((y_j+c)^2+g)^-1/2], c_j = 1/2 at both ends, term by term."""
     y = (np.longdouble(y1) + np.arange(M, dtype=np.longdouble) * np.longdouble(dy))[None, :]
@@ -500,7 +524,7 @@ def test_host_api_matches_device_api(sws):
         assert np.array_equal(JVd.cpu().numpy(), JVh)
         assert np.array_equal(Fpd.cpu().numpy(), Fph)
         assert np.array_equal(F0d.cpu().numpy(), F0h)
-        assert ctx.last_launch_count == 8   # 2 (shift) + 5 (a0-a9) + 1 (quotient)
+        assert ctx.last_launch_count == 5   # 2 (shift) + fused fields + all-pairs (with assembly) + quotient
 
 
 def test_layout_unit_perturbations(sws, oracle64):
