@@ -51,6 +51,12 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
  * Asynchronous on `cuda_stream`. */
 int sws_precond_apply(sws_precond* pc, const double* v_dev, double* r_dev, void* cuda_stream);
 
+/* The same for t vectors at once (1 <= t <= 16): R_dev[q][0..n) = P^-1 V_dev[q][0..n), both [t][n] row-major.
+ * The block sweeps read every factor panel once for up to 16 vectors instead of once per vector (the
+ * panels are what an apply streams from HBM).  Each vector's result agrees with sws_precond_apply to
+ * summation round-off.  The first call with t > 1 grows the internal vectors (synchronises once). */
+int sws_precond_apply_multi(sws_precond* pc, const double* V_dev, int32_t t, double* R_dev, void* cuda_stream);
+
 /* Block (l, m) (0-based y-lines) of the ASSEMBLED matrices, (N+1) x (N+1) row-major into
  * out_host: which = 0: D block of (B.6) and the radiation rows E5, E6; which = 1: the Schur
  * complement block D - C A^-1 B.  Needs flags bit 0 at creation and |l - m| within the band. */
@@ -69,6 +75,15 @@ typedef struct {
                        sws_jv_batch (base and shifted state evaluated per product); 2 eq. (25)
                        with the base residual E(u) the driver already holds: ONE sws_residual
                        per product, the paper's own scheme (L219), same shift sigma        */
+  int32_t block;    /* 0 or 1: plain GMRES.  t in 2..16 (t <= the context's max_batch): ENLARGED GMRES - the
+                       right-hand side is split by groups of y-lines into t pieces that sum to it and the block
+                       Krylov space K_m(J P^-1, [T_1 r .. T_t r]) is built with ONE t-vector Jacobian action
+                       (sws_jv_apply(V[t]), or sws_jv_batch for jv_mode 1, 2) and ONE t-vector preconditioner
+                       sweep per iteration; the iterate minimises the residual over that space, which contains the
+                       plain Krylov space of the same depth.  One cycle of at most min(restart / t,
+                       (max_restart + 1) / t - 1) blocks, no restart; its, maxit and hist count / index products
+                       resp. block iterations (hist[j] after block j).  Falls back to plain GMRES when a piece of
+                       the right-hand side is zero.                                                       */
 } sws_gmres_opts;
 
 typedef struct {

@@ -254,3 +254,79 @@ def newton(residual, jv, apply_Pinv, u0, *, ftol: float, eta: float, restart: in
     log.append({"newton": len(log), "fnorm": float(np.linalg.norm(E)), "finf": float(np.abs(E).max()),
                 "gmres_its": 0, "gmres_rel": 0.0, "lambda": 0.0})
     return u, log
+
+
+# ---------------------------------------------------------------------------------------
+# Enlarged (block) GMRES: a Krylov method that uses b > 1 Jacobian-vector products per iteration
+# ("block/s-step Krylov that actually uses b>1"; the paper's own solver is plain GMRES,
+# section 4.1).  Plain restatement of the enlarged Krylov idea: the right-hand side is split by a
+# partition of the unknowns into t vectors that sum to it,
+#     R0 = [T_1 r, ..., T_t r],   r = R0 1,
+# the BLOCK Krylov space K_m(J P^-1, R0) is built by block Arnoldi - ONE application of J to t vectors per
+# iteration - and the iterate is d = P^-1 V y with y minimising ||r - J P^-1 V y||_2 over that space, which
+# contains K_m(J P^-1, r) (so m block iterations are at least as good as m plain GMRES iterations).
+def line_partition(p: dict, t: int) -> np.ndarray:
+    """group[idx] in 0..t-1 for every unknown idx of eq. (18): the y-lines are cut into t contiguous
+    groups, line l (0-based) belongs to group floor(l t / M); the phi and the zeta unknowns of a line go
+    together."""
+    N, M = int(p["N"]), int(p["M"])
+    line = np.tile(np.repeat(np.arange(M), N + 1), 2)
+    return (line * t) // M
+
+
+def _mgs_qr(W: np.ndarray):
+    """W [t, n] (rows are vectors) = R^T-combination of orthonormal rows Q: modified Gram-Schmidt, column by
+    column, positive diagonal.  Returns (Q [t, n], R [t, t] upper triangular) with W^T = Q^T R."""
+    t = W.shape[0]
+    Q = np.zeros_like(W)
+    R = np.zeros((t, t))
+    for c in range(t):
+        w = W[c].copy()
+        for i in range(c):
+            R[i, c] = float(Q[i] @ w)
+            w = w - R[i, c] * Q[i]
+        R[c, c] = float(np.linalg.norm(w))
+        if R[c, c] == 0.0:
+            raise np.linalg.LinAlgError("enlarged GMRES: rank-deficient block (breakdown)")
+        Q[c] = w / R[c, c]
+    return Q, R
+
+
+def egmres_right(apply_J_block, apply_Pinv, rhs, group, t: int, tol: float, max_blocks: int):
+    """Solve J d = rhs by enlarged GMRES with t right-hand-side pieces (no restart), right preconditioned.
+      apply_J_block(Z) -> J Z for Z [t, n] (rows are vectors): the ONE batched product per iteration.
+      group: partition of the unknowns (line_partition).
+    Block Arnoldi with block modified Gram-Schmidt; the (m+1)t x mt band Hessenberg least-squares problem
+    min ||e_1 (x) (B 1) - H y||_2 is solved by numpy.linalg.lstsq from scratch after every block (plain).
+    Returns (d, history): history[j] = ||rhs - J d_j||_2 / ||rhs||_2 after j+1 block iterations."""
+    n = rhs.size
+    bnorm = float(np.linalg.norm(rhs))
+    hist = []
+    d = np.zeros(n)
+    if bnorm == 0.0:
+        return d, hist
+    R0 = np.stack([np.where(group == i, rhs, 0.0) for i in range(t)])         # [t, n], rows sum to rhs
+    V = np.zeros(((max_blocks + 1) * t, n))
+    Hh = np.zeros(((max_blocks + 1) * t, max_blocks * t))
+    V[:t], B = _mgs_qr(R0)
+    g0 = B @ np.ones(t)                                                        # rhs = V_1^T (B 1)
+    for j in range(max_blocks):
+        Z = np.stack([apply_Pinv(V[j * t + c]) for c in range(t)])
+        W = apply_J_block(Z)                                                   # t products at once
+        for i in range(j + 1):                                                 # block modified Gram-Schmidt
+            Vi = V[i * t:(i + 1) * t]
+            Hij = Vi @ W.T                                                     # [t, t]: (V_i^T W)
+            Hh[i * t:(i + 1) * t, j * t:(j + 1) * t] = Hij
+            W = W - Hij.T @ Vi
+        Q, R = _mgs_qr(W)
+        V[(j + 1) * t:(j + 2) * t] = Q
+        Hh[(j + 1) * t:(j + 2) * t, j * t:(j + 1) * t] = R
+        rows, cols = (j + 2) * t, (j + 1) * t
+        g = np.zeros(rows)
+        g[:t] = g0
+        y, *_ = np.linalg.lstsq(Hh[:rows, :cols], g, rcond=None)
+        hist.append(float(np.linalg.norm(g - Hh[:rows, :cols] @ y)) / bnorm)
+        if hist[-1] <= tol or j == max_blocks - 1:
+            d = apply_Pinv(y @ V[:cols])
+            break
+    return d, hist

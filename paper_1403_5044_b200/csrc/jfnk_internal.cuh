@@ -61,6 +61,7 @@ struct sws_precond {
   double* t2;      // [H]  b2 - C s1
   double* y;       // [H]  forward / backward substitution vector
   double* panel;   // scratch: one assembled block row (sws_precond_block_host)
+  int multi_cap;   // right-hand sides s1, t2, y have room for (1, or 16 after the first sws_precond_apply_multi)
   // the 2 M dependent sweep launches of sws_precond_apply as one CUDA graph (they touch internal buffers only)
   cudaGraphExec_t sweep_graph;
   int sweep_graph_state;  // 0: not built yet, 1: built, -1: capture failed, launch directly

@@ -144,6 +144,8 @@ __global__ void __launch_bounds__(256) k_stage1(LinMesh m, const double* __restr
   double* a = sh;            // [n1]
   double* c = sh + m.n1;     // [n1]
   const int l = blockIdx.x;
+  const size_t q = blockIdx.y;  // right-hand side of a multi-vector apply
+  v += q * 2 * (size_t)m.H; s1 += q * (size_t)m.H; t2 += q * (size_t)m.H;
   const double* b1 = v + (size_t)l * m.n1;
   const double* b2 = v + (size_t)m.H + (size_t)l * m.n1;
   for (int i = threadIdx.x; i < m.n1; i += blockDim.x) a[i] = b1[i];
@@ -166,6 +168,8 @@ __global__ void __launch_bounds__(256) k_stage3(LinMesh m, const double* __restr
   double* a = sh;
   double* c = sh + m.n1;
   const int l = blockIdx.x;
+  const size_t q = blockIdx.y;
+  s1 += q * (size_t)m.H; s2 += q * (size_t)m.H; r += q * 2 * (size_t)m.H;
   for (int i = threadIdx.x; i < m.n1; i += blockDim.x) a[i] = s2[(size_t)l * m.n1 + i];
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -257,6 +261,79 @@ __global__ void __launch_bounds__(kGemvThreads) k_bwd_row(const double* __restri
   if (threadIdx.x == 0) yk[r] -= s;
 }
 
+// The same sweeps for T right-hand sides at once (enlarged GMRES: one sweep over the factor panels serves the T
+// vectors of a block, so the panels - 30 GB at 721x241 - are streamed once instead of T times).  Vector q of a
+// buffer starts at base + q ldv.  One CTA per matrix row, the row read once, T accumulators per thread.
+template <int T>
+__device__ __forceinline__ void row_dot_multi(const double* __restrict__ row, const double* __restrict__ x, size_t ldv,
+                                              int K, double (&acc)[T]) {
+  int c = threadIdx.x;
+  for (; c + kGemvThreads < K; c += 2 * kGemvThreads) {
+    const double a0 = __ldcs(row + c), a1 = __ldcs(row + c + kGemvThreads);
+#pragma unroll
+    for (int q = 0; q < T; ++q) {
+      acc[q] = fma(a0, x[q * ldv + c], acc[q]);
+      acc[q] = fma(a1, x[q * ldv + c + kGemvThreads], acc[q]);
+    }
+  }
+  for (; c < K; c += kGemvThreads) {
+    const double a0 = __ldcs(row + c);
+#pragma unroll
+    for (int q = 0; q < T; ++q) acc[q] = fma(a0, x[q * ldv + c], acc[q]);
+  }
+}
+
+template <int T>
+__device__ __forceinline__ void cta_sum_multi(double (&acc)[T], double* red /* [T][warps] */) {
+  const int w = threadIdx.x >> 5, nw = kGemvThreads / 32;
+#pragma unroll
+  for (int q = 0; q < T; ++q) {
+    double v = acc[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) red[q * nw + w] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < T) {
+    double s = 0.0;
+    for (int i = 0; i < nw; ++i) s += red[threadIdx.x * nw + i];
+    acc[0] = s;  // thread q < T holds the sum of right-hand side q
+  }
+}
+
+template <int T>
+__global__ void __launch_bounds__(kGemvThreads) k_fwd_row_multi(const double* __restrict__ panel, int n1, int lk,
+                                                                const double* __restrict__ yprev,
+                                                                const double* __restrict__ tk,
+                                                                double* __restrict__ yk, size_t ldv) {
+  __shared__ double red[T * (kGemvThreads / 32)];
+  const int r = blockIdx.x;
+  const int K0 = lk * n1;
+  const double* row = panel + (size_t)r * (K0 + n1);
+  double acc[T];
+#pragma unroll
+  for (int q = 0; q < T; ++q) acc[q] = 0.0;
+  row_dot_multi<T>(row, yprev, ldv, K0, acc);
+  row_dot_multi<T>(row + K0, tk, ldv, n1, acc);
+  cta_sum_multi<T>(acc, red);
+  if (threadIdx.x < T) yk[threadIdx.x * ldv + r] = acc[0];
+}
+
+template <int T>
+__global__ void __launch_bounds__(kGemvThreads) k_bwd_row_multi(const double* __restrict__ panel, int n1, int uk,
+                                                                const double* __restrict__ xnext,
+                                                                double* __restrict__ yk, size_t ldv) {
+  __shared__ double red[T * (kGemvThreads / 32)];
+  const int r = blockIdx.x;
+  const int K = uk * n1;
+  double acc[T];
+#pragma unroll
+  for (int q = 0; q < T; ++q) acc[q] = 0.0;
+  row_dot_multi<T>(panel + (size_t)r * K, xnext, ldv, K, acc);
+  cta_sum_multi<T>(acc, red);
+  if (threadIdx.x < T) yk[threadIdx.x * ldv + r] -= acc[0];
+}
+
 __global__ void k_identity(double* a, int n) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n * n) a[i] = (i / n == i % n) ? 1.0 : 0.0;
@@ -338,6 +415,23 @@ void host_G(const LinMesh& m, std::vector<double>& G) {
 
 }  // namespace
 
+template <int T>
+static void launch_sweeps_multi(sws_precond* pc, cudaStream_t st) {
+  const int n1 = pc->lm.n1, M = pc->lm.M, hb = pc->hb;
+  const size_t ldv = (size_t)pc->lm.H;
+  for (int k = 0; k < M; ++k) {
+    const int lk = k < hb ? k : hb;
+    k_fwd_row_multi<T><<<n1, kGemvThreads, 0, st>>>(pc->fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
+                                                    pc->t2 + (size_t)k * n1, pc->y + (size_t)k * n1, ldv);
+  }
+  for (int k = M - 2; k >= 0; --k) {
+    const int uk = (M - 1 - k) < hb ? (M - 1 - k) : hb;
+    if (uk > 0)
+      k_bwd_row_multi<T><<<n1, kGemvThreads, 0, st>>>(pc->bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
+                                                      pc->y + (size_t)k * n1, ldv);
+  }
+}
+
 extern "C" {
 
 const char* sws_jfnk_last_error(void) { return g_err; }
@@ -369,6 +463,7 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
   pc->factored = 0;
   pc->bytes = 0;
   pc->G = pc->corr = pc->fwd = pc->bwd = pc->s1 = pc->t2 = pc->y = pc->panel = nullptr;
+  pc->multi_cap = 1;
 
   const int n1 = m.n1, M = m.M, T = (m.N - 1) * M;
   const size_t blk = (size_t)n1 * n1;
@@ -561,6 +656,52 @@ int sws_precond_apply(sws_precond* pc, const double* v_dev, double* r_dev, void*
   k_stage3<<<M, 256, sh, st>>>(m, pc->s1, pc->y, r_dev);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? SWS_OK : fail_cuda(e, "sws_precond_apply");
+}
+
+int sws_precond_apply_multi(sws_precond* pc, const double* V_dev, int32_t t, double* R_dev, void* cuda_stream) {
+  if (!pc || !V_dev || !R_dev || t < 1 || t > 16) return SWS_EINVAL;
+  if (!pc->factored) return SWS_EINVAL;
+  if (t == 1) return sws_precond_apply(pc, V_dev, R_dev, cuda_stream);
+  DevGuard dg(pc->device);
+  if (dg.err != cudaSuccess) return fail_cuda(dg.err, "sws_precond_apply_multi (device)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const LinMesh& m = pc->lm;
+  const int n1 = m.n1, M = m.M;
+  if (t > pc->multi_cap) {  // grow the internal vectors once (synchronises)
+    cudaError_t e = cudaDeviceSynchronize();
+    double* nb[3] = {nullptr, nullptr, nullptr};
+    for (int i = 0; i < 3 && e == cudaSuccess; ++i) e = cudaMalloc(&nb[i], (size_t)16 * m.H * sizeof(double));
+    if (e != cudaSuccess) {
+      for (double* b : nb) if (b) cudaFree(b);
+      return e == cudaErrorMemoryAllocation ? SWS_ENOMEM : fail_cuda(e, "sws_precond_apply_multi (workspace)");
+    }
+    cudaFree(pc->s1); cudaFree(pc->t2); cudaFree(pc->y);
+    pc->s1 = nb[0]; pc->t2 = nb[1]; pc->y = nb[2];
+    pc->bytes += (size_t)3 * 15 * m.H * sizeof(double);
+    pc->multi_cap = 16;
+    if (pc->sweep_graph) { cudaGraphExecDestroy(pc->sweep_graph); pc->sweep_graph = nullptr; }
+    pc->sweep_graph_state = 0;  // the captured single-vector sweeps point at the old buffers
+  }
+  const size_t sh = 2 * (size_t)n1 * sizeof(double);
+  int done = 0;
+  while (done < t) {  // tiles of 16, 8, 4, 2, 1 right-hand sides
+    const int left = t - done;
+    const int T = left >= 16 ? 16 : left >= 8 ? 8 : left >= 4 ? 4 : left >= 2 ? 2 : 1;
+    const double* v = V_dev + (size_t)done * 2 * m.H;
+    double* r = R_dev + (size_t)done * 2 * m.H;
+    k_stage1<<<dim3(M, T), 256, sh, st>>>(m, v, pc->s1, pc->t2);
+    switch (T) {
+      case 16: launch_sweeps_multi<16>(pc, st); break;
+      case 8: launch_sweeps_multi<8>(pc, st); break;
+      case 4: launch_sweeps_multi<4>(pc, st); break;
+      case 2: launch_sweeps_multi<2>(pc, st); break;
+      default: launch_sweeps(pc, st); break;
+    }
+    k_stage3<<<dim3(M, T), 256, sh, st>>>(m, pc->s1, pc->y, r);
+    done += T;
+  }
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? SWS_OK : fail_cuda(e, "sws_precond_apply_multi");
 }
 
 int sws_precond_block_host(sws_precond* pc, int32_t which, int32_t l, int32_t mm, double* out_host) {

@@ -131,6 +131,19 @@ __global__ void k_norms_finish(const double* __restrict__ partial, int nblk, dou
   out[1] = m;
 }
 
+// Enlarged GMRES: piece c of the right-hand side, R0_c = T_c r: the entries of r that belong to the y-lines of
+// group c (line l -> group floor(l t / M); the phi and zeta unknowns of a line together), zero elsewhere.
+__global__ void __launch_bounds__(256) k_split(double* __restrict__ R0, const double* __restrict__ r, int n, int n1,
+                                               int M, int t) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n) return;
+  const int H = n1 * M;
+  const int line = (idx >= H ? idx - H : idx) / n1;
+  const int grp = (int)(((long long)line * t) / M);
+  const double v = r[idx];
+  for (int c = 0; c < t; ++c) R0[(size_t)c * n + idx] = (c == grp) ? v : 0.0;
+}
+
 }  // namespace jfnk
 
 using namespace jfnk;
@@ -148,6 +161,13 @@ struct sws_solver {
   double* hdev;     // [2 (m_max + 1) + 2]: h1 | h2 | normsq, scratch
   double* ydev;     // [m_max]
   double* hpin;     // pinned host mirror of hdev
+  // enlarged (block) GMRES, allocated at its first use
+  int N, M, max_batch;
+  int blk_t;        // pieces the block workspace was sized for (0: none)
+  double *Zb, *Wb;  // [t][n] each: P^-1 V_j and J P^-1 V_j
+  double* hblk;     // device: per column of a block [2 nv_max | 2 t | 1] orthogonalisation coefficients
+  double* hblk_pin; // pinned host mirror
+  size_t hblk_len;
   cudaEvent_t ev[4];
   // accounting of the current driver call
   int n_jv, n_pc, n_res;
@@ -353,6 +373,203 @@ int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opt
   return SWS_OK;
 }
 
+// ---------------------------------------------------------------------------------------
+// Enlarged (block) GMRES: the Krylov method that uses b > 1 products per iteration.
+// The right-hand side is split by groups of y-lines into t pieces that sum to it, R0 = [T_1 r .. T_t r]; block
+// Arnoldi builds K_m(J P^-1, R0) with ONE sws_jv_apply(V[t]) (or one sws_jv_batch) and ONE multi-vector
+// preconditioner sweep per iteration; the iterate minimises ||r - J P^-1 V y|| over that space, which contains
+// the plain Krylov space of the same depth.  One cycle (no restart): at most (m_max + 1) / t - 1 blocks.
+
+int ensure_block_workspace(sws_solver* s, int t) {
+  if (s->blk_t >= t) return SWS_OK;
+  CU(cudaDeviceSynchronize());
+  if (s->Zb) cudaFree(s->Zb);
+  if (s->hblk) cudaFree(s->hblk);
+  if (s->hblk_pin) cudaFreeHost(s->hblk_pin);
+  s->Zb = s->Wb = s->hblk = s->hblk_pin = nullptr;
+  s->blk_t = 0;
+  const size_t n = (size_t)s->n;
+  s->hblk_len = (size_t)t * (2 * (size_t)(s->m_max + 1) + 2 * t + 1);
+  cudaError_t e = cudaMalloc(&s->Zb, 2 * (size_t)t * n * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&s->hblk, s->hblk_len * sizeof(double));
+  if (e == cudaSuccess) e = cudaMallocHost(&s->hblk_pin, s->hblk_len * sizeof(double));
+  if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? SWS_ENOMEM : fail_cuda(e, "enlarged GMRES workspace");
+  s->Wb = s->Zb + (size_t)t * n;
+  s->blk_t = t;
+  return SWS_OK;
+}
+
+// Orthogonalise the t vectors W_c (ld n) against the nv basis vectors V (classical Gram-Schmidt, twice) and
+// against one another, in order; the normalised vectors go to Q_c (Q may be W).  Coefficients of column c to
+// hblk + c stride: [h1 | h2] against V, [q1 | q2] against Q_0..Q_{c-1}, then the squared norm.  No host sync.
+void orth_block(sws_solver* s, double* W, int t, const double* V, int nv, double* Q, cudaStream_t st) {
+  const int n = s->n, nvmax = s->m_max + 1;
+  const size_t ld = (size_t)n, stride = 2 * (size_t)nvmax + 2 * t + 1;
+  for (int c = 0; c < t; ++c) {
+    double* w = W + (size_t)c * ld;
+    double* h = s->hblk + (size_t)c * stride;
+    for (int pass = 0; pass < 2; ++pass) {
+      if (nv > 0) {
+        double* hp = h + (size_t)pass * nvmax;
+        k_dots<<<kDotBlocks, kDotThreads, 0, st>>>(V, ld, nv, w, n, s->partial);
+        k_dots_finish<<<(nv + 127) / 128, 128, 0, st>>>(s->partial, kDotBlocks, nv, hp, 0);
+        k_project<<<nblk(n), 256, 0, st>>>(w, V, ld, nv, hp, n);
+      }
+      if (c > 0) {
+        double* qp = h + 2 * (size_t)nvmax + (size_t)pass * t;
+        k_dots<<<kDotBlocks, kDotThreads, 0, st>>>(Q, ld, c, w, n, s->partial);
+        k_dots_finish<<<1, 128, 0, st>>>(s->partial, kDotBlocks, c, qp, 0);
+        k_project<<<nblk(n), 256, 0, st>>>(w, Q, ld, c, qp, n);
+      }
+    }
+    double* nq = h + 2 * (size_t)nvmax + 2 * t;
+    k_dots<<<kDotBlocks, kDotThreads, 0, st>>>(w, ld, 1, w, n, s->partial);
+    k_dots_finish<<<1, 128, 0, st>>>(s->partial, kDotBlocks, 1, nq, 0);
+    k_normalise<<<nblk(n), 256, 0, st>>>(Q + (size_t)c * ld, w, nq, n);
+  }
+}
+
+// returns SWS_OK; *fallback = 1 when a piece of the split right-hand side vanishes (the caller runs plain GMRES)
+int egmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opts* o, double* d,
+           sws_gmres_stats* stats, double* hist, cudaStream_t st, int* fallback) {
+  const int n = s->n, t = o->block;
+  *fallback = 0;
+  if (t < 2 || t > 16 || t > s->max_batch || o->jv_mode < 0 || o->jv_mode > 2 || o->maxit < 1) return SWS_EINVAL;
+  int mb = (s->m_max + 1) / t - 1;
+  if (o->restart / t < mb) mb = o->restart / t;
+  if (mb < 1) return SWS_EINVAL;
+  RC(ensure_block_workspace(s, t));
+  const size_t ld = (size_t)n;
+  const int nvmax = s->m_max + 1;
+  const size_t stride = 2 * (size_t)nvmax + 2 * t + 1;
+  double bnorm = 0.0;
+  RC(norms(s, rhs, &bnorm, nullptr, st));
+  CU(cudaMemsetAsync(d, 0, sizeof(double) * n, st));
+  stats->its = 0; stats->converged = 0; stats->rel_res = 0.0; stats->rhs_norm = bnorm;
+  if (bnorm == 0.0) { stats->converged = 1; return SWS_OK; }
+  if (o->jv_mode == 0) {
+    CU(cudaEventRecord(s->ev[0], st));
+    RC(sws_linearize(s->ctx, u, st));
+    CU(cudaEventRecord(s->ev[1], st));
+    CU(cudaStreamSynchronize(st));
+    float a = 0.f;
+    cudaEventElapsedTime(&a, s->ev[0], s->ev[1]);
+    s->ms_jv += a;
+  }
+  // R0 = V_1 B
+  k_split<<<nblk(n), 256, 0, st>>>(s->V, rhs, n, s->N + 1, s->M, t);
+  orth_block(s, s->V, t, s->V, 0, s->V, st);
+  CU(cudaMemcpyAsync(s->hblk_pin, s->hblk, s->hblk_len * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  const int rows_max = (mb + 1) * t, cols_max = mb * t;
+  std::vector<double> H((size_t)rows_max * cols_max, 0.0), g(rows_max, 0.0), y(cols_max, 0.0);
+  std::vector<double> rc, rs;   // Givens rotations in the order they were made ...
+  std::vector<int> rr;          // ... each acting on rows (rr, rr + 1)
+  auto Hm = [&](int i, int j) -> double& { return H[(size_t)i * cols_max + j]; };
+  {
+    // g = e_1 (x) (B 1): B[i][c] = coefficient of V_i in piece c
+    for (int c = 0; c < t; ++c) {
+      const double* h = s->hblk_pin + (size_t)c * stride;
+      const double rcc = std::sqrt(h[2 * nvmax + 2 * t]);
+      if (!(rcc > 0.0)) { *fallback = 1; return SWS_OK; }
+      for (int i = 0; i < c; ++i) g[i] += h[2 * nvmax + i] + h[2 * nvmax + t + i];
+      g[c] += rcc;
+    }
+  }
+  double rel = 1.0;
+  int blocks = 0;
+  bool broke = false;
+  for (int j = 0; j < mb && !broke; ++j) {
+    const int nv = (j + 1) * t;
+    CU(cudaEventRecord(s->ev[0], st));
+    if (s->pc) {
+      s->n_pc += t;
+      RC(sws_precond_apply_multi(s->pc, s->V + (size_t)j * t * ld, t, s->Zb, st));
+    } else {
+      CU(cudaMemcpyAsync(s->Zb, s->V + (size_t)j * t * ld, sizeof(double) * t * ld, cudaMemcpyDeviceToDevice, st));
+    }
+    CU(cudaEventRecord(s->ev[1], st));
+    s->n_jv += t;
+    if (o->jv_mode == 0) RC(sws_jv_apply(s->ctx, s->Zb, t, s->Wb, st));   // ONE call, t products
+    else RC(sws_jv_batch(s->ctx, u, s->Zb, t, nullptr, s->Wb, nullptr, nullptr, st));
+    CU(cudaEventRecord(s->ev[2], st));
+    orth_block(s, s->Wb, t, s->V, nv, s->V + (size_t)nv * ld, st);
+    CU(cudaMemcpyAsync(s->hblk_pin, s->hblk, s->hblk_len * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    {
+      float a = 0.f, b = 0.f;
+      cudaEventElapsedTime(&a, s->ev[0], s->ev[1]);
+      cudaEventElapsedTime(&b, s->ev[1], s->ev[2]);
+      s->ms_pc += a; s->ms_jv += b;
+    }
+    stats->its += t;
+    for (int c = 0; c < t; ++c) {
+      const int col = j * t + c;
+      const double* h = s->hblk_pin + (size_t)c * stride;
+      for (int i = 0; i < nv; ++i) Hm(i, col) = h[i] + h[nvmax + i];
+      for (int i = 0; i < c; ++i) Hm(nv + i, col) = h[2 * nvmax + i] + h[2 * nvmax + t + i];
+      const double rcc = std::sqrt(h[2 * nvmax + 2 * t]);
+      Hm(nv + c, col) = rcc;
+      double hmax = 0.0;
+      for (int i = 0; i < nv + c; ++i) hmax = std::max(hmax, std::fabs(Hm(i, col)));
+      if (!(rcc > 1e-14 * hmax)) broke = true;   // the block lost rank: stop after this block with what was reached
+      for (size_t q = 0; q < rr.size(); ++q) {   // the rotations made so far
+        const int r = rr[q];
+        const double a = Hm(r, col), b = Hm(r + 1, col);
+        Hm(r, col) = rc[q] * a + rs[q] * b;
+        Hm(r + 1, col) = -rs[q] * a + rc[q] * b;
+      }
+      for (int r = col + t; r > col; --r) {      // zero the t entries below the diagonal, bottom up
+        const double a = Hm(r - 1, col), b = Hm(r, col);
+        const double rho = std::hypot(a, b);
+        const double cc = rho > 0.0 ? a / rho : 1.0, ss = rho > 0.0 ? b / rho : 0.0;
+        Hm(r - 1, col) = rho; Hm(r, col) = 0.0;
+        const double ga = g[r - 1], gb = g[r];
+        g[r - 1] = cc * ga + ss * gb;
+        g[r] = -ss * ga + cc * gb;
+        rr.push_back(r - 1); rc.push_back(cc); rs.push_back(ss);
+      }
+    }
+    blocks = j + 1;
+    double res2 = 0.0;
+    for (int i = blocks * t; i < (blocks + 1) * t; ++i) res2 += g[i] * g[i];
+    rel = std::sqrt(res2) / bnorm;
+    if (hist) hist[j] = rel;
+    if (rel <= o->tol || stats->its + t > o->maxit) break;
+  }
+  const int cols = blocks * t;
+  for (int i = cols - 1; i >= 0; --i) {
+    double acc = g[i];
+    for (int k = i + 1; k < cols; ++k) acc -= Hm(i, k) * y[k];
+    y[i] = Hm(i, i) != 0.0 ? acc / Hm(i, i) : 0.0;
+  }
+  // the basis may be longer than ydev (m_max): the combination is formed in slices of m_max vectors
+  for (int off = 0; off < cols; off += s->m_max) {
+    const int cnt = std::min(s->m_max, cols - off);
+    CU(cudaMemcpyAsync(s->ydev, y.data() + off, sizeof(double) * cnt, cudaMemcpyHostToDevice, st));
+    k_lincomb<<<nblk(n), 256, 0, st>>>(off == 0 ? s->t : s->w, s->V + (size_t)off * ld, ld, cnt, s->ydev, n);
+    if (off > 0) k_axpby<<<nblk(n), 256, 0, st>>>(s->t, 1.0, s->t, 1.0, s->w, n);
+    CU(cudaStreamSynchronize(st));
+  }
+  RC(apply_pinv(s, s->t, d, st));
+  CU(cudaStreamSynchronize(st));
+  stats->rel_res = rel;
+  stats->converged = rel <= o->tol ? 1 : 0;
+  CU(cudaGetLastError());
+  return SWS_OK;
+}
+
+// plain GMRES (block <= 1) or enlarged GMRES with opts->block pieces
+int solve_linear(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opts* o, double* d,
+                 sws_gmres_stats* stats, double* hist, cudaStream_t st, const double* E0) {
+  if (o->block >= 2) {
+    int fallback = 0;
+    RC(egmres(s, u, rhs, o, d, stats, hist, st, &fallback));
+    if (!fallback) return SWS_OK;
+  }
+  return gmres(s, u, rhs, o, d, stats, hist, st, E0);
+}
+
 int residual(sws_solver* s, const double* u, double* E, cudaStream_t st) {
   ++s->n_res;
   CU(cudaEventRecord(s->ev[0], st));
@@ -386,6 +603,8 @@ int sws_solver_create(sws_ctx* ctx, sws_precond* pc, int32_t max_restart, sws_so
   sws_solver* s = new (std::nothrow) sws_solver();
   if (!s) return SWS_ENOMEM;
   s->ctx = ctx; s->pc = pc; s->device = p.device;
+  s->N = p.N; s->M = p.M; s->max_batch = p.max_batch;
+  s->blk_t = 0; s->Zb = s->Wb = s->hblk = s->hblk_pin = nullptr; s->hblk_len = 0;
   s->n = (int)sws_num_unknowns(ctx);
   s->m_max = max_restart;
   reset_accounting(s);
@@ -420,7 +639,7 @@ int sws_solver_gmres(sws_solver* s, const double* u_dev, const double* rhs_dev, 
   DevGuard dg(s->device);
   CU(dg.err);
   reset_accounting(s);
-  return gmres(s, u_dev, rhs_dev, opts, d_dev, stats, hist_host, (cudaStream_t)cuda_stream);
+  return solve_linear(s, u_dev, rhs_dev, opts, d_dev, stats, hist_host, (cudaStream_t)cuda_stream, nullptr);
 }
 
 int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sws_newton_log* log, int32_t* nlog,
@@ -447,7 +666,7 @@ int sws_solver_newton(sws_solver* s, double* u_dev, const sws_newton_opts* o, sw
     k_axpby<<<nblk(n), 256, 0, st>>>(s->rhs, -1.0, s->E, 0.0, s->E, n);
     sws_gmres_stats gs;
     go.tol = eta_k;
-    RC(gmres(s, u_dev, s->rhs, &go, s->du, &gs, nullptr, st, s->E));
+    RC(solve_linear(s, u_dev, s->rhs, &go, s->du, &gs, nullptr, st, s->E));
     double lam = 1.0, fnt = 0.0, finft = 0.0;
     bool ok = false;
     for (int hv = 0; hv <= o->max_halvings; ++hv) {
@@ -514,6 +733,9 @@ int sws_solver_destroy(sws_solver* s) {
   if (s->hdev) cudaFree(s->hdev);
   if (s->ydev) cudaFree(s->ydev);
   if (s->hpin) cudaFreeHost(s->hpin);
+  if (s->Zb) cudaFree(s->Zb);
+  if (s->hblk) cudaFree(s->hblk);
+  if (s->hblk_pin) cudaFreeHost(s->hblk_pin);
   for (int i = 0; i < 4; ++i)
     if (s->ev[i]) cudaEventDestroy(s->ev[i]);
   delete s;

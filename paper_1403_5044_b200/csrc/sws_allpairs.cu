@@ -258,6 +258,10 @@ __global__ void __launch_bounds__(kThreads64, MINB) k_allpairs(const PairArgs a)
   uint64_t* s_bar = reinterpret_cast<uint64_t*>(s_y + (size_t)kStages * seg_pad);       // [kStages]
 
   const int tid = threadIdx.x;
+  // Programmatic dependent launch: this grid may have been scheduled while the kernel that produces the source /
+  // target records was still in its last phase (it said so with griddepcontrol.launch_dependents); nothing of
+  // global memory is touched before that kernel has completed and flushed.  A no-op otherwise.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   // With fused assembly (tile_count != NULL) CTA row y = 0 is the LOCAL row: it evaluates a5 + a6's local part
   // (the closed form I: 8 asinh per target) for the tile while the other rows walk their column groups.
   const int tile = blockIdx.x, chunk = (int)blockIdx.y - (a.tile_count ? 1 : 0), state0 = blockIdx.z * NS;
@@ -559,11 +563,17 @@ cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaSt
   const int ns = pair_ns(c, states), nt = pair_nt(c);
   dim3 grid(plan.tiles, plan.chunks + (a.tile_count ? 1 : 0), (states + ns - 1) / ns);
   const size_t smem = allpairs_smem_bytes(plan, ns);
-  if (nt == 2 && ns == 2) k_allpairs<kMinB22, 2, 2><<<grid, kThreads64, smem, st>>>(a);
-  else if (nt == 2) k_allpairs<kMinB2, 2, 1><<<grid, kThreads64, smem, st>>>(a);
-  else if (ns == 2) k_allpairs<kMinB12, 1, 2><<<grid, kThreads64, smem, st>>>(a);
-  else k_allpairs<kMinB, 1, 1><<<grid, kThreads64, smem, st>>>(a);
-  return cudaGetLastError();
+  // launched with programmatic stream serialisation allowed: see griddepcontrol.wait at the top of the kernel
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = dim3(kThreads64); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  if (nt == 2 && ns == 2) return cudaLaunchKernelEx(&cfg, k_allpairs<kMinB22, 2, 2>, a);
+  if (nt == 2) return cudaLaunchKernelEx(&cfg, k_allpairs<kMinB2, 2, 1>, a);
+  if (ns == 2) return cudaLaunchKernelEx(&cfg, k_allpairs<kMinB12, 1, 2>, a);
+  return cudaLaunchKernelEx(&cfg, k_allpairs<kMinB, 1, 1>, a);
 }
 
 // --- far-field statistics (bench.py: executed work of a launch) ----------------------------

@@ -378,6 +378,7 @@ __global__ void __launch_bounds__(128) k_targets(Mesh m, const double* __restric
                                                  const double* __restrict__ py, SrcRec* src,
                                                  SrcRecF* srcf, TgtRec* tgt, double* e2loc, double4* tgtI,
                                                  double* F0, double* Fpert) {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // see k_fields_fused
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= m.N) return;
   target_node(m, k, blockIdx.y, blockIdx.z, x, y, zeta, phi, zx, px, zy, py, src, srcf, tgt, e2loc, tgtI, F0, Fpert);
@@ -428,6 +429,9 @@ __global__ void __launch_bounds__(256) k_fields_fused(const FusedArgs a) {
                       a.zy, a.py);
   }
   grid.sync();
+  // the all-pairs launch that follows may be scheduled from here on (it waits for this grid to complete before it
+  // reads anything: griddepcontrol.wait at its top), which hides its launch latency behind phase 3
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   // phase 3: midpoints, A/B/C, Bernoulli rows, closed-form I, source/target records: one node per thread pass
   const size_t total = (size_t)m.S * a.states;
   for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {

@@ -14,7 +14,7 @@ from . import SWS_ECUDA, SWS_OK, Context, SwsError, SwsParams, load_library
 LIB_PATH = Path(__file__).resolve().parent / "libsws_jfnk.so"
 
 SYMBOLS = (
-    "sws_precond_create", "sws_precond_apply", "sws_precond_block_host", "sws_precond_bytes",
+    "sws_precond_create", "sws_precond_apply", "sws_precond_apply_multi", "sws_precond_block_host", "sws_precond_bytes",
     "sws_precond_bandwidth", "sws_precond_setup_ms", "sws_precond_destroy",
     "sws_solver_create", "sws_solver_gmres", "sws_solver_newton", "sws_solver_continuation", "sws_solver_destroy",
     "sws_jfnk_last_error", "sws_solver_last_error",
@@ -22,7 +22,8 @@ SYMBOLS = (
 
 
 class GmresOpts(C.Structure):
-    _fields_ = [("tol", C.c_double), ("restart", C.c_int32), ("maxit", C.c_int32), ("jv_mode", C.c_int32)]
+    _fields_ = [("tol", C.c_double), ("restart", C.c_int32), ("maxit", C.c_int32), ("jv_mode", C.c_int32),
+                ("block", C.c_int32)]
 
 
 class GmresStats(C.Structure):
@@ -60,6 +61,7 @@ def load_jfnk() -> C.CDLL:
     proto = {
         "sws_precond_create": (C.c_int, [C.POINTER(SwsParams), C.c_int32, C.c_int32, C.POINTER(vp)]),
         "sws_precond_apply": (C.c_int, [vp, dp, dp, vp]),
+        "sws_precond_apply_multi": (C.c_int, [vp, dp, C.c_int32, dp, vp]),
         "sws_precond_block_host": (C.c_int, [vp, C.c_int32, C.c_int32, C.c_int32, dp]),
         "sws_precond_bytes": (C.c_size_t, [vp]),
         "sws_precond_bandwidth": (C.c_int, [vp]),
@@ -142,6 +144,16 @@ class Preconditioner:
         _check(self.lib.sws_precond_apply(self._h, v.data_ptr(), out.data_ptr(), _stream(stream)), "sws_precond_apply")
         return out
 
+    def apply_multi(self, V, out=None, stream=None):
+        """P^-1 v_q for the t rows of V [t, n] in one sweep over the factor panels (sws_precond_apply_multi)."""
+        import torch
+        assert V.is_cuda and V.dtype == torch.float64 and V.is_contiguous() and V.dim() == 2 and V.shape[1] == self.n
+        if out is None:
+            out = torch.empty_like(V)
+        _check(self.lib.sws_precond_apply_multi(self._h, V.data_ptr(), int(V.shape[0]), out.data_ptr(),
+                                                _stream(stream)), "sws_precond_apply_multi")
+        return out
+
     def block(self, which: int, l: int, m: int) -> np.ndarray:
         out = np.empty((self.n1, self.n1))
         _check(self.lib.sws_precond_block_host(self._h, int(which), int(l), int(m), out.ctypes.data_as(C.c_void_p)),
@@ -189,11 +201,12 @@ class Solver:
         self.close()
 
     def gmres(self, u, rhs, tol: float, restart: int | None = None, maxit: int = 200, jv_mode: int = 0,
-              stream=None):
-        """Solve J(u) d = rhs; returns (d, stats dict, history array)."""
+              block: int = 0, stream=None):
+        """Solve J(u) d = rhs; returns (d, stats dict, history array).  block = t >= 2: enlarged GMRES with t
+        pieces (history then has one entry per block iteration)."""
         import torch
         restart = self.max_restart if restart is None else int(restart)
-        o = GmresOpts(float(tol), restart, int(maxit), int(jv_mode))
+        o = GmresOpts(float(tol), restart, int(maxit), int(jv_mode), int(block))
         st = GmresStats()
         hist = np.full(int(maxit), np.nan)
         d = torch.empty_like(u)
@@ -201,15 +214,16 @@ class Solver:
                                          C.byref(st), hist.ctypes.data_as(C.c_void_p), _stream(stream)),
                "sws_solver_gmres")
         return d, {"its": st.its, "converged": bool(st.converged), "rel_res": st.rel_res,
-                   "rhs_norm": st.rhs_norm}, hist[:st.its]
+                   "rhs_norm": st.rhs_norm}, (hist[:st.its] if block < 2 else hist[~np.isnan(hist)])
 
     def newton(self, u0, ftol: float = 1e-9, eta: float = 1e-3, restart: int | None = None,
                gmres_maxit: int = 200, max_newton: int = 30, alpha: float = 1e-4, max_halvings: int = 20,
-               jv_mode: int = 0, forcing: int = 0, eta_max: float = 0.5, stream=None):
+               jv_mode: int = 0, forcing: int = 0, eta_max: float = 0.5, block: int = 0, stream=None):
         """Damped Newton from u0 (device tensor, not modified); returns (u, log list, stats dict)."""
         restart = self.max_restart if restart is None else int(restart)
         o = NewtonOpts(float(ftol), float(eta), float(alpha), int(max_newton), int(max_halvings),
-                       GmresOpts(float(eta), restart, int(gmres_maxit), int(jv_mode)), int(forcing), float(eta_max))
+                       GmresOpts(float(eta), restart, int(gmres_maxit), int(jv_mode), int(block)), int(forcing),
+                       float(eta_max))
         log = (NewtonLog * (int(max_newton) + 1))()
         nlog = C.c_int32(0)
         st = NewtonStats()
@@ -230,7 +244,7 @@ class Solver:
         number of values that converged).  The context keeps the last epsilon."""
         restart = self.max_restart if restart is None else int(restart)
         o = NewtonOpts(float(ftol), float(eta), float(alpha), int(max_newton), int(max_halvings),
-                       GmresOpts(float(eta), restart, int(gmres_maxit), int(jv_mode)), int(forcing), float(eta_max))
+                       GmresOpts(float(eta), restart, int(gmres_maxit), int(jv_mode), 0), int(forcing), float(eta_max))
         eps = np.ascontiguousarray(eps_values, dtype=np.float64)
         st = (NewtonStats * eps.size)()
         ndone = C.c_int32(0)

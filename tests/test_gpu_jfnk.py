@@ -348,3 +348,80 @@ def test_solve_command_line(mods, oracle64, tmp_path):
     assert np.array_equal(z["zeta"][:, 0], zb[:, 0])                    # zeta_1 is the first unknown of each line
     assert np.allclose(np.diff(z["zeta"], axis=1), 0.5 * 0.4 * (zb[:, 2:] + zb[:, 1:-1]), atol=1e-15)
     assert np.abs(z["zeta"]).max() > 0.02
+
+
+# ---------------------------------------------------------------------------------------
+# Enlarged (block) GMRES: SURVEY.md 8(f)2 "block Krylov that actually uses b > 1"
+def test_precond_apply_multi_equals_single(mods, oracle64):
+    """One sweep over the factor panels for t vectors (tiles of 16/8/4/2/1) = t single-vector applies; the
+    single-vector path still works after the internal vectors were regrown."""
+    import torch
+    sws, jf = mods
+    c = W.CONFIGS[1]
+    p = c.params()
+    rng = np.random.default_rng(12)
+    with jf.Preconditioner(p, bandwidth=7) as pc:
+        v0 = dev(rng.standard_normal(c.n))
+        r0 = pc.apply(v0).cpu().numpy()
+        for t in (2, 7, 16):
+            V = dev(rng.standard_normal((t, c.n)))
+            R = pc.apply_multi(V).cpu().numpy()
+            for q in range(t):
+                ref = pc.apply(V[q].contiguous()).cpu().numpy()
+                assert np.abs(R[q] - ref).max() <= 1e-11 * np.abs(ref).max(), (t, q)
+        assert np.abs(pc.apply(v0).cpu().numpy() - r0).max() <= 1e-12 * np.abs(r0).max()
+        with pytest.raises(sws.SwsError):
+            pc.apply_multi(dev(rng.standard_normal((17, c.n))))
+
+
+@pytest.mark.parametrize("t,jv_mode", [(4, 0), (2, 0), (4, 1)])
+def test_egmres_parity_cfg1(mods, oracle64, oracleC, t, jv_mode):
+    """Enlarged GMRES with t pieces at the seeded nonlinear state of cfg1, block-banded preconditioner: the
+    residual after every block iteration and the iterate against oracle/jfnk.py's plain block Arnoldi (dense
+    oracle Jacobian action, dense oracle preconditioner).  The iterate is the unique minimiser over the block
+    Krylov space, so the two bases (modified vs twice-classical Gram-Schmidt) do not matter."""
+    sws, jf = mods
+    c = W.CONFIGS[0]
+    p = c.params()
+    u = W.state(c)
+    P = OJ.band_truncate(OJ.linear_jacobian(p, oracle64.box_integral), p, 3)
+    res, jv, pinv = _oracle_ops(oracle64, oracleC, p, P)
+    rhs = -res(u)
+    grp = OJ.line_partition(p, t)
+    blocks = 5
+    d_ref, h_ref = OJ.egmres_right(lambda Z: np.stack([jv(u, z) for z in Z]), pinv, rhs, grp, t, 0.0, blocks)
+    with sws.Context(p, max_batch=t) as ctx, jf.Preconditioner(p, bandwidth=3) as pc, jf.Solver(ctx, pc, 160) as s:
+        d, st, hist = s.gmres(dev(u), dev(rhs), tol=0.0, restart=blocks * t, maxit=blocks * t, jv_mode=jv_mode, block=t)
+        d = d.cpu().numpy()
+        # the same solve to convergence, and plain GMRES beside it
+        tol = 1e-9 if jv_mode == 0 else 1e-6
+        d2, st2, hist2 = s.gmres(dev(u), dev(rhs), tol=tol, restart=160, maxit=400, jv_mode=jv_mode, block=t)
+        d1, st1, hist1 = s.gmres(dev(u), dev(rhs), tol=tol, restart=160, maxit=400, jv_mode=jv_mode)
+    assert st["its"] == blocks * t and len(hist) == blocks
+    h_ref = np.array(h_ref)
+    rtol = 1e-5 if jv_mode == 0 else 2e-3           # jv_mode 1: first-order difference quotients
+    big = h_ref > 1e-7
+    assert np.allclose(hist[big], h_ref[big], rtol=rtol)
+    assert np.abs(d - d_ref).max() <= (1e-6 if jv_mode == 0 else 1e-3) * np.abs(d_ref).max()
+    assert st2["converged"] and st1["converged"]
+    assert len(hist2) <= len(hist1)                 # block iterations never exceed plain iterations (nested spaces)
+    if jv_mode == 0:
+        assert np.linalg.norm(jv(u, d2.cpu().numpy()) - rhs) <= 5e-9 * np.linalg.norm(rhs)
+        assert np.abs((d2 - d1).cpu().numpy()).max() <= 1e-6 * np.abs(d_ref).max()
+
+
+def test_newton_with_enlarged_gmres_reaches_the_same_root(mods, oracle64):
+    """The JFNK solve on the 45x13 paper mesh (L247) with enlarged GMRES (t = 4) as the inner solver: same root
+    as with plain GMRES, and it is a root of the oracle's residual."""
+    sws, jf = mods
+    c = W.PAPER_BY_NAME["paper_45x13"]
+    p = c.params()
+    u0 = dev(W.flat_state(c))
+    kw = dict(ftol=1e-10, eta=1e-3, restart=48, gmres_maxit=96)
+    with sws.Context(p, max_batch=4) as ctx, jf.Preconditioner(p, bandwidth=5) as pc, jf.Solver(ctx, pc, 60) as s:
+        u1, log1, st1 = s.newton(u0, **kw)
+        u4, log4, st4 = s.newton(u0, block=4, **kw)
+    assert st1["converged"] and st4["converged"]
+    assert float((u1 - u4).abs().max()) <= 1e-8
+    assert np.abs(oracle64.residual(p, u4.cpu().numpy())).max() <= 1e-9
+    assert st4["jv_products"] % 4 == 0

@@ -298,3 +298,55 @@ def test_oracle_root_is_the_kelvin_wave_pattern(oracle64, oracleC):
     assert quiet3 <= 0.12 and quiet2 <= 0.12               # waves trail the source
     lam9, _ = _centreline_waves(oracle64, oracleC, 91, 11, 0.3, -9.0, 0.9)
     assert lam9 / lam3 == pytest.approx((0.9 / 0.7) ** 2, rel=0.10)
+
+
+# ----------------------------------------------------------------------------
+# Enlarged (block) GMRES: SURVEY 8(f)2 "block Krylov that actually uses b > 1"
+# ----------------------------------------------------------------------------
+def _groups(n, t):
+    return (np.arange(n) * t) // n
+
+
+def test_egmres_with_one_piece_is_gmres():
+    A, Pm, b = _system(n=50, seed=7)
+    Pinv = np.linalg.inv(Pm)
+    d1, h1 = J.gmres_right(lambda v: A @ v, lambda v: Pinv @ v, b, 0.0, restart=8, maxit=8)
+    d2, h2 = J.egmres_right(lambda Z: Z @ A.T, lambda v: Pinv @ v, b, _groups(50, 1), 1, 0.0, 8)
+    assert np.allclose(h1, h2, rtol=1e-9, atol=1e-14)
+    assert np.allclose(d1, d2, rtol=1e-9, atol=1e-12)
+
+
+@pytest.mark.parametrize("t", [2, 4, 8])
+def test_egmres_minimises_over_the_block_krylov_space(t):
+    """After m block iterations the iterate minimises ||b - A P^-1 z|| over the block Krylov space
+    span{(A P^-1)^i T_c b}: compared with a least-squares solve on the explicit block Krylov matrix; the
+    space contains K_m(A P^-1, b), so the residual is no larger than plain GMRES's after m products; the
+    reported history is the true residual; at m t = n the solve is exact."""
+    n = 48
+    A, Pm, b = _system(n=n, seed=13, cond_shift=2.0)
+    Pinv = np.linalg.inv(Pm)
+    Bm = A @ Pinv
+    grp = _groups(n, t)
+    m = 3
+    d, hist = J.egmres_right(lambda Z: Z @ A.T, lambda v: Pinv @ v, b, grp, t, 0.0, m)
+    pieces = [np.where(grp == c, b, 0.0) for c in range(t)]
+    K = np.stack([np.linalg.matrix_power(Bm, i) @ pc for i in range(m) for pc in pieces], axis=1)
+    y, *_ = np.linalg.lstsq(Bm @ K, b, rcond=None)
+    best = np.linalg.norm(b - Bm @ K @ y) / np.linalg.norm(b)
+    assert hist[-1] == pytest.approx(best, rel=1e-6, abs=1e-13)
+    assert np.linalg.norm(b - A @ d) / np.linalg.norm(b) == pytest.approx(hist[-1], rel=1e-6, abs=1e-13)
+    assert np.allclose(d, Pinv @ (K @ y), rtol=1e-6, atol=1e-9)
+    _, hp = J.gmres_right(lambda v: A @ v, lambda v: Pinv @ v, b, 0.0, restart=m, maxit=m)
+    assert hist[-1] <= hp[-1] * (1 + 1e-9)
+    assert all(b2 <= b1 * (1 + 1e-12) for b1, b2 in zip(hist, hist[1:]))
+    dfull, hfull = J.egmres_right(lambda Z: Z @ A.T, lambda v: Pinv @ v, b, grp, t, 1e-12, n // t)
+    assert hfull[-1] <= 1e-12 and np.allclose(dfull, np.linalg.solve(A, b), rtol=1e-8, atol=1e-10)
+
+
+def test_line_partition_groups_whole_lines():
+    p = dict(N=5, M=7)
+    g = J.line_partition(p, 3)
+    assert g.shape == (2 * 6 * 7,)
+    blk = g[:42].reshape(7, 6)
+    assert (blk == blk[:, :1]).all() and np.array_equal(g[:42], g[42:])       # a line's phi and zeta unknowns together
+    assert np.array_equal(blk[:, 0], [0, 0, 0, 1, 1, 2, 2])
