@@ -44,7 +44,11 @@ typedef struct sws_solver sws_solver;   /* opaque */
  * y-derivative scheme do not enter, App. B) on p->device, truncate D to block bandwidth
  * `bandwidth` (odd; b = 1 block diagonal, 3 block tridiagonal, ...; <= 0 or >= 2M-1 keeps all
  * of D) and factorise.  flags bit 0: do NOT factorise (the blocks stay as assembled; only
- * sws_precond_block_host is then valid).  Synchronises.  SWS_ENOMEM if the band does not fit. */
+ * sws_precond_block_host is then valid).  flags bit 1: store the factor panels in FP32 (the block LU itself
+ * stays FP64; the apply streams half the bytes and accumulates in FP64; P^-1 v then carries a relative error of
+ * ~1e-7 x the conditioning of the Schur complement instead of ~1e-16 x: enough for a preconditioner - the GMRES
+ * iteration counts of the paper's meshes are unchanged, DESIGN.md - not for a direct solve).  Synchronises.
+ * SWS_ENOMEM if the band does not fit. */
 int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sws_precond** out);
 
 /* r_dev[0..n) = P^-1 v_dev[0..n), n = 2(N+1)M, App. C L511-513.  v and r may alias.

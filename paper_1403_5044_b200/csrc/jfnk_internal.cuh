@@ -54,8 +54,9 @@ struct sws_precond {
   // device
   double* G;       // [n1][n1] column-major: C_0 A_0^-1 B_0 (the block every diagonal block of the Schur complement loses)
   double* corr;    // [T] (sum_ij w K3 - I) / 2 per target, t = l (N-1) + (k-1)        (B.6) L499
-  double* fwd;     // per block row k: row-major [n1][(lk+1) n1] = [ -S~kk^-1 L~k,k-lk..k-1 | S~kk^-1 ]
-  double* bwd;     // per block row k: row-major [n1][uk n1]     = S~kk^-1 S~k,k+1..k+uk
+  void* fwd;       // per block row k: row-major [n1][(lk+1) n1] = [ -S~kk^-1 L~k,k-lk..k-1 | S~kk^-1 ]
+  void* bwd;       // per block row k: row-major [n1][uk n1]     = S~kk^-1 S~k,k+1..k+uk
+  int f32;         // the two panels are stored in FP32 (flags bit 1): the factorisation itself is FP64
   std::vector<size_t> fwd_off, bwd_off;  // element offsets of row k's panels
   double* s1;      // [H]  A^-1 b1
   double* t2;      // [H]  b2 - C s1

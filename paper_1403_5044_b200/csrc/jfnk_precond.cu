@@ -235,6 +235,80 @@ __device__ __forceinline__ double row_dot(const double* __restrict__ row, const 
   return (acc0 + acc1) + (acc2 + acc3);
 }
 
+// The same with the panel stored in FP32 (sws_precond_create flags bit 1): half the bytes to stream; the vector
+// and the accumulation stay FP64.  8-byte loads of two panel entries (K even, rows 8-byte aligned), eight in
+// flight per thread.
+__device__ __forceinline__ double row_dot_f32(const float* __restrict__ row, const double* __restrict__ x, int K) {
+  double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+  if ((K & 1) == 0 && ((reinterpret_cast<uintptr_t>(row) | reinterpret_cast<uintptr_t>(x)) & 7) == 0 &&
+      (reinterpret_cast<uintptr_t>(x) & 15) == 0) {
+    const float2* r2 = reinterpret_cast<const float2*>(row);
+    const double2* x2 = reinterpret_cast<const double2*>(x);
+    const int K2 = K >> 1;
+    int c = threadIdx.x;
+    for (; c + 7 * kGemvThreads < K2; c += 8 * kGemvThreads) {
+      float2 a[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) a[i] = __ldcs(r2 + c + i * kGemvThreads);
+#pragma unroll
+      for (int i = 0; i < 8; i += 4) {
+        const double2 b0 = x2[c + i * kGemvThreads], b1 = x2[c + (i + 1) * kGemvThreads],
+                      b2 = x2[c + (i + 2) * kGemvThreads], b3 = x2[c + (i + 3) * kGemvThreads];
+        acc0 = fma((double)a[i].x, b0.x, acc0); acc0 = fma((double)a[i].y, b0.y, acc0);
+        acc1 = fma((double)a[i + 1].x, b1.x, acc1); acc1 = fma((double)a[i + 1].y, b1.y, acc1);
+        acc2 = fma((double)a[i + 2].x, b2.x, acc2); acc2 = fma((double)a[i + 2].y, b2.y, acc2);
+        acc3 = fma((double)a[i + 3].x, b3.x, acc3); acc3 = fma((double)a[i + 3].y, b3.y, acc3);
+      }
+    }
+    for (; c < K2; c += kGemvThreads) {
+      const float2 a0 = __ldcs(r2 + c);
+      const double2 b0 = x2[c];
+      acc0 = fma((double)a0.x, b0.x, acc0); acc0 = fma((double)a0.y, b0.y, acc0);
+    }
+  } else {
+    for (int c = threadIdx.x; c < K; c += kGemvThreads) acc0 = fma((double)row[c], x[c], acc0);
+  }
+  return (acc0 + acc1) + (acc2 + acc3);
+}
+
+__global__ void __launch_bounds__(kGemvThreads) k_fwd_row_f32(const float* __restrict__ panel, int n1, int lk,
+                                                              const double* __restrict__ yprev,
+                                                              const double* __restrict__ tk, double* __restrict__ yk) {
+  __shared__ double red[kGemvThreads / 32];
+  const int r = blockIdx.x;
+  const int K0 = lk * n1;
+  const float* row = panel + (size_t)r * (K0 + n1);
+  const double s = cta_sum(row_dot_f32(row, yprev, K0) + row_dot_f32(row + K0, tk, n1), red);
+  if (threadIdx.x == 0) yk[r] = s;
+}
+
+__global__ void __launch_bounds__(kGemvThreads) k_bwd_row_f32(const float* __restrict__ panel, int n1, int uk,
+                                                              const double* __restrict__ xnext, double* __restrict__ yk) {
+  __shared__ double red[kGemvThreads / 32];
+  const int r = blockIdx.x;
+  const int K = uk * n1;
+  const double s = cta_sum(row_dot_f32(panel + (size_t)r * K, xnext, K), red);
+  if (threadIdx.x == 0) yk[r] -= s;
+}
+
+// out (row-major, row stride ldo, type PT) [r][c] = scale * in (column-major, n1 rows) (r, c), c < cols: the
+// transposing (and, for FP32 panels, converting) copy of a factor block into the apply form
+template <typename PT>
+__global__ void k_to_apply_form(const double* __restrict__ in, int n1, int cols, double scale, PT* __restrict__ out,
+                                size_t ldo) {
+  __shared__ double tile[32][33];
+  const int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    const int r = r0 + threadIdx.x, c = c0 + j;
+    if (r < n1 && c < cols) tile[j][threadIdx.x] = in[(size_t)c * n1 + r];
+  }
+  __syncthreads();
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    const int r = r0 + j, c = c0 + threadIdx.x;
+    if (r < n1 && c < cols) out[(size_t)r * ldo + c] = (PT)(scale * tile[threadIdx.x][j]);
+  }
+}
+
 // y_k = [ -W_k | Sinv_k ] [ y_{k-lk..k-1} ; t_k ]      (forward: L~ y = t with unit... see header)
 template <bool VEC>
 __global__ void __launch_bounds__(kGemvThreads) k_fwd_row(const double* __restrict__ panel, int n1, int lk,
@@ -264,12 +338,12 @@ __global__ void __launch_bounds__(kGemvThreads) k_bwd_row(const double* __restri
 // The same sweeps for T right-hand sides at once (enlarged GMRES: one sweep over the factor panels serves the T
 // vectors of a block, so the panels - 30 GB at 721x241 - are streamed once instead of T times).  Vector q of a
 // buffer starts at base + q ldv.  One CTA per matrix row, the row read once, T accumulators per thread.
-template <int T>
-__device__ __forceinline__ void row_dot_multi(const double* __restrict__ row, const double* __restrict__ x, size_t ldv,
+template <int T, typename PT>
+__device__ __forceinline__ void row_dot_multi(const PT* __restrict__ row, const double* __restrict__ x, size_t ldv,
                                               int K, double (&acc)[T]) {
   int c = threadIdx.x;
   for (; c + kGemvThreads < K; c += 2 * kGemvThreads) {
-    const double a0 = __ldcs(row + c), a1 = __ldcs(row + c + kGemvThreads);
+    const double a0 = (double)__ldcs(row + c), a1 = (double)__ldcs(row + c + kGemvThreads);
 #pragma unroll
     for (int q = 0; q < T; ++q) {
       acc[q] = fma(a0, x[q * ldv + c], acc[q]);
@@ -277,7 +351,7 @@ __device__ __forceinline__ void row_dot_multi(const double* __restrict__ row, co
     }
   }
   for (; c < K; c += kGemvThreads) {
-    const double a0 = __ldcs(row + c);
+    const double a0 = (double)__ldcs(row + c);
 #pragma unroll
     for (int q = 0; q < T; ++q) acc[q] = fma(a0, x[q * ldv + c], acc[q]);
   }
@@ -301,26 +375,26 @@ __device__ __forceinline__ void cta_sum_multi(double (&acc)[T], double* red /* [
   }
 }
 
-template <int T>
-__global__ void __launch_bounds__(kGemvThreads) k_fwd_row_multi(const double* __restrict__ panel, int n1, int lk,
+template <int T, typename PT>
+__global__ void __launch_bounds__(kGemvThreads) k_fwd_row_multi(const PT* __restrict__ panel, int n1, int lk,
                                                                 const double* __restrict__ yprev,
                                                                 const double* __restrict__ tk,
                                                                 double* __restrict__ yk, size_t ldv) {
   __shared__ double red[T * (kGemvThreads / 32)];
   const int r = blockIdx.x;
   const int K0 = lk * n1;
-  const double* row = panel + (size_t)r * (K0 + n1);
+  const PT* row = panel + (size_t)r * (K0 + n1);
   double acc[T];
 #pragma unroll
   for (int q = 0; q < T; ++q) acc[q] = 0.0;
-  row_dot_multi<T>(row, yprev, ldv, K0, acc);
-  row_dot_multi<T>(row + K0, tk, ldv, n1, acc);
+  row_dot_multi<T, PT>(row, yprev, ldv, K0, acc);
+  row_dot_multi<T, PT>(row + K0, tk, ldv, n1, acc);
   cta_sum_multi<T>(acc, red);
   if (threadIdx.x < T) yk[threadIdx.x * ldv + r] = acc[0];
 }
 
-template <int T>
-__global__ void __launch_bounds__(kGemvThreads) k_bwd_row_multi(const double* __restrict__ panel, int n1, int uk,
+template <int T, typename PT>
+__global__ void __launch_bounds__(kGemvThreads) k_bwd_row_multi(const PT* __restrict__ panel, int n1, int uk,
                                                                 const double* __restrict__ xnext,
                                                                 double* __restrict__ yk, size_t ldv) {
   __shared__ double red[T * (kGemvThreads / 32)];
@@ -329,7 +403,7 @@ __global__ void __launch_bounds__(kGemvThreads) k_bwd_row_multi(const double* __
   double acc[T];
 #pragma unroll
   for (int q = 0; q < T; ++q) acc[q] = 0.0;
-  row_dot_multi<T>(panel + (size_t)r * K, xnext, ldv, K, acc);
+  row_dot_multi<T, PT>(panel + (size_t)r * K, xnext, ldv, K, acc);
   cta_sum_multi<T>(acc, red);
   if (threadIdx.x < T) yk[threadIdx.x * ldv + r] -= acc[0];
 }
@@ -415,21 +489,28 @@ void host_G(const LinMesh& m, std::vector<double>& G) {
 
 }  // namespace
 
-template <int T>
-static void launch_sweeps_multi(sws_precond* pc, cudaStream_t st) {
+template <int T, typename PT>
+static void launch_sweeps_multi_t(sws_precond* pc, cudaStream_t st) {
   const int n1 = pc->lm.n1, M = pc->lm.M, hb = pc->hb;
   const size_t ldv = (size_t)pc->lm.H;
+  const PT* fwd = static_cast<const PT*>(pc->fwd);
+  const PT* bwd = static_cast<const PT*>(pc->bwd);
   for (int k = 0; k < M; ++k) {
     const int lk = k < hb ? k : hb;
-    k_fwd_row_multi<T><<<n1, kGemvThreads, 0, st>>>(pc->fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
-                                                    pc->t2 + (size_t)k * n1, pc->y + (size_t)k * n1, ldv);
+    k_fwd_row_multi<T, PT><<<n1, kGemvThreads, 0, st>>>(fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
+                                                        pc->t2 + (size_t)k * n1, pc->y + (size_t)k * n1, ldv);
   }
   for (int k = M - 2; k >= 0; --k) {
     const int uk = (M - 1 - k) < hb ? (M - 1 - k) : hb;
     if (uk > 0)
-      k_bwd_row_multi<T><<<n1, kGemvThreads, 0, st>>>(pc->bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
-                                                      pc->y + (size_t)k * n1, ldv);
+      k_bwd_row_multi<T, PT><<<n1, kGemvThreads, 0, st>>>(bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
+                                                          pc->y + (size_t)k * n1, ldv);
   }
+}
+template <int T>
+static void launch_sweeps_multi(sws_precond* pc, cudaStream_t st) {
+  if (pc->f32) launch_sweeps_multi_t<T, float>(pc, st);
+  else launch_sweeps_multi_t<T, double>(pc, st);
 }
 
 extern "C" {
@@ -462,7 +543,9 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
   pc->hb = hb;
   pc->factored = 0;
   pc->bytes = 0;
-  pc->G = pc->corr = pc->fwd = pc->bwd = pc->s1 = pc->t2 = pc->y = pc->panel = nullptr;
+  pc->G = pc->corr = pc->s1 = pc->t2 = pc->y = pc->panel = nullptr;
+  pc->fwd = pc->bwd = nullptr;
+  pc->f32 = (flags & 2) ? 1 : 0;
   pc->multi_cap = 1;
 
   const int n1 = m.n1, M = m.M, T = (m.N - 1) * M;
@@ -503,9 +586,10 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
       pc->bwd_off[k] = bo; bo += blk * uk;
     }
     pc->fwd_off[M] = fo; pc->bwd_off[M] = bo;
-    CK(cudaMalloc(&pc->fwd, fo * sizeof(double)));
-    CK(cudaMalloc(&pc->bwd, (bo ? bo : 1) * sizeof(double)));
-    pc->bytes += (fo + bo) * sizeof(double);
+    const size_t esz = pc->f32 ? sizeof(float) : sizeof(double);
+    CK(cudaMalloc(&pc->fwd, fo * esz));
+    CK(cudaMalloc(&pc->bwd, (bo ? bo : 1) * esz));
+    pc->bytes += (fo + bo) * esz;
 
     // factorisation scratch (freed below)
     const int R = hb + 1;  // live block rows
@@ -537,15 +621,27 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
       k_identity<<<(int)((blk + 255) / 256), 256, 0, st>>>(Sinv, n1);
       CK(cudaGetLastError());
       CKB(cusolverDnDgetrs(hb_sol, CUBLAS_OP_N, n1, n1, Dkk, n1, ipiv, Sinv, n1, info + 2 * k + 1));
-      double* Fk = pc->fwd + pc->fwd_off[k];  // row-major [n1][(lk+1) n1] == column-major [(lk+1) n1][n1]
+      // apply form of block row k: row-major [n1][(lk+1) n1] = [ -S~kk^-1 L~k,* | S~kk^-1 ] and [n1][uk n1] =
+      // S~kk^-1 S~k,*, written by a transposing copy that also converts when the panels are FP32
       const int Kf = (lk + 1) * n1;
+      const dim3 tb(32, 8);
+      auto to_apply = [&](const double* in, int cols, double scale, size_t off_elems, size_t col0, size_t ldo, bool fwd) {
+        const dim3 tg((cols + 31) / 32, (n1 + 31) / 32);
+        if (pc->f32) {
+          float* base = static_cast<float*>(fwd ? pc->fwd : pc->bwd) + off_elems + col0;
+          k_to_apply_form<float><<<tg, tb, 0, st>>>(in, n1, cols, scale, base, ldo);
+        } else {
+          double* base = static_cast<double*>(fwd ? pc->fwd : pc->bwd) + off_elems + col0;
+          k_to_apply_form<double><<<tg, tb, 0, st>>>(in, n1, cols, scale, base, ldo);
+        }
+      };
       if (lk > 0) {
         const double* Lk = Pk + blk * (hb - lk);  // L~k,k-lk..k-1, column-major n1 x lk n1
         CKB(cublasDgemm(hb_blas, CUBLAS_OP_N, CUBLAS_OP_N, n1, lk * n1, n1, &one, Sinv, n1, Lk, n1, &zero, W, n1));
-        CKB(cublasDgeam(hb_blas, CUBLAS_OP_T, CUBLAS_OP_N, lk * n1, n1, &mone, W, n1, &zero, Fk, Kf, Fk, Kf));
+        to_apply(W, lk * n1, -1.0, pc->fwd_off[k], 0, Kf, true);
       }
-      CKB(cublasDgeam(hb_blas, CUBLAS_OP_T, CUBLAS_OP_N, n1, n1, &one, Sinv, n1, &zero, Fk + (size_t)lk * n1, Kf,
-                      Fk + (size_t)lk * n1, Kf));
+      to_apply(Sinv, n1, 1.0, pc->fwd_off[k], (size_t)lk * n1, Kf, true);
+      CK(cudaGetLastError());
       if (uk > 0) {
         // S~kk^-1 S~k,k+1..k+uk by ONE product with the explicit inverse formed above (a getrs on this
         // wide right-hand side spends most of its time in row interchanges and triangular solves: 60 % of
@@ -553,8 +649,8 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
         const double* Uk0 = Pk + blk * (hb + 1);
         double* Uk = W;  // n1 x uk n1, column-major (W's use for the forward panel above is stream-ordered)
         CKB(cublasDgemm(hb_blas, CUBLAS_OP_N, CUBLAS_OP_N, n1, uk * n1, n1, &one, Sinv, n1, Uk0, n1, &zero, Uk, n1));
-        double* Bk = pc->bwd + pc->bwd_off[k];
-        CKB(cublasDgeam(hb_blas, CUBLAS_OP_T, CUBLAS_OP_N, uk * n1, n1, &one, Uk, n1, &zero, Bk, uk * n1, Bk, uk * n1));
+        to_apply(Uk, uk * n1, 1.0, pc->bwd_off[k], 0, (size_t)uk * n1, false);
+        CK(cudaGetLastError());
         for (int i = k + 1; i <= k + uk; ++i) {
           double* Pi = ring + panel_elems * (i % R);
           const double* Lik = Pi + blk * (k - i + hb);
@@ -599,22 +695,40 @@ done:
 static void launch_sweeps(sws_precond* pc, cudaStream_t st) {
   const int n1 = pc->lm.n1, M = pc->lm.M, hb = pc->hb;
   const bool vec = (n1 % 2) == 0;  // rows, y and t blocks then start on 16-byte boundaries
+  if (pc->f32) {
+    const float* fwd = static_cast<const float*>(pc->fwd);
+    const float* bwd = static_cast<const float*>(pc->bwd);
+    for (int k = 0; k < M; ++k) {
+      const int lk = k < hb ? k : hb;
+      k_fwd_row_f32<<<n1, kGemvThreads, 0, st>>>(fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
+                                                 pc->t2 + (size_t)k * n1, pc->y + (size_t)k * n1);
+    }
+    for (int k = M - 2; k >= 0; --k) {
+      const int uk = (M - 1 - k) < hb ? (M - 1 - k) : hb;
+      if (uk > 0)
+        k_bwd_row_f32<<<n1, kGemvThreads, 0, st>>>(bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
+                                                   pc->y + (size_t)k * n1);
+    }
+    return;
+  }
+  const double* fwd = static_cast<const double*>(pc->fwd);
+  const double* bwd = static_cast<const double*>(pc->bwd);
   for (int k = 0; k < M; ++k) {
     const int lk = k < hb ? k : hb;
     if (vec)
-      k_fwd_row<true><<<n1, kGemvThreads, 0, st>>>(pc->fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
+      k_fwd_row<true><<<n1, kGemvThreads, 0, st>>>(fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
                                                    pc->t2 + (size_t)k * n1, pc->y + (size_t)k * n1);
     else
-      k_fwd_row<false><<<n1, kGemvThreads, 0, st>>>(pc->fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
+      k_fwd_row<false><<<n1, kGemvThreads, 0, st>>>(fwd + pc->fwd_off[k], n1, lk, pc->y + (size_t)(k - lk) * n1,
                                                     pc->t2 + (size_t)k * n1, pc->y + (size_t)k * n1);
   }
   for (int k = M - 2; k >= 0; --k) {
     const int uk = (M - 1 - k) < hb ? (M - 1 - k) : hb;
     if (uk > 0 && vec)
-      k_bwd_row<true><<<n1, kGemvThreads, 0, st>>>(pc->bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
+      k_bwd_row<true><<<n1, kGemvThreads, 0, st>>>(bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
                                                    pc->y + (size_t)k * n1);
     else if (uk > 0)
-      k_bwd_row<false><<<n1, kGemvThreads, 0, st>>>(pc->bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
+      k_bwd_row<false><<<n1, kGemvThreads, 0, st>>>(bwd + pc->bwd_off[k], n1, uk, pc->y + (size_t)(k + 1) * n1,
                                                     pc->y + (size_t)k * n1);
   }
 }
@@ -730,8 +844,8 @@ int sws_precond_destroy(sws_precond* pc) {
   if (!pc) return SWS_OK;
   DevGuard dg(pc->device);
   if (pc->sweep_graph) cudaGraphExecDestroy(pc->sweep_graph);
-  double* bufs[] = {pc->G, pc->corr, pc->fwd, pc->bwd, pc->s1, pc->t2, pc->y, pc->panel};
-  for (double* b : bufs)
+  void* bufs[] = {pc->G, pc->corr, pc->fwd, pc->bwd, pc->s1, pc->t2, pc->y, pc->panel};
+  for (void* b : bufs)
     if (b) cudaFree(b);
   delete pc;
   return SWS_OK;

@@ -110,7 +110,8 @@ class Preconditioner:
     """sws_precond_create / sws_precond_destroy.  bandwidth: odd block bandwidth b (L241);
     0 keeps the whole dense block D."""
 
-    def __init__(self, params: dict, bandwidth: int = 0, device: int = 0, factorise: bool = True):
+    def __init__(self, params: dict, bandwidth: int = 0, device: int = 0, factorise: bool = True,
+                 f32_panels: bool = False):
         self._h = None
         self.lib = load_jfnk()
         self.n1 = int(params["N"]) + 1
@@ -118,7 +119,8 @@ class Preconditioner:
         self.device = int(device)
         h = C.c_void_p()
         p = _params_struct(params, device)
-        _check(self.lib.sws_precond_create(C.byref(p), int(bandwidth), 0 if factorise else 1, C.byref(h)),
+        flags = (0 if factorise else 1) | (2 if f32_panels else 0)   # bit 1: factor panels stored in FP32
+        _check(self.lib.sws_precond_create(C.byref(p), int(bandwidth), flags, C.byref(h)),
                "sws_precond_create")
         self._h = h
 

@@ -36,6 +36,7 @@ def main(argv=None) -> int:
     ap.add_argument("--eta", type=float, default=1e-3)
     ap.add_argument("--restart", type=int, default=60)
     ap.add_argument("--device", type=int, default=0)
+    ap.add_argument("--f64-panels", action="store_true", help="keep the preconditioner's factor panels in FP64 (default FP32)")
     ap.add_argument("--out", default="")
     a = ap.parse_args(argv)
 
@@ -59,7 +60,7 @@ def main(argv=None) -> int:
               forcing=int(a.forcing), eta_max=0.5)
     t0 = time.perf_counter()
     with sws.Context(p, max_batch=1, device=a.device) as ctx, \
-            jf.Preconditioner(p, bandwidth=a.bandwidth, device=a.device) as pc, jf.Solver(ctx, pc, a.restart) as s:
+            jf.Preconditioner(p, bandwidth=a.bandwidth, device=a.device, f32_panels=not a.f64_panels) as pc, jf.Solver(ctx, pc, a.restart) as s:
         t1 = time.perf_counter()
         u, stats, done = s.continuation(torch.from_numpy(u0).cuda(a.device), stages, **kw)
         torch.cuda.synchronize()

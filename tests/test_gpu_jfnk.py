@@ -425,3 +425,32 @@ def test_newton_with_enlarged_gmres_reaches_the_same_root(mods, oracle64):
     assert float((u1 - u4).abs().max()) <= 1e-8
     assert np.abs(oracle64.residual(p, u4.cpu().numpy())).max() <= 1e-9
     assert st4["jv_products"] % 4 == 0
+
+
+def test_f32_panels_precondition_as_well(mods, oracle64):
+    """sws_precond_create flags bit 1: factor panels stored in FP32 (half the bytes per apply).  P^-1 v moves by
+    ~1e-7 x conditioning - far from a direct solve, irrelevant for a preconditioner: the Newton-GMRES histories on
+    the 45x13 and 91x31 paper meshes are the FP64-panel histories, iteration for iteration, same root."""
+    sws, jf = mods
+    rng = np.random.default_rng(5)
+    for name, bw in (("paper_45x13", 5), ("paper_91x31", 15)):
+        c = W.PAPER_BY_NAME[name]
+        p = c.params()
+        u0 = dev(W.flat_state(c))
+        kw = dict(ftol=1e-10, eta=1e-3, restart=40, gmres_maxit=120)
+        V = dev(rng.standard_normal((3, c.n)))
+        with sws.Context(p, max_batch=1) as ctx, jf.Preconditioner(p, bandwidth=bw) as p64, \
+                jf.Preconditioner(p, bandwidth=bw, f32_panels=True) as p32:
+            assert p32.bytes < 0.62 * p64.bytes
+            r64, r32 = p64.apply(V[0].contiguous()), p32.apply(V[0].contiguous())
+            err = float((r64 - r32).abs().max() / r64.abs().max())
+            assert 0.0 < err <= 1e-3, err
+            m32 = p32.apply_multi(V)
+            assert float((m32[0] - r32).abs().max()) <= 1e-11 * float(r32.abs().max())
+            with jf.Solver(ctx, p64, 40) as s64:
+                u64, log64, st64 = s64.newton(u0, **kw)
+            with jf.Solver(ctx, p32, 40) as s32:
+                u32, log32, st32 = s32.newton(u0, **kw)
+        assert st64["converged"] and st32["converged"]
+        assert [e["gmres_its"] for e in log32] == [e["gmres_its"] for e in log64]
+        assert float((u64 - u32).abs().max()) <= 1e-8
