@@ -47,8 +47,8 @@ FP64_INSTR_FAR, FLOPS_FAR = 28, 43
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
 # dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
 # ncu --set full capture summarised in NCU_PROFILE (a static figure: this run does not measure it)
-NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 56.46e6}
-NCU_PROFILE = "profiles/r1e_allpairs_ncu.md"
+NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 160.42e6}
+NCU_PROFILE = "profiles/r2a_allpairs_ncu.md"
 
 
 def dist_env():
@@ -732,6 +732,50 @@ def run_microbench(args) -> None:
                       "rows": rows, "dfma_probe": sws_debug.probe_fp64_peak(0)}), flush=True)
 
 
+def run_experiments(args) -> None:
+    """--experiments: the measurements behind profiles/r2_experiments.md and profiles/r2_small_meshes.md, one JSON
+    line (not a bench value).  batch_sharing: the all-pairs kernel alone for a single state and for the b + 1 states
+    of each config's batch with one and with two states per CTA (sws_set_states_per_cta).  small_meshes:
+    sws_time_residual (evaluations back to back, issued inside the library) with the fused cooperative fields launch
+    and with the three separate launches, and the all-pairs kernel alone."""
+    import torch
+
+    import paper_1403_5044_b200 as sws
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --experiments: no CUDA device")
+    out = {"experiments": "round 2", "batch_sharing": {}, "small_meshes": {}}
+    for name in ("cfg5_721x241", "cfg4_361x121", "cfg3_181x61"):
+        cfg = W.BY_NAME[name]
+        b = cfg.b
+        with sws.Context(cfg.params(), max_batch=b) as ctx:
+            u = torch.from_numpy(W.state(cfg)).cuda()
+            V = torch.from_numpy(W.directions(cfg, b)).cuda()
+            ctx.jv_batch(u, V)
+            torch.cuda.synchronize()
+            one = ctx.time_allpairs(1, 5)
+            row = {"b": b, "single_ms": one}
+            for ns in (1, 2):
+                ctx.set_states_per_cta(ns)
+                ms = ctx.time_allpairs(b + 1, 3)
+                row[f"ns{ns}_ms"] = ms
+                row[f"ns{ns}_over_states_x_single"] = ms / ((b + 1) * one)
+            out["batch_sharing"][name] = row
+    for (N, M, h, x1) in [(31, 11, 0.8, -8.0), (61, 21, 0.4, -8.0), (91, 31, 0.3, -9.0), (181, 61, 0.3, -14.0),
+                          (361, 121, 0.15, -14.0)]:
+        cfg = W.custom(N, M, h, x1, eps=1.0, amp=0.05, seed=40 + N)
+        with sws.Context(cfg.params()) as ctx:
+            u = torch.from_numpy(W.state(cfg)).cuda()
+            F = ctx.residual(u)
+            torch.cuda.synchronize()
+            row = {"allpairs_alone_us": ctx.time_allpairs(1, 50) * 1e3}
+            for fused in (1, 0):
+                ctx.set_fused_fields(bool(fused))
+                row["fused_us" if fused else "separate_us"] = ctx.time_residual(u, F, 100) * 1e3
+                row["launches_fused" if fused else "launches_separate"] = ctx.last_launch_count
+            out["small_meshes"][f"{N}x{M}"] = row
+    print(json.dumps(out), flush=True)
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -748,9 +792,14 @@ def main() -> None:
     ap.add_argument("--no-table1", action="store_true", help="skip the paper's Table 1 meshes")
     ap.add_argument("--no-configs", action="store_true", help="skip the FP64 section on BASELINE configs 1-4")
     ap.add_argument("--microbench", action="store_true", help="only run the FP64 instruction-mix probes")
+    ap.add_argument("--experiments", action="store_true",
+                    help="only run the round-2 experiments (states per CTA, small-mesh launch paths)")
     args = ap.parse_args()
     if args.microbench:
         run_microbench(args)
+        return
+    if args.experiments:
+        run_experiments(args)
         return
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)

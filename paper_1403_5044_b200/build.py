@@ -4,6 +4,7 @@
 """
 from __future__ import annotations
 
+import os
 import shutil
 import subprocess
 import sys
@@ -44,7 +45,9 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not needs_build():
         return LIB
-    cmd = [_nvcc(), *NVCC_FLAGS, f"-I{ROOT / 'include'}"]
+    # SWS_NVCC_EXTRA: extra flags for the build-time experiments of DESIGN.md section 6 (e.g. -DSWS_RSQRT_F32SEED)
+    extra = os.environ.get("SWS_NVCC_EXTRA", "").split()
+    cmd = [_nvcc(), *NVCC_FLAGS, *extra, f"-I{ROOT / 'include'}"]
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += [str(CSRC / s) for s in SOURCES] + ["-Xlinker", "-soname=libsws.so", "-o", str(LIB)]
