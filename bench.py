@@ -38,12 +38,13 @@ import workloads as W  # noqa: E402
 METRIC = "fp64_residual_evals_per_s"
 UNIT = "evals/s"
 # Work of the all-pairs kernel per pair interaction, from its SASS inner loops:
-#   near columns (S2 summed pair by pair): 44 FP64-pipe instructions = 23 DFMA (2 flops) + 21 DMUL/DADD;
-#   far columns (S2 column sum from its Euler-Maclaurin form): 28 = 15 DFMA + 13 DMUL/DADD.
+#   near columns (S2 summed pair by pair): 43 FP64-pipe instructions = 24 DFMA (2 flops) + 19 DMUL/DADD;
+#   far columns (S2 column sum from its Euler-Maclaurin form): 27 = 16 DFMA + 11 DMUL/DADD
+#   (round 2, last session: the cube's third factor and the K2 sum ride the accumulating FMAs; 44 / 28 before).
 # The 216 FP64 instructions (SASS count, sws_farfield.cuh) of the expansion per (target, far column) - 0.9 per
 # pair at M = 241 - are NOT counted as achieved work.
-FP64_INSTR_NEAR, FLOPS_NEAR = 44, 67
-FP64_INSTR_FAR, FLOPS_FAR = 28, 43
+FP64_INSTR_NEAR, FLOPS_NEAR = 43, 67
+FP64_INSTR_FAR, FLOPS_FAR = 27, 43
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
 # dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
 # ncu --set full capture summarised in NCU_PROFILE (a static figure: this run does not measure it)
@@ -362,7 +363,7 @@ def block_krylov_report(sws, jf, device: int, bandwidth: int) -> dict:
     with enlarged GMRES (sws_gmres_opts.block = t pieces of the right-hand side by groups of y-lines, ONE
     sws_jv_apply(V[t]) and ONE t-vector preconditioner sweep per block iteration) for t = 1 (plain GMRES), 4, 16;
     analytic Jv, eta = 1e-3.  pair_instructions = FP64 instructions of the all-pairs kernels to convergence:
-    71 per pair per sws_linearize, 41 + 4 t per pair per sws_jv_apply(t), 28.4 per pair per sws_residual
+    71 per pair per sws_linearize, 41 + 4 t per pair per sws_jv_apply(t), 27.4 per pair per sws_residual
     (SASS counts)."""
     import torch
     cfg = W.PAPER_BY_NAME["paper_721x241"]
@@ -388,7 +389,7 @@ def block_krylov_report(sws, jf, device: int, bandwidth: int) -> dict:
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
             calls = st["jv_products"] // t
-            instr = cfg.pairs * (st["steps"] * 71 + calls * (41 + 4 * t) + st["residual_evals"] * 28.4)
+            instr = cfg.pairs * (st["steps"] * 71 + calls * (41 + 4 * t) + st["residual_evals"] * 27.4)
             out[f"t{t}"] = {"solve_s": dt, "converged": st["converged"], "newton_steps": st["steps"],
                             "jv_products": st["jv_products"], "block_iterations_per_step":
                             [e["gmres_its"] // t for e in log[:-1]], "pair_instructions": instr,

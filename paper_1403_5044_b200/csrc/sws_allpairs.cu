@@ -13,8 +13,8 @@
 // warp reads the same record (shared-memory broadcast), so the kernel is bound by the FP64
 // pipe.  Columns at least 8 dy away from all 32 targets of a warp ("far", 97.8 % at 721x241)
 // take their S2 terms - which do not depend on the source data - from the Euler-Maclaurin form of
-// the column sum (sws_farfield.cuh): 28 FP64 instructions + 2 MUFU.RSQ64H per pair; the others
-// sum S2 pair by pair: 44 + 4.  Everything that depends only on (target, column) - dx, dx^2 and
+// the column sum (sws_farfield.cuh): 27 FP64 instructions + 2 MUFU.RSQ64H per pair; the others
+// sum S2 pair by pair: 43 + 4.  Everything that depends only on (target, column) - dx, dx^2 and
 // the completed-square constants of S2 - is hoisted out of the j loop; the half weights are
 // applied by peeling the first/last node and scaling edge columns, so the inner loop carries no
 // weight multiply.  Partial sums per (state, chunk, target) are written to global memory and
@@ -83,7 +83,7 @@ struct ColS {
 
 // One source node against one target: adds (phi-phi*-x+x*) K1 + zeta_x K2 to a1 and, if S2T,
 // sqrt(C) S2 to aS (unit weight).  S2T = false is the far-field form: the S2 terms of the
-// whole column come from s2_column_em() below, 28 FP64 instructions + 2 MUFU.RSQ64H remain.
+// whole column come from s2_column_em() below, 27 FP64 instructions + 2 MUFU.RSQ64H remain.
 // dm = y_j - y* is passed in: it is geometry, formed once per (target, node) for all states of the CTA.
 template <bool S2T>
 __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, const double yj, const double dm,
@@ -103,12 +103,23 @@ __device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, co
   const double n0 = fma(-cg.dx, zx, dz);
   const double nm = fma(-dm, zy, n0);
   const double np = fma(-tg.ys2, zy, nm);
+  const double dpsi = psi - ts.psis;
+#ifdef SWS_TAIL_CUBES
+  // rounds 1-2: K1 with explicit cubes, then K2; 10 FP64 instructions (-DSWS_TAIL_CUBES, kept for the record)
   const double rm3 = (rm * rm) * rm;
   const double rp3 = (rp * rp) * rp;
   const double k1 = fma(np, rp3, nm * rm3);
-  const double dpsi = psi - ts.psis;
   a1 = fma(dpsi, k1, a1);
   a1 = fma(zx, rm + rp, a1);  // K2 = 1/R- + 1/R+
+#else
+  // dpsi K1 + zeta_x K2 = (1/R-) [zeta_x + dpsi n- / R-^2] + (1/R+) [zeta_x + dpsi n+ / R+^2]: the third factor of
+  // each cube and the K2 sum ride the two accumulating FMAs - 9 FP64 instructions instead of 10 (cfg5: 54.5 -> 53.2 ms)
+  const double bm = dpsi * nm, bp = dpsi * np;
+  const double cm = fma(bm, rm * rm, zx);
+  const double cp = fma(bp, rp * rp, zx);
+  a1 = fma(rm, cm, a1);
+  a1 = fma(rp, cp, a1);
+#endif
   if (S2T) {
     // S2 (eqs. (21), (22)) up to the factor 1/sqrt(C)
     const double sm = yj - cs.c;
