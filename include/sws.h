@@ -200,6 +200,19 @@ int sws_set_tuning(sws_ctx* ctx, int32_t chunks);
  * default (1: measured 4-5 % faster than 2 on B200).  Results do not depend on ns, bit for bit. */
 int sws_set_states_per_cta(sws_ctx* ctx, int32_t ns);
 
+/* The uniform-operand ("constant-bank") form of the all-pairs quadrature, step a4 (eq. (12), same pair
+ * arithmetic as the staged kernel): the source records of a slab of columns are copied into a 64 KB constant bank,
+ * from where the kernel takes them as uniform-register operands of its FP64 instructions (DESIGN.md section 6:
+ * no three-vector-register DFMAs on the source data, no shared-memory loads); one launch per slab, two banks fed
+ * through two library-owned streams that fork from and join the caller's stream (asynchronous as before).
+ * mode -1 (default): used on FP64 meshes with at least 40,000 targets whose columns fit a bank at least four at a
+ * time (M <= 479); 0: never (always the staged kernel); 1: whenever the columns fit (SWS_EINVAL otherwise).
+ * Results are bitwise repeatable in either form and slot b of a batch is bitwise the single evaluation of u_b;
+ * the two forms differ from each other in summation order only (~1e-13 of |F|). */
+int sws_set_const_path(sws_ctx* ctx, int32_t mode);
+/* out = {path active for this context now (0/1), columns per slab, slabs per state, target tiles (CTAs per column)} */
+int sws_const_plan_info(const sws_ctx* ctx, int32_t out[4]);
+
 /* Change the source strength epsilon (eq. (6)) of an existing context: the parameter of the
  * bootstrapping / continuation process of L229.  Nothing else of the set-up depends on it.  A
  * linearisation kept by sws_linearize is invalidated. */

@@ -32,6 +32,10 @@ int sws_probe_fp64_mix(int32_t device, int32_t kind, int32_t warps_per_sm, doubl
 /* y[i] = the library's device reciprocal square root of x[i] (host buffers), for the
  * unit test of that primitive. */
 int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, int32_t n);
+/* The same for the form the pair term uses for 1/R-: the seed's low 32 bits are lo_host[i] instead of zero
+ * (in the kernel: whatever the low word of a dead register pair holds, so that no move follows the MUFU.RSQ64H);
+ * any value must give a result within 1 ulp. */
+int sws_debug_rsqrt_lo_host(int32_t device, const double* x_host, const int32_t* lo_host, double* y_host, int32_t n);
 
 /* Unit test of the far-field expansion: for n pairs (c, g) and the column y1, y1+dy, ..., M nodes,
  * with u-+ = ((y_j -+ c)^2 + g)^-1/2, s-+ = y_j -+ c and c_j = 1/2 at both ends,

@@ -27,6 +27,7 @@ SYMBOLS = (
     "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
     "sws_get_params", "sws_linearize", "sws_jv_apply",
     "sws_set_farfield", "sws_farfield_stats", "sws_set_eps", "sws_get_fields_host", "sws_set_states_per_cta", "sws_time_residual", "sws_set_fused_fields",
+    "sws_set_const_path", "sws_const_plan_info",
 )
 
 
@@ -86,6 +87,8 @@ def load_library() -> C.CDLL:
         "sws_set_farfield": (C.c_int, [vp, C.c_double]),
         "sws_set_eps": (C.c_int, [vp, C.c_double]),
         "sws_set_states_per_cta": (C.c_int, [vp, C.c_int32]),
+        "sws_set_const_path": (C.c_int, [vp, C.c_int32]),
+        "sws_const_plan_info": (C.c_int, [vp, C.POINTER(C.c_int32)]),
         "sws_time_residual": (C.c_int, [vp, dp, dp, C.c_int32, C.POINTER(C.c_float), vp]),
         "sws_set_fused_fields": (C.c_int, [vp, C.c_int32]),
         "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
@@ -328,6 +331,15 @@ class Context:
     def set_states_per_cta(self, ns: int = 0) -> None:
         """sws_set_states_per_cta: states one CTA of a batched all-pairs launch carries (0 default, 1, 2)."""
         _check(self.lib.sws_set_states_per_cta(self._h, int(ns)), "sws_set_states_per_cta")
+
+    def set_const_path(self, mode: int = -1) -> None:
+        """sws_set_const_path: -1 automatic (large meshes), 0 staged kernel only, 1 constant-bank kernel whenever it fits."""
+        _check(self.lib.sws_set_const_path(self._h, int(mode)), "sws_set_const_path")
+
+    def const_plan_info(self) -> dict:
+        out = (C.c_int32 * 4)()
+        _check(self.lib.sws_const_plan_info(self._h, out), "sws_const_plan_info")
+        return dict(active=bool(out[0]), cols_per_slab=out[1], slabs=out[2], tiles=out[3])
 
     def set_eps(self, eps: float) -> None:
         """sws_set_eps: the source strength of the continuation process."""

@@ -17,7 +17,8 @@ LIB = PKG / "libsws.so"
 LIB_JFNK = PKG / "libsws_jfnk.so"  # the Newton-Krylov driver: calls libsws through its C-ABI, + cuBLAS/cuSOLVER
 SOURCES_JFNK = ["jfnk_precond.cu", "jfnk_solver.cu"]
 CUDA_LIB64 = "/usr/local/cuda/lib64"
-SOURCES = ["sws_api.cu", "sws_fields.cu", "sws_allpairs.cu", "sws_allpairs_f32.cu", "sws_jv_exact.cu"]
+SOURCES = ["sws_api.cu", "sws_fields.cu", "sws_allpairs.cu", "sws_allpairs_c0.cu", "sws_allpairs_c1.cu",
+           "sws_allpairs_f32.cu", "sws_jv_exact.cu"]
 # test hooks and FP64 issue-rate probes (include/sws_debug.h): a library of its own, not part of the product
 LIB_DEBUG = PKG / "libsws_debug.so"
 SOURCES_DEBUG = ["sws_debug.cu", "sws_probe.cu"]
@@ -36,7 +37,8 @@ def needs_build() -> bool:
     if not LIB.exists() or not LIB_JFNK.exists() or not LIB_DEBUG.exists():
         return True
     t = min(LIB.stat().st_mtime, LIB_JFNK.stat().st_mtime, LIB_DEBUG.stat().st_mtime)
-    deps = [CSRC / s for s in SOURCES + SOURCES_JFNK + SOURCES_DEBUG] + [ROOT / "include" / "sws_debug.h"] + [CSRC / "sws_internal.cuh", CSRC / "sws_stage.cuh", CSRC / "sws_farfield.cuh",
+    deps = [CSRC / s for s in SOURCES + SOURCES_JFNK + SOURCES_DEBUG] + [ROOT / "include" / "sws_debug.h"] + [CSRC / "sws_internal.cuh", CSRC / "sws_stage.cuh", CSRC / "sws_farfield.cuh", CSRC / "sws_pair.cuh",
+                                                         CSRC / "sws_const.cuh", CSRC / "sws_allpairs_const.cuh", CSRC / "sws_closed_form.cuh",
                                                          CSRC / "jfnk_internal.cuh", ROOT / "include" / "sws.h",
                                                          ROOT / "include" / "sws_jfnk.h"]
     return any(d.stat().st_mtime > t for d in deps)

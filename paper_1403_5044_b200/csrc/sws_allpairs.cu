@@ -19,9 +19,13 @@
 // applied by peeling the first/last node and scaling edge columns, so the inner loop carries no
 // weight multiply.  Partial sums per (state, chunk, target) are written to global memory and
 // added in a fixed order by the assemble kernel: no atomics, bitwise repeatable.
+#include <mutex>
+
 #include "sws_closed_form.cuh"
+#include "sws_const.cuh"
 #include "sws_farfield.cuh"
 #include "sws_internal.cuh"
+#include "sws_pair.cuh"
 #include "sws_stage.cuh"
 
 // build-time tuning of the all-pairs kernel (defaults measured on B200)
@@ -59,76 +63,6 @@ constexpr int kMinB2 = 6;  // resident CTAs per SM of the two-target kernel
 #endif
 constexpr int kMinB12 = SWS_MINB12;  // ... of the one-target, two-state kernel (batches on small meshes)
 constexpr int kMinB22 = SWS_MINB22;  // ... of the two-target, two-state kernel (batches on large meshes)
-
-// Per-thread constants of one target and of the current source column, split into what is GEOMETRY (the same
-// for every state of a batch: the mesh does not move) and what depends on the state.
-// The S2 quadratic forms are used with the square completed (C > 0):
-//   A dx^2 + B dx (y-y*) + C (y-y*)^2 = C [ (y - c)^2 + g ],
-//   A dx^2 - B dx (y+y*) + C (y+y*)^2 = C [ (y + c)^2 + g ],
-//   c = y* - (B / 2C) dx,   g = (A/C - (B/2C)^2) dx^2 = (4AC - B^2) dx^2 / (4 C^2) > 0,
-// so that each form costs one add and one two-register FMA per pair, c and g are per
-// (target, column), and the common factor 1/sqrt(C) is applied once per target at the end.
-struct TgtG {
-  double ys, ys2, ys4;  // y*, 2 y*, 4 y*: the image terms follow from the direct ones (below)
-};
-struct TgtS {
-  double zs, psis;  // zeta*, phi* - x*
-};
-struct ColG {
-  double dx, dx2;  // x_i - x*, its square
-};
-struct ColS {
-  double c, g;  // the S2 constants above (A, B, C belong to the state)
-};
-
-// One source node against one target: adds (phi-phi*-x+x*) K1 + zeta_x K2 to a1 and, if S2T,
-// sqrt(C) S2 to aS (unit weight).  S2T = false is the far-field form: the S2 terms of the
-// whole column come from s2_column_em() below, 27 FP64 instructions + 2 MUFU.RSQ64H remain.
-// dm = y_j - y* is passed in: it is geometry, formed once per (target, node) for all states of the CTA.
-template <bool S2T>
-__device__ __forceinline__ void pair_term(const double2 zp, const double2 sl, const double yj, const double dm,
-                                          const TgtG& tg, const TgtS& ts, const ColG& cg, const ColS& cs,
-                                          double& a1, double& aS) {
-  const double z = zp.x, psi = zp.y, zx = sl.x, zy = sl.y;
-  // Image terms from the direct ones (all y >= 0, sws_setup): (y + y*)^2 = (y - y*)^2 + 4 y y* and
-  // y + y* = (y - y*) + 2 y*, so y + y* itself is never formed: one DADD less per pair.  R+^2 >= R-^2, so
-  // the rounding of R-^2 it inherits is below its own.
-  const double dz = z - ts.zs;
-  const double q = fma(dz, dz, cg.dx2);
-  const double Rm2 = fma(dm, dm, q);
-  const double Rp2 = fma(tg.ys4, yj, Rm2);
-  const double rm = rsqrt_fp64(Rm2);
-  const double rp = rsqrt_fp64(Rp2);
-  // K1 numerators: zeta - zeta* - (x-x*) zeta_x - (y -+ y*) zeta_y, slopes at the source (Q2)
-  const double n0 = fma(-cg.dx, zx, dz);
-  const double nm = fma(-dm, zy, n0);
-  const double np = fma(-tg.ys2, zy, nm);
-  const double dpsi = psi - ts.psis;
-#ifdef SWS_TAIL_CUBES
-  // rounds 1-2: K1 with explicit cubes, then K2; 10 FP64 instructions (-DSWS_TAIL_CUBES, kept for the record)
-  const double rm3 = (rm * rm) * rm;
-  const double rp3 = (rp * rp) * rp;
-  const double k1 = fma(np, rp3, nm * rm3);
-  a1 = fma(dpsi, k1, a1);
-  a1 = fma(zx, rm + rp, a1);  // K2 = 1/R- + 1/R+
-#else
-  // dpsi K1 + zeta_x K2 = (1/R-) [zeta_x + dpsi n- / R-^2] + (1/R+) [zeta_x + dpsi n+ / R+^2]: the third factor of
-  // each cube and the K2 sum ride the two accumulating FMAs - 9 FP64 instructions instead of 10 (cfg5: 54.5 -> 53.2 ms)
-  const double bm = dpsi * nm, bp = dpsi * np;
-  const double cm = fma(bm, rm * rm, zx);
-  const double cp = fma(bp, rp * rp, zx);
-  a1 = fma(rm, cm, a1);
-  a1 = fma(rp, cp, a1);
-#endif
-  if (S2T) {
-    // S2 (eqs. (21), (22)) up to the factor 1/sqrt(C)
-    const double sm = yj - cs.c;
-    const double sp = yj + cs.c;
-    const double Qm = fma(sm, sm, cs.g);
-    const double Qp = fma(sp, sp, cs.g);
-    aS += rsqrt_fp64(Qm) + rsqrt_fp64(Qp);
-  }
-}
 
 // One staged segment [j0, j0 + len) of a column for the NT targets x NS states of a thread: trapezoid half
 // weights on the column's first and last node by peeling (Q4), unit weights inside.  A node's y_j and
@@ -461,7 +395,10 @@ size_t allpairs_smem_bytes(const PairPlan& p, int ns) {
 }
 
 // targets per thread of the FP64 kernel for this mesh (depends on the mesh only)
-int pair_nt(const sws_ctx* c) { return c->params.precision == 0 && c->mesh.T >= kNT2MinTargets ? 2 : 1; }
+int pair_nt(const sws_ctx* c) {
+  if (const_path_active(c)) return 1;  // the constant-bank kernel: one target per thread
+  return c->params.precision == 0 && c->mesh.T >= kNT2MinTargets ? 2 : 1;
+}
 
 // states per CTA of a launch with `states` states: 1 for a single evaluation; kBatchNS for a batch unless
 // sws_set_states_per_cta says otherwise.  Results do not depend on it (bitwise).  Measured on B200 (DESIGN.md
@@ -585,6 +522,122 @@ cudaError_t launch_allpairs(sws_ctx* c, int states, const PairPlan& plan, cudaSt
   if (nt == 2) return cudaLaunchKernelEx(&cfg, k_allpairs<kMinB2, 2, 1>, a);
   if (ns == 2) return cudaLaunchKernelEx(&cfg, k_allpairs<kMinB12, 1, 2>, a);
   return cudaLaunchKernelEx(&cfg, k_allpairs<kMinB, 1, 1>, a);
+}
+
+
+// ---------------------------------------------------------------------------------------
+// host side of the uniform-operand (constant-bank) path, sws_allpairs_const.cuh
+
+int const_slab_cols(int M) {
+  const int ypad = (M + 3) & ~3;
+  int cols = (kConstDoubles - ypad) / (4 * M);
+  if (cols > kConstMaxCols) cols = kConstMaxCols;
+  return cols < 0 ? 0 : cols;
+}
+
+// Columns per CTA.  Measured at 721x241 / 361x121 (ms per state): 1: 50.2 / 3.41, 2: 49.4 / 3.34, 4: 49.2 / 3.33 -
+// a CTA's set-up (target record, divisions) and its Euler-Maclaurin epilogues run at dependent-instruction latency,
+// so longer CTAs are better as long as a launch still fills the GPU twice; 181x61: 1 is best (0.28 against 0.29 / 0.34).
+int const_cols_per_cta(const sws_ctx* c) {
+  const int cols = const_slab_cols(c->mesh.M);
+  const long tiles = (c->mesh.T + kConstThreads - 1) / kConstThreads;
+  const long slots = (long)c->sm_count * 8;
+  for (int cpc = 4; cpc > 1; cpc /= 2)
+    if (tiles * ((cols + cpc - 1) / cpc) >= 2 * slots) return cpc;
+  return 1;
+}
+
+bool const_path_active(const sws_ctx* c) {
+  if (c->params.precision != 0 || !c->acc_c || c->const_mode == 0) return false;
+  return c->const_mode == 1 || c->mesh.T >= kConstMinTargets;
+}
+
+// a5 + a6 + a9 after the slabs of all states: E2 = 2 pi (phi* - x*) + eps / rho* - zeta_x* I - [quadrature]
+__global__ void __launch_bounds__(128) k_finish_const(const TgtRec* tgt, const double* acc0, const double* acc1,
+                                                      const double* x, const double* y, int N, int M, int T,
+                                                      double eps, double* F0, double* Fpert, int n) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x, state = blockIdx.y;
+  if (t >= T) return;
+  const double xa = __ldg(x), xb = __ldg(x + N - 1), ya = __ldg(y), yb = __ldg(y + M - 1);
+  const size_t ts = (size_t)state * T + t;
+  double sum = acc0[ts];
+  if (acc1) sum += acc1[ts];
+  double* F = state == 0 ? F0 : Fpert + (size_t)(state - 1) * n;
+  const int l = t / (N - 1), k = t - l * (N - 1);
+  F[(size_t)(N + 1) * M + (size_t)l * (N + 1) + 2 + k] = e2_local(tgt[ts], eps, xa, xb, ya, yb) - sum;
+}
+
+namespace {
+// The two banks belong to the process (one copy per device), not to a context: every context of a device feeds
+// them through the same two streams, so that slabs of different contexts can never be in a bank at the same time.
+struct ConstDevice {
+  bool ready = false;
+  cudaStream_t stream[kConstBanks] = {};
+  cudaEvent_t fork = nullptr, join[kConstBanks] = {};
+  long long y_owner[kConstBanks] = {0, 0};  // const_id of the context whose y table sits in the bank
+};
+constexpr int kMaxDevices = 64;
+ConstDevice g_const_dev[kMaxDevices];
+std::mutex g_const_mu;
+}  // namespace
+
+cudaError_t launch_allpairs_const(sws_ctx* c, int states, cudaStream_t st, double* F0, double* Fpert, int* launches) {
+  const Mesh& m = c->mesh;
+  if (c->device < 0 || c->device >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_const_mu);
+  ConstDevice& d = g_const_dev[c->device];
+  cudaError_t e = cudaSuccess;
+  if (!d.ready) {
+    for (int b = 0; b < kConstBanks && e == cudaSuccess; ++b) {
+      e = cudaStreamCreateWithFlags(&d.stream[b], cudaStreamNonBlocking);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&d.join[b], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&d.fork, cudaEventDisableTiming);
+    if (e != cudaSuccess) return e;
+    d.ready = true;
+  }
+  const int cols = const_slab_cols(m.M), ypad = (m.M + 3) & ~3;
+  const int tiles = (m.T + kConstThreads - 1) / kConstThreads;
+  const int slabs = (m.N + cols - 1) / cols;
+  const int banks = slabs > 1 ? kConstBanks : 1;
+  // fork: both bank streams wait for what the caller's stream has enqueued so far (the fields kernels)
+  if ((e = cudaEventRecord(d.fork, st)) != cudaSuccess) return e;
+  for (int b = 0; b < banks; ++b)
+    if ((e = cudaStreamWaitEvent(d.stream[b], d.fork, 0)) != cudaSuccess) return e;
+  ConstArgs a;
+  a.x = c->x; a.N = m.N; a.M = m.M; a.T = m.T; a.ypad = ypad; a.dxdy = m.dx * m.dy; a.em = em_geometry(c);
+  a.cpc = const_cols_per_cta(c);
+  for (int s = 0; s < states; ++s) {
+    for (int q = 0; q < slabs; ++q) {
+      const int b = q % kConstBanks;  // slab q of a state always goes to bank q mod 2 (fixed summation order)
+      a.tgt = c->tgt + (size_t)s * m.T;
+      a.part = c->part_c + (size_t)b * kConstMaxCols * m.T;
+      a.acc = c->acc_c + ((size_t)b * c->max_states + s) * m.T;
+      a.cnt = c->cnt_c + (size_t)b * tiles;
+      a.col0 = q * cols;
+      a.ncols = m.N - a.col0 < cols ? m.N - a.col0 : cols;
+      a.first = q < kConstBanks;
+      const double* y = nullptr;
+      if (d.y_owner[b] != c->const_id) { y = c->y; d.y_owner[b] = c->const_id; }
+      const SrcRec* slab = c->src + (size_t)s * m.S + (size_t)a.col0 * m.M;
+      e = b == 0 ? const_bank_launch_0(a, slab, y, tiles, d.stream[b]) : const_bank_launch_1(a, slab, y, tiles, d.stream[b]);
+      if (e != cudaSuccess) return e;
+      if (launches) *launches += 1;
+    }
+  }
+  // join: the caller's stream continues after both banks have drained
+  for (int b = 0; b < banks; ++b) {
+    if ((e = cudaEventRecord(d.join[b], d.stream[b])) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(st, d.join[b], 0)) != cudaSuccess) return e;
+  }
+  if (F0) {
+    const double* acc1 = banks > 1 ? c->acc_c + (size_t)c->max_states * m.T : nullptr;
+    k_finish_const<<<dim3((m.T + 127) / 128, states), 128, 0, st>>>(c->tgt, c->acc_c, acc1, c->x, c->y, m.N, m.M, m.T,
+                                                                 m.eps, F0, Fpert, m.n);
+    if (launches) *launches += 1;
+    e = cudaGetLastError();
+  }
+  return e;
 }
 
 // --- far-field statistics (bench.py: executed work of a launch) ----------------------------

@@ -1,0 +1,4 @@
+// Bank 1 of the uniform-operand all-pairs kernel (see sws_allpairs_const.cuh): a module of its own, so that it has a
+// 64 KB __constant__ bank of its own.
+#define SWS_CONST_BANK 1
+#include "sws_allpairs_const.cuh"

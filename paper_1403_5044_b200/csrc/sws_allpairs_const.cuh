@@ -1,0 +1,165 @@
+// Step a4 with the source data in UNIFORM registers (the "constant-bank" all-pairs kernel).
+//
+// Why.  Every lane of a warp works on the same source node, so the node's record {zeta, phi - x, zeta_x, zeta_y}
+// and y_j are warp-uniform.  The staged kernel (sws_allpairs.cu) broadcasts them from shared memory into VECTOR
+// registers; the FP64 instructions that combine a per-source, a per-target and a per-pair value then read three
+// distinct 64-bit vector registers, which the register file of a B200 sub-partition delivers in 3 cycles instead of
+// the pipe's 2 (8 such DFMAs per pair).  An FP64 instruction can take one operand from a
+// UNIFORM register instead (DFMA R, R, UR, R issues at full rate: measured 62.2 of 64 per SM per clock), and a
+// uniform register is loaded from a constant bank (LDCU.64 UR, c[0x3][UR + imm]) without touching the vector
+// register file or the shared-memory pipe.  With the node data in uniform registers only the two accumulating
+// FMAs of a pair keep three vector sources.
+//
+// How.  A module's __constant__ bank holds 64 KB, i.e. one SLAB of source columns (8 columns at M = 241, 16 at
+// M = 121) plus the y_j of the mesh.  The host (launch_allpairs_const, sws_allpairs.cu) walks the slabs of every
+// state: device-to-device copy of the slab's records into the bank, then one launch of this kernel with
+// grid = (target tiles, groups of cpc columns of the slab): one CTA = 64 targets x cpc source columns (cpc = 4, 2 or
+// 1: as many as leave two waves of CTAs per launch).  There are two copies of
+// this kernel in two modules (sws_allpairs_c0.cu / _c1.cu, each with its own bank) fed through two streams, so the
+// copy and the tail of one slab overlap the other slab's kernel.  The CTA that completes a target tile (arrival
+// counter, as in the staged kernel) adds the slab's group sums in the fixed order g = 0 .. G-1 and accumulates
+// them into acc[bank][state][t]; k_finish_const (sws_allpairs.cu) forms E2 = e2_local - (acc[0] + acc[1]).
+// Slab s of a state always goes to bank s mod 2, and the split into slabs depends on the mesh only: results are
+// bitwise repeatable and slot b of a batch is bitwise the single evaluation of u_b.
+//
+// The arithmetic of a pair is pair_term() of sws_pair.cuh, the same code the staged kernel runs.
+//
+// This file is the body of ONE bank: it is included by sws_allpairs_c0.cu / sws_allpairs_c1.cu with
+// SWS_CONST_BANK defined as 0 / 1.
+#include "sws_const.cuh"
+#include "sws_pair.cuh"
+
+#ifndef SWS_CONST_BANK
+#error "SWS_CONST_BANK must be 0 or 1"
+#endif
+#ifndef SWS_CONST_UNROLL
+#define SWS_CONST_UNROLL 8  // nodes per inner-loop iteration (4 / 8 / 12: 50.9 / 49.4 / 49.8 ms per state at 721x241)
+#endif
+#ifndef SWS_CONST_MINB
+#define SWS_CONST_MINB 8  // resident CTAs per SM (caps the kernel at 128 registers)
+#endif
+
+namespace sws {
+namespace {
+
+constexpr int kConstUnroll = SWS_CONST_UNROLL;
+
+// [0, ypad): y_j of the mesh;  [ypad, ypad + 4 M ncols): the slab's SrcRec, [column][j]
+__constant__ double c_buf[kConstDoubles];
+
+// One source column (records at c_buf[rbase + 4 j]) against one target: trapezoid half weights on the first and
+// last node by peeling (Q4), in the order walk_segment() of the staged kernel takes them.
+template <bool S2T>
+__device__ __forceinline__ void walk_column_const(const int rbase, const int M, const TgtG& tg, const TgtS& ts,
+                                                  const ColG& cg, const ColS& cs, double& col1, double& colS) {
+  auto node = [&](const int j, double& o1, double& oS) {
+    const double yj = c_buf[j];
+    const double* r = c_buf + rbase + 4 * j;
+    const double2 zp = make_double2(r[0], r[1]), sl = make_double2(r[2], r[3]);
+    pair_term<S2T>(zp, sl, yj, yj - tg.ys, tg, ts, cg, cs, o1, oS);
+  };
+  double h1 = 0.0, hS = 0.0;
+  node(0, h1, hS);
+  col1 = 0.5 * h1;
+  colS = 0.5 * hS;
+#pragma unroll kConstUnroll
+  for (int j = 1; j < M - 1; ++j) node(j, col1, colS);
+  h1 = hS = 0.0;
+  node(M - 1, h1, hS);
+  col1 = fma(0.5, h1, col1);
+  colS = fma(0.5, hS, colS);
+}
+
+__global__ void __launch_bounds__(kConstThreads, SWS_CONST_MINB) k_allpairs_const(const ConstArgs a) {
+  const int tid = threadIdx.x, tile = blockIdx.x, g = blockIdx.y;
+  // targets in TRANSPOSED order (sws_farfield.cuh): the 32 targets of a warp share one x*
+  const int slot = tile * kConstThreads + tid;
+  const int tc = target_of_slot(slot < a.T ? slot : a.T - 1, a.N, a.M);  // ragged tail: recomputed, never stored
+  const int t = slot < a.T ? tc : a.T;
+  const TgtRec tr = a.tgt[tc];
+  const TgtG tg = {tr.ys, 2.0 * tr.ys, 4.0 * tr.ys};
+  const TgtS ts = {tr.zs, tr.psis};
+  const double kb = tr.B / (2.0 * tr.C);           // B / 2C
+  const double kg = tr.A / tr.C - kb * kb;         // (4AC - B^2) / (4 C^2)
+  const double sfac = -tr.zxs * rsqrt_fp64(tr.C);  // - zeta_x* / sqrt(C)
+
+  // this CTA's columns of the slab: g cpc .. g cpc + cpc - 1
+  double tot1 = 0.0, totS = 0.0;
+#pragma unroll 1
+  for (int cc = 0; cc < a.cpc; ++cc) {
+    const int gc = g * a.cpc + cc;
+    if (gc >= a.ncols) break;
+    const int i = a.col0 + gc;
+    ColG cg;
+    ColS cs;
+    cg.dx = __ldg(a.x + i) - tr.xs;
+    cg.dx2 = cg.dx * cg.dx;
+    cs.c = fma(-kb, cg.dx, tg.ys);
+    cs.g = kg * cg.dx2;
+    const bool far = column_is_far(cs.g, a.em.gmin);  // warp-uniform, as the staged kernel takes it
+    const int rbase = a.ypad + 4 * a.M * gc;
+    double col1, colS;
+    if (far) {
+      walk_column_const<false>(rbase, a.M, tg, ts, cg, cs, col1, colS);
+      colS = s2_column_em(a.em, cs.c, cs.g);  // the column's S2 terms from their Euler-Maclaurin form
+    } else {
+      walk_column_const<true>(rbase, a.M, tg, ts, cg, cs, col1, colS);
+    }
+    const double ci = (i == 0 || i == a.N - 1) ? 0.5 : 1.0;  // trapezoid weight in x (Q4)
+    tot1 = fma(ci, col1, tot1);
+    totS = fma(ci, colS, totS);
+  }
+  if (t < a.T) a.part[(size_t)g * a.T + t] = a.dxdy * fma(sfac, totS, tot1);
+
+  // the last CTA of this tile adds the slab's columns in fixed order and accumulates (no floating-point atomics)
+  __shared__ int s_last;
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) {
+    unsigned int* cnt = a.cnt + tile;
+    const unsigned int seen = atomicAdd(cnt, 1u);
+    s_last = (seen == gridDim.y - 1u);
+    if (s_last) *cnt = 0u;  // ready for the next launch of this bank
+  }
+  __syncthreads();
+  if (!s_last || t >= a.T) return;
+  __threadfence();
+  double sum = 0.0;
+  for (int q = 0; q < (int)gridDim.y; ++q) sum += __ldcg(a.part + (size_t)q * a.T + t);
+  a.acc[t] = a.first ? sum : a.acc[t] + sum;
+}
+
+}  // namespace
+
+#define SWS_CAT2(a, b) a##b
+#define SWS_CAT(a, b) SWS_CAT2(a, b)
+
+// Copies the slab (and, if y != NULL, the mesh's y_j) into this module's bank and launches the kernel on `st`.
+cudaError_t SWS_CAT(const_bank_launch_, SWS_CONST_BANK)(const ConstArgs& a, const SrcRec* slab, const double* y,
+                                                        int tiles, cudaStream_t st) {
+  static void* base_of_device[64] = {};  // the bank's device address, per device (the caller holds the path's mutex)
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  if (!base_of_device[dev]) {
+    e = cudaGetSymbolAddress(&base_of_device[dev], c_buf);
+    if (e != cudaSuccess) return e;
+  }
+  void* base = base_of_device[dev];
+  if (y) {
+    e = cudaMemcpyAsync(base, y, (size_t)a.M * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return e;
+  }
+  e = cudaMemcpyAsync(static_cast<double*>(base) + a.ypad, slab, (size_t)a.ncols * a.M * sizeof(SrcRec),
+                      cudaMemcpyDeviceToDevice, st);
+  if (e != cudaSuccess) return e;
+  k_allpairs_const<<<dim3(tiles, (a.ncols + a.cpc - 1) / a.cpc), kConstThreads, 0, st>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t SWS_CAT(const_bank_occupancy_, SWS_CONST_BANK)(int* occ) {
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, k_allpairs_const, kConstThreads, 0);
+}
+
+}  // namespace sws

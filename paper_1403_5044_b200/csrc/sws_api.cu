@@ -7,9 +7,11 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <atomic>
 #include <new>
 #include <vector>
 
+#include "sws_const.cuh"
 #include "sws_internal.cuh"
 
 static thread_local char g_cuda_err[256] = "";
@@ -54,7 +56,7 @@ static cudaError_t dev_alloc(T** p, size_t count, size_t* total) {
 static void free_all(sws_ctx* c) {
   void* ptrs[] = {c->x, c->y, c->sp_cp, c->sp_inv, c->zeta, c->phi, c->zx, c->px, c->zy, c->py,
                   c->src, c->srcf, c->tgt, c->e2loc, c->tile_count, c->part, c->F0, c->Fpert, c->sigma, c->norm_part,
-                  c->dsrc, c->dtgt, c->e2lin, c->tgtI, c->lin_sums,
+                  c->dsrc, c->dtgt, c->e2lin, c->tgtI, c->lin_sums, c->acc_c, c->part_c, c->cnt_c,
                   c->u_stage, c->V_stage, c->out_stage};
   for (void* p : ptrs)
     if (p) cudaFree(p);
@@ -167,6 +169,14 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   ALLOC(u_stage, n);
   ALLOC(V_stage, mb * n);
   ALLOC(out_stage, (2 * mb + 1) * n);
+  c->const_mode = -1;
+  if (p->precision == 0 && sws::const_slab_cols(m.M) >= sws::kConstMinCols) {  // uniform-operand all-pairs path
+    static std::atomic<long long> next_id{1};
+    c->const_id = next_id.fetch_add(1);
+    ALLOC(acc_c, (size_t)sws::kConstBanks * st * T);
+    ALLOC(part_c, (size_t)sws::kConstBanks * sws::kConstMaxCols * T);
+    ALLOC(cnt_c, (size_t)sws::kConstBanks * ((T + sws::kConstThreads - 1) / sws::kConstThreads));
+  }
   if (mb > 0) {
     ALLOC(dsrc, (size_t)lin_groups * lin_bt * S);
     ALLOC(dtgt, mb * T);
@@ -206,6 +216,8 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   if (e == cudaSuccess) e = cudaMemcpy(c->sp_cp, cp.data(), cp.size() * 8, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(c->sp_inv, inv.data(), inv.size() * 8, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemset(c->tile_count, 0, st * ((T + 63) / 64) * sizeof(unsigned int));
+  if (e == cudaSuccess && c->cnt_c)
+    e = cudaMemset(c->cnt_c, 0, (size_t)sws::kConstBanks * ((T + sws::kConstThreads - 1) / sws::kConstThreads) * sizeof(unsigned int));
   if (e == cudaSuccess && c->dsrc)  // unused direction slots of the last tile stay zero
     e = cudaMemset(c->dsrc, 0, (size_t)lin_groups * lin_bt * S * sizeof(double4));
   if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
@@ -260,6 +272,23 @@ int sws_set_tuning(sws_ctx* c, int32_t chunks) {
   if (!c || chunks < 0) return SWS_EINVAL;
   if (chunks > c->part_chunks) chunks = c->part_chunks;  // the partial-sum buffer is sized at setup
   c->chunks_user = chunks;
+  return SWS_OK;
+}
+
+int sws_set_const_path(sws_ctx* c, int32_t mode) {
+  if (!c || mode < -1 || mode > 1) return SWS_EINVAL;
+  if (mode == 1 && !c->acc_c) return SWS_EINVAL;  // a source column does not fit a constant bank (or precision = 1)
+  c->const_mode = mode;
+  return SWS_OK;
+}
+
+int sws_const_plan_info(const sws_ctx* c, int32_t out[4]) {
+  if (!c || !out) return SWS_EINVAL;
+  const int cols = c->acc_c ? sws::const_slab_cols(c->mesh.M) : 0;
+  out[0] = sws::const_path_active(c) ? 1 : 0;
+  out[1] = cols;
+  out[2] = cols > 0 ? (c->mesh.N + cols - 1) / cols : 0;
+  out[3] = (c->mesh.T + sws::kConstThreads - 1) / sws::kConstThreads;
   return SWS_OK;
 }
 
@@ -339,7 +368,10 @@ static int run_states(sws_ctx* c, const double* u, const double* V, int states, 
   cudaEvent_t pe0 = nullptr, pe1 = nullptr;
   int rc = prof_begin(c, st, &pe0, &pe1);
   if (rc != SWS_OK) return rc;
-  if (c->params.precision == 0) {  // the FP64 kernel assembles E2 itself (last CTA of each target tile)
+  if (sws::const_path_active(c)) {  // source data in uniform registers: one launch per slab of columns, two banks
+    CK(sws::launch_allpairs_const(c, states, st, F0, Fpert, launches));
+    if (pe1) CK(cudaEventRecord(pe1, st));
+  } else if (c->params.precision == 0) {  // the FP64 kernel assembles E2 itself (last CTA of each target tile)
     CK(sws::launch_allpairs(c, states, plan, st, F0, Fpert));
     if (pe1) CK(cudaEventRecord(pe1, st));
     *launches += 1;
@@ -563,9 +595,13 @@ int sws_time_allpairs(sws_ctx* c, int32_t states, int32_t reps, float* ms_per_la
   ON_DEVICE(c->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const sws::PairPlan plan = sws::make_plan(c);
-  CK(sws::launch_allpairs(c, states, plan, st));  // warm-up
+  auto once = [&]() -> cudaError_t {
+    return sws::const_path_active(c) ? sws::launch_allpairs_const(c, states, st, nullptr, nullptr, nullptr)
+                                     : sws::launch_allpairs(c, states, plan, st);
+  };
+  CK(once());  // warm-up
   CK(cudaEventRecord(c->ev0, st));
-  for (int r = 0; r < reps; ++r) CK(sws::launch_allpairs(c, states, plan, st));
+  for (int r = 0; r < reps; ++r) CK(once());
   CK(cudaEventRecord(c->ev1, st));
   CK(cudaEventSynchronize(c->ev1));
   float ms = 0.f;

@@ -83,6 +83,17 @@ cudaError_t launch_debug_rsqrt(const double* x, double* y, int n, cudaStream_t s
   return cudaGetLastError();
 }
 
+// the variant whose seed takes its low word from the caller (rsqrt_fp64_lo, sws_farfield.cuh)
+__global__ void k_debug_rsqrt_lo(const double* x, const int* lo, double* y, int n) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) y[i] = rsqrt_fp64_lo(x[i], lo[i]);
+}
+
+cudaError_t launch_debug_rsqrt_lo(const double* x, const int* lo, double* y, int n, cudaStream_t st) {
+  k_debug_rsqrt_lo<<<(n + 255) / 256, 256, 0, st>>>(x, lo, y, n);
+  return cudaGetLastError();
+}
+
 }  // namespace sws
 
 static thread_local char g_dbg_err[256] = "";
@@ -206,6 +217,24 @@ int sws_debug_rsqrt_host(int32_t device, const double* x_host, double* y_host, i
   CK(cudaMemcpy(y_host, y, (size_t)n * 8, cudaMemcpyDeviceToHost));
   cudaFree(x);
   cudaFree(y);
+  return SWS_OK;
+}
+
+int sws_debug_rsqrt_lo_host(int32_t device, const double* x_host, const int32_t* lo_host, double* y_host, int32_t n) {
+  if (!x_host || !lo_host || !y_host || n < 1) return SWS_EINVAL;
+  ON_DEVICE(device);
+  double *x = nullptr, *y = nullptr;
+  int* lo = nullptr;
+  CK(cudaMalloc((void**)&x, (size_t)n * 8));
+  CK(cudaMalloc((void**)&y, (size_t)n * 8));
+  CK(cudaMalloc((void**)&lo, (size_t)n * 4));
+  CK(cudaMemcpy(x, x_host, (size_t)n * 8, cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(lo, lo_host, (size_t)n * 4, cudaMemcpyHostToDevice));
+  CK(sws::launch_debug_rsqrt_lo(x, lo, y, n, 0));
+  CK(cudaMemcpy(y_host, y, (size_t)n * 8, cudaMemcpyDeviceToHost));
+  cudaFree(x);
+  cudaFree(y);
+  cudaFree(lo);
   return SWS_OK;
 }
 

@@ -38,6 +38,18 @@ __device__ __forceinline__ double rsqrt_seed(double x) {
 #endif
 }
 
+// The same with the seed's low word taken from `lo` instead of being zeroed (any value does: the seed carries 20
+// bits anyway).  When `lo` is the low word of a value that dies where x is formed, ptxas writes the MUFU result
+// into that value's register pair and the move that zeroes the low word disappears.
+__device__ __forceinline__ double rsqrt_fp64_lo(double x, int lo) {
+  const double y0 = __hiloint2double(__double2hiint(rsqrt_seed(x)), lo);
+  const double t = x * y0;
+  const double e = fma(-t, y0, 1.0);
+  const double p = fma(0.375, e, 0.5);
+  const double w = e * p;
+  return fma(y0, w, y0);
+}
+
 __device__ __forceinline__ double rsqrt_fp64(double x) {
   const double y0 = rsqrt_seed(x);
   const double t = x * y0;

@@ -10,7 +10,7 @@ import numpy as np
 from . import SWS_ECUDA, SWS_OK, SwsError, _PKG, _np_ptr, load_library
 
 LIB_PATH = _PKG / "libsws_debug.so"
-SYMBOLS = ("sws_probe_fp64_peak", "sws_probe_fp64_mix", "sws_debug_rsqrt_host", "sws_debug_s2col_host",
+SYMBOLS = ("sws_probe_fp64_peak", "sws_probe_fp64_mix", "sws_debug_rsqrt_host", "sws_debug_rsqrt_lo_host", "sws_debug_s2col_host",
            "sws_debug_last_cuda_error")
 _lib = None
 
@@ -27,6 +27,7 @@ def load_debug_library() -> C.CDLL:
         "sws_probe_fp64_peak": (C.c_int, [C.c_int32, C.POINTER(C.c_double), ip, C.POINTER(C.c_double)]),
         "sws_probe_fp64_mix": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
         "sws_debug_rsqrt_host": (C.c_int, [C.c_int32, dp, dp, C.c_int32]),
+        "sws_debug_rsqrt_lo_host": (C.c_int, [C.c_int32, dp, C.POINTER(C.c_int32), dp, C.c_int32]),
         "sws_debug_s2col_host": (C.c_int, [C.c_int32, C.c_double, C.c_double, C.c_int32, dp, dp, C.c_int32,
                                            C.c_int32, dp, dp]),
         "sws_debug_last_cuda_error": (C.c_char_p, []),
@@ -74,6 +75,18 @@ def debug_rsqrt(x: np.ndarray, device: int = 0) -> np.ndarray:
     x = np.ascontiguousarray(x, dtype=np.float64)
     y = np.empty_like(x)
     _check(lib.sws_debug_rsqrt_host(int(device), _np_ptr(x), _np_ptr(y), int(x.size)), "sws_debug_rsqrt_host")
+    return y
+
+
+def debug_rsqrt_lo(x: np.ndarray, lo: np.ndarray, device: int = 0) -> np.ndarray:
+    """rsqrt_fp64_lo: the reciprocal square root whose seed carries the caller's low word (unit test hook)."""
+    lib = load_debug_library()
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    lo = np.ascontiguousarray(lo, dtype=np.int32)
+    assert lo.shape == x.shape
+    y = np.empty_like(x)
+    _check(lib.sws_debug_rsqrt_lo_host(int(device), _np_ptr(x), lo.ctypes.data_as(C.POINTER(C.c_int32)), _np_ptr(y),
+                                       int(x.size)), "sws_debug_rsqrt_lo_host")
     return y
 
 

@@ -55,6 +55,12 @@ def test_rsqrt_primitive(sws):
     ref = 1.0 / np.sqrt(x.astype(np.longdouble))
     rel = np.abs((y.astype(np.longdouble) - ref) / ref).astype(np.float64)
     assert rel.max() <= 2.0 ** -52, rel.max()
+    # the form 1/R- uses: the seed's low word is whatever a dead register pair holds; any value must do
+    for lo in (np.full(x.shape, -1, np.int32), rng.integers(-2**31, 2**31 - 1, x.shape).astype(np.int32),
+               np.zeros(x.shape, np.int32)):
+        y = debug.debug_rsqrt_lo(x, lo)
+        rel = np.abs((y.astype(np.longdouble) - ref) / ref).astype(np.float64)
+        assert rel.max() <= 2.0 ** -52, rel.max()
 
 
 @pytest.mark.parametrize("i", [0, 1, 2])
@@ -216,6 +222,7 @@ def test_states_per_cta_is_bitwise_invisible(sws, name, b):
         sigma = None
     u, V = dev(W.state(cfg)), dev(W.directions(cfg, b))
     with sws.Context(cfg.params(), max_batch=b) as ctx:
+        ctx.set_const_path(0)     # the staged kernel (cfg4 would otherwise take the constant-bank path)
         out = {}
         for ns in (1, 2, 0):
             ctx.set_states_per_cta(ns)
@@ -249,9 +256,14 @@ def test_fused_and_separate_field_launches(sws, oracle80):
     mask = ~np.isnan(Eb)
     with sws.Context(big.params()) as ctx:
         Fb = ctx.residual(dev(ub)).cpu().numpy()
-        assert ctx.last_launch_count == 4
-        Fb2 = ctx.residual(dev(ub)).cpu().numpy()
-    assert np.abs(Fb[mask] - Eb[mask]).max() / np.abs(Eb[mask]).max() <= TOL and np.array_equal(Fb, Fb2)
+        assert ctx.last_launch_count == 3 + 91 + 1      # three field launches, 91 slabs (constant-bank path), finish
+        ctx.set_const_path(0)
+        Fs = ctx.residual(dev(ub)).cpu().numpy()
+        assert ctx.last_launch_count == 4               # three field launches + the staged all-pairs kernel
+        Fs2 = ctx.residual(dev(ub)).cpu().numpy()
+    assert np.abs(Fb[mask] - Eb[mask]).max() / np.abs(Eb[mask]).max() <= TOL
+    assert np.abs(Fs[mask] - Eb[mask]).max() / np.abs(Eb[mask]).max() <= TOL and np.array_equal(Fs, Fs2)
+    assert relerr(Fb, Fs) <= 1e-13
 
 
 def _column_sum_longdouble(y1, dy, M, c, g):
@@ -376,9 +388,11 @@ def test_farfield_on_off_equivalence(sws, oracle80, name):
     assert relerr(F_on, E) <= TOL and relerr(F_off, E) <= TOL
 
 
+@pytest.mark.parametrize("path", ["const", "staged"])
 @pytest.mark.parametrize("i,rows", [(3, 2048), (4, 2048)])
-def test_large_configs_sampled_rows(sws, oracle80, i, rows):
-    """cfg 4 and cfg 5 at full size in the launch configuration bench.py times: the O(NM) rows
+def test_large_configs_sampled_rows(sws, oracle80, i, rows, path):
+    """cfg 4 and cfg 5 at full size in the launch configuration bench.py times (the constant-bank all-pairs
+    path these meshes take by default) and on the staged kernel: the O(NM) rows
     in full, and a seeded sample of integral-equation rows the oracle computes one by one."""
     cfg = W.CONFIGS[i]
     u = W.state(cfg)
@@ -389,7 +403,12 @@ def test_large_configs_sampled_rows(sws, oracle80, i, rows):
         [0, cfg.N - 2, T - 1, T - (cfg.N - 1), (cfg.M // 2) * (cfg.N - 1) + cfg.N // 2],  # corners, centre
     ])).astype(np.int32)
     E = oracle80.residual(cfg.params(), u, rows=pick)
-    F = gpu_residual(sws, cfg, u)
+    with sws.Context(cfg.params()) as ctx:
+        assert ctx.const_plan_info()["active"]          # what bench.py times
+        if path == "staged":
+            ctx.set_const_path(0)
+            assert not ctx.const_plan_info()["active"] and ctx.plan_info(1)["tiles"] == -(-T // 128)
+        F = ctx.residual(dev(u)).cpu().numpy()
     mask = ~np.isnan(E)
     assert mask.sum() == (cfg.N + 1) * cfg.M + 2 * cfg.M + pick.size
     assert np.isfinite(F).all()
@@ -446,6 +465,8 @@ def test_jv_batch_cfg5_bench_configuration(sws, oracle80):
     T = cfg.targets
     pick = np.unique(np.concatenate([rng.integers(0, T, 512), [0, T - 1, cfg.N - 2]])).astype(np.int32)
     with sws.Context(p, max_batch=b) as ctx:
+        info = ctx.const_plan_info()          # the launch shape bench.py times: 17 states x 91 slabs of 8 columns
+        assert info["active"] and info["cols_per_slab"] == 8 and info["slabs"] == 91
         ud, Vd = dev(u), dev(V)
         JV, Fp, F0 = ctx.jv_batch(ud, Vd, want_fpert=True, want_f0=True)
         torch.cuda.synchronize()
@@ -467,9 +488,11 @@ def test_jv_batch_cfg5_bench_configuration(sws, oracle80):
         assert np.array_equal(JV[k], (Fp[k] - F0) / sig[k])
 
 
-def test_jv_batch_cfg4_b32(sws, oracle80):
-    """BASELINE.json config 4 in FP64: 361x121, single F(u) and the b = 32 finite-difference batch (33 states in
-    one all-pairs launch of the two-targets-per-thread kernel).  F(u) and the perturbed residuals of the first
+@pytest.mark.parametrize("path", ["const", "staged"])
+def test_jv_batch_cfg4_b32(sws, oracle80, path):
+    """BASELINE.json config 4 in FP64: 361x121, single F(u) and the b = 32 finite-difference batch (33 states:
+    23 slab launches each on the constant-bank path, the default here; or one all-pairs launch of the
+    two-targets-per-thread staged kernel).  F(u) and the perturbed residuals of the first
     and last direction on seeded rows the oracle computes one by one, at the library's own shifts, to 1e-10 of
     the oracle's |F|_inf; one slot bitwise against sws_residual(fma(sigma, v, u)); a zero direction gives a
     zero row (J 0 = 0), not NaN."""
@@ -484,6 +507,9 @@ def test_jv_batch_cfg4_b32(sws, oracle80):
     V = V.copy()
     V[7] = 0.0                                  # sigma = 1e-7 (1 + |u|) / |v| must not poison the batch
     with sws.Context(p, max_batch=b) as ctx:
+        assert ctx.const_plan_info()["active"]
+        if path == "staged":
+            ctx.set_const_path(0)
         ud, Vd = dev(u), dev(V)
         JV, Fp, F0 = ctx.jv_batch(ud, Vd, want_fpert=True, want_f0=True)
         torch.cuda.synchronize()
