@@ -46,10 +46,11 @@ UNIT = "evals/s"
 FP64_INSTR_NEAR, FLOPS_NEAR = 43, 67
 FP64_INSTR_FAR, FLOPS_FAR = 27, 43
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM per clock on B200
-# dram__bytes_read.sum + dram__bytes_write.sum of one single-state all-pairs launch at cfg5 from the
-# ncu --set full capture summarised in NCU_PROFILE (a static figure: this run does not measure it)
-NCU_DRAM_BYTES_PER_STATE_LAUNCH = {"cfg5_721x241": 160.42e6}
-NCU_PROFILE = "profiles/r2a_allpairs_ncu.md"
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel at cfg5 from the ncu --set full
+# capture summarised in NCU_PROFILE (a static figure: this run does not measure it).  The constant-bank kernel is
+# launched once per slab of 8 source columns (91 launches per state); the staged kernel once per call.
+NCU_DRAM_BYTES_PER_LAUNCH = {"k_allpairs_const": {"cfg5_721x241": 13.61e6}, "k_allpairs": {"cfg5_721x241": 160.42e6}}
+NCU_PROFILE = {"k_allpairs_const": "profiles/r2b_allpairs_const_ncu.md", "k_allpairs": "profiles/r2a_allpairs_ncu.md"}
 
 
 def dist_env():
@@ -498,7 +499,8 @@ def configs_report(sws, device: int, peak_tf: float, names, steps: int = 20) -> 
                          "launches_per_step": launches, "allpairs_share_of_step": ap_ms / steps / ms,
                          "near_column_fraction": near, "flops_per_pair": flops_pair,
                          "allpairs_achieved_tflops": ach, "allpairs_frac_of_fp64_peak": ach / peak_tf,
-                         "plan": ctx.plan_info(1)}
+                         "allpairs_path": "k_allpairs_const" if ctx.const_plan_info()["active"] else "k_allpairs",
+                         "plan": ctx.const_plan_info() if ctx.const_plan_info()["active"] else ctx.plan_info(1)}
     out["note"] = ("FP64, step = sws_residual(u) + sws_jv_batch(u, V[b]) as BASELINE.json states each config (cfg1: one "
                    "F(u)); parity of every one of these steps: tests/test_gpu_parity.py")
     return out
@@ -623,19 +625,31 @@ def run_ours(args) -> None:
     achieved_tf = flops_pair * pairs_timed / ap_s / 1e12
     sm_mhz = (clocks or {}).get("sm_mhz") or sm_max
     pipe_frac = instr_pair * pairs_timed / (sm_count * FP64_LANES_PER_SM * sm_mhz * 1e6 * ap_s)
+    cinfo = ctx.const_plan_info()
+    kernel = "k_allpairs_const" if cinfo["active"] else "k_allpairs"
+    # kernel launches inside the timed all-pairs phases: one per (state, slab) on the constant-bank path
+    kernels_timed = args.steps * evals_per_step * cinfo["slabs"] if cinfo["active"] else ap_launches
+    if cinfo["active"]:   # per launch: the tile's target records once, the slab, the accumulators read + written
+        alg_bytes = cfg.targets * 64 + cinfo["cols_per_slab"] * cfg.M * 32 + 2 * cfg.targets * 8
+        alg_note = ("algorithmic bytes per launch = T*64 (target records) + 8 columns x M x 32 (the slab, through the "
+                    "constant bank) + T*8 read + T*8 written (accumulators); the slab's group sums (one 8 B value per "
+                    "target per group of columns) are written and read back inside the launch")
+    else:
+        alg_bytes = cfg.sources * 32 + cfg.targets * 64 + ctx.plan_info(1)["chunks"] * cfg.targets * 8
+        alg_note = ("algorithmic bytes per state = S*32 + T*64 bytes read once + one 8 B partial sum per target per "
+                    "column group written")
     roofline = {
-        "bound": "alu", "kernel": "k_allpairs", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-        "frac": achieved_tf / peak_tf, "traffic": NCU_DRAM_BYTES_PER_STATE_LAUNCH.get(cfg.name),
-        "traffic_source": f"{NCU_PROFILE} (static: one ncu --set full capture of this kernel, not measured by this run)",
+        "bound": "alu", "kernel": kernel, "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+        "frac": achieved_tf / peak_tf, "traffic": NCU_DRAM_BYTES_PER_LAUNCH[kernel].get(cfg.name),
+        "traffic_source": f"{NCU_PROFILE[kernel]} (static: one ncu --set full capture of one launch of this kernel, "
+                          "not measured by this run)",
         "peak_measured": peak_measured_tf,
         "peak_measured_source": f"sws_probe_fp64_mix kind 0 (register-only two-register DFMA loop, libsws_debug): "
                                 f"{mix['fp64_instr_per_sm_clk']:.2f} of {FP64_LANES_PER_SM} FP64 thread-instructions/SM/clk "
                                 f"x 2 flops x {sm_count} SMs x {sm_max:.0f} MHz",
         "frac_of_peak_measured": achieved_tf / peak_measured_tf if peak_measured_tf else None,
-        "traffic_note": "DRAM bytes per state per all-pairs launch; "
-                        "algorithmic = S*32 + T*64 bytes read once + one 8 B partial sum per target per column group "
-                        "written (part of which stays in L2 until k_assemble reads it)",
-        "algorithmic_bytes_per_state": cfg.sources * 32 + cfg.targets * 64 + ctx.plan_info(1)["chunks"] * cfg.targets * 8,
+        "traffic_note": "DRAM bytes (read + written) of one launch; " + alg_note,
+        "algorithmic_bytes_per_launch": alg_bytes,
         "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz "
                        "(FP64 is not in MEASURED_PEAKS.json; DESIGN.md 'Peak')",
         "flops_per_pair": flops_pair, "fp64_instr_per_pair": instr_pair,
@@ -644,7 +658,12 @@ def run_ours(args) -> None:
                      f"{FLOPS_FAR} on the far ones (S2 column sum in closed form + Euler-Maclaurin, sws_set_farfield); "
                      "with the plain 67 flops/pair definition the same time reads "
                      f"{FLOPS_NEAR * pairs_timed / ap_s / 1e12:.1f} TFLOP/s-equivalent",
-        "launches_timed": ap_launches, "avg_launch_ms": ap_ms / max(ap_launches, 1),
+        "launches_timed": kernels_timed, "avg_launch_ms": ap_ms / max(kernels_timed, 1),
+        "phases_timed": ap_launches,
+        "timing_note": "achieved = flops of all pairs of the timed steps / summed live CUDA-event time of the all-pairs "
+                       "phases on the caller's stream (sws_set_profiling); on the constant-bank path a phase is the "
+                       "slab launches of its states on the library's two streams (fork / join on the caller's stream, "
+                       "slab copies included) and avg_launch_ms = that time / kernel launches",
         "share_of_step": ap_ms / ms_total if world == 1 else None,
         "dfma_probe_tflops": probe["tflops"], "dfma_probe_sm_mhz": probe["sm_mhz"],
         "frac_of_dfma_probe": achieved_tf / probe["tflops"] if probe["tflops"] else None,
@@ -695,7 +714,8 @@ def run_ours(args) -> None:
                    "pairs_per_eval": cfg.pairs, "step": "sws_residual(u) + sws_jv_batch(u, V[b])",
                    "l2": "256 MB buffer written between timed iterations (L2 flush)",
                    "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "plan": {"single": ctx.plan_info(1), "batch": ctx.plan_info(b + 1)}},
+                   "plan": {"allpairs_path": kernel, "const": cinfo,
+                            "staged_single": ctx.plan_info(1), "staged_batch": ctx.plan_info(b + 1)}},
         "pairs_per_s": value * cfg.pairs,
         # the step evaluates E(u) twice (sws_residual and state 0 of the batch, as BASELINE.json words the config):
         # a JFNK consumer that takes F0 from the batch needs the b + 1 DISTINCT states of sws_jv_batch alone

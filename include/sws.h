@@ -205,10 +205,13 @@ int sws_set_states_per_cta(sws_ctx* ctx, int32_t ns);
  * from where the kernel takes them as uniform-register operands of its FP64 instructions (DESIGN.md section 6:
  * no three-vector-register DFMAs on the source data, no shared-memory loads); one launch per slab, two banks fed
  * through two library-owned streams that fork from and join the caller's stream (asynchronous as before).
- * mode -1 (default): used on FP64 meshes with at least 40,000 targets whose columns fit a bank at least four at a
+ * mode -1 (default): used on FP64 meshes with at least 16,000 targets whose columns fit a bank at least four at a
  * time (M <= 479); 0: never (always the staged kernel); 1: whenever the columns fit (SWS_EINVAL otherwise).
  * Results are bitwise repeatable in either form and slot b of a batch is bitwise the single evaluation of u_b;
- * the two forms differ from each other in summation order only (~1e-13 of |F|). */
+ * the two forms differ from each other in summation order only (~1e-13 of |F|).  The two banks and streams belong to
+ * the process (per device): calls of any number of contexts and host threads are serialised through them.  A call may
+ * be captured into a CUDA graph after one eager call; a replay of such a graph must not run concurrently with other
+ * calls of this library on the same device (the replayed copies into the banks are not ordered against them). */
 int sws_set_const_path(sws_ctx* ctx, int32_t mode);
 /* out = {path active for this context now (0/1), columns per slab, slabs per state, target tiles (CTAs per column)} */
 int sws_const_plan_info(const sws_ctx* ctx, int32_t out[4]);

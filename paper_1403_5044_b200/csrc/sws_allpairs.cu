@@ -553,15 +553,15 @@ bool const_path_active(const sws_ctx* c) {
 }
 
 // a5 + a6 + a9 after the slabs of all states: E2 = 2 pi (phi* - x*) + eps / rho* - zeta_x* I - [quadrature]
-__global__ void __launch_bounds__(128) k_finish_const(const TgtRec* tgt, const double* acc0, const double* acc1,
+__global__ void __launch_bounds__(128) k_finish_const(const TgtRec* tgt, const double* acc, size_t bank_stride, int banks,
                                                       const double* x, const double* y, int N, int M, int T,
                                                       double eps, double* F0, double* Fpert, int n) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x, state = blockIdx.y;
   if (t >= T) return;
   const double xa = __ldg(x), xb = __ldg(x + N - 1), ya = __ldg(y), yb = __ldg(y + M - 1);
   const size_t ts = (size_t)state * T + t;
-  double sum = acc0[ts];
-  if (acc1) sum += acc1[ts];
+  double sum = acc[ts];
+  for (int b = 1; b < banks; ++b) sum += acc[b * bank_stride + ts];  // fixed order
   double* F = state == 0 ? F0 : Fpert + (size_t)(state - 1) * n;
   const int l = t / (N - 1), k = t - l * (N - 1);
   F[(size_t)(N + 1) * M + (size_t)l * (N + 1) + 2 + k] = e2_local(tgt[ts], eps, xa, xb, ya, yb) - sum;
@@ -574,7 +574,6 @@ struct ConstDevice {
   bool ready = false;
   cudaStream_t stream[kConstBanks] = {};
   cudaEvent_t fork = nullptr, join[kConstBanks] = {};
-  long long y_owner[kConstBanks] = {0, 0};  // const_id of the context whose y table sits in the bank
 };
 constexpr int kMaxDevices = 64;
 ConstDevice g_const_dev[kMaxDevices];
@@ -599,7 +598,7 @@ cudaError_t launch_allpairs_const(sws_ctx* c, int states, cudaStream_t st, doubl
   const int cols = const_slab_cols(m.M), ypad = (m.M + 3) & ~3;
   const int tiles = (m.T + kConstThreads - 1) / kConstThreads;
   const int slabs = (m.N + cols - 1) / cols;
-  const int banks = slabs > 1 ? kConstBanks : 1;
+  const int banks = slabs < kConstBanks ? slabs : kConstBanks;
   // fork: both bank streams wait for what the caller's stream has enqueued so far (the fields kernels)
   if ((e = cudaEventRecord(d.fork, st)) != cudaSuccess) return e;
   for (int b = 0; b < banks; ++b)
@@ -609,7 +608,7 @@ cudaError_t launch_allpairs_const(sws_ctx* c, int states, cudaStream_t st, doubl
   a.cpc = const_cols_per_cta(c);
   for (int s = 0; s < states; ++s) {
     for (int q = 0; q < slabs; ++q) {
-      const int b = q % kConstBanks;  // slab q of a state always goes to bank q mod 2 (fixed summation order)
+      const int b = q % kConstBanks;  // slab q of a state always goes to bank q mod kConstBanks (fixed summation order)
       a.tgt = c->tgt + (size_t)s * m.T;
       a.part = c->part_c + (size_t)b * kConstMaxCols * m.T;
       a.acc = c->acc_c + ((size_t)b * c->max_states + s) * m.T;
@@ -617,8 +616,9 @@ cudaError_t launch_allpairs_const(sws_ctx* c, int states, cudaStream_t st, doubl
       a.col0 = q * cols;
       a.ncols = m.N - a.col0 < cols ? m.N - a.col0 : cols;
       a.first = q < kConstBanks;
-      const double* y = nullptr;
-      if (d.y_owner[b] != c->const_id) { y = c->y; d.y_owner[b] = c->const_id; }
+      // every call puts its own y table into a bank before its first slab there: the banks belong to the process,
+      // and a CUDA graph replayed by a caller may have refilled them since this context's last call
+      const double* y = (s == 0 && q < kConstBanks) ? c->y : nullptr;
       const SrcRec* slab = c->src + (size_t)s * m.S + (size_t)a.col0 * m.M;
       e = b == 0 ? const_bank_launch_0(a, slab, y, tiles, d.stream[b]) : const_bank_launch_1(a, slab, y, tiles, d.stream[b]);
       if (e != cudaSuccess) return e;
@@ -631,9 +631,8 @@ cudaError_t launch_allpairs_const(sws_ctx* c, int states, cudaStream_t st, doubl
     if ((e = cudaStreamWaitEvent(st, d.join[b], 0)) != cudaSuccess) return e;
   }
   if (F0) {
-    const double* acc1 = banks > 1 ? c->acc_c + (size_t)c->max_states * m.T : nullptr;
-    k_finish_const<<<dim3((m.T + 127) / 128, states), 128, 0, st>>>(c->tgt, c->acc_c, acc1, c->x, c->y, m.N, m.M, m.T,
-                                                                 m.eps, F0, Fpert, m.n);
+    k_finish_const<<<dim3((m.T + 127) / 128, states), 128, 0, st>>>(c->tgt, c->acc_c, (size_t)c->max_states * m.T, banks,
+                                                                 c->x, c->y, m.N, m.M, m.T, m.eps, F0, Fpert, m.n);
     if (launches) *launches += 1;
     e = cudaGetLastError();
   }

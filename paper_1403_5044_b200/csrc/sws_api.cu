@@ -7,7 +7,6 @@
 #include <stdlib.h>
 #include <string.h>
 
-#include <atomic>
 #include <new>
 #include <vector>
 
@@ -171,8 +170,6 @@ int sws_setup(const sws_params* p, sws_ctx** out) {
   ALLOC(out_stage, (2 * mb + 1) * n);
   c->const_mode = -1;
   if (p->precision == 0 && sws::const_slab_cols(m.M) >= sws::kConstMinCols) {  // uniform-operand all-pairs path
-    static std::atomic<long long> next_id{1};
-    c->const_id = next_id.fetch_add(1);
     ALLOC(acc_c, (size_t)sws::kConstBanks * st * T);
     ALLOC(part_c, (size_t)sws::kConstBanks * sws::kConstMaxCols * T);
     ALLOC(cnt_c, (size_t)sws::kConstBanks * ((T + sws::kConstThreads - 1) / sws::kConstThreads));

@@ -7,12 +7,14 @@
 namespace sws {
 
 constexpr int kConstBanks = 2;         // copies of the kernel, each in a module with a __constant__ bank of its own
+                                       // (three and four banks were measured: no faster than two)
 constexpr int kConstDoubles = 8160;    // 65,280 B of a module's 64 KB bank: y_j of the mesh + one slab of records
 constexpr int kConstThreads = 64;      // targets per CTA (one per thread)
 constexpr int kConstMaxCols = 16;      // columns of a slab = CTA rows of a launch (capacity of the scratch rows)
 constexpr int kConstMinCols = 4;       // the path is used only when a slab holds at least this many columns
 #ifndef SWS_CONST_MIN_TARGETS
-#define SWS_CONST_MIN_TARGETS 40000    // ... and the mesh has at least this many targets (smaller: staged kernel)
+#define SWS_CONST_MIN_TARGETS 16000    // ... and the mesh has at least this many targets (226x76: 3 %, 271x91: 7 % faster
+                                       // than the staged kernel, 181x61: equal)
 #endif
 constexpr int kConstMinTargets = SWS_CONST_MIN_TARGETS;
 

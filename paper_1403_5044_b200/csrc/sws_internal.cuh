@@ -108,7 +108,6 @@ struct sws_ctx {
 
   // uniform-operand (constant-bank) all-pairs path, sws_allpairs_const.cuh; NULL when a column does not fit a bank
   int const_mode;          // sws_set_const_path: -1 automatic (large meshes), 0 off, 1 on whenever a column fits
-  long long const_id;      // identifies this context's y table in the banks (they are shared by all contexts)
   double* acc_c;           // [bank][state][t] accumulated quadrature
   double* part_c;          // [bank][kConstMaxCols][t] column sums of the slab in flight
   unsigned int* cnt_c;     // [bank][tiles] arrival counters

@@ -188,3 +188,29 @@ def test_const_path_refused_where_it_does_not_fit(sws):
     with sws.Context(W.CONFIGS[0].params(), precision=1) as ctx:
         with pytest.raises(sws.SwsError):
             ctx.set_const_path(1)
+
+
+def test_const_path_cuda_graph_capture_and_replay(sws):
+    """sws_residual on the constant-bank path forks onto the library's two streams and joins again: a caller may
+    capture it into a CUDA graph (after one eager call, which loads the modules and creates the streams) and
+    replay it, also after another context has had its own y table in the banks."""
+    import torch
+    cfgA, cfgB = W.CONFIGS[1], W.custom(N=40, M=27, h=0.3, x1=-4.0, eps=0.3, amp=0.05, seed=43)
+    with sws.Context(cfgA.params()) as a, sws.Context(cfgB.params()) as b:
+        a.set_const_path(1)
+        b.set_const_path(1)
+        uA, uB = dev(W.state(cfgA)), dev(W.state(cfgB))
+        FA = torch.empty_like(uA)
+        ref = a.residual(uA).clone()
+        refB = b.residual(uB).clone()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            a.residual(uA, out=FA)
+        for _ in range(3):
+            FA.zero_()
+            assert torch.equal(b.residual(uB), refB)     # the banks now hold b's y table
+            g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(FA, ref)
+        assert torch.equal(a.residual(uA), ref)          # eager again after the capture
