@@ -24,7 +24,9 @@ int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, doubl
  * of 256-thread CTAs, warps_per_sm in {8, 16, ..., 64}).  kind: 0 DFMA with two distinct register
  * sources; 1 DFMA with three distinct register sources; 2 DADD; 3 DMUL; 4 eleven two-register DFMA +
  * DADD + DMUL + one MUFU.RSQ64H (+ the move that zeroes the seed's low word); 5 eleven two-register
- * DFMA + three integer instructions.  Reports FP64 thread-instructions per SM per clock (64 = the
+ * DFMA + three integer instructions; 6 DFMA with two distinct vector registers and one uniform-register operand
+ * loaded from a constant bank (the operand form of the constant-bank all-pairs kernel); 7-10 twelve two-register
+ * DFMA + two MUFU.RSQ64H / two FP32 MUFU.RSQ / two FFMA / two LOP3.  Reports FP64 thread-instructions per SM per clock (64 = the
  * pipe's issue limit) and the SM clock during the loop. */
 int sws_probe_fp64_mix(int32_t device, int32_t kind, int32_t warps_per_sm, double* fp64_instr_per_sm_clk,
                        double* sm_mhz);

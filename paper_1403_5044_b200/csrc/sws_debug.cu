@@ -160,7 +160,7 @@ int sws_probe_fp64_peak(int32_t device, double* tflops, int32_t* sm_count, doubl
 
 int sws_probe_fp64_mix(int32_t device, int32_t kind, int32_t warps_per_sm, double* fp64_instr_per_sm_clk,
                        double* sm_mhz) {
-  if (!fp64_instr_per_sm_clk || kind < 0 || kind > 5) return SWS_EINVAL;
+  if (!fp64_instr_per_sm_clk || kind < 0 || kind > 10) return SWS_EINVAL;
   if (warps_per_sm < 8 || warps_per_sm > 64 || warps_per_sm % 8) return SWS_EINVAL;
   int ndev = 0;
   CK(cudaGetDeviceCount(&ndev));
@@ -169,8 +169,8 @@ int sws_probe_fp64_mix(int32_t device, int32_t kind, int32_t warps_per_sm, doubl
   cudaDeviceProp prop;
   CK(cudaGetDeviceProperties(&prop, device));
   const int sms = prop.multiProcessorCount;
-  const int blocks = sms * (warps_per_sm / 8), threads = 256, iters = 1 << 15;
-  static const int fp64_per_iter[6] = {12, 12, 12, 12, 13, 11};
+  const int blocks = sms * (warps_per_sm / 8), threads = 256, iters = kind >= 6 ? 1 << 13 : 1 << 15;
+  static const int fp64_per_iter[11] = {12, 12, 12, 12, 13, 11, 48, 48, 48, 48, 48};
   double* sink = nullptr;
   unsigned long long* clk = nullptr;
   CK(cudaMalloc((void**)&sink, (size_t)blocks * threads * sizeof(double)));

@@ -40,6 +40,12 @@ __global__ void __launch_bounds__(256) k_fp64_probe(int iters, double* sink, uns
 //   3  DMUL, two distinct registers                 r = r * a
 //   4  11 two-register DFMA + 1 MUFU.RSQ64H
 //   5  11 two-register DFMA + 3 integer instructions
+//   6  DFMA with two distinct vector registers and one UNIFORM-register operand taken from a constant bank
+//      r_i = fma(r_i, c[it], s_i)   (LDCU.64 + DFMA R, R, UR, R: the operand form of the constant-bank all-pairs kernel)
+//   7-10  12 two-register DFMA + 2 more instructions that do not go to the FP64 pipe (four such rounds per iteration): 2 MUFU.RSQ64H (7),
+//      2 MUFU.RSQ (FP32) (8), 2 FFMA (9), 2 LOP3 (10) - each of them costs about one cycle of FP64 issue
+__constant__ double c_probe[64];
+
 template <int KIND>
 __global__ void __launch_bounds__(256) k_fp64_mix(int iters, double* sink, unsigned long long* clk) {
   const double a = 1.0 - 1e-9 * (threadIdx.x + 1), b = 1e-3 + 1e-12 * (blockIdx.x + 1);
@@ -51,6 +57,8 @@ __global__ void __launch_bounds__(256) k_fp64_mix(int iters, double* sink, unsig
     s[i] = 1e-4 * (i + 1) + 1e-10 * threadIdx.x;
   }
   unsigned int n0 = threadIdx.x, n1 = blockIdx.x, n2 = 12345u;
+  double m0 = 1.5 + 1e-3 * threadIdx.x, m1 = 2.5 + 1e-3 * threadIdx.x;
+  float f0 = 1.5f + 1e-3f * threadIdx.x, f1 = 2.5f + 1e-3f * threadIdx.x;
   unsigned long long c0 = 0, g0 = 0;
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     c0 = clock64();
@@ -76,12 +84,38 @@ __global__ void __launch_bounds__(256) k_fp64_mix(int iters, double* sink, unsig
 #pragma unroll
       for (int i = 0; i < 10; ++i) r[i] = fma(r[i], r[i], b);
       r[10] = fma(r[10], r[10], t * 1e-3);  // DMUL + DFMA: 12 FP64 instructions + 1 DADD above, see host
-    } else {
+    } else if (KIND == 5) {
 #pragma unroll
       for (int i = 0; i < 11; ++i) r[i] = fma(r[i], r[i], b);
       n0 = n0 * 3u + n1;
       n1 = n1 + n2;
       n2 = n2 ^ n0;
+    } else if (KIND == 6) {  // 4 x 12 DFMA per iteration, each round with its own uniform operand
+#pragma unroll
+      for (int rd = 0; rd < 4; ++rd) {
+        const double cu = c_probe[(it & 15) * 4 + rd];  // uniform address: LDCU.64 into a uniform register
+#pragma unroll
+        for (int i = 0; i < 12; ++i) r[i] = fma(r[i], cu, s[i]);
+      }
+    } else {  // 4 x (12 two-register DFMA + 2 instructions of another pipe) per iteration
+#pragma unroll
+      for (int rd = 0; rd < 4; ++rd) {
+#pragma unroll
+        for (int i = 0; i < 12; ++i) r[i] = fma(r[i], r[i], b);
+        if (KIND == 7) {
+          asm volatile("rsqrt.approx.ftz.f64 %0, %0;" : "+d"(m0));
+          asm volatile("rsqrt.approx.ftz.f64 %0, %0;" : "+d"(m1));
+        } else if (KIND == 8) {
+          asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(f0));
+          asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(f1));
+        } else if (KIND == 9) {
+          asm volatile("fma.rn.f32 %0, %0, 0f3F7FF000, 0f3A000000;" : "+f"(f0));
+          asm volatile("fma.rn.f32 %0, %0, 0f3F7FF000, 0f3A000000;" : "+f"(f1));
+        } else {
+          asm volatile("lop3.b32 %0, %0, 0x5a5a5a5a, %1, 0x96;" : "+r"(n0) : "r"(n1));
+          asm volatile("lop3.b32 %0, %0, 0x5a5a5a5a, %1, 0x96;" : "+r"(n1) : "r"(n0));
+        }
+      }
     }
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -89,7 +123,7 @@ __global__ void __launch_bounds__(256) k_fp64_mix(int iters, double* sink, unsig
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
     clk[0] = c0; clk[1] = c1; clk[2] = g0; clk[3] = g1;
   }
-  double acc = (double)(n0 ^ n1 ^ n2) * 1e-300;
+  double acc = (double)(n0 ^ n1 ^ n2) * 1e-300 + (m0 + m1 + (double)(f0 + f1)) * 1e-300;
 #pragma unroll
   for (int i = 0; i < 12; ++i) acc += r[i] + q[i] * s[i];
   sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
@@ -102,7 +136,12 @@ cudaError_t launch_fp64_mix(int kind, int blocks, int iters, double* sink, unsig
     case 2: k_fp64_mix<2><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
     case 3: k_fp64_mix<3><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
     case 4: k_fp64_mix<4><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
-    default: k_fp64_mix<5><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    case 5: k_fp64_mix<5><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    case 6: k_fp64_mix<6><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    case 7: k_fp64_mix<7><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    case 8: k_fp64_mix<8><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    case 9: k_fp64_mix<9><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
+    default: k_fp64_mix<10><<<blocks, 256, 0, st>>>(iters, sink, clk); break;
   }
   return cudaGetLastError();
 }

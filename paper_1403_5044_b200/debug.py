@@ -56,7 +56,9 @@ def probe_fp64_peak(device: int = 0) -> dict:
     return dict(tflops=tf.value, sm_count=int(sms.value), sm_mhz=mhz.value)
 
 
-FP64_MIX_KINDS = ("dfma_2reg", "dfma_3reg", "dadd", "dmul", "dfma11_dadd_dmul_mufu_rsq64h", "dfma11_int3")
+FP64_MIX_KINDS = ("dfma_2reg", "dfma_3reg", "dadd", "dmul", "dfma11_dadd_dmul_mufu_rsq64h", "dfma11_int3",
+                  "dfma_2reg_plus_uniform", "dfma12_mufu_rsq64h_x2", "dfma12_mufu_rsq_f32_x2", "dfma12_ffma_x2",
+                  "dfma12_lop3_x2")
 
 
 def probe_fp64_mix(kind: int, warps_per_sm: int = 16, device: int = 0) -> dict:
