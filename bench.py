@@ -435,8 +435,10 @@ def table1_report(sws, device: int, steps: int = 5) -> dict:
         out[f"{N}x{M}"] = {"seconds_per_evaluation": sec, "pairs_per_s": cfg.pairs / sec,
                            "seconds_per_evaluation_back_to_back": loop_ms * 1e-3,
                            "paper_workstation_matlab_s": cpu, "paper_m2090_s": gpu, "ratio_to_paper_m2090": gpu / sec}
-    out["note"] = ("one sws_residual (whole u -> F path: 2 kernel launches on these meshes - a cooperative launch for the "
-                   "O(NM) stages, then the all-pairs kernel, which also assembles E2) per evaluation, synthetic state; "
+    out["note"] = ("one sws_residual (whole u -> F path: up to 181x61 2 kernel launches - a cooperative launch for the "
+                   "O(NM) stages, then the staged all-pairs kernel, which also assembles E2; from 271x91 the constant-bank "
+                   "all-pairs path: one launch per slab of 16 source columns on two streams + a finishing launch) per "
+                   "evaluation, synthetic state; "
                    "`seconds_per_evaluation` = an isolated call between synchronisations after an L2 flush, "
                    "`..._back_to_back` = sws_time_residual (a solver's view); the "
                    "paper's numbers are other hardware (2x Xeon E5-2670 / Tesla M2090, L265) and its own converged "
