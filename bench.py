@@ -766,11 +766,30 @@ def run_experiments(args) -> None:
     import paper_1403_5044_b200 as sws
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --experiments: no CUDA device")
-    out = {"experiments": "round 2", "batch_sharing": {}, "small_meshes": {}}
+    out = {"experiments": "round 2", "allpairs_paths": {}, "batch_sharing": {}, "small_meshes": {}}
+    # the all-pairs phase of ONE state alone (sws_time_allpairs) on the constant-bank path and on the staged kernel,
+    # and whole evaluations back to back (sws_time_residual), on the BASELINE meshes and the sizes in between
+    for (N, M, h) in ((181, 61, 0.3), (226, 76, 0.24), (271, 91, 0.2), (316, 106, 0.17), (361, 121, 0.15),
+                      (721, 241, 0.075)):
+        cfg = W.custom(N, M, h, -16.0, eps=1.0, amp=0.1, seed=5)
+        with sws.Context(cfg.params()) as ctx:
+            u = torch.from_numpy(W.state(cfg)).cuda()
+            F = torch.empty_like(u)
+            row = {"targets": cfg.targets, "default_path": "const" if ctx.const_plan_info()["active"] else "staged"}
+            for mode, key in ((1, "const"), (0, "staged")):
+                ctx.set_const_path(mode)
+                ctx.residual(u, out=F)
+                torch.cuda.synchronize()
+                reps = 5 if N > 400 else 30
+                row[f"{key}_allpairs_ms"] = min(ctx.time_allpairs(1, reps) for _ in range(3))
+                row[f"{key}_residual_ms"] = min(ctx.time_residual(u, F, reps) for _ in range(3))
+            row["const_plan"] = ctx.const_plan_info()
+            out["allpairs_paths"][f"{N}x{M}"] = row
     for name in ("cfg5_721x241", "cfg4_361x121", "cfg3_181x61"):
         cfg = W.BY_NAME[name]
         b = cfg.b
         with sws.Context(cfg.params(), max_batch=b) as ctx:
+            ctx.set_const_path(0)      # this section is about the staged kernel's batched mode
             u = torch.from_numpy(W.state(cfg)).cuda()
             V = torch.from_numpy(W.directions(cfg, b)).cuda()
             ctx.jv_batch(u, V)

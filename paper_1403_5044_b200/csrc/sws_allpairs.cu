@@ -539,6 +539,9 @@ int const_slab_cols(int M) {
 // a CTA's set-up (target record, divisions) and its Euler-Maclaurin epilogues run at dependent-instruction latency,
 // so longer CTAs are better as long as a launch still fills the GPU twice; 181x61: 1 is best (0.28 against 0.29 / 0.34).
 int const_cols_per_cta(const sws_ctx* c) {
+#ifdef SWS_CONST_CPC
+  return SWS_CONST_CPC;  // build-time override for the measurements of profiles/r2_experiments.md
+#endif
   const int cols = const_slab_cols(c->mesh.M);
   const long tiles = (c->mesh.T + kConstThreads - 1) / kConstThreads;
   const long slots = (long)c->sm_count * 8;
