@@ -510,13 +510,13 @@ constexpr int kFusedMaxNodes = 1 << 17;  // the fused fields launch is used up t
 static size_t dy_staged_smem_bytes(int M) { return ((size_t)2 * M * 32 + 2 * M) * sizeof(double); }
 
 cudaError_t fields_configure(const sws_ctx* c) {
-  cudaError_t e = cudaFuncSetAttribute(k_reconstruct, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)reconstruct_smem_bytes(c->mesh.N));
+  // The attribute belongs to the FUNCTION (per device), not to a context: it is always set to the largest size any
+  // context may ask for (sws_setup bounds N; kDyStagedMaxSmem bounds the staged column), so that setting up a small
+  // mesh cannot take the limit away from a larger context that is still alive.
+  cudaError_t e = cudaFuncSetAttribute(k_reconstruct, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e != cudaSuccess) return e;
-  const size_t smem = dy_staged_smem_bytes(c->mesh.M);
-  if (smem <= kDyStagedMaxSmem)
-    e = cudaFuncSetAttribute(k_dy_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  return e;
+  (void)c;
+  return cudaFuncSetAttribute(k_dy_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDyStagedMaxSmem);
 }
 
 // The fused launch is used when both the line buffers of phase 1 and the staged block of phase 2 fit the CTA's
@@ -536,7 +536,7 @@ cudaError_t fused_configure(sws_ctx* c) {
   int coop = 0;
   cudaError_t e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device);
   if (e != cudaSuccess || !coop) return e;
-  e = cudaFuncSetAttribute(k_fields_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  e = cudaFuncSetAttribute(k_fields_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDyStagedMaxSmem);  // see fields_configure
   if (e != cudaSuccess) return e;
   int occ = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_fields_fused, 256, smem);

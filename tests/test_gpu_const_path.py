@@ -214,3 +214,37 @@ def test_const_path_cuda_graph_capture_and_replay(sws):
             torch.cuda.synchronize()
             assert torch.equal(FA, ref)
         assert torch.equal(a.residual(uA), ref)          # eager again after the capture
+
+
+def test_const_path_host_threads(sws, oracle80):
+    """Two host threads, each with a context and a stream of its own, call the constant-bank path at the same time:
+    the library serialises them through its two banks (a mutex around the enqueue, stream order on the device)."""
+    import threading
+    import torch
+    cfgs = [W.CONFIGS[1], W.custom(N=47, M=29, h=0.3, x1=-4.0, eps=0.3, amp=0.05, seed=44)]
+    refs = [oracle80.residual(c.params(), W.state(c)) for c in cfgs]
+    results, errors = [None, None], []
+
+    def work(i):
+        try:
+            torch.cuda.set_device(0)
+            st = torch.cuda.Stream()
+            with sws.Context(cfgs[i].params()) as ctx, torch.cuda.stream(st):
+                ctx.set_const_path(1)
+                u = dev(W.state(cfgs[i]))
+                outs = [ctx.residual(u) for _ in range(25)]
+                st.synchronize()
+                first = outs[0].cpu().numpy()
+                assert all(np.array_equal(o.cpu().numpy(), first) for o in outs)
+                results[i] = first
+        except Exception as e:  # noqa: BLE001 - reported below
+            errors.append(e)
+
+    threads = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for i in range(2):
+        assert relerr(results[i], refs[i]) <= TOL

@@ -856,3 +856,27 @@ def test_jv_apply_cfg5_sampled_rows_and_state(sws, oracleC):
         mask = ~np.isnan(ref)
         err = np.abs(got[mask] - ref[mask]).max() / np.abs(got).max()
         assert err <= TOL, (k, err)
+
+
+def test_contexts_of_different_sizes_alive_together(sws, oracle80):
+    """The dynamic shared-memory limits of the O(NM) kernels belong to the functions, not to a context: setting up
+    a small mesh while a context with long lines / long columns is alive must not take its launches away
+    (regression: the second sws_setup used to lower cudaFuncAttributeMaxDynamicSharedMemorySize)."""
+    big = W.custom(N=700, M=300, h=0.05, x1=-10.0, eps=0.3, amp=0.05, seed=51)     # long lines and columns
+    small = W.custom(N=3, M=4, h=0.5, x1=-1.0)
+    ub, us = W.state(big), W.state(small)
+    pick = np.arange(0, big.targets, 4001, dtype=np.int32)
+    Eb = oracle80.residual(big.params(), ub, rows=pick)
+    mask = ~np.isnan(Eb)
+    with sws.Context(big.params()) as a:
+        Fa = a.residual(dev(ub)).cpu().numpy()
+        with sws.Context(small.params()) as b:
+            Fs = b.residual(dev(us)).cpu().numpy()
+            Fa2 = a.residual(dev(ub)).cpu().numpy()        # the large context after the small one was set up
+            a.set_const_path(0)
+            a.set_fused_fields(False)
+            Fa3 = a.residual(dev(ub)).cpu().numpy()        # and on its separate field launches
+    assert np.array_equal(Fa, Fa2)
+    assert relerr(Fa3, Fa) <= 1e-13
+    assert np.abs(Fa[mask] - Eb[mask]).max() / np.abs(Eb[mask]).max() <= TOL
+    assert relerr(Fs, oracle80.residual(small.params(), us)) <= TOL
