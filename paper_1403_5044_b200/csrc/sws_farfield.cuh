@@ -81,7 +81,11 @@ __device__ __forceinline__ double rsqrt_fp64(double x) {
 // x M pairs: 0.9 per pair at M = 241.
 // (default r = kEmRadius of sws_internal.cuh; sws_set_farfield changes it, r <= 0 sums directly)
 
-// sum_{k=1..7} (B_2k / 2k) s^k P_{2k-1}(mu) at the end point u = y_e - c;  *rho = sqrt(u^2 + g)
+// sum_{k=1..K} (B_2k / 2k) s^k P_{2k-1}(mu) at the end point u = y_e - c, s = (dy / rho)^2;  *rho = sqrt(u^2 + g).
+// K = 7 in general (s <= 1/64 at the far-field radius).  Most end points are much farther from the target than the
+// radius, and the series is cut where its next term is below 1e-18: K = 3 when s <= 1e-4 (rho >= 100 dy; next term
+// s^4 / 240 <= 4e-19), K = 5 when s <= 1.5e-3 (rho >= 26 dy; next term 0.021 s^6 <= 3e-19).  The choice depends on
+// the lane's own s only (lanes of a warp are neighbouring targets and mostly agree).
 __device__ __forceinline__ double em_tail(const double u, const double g, const double h2, double* rho) {
   const double r2 = fma(u, u, g);
   const double ri = rsqrt_fp64(r2);
@@ -92,7 +96,31 @@ __device__ __forceinline__ double em_tail(const double u, const double g, const 
   P[0] = 1.0;
   P[1] = mu;
 #pragma unroll
-  for (int n = 1; n <= 12; ++n)  // (n+1) P_{n+1} = (2n+1) mu P_n - n P_{n-1}
+  for (int n = 1; n <= 4; ++n)  // (n+1) P_{n+1} = (2n+1) mu P_n - n P_{n-1}
+    P[n + 1] = ((2.0 * n + 1.0) / (n + 1.0)) * (mu * P[n]) - (n / (n + 1.0)) * P[n - 1];
+#ifndef SWS_EM_FULL_SERIES
+  if (s <= 1e-4) {
+    double t = (1.0 / 252.0) * P[5];            // B_6 / 6
+    t = fma(s, t, (-1.0 / 120.0) * P[3]);       // B_4 / 4
+    t = fma(s, t, (1.0 / 12.0) * P[1]);         // B_2 / 2
+    return s * t;
+  }
+#endif
+#pragma unroll
+  for (int n = 5; n <= 8; ++n)
+    P[n + 1] = ((2.0 * n + 1.0) / (n + 1.0)) * (mu * P[n]) - (n / (n + 1.0)) * P[n - 1];
+#ifndef SWS_EM_FULL_SERIES
+  if (s <= 1.5e-3) {
+    double t = (1.0 / 132.0) * P[9];            // B_10 / 10
+    t = fma(s, t, (-1.0 / 240.0) * P[7]);       // B_8 / 8
+    t = fma(s, t, (1.0 / 252.0) * P[5]);
+    t = fma(s, t, (-1.0 / 120.0) * P[3]);
+    t = fma(s, t, (1.0 / 12.0) * P[1]);
+    return s * t;
+  }
+#endif
+#pragma unroll
+  for (int n = 9; n <= 12; ++n)
     P[n + 1] = ((2.0 * n + 1.0) / (n + 1.0)) * (mu * P[n]) - (n / (n + 1.0)) * P[n - 1];
   double t = (1.0 / 12.0) * P[13];              // B_14 / 14
   t = fma(s, t, (-691.0 / 32760.0) * P[11]);    // B_12 / 12
