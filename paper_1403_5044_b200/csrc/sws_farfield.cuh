@@ -145,8 +145,9 @@ __device__ __forceinline__ double em_interval(const double a, const double b, co
   // keeps full relative accuracy when the interval is short against sqrt(g) (q -> 1).
   const double nb = ub >= 0.0 ? ub + rhob : g, db = ub >= 0.0 ? 1.0 : rhob - ub;
   const double na = ua >= 0.0 ? ua + rhoa : g, da = ua >= 0.0 ? 1.0 : rhoa - ua;
-  const double q = (nb * da) / (db * na);
-  return log1p((b - a) * (1.0 + q) / (rhoa + rhob)) - (tb - ta);
+  // (b - a)(1 + q) / (rho_a + rho_b) with q = (nb da) / (db na), as ONE quotient of sums of positive products
+  const double den = db * na;
+  return log1p((b - a) * fma(nb, da, den) / ((rhoa + rhob) * den)) - (tb - ta);
 }
 
 struct EmGeom {
