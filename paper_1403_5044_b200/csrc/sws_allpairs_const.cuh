@@ -158,8 +158,4 @@ cudaError_t SWS_CAT(const_bank_launch_, SWS_CONST_BANK)(const ConstArgs& a, cons
   return cudaGetLastError();
 }
 
-cudaError_t SWS_CAT(const_bank_occupancy_, SWS_CONST_BANK)(int* occ) {
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, k_allpairs_const, kConstThreads, 0);
-}
-
 }  // namespace sws

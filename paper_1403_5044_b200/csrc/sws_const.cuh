@@ -35,8 +35,6 @@ struct ConstArgs {
 
 cudaError_t const_bank_launch_0(const ConstArgs& a, const SrcRec* slab, const double* y, int tiles, cudaStream_t st);
 cudaError_t const_bank_launch_1(const ConstArgs& a, const SrcRec* slab, const double* y, int tiles, cudaStream_t st);
-cudaError_t const_bank_occupancy_0(int* occ);
-cudaError_t const_bank_occupancy_1(int* occ);
 
 // host side (sws_allpairs.cu)
 int const_slab_cols(int M);                 // columns per slab for this M (0: a column does not fit)
