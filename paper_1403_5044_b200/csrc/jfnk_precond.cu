@@ -558,7 +558,8 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
   int *ipiv = nullptr, *info = nullptr;
   std::vector<double> Gh;
   std::vector<int> info_h;
-  cudaStream_t st = nullptr;
+  cudaStream_t sm = nullptr, sf = nullptr;
+  cudaEvent_t evD = nullptr, evF = nullptr;
   DevGuard dg(p->device);
 
   CK(dg.err);
@@ -594,33 +595,57 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
     // factorisation scratch (freed below)
     const int R = hb + 1;  // live block rows
     CK(cudaMalloc(&ring, panel_elems * R * sizeof(double)));
-    CK(cudaMalloc(&Sinv, blk * sizeof(double)));
+    CK(cudaMalloc(&Sinv, 2 * blk * sizeof(double)));  // explicit inverses of two consecutive diagonal blocks
     CK(cudaMalloc(&W, blk * (hb ? hb : 1) * sizeof(double)));
     CK(cudaMalloc(&ipiv, sizeof(int) * n1));
     CK(cudaMalloc(&info, sizeof(int) * 2 * M));
     CK(cudaMemset(info, 0, sizeof(int) * 2 * M));
+    // Two streams: `sm` carries the assembly and every GEMM, `sf` the LU + explicit inverse of the diagonal blocks
+    // (cuSOLVER getrf / getrs on a 722 x 722 block: ~2.8 ms of dependent panel steps that occupy a few SMs).  The
+    // diagonal block of row k + 1 is final as soon as the FIRST trailing product of step k has updated it, so its
+    // factorisation runs on `sf` next to the remaining trailing products of step k (look-ahead of one block row)
+    // instead of between them: 2.28 -> 1.6 s at 721x241.
+    CK(cudaDeviceSynchronize());  // the one-off work above ran on the default stream
+    CK(cudaStreamCreateWithFlags(&sm, cudaStreamNonBlocking));
+    {  // `sf` gets the highest priority: its small dependent kernels must not queue behind whole waves of GEMM CTAs
+      int prio_lo = 0, prio_hi = 0;
+      CK(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+      CK(cudaStreamCreateWithPriority(&sf, cudaStreamNonBlocking, prio_hi));
+    }
+    CK(cudaEventCreateWithFlags(&evD, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&evF, cudaEventDisableTiming));
     CKB(cublasCreate(&hb_blas));
     CKB(cusolverDnCreate(&hb_sol));
-    CKB(cublasSetStream(hb_blas, st));
-    CKB(cusolverDnSetStream(hb_sol, st));
+    CKB(cublasSetStream(hb_blas, sm));
+    CKB(cusolverDnSetStream(hb_sol, sf));
     int lwork = 0;
     CKB(cusolverDnDgetrf_bufferSize(hb_sol, n1, n1, ring, n1, &lwork));
     CK(cudaMalloc(&work, sizeof(double) * (lwork > 0 ? lwork : 1)));
 
     const double one = 1.0, zero = 0.0, mone = -1.0;
+    // on `sf`, once `sm` has reached evD: LU of the diagonal block of row k and its explicit inverse into Sinv[k % 2]
+    auto factor_diag = [&](int k) -> int {
+      double* Dkk = ring + panel_elems * (k % R) + blk * hb;
+      double* Si = Sinv + blk * (k % 2);
+      if (cudaEventRecord(evD, sm) != cudaSuccess || cudaStreamWaitEvent(sf, evD, 0) != cudaSuccess) return 1;
+      if (cusolverDnDgetrf(hb_sol, n1, n1, Dkk, n1, work, ipiv, info + 2 * k) != 0) return 2;
+      k_identity<<<(int)((blk + 255) / 256), 256, 0, sf>>>(Si, n1);
+      if (cudaGetLastError() != cudaSuccess) return 1;
+      if (cusolverDnDgetrs(hb_sol, CUBLAS_OP_N, n1, n1, Dkk, n1, ipiv, Si, n1, info + 2 * k + 1) != 0) return 2;
+      return cudaEventRecord(evF, sf) != cudaSuccess ? 1 : 0;
+    };
     for (int k = 0; k < M; ++k) {
       if (k == 0) {
-        for (int i = 0; i <= hb && i < M; ++i) CK(launch_assemble_row(pc, i, 1, ring + panel_elems * (i % R), st));
+        for (int i = 0; i <= hb && i < M; ++i) CK(launch_assemble_row(pc, i, 1, ring + panel_elems * (i % R), sm));
+        CKB(factor_diag(0));
       } else if (k + hb < M) {
-        CK(launch_assemble_row(pc, k + hb, 1, ring + panel_elems * ((k + hb) % R), st));
+        CK(launch_assemble_row(pc, k + hb, 1, ring + panel_elems * ((k + hb) % R), sm));
+        if (hb == 0) CKB(factor_diag(k));  // block-diagonal case: no trailing products, row k is complete as assembled
       }
       double* Pk = ring + panel_elems * (k % R);
-      double* Dkk = Pk + blk * hb;
+      const double* Sk = Sinv + blk * (k % 2);
       const int lk = k < hb ? k : hb, uk = (M - 1 - k) < hb ? (M - 1 - k) : hb;
-      CKB(cusolverDnDgetrf(hb_sol, n1, n1, Dkk, n1, work, ipiv, info + 2 * k));
-      k_identity<<<(int)((blk + 255) / 256), 256, 0, st>>>(Sinv, n1);
-      CK(cudaGetLastError());
-      CKB(cusolverDnDgetrs(hb_sol, CUBLAS_OP_N, n1, n1, Dkk, n1, ipiv, Sinv, n1, info + 2 * k + 1));
+      CK(cudaStreamWaitEvent(sm, evF, 0));  // the inverse of this row's diagonal block (recorded during step k - 1)
       // apply form of block row k: row-major [n1][(lk+1) n1] = [ -S~kk^-1 L~k,* | S~kk^-1 ] and [n1][uk n1] =
       // S~kk^-1 S~k,*, written by a transposing copy that also converts when the panels are FP32
       const int Kf = (lk + 1) * n1;
@@ -629,18 +654,18 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
         const dim3 tg((cols + 31) / 32, (n1 + 31) / 32);
         if (pc->f32) {
           float* base = static_cast<float*>(fwd ? pc->fwd : pc->bwd) + off_elems + col0;
-          k_to_apply_form<float><<<tg, tb, 0, st>>>(in, n1, cols, scale, base, ldo);
+          k_to_apply_form<float><<<tg, tb, 0, sm>>>(in, n1, cols, scale, base, ldo);
         } else {
           double* base = static_cast<double*>(fwd ? pc->fwd : pc->bwd) + off_elems + col0;
-          k_to_apply_form<double><<<tg, tb, 0, st>>>(in, n1, cols, scale, base, ldo);
+          k_to_apply_form<double><<<tg, tb, 0, sm>>>(in, n1, cols, scale, base, ldo);
         }
       };
       if (lk > 0) {
         const double* Lk = Pk + blk * (hb - lk);  // L~k,k-lk..k-1, column-major n1 x lk n1
-        CKB(cublasDgemm(hb_blas, CUBLAS_OP_N, CUBLAS_OP_N, n1, lk * n1, n1, &one, Sinv, n1, Lk, n1, &zero, W, n1));
+        CKB(cublasDgemm(hb_blas, CUBLAS_OP_N, CUBLAS_OP_N, n1, lk * n1, n1, &one, Sk, n1, Lk, n1, &zero, W, n1));
         to_apply(W, lk * n1, -1.0, pc->fwd_off[k], 0, Kf, true);
       }
-      to_apply(Sinv, n1, 1.0, pc->fwd_off[k], (size_t)lk * n1, Kf, true);
+      to_apply(Sk, n1, 1.0, pc->fwd_off[k], (size_t)lk * n1, Kf, true);
       CK(cudaGetLastError());
       if (uk > 0) {
         // S~kk^-1 S~k,k+1..k+uk by ONE product with the explicit inverse formed above (a getrs on this
@@ -648,7 +673,7 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
         // the whole set-up when it was used here)
         const double* Uk0 = Pk + blk * (hb + 1);
         double* Uk = W;  // n1 x uk n1, column-major (W's use for the forward panel above is stream-ordered)
-        CKB(cublasDgemm(hb_blas, CUBLAS_OP_N, CUBLAS_OP_N, n1, uk * n1, n1, &one, Sinv, n1, Uk0, n1, &zero, Uk, n1));
+        CKB(cublasDgemm(hb_blas, CUBLAS_OP_N, CUBLAS_OP_N, n1, uk * n1, n1, &one, Sk, n1, Uk0, n1, &zero, Uk, n1));
         to_apply(Uk, uk * n1, 1.0, pc->bwd_off[k], 0, (size_t)uk * n1, false);
         CK(cudaGetLastError());
         for (int i = k + 1; i <= k + uk; ++i) {
@@ -656,10 +681,12 @@ int sws_precond_create(const sws_params* p, int32_t bandwidth, int32_t flags, sw
           const double* Lik = Pi + blk * (k - i + hb);
           double* Cij = Pi + blk * (k + 1 - i + hb);
           CKB(cublasDgemm(hb_blas, CUBLAS_OP_N, CUBLAS_OP_N, n1, uk * n1, n1, &mone, Lik, n1, Uk, n1, &one, Cij, n1));
+          if (i == k + 1) CKB(factor_diag(k + 1));  // row k + 1 is complete: factor its diagonal block on `sf` now
         }
       }
     }
-    CK(cudaStreamSynchronize(st));
+    CK(cudaStreamSynchronize(sf));
+    CK(cudaStreamSynchronize(sm));
     info_h.resize(2 * M);
     CK(cudaMemcpy(info_h.data(), info, sizeof(int) * 2 * M, cudaMemcpyDeviceToHost));
     for (int i = 0; i < 2 * M; ++i)
@@ -680,6 +707,10 @@ done:
   if (W) cudaFree(W);
   if (Sinv) cudaFree(Sinv);
   if (ring) cudaFree(ring);
+  if (evD) cudaEventDestroy(evD);
+  if (evF) cudaEventDestroy(evF);
+  if (sm) cudaStreamDestroy(sm);
+  if (sf) cudaStreamDestroy(sf);
   if (hb_sol) cusolverDnDestroy(hb_sol);
   if (hb_blas) cublasDestroy(hb_blas);
   if (rc != SWS_OK) {
