@@ -248,3 +248,28 @@ def test_const_path_host_threads(sws, oracle80):
     assert not errors, errors
     for i in range(2):
         assert relerr(results[i], refs[i]) <= TOL
+
+
+def test_const_path_repeatability_stress(sws):
+    """300 evaluations and 10 batches in a row on a mesh that takes the path by default (226x76, 15 slabs of 16
+    columns, two banks): every result bitwise equal to the first (arrival counters return to zero, the two bank
+    streams keep their slab order, no stale group sums)."""
+    import torch
+    cfg = W.custom(N=226, M=76, h=0.24, x1=-16.0, eps=1.0, amp=0.1, seed=5)
+    u, V = dev(W.state(cfg)), dev(W.directions(cfg, 3))
+    with sws.Context(cfg.params(), max_batch=3) as ctx:
+        assert ctx.const_plan_info()["active"]
+        F = torch.empty_like(u)
+        ref = ctx.residual(u).clone()
+        bad = 0
+        for _ in range(300):
+            ctx.residual(u, out=F)
+            bad += int(not torch.equal(F, ref))
+        JV0, Fp0, F00 = ctx.jv_batch(u, V, want_fpert=True, want_f0=True)
+        JV0, Fp0 = JV0.clone(), Fp0.clone()
+        assert torch.equal(F00, ref)
+        for _ in range(10):
+            JV, Fp, F0 = ctx.jv_batch(u, V, want_fpert=True, want_f0=True)
+            bad += int(not (torch.equal(JV, JV0) and torch.equal(Fp, Fp0) and torch.equal(F0, ref)))
+        torch.cuda.synchronize()
+    assert bad == 0
