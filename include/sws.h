@@ -155,9 +155,10 @@ size_t sws_workspace_bytes(const sws_ctx* ctx);
 /* Number of kernels the last sws_residual / sws_jv_batch call launched. */
 int sws_last_launch_count(const sws_ctx* ctx);
 
-/* Time (ms, CUDA events on `cuda_stream`) of the all-pairs kernel alone for `states`
- * states (1 = single residual) using the fields left by the previous call; used by
- * bench.py for the roofline of the dominant kernel.  Synchronises. */
+/* Time (ms, CUDA events on `cuda_stream`) of the all-pairs phase alone for `states`
+ * states (1 = single residual) using the fields left by the previous call: one launch of the staged
+ * kernel, or the slab launches of the constant-bank path (sws_set_const_path) without the finishing
+ * kernel; used by bench.py --experiments.  Synchronises. */
 int sws_time_allpairs(sws_ctx* ctx, int32_t states, int32_t reps, float* ms_per_launch,
                       void* cuda_stream);
 
@@ -181,16 +182,17 @@ int sws_time_allpairs_lin(sws_ctx* ctx, int32_t reps, float* ms_per_launch, void
 int sws_lin_plan_info(sws_ctx* ctx, int32_t b, int32_t* out6);
 
 /* Live timing of the dominant kernel inside ordinary calls.  While profiling is on, every
- * sws_residual / sws_jv_batch / sws_jv_exact_batch brackets its all-pairs launch with a CUDA event pair on the
+ * sws_residual / sws_jv_batch / sws_jv_exact_batch brackets its all-pairs phase (one launch of the staged kernel, or
+ * the slab launches of the constant-bank path with their fork / join) with a CUDA event pair on the
  * call's stream (no synchronisation, two event records per call).  sws_profile_read
  * synchronises those events and returns the summed all-pairs time (ms) and the number of
- * launches since the last reset; reset != 0 clears the list. */
+ * phases since the last reset; reset != 0 clears the list. */
 int sws_set_profiling(sws_ctx* ctx, int32_t on);
 int sws_profile_read(sws_ctx* ctx, double* allpairs_ms, int32_t* launches, int32_t reset);
 
-/* Tuning knob of the all-pairs launch: number of source-column groups a target tile's
+/* Tuning knob of the STAGED all-pairs launch: number of source-column groups a target tile's
  * quadrature is split into (0 = library default, chosen from the SM count and occupancy;
- * clamped to what the workspace was sized for). */
+ * clamped to what the workspace was sized for).  The constant-bank path ignores it. */
 int sws_set_tuning(sws_ctx* ctx, int32_t chunks);
 
 /* Batched all-pairs launches (sws_jv_batch) let one CTA carry `ns` states: the y_j run is staged once and
