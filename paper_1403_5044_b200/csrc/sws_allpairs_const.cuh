@@ -35,6 +35,9 @@
 #ifndef SWS_CONST_UNROLL
 #define SWS_CONST_UNROLL 8  // nodes per inner-loop iteration (4 / 8 / 12: 50.9 / 49.4 / 49.8 ms per state at 721x241)
 #endif
+#ifndef SWS_CONST_ROTATE
+#define SWS_CONST_ROTATE 1  // 0: plain unrolled loop
+#endif
 #ifndef SWS_CONST_MINB
 #define SWS_CONST_MINB 8  // resident CTAs per SM (caps the kernel at 128 registers)
 #endif
@@ -62,8 +65,36 @@ __device__ __forceinline__ void walk_column_const(const int rbase, const int M, 
   node(0, h1, hS);
   col1 = 0.5 * h1;
   colS = 0.5 * hS;
+#if SWS_CONST_ROTATE
+  {
+    // The first node of every unrolled group is loaded one group ahead: ptxas issues the LDCU.64 of a group at the
+    // top of its body, so the group's first DADDs (y_j - y*, zeta_j - zeta*) would wait out the whole load latency
+    // (short-scoreboard stalls, profiles/r2b_allpairs_const_ncu.md); with one node in flight across the back edge they
+    // do not: 48.9 -> 48.6 ms per state at 721x241, 3.32 -> 3.28 ms at 361x121.  Same terms in the same order.
+    struct NodeData { double yj; double2 zp, sl; };
+    auto load = [&](const int j) {
+      NodeData d;
+      d.yj = c_buf[j];
+      const double* r = c_buf + rbase + 4 * j;
+      d.zp = make_double2(r[0], r[1]);
+      d.sl = make_double2(r[2], r[3]);
+      return d;
+    };
+    int j = 1;
+    NodeData pre = load(j);
+    for (; j + kConstUnroll <= M - 1; j += kConstUnroll) {
+      const NodeData nxt = load(j + kConstUnroll < M ? j + kConstUnroll : M - 1);  // stays inside the column
+      pair_term<S2T>(pre.zp, pre.sl, pre.yj, pre.yj - tg.ys, tg, ts, cg, cs, col1, colS);
+#pragma unroll
+      for (int u = 1; u < kConstUnroll; ++u) node(j + u, col1, colS);
+      pre = nxt;
+    }
+    for (; j < M - 1; ++j) node(j, col1, colS);
+  }
+#else
 #pragma unroll kConstUnroll
   for (int j = 1; j < M - 1; ++j) node(j, col1, colS);
+#endif
   h1 = hS = 0.0;
   node(M - 1, h1, hS);
   col1 = fma(0.5, h1, col1);
