@@ -241,6 +241,34 @@ int sws_farfield_stats(sws_ctx* ctx, int32_t states, double* near_fraction, void
  * columns per group, nodes staged per bulk copy, segments per column}. */
 int sws_plan_info(sws_ctx* ctx, int32_t states, int32_t* out5);
 
+/* The shifts of eq. (25), sigma_b = 1e-7 (1 + ||u||_2) / ||v_b||_2 (0 for a zero direction), WITHOUT a context
+ * and without any allocation: sigma_dev[r] for the b rows v_r of V_dev[b][n] (row-major), r = 0 .. b-1.  The values are
+ * bitwise those sws_jv_batch(sigma_host = NULL) uses and sws_last_sigma reports.
+ *
+ * For callers that cannot allocate device memory where they need the shifts - a solver embedded in an application
+ * that handed all device memory to its own pool at start-up (cudaMalloc fails there, or takes what the application
+ * thinks it owns), or a continuation / time-stepping loop that cannot afford the device-wide stall of cudaMalloc and
+ * cudaFree - and for Krylov drivers that want the shifts alone and no context (sws_setup allocates the whole
+ * workspace).  The call itself never calls cudaMalloc, cudaFree or a library routine that allocates.
+ *
+ * Where the scratch memory is: the block partial sums of the two-stage 2-norm live in ONE fixed array inside the
+ * library's device image, (SWS_NOALLOC_MAX_B + 1) x 64 doubles = 33,280 bytes.  Every GPU that loads libsws.so
+ * holds that array until the process exits, whether this function is called or not.  Consequences:
+ *   - b > SWS_NOALLOC_MAX_B is refused with SWS_EBATCH (split the batch); n must be 1 .. 2^31 - 1.
+ *   - All calls on one device share the array.  It keeps the last call's contents; no slot is read before the same
+ *     call has written it, so nothing needs clearing between calls.  Two calls whose kernels can OVERLAP on the GPU
+ *     (different streams without an ordering between them, or two host threads) race on it and both results are
+ *     undefined: order them with an event or keep them on one stream.  Calls on different devices do not interact.
+ *   - The FIRST call on each device also asks the runtime for the array's device address (cudaGetSymbolAddress, once
+ *     per device, kept for the life of the process).  Make that first call eagerly, before any stream capture begins.
+ * u_dev [n], V_dev [b][n], sigma_dev [b]: device memory on `device`, owned by the caller, FP64.  Asynchronous on
+ * `cuda_stream`; runs on `device` and restores the caller's current device.  Returns SWS_OK, SWS_EINVAL, SWS_EBATCH or
+ * SWS_ECUDA; sws_noalloc_last_error() returns this thread's message for the last failed call ("" after a success). */
+#define SWS_NOALLOC_MAX_B 64
+int sws_fd_shifts_noalloc(const double* u_dev, const double* V_dev, int64_t n, int32_t b, double* sigma_dev,
+                          int32_t device, void* cuda_stream);
+const char* sws_noalloc_last_error(void);
+
 int sws_destroy(sws_ctx* ctx);
 
 const char* sws_strerror(int code);

@@ -28,7 +28,10 @@ SYMBOLS = (
     "sws_get_params", "sws_linearize", "sws_jv_apply",
     "sws_set_farfield", "sws_farfield_stats", "sws_set_eps", "sws_get_fields_host", "sws_set_states_per_cta", "sws_time_residual", "sws_set_fused_fields",
     "sws_set_const_path", "sws_const_plan_info",
+    "sws_fd_shifts_noalloc", "sws_noalloc_last_error",
 )
+
+NOALLOC_MAX_B = 64  # SWS_NOALLOC_MAX_B of include/sws.h
 
 
 class SwsParams(C.Structure):
@@ -92,6 +95,8 @@ def load_library() -> C.CDLL:
         "sws_time_residual": (C.c_int, [vp, dp, dp, C.c_int32, C.POINTER(C.c_float), vp]),
         "sws_set_fused_fields": (C.c_int, [vp, C.c_int32]),
         "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
+        "sws_fd_shifts_noalloc": (C.c_int, [dp, dp, C.c_int64, C.c_int32, dp, C.c_int32, vp]),
+        "sws_noalloc_last_error": (C.c_char_p, []),
     }
     for name, (res, args) in proto.items():
         fn = getattr(lib, name)
@@ -116,6 +121,32 @@ def _np_ptr(a: np.ndarray):
 def _torch():
     import torch
     return torch
+
+
+def fd_shifts_noalloc(u, V, out, stream=None):
+    """sws_fd_shifts_noalloc: out[r] = 1e-7 (1 + |u|_2) / |V[r]|_2 (eq. (25) L219 shifts; 0 for a zero row), with no
+    context and no device allocation anywhere in the call - for programs that cannot cudaMalloc where they need the
+    shifts (all device memory already handed to the host application's pool; a loop that cannot take cudaMalloc's
+    device-wide stall).  The caller therefore brings the output too: u [n], V [b, n], out [b], contiguous float64
+    CUDA tensors on one device, b <= NOALLOC_MAX_B.  The scratch of the reduction is one fixed 33 KB array inside
+    libsws.so that all calls on a device share: do not let two calls overlap on the GPU (keep them on one stream or
+    order them with an event).  Asynchronous on `stream` (default: torch's current stream).  Returns `out`."""
+    torch = _torch()
+    lib = load_library()
+    for name, t in (("u", u), ("V", V), ("out", out)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and t.device == u.device):
+            raise SwsError(f"{name}: need a contiguous float64 CUDA tensor on the device of u")
+    if u.dim() != 1 or V.dim() != 2 or V.shape[1] != u.shape[0] or tuple(out.shape) != (V.shape[0],):
+        raise SwsError("fd_shifts_noalloc: need u [n], V [b, n], out [b]")
+    dev_index = u.device.index if u.device.index is not None else torch.cuda.current_device()
+    s = stream if stream is not None else torch.cuda.current_stream(dev_index)
+    rc = lib.sws_fd_shifts_noalloc(C.c_void_p(u.data_ptr()), C.c_void_p(V.data_ptr()), int(u.shape[0]),
+                                   int(V.shape[0]), C.c_void_p(out.data_ptr()), int(dev_index),
+                                   C.c_void_p(s.cuda_stream))
+    if rc != SWS_OK:
+        raise SwsError(f"sws_fd_shifts_noalloc failed ({rc}): {lib.sws_noalloc_last_error().decode()}")
+    return out
 
 
 class Context:

@@ -18,7 +18,7 @@ LIB_JFNK = PKG / "libsws_jfnk.so"  # the Newton-Krylov driver: calls libsws thro
 SOURCES_JFNK = ["jfnk_precond.cu", "jfnk_solver.cu"]
 CUDA_LIB64 = "/usr/local/cuda/lib64"
 SOURCES = ["sws_api.cu", "sws_fields.cu", "sws_allpairs.cu", "sws_allpairs_c0.cu", "sws_allpairs_c1.cu",
-           "sws_allpairs_f32.cu", "sws_jv_exact.cu"]
+           "sws_allpairs_f32.cu", "sws_jv_exact.cu", "sws_noalloc.cu"]
 # test hooks and FP64 issue-rate probes (include/sws_debug.h): a library of its own, not part of the product
 LIB_DEBUG = PKG / "libsws_debug.so"
 SOURCES_DEBUG = ["sws_debug.cu", "sws_probe.cu"]
