@@ -73,6 +73,7 @@ class Oracle:
             ("sigma", C.c_double, [C.c_int, _dp, _dp]),
             ("fields", C.c_int, [C.POINTER(_Params), _dp, _dp, _dp, _dp, _dp]),
             ("e2_terms", C.c_int, [C.POINTER(_Params), _dp, C.c_int, C.c_int, _dp]),
+            ("row_abc", C.c_int, [C.POINTER(_Params), _dp, C.c_int, C.c_int, _dp, _dp]),
             ("pair_kernels", None, [C.c_double] * 11 + [_dp]),
             ("s2_integral", C.c_double, [C.c_double] * 9),
             ("box_integral", C.c_double, [C.c_double] * 7),
@@ -169,6 +170,15 @@ class Oracle:
         if rc:
             raise RuntimeError(f"sws_oracle_e2_terms rc={rc}")
         return out
+
+    def row_abc(self, p: dict, u, k: int, l: int):
+        """(A, B, C, zeta*) of L177 / L162 exactly as the row E2_{k,l} of the residual uses them (0-based k, l)."""
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        out, zs = np.empty(3), C.c_double()
+        rc = self._f["row_abc"](C.byref(self._params(p)), _d(u), int(k), int(l), _d(out), C.byref(zs))
+        if rc:
+            raise RuntimeError(f"sws_oracle_row_abc rc={rc}")
+        return float(out[0]), float(out[1]), float(out[2]), float(zs.value)
 
     def pair_kernels(self, x, y, zeta, zeta_x, zeta_y, xs, ys, zetas, A, B, C_):
         out = np.empty(3)

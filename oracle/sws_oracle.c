@@ -48,8 +48,11 @@
  * single-line mutations of THIS file and requires the named pin to fail on each.
  * The paper prints no numeric value of E for any worked example, so what pins
  * the residual at an arbitrary u is PG2 (to the O(h^2) discretisation error)
- * and P1b/P7 (to round-off); the nonlinear cross terms of the Bernoulli row E1
- * and A, B, C of L177 are pinned by restating the printed formula only.
+ * and P1b/P7 (to round-off).  The nonlinear terms of the Bernoulli row E1 are pinned
+ * by PB (an exact potential flow a x + b y + c z under a doubly tilted plane: the first
+ * term of (13) must return (a^2 + b^2 + c^2)/2 with all four slopes and the cross term
+ * live) and A, B, C of L177 by PS (S2 is the singular part of K2: h (K2 - S2) -> 0 at
+ * the nodes next to a target under refinement, only for these A, B, C).
  */
 #include <math.h>
 #include <stdlib.h>
@@ -320,6 +323,19 @@ static REAL weight(const sws_oracle_params *p, int i, int j) {
   return (REAL)p->dx * (REAL)p->dy * ci * cj;
 }
 
+/* A, B, C of L177 at the half-mesh point (k, l): the coefficients of the quadratic form
+ *   A (x - x*)^2 + B (x - x*)(y - y*) + C (y - y*)^2
+ * under the square root of S2 (L169-172), from the starred slopes.  The ONE place they are
+ * formed: E2_row, E2_terms and sws_oracle_row_abc all call this.
+ * Pin (test_PS_S2_is_the_singular_part_of_K2): S2 exists to cancel the 1/R singularity of K2
+ * at the target, so R^2 = Q + O(h^3) at the nodes next to it, i.e. h (K2 - S2) -> 0 under
+ * mesh refinement - which holds only for these A, B, C. */
+static void star_ABC(const fields_t *f, int k, int l, REAL *A, REAL *B, REAL *C) {
+  int N = f->N;
+  REAL zxs = STAR(f->zeta_x, k, l), zys = STAR(f->zeta_y, k, l);
+  *A = 1 + zxs * zxs; *B = 2 * zxs * zys; *C = 1 + zys * zys; /* L177 */
+}
+
 /* The six pieces of E2_{k,l} (0-based k = 0..N-2, l = 0..M-1):
  * out[0] = 2 pi (phi* - x*)
  * out[1] = eps / sqrt(x*^2 + y*^2 + (zeta* + 1)^2)
@@ -333,8 +349,9 @@ static void E2_terms(const sws_oracle_params *p, const fields_t *f, int k, int l
   int N = f->N, M = f->M;
   REAL xs = (f->x[k] + f->x[k + 1]) / 2, ys = f->y[l];        /* L162 */
   REAL zs = STAR(f->zeta, k, l), ps = STAR(f->phi, k, l);
-  REAL zxs = STAR(f->zeta_x, k, l), zys = STAR(f->zeta_y, k, l);
-  REAL A = 1 + zxs * zxs, B = 2 * zxs * zys, C = 1 + zys * zys; /* L177 */
+  REAL zxs = STAR(f->zeta_x, k, l);
+  REAL A, B, C;
+  star_ABC(f, k, l, &A, &B, &C);
   REAL s1 = 0, s2 = 0, s3 = 0;
   for (int j = 0; j < M; ++j)
     for (int i = 0; i < N; ++i) {
@@ -358,8 +375,9 @@ static REAL E2_row(const sws_oracle_params *p, const fields_t *f, int k, int l) 
   int N = f->N, M = f->M;
   REAL xs = (f->x[k] + f->x[k + 1]) / 2, ys = f->y[l];
   REAL zs = STAR(f->zeta, k, l), ps = STAR(f->phi, k, l);
-  REAL zxs = STAR(f->zeta_x, k, l), zys = STAR(f->zeta_y, k, l);
-  REAL A = 1 + zxs * zxs, B = 2 * zxs * zys, C = 1 + zys * zys;
+  REAL zxs = STAR(f->zeta_x, k, l);
+  REAL A, B, C;
+  star_ABC(f, k, l, &A, &B, &C);
   REAL sum = 0;
   for (int j = 0; j < M; ++j)
     for (int i = 0; i < N; ++i) {
@@ -501,6 +519,21 @@ int FN(sws_oracle_e2_terms)(const sws_oracle_params *p, const double *u, int k, 
   E2_terms(p, &f, k, l, o, &zxs);
   for (int i = 0; i < 6; ++i) out[i] = (double)RE(o[i]);
   out[6] = (double)RE(zxs);
+  fields_free(&f);
+  return 0;
+}
+
+/* out3 = {A, B, C} the rows E2_{k,l} use (0-based k, l), and *zs_out = zeta* (optional). */
+int FN(sws_oracle_row_abc)(const sws_oracle_params *p, const double *u, int k, int l, double *out3, double *zs_out) {
+  if (k < 0 || k >= p->N - 1 || l < 0 || l >= p->M) return -1;
+  fields_t f;
+  int rc = fields_build(p, u, u, 0, &f);
+  if (rc) return rc;
+  int N = f.N;
+  REAL A, B, C;
+  star_ABC(&f, k, l, &A, &B, &C);
+  out3[0] = (double)RE(A); out3[1] = (double)RE(B); out3[2] = (double)RE(C);
+  if (zs_out) *zs_out = (double)RE(STAR(f.zeta, k, l));
   fields_free(&f);
   return 0;
 }

@@ -104,11 +104,23 @@ MUTANTS = [
      "+ 0 * box_integral(A, B, C, xa - xs, xb - xs, -(yb + ys), -(ya + ys));",
      f"{PINS}::test_P5_S2_integral_is_direct_plus_image"),
     ("A, B, C: B = zeta_x* zeta_y* (factor 2 lost)",
-     "REAL A = 1 + zxs * zxs, B = 2 * zxs * zys, C = 1 + zys * zys;\n  REAL sum = 0;",
-     "REAL A = 1 + zxs * zxs, B = zxs * zys, C = 1 + zys * zys;\n  REAL sum = 0;",
+     "*A = 1 + zxs * zxs; *B = 2 * zxs * zys; *C = 1 + zys * zys;",
+     "*A = 1 + zxs * zxs; *B = zxs * zys; *C = 1 + zys * zys;",
      # (any A, B, C used in both S2 and I still converges -- only more slowly -- so Green's identity cannot
-     # see this one; L177 as printed, restated in the pin, does)
-     f"{PINS}::test_P1b_residual_row_is_eq12_with_its_printed_signs"),
+     # see this one; what sees it is that S2 must cancel the singularity of K2 at the target)
+     f"{PINS}::test_PS_S2_is_the_singular_part_of_K2"),
+    ("A, B, C: A and C from the wrong slopes",
+     "*A = 1 + zxs * zxs; *B = 2 * zxs * zys; *C = 1 + zys * zys;",
+     "*A = 1 + zys * zys; *B = 2 * zxs * zys; *C = 1 + zxs * zxs;",
+     f"{PINS}::test_PS_S2_is_the_singular_part_of_K2"),
+    ("A, B, C: sign of B",
+     "*A = 1 + zxs * zxs; *B = 2 * zxs * zys; *C = 1 + zys * zys;",
+     "*A = 1 + zxs * zxs; *B = -2 * zxs * zys; *C = 1 + zys * zys;",
+     f"{PINS}::test_PS_S2_is_the_singular_part_of_K2"),
+    ("A, B, C: the row and the term-by-term routine no longer share them",
+     "  star_ABC(f, k, l, &A, &B, &C);\n  REAL sum = 0;",
+     "  star_ABC(f, k, l, &A, &B, &C); B = B / 2;\n  REAL sum = 0;",
+     f"{PINS}::test_e2_terms_tie_to_residual_row"),
     # --- weights, reconstruction, spline, midpoints ---
     ("trapezoid weight: full weight on the first/last column",
      "REAL ci = (i == 0 || i == p->N - 1) ? (REAL)0.5 : (REAL)1;",
@@ -142,11 +154,19 @@ MUTANTS = [
     ("E1: sign of the cross term",
      "- 2 * zx * zy * px * py)",
      "+ 2 * zx * zy * px * py)",
-     f"{PINS}::test_E1_bernoulli_formula"),
+     f"{PINS}::test_PB_bernoulli_row_on_exact_tilted_plane_flow"),
     ("E1: phi_x and phi_y transposed",
      "((1 + zx * zx) * py * py + (1 + zy * zy) * px * px",
      "((1 + zx * zx) * px * px + (1 + zy * zy) * py * py",
-     f"{PINS}::test_E1_bernoulli_formula"),
+     f"{PINS}::test_PB_bernoulli_row_on_exact_tilted_plane_flow"),
+    ("E1: factor 2 of the cross term lost",
+     "- 2 * zx * zy * px * py)",
+     "- zx * zy * px * py)",
+     f"{PINS}::test_PB_bernoulli_row_on_exact_tilted_plane_flow"),
+    ("E1: denominator without zeta_y^2",
+     "/ (1 + zx * zx + zy * zy) / 2",
+     "/ (1 + zx * zx) / 2",
+     f"{PINS}::test_PB_bernoulli_row_on_exact_tilted_plane_flow"),
     ("E4: second derivative taken at the wrong nodes",
      "e[1] = x1 * ((f.phi_x[AT(1, l)] - f.phi_x[AT(0, l)]) / dx)",
      "e[1] = x1 * ((f.phi_x[AT(2, l)] - f.phi_x[AT(1, l)]) / dx)",

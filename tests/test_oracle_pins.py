@@ -444,6 +444,109 @@ def test_E1_bernoulli_formula(oracle64):
 
 
 # ----------------------------------------------------------------------------
+# PB the Bernoulli row on an EXACT potential flow (pins the nonlinear terms of eq. (13) L113 with all
+# four slopes and the cross term live, by something the formula is not: the speed of a uniform stream).
+#   Phi = a x + b y + c z is harmonic; the plane zeta = alpha x + beta y + gamma is a stream surface of it iff
+#   Phi_x zeta_x + Phi_y zeta_y = Phi_z, i.e. c = a alpha + b beta (the kinematic condition, eq. (8)).
+#   On the surface phi(x, y) = Phi(x, y, zeta(x, y)):  phi_x = a + c alpha,  phi_y = b + c beta.
+#   The first term of (13) is |grad Phi|^2 / 2 written in (phi_x, phi_y, zeta_x, zeta_y) with the kinematic
+#   condition eliminated, so here it must return (a^2 + b^2 + c^2) / 2 EXACTLY:
+#       E1 = (a^2 + b^2 + c^2) / 2 + zeta* / F^2 - 1/2.
+#   A wrong sign of the cross term, phi_x / phi_y (or zeta_x / zeta_y) transposed, a lost factor 2 or a wrong
+#   denominator all change the value at O(1) of the slopes.  y_1 != 0, so that the y-derivatives of data linear
+#   in y are exact in both schemes (not-a-knot spline at both ends; one-sided 3-point differences) - with
+#   y_1 = 0 the even-extension end condition of reading Q3 would force zeta_y = 0 on the first line.
+# ----------------------------------------------------------------------------
+@pytest.mark.parametrize("scheme", [0, 1])
+@pytest.mark.parametrize("flow", [(1.0, 0.35, 0.3, -0.2), (0.8, -0.5, -0.25, 0.4), (1.1, 0.0, 0.2, 0.3)])
+def test_PB_bernoulli_row_on_exact_tilted_plane_flow(oracle64, oracle80, scheme, flow):
+    a, b, alpha, beta = flow
+    gamma = 0.07
+    cz = a * alpha + b * beta                                  # kinematic condition
+    c = dataclasses.replace(small(N=9, M=7, h=0.35, x1=-1.3), y1=0.6, froude=0.8)
+    x, y = W.mesh(c)
+    zeta1 = alpha * x[0] + beta * y + gamma
+    phi1 = a * x[0] + b * y + cz * zeta1
+    u = W.pack(c, phi1, np.full((c.M, c.N), a + cz * alpha), zeta1, np.full((c.M, c.N), alpha))
+    for orc, tol in ((oracle64, 2e-15), (oracle80, 1e-15)):
+        zeta, phi, zeta_y, phi_y = orc.fields(c.params(scheme), u)
+        # the reconstruction hands the row the slopes of the exact flow (else the pin below tests nothing)
+        np.testing.assert_allclose(zeta_y, beta, rtol=0, atol=1e-13)
+        np.testing.assert_allclose(phi_y, b + cz * beta, rtol=0, atol=1e-13)
+        E = orc.residual(c.params(scheme), u, rows=[])
+        E1 = E[: (c.N + 1) * c.M].reshape(c.M, c.N + 1)[:, 2:]
+        xs = 0.5 * (x[:-1] + x[1:])
+        zs = alpha * xs[None, :] + beta * y[:, None] + gamma
+        ref = 0.5 * (a * a + b * b + cz * cz) + zs / c.froude ** 2 - 0.5
+        np.testing.assert_allclose(E1, ref, rtol=0, atol=200 * tol)
+    # the pin has power: the slopes and the cross term are all of order 0.1 .. 1
+    zx, zy, px, py = alpha, beta, a + cz * alpha, b + cz * beta
+    assert min(abs(zx), abs(zy), abs(px)) > 0.1 and abs(2 * zx * zy * px * py) > 1e-3 or b == 0.0
+    assert abs(((1 + zx * zx) * px * px + (1 + zy * zy) * py * py) - ((1 + zx * zx) * py * py + (1 + zy * zy) * px * px)) > 1e-2
+
+
+# ----------------------------------------------------------------------------
+# PS  A, B, C of L177: S2 is the singular part of K2.
+#   L164-181: S2 = 1/sqrt(A dx^2 + B dx dy + C dy^2) is subtracted because it has the SAME singularity as
+#   K2 = 1/R at the target, R^2 = dx^2 + dy^2 + (zeta - zeta*)^2.  With zeta - zeta* = zeta_x* dx + zeta_y* dy
+#   + O(h^2) at a node next to the target, R^2 = Q + O(h^3) if and only if Q's coefficients are
+#   A = 1 + zeta_x*^2, B = 2 zeta_x* zeta_y*, C = 1 + zeta_y*^2; then 1/R - 1/sqrt(Q) stays bounded and
+#       h (K2 - S2) = O(h) -> 0   under h -> h/3 -> h/9 (the half-mesh points of mesh h are half-mesh points of
+#   mesh h/3: k' = 3k + 1, l' = 3l), whereas any other coefficient leaves R^2 - Q = O(h^2) and h (K2 - S2) tends
+#   to a non-zero constant.  The six nodes around the target see all three coefficients: (dx, dy) =
+#   (+-h/2, 0) isolates A, (+-h/2, +-h) mixes A, B, C with both signs of dx dy.  A, B, C are the ROW'S OWN
+#   (oracle.row_abc calls the helper E2_row calls), K2 and S2 are the oracle's pair kernels (pinned by P1/P2);
+#   the image parts of both are smooth at the target (y* >= 2 h_0) and drop out of the limit.
+# ----------------------------------------------------------------------------
+def _near_field_mismatch(orc, c, k, l, abc_of=lambda A, B, C: (A, B, C)):
+    """max over the six nodes around target (k, l) of h |K2 - S2|, and the row's (A, B, C)."""
+    p, u = c.params(), W.state(c)
+    x, y = W.mesh(c)
+    zeta, _, zeta_y, _ = orc.fields(p, u)
+    zeta_x = u[(c.N + 1) * c.M:].reshape(c.M, c.N + 1)[:, 1:]
+    A, B, C, zs = orc.row_abc(p, u, k, l)
+    A2, B2, C2 = abc_of(A, B, C)
+    xs, ys = 0.5 * (x[k] + x[k + 1]), y[l]
+    worst = 0.0
+    for j in (l - 1, l, l + 1):
+        for i in (k, k + 1):
+            K1, K2, S2 = orc.pair_kernels(x[i], y[j], zeta[j, i], zeta_x[j, i], zeta_y[j, i], xs, ys, zs, A2, B2, C2)
+            worst = max(worst, c.h * abs(K2 - S2))
+    return worst, (A, B, C)
+
+
+def test_PS_S2_is_the_singular_part_of_K2(oracle64):
+    base = W.custom(N=9, M=7, h=0.6, x1=8.3, amp=0.6, seed=20, eps=0.3)
+    # the interior target where zeta_x* zeta_y* is largest on the coarse mesh (B matters most there)
+    best, kl = 0.0, None
+    for l in range(2, base.M - 1):
+        for k in range(1, base.N - 2):
+            A, B, C, _ = oracle64.row_abc(base.params(), W.state(base), k, l)
+            if abs(B) > best:
+                best, kl = abs(B), (k, l)
+    assert best > 0.05, best                  # slopes of order 0.2: the wrong-B constant is far above round-off
+    got, wrong_B, wrong_AC = [], [], []
+    k, l = kl
+    for r in range(3):
+        f = 3 ** r
+        c = dataclasses.replace(base, N=(base.N - 1) * f + 1, M=(base.M - 1) * f + 1, h=base.h / f)
+        d, (A, B, C) = _near_field_mismatch(oracle64, c, k, l)
+        got.append(d)
+        # L177 restated nowhere: what the row's own coefficients must do is make `got` vanish; for contrast,
+        # the same measurement with B halved and with A, C swapped
+        wrong_B.append(_near_field_mismatch(oracle64, c, k, l, lambda A, B, C: (A, B / 2, C))[0])
+        wrong_AC.append(_near_field_mismatch(oracle64, c, k, l, lambda A, B, C: (C, B, A))[0])
+        k, l = 3 * k + 1, 3 * l
+    got, wrong_B, wrong_AC = map(np.array, (got, wrong_B, wrong_AC))
+    # O(h): each refinement by 3 divides it by about 3 (measured 4.9, 4.0, then 3.4: the O(h^2) part dies out;
+    # accept 2 .. 6), and it ends far below the wrong ones, which stay where they were
+    assert (got[:-1] / got[1:] > 2.0).all() and (got[:-1] / got[1:] < 6.0).all(), got
+    assert got[-1] < 0.15 * got[0]
+    assert (wrong_B[-1] > 0.7 * wrong_B[0]) and (wrong_AC[-1] > 0.7 * wrong_AC[0]), (wrong_B, wrong_AC)
+    assert got[-1] < 0.2 * min(wrong_B[-1], wrong_AC[-1]), (got, wrong_B, wrong_AC)
+
+
+# ----------------------------------------------------------------------------
 # P8 O(h^2) convergence of E2 under h -> h/3 (midpoints coincide: k' = 3k+1, l' = 3l, 0-based)
 # ----------------------------------------------------------------------------
 def test_P8_second_order_convergence(oracle64):
