@@ -316,7 +316,7 @@ def solve_report(sws, device: int, names=("paper_361x121", "paper_721x241"), ban
             u, log, st = s.newton(u0, **kw)
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
-            out[name] = {"solve_s": dt,
+            out[name] = {"solve_s": dt, "precond_panels": "fp32",
                          "fd_jv": {"solve_s": dt_fd, "newton_steps": st_fd["steps"], "converged": st_fd["converged"],
                                    "jv_products": st_fd["jv_products"], "residual_evals": st_fd["residual_evals"],
                                    "final_residual_inf": log_fd[-1]["finf"], "ms_jv": st_fd["ms_jv"],
@@ -350,11 +350,13 @@ def solve_report(sws, device: int, names=("paper_361x121", "paper_721x241"), ban
                               "jv_products": st["jv_products"], "residual_evals": st["residual_evals"],
                               "final_residual_inf": log[-1]["finf"],
                               "gmres_its_per_step": [e["gmres_its"] for e in log[:-1]]},
-            "precond_setup_s": pc.setup_ms * 1e-3, "block_bandwidth": pc.bandwidth}
+            "precond_setup_s": pc.setup_ms * 1e-3, "block_bandwidth": pc.bandwidth, "precond_panels": "fp32"}
     out["block_krylov_721x241"] = block_krylov_report(sws, jf, device, bandwidth)
     out["note"] = ("flat initial guess, eps=1, F=0.7, ||E||_inf <= 1e-9, inexact Newton eta=1e-3, analytic Jv "
                    "(sws_linearize + sws_jv_apply; `fd_jv`: eq. (25) quotients, jv_mode 2, one sws_residual per "
-                   "product; `fd_jv_forcing`: the same with Eisenstat-Walker forcing terms, eta_max 0.5), block-banded linear-Jacobian preconditioner; paper (other "
+                   "product; `fd_jv_forcing`: the same with Eisenstat-Walker forcing terms, eta_max 0.5), block-banded linear-Jacobian preconditioner "
+                   "with its factor panels stored in FP32 (`precond_panels`; since round 2: solve and apply times are not "
+                   "comparable with round 1's FP64 panels); paper (other "
                    "hardware, KINSOL + FD Jv): 361x121 in ~3.5 min and 721x241 in 1.5 h on a Tesla M2090 workstation")
     return out
 
@@ -652,6 +654,15 @@ def run_ours(args) -> None:
         "frac_of_peak_measured": achieved_tf / peak_measured_tf if peak_measured_tf else None,
         "traffic_note": "DRAM bytes (read + written) of one launch; " + alg_note,
         "algorithmic_bytes_per_launch": alg_bytes,
+        # per STATE the picture differs on the constant-bank path: every one of the slab launches re-reads the target
+        # records and the accumulators, so one state moves (launches x per-launch traffic) through DRAM / L2 where the
+        # algorithm needs the fields once: S*32 + T*64 + 2*T*8 bytes.  The re-read costs ~25 GB/s (0.4 % of HBM
+        # bandwidth) at cfg5 - the kernel is bound by the FP64 pipe - but it is stated here, not hidden.
+        "traffic_per_state": (NCU_DRAM_BYTES_PER_LAUNCH[kernel].get(cfg.name) or 0) * (cinfo["slabs"] if cinfo["active"] else 1) or None,
+        "algorithmic_bytes_per_state": cfg.sources * 32 + cfg.targets * 64 + 2 * cfg.targets * 8,
+        "traffic_per_state_over_algorithmic": ((NCU_DRAM_BYTES_PER_LAUNCH[kernel].get(cfg.name) or 0)
+                                                * (cinfo["slabs"] if cinfo["active"] else 1)
+                                                / (cfg.sources * 32 + cfg.targets * 64 + 2 * cfg.targets * 8)) or None,
         "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz "
                        "(FP64 is not in MEASURED_PEAKS.json; DESIGN.md 'Peak')",
         "flops_per_pair": flops_pair, "fp64_instr_per_pair": instr_pair,

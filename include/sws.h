@@ -152,56 +152,6 @@ size_t sws_num_targets(const sws_ctx* ctx);  /* (N-1)M half-mesh points */
 size_t sws_num_sources(const sws_ctx* ctx);  /* NM nodes */
 size_t sws_workspace_bytes(const sws_ctx* ctx);
 
-/* Number of kernels the last sws_residual / sws_jv_batch call launched. */
-int sws_last_launch_count(const sws_ctx* ctx);
-
-/* Time (ms, CUDA events on `cuda_stream`) of the all-pairs phase alone for `states`
- * states (1 = single residual) using the fields left by the previous call: one launch of the staged
- * kernel, or the slab launches of the constant-bank path (sws_set_const_path) without the finishing
- * kernel; used by bench.py --experiments.  Synchronises. */
-int sws_time_allpairs(sws_ctx* ctx, int32_t states, int32_t reps, float* ms_per_launch,
-                      void* cuda_stream);
-
-/* Time (ms per call, CUDA events on `cuda_stream`) of `reps` back-to-back sws_residual calls issued from
- * inside the library (no binding overhead between the calls): what a compiled driver such as
- * libsws_jfnk sees on small meshes, where an evaluation takes tens of microseconds.  Synchronises. */
-int sws_time_residual(sws_ctx* ctx, const double* u_dev, double* F_dev, int32_t reps, float* ms_per_call,
-                      void* cuda_stream);
-
-/* Steps a0-a3, a5-a8 run as ONE cooperative launch on meshes of up to 2^17 nodes (three phases separated by
- * grid-wide barriers) and as three launches above that.  on = 0 forces the three launches; on != 0 restores
- * the default choice.  Results do not depend on it (the phases call the same device functions). */
-int sws_set_fused_fields(sws_ctx* ctx, int32_t on);
-
-/* The same for the all-pairs kernel of sws_jv_exact_batch, with the fields and the batch size
- * of the previous sws_jv_exact_batch call (SWS_EBATCH if there was none). */
-int sws_time_allpairs_lin(sws_ctx* ctx, int32_t reps, float* ms_per_launch, void* cuda_stream);
-
-/* Launch geometry of that kernel for b directions: out6 = {target tiles, column groups, columns
- * per group, nodes staged per bulk copy, segments per column, directions per tile}. */
-int sws_lin_plan_info(sws_ctx* ctx, int32_t b, int32_t* out6);
-
-/* Live timing of the dominant kernel inside ordinary calls.  While profiling is on, every
- * sws_residual / sws_jv_batch / sws_jv_exact_batch brackets its all-pairs phase (one launch of the staged kernel, or
- * the slab launches of the constant-bank path with their fork / join) with a CUDA event pair on the
- * call's stream (no synchronisation, two event records per call).  sws_profile_read
- * synchronises those events and returns the summed all-pairs time (ms) and the number of
- * phases since the last reset; reset != 0 clears the list. */
-int sws_set_profiling(sws_ctx* ctx, int32_t on);
-int sws_profile_read(sws_ctx* ctx, double* allpairs_ms, int32_t* launches, int32_t reset);
-
-/* Tuning knob of the STAGED all-pairs launch: number of source-column groups a target tile's
- * quadrature is split into (0 = library default, chosen from the SM count and occupancy;
- * clamped to what the workspace was sized for).  The constant-bank path ignores it. */
-int sws_set_tuning(sws_ctx* ctx, int32_t chunks);
-
-/* Batched all-pairs launches (sws_jv_batch) let one CTA carry `ns` states: the y_j run is staged once and
- * y_j - y* is formed once per (target, node) for the ns states (north_star: "a batched mode that shares each
- * staged source tile across b perturbed states" - what the states share is the mesh geometry; the source
- * records differ).  ns = 1: one state per CTA, states on the grid's z axis; 2: two states per CTA; 0 = library
- * default (1: measured 4-5 % faster than 2 on B200).  Results do not depend on ns, bit for bit. */
-int sws_set_states_per_cta(sws_ctx* ctx, int32_t ns);
-
 /* The uniform-operand ("constant-bank") form of the all-pairs quadrature, step a4 (eq. (12), same pair
  * arithmetic as the staged kernel): the source records of a slab of columns are copied into a 64 KB constant bank,
  * from where the kernel takes them as uniform-register operands of its FP64 instructions (DESIGN.md section 6:
@@ -212,11 +162,14 @@ int sws_set_states_per_cta(sws_ctx* ctx, int32_t ns);
  * Results are bitwise repeatable in either form and slot b of a batch is bitwise the single evaluation of u_b;
  * the two forms differ from each other in summation order only (~1e-13 of |F|).  The two banks and streams belong to
  * the process (per device): calls of any number of contexts and host threads are serialised through them.  A call may
- * be captured into a CUDA graph after one eager call; a replay of such a graph must not run concurrently with other
- * calls of this library on the same device (the replayed copies into the banks are not ordered against them). */
+ * be captured into a CUDA graph after one eager call.  A captured call does not fork: it keeps the copies and launches
+ * of both banks on the capturing stream, in the same slab order (bitwise the same result, no overlap between the
+ * banks), so the library's own streams never become part of a caller's capture and eager calls of other host threads
+ * and contexts proceed normally while a capture is open.  What remains the caller's duty: a REPLAY of such a graph must
+ * not run concurrently with other calls of this library on the same device (the replayed copies into the banks are not
+ * ordered against them); order them with an event, or use sws_set_const_path(ctx, 0) for contexts whose calls are
+ * replayed from graphs next to eager work. */
 int sws_set_const_path(sws_ctx* ctx, int32_t mode);
-/* out = {path active for this context now (0/1), columns per slab, slabs per state, target tiles (CTAs per column)} */
-int sws_const_plan_info(const sws_ctx* ctx, int32_t out[4]);
 
 /* Change the source strength epsilon (eq. (6)) of an existing context: the parameter of the
  * bootstrapping / continuation process of L229.  Nothing else of the set-up depends on it.  A
@@ -232,14 +185,6 @@ int sws_set_eps(sws_ctx* ctx, double eps);
  * radius_in_dy <= 0 switches the expansion off (every S2 term summed directly, the plain
  * definition); 0 < radius < 6 is refused (SWS_EINVAL).  Default 8. */
 int sws_set_farfield(sws_ctx* ctx, double radius_in_dy);
-
-/* Fraction of (warp, source column) combinations of the first `states` states of the last call
- * that take the direct S2 loop (bench.py: executed FP64 work of a launch).  Synchronises. */
-int sws_farfield_stats(sws_ctx* ctx, int32_t states, double* near_fraction, void* cuda_stream);
-
-/* The all-pairs launch geometry for `states` states: out5 = {target tiles, column groups,
- * columns per group, nodes staged per bulk copy, segments per column}. */
-int sws_plan_info(sws_ctx* ctx, int32_t states, int32_t* out5);
 
 /* The shifts of eq. (25), sigma_b = 1e-7 (1 + ||u||_2) / ||v_b||_2 (0 for a zero direction), WITHOUT a context
  * and without any allocation: sigma_dev[r] for the b rows v_r of V_dev[b][n] (row-major), r = 0 .. b-1.  The values are

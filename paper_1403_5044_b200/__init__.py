@@ -18,18 +18,25 @@ LIB_PATH = _PKG / "libsws.so"
 
 SWS_OK, SWS_EINVAL, SWS_ENOMEM, SWS_ECUDA, SWS_EBATCH, SWS_ESTATE = 0, -1, -2, -3, -4, -5
 
-# every symbol include/sws.h declares
+# every symbol include/sws.h declares (the boundary: libsws.so)
 SYMBOLS = (
     "sws_setup", "sws_residual", "sws_jv_batch", "sws_residual_host", "sws_jv_batch_host",
     "sws_last_sigma", "sws_num_unknowns", "sws_num_targets", "sws_num_sources",
-    "sws_workspace_bytes", "sws_last_launch_count", "sws_time_allpairs", "sws_set_tuning",
-    "sws_plan_info", "sws_set_profiling", "sws_profile_read", "sws_destroy", "sws_strerror", "sws_last_cuda_error",
-    "sws_jv_exact_batch", "sws_jv_exact_batch_host", "sws_time_allpairs_lin", "sws_lin_plan_info",
+    "sws_workspace_bytes", "sws_destroy", "sws_strerror", "sws_last_cuda_error",
+    "sws_jv_exact_batch", "sws_jv_exact_batch_host",
     "sws_get_params", "sws_linearize", "sws_jv_apply",
-    "sws_set_farfield", "sws_farfield_stats", "sws_set_eps", "sws_get_fields_host", "sws_set_states_per_cta", "sws_time_residual", "sws_set_fused_fields",
-    "sws_set_const_path", "sws_const_plan_info",
+    "sws_set_farfield", "sws_set_eps", "sws_get_fields_host",
+    "sws_set_const_path",
     "sws_fd_shifts_noalloc", "sws_noalloc_last_error",
 )
+# every symbol include/sws_tuning.h declares (timing / profiling / launch-shape calls: libsws_tuning.so)
+TUNING_SYMBOLS = (
+    "sws_last_launch_count", "sws_time_allpairs", "sws_time_residual", "sws_set_fused_fields",
+    "sws_time_allpairs_lin", "sws_lin_plan_info", "sws_set_profiling", "sws_profile_read", "sws_set_tuning",
+    "sws_set_states_per_cta", "sws_const_plan_info", "sws_farfield_stats", "sws_plan_info",
+    "sws_tuning_last_cuda_error",
+)
+TUNING_LIB_PATH = _PKG / "libsws_tuning.so"
 
 NOALLOC_MAX_B = 64  # SWS_NOALLOC_MAX_B of include/sws.h
 
@@ -68,8 +75,6 @@ def load_library() -> C.CDLL:
         "sws_jv_batch": (C.c_int, [vp, dp, dp, C.c_int32, dp, dp, dp, dp, vp]),
         "sws_jv_exact_batch": (C.c_int, [vp, dp, dp, C.c_int32, dp, vp]),
         "sws_jv_exact_batch_host": (C.c_int, [vp, dp, dp, C.c_int32, dp, vp]),
-        "sws_time_allpairs_lin": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_float), vp]),
-        "sws_lin_plan_info": (C.c_int, [vp, C.c_int32, ip]),
         "sws_residual_host": (C.c_int, [vp, dp, dp, vp]),
         "sws_jv_batch_host": (C.c_int, [vp, dp, dp, C.c_int32, dp, dp, dp, dp, vp]),
         "sws_last_sigma": (C.c_int, [vp, C.c_int32, dp, vp]),
@@ -77,24 +82,13 @@ def load_library() -> C.CDLL:
         "sws_num_targets": (C.c_size_t, [vp]),
         "sws_num_sources": (C.c_size_t, [vp]),
         "sws_workspace_bytes": (C.c_size_t, [vp]),
-        "sws_last_launch_count": (C.c_int, [vp]),
-        "sws_time_allpairs": (C.c_int, [vp, C.c_int32, C.c_int32, C.POINTER(C.c_float), vp]),
-        "sws_set_tuning": (C.c_int, [vp, C.c_int32]),
-        "sws_plan_info": (C.c_int, [vp, C.c_int32, ip]),
-        "sws_set_profiling": (C.c_int, [vp, C.c_int32]),
-        "sws_profile_read": (C.c_int, [vp, C.POINTER(C.c_double), ip, C.c_int32]),
         "sws_destroy": (C.c_int, [vp]),
         "sws_strerror": (C.c_char_p, [C.c_int]),
         "sws_last_cuda_error": (C.c_char_p, []),
         "sws_get_fields_host": (C.c_int, [vp, dp, dp, dp, dp, vp]),
         "sws_set_farfield": (C.c_int, [vp, C.c_double]),
         "sws_set_eps": (C.c_int, [vp, C.c_double]),
-        "sws_set_states_per_cta": (C.c_int, [vp, C.c_int32]),
         "sws_set_const_path": (C.c_int, [vp, C.c_int32]),
-        "sws_const_plan_info": (C.c_int, [vp, C.POINTER(C.c_int32)]),
-        "sws_time_residual": (C.c_int, [vp, dp, dp, C.c_int32, C.POINTER(C.c_float), vp]),
-        "sws_set_fused_fields": (C.c_int, [vp, C.c_int32]),
-        "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
         "sws_fd_shifts_noalloc": (C.c_int, [dp, dp, C.c_int64, C.c_int32, dp, C.c_int32, vp]),
         "sws_noalloc_last_error": (C.c_char_p, []),
     }
@@ -105,12 +99,51 @@ def load_library() -> C.CDLL:
     return lib
 
 
+_tlib = None
+
+
+def load_tuning_library() -> C.CDLL:
+    """dlopen libsws_tuning.so (include/sws_tuning.h): the timing, profiling and launch-shape calls bench.py
+    --experiments and the tests use.  Not needed for the hot path."""
+    global _tlib
+    if _tlib is not None:
+        return _tlib
+    load_library()  # libsws_tuning.so resolves the context and the launchers against libsws.so
+    if not TUNING_LIB_PATH.exists():
+        raise SwsError(f"{TUNING_LIB_PATH} is missing: run `python -m paper_1403_5044_b200.build`")
+    lib = C.CDLL(str(TUNING_LIB_PATH))
+    vp, dp, ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)
+    proto = {
+        "sws_time_allpairs_lin": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_float), vp]),
+        "sws_lin_plan_info": (C.c_int, [vp, C.c_int32, ip]),
+        "sws_last_launch_count": (C.c_int, [vp]),
+        "sws_time_allpairs": (C.c_int, [vp, C.c_int32, C.c_int32, C.POINTER(C.c_float), vp]),
+        "sws_set_tuning": (C.c_int, [vp, C.c_int32]),
+        "sws_plan_info": (C.c_int, [vp, C.c_int32, ip]),
+        "sws_set_profiling": (C.c_int, [vp, C.c_int32]),
+        "sws_profile_read": (C.c_int, [vp, C.POINTER(C.c_double), ip, C.c_int32]),
+        "sws_set_states_per_cta": (C.c_int, [vp, C.c_int32]),
+        "sws_const_plan_info": (C.c_int, [vp, C.POINTER(C.c_int32)]),
+        "sws_time_residual": (C.c_int, [vp, dp, dp, C.c_int32, C.POINTER(C.c_float), vp]),
+        "sws_set_fused_fields": (C.c_int, [vp, C.c_int32]),
+        "sws_farfield_stats": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_double), vp]),
+        "sws_tuning_last_cuda_error": (C.c_char_p, []),
+    }
+    for name, (res, args) in proto.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    _tlib = lib
+    return lib
+
+
 def _check(rc: int, what: str) -> None:
     if rc != SWS_OK:
         lib = load_library()
         msg = lib.sws_strerror(rc).decode()
         if rc == SWS_ECUDA:
             msg += ": " + lib.sws_last_cuda_error().decode()
+            if _tlib is not None and what in TUNING_SYMBOLS:
+                msg += _tlib.sws_tuning_last_cuda_error().decode()
         raise SwsError(f"{what} failed ({rc}): {msg}")
 
 
@@ -156,6 +189,7 @@ class Context:
     def __init__(self, params: dict, max_batch: int = 0, device: int = 0, precision: int = 0):
         self._h = None
         self.lib = load_library()
+        self._tlib = None
         p = SwsParams(int(params["N"]), int(params["M"]), float(params["x1"]), float(params["y1"]),
                       float(params["dx"]), float(params["dy"]), float(params["froude"]),
                       float(params["eps"]), float(params["n_rad"]), int(params.get("dy_scheme", 0)),
@@ -189,6 +223,13 @@ class Context:
         self.close()
 
     # -- helpers ---------------------------------------------------------------------
+    @property
+    def tlib(self) -> C.CDLL:
+        """libsws_tuning.so, loaded on first use (measurement / tuning methods only)."""
+        if self._tlib is None:
+            self._tlib = load_tuning_library()
+        return self._tlib
+
     def _stream(self, stream=None) -> C.c_void_p:
         torch = _torch()
         s = stream if stream is not None else torch.cuda.current_stream(self.device)
@@ -318,50 +359,50 @@ class Context:
     def time_allpairs(self, states: int = 1, reps: int = 1, stream=None) -> float:
         """ms per launch of the all-pairs kernel alone (CUDA events on the stream)."""
         ms = C.c_float()
-        _check(self.lib.sws_time_allpairs(self._h, int(states), int(reps), C.byref(ms),
+        _check(self.tlib.sws_time_allpairs(self._h, int(states), int(reps), C.byref(ms),
                                           self._stream(stream)), "sws_time_allpairs")
         return float(ms.value)
 
     def time_residual(self, u, F, reps: int = 20, stream=None) -> float:
         """ms per sws_residual call, `reps` calls issued back to back inside the library (sws_time_residual)."""
         ms = C.c_float()
-        _check(self.lib.sws_time_residual(self._h, self._dev(u, (self.n,), "u"), self._dev(F, (self.n,), "F"),
+        _check(self.tlib.sws_time_residual(self._h, self._dev(u, (self.n,), "u"), self._dev(F, (self.n,), "F"),
                                           int(reps), C.byref(ms), self._stream(stream)), "sws_time_residual")
         return float(ms.value)
 
     def set_fused_fields(self, on: bool = True) -> None:
         """sws_set_fused_fields: one cooperative launch (default on small meshes) or three for the O(NM) stages."""
-        _check(self.lib.sws_set_fused_fields(self._h, int(bool(on))), "sws_set_fused_fields")
+        _check(self.tlib.sws_set_fused_fields(self._h, int(bool(on))), "sws_set_fused_fields")
 
     def time_allpairs_lin(self, reps: int = 1, stream=None) -> float:
         """ms per launch of the analytic-Jv all-pairs kernel alone (after a jv_exact_batch call)."""
         ms = C.c_float()
-        _check(self.lib.sws_time_allpairs_lin(self._h, int(reps), C.byref(ms), self._stream(stream)),
+        _check(self.tlib.sws_time_allpairs_lin(self._h, int(reps), C.byref(ms), self._stream(stream)),
                "sws_time_allpairs_lin")
         return float(ms.value)
 
     def lin_plan_info(self, b: int) -> dict:
         out = (C.c_int32 * 6)()
-        _check(self.lib.sws_lin_plan_info(self._h, int(b), out), "sws_lin_plan_info")
+        _check(self.tlib.sws_lin_plan_info(self._h, int(b), out), "sws_lin_plan_info")
         return dict(tiles=out[0], chunks=out[1], cols_per_chunk=out[2], seg_len=out[3], nseg=out[4],
                     dirs_per_tile=out[5])
 
     def set_profiling(self, on: bool = True) -> None:
-        _check(self.lib.sws_set_profiling(self._h, int(bool(on))), "sws_set_profiling")
+        _check(self.tlib.sws_set_profiling(self._h, int(bool(on))), "sws_set_profiling")
 
     def profile_read(self, reset: bool = True):
         """(summed all-pairs kernel ms, launches) since the last reset; synchronises."""
         ms, n = C.c_double(), C.c_int32()
-        _check(self.lib.sws_profile_read(self._h, C.byref(ms), C.byref(n), int(bool(reset))),
+        _check(self.tlib.sws_profile_read(self._h, C.byref(ms), C.byref(n), int(bool(reset))),
                "sws_profile_read")
         return float(ms.value), int(n.value)
 
     def set_tuning(self, chunks: int = 0) -> None:
-        _check(self.lib.sws_set_tuning(self._h, int(chunks)), "sws_set_tuning")
+        _check(self.tlib.sws_set_tuning(self._h, int(chunks)), "sws_set_tuning")
 
     def set_states_per_cta(self, ns: int = 0) -> None:
         """sws_set_states_per_cta: states one CTA of a batched all-pairs launch carries (0 default, 1, 2)."""
-        _check(self.lib.sws_set_states_per_cta(self._h, int(ns)), "sws_set_states_per_cta")
+        _check(self.tlib.sws_set_states_per_cta(self._h, int(ns)), "sws_set_states_per_cta")
 
     def set_const_path(self, mode: int = -1) -> None:
         """sws_set_const_path: -1 automatic (large meshes), 0 staged kernel only, 1 constant-bank kernel whenever it fits."""
@@ -369,7 +410,7 @@ class Context:
 
     def const_plan_info(self) -> dict:
         out = (C.c_int32 * 4)()
-        _check(self.lib.sws_const_plan_info(self._h, out), "sws_const_plan_info")
+        _check(self.tlib.sws_const_plan_info(self._h, out), "sws_const_plan_info")
         return dict(active=bool(out[0]), cols_per_slab=out[1], slabs=out[2], tiles=out[3])
 
     def set_eps(self, eps: float) -> None:
@@ -383,17 +424,17 @@ class Context:
     def farfield_stats(self, states: int = 1) -> float:
         """Fraction of (warp, column) combinations that take the direct S2 loop."""
         f = C.c_double()
-        _check(self.lib.sws_farfield_stats(self._h, int(states), C.byref(f), self._stream()), "sws_farfield_stats")
+        _check(self.tlib.sws_farfield_stats(self._h, int(states), C.byref(f), self._stream()), "sws_farfield_stats")
         return float(f.value)
 
     def plan_info(self, states: int = 1) -> dict:
         out = (C.c_int32 * 5)()
-        _check(self.lib.sws_plan_info(self._h, int(states), out), "sws_plan_info")
+        _check(self.tlib.sws_plan_info(self._h, int(states), out), "sws_plan_info")
         return dict(tiles=out[0], chunks=out[1], cols_per_chunk=out[2], seg_len=out[3], nseg=out[4])
 
     @property
     def last_launch_count(self) -> int:
-        return int(self.lib.sws_last_launch_count(self._h))
+        return int(self.tlib.sws_last_launch_count(self._h))
 
     @property
     def workspace_bytes(self) -> int:

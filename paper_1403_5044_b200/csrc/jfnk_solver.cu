@@ -339,6 +339,7 @@ int gmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_opt
       const double rho = std::hypot(Hm(j, j), Hm(j + 1, j));
       if (rho == 0.0) {  // J P^-1 v_j = 0: the column adds nothing; stop with what was reached
         jd = j;
+        if (hist) hist[its - 1] = rel;  // the iteration was counted: its history slot holds the residual reached
         break;
       }
       cs[j] = Hm(j, j) / rho; sn[j] = Hm(j + 1, j) / rho;
@@ -477,7 +478,7 @@ int egmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_op
     }
   }
   double rel = 1.0;
-  int blocks = 0;
+  int cols = 0;  // columns of the band Hessenberg matrix that entered the least-squares problem
   bool broke = false;
   for (int j = 0; j < mb && !broke; ++j) {
     const int nv = (j + 1) * t;
@@ -512,7 +513,15 @@ int egmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_op
       Hm(nv + c, col) = rcc;
       double hmax = 0.0;
       for (int i = 0; i < nv + c; ++i) hmax = std::max(hmax, std::fabs(Hm(i, col)));
-      if (!(rcc > 1e-14 * hmax)) broke = true;   // the block lost rank: stop after this block with what was reached
+      if (!(rcc > 1e-14 * hmax)) {
+        // The block lost rank at this column: k_normalise left Q_c as it was (stale data of an earlier solve when the
+        // squared norm is exactly 0, normalised rounding noise otherwise) and the later columns of the block were
+        // projected against it.  Neither this column nor the later ones of the block enter H, the residual estimate
+        // or the combination V y: the solve stops with the col columns that are orthonormal.
+        broke = true;
+        break;
+      }
+      cols = col + 1;
       for (size_t q = 0; q < rr.size(); ++q) {   // the rotations made so far
         const int r = rr[q];
         const double a = Hm(r, col), b = Hm(r + 1, col);
@@ -530,19 +539,19 @@ int egmres(sws_solver* s, const double* u, const double* rhs, const sws_gmres_op
         rr.push_back(r - 1); rc.push_back(cc); rs.push_back(ss);
       }
     }
-    blocks = j + 1;
+    // least-squares residual with the first `cols` columns: the t entries of g below them
     double res2 = 0.0;
-    for (int i = blocks * t; i < (blocks + 1) * t; ++i) res2 += g[i] * g[i];
+    for (int i = cols; i < cols + t; ++i) res2 += g[i] * g[i];
     rel = std::sqrt(res2) / bnorm;
     if (hist) hist[j] = rel;
     if (rel <= o->tol || stats->its + t > o->maxit) break;
   }
-  const int cols = blocks * t;
   for (int i = cols - 1; i >= 0; --i) {
     double acc = g[i];
     for (int k = i + 1; k < cols; ++k) acc -= Hm(i, k) * y[k];
     y[i] = Hm(i, i) != 0.0 ? acc / Hm(i, i) : 0.0;
   }
+  if (cols == 0) CU(cudaMemsetAsync(s->t, 0, sizeof(double) * n, st));  // rank lost in the very first column: d = 0
   // the basis may be longer than ydev (m_max): the combination is formed in slices of m_max vectors
   for (int off = 0; off < cols; off += s->m_max) {
     const int cnt = std::min(s->m_max, cols - off);

@@ -543,7 +543,7 @@ int const_cols_per_cta(const sws_ctx* c) {
   return SWS_CONST_CPC;  // build-time override for the measurements of profiles/r2_experiments.md
 #endif
   const int cols = const_slab_cols(c->mesh.M);
-  const long tiles = (c->mesh.T + kConstThreads - 1) / kConstThreads;
+  const long tiles = const_tiles(c->mesh.N, c->mesh.M);
   const long slots = (long)c->sm_count * 8;
   for (int cpc = 4; cpc > 1; cpc /= 2)
     if (tiles * ((cols + cpc - 1) / cpc) >= 2 * slots) return cpc;
@@ -583,34 +583,63 @@ ConstDevice g_const_dev[kMaxDevices];
 std::mutex g_const_mu;
 }  // namespace
 
-cudaError_t launch_allpairs_const(sws_ctx* c, int states, cudaStream_t st, double* F0, double* Fpert, int* launches) {
-  const Mesh& m = c->mesh;
-  if (c->device < 0 || c->device >= kMaxDevices) return cudaErrorInvalidDevice;
-  std::lock_guard<std::mutex> lock(g_const_mu);
-  ConstDevice& d = g_const_dev[c->device];
+// Streams, events and bank addresses of a device: created once, by the first sws_setup on that device that allocates the
+// path's workspace (so that no call - in particular no call a user is capturing into a CUDA graph - has to create them).
+static cudaError_t const_device_ready(int device, ConstDevice** out) {  // the caller holds g_const_mu
+  if (device < 0 || device >= kMaxDevices) return cudaErrorInvalidDevice;
+  ConstDevice& d = g_const_dev[device];
   cudaError_t e = cudaSuccess;
   if (!d.ready) {
     for (int b = 0; b < kConstBanks && e == cudaSuccess; ++b) {
-      e = cudaStreamCreateWithFlags(&d.stream[b], cudaStreamNonBlocking);
-      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&d.join[b], cudaEventDisableTiming);
+      if (!d.stream[b]) e = cudaStreamCreateWithFlags(&d.stream[b], cudaStreamNonBlocking);
+      if (e == cudaSuccess && !d.join[b]) e = cudaEventCreateWithFlags(&d.join[b], cudaEventDisableTiming);
     }
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&d.fork, cudaEventDisableTiming);
+    if (e == cudaSuccess && !d.fork) e = cudaEventCreateWithFlags(&d.fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = const_bank_prepare_0();
+    if (e == cudaSuccess) e = const_bank_prepare_1();
     if (e != cudaSuccess) return e;
     d.ready = true;
   }
+  *out = &d;
+  return cudaSuccess;
+}
+
+cudaError_t const_path_prepare(int device) {
+  std::lock_guard<std::mutex> lock(g_const_mu);
+  ConstDevice* d = nullptr;
+  return const_device_ready(device, &d);
+}
+
+cudaError_t launch_allpairs_const(sws_ctx* c, int states, cudaStream_t st, double* F0, double* Fpert, int* launches) {
+  const Mesh& m = c->mesh;
+  std::lock_guard<std::mutex> lock(g_const_mu);
+  ConstDevice* dp = nullptr;
+  cudaError_t e = const_device_ready(c->device, &dp);
+  if (e != cudaSuccess) return e;
+  ConstDevice& d = *dp;
+  // A call that is being CAPTURED into a CUDA graph must not touch the two shared streams: a stream that waits on an
+  // event of a capturing stream joins that capture and stays in it until cudaStreamEndCapture, and an eager call of
+  // another host thread or context in that window would enqueue its slabs into the foreign capture (its F silently
+  // stale).  Captured calls therefore put the copies and launches of both banks on the caller's stream itself, in the
+  // same slab order: same summation order, bitwise the same result, no fork / join (and no overlap between the banks).
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if ((e = cudaStreamIsCapturing(st, &cap)) != cudaSuccess) return e;
+  const bool inline_banks = cap != cudaStreamCaptureStatusNone;
   const int cols = const_slab_cols(m.M), ypad = (m.M + 3) & ~3;
-  const int tiles = (m.T + kConstThreads - 1) / kConstThreads;
+  const int tiles = const_tiles(m.N, m.M);
   const int slabs = (m.N + cols - 1) / cols;
   const int banks = slabs < kConstBanks ? slabs : kConstBanks;
   // fork: both bank streams wait for what the caller's stream has enqueued so far (the fields kernels)
-  if ((e = cudaEventRecord(d.fork, st)) != cudaSuccess) return e;
-  for (int b = 0; b < banks; ++b)
-    if ((e = cudaStreamWaitEvent(d.stream[b], d.fork, 0)) != cudaSuccess) return e;
+  if (!inline_banks) {
+    if ((e = cudaEventRecord(d.fork, st)) != cudaSuccess) return e;
+    for (int b = 0; b < banks; ++b)
+      if ((e = cudaStreamWaitEvent(d.stream[b], d.fork, 0)) != cudaSuccess) return e;
+  }
   ConstArgs a;
   a.x = c->x; a.N = m.N; a.M = m.M; a.T = m.T; a.ypad = ypad; a.dxdy = m.dx * m.dy; a.em = em_geometry(c);
   a.cpc = const_cols_per_cta(c);
-  for (int s = 0; s < states; ++s) {
-    for (int q = 0; q < slabs; ++q) {
+  for (int s = 0; s < states && e == cudaSuccess; ++s) {
+    for (int q = 0; q < slabs && e == cudaSuccess; ++q) {
       const int b = q % kConstBanks;  // slab q of a state always goes to bank q mod kConstBanks (fixed summation order)
       a.tgt = c->tgt + (size_t)s * m.T;
       a.part = c->part_c + (size_t)b * kConstMaxCols * m.T;
@@ -623,16 +652,21 @@ cudaError_t launch_allpairs_const(sws_ctx* c, int states, cudaStream_t st, doubl
       // and a CUDA graph replayed by a caller may have refilled them since this context's last call
       const double* y = (s == 0 && q < kConstBanks) ? c->y : nullptr;
       const SrcRec* slab = c->src + (size_t)s * m.S + (size_t)a.col0 * m.M;
-      e = b == 0 ? const_bank_launch_0(a, slab, y, tiles, d.stream[b]) : const_bank_launch_1(a, slab, y, tiles, d.stream[b]);
-      if (e != cudaSuccess) return e;
-      if (launches) *launches += 1;
+      cudaStream_t bs = inline_banks ? st : d.stream[b];
+      e = b == 0 ? const_bank_launch_0(a, slab, y, tiles, bs) : const_bank_launch_1(a, slab, y, tiles, bs);
+      if (e == cudaSuccess && launches) *launches += 1;
     }
   }
-  // join: the caller's stream continues after both banks have drained
-  for (int b = 0; b < banks; ++b) {
-    if ((e = cudaEventRecord(d.join[b], d.stream[b])) != cudaSuccess) return e;
-    if ((e = cudaStreamWaitEvent(st, d.join[b], 0)) != cudaSuccess) return e;
+  // join: the caller's stream continues after both banks have drained.  Also after a failed enqueue: the bank streams
+  // may already hold work that reads this context's buffers, and the caller must not run ahead of it.
+  if (!inline_banks) {
+    for (int b = 0; b < banks; ++b) {
+      cudaError_t ej = cudaEventRecord(d.join[b], d.stream[b]);
+      if (ej == cudaSuccess) ej = cudaStreamWaitEvent(st, d.join[b], 0);
+      if (e == cudaSuccess) e = ej;
+    }
   }
+  if (e != cudaSuccess) return e;
   if (F0) {
     k_finish_const<<<dim3((m.T + 127) / 128, states), 128, 0, st>>>(c->tgt, c->acc_c, (size_t)c->max_states * m.T, banks,
                                                                  c->x, c->y, m.N, m.M, m.T, m.eps, F0, Fpert, m.n);

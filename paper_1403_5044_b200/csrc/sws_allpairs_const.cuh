@@ -39,13 +39,21 @@
 #define SWS_CONST_ROTATE 1  // 0: plain unrolled loop
 #endif
 #ifndef SWS_CONST_MINB
+#if SWS_CONST_NT == 2
+#define SWS_CONST_MINB 6  // two targets per thread: 168 registers
+#else
 #define SWS_CONST_MINB 8  // resident CTAs per SM (caps the kernel at 128 registers)
+#endif
+#endif
+#ifndef SWS_CONST_UNROLL2
+#define SWS_CONST_UNROLL2 4  // nodes per inner-loop iteration of the two-target kernel
 #endif
 
 namespace sws {
 namespace {
 
 constexpr int kConstUnroll = SWS_CONST_UNROLL;
+constexpr int kConstUnroll2 = SWS_CONST_UNROLL2;
 
 // [0, ypad): y_j of the mesh;  [ypad, ypad + 4 M ncols): the slab's SrcRec, [column][j]
 __constant__ double c_buf[kConstDoubles];
@@ -101,6 +109,104 @@ __device__ __forceinline__ void walk_column_const(const int rbase, const int M, 
   colS = fma(0.5, hS, colS);
 }
 
+#if SWS_CONST_NT == 2
+// Two targets per thread: the midpoints (k, l) and (k + 1, l) of one y-line.  They share y*, so a node's five uniform
+// loads, its y_j - y* and the loop control serve two pair terms; each target's terms and their order are those of the
+// one-target kernel.
+template <bool S2T>
+__device__ __forceinline__ void walk_column_const2(const int rbase, const int M, const TgtG& tg, const TgtS& ts0,
+                                                   const TgtS& ts1, const ColG& cg0, const ColG& cg1, const ColS& cs0,
+                                                   const ColS& cs1, double& c1a, double& cSa, double& c1b, double& cSb) {
+  auto node = [&](const int j, double& o1a, double& oSa, double& o1b, double& oSb) {
+    const double yj = c_buf[j];
+    const double* r = c_buf + rbase + 4 * j;
+    const double2 zp = make_double2(r[0], r[1]), sl = make_double2(r[2], r[3]);
+    const double dm = yj - tg.ys;
+    pair_term<S2T>(zp, sl, yj, dm, tg, ts0, cg0, cs0, o1a, oSa);
+    pair_term<S2T>(zp, sl, yj, dm, tg, ts1, cg1, cs1, o1b, oSb);
+  };
+  double h1a = 0.0, hSa = 0.0, h1b = 0.0, hSb = 0.0;
+  node(0, h1a, hSa, h1b, hSb);
+  c1a = 0.5 * h1a; cSa = 0.5 * hSa; c1b = 0.5 * h1b; cSb = 0.5 * hSb;
+#pragma unroll kConstUnroll2
+  for (int j = 1; j < M - 1; ++j) node(j, c1a, cSa, c1b, cSb);
+  h1a = hSa = h1b = hSb = 0.0;
+  node(M - 1, h1a, hSa, h1b, hSb);
+  c1a = fma(0.5, h1a, c1a); cSa = fma(0.5, hSa, cSa);
+  c1b = fma(0.5, h1b, c1b); cSb = fma(0.5, hSb, cSb);
+}
+
+__global__ void __launch_bounds__(kConstThreads, SWS_CONST_MINB) k_allpairs_const(const ConstArgs a) {
+  const int tid = threadIdx.x, tile = blockIdx.x, g = blockIdx.y;
+  // slots in TRANSPOSED order over PAIRS of x columns: slot = kk M + l, targets (2 kk, l) and (2 kk + 1, l)
+  const int npc = (a.N - 1 + 1) / 2, nslots = npc * a.M;
+  const int slot = tile * kConstThreads + tid;
+  const int sc = slot < nslots ? slot : nslots - 1;  // ragged tail: recomputed, never stored
+  const int kk = sc / a.M, l = sc - kk * a.M;
+  const bool has1 = 2 * kk + 1 <= a.N - 2;           // odd N - 1: the last pair column holds one target
+  const int tc0 = l * (a.N - 1) + 2 * kk, tc1 = has1 ? tc0 + 1 : tc0;
+  const int t0 = slot < nslots ? tc0 : a.T, t1 = (slot < nslots && has1) ? tc1 : a.T;
+  const TgtRec tr0 = a.tgt[tc0], tr1 = a.tgt[tc1];
+  const TgtG tg = {tr0.ys, 2.0 * tr0.ys, 4.0 * tr0.ys};
+  const TgtS ts0 = {tr0.zs, tr0.psis}, ts1 = {tr1.zs, tr1.psis};
+  const double kb0 = tr0.B / (2.0 * tr0.C), kb1 = tr1.B / (2.0 * tr1.C);
+  const double kg0 = tr0.A / tr0.C - kb0 * kb0, kg1 = tr1.A / tr1.C - kb1 * kb1;
+  const double sfac0 = -tr0.zxs * rsqrt_fp64(tr0.C), sfac1 = -tr1.zxs * rsqrt_fp64(tr1.C);
+
+  double tot1a = 0.0, totSa = 0.0, tot1b = 0.0, totSb = 0.0;
+#pragma unroll 1
+  for (int cc = 0; cc < a.cpc; ++cc) {
+    const int gc = g * a.cpc + cc;
+    if (gc >= a.ncols) break;
+    const int i = a.col0 + gc;
+    ColG cg0, cg1;
+    ColS cs0, cs1;
+    const double xi = __ldg(a.x + i);
+    cg0.dx = xi - tr0.xs; cg0.dx2 = cg0.dx * cg0.dx;
+    cg1.dx = xi - tr1.xs; cg1.dx2 = cg1.dx * cg1.dx;
+    cs0.c = fma(-kb0, cg0.dx, tg.ys); cs0.g = kg0 * cg0.dx2;
+    cs1.c = fma(-kb1, cg1.dx, tg.ys); cs1.g = kg1 * cg1.dx2;
+    const bool far = column_is_far(fmin(cs0.g, cs1.g), a.em.gmin);  // warp-uniform: both targets of all 32 threads
+    const int rbase = a.ypad + 4 * a.M * gc;
+    double c1a, cSa, c1b, cSb;
+    if (far) {
+      walk_column_const2<false>(rbase, a.M, tg, ts0, ts1, cg0, cg1, cs0, cs1, c1a, cSa, c1b, cSb);
+      cSa = s2_column_em(a.em, cs0.c, cs0.g);
+      cSb = s2_column_em(a.em, cs1.c, cs1.g);
+    } else {
+      walk_column_const2<true>(rbase, a.M, tg, ts0, ts1, cg0, cg1, cs0, cs1, c1a, cSa, c1b, cSb);
+    }
+    const double ci = (i == 0 || i == a.N - 1) ? 0.5 : 1.0;  // trapezoid weight in x (Q4)
+    tot1a = fma(ci, c1a, tot1a); totSa = fma(ci, cSa, totSa);
+    tot1b = fma(ci, c1b, tot1b); totSb = fma(ci, cSb, totSb);
+  }
+  if (t0 < a.T) a.part[(size_t)g * a.T + t0] = a.dxdy * fma(sfac0, totSa, tot1a);
+  if (t1 < a.T) a.part[(size_t)g * a.T + t1] = a.dxdy * fma(sfac1, totSb, tot1b);
+
+  __shared__ int s_last;
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) {
+    unsigned int* cnt = a.cnt + tile;
+    const unsigned int seen = atomicAdd(cnt, 1u);
+    s_last = (seen == gridDim.y - 1u);
+    if (s_last) *cnt = 0u;  // ready for the next launch of this bank
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (t0 < a.T) {
+    double sum = 0.0;
+    for (int q = 0; q < (int)gridDim.y; ++q) sum += __ldcg(a.part + (size_t)q * a.T + t0);
+    a.acc[t0] = a.first ? sum : a.acc[t0] + sum;
+  }
+  if (t1 < a.T) {
+    double sum = 0.0;
+    for (int q = 0; q < (int)gridDim.y; ++q) sum += __ldcg(a.part + (size_t)q * a.T + t1);
+    a.acc[t1] = a.first ? sum : a.acc[t1] + sum;
+  }
+}
+#else
 __global__ void __launch_bounds__(kConstThreads, SWS_CONST_MINB) k_allpairs_const(const ConstArgs a) {
   const int tid = threadIdx.x, tile = blockIdx.x, g = blockIdx.y;
   // targets in TRANSPOSED order (sws_farfield.cuh): the 32 targets of a warp share one x*
@@ -159,25 +265,41 @@ __global__ void __launch_bounds__(kConstThreads, SWS_CONST_MINB) k_allpairs_cons
   for (int q = 0; q < (int)gridDim.y; ++q) sum += __ldcg(a.part + (size_t)q * a.T + t);
   a.acc[t] = a.first ? sum : a.acc[t] + sum;
 }
+#endif  // SWS_CONST_NT
 
 }  // namespace
 
 #define SWS_CAT2(a, b) a##b
 #define SWS_CAT(a, b) SWS_CAT2(a, b)
 
-// Copies the slab (and, if y != NULL, the mesh's y_j) into this module's bank and launches the kernel on `st`.
-cudaError_t SWS_CAT(const_bank_launch_, SWS_CONST_BANK)(const ConstArgs& a, const SrcRec* slab, const double* y,
-                                                        int tiles, cudaStream_t st) {
-  static void* base_of_device[64] = {};  // the bank's device address, per device (the caller holds the path's mutex)
+namespace {
+void* g_base_of_device[64] = {};  // the bank's device address, per device (callers hold the path's mutex)
+
+cudaError_t bank_base(void** out) {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-  if (!base_of_device[dev]) {
-    e = cudaGetSymbolAddress(&base_of_device[dev], c_buf);
+  if (!g_base_of_device[dev]) {
+    e = cudaGetSymbolAddress(&g_base_of_device[dev], c_buf);
     if (e != cudaSuccess) return e;
   }
-  void* base = base_of_device[dev];
+  *out = g_base_of_device[dev];
+  return cudaSuccess;
+}
+}  // namespace
+
+cudaError_t SWS_CAT(const_bank_prepare_, SWS_CONST_BANK)() {
+  void* base = nullptr;
+  return bank_base(&base);
+}
+
+// Copies the slab (and, if y != NULL, the mesh's y_j) into this module's bank and launches the kernel on `st`.
+cudaError_t SWS_CAT(const_bank_launch_, SWS_CONST_BANK)(const ConstArgs& a, const SrcRec* slab, const double* y,
+                                                        int tiles, cudaStream_t st) {
+  void* base = nullptr;
+  cudaError_t e = bank_base(&base);
+  if (e != cudaSuccess) return e;
   if (y) {
     e = cudaMemcpyAsync(base, y, (size_t)a.M * sizeof(double), cudaMemcpyDeviceToDevice, st);
     if (e != cudaSuccess) return e;

@@ -9,7 +9,11 @@ namespace sws {
 constexpr int kConstBanks = 2;         // copies of the kernel, each in a module with a __constant__ bank of its own
                                        // (three and four banks were measured: no faster than two)
 constexpr int kConstDoubles = 8160;    // 65,280 B of a module's 64 KB bank: y_j of the mesh + one slab of records
-constexpr int kConstThreads = 64;      // targets per CTA (one per thread)
+constexpr int kConstThreads = 64;      // threads per CTA
+#ifndef SWS_CONST_NT
+#define SWS_CONST_NT 1                 // targets per thread: 1, or 2 = the midpoints (k, l) and (k + 1, l) of one y-line
+#endif
+constexpr int kConstNT = SWS_CONST_NT;
 constexpr int kConstMaxCols = 16;      // columns of a slab = CTA rows of a launch (capacity of the scratch rows)
 constexpr int kConstMinCols = 4;       // the path is used only when a slab holds at least this many columns
 #ifndef SWS_CONST_MIN_TARGETS
@@ -35,6 +39,16 @@ struct ConstArgs {
 
 cudaError_t const_bank_launch_0(const ConstArgs& a, const SrcRec* slab, const double* y, int tiles, cudaStream_t st);
 cudaError_t const_bank_launch_1(const ConstArgs& a, const SrcRec* slab, const double* y, int tiles, cudaStream_t st);
+// resolves the bank's device address on the CURRENT device (cudaGetSymbolAddress; once per device, kept)
+cudaError_t const_bank_prepare_0();
+cudaError_t const_bank_prepare_1();
+
+// target tiles (CTAs per group of columns) of a launch: 64 threads x kConstNT targets each; with two targets per thread
+// the slots are (pair of x columns, y-line) and an odd last column is half empty
+inline int const_tiles(int N, int M) {
+  const long slots = (long)((N - 1 + kConstNT - 1) / kConstNT) * M;
+  return (int)((slots + kConstThreads - 1) / kConstThreads);
+}
 
 // host side (sws_allpairs.cu)
 int const_slab_cols(int M);                 // columns per slab for this M (0: a column does not fit)
@@ -42,5 +56,7 @@ int const_cols_per_cta(const sws_ctx* c);   // 4, 2 or 1: as many as leave two w
 bool const_path_active(const sws_ctx* c);   // the FP64 residual / batch of this context runs on this path
 // a4 (+ a5, a6, a9 when F0 != NULL) for `states` states on the constant-bank path; asynchronous on `st`
 cudaError_t launch_allpairs_const(sws_ctx* c, int states, cudaStream_t st, double* F0, double* Fpert, int* launches);
+// the per-device streams / events of the path and the banks' addresses; called by sws_setup with `device` current
+cudaError_t const_path_prepare(int device);
 
 }  // namespace sws

@@ -36,6 +36,22 @@ def test_header_symbols_exported(sws):
     assert sorted(sws.SYMBOLS) == names, "binding's SYMBOLS list and sws.h disagree"
 
 
+def test_tuning_header_symbols_exported(sws):
+    """The timing / profiling / launch-shape calls live in libsws_tuning.so (include/sws_tuning.h); the boundary
+    library exports none of them and its header declares none of them."""
+    lib = sws.load_tuning_library()
+    names = declared_functions(ROOT / "include" / "sws_tuning.h")
+    assert sorted(names) == sorted(sws.TUNING_SYMBOLS)
+    prod = sws.load_library()
+    boundary = set(declared_functions())
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in sws_tuning.h but not exported by libsws_tuning.so"
+        assert not hasattr(prod, n), f"{n} leaked into the product library"
+        assert n not in boundary
+    assert len(boundary) <= 26, "include/sws.h is the boundary: timing and tuning calls belong in sws_tuning.h"
+    assert lib.sws_plan_info(None, 1, None) == sws.SWS_EINVAL and lib.sws_last_launch_count(None) == 0
+
+
 def test_debug_header_symbols_exported(sws):
     """libsws_debug.so (test hooks + probes) exports what sws_debug.h declares; the product library has none of them."""
     from paper_1403_5044_b200 import debug

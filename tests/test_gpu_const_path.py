@@ -216,6 +216,64 @@ def test_const_path_cuda_graph_capture_and_replay(sws):
         assert torch.equal(a.residual(uA), ref)          # eager again after the capture
 
 
+def test_const_path_capture_leaves_eager_calls_of_another_thread_alone(sws):
+    """While host thread A has a CUDA-graph capture open that contains a constant-bank call, host thread B evaluates
+    eagerly on a context and stream of its own.  A captured call keeps both banks on the capturing stream, so the
+    library's two shared streams never join A's capture: B's calls run at once and are correct (they used to be
+    enqueued into streams that belonged to A's open capture - swallowed into A's graph or refused), and A's graph
+    holds A's work only."""
+    import threading
+    import torch
+    cfgA, cfgB = W.CONFIGS[1], W.custom(N=47, M=29, h=0.3, x1=-4.0, eps=0.3, amp=0.05, seed=44)
+    with sws.Context(cfgA.params()) as a, sws.Context(cfgB.params()) as b:
+        a.set_const_path(1)
+        b.set_const_path(1)
+        uA, uB = dev(W.state(cfgA)), dev(W.state(cfgB))
+        refA, refB = a.residual(uA).clone(), b.residual(uB).clone()
+        FA1, FA2 = torch.zeros_like(uA), torch.zeros_like(uA)
+        FB = [torch.zeros_like(uB) for _ in range(6)]          # B allocates nothing while A captures
+        stB = torch.cuda.Stream()
+        torch.cuda.synchronize()
+        in_capture, b_done, errors = threading.Event(), threading.Event(), []
+
+        def thread_b():
+            try:
+                torch.cuda.set_device(0)
+                assert in_capture.wait(60)
+                with torch.cuda.stream(stB):
+                    for F in FB:
+                        b.residual(uB, out=F)
+                stB.synchronize()                               # B's work finishes while A's capture is still open
+            except Exception as e:  # noqa: BLE001 - reported below
+                errors.append(e)
+            finally:
+                b_done.set()
+
+        t = threading.Thread(target=thread_b)
+        t.start()
+        g = torch.cuda.CUDAGraph()
+        try:
+            with torch.cuda.graph(g, capture_error_mode="thread_local"):
+                a.residual(uA, out=FA1)
+                in_capture.set()
+                assert b_done.wait(120)
+                a.residual(uA, out=FA2)
+        finally:
+            in_capture.set()
+            t.join()
+        assert not errors, errors
+        for F in FB:
+            assert torch.equal(F, refB)
+        assert not FA1.any() and not FA2.any()                  # captured, not executed
+        for _ in range(3):
+            FA1.zero_()
+            FA2.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(FA1, refA) and torch.equal(FA2, refA)
+        assert torch.equal(b.residual(uB), refB) and torch.equal(a.residual(uA), refA)
+
+
 def test_const_path_host_threads(sws, oracle80):
     """Two host threads, each with a context and a stream of its own, call the constant-bank path at the same time:
     the library serialises them through its two banks (a mutex around the enqueue, stream order on the device)."""
