@@ -52,7 +52,9 @@
  * by PB (an exact potential flow a x + b y + c z under a doubly tilted plane: the first
  * term of (13) must return (a^2 + b^2 + c^2)/2 with all four slopes and the cross term
  * live) and A, B, C of L177 by PS (S2 is the singular part of K2: h (K2 - S2) -> 0 at
- * the nodes next to a target under refinement, only for these A, B, C).
+ * the nodes next to a target under refinement, only for these A, B, C); (zeta* + 1)^2
+ * in the source term by PH (the term is harmonic in (x*, y*, zeta*) and symmetric
+ * about z = -1).
  */
 #include <math.h>
 #include <stdlib.h>

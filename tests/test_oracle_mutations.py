@@ -55,7 +55,7 @@ MUTANTS = [
     ("E2_row: (zeta*+1)^2 -> zeta*^2 + 1 in the source term",
      "- sum - zxs * I_S2;",
      "- sum - zxs * I_S2 + (REAL)p->eps * (1 / sqrt(xs * xs + ys * ys + zs * zs + 1) - 1 / sqrt(xs * xs + ys * ys + (zs + 1) * (zs + 1)));",
-     f"{PINS}::test_P7_tilted_plane"),
+     f"{PINS}::test_PH_source_term_is_harmonic_and_centred_at_minus_one"),
     # --- the parallel routine the term-by-term pins look at ---
     ("E2_terms: sign of the K1 sum",
      "s1 += w * (f->phi[AT(i, j)] - ps - f->x[i] + xs) * K1;",

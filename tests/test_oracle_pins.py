@@ -393,6 +393,38 @@ def test_source_term_at_flat_state(oracle64):
 
 
 # ----------------------------------------------------------------------------
+# PH the source term of eq. (12) L101 away from zeta = 0: eps / sqrt(x*^2 + y*^2 + (zeta* + 1)^2) is the potential
+# of a point source at (0, 0, -1) (L72), i.e. as a function of the surface point (x*, y*, zeta*) it is HARMONIC and
+# symmetric about the plane z = -1.  At a level surface zeta = c under the uniform stream phi = x every other term
+# of the row vanishes (K1 multiplies phi - phi* - x + x* = 0, the K2 / S2 / I terms multiply zeta_x = 0), so the
+# rows E2 of three states c - h, c, c + h sample the source term on a 3-D lattice: its 7-point Laplacian must vanish
+# at O(h^2), and the rows at c = -1 + d and c = -1 - d must coincide.  (zeta*^2 + 1 in place of (zeta* + 1)^2 has
+# Laplacian -3 eps / (r^2 + 1)^(5/2) and no such symmetry.)
+# ----------------------------------------------------------------------------
+def _level_rows(orc, c, level):
+    u = W.pack(c, np.full(c.M, c.x1), np.ones((c.M, c.N)), np.full(c.M, level), np.zeros((c.M, c.N)))
+    E = orc.residual(c.params(), u)
+    return E[(c.N + 1) * c.M:].reshape(c.M, c.N + 1)[:, 2:]
+
+
+def test_PH_source_term_is_harmonic_and_centred_at_minus_one(oracle64):
+    worst = []
+    for h, N, M in ((0.2, 9, 6), (0.1, 17, 11)):
+        c = dataclasses.replace(small(N=N, M=M, h=h, x1=0.45), eps=1.0)
+        lo, mid, hi = (_level_rows(oracle64, c, 0.3 + d) for d in (-h, 0.0, h))
+        lap = (mid[1:-1, 2:] + mid[1:-1, :-2] + mid[2:, 1:-1] + mid[:-2, 1:-1] + hi[1:-1, 1:-1] + lo[1:-1, 1:-1]
+               - 6 * mid[1:-1, 1:-1]) / h ** 2
+        worst.append(np.abs(lap).max())
+        assert mid.min() > 0.3                                  # the term is O(eps) here, not round-off
+    # discretisation error of the 7-point stencil only: small and shrinking with h (4.2e-3, 1.5e-3; the finer mesh
+    # also has interior points nearer the source); zeta*^2 + 1 would leave a Laplacian of order 1 at either h
+    assert worst[1] < 0.5 * worst[0] and worst[0] < 1e-2, worst
+    c = dataclasses.replace(small(N=9, M=6, h=0.2, x1=0.45), eps=1.0)
+    np.testing.assert_allclose(_level_rows(oracle64, c, -1 + 0.4), _level_rows(oracle64, c, -1 - 0.4), rtol=1e-13)
+    assert np.abs(_level_rows(oracle64, c, -1 + 0.4) - _level_rows(oracle64, c, -1 + 0.5)).max() > 1e-2
+
+
+# ----------------------------------------------------------------------------
 # P7 tilted plane zeta = alpha x + beta: K1 == 0, K2 == S2 pointwise, so
 #   E2 = 2 pi (phi* - x*) + eps / rho* - alpha I(A = 1 + alpha^2, B = 0, C = 1)
 # with I evaluated HERE by quadrature-pinned closed form; E1 in closed form too
