@@ -52,6 +52,23 @@ def test_tuning_header_symbols_exported(sws):
     assert lib.sws_plan_info(None, 1, None) == sws.SWS_EINVAL and lib.sws_last_launch_count(None) == 0
 
 
+def test_noalloc_entry_point_validates_before_touching_cuda(sws):
+    """sws_fd_shifts_noalloc refuses what its built-in scratch array cannot hold (and bad arguments) with a clear
+    message, before any CUDA call: checkable without a GPU."""
+    lib = sws.load_library()
+    fake = ctypes.c_void_p(256)                                  # never dereferenced: the checks come first
+    assert lib.sws_fd_shifts_noalloc(None, fake, 10, 1, fake, 0, None) == sws.SWS_EINVAL
+    assert b"NULL" in lib.sws_noalloc_last_error()
+    assert lib.sws_fd_shifts_noalloc(fake, fake, 10, sws.NOALLOC_MAX_B + 1, fake, 0, None) == sws.SWS_EBATCH
+    assert b"at most 64" in lib.sws_noalloc_last_error()
+    assert lib.sws_fd_shifts_noalloc(fake, fake, 10, 0, fake, 0, None) == sws.SWS_EBATCH
+    assert lib.sws_fd_shifts_noalloc(fake, fake, 0, 1, fake, 0, None) == sws.SWS_EINVAL
+    assert lib.sws_fd_shifts_noalloc(fake, fake, 2 ** 31, 1, fake, 0, None) == sws.SWS_EINVAL
+    assert lib.sws_fd_shifts_noalloc(fake, fake, 10, 1, fake, 64, None) == sws.SWS_EINVAL
+    text = HEADER.read_text()
+    assert "#define SWS_NOALLOC_MAX_B 64" in text and "33,280" in text
+
+
 def test_debug_header_symbols_exported(sws):
     """libsws_debug.so (test hooks + probes) exports what sws_debug.h declares; the product library has none of them."""
     from paper_1403_5044_b200 import debug
